@@ -1,0 +1,323 @@
+// oracle/autoddl_ref.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see autoddl_ref.h).
+//
+// Plain single-threaded C++.  Every function follows one passage of PAPER.md
+// (cited) in the reading DESIGN.md section 3 fixes (R1..R18).  No blocking, no
+// factorisation of the K x K table into state tables, no caching: each cell of
+// T is evaluated from scratch from its definition.
+//
+// Build: g++ -O2 -std=c++17 -shared -fPIC oracle/autoddl_ref.cpp -o oracle/libautoddl_ref.so
+#include "autoddl_ref.h"
+
+#include <vector>
+
+namespace {
+
+inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// ---- R1: signature table --------------------------------------------------
+// Rows 0..2 are the three factors of the paper's SBP matmul (PAPER.md:193:
+// I=(S0,B,S1), W=(B,S1,S0), O=(S0,S1,P)); row 3 replicates everything; rows 4
+// and 5 let a partial-sum operand pass through the (linear) matmul.
+const int32_t GEMM_I[6] = {REF_S0, REF_B,  REF_S1, REF_B, REF_P, REF_B};
+const int32_t GEMM_W[6] = {REF_B,  REF_S1, REF_S0, REF_B, REF_B, REF_P};
+const int32_t GEMM_O[6] = {REF_S0, REF_S1, REF_P,  REF_B, REF_P, REF_P};
+// Attention has no weight and is not linear in a partial-sum input: it may be
+// split over rows (batch), over columns (heads) or replicated.
+const int32_t ATTN_IO[6]    = {REF_S0, REF_S1, -1, REF_B, -1, -1};
+
+inline int ipow6(int d) { int k = 1; for (int t = 0; t < d; ++t) k *= 6; return k; }
+
+// digit of level d in signature index j, level 0 most significant
+inline int sig_digit(int j, int d, int D) {
+  int div = 1;
+  for (int t = 0; t < D - 1 - d; ++t) div *= 6;
+  return (j / div) % 6;
+}
+
+inline int32_t dual_state(int32_t s) {   // R9: S0->S0, S1->S1, B->P, P->B
+  if (s == REF_B) return REF_P;
+  if (s == REF_P) return REF_B;
+  return s;
+}
+
+}  // namespace
+
+extern "C" int autoddl_ref_num_signatures(const ref_mesh* mesh) {
+  if (!mesh || mesh->ndim < 1 || mesh->ndim > 3) return -1;
+  return ipow6(mesh->ndim);
+}
+
+extern "C" int autoddl_ref_sig_states(int kind, int sig, const ref_mesh* mesh,
+                                      int32_t* I, int32_t* W, int32_t* O) {
+  const int D = mesh->ndim;
+  int valid = 1;
+  for (int d = 0; d < D; ++d) {
+    const int g = sig_digit(sig, d, D);
+    if (kind == REF_GEMM) {
+      I[d] = GEMM_I[g]; W[d] = GEMM_W[g]; O[d] = GEMM_O[g];
+    } else {
+      if (ATTN_IO[g] < 0) { valid = 0; I[d] = W[d] = O[d] = REF_B; }
+      else { I[d] = ATTN_IO[g]; O[d] = ATTN_IO[g]; W[d] = REF_B; }
+    }
+  }
+  return valid;
+}
+
+// ---- R2: local size (Fig. 5: S splits an axis, B and P keep the full extent)
+extern "C" int64_t autoddl_ref_local_size(int64_t R, int64_t C, const int32_t* st, const ref_mesh* mesh) {
+  int64_t f0 = 1, f1 = 1;
+  for (int d = 0; d < mesh->ndim; ++d) {
+    if (st[d] == REF_S0) f0 *= mesh->size[d];
+    if (st[d] == REF_S1) f1 *= mesh->size[d];
+  }
+  return ceil_div(R, f0) * ceil_div(C, f1);
+}
+
+// ---- R3: Table 2, n in bytes, (p-1)/p*n evaluated as (p-1)*ceil(n/p)
+extern "C" int64_t autoddl_ref_collective(int which, int64_t n, int64_t p, int64_t alpha, int64_t beta) {
+  if (p <= 1) return 0;                       // R3/A3: a group of one does not communicate
+  const int64_t sh = ceil_div(n, p);
+  switch (which) {
+    case 0:                                   // AllGather      (p-1)a + (p-1)/p n b
+    case 1:                                   // ReduceScatter  same row of Table 2
+      return (p - 1) * alpha + (p - 1) * sh * beta;
+    case 2:                                   // AllReduce      (2p-1)a + 2 (p-1)/p n b
+      return (2 * p - 1) * alpha + 2 * (p - 1) * sh * beta;
+    case 3:                                   // AlltoAll       (p-1)a + n b
+      return (p - 1) * alpha + n * beta;
+  }
+  return -1;
+}
+
+// ---- R4: forward redistribution a -> b (reduce-scatter, all-to-all, all-gather)
+extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
+                                       const int32_t* a, const int32_t* b,
+                                       const ref_mesh* mesh, const ref_net* net) {
+  const int D = mesh->ndim;
+  int32_t cur[3];
+  for (int d = 0; d < D; ++d) cur[d] = a[d];
+  int64_t cost = 0;
+
+  // Ph0 slice (free): a replicated level that must become split just keeps its slice
+  for (int d = 0; d < D; ++d)
+    if (cur[d] == REF_B && (b[d] == REF_S0 || b[d] == REF_S1)) cur[d] = b[d];
+
+  // Ph1 reduce, innermost level first: P -> S by reduce-scatter ("(S0,S1,P) -> (S0,S1*p2)")
+  for (int d = D - 1; d >= 0; --d)
+    if (cur[d] == REF_P && b[d] != REF_P) {
+      const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // RS input size (Table 2 caption)
+      const int c = mesh->link[d];
+      cost += autoddl_ref_collective(1, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
+      cur[d] = (b[d] == REF_B) ? REF_S1 : b[d];
+    }
+
+  // Ph2 all-to-all, innermost first: change of split axis
+  for (int d = D - 1; d >= 0; --d) {
+    const bool cs = (cur[d] == REF_S0 || cur[d] == REF_S1);
+    const bool bs = (b[d] == REF_S0 || b[d] == REF_S1);
+    if (cs && bs && cur[d] != b[d]) {
+      cur[d] = b[d];
+      const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // output size
+      const int c = mesh->link[d];
+      cost += autoddl_ref_collective(3, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
+    }
+  }
+
+  // Ph3 gather, outermost level first: S -> B by all-gather
+  for (int d = 0; d < D; ++d)
+    if ((cur[d] == REF_S0 || cur[d] == REF_S1) && b[d] == REF_B) {
+      cur[d] = REF_B;
+      const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // output size
+      const int c = mesh->link[d];
+      cost += autoddl_ref_collective(0, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
+    }
+
+  // Ph4 fill (free): a value becomes a partial sum by zero-padding
+  for (int d = 0; d < D; ++d)
+    if (b[d] == REF_P) cur[d] = REF_P;
+
+  for (int d = 0; d < D; ++d)
+    if (cur[d] != b[d]) return -1;            // cannot happen; caught by tests
+  return cost;
+}
+
+// ---- R5: edge cost = forward redistribution + backward redistribution (PAPER.md:197
+// "in both the forward path and the backward path").  The tensor is the consumer's input.
+extern "C" int64_t autoddl_ref_edge_cost(const ref_layer* prev, const ref_layer* cur, int i, int j,
+                                         const ref_mesh* mesh, const ref_net* net) {
+  int32_t Ii[3], Wi[3], Oi[3], Ij[3], Wj[3], Oj[3];
+  const int vi = autoddl_ref_sig_states(prev->kind, i, mesh, Ii, Wi, Oi);
+  const int vj = autoddl_ref_sig_states(cur->kind, j, mesh, Ij, Wj, Oj);
+  if (!vi || !vj) return 0;
+  int32_t da[3], db[3];
+  for (int d = 0; d < mesh->ndim; ++d) { da[d] = dual_state(Oi[d]); db[d] = dual_state(Ij[d]); }
+  const int64_t fwd = autoddl_ref_reshard(cur->in_rows, cur->in_cols, cur->act_bytes, Oi, Ij, mesh, net);
+  const int64_t bwd = autoddl_ref_reshard(cur->in_rows, cur->in_cols, cur->act_bytes, db, da, mesh, net);
+  return fwd + bwd;
+}
+
+// ---- R6: weight-gradient synchronisation: every level on which W is
+// replicated (B) all-reduces the local weight gradient.
+extern "C" int64_t autoddl_ref_node_cost(const ref_layer* cur, int j, const ref_mesh* mesh, const ref_net* net) {
+  if (cur->kind != REF_GEMM) return 0;
+  int32_t I[3], W[3], O[3];
+  if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
+  const int64_t nw = autoddl_ref_local_size(cur->Kd, cur->N, W, mesh);
+  int64_t v = 0;
+  for (int d = 0; d < mesh->ndim; ++d)
+    if (W[d] == REF_B) {
+      const int c = mesh->link[d];
+      v += autoddl_ref_collective(2, nw * cur->wgrad_bytes, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
+    }
+  return v;
+}
+
+// ---- R7: per-device memory of one layer under signature j (PARITY UNPINNED: PAPER.md:221-223
+// uses a OneFlow CPU dry run and prints no formula; this one is ours).
+extern "C" int64_t autoddl_ref_layer_mem(const ref_layer* cur, int j, const ref_mesh* mesh) {
+  int32_t I[3], W[3], O[3];
+  if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
+  int64_t mem = 0;
+  if (cur->kind == REF_GEMM) mem += autoddl_ref_local_size(cur->Kd, cur->N, W, mesh) * cur->wstate_bytes;
+  mem += (autoddl_ref_local_size(cur->in_rows, cur->in_cols, I, mesh) +
+          autoddl_ref_local_size(cur->M, cur->N, O, mesh)) * cur->act_bytes;
+  return mem;
+}
+
+extern "C" int autoddl_ref_feasible(const ref_layer* cur, int j, int32_t L, const ref_mesh* mesh, const ref_net* net) {
+  int32_t I[3], W[3], O[3];
+  if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
+  int64_t rowsplit = 1, colsplit = 1;
+  for (int d = 0; d < mesh->ndim; ++d) {
+    if (I[d] == REF_S0 || O[d] == REF_S0) rowsplit *= mesh->size[d];
+    if (O[d] == REF_S1) colsplit *= mesh->size[d];
+  }
+  if (rowsplit > cur->max_split_rows) return 0;      // PAPER.md:189 "constraints on input split dimensions"
+  if (colsplit > cur->max_split_cols) return 0;
+  if (net->mem_cap_bytes != 0 && autoddl_ref_layer_mem(cur, j, mesh) > net->mem_cap_bytes / L) return 0;
+  return 1;
+}
+
+// ---- R8: the table.  T[l][i][j] = E(l,i,j) + V(l,j) + PEN*[not feasible(l,j)], E(0,.,.) = 0.
+extern "C" int autoddl_ref_build_tables(const ref_layer* layers, int32_t Bp, int32_t L, const ref_mesh* mesh,
+                                        const ref_net* net, int64_t* T, int64_t* node, uint8_t* mask) {
+  if (!layers || !mesh || !net || !T || Bp < 1 || L < 1) return -1;
+  const int K = autoddl_ref_num_signatures(mesh);
+  if (K < 0) return -1;
+  for (int64_t p = 0; p < Bp; ++p)
+    for (int64_t l = 0; l < L; ++l) {
+      const ref_layer* cur = &layers[p * L + l];
+      const ref_layer* prev = (l > 0) ? &layers[p * L + l - 1] : nullptr;
+      int64_t* tile = T + ((p * L + l) * K) * K;
+      for (int j = 0; j < K; ++j) {
+        const int64_t v = autoddl_ref_node_cost(cur, j, mesh, net);
+        const int ok = autoddl_ref_feasible(cur, j, L, mesh, net);
+        if (node) node[(p * L + l) * K + j] = v;
+        if (mask) mask[(p * L + l) * K + j] = (uint8_t)ok;
+        for (int i = 0; i < K; ++i) {
+          const int64_t e = prev ? autoddl_ref_edge_cost(prev, cur, i, j, mesh, net) : 0;
+          tile[(int64_t)i * K + j] = e + v + (ok ? 0 : REF_PEN);
+        }
+      }
+    }
+  return 0;
+}
+
+// ---- R8: Cost(S) = sum_l T[l][s_{l-1}][s_l], s_{-1} := 0  ("a sequence of collectives")
+extern "C" int64_t autoddl_ref_chain_cost(const int64_t* T, int32_t L, int32_t K, const int32_t* s) {
+  int64_t c = 0;
+  int32_t prev = 0;
+  for (int32_t l = 0; l < L; ++l) {
+    c += T[((int64_t)l * K + prev) * K + s[l]];
+    prev = s[l];
+  }
+  return c;
+}
+
+// ---- R9: exact optimum by min-plus DP over the layered graph; smallest index wins every tie.
+extern "C" int autoddl_ref_chain_dp(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                                    int64_t* opt_cost, int32_t* strategy) {
+  if (!T || !opt_cost || !strategy || Bp < 1 || L < 1 || K < 1) return -1;
+  std::vector<int64_t> f(K), g(K);
+  std::vector<int32_t> bp((size_t)L * K);
+  for (int64_t p = 0; p < Bp; ++p) {
+    const int64_t* Tp = T + p * L * K * K;
+    for (int j = 0; j < K; ++j) f[j] = Tp[j];                       // f_0[j] = T[0][0][j]
+    for (int32_t l = 1; l < L; ++l) {
+      const int64_t* tile = Tp + (int64_t)l * K * K;
+      for (int j = 0; j < K; ++j) {
+        int64_t best = f[0] + tile[j];
+        int32_t arg = 0;
+        for (int i = 1; i < K; ++i) {
+          const int64_t v = f[i] + tile[(int64_t)i * K + j];
+          if (v < best) { best = v; arg = i; }                      // strict: smallest i kept
+        }
+        g[j] = best;
+        bp[(size_t)l * K + j] = arg;
+      }
+      f.swap(g);
+    }
+    int32_t js = 0;
+    for (int j = 1; j < K; ++j) if (f[j] < f[js]) js = j;
+    opt_cost[p] = f[js];
+    int32_t* s = strategy + p * L;
+    s[L - 1] = js;
+    for (int32_t l = L - 1; l >= 1; --l) s[l - 1] = bp[(size_t)l * K + s[l]];
+  }
+  return 0;
+}
+
+// ---- exhaustive search: odometer over all K^L strategies of one problem;
+// the first strategy in lexicographic order attaining the minimum is returned.
+extern "C" int autoddl_ref_brute_force(const int64_t* T, int32_t L, int32_t K,
+                                       int64_t* opt_cost, int32_t* strategy) {
+  if (!T || !opt_cost || !strategy || L < 1 || K < 1) return -1;
+  std::vector<int32_t> s(L, 0);
+  int64_t best = -1;
+  for (;;) {
+    const int64_t c = autoddl_ref_chain_cost(T, L, K, s.data());
+    if (best < 0 || c < best) { best = c; for (int l = 0; l < L; ++l) strategy[l] = s[l]; }
+    int l = L - 1;
+    while (l >= 0 && ++s[l] == K) { s[l] = 0; --l; }
+    if (l < 0) break;
+  }
+  *opt_cost = best;
+  return 0;
+}
+
+// ---- R10: coordinate descent.  One update: S[l] = argmin over s_l of Cost(S)
+// with all other layers fixed.  Only the two table entries touching s_l depend on it.
+extern "C" int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                                         const int32_t* init, int32_t S, int32_t max_sweeps,
+                                         int64_t* cost, int32_t* strategy, int32_t* sweeps, int64_t* trace) {
+  if (!T || !init || !cost || !strategy || !sweeps || Bp < 1 || L < 1 || K < 1 || S < 1 || max_sweeps < 1) return -1;
+  std::vector<int32_t> s(L);
+  for (int64_t p = 0; p < Bp; ++p) {
+    const int64_t* Tp = T + p * L * K * K;
+    for (int64_t r = 0; r < S; ++r) {
+      for (int l = 0; l < L; ++l) s[l] = init[(p * S + r) * L + l];
+      int32_t nsweeps = 0;
+      for (;;) {
+        bool changed = false;
+        for (int32_t l = 0; l < L; ++l) {
+          const int32_t left = (l > 0) ? s[l - 1] : 0;
+          int64_t best = 0;
+          int32_t arg = -1;
+          for (int c = 0; c < K; ++c) {
+            int64_t g = Tp[((int64_t)l * K + left) * K + c];
+            if (l < L - 1) g += Tp[((int64_t)(l + 1) * K + c) * K + s[l + 1]];
+            if (arg < 0 || g < best) { best = g; arg = c; }
+          }
+          if (arg != s[l]) { s[l] = arg; changed = true; }
+          if (trace) trace[(((p * S + r) * max_sweeps) + nsweeps) * L + l] = autoddl_ref_chain_cost(Tp, L, K, s.data());
+        }
+        ++nsweeps;
+        if (!changed || nsweeps >= max_sweeps) break;
+      }
+      cost[p * S + r] = autoddl_ref_chain_cost(Tp, L, K, s.data());
+      sweeps[p * S + r] = nsweeps;
+      for (int l = 0; l < L; ++l) strategy[(p * S + r) * L + l] = s[l];
+    }
+  }
+  return 0;
+}

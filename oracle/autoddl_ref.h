@@ -1,0 +1,98 @@
+/*
+ * oracle/autoddl_ref.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU restatement of the AutoDDL strategy-search
+ * hot path (arxiv 2301.06813), written from PAPER.md and the readings listed
+ * in DESIGN.md section 3 ("Readings").  It shares no code, header, table or
+ * helper with the CUDA path under paper_2301_06813_b200/csrc; the struct
+ * layouts below are restated here on purpose.  Only tests/, bench.py's
+ * cpu_baseline / --impl reference legs and __graft_entry__.smoke() may load it.
+ *
+ * All costs are int64 picoseconds.  All pointers are HOST pointers.
+ *
+ * Parity status (see DESIGN.md section 4 "Pins"):
+ *   collectives (Table 2)        pinned  (hand values, identities)
+ *   reshard path                pinned  (paper's 15 GB example, hand cell, symmetry)
+ *   weight-gradient sync        pinned  (data-parallel closed form)
+ *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours)
+ *   chain DP optimum (PAPER.md:225 exhaustive)     pinned  (brute force over K^L)
+ *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
+ */
+#ifndef AUTODDL_REF_H
+#define AUTODDL_REF_H
+
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* tensor states per mesh level, PAPER.md:140,160 (Split axis 0 / axis 1, Broadcast, Partial-sum) */
+enum { REF_S0 = 0, REF_S1 = 1, REF_B = 2, REF_P = 3 };
+/* layer kinds */
+enum { REF_GEMM = 0, REF_ATTN = 1 };
+
+typedef struct {
+  int64_t M, Kd, N;          /* O[M,N] = I[M,Kd] * W[Kd,N] */
+  int64_t in_rows, in_cols;  /* activation resharded into this layer */
+  int32_t kind;
+  int32_t act_bytes;
+  int32_t wgrad_bytes;
+  int32_t wstate_bytes;
+  int32_t max_split_rows;
+  int32_t max_split_cols;
+} ref_layer;                 /* 64 bytes */
+
+typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } ref_mesh;   /* link: 0 intra, 1 inter */
+typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; } ref_net;
+
+#define REF_PEN ((int64_t)1 << 50)
+
+/* 6^ndim signatures per layer */
+int autoddl_ref_num_signatures(const ref_mesh* mesh);
+
+/* Table 2. which: 0 AllGather, 1 ReduceScatter, 2 AllReduce, 3 AlltoAll */
+int64_t autoddl_ref_collective(int which, int64_t n_bytes, int64_t p, int64_t alpha, int64_t beta);
+
+/* local element count of an R x C tensor in state vector st[ndim] (Fig. 5) */
+int64_t autoddl_ref_local_size(int64_t R, int64_t C, const int32_t* st, const ref_mesh* mesh);
+
+/* (I, W, O) state vectors of signature sig for a layer kind; returns 1 if valid, 0 if not */
+int autoddl_ref_sig_states(int kind, int sig, const ref_mesh* mesh, int32_t* I, int32_t* W, int32_t* O);
+
+/* forward redistribution cost a -> b of a rows x cols tensor with eb bytes/element */
+int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb, const int32_t* a, const int32_t* b,
+                            const ref_mesh* mesh, const ref_net* net);
+
+/* edge / node / feasibility of one cell, straight from the definitions */
+int64_t autoddl_ref_edge_cost(const ref_layer* prev, const ref_layer* cur, int i, int j,
+                              const ref_mesh* mesh, const ref_net* net);
+int64_t autoddl_ref_node_cost(const ref_layer* cur, int j, const ref_mesh* mesh, const ref_net* net);
+int     autoddl_ref_feasible(const ref_layer* cur, int j, int32_t L, const ref_mesh* mesh, const ref_net* net);
+int64_t autoddl_ref_layer_mem(const ref_layer* cur, int j, const ref_mesh* mesh);
+
+/* (a1) T[Bp][L][K][K], node[Bp][L][K], mask[Bp][L][K]; node/mask may be NULL */
+int autoddl_ref_build_tables(const ref_layer* layers, int32_t Bp, int32_t L, const ref_mesh* mesh,
+                             const ref_net* net, int64_t* T, int64_t* node, uint8_t* mask);
+
+/* Cost(S) = sum_l T[l][s_{l-1}][s_l], s_{-1} = 0 (one problem) */
+int64_t autoddl_ref_chain_cost(const int64_t* T, int32_t L, int32_t K, const int32_t* s);
+
+/* (a2) exact min-plus chain DP, lowest-index tie-breaks */
+int autoddl_ref_chain_dp(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                         int64_t* opt_cost, int32_t* strategy);
+
+/* exhaustive enumeration of all K^L strategies of one problem (the paper's "exhaustive search") */
+int autoddl_ref_brute_force(const int64_t* T, int32_t L, int32_t K, int64_t* opt_cost, int32_t* strategy);
+
+/* (a3) coordinate descent; trace (optional) receives Cost(s) after every layer update:
+ * trace[Bp][S][max_sweeps][L], unused tail untouched */
+int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                              const int32_t* init, int32_t S, int32_t max_sweeps,
+                              int64_t* cost, int32_t* strategy, int32_t* sweeps, int64_t* trace);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,210 @@
+"""ctypes loader for the CPU oracle (oracle/autoddl_ref.cpp).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, bench.py's cpu_baseline / --impl reference legs and __graft_entry__.smoke() may
+import this.  It never touches the CUDA library and takes numpy (host) arrays only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libautoddl_ref.so")
+_SRC = os.path.join(_HERE, "autoddl_ref.cpp")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with plain g++ -O2 (never tuned)."""
+    hdr = os.path.join(_HERE, "autoddl_ref.h")
+    stale = (not os.path.exists(_SO)) or any(os.path.getmtime(f) > os.path.getmtime(_SO) for f in (_SRC, hdr))
+    if force or stale:
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _SO])
+    return _SO
+
+
+class RefMesh(C.Structure):
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 3), ("link", C.c_int32 * 3)]
+
+
+class RefNet(C.Structure):
+    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_SO)
+        i64, i32, vp = C.c_int64, C.c_int32, C.c_void_p
+        L.autoddl_ref_num_signatures.restype = C.c_int
+        L.autoddl_ref_num_signatures.argtypes = [vp]
+        L.autoddl_ref_collective.restype = i64
+        L.autoddl_ref_collective.argtypes = [C.c_int, i64, i64, i64, i64]
+        L.autoddl_ref_local_size.restype = i64
+        L.autoddl_ref_local_size.argtypes = [i64, i64, vp, vp]
+        L.autoddl_ref_sig_states.restype = C.c_int
+        L.autoddl_ref_sig_states.argtypes = [C.c_int, C.c_int, vp, vp, vp, vp]
+        L.autoddl_ref_reshard.restype = i64
+        L.autoddl_ref_reshard.argtypes = [i64, i64, i64, vp, vp, vp, vp]
+        L.autoddl_ref_edge_cost.restype = i64
+        L.autoddl_ref_edge_cost.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
+        L.autoddl_ref_node_cost.restype = i64
+        L.autoddl_ref_node_cost.argtypes = [vp, C.c_int, vp, vp]
+        L.autoddl_ref_feasible.restype = C.c_int
+        L.autoddl_ref_feasible.argtypes = [vp, C.c_int, i32, vp, vp]
+        L.autoddl_ref_layer_mem.restype = i64
+        L.autoddl_ref_layer_mem.argtypes = [vp, C.c_int, vp]
+        L.autoddl_ref_build_tables.restype = C.c_int
+        L.autoddl_ref_build_tables.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
+        L.autoddl_ref_chain_cost.restype = i64
+        L.autoddl_ref_chain_cost.argtypes = [vp, i32, i32, vp]
+        L.autoddl_ref_chain_dp.restype = C.c_int
+        L.autoddl_ref_chain_dp.argtypes = [vp, i32, i32, i32, vp, vp]
+        L.autoddl_ref_brute_force.restype = C.c_int
+        L.autoddl_ref_brute_force.argtypes = [vp, i32, i32, vp, vp]
+        L.autoddl_ref_coord_descent.restype = C.c_int
+        L.autoddl_ref_coord_descent.argtypes = [vp, i32, i32, i32, vp, i32, i32, vp, vp, vp, vp]
+        _lib = L
+    return _lib
+
+
+def make_mesh(size, link) -> RefMesh:
+    m = RefMesh()
+    m.ndim = len(size)
+    for d in range(len(size)):
+        m.size[d] = int(size[d])
+        m.link[d] = int(link[d])
+    return m
+
+
+def make_net(alpha_ps, beta_ps_per_byte, mem_cap_bytes=0) -> RefNet:
+    n = RefNet()
+    n.alpha_ps[0], n.alpha_ps[1] = int(alpha_ps[0]), int(alpha_ps[1])
+    n.beta_ps_per_byte[0], n.beta_ps_per_byte[1] = int(beta_ps_per_byte[0]), int(beta_ps_per_byte[1])
+    n.mem_cap_bytes = int(mem_cap_bytes)
+    return n
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _st(v):
+    return np.ascontiguousarray(np.asarray(v, dtype=np.int32))
+
+
+def mesh_of(w) -> RefMesh:
+    return make_mesh(w.mesh.size, w.mesh.link)
+
+
+def net_of(w) -> RefNet:
+    return make_net(w.net.alpha_ps, w.net.beta_ps_per_byte, w.net.mem_cap_bytes)
+
+
+# ---- scalar pieces (for the pins) -------------------------------------------------------------
+AG, RS, AR, A2A = 0, 1, 2, 3
+
+
+def collective(which, n, p, alpha, beta) -> int:
+    return int(lib().autoddl_ref_collective(which, n, p, alpha, beta))
+
+
+def local_size(R, Cc, st, mesh: RefMesh) -> int:
+    s = _st(st)
+    return int(lib().autoddl_ref_local_size(R, Cc, _p(s), C.addressof(mesh)))
+
+
+def sig_states(kind, sig, mesh: RefMesh):
+    I = np.zeros(3, np.int32); W = np.zeros(3, np.int32); O = np.zeros(3, np.int32)
+    v = lib().autoddl_ref_sig_states(kind, sig, C.addressof(mesh), _p(I), _p(W), _p(O))
+    D = mesh.ndim
+    return int(v), tuple(I[:D].tolist()), tuple(W[:D].tolist()), tuple(O[:D].tolist())
+
+
+def reshard(rows, cols, eb, a, b, mesh: RefMesh, net: RefNet) -> int:
+    aa, bb = _st(a), _st(b)
+    return int(lib().autoddl_ref_reshard(rows, cols, eb, _p(aa), _p(bb), C.addressof(mesh), C.addressof(net)))
+
+
+def edge_cost(prev_rec, cur_rec, i, j, mesh, net) -> int:
+    a = np.ascontiguousarray(prev_rec).reshape(1); b = np.ascontiguousarray(cur_rec).reshape(1)
+    return int(lib().autoddl_ref_edge_cost(_p(a), _p(b), i, j, C.addressof(mesh), C.addressof(net)))
+
+
+def node_cost(rec, j, mesh, net) -> int:
+    a = np.ascontiguousarray(rec).reshape(1)
+    return int(lib().autoddl_ref_node_cost(_p(a), j, C.addressof(mesh), C.addressof(net)))
+
+
+def feasible(rec, j, L, mesh, net) -> int:
+    a = np.ascontiguousarray(rec).reshape(1)
+    return int(lib().autoddl_ref_feasible(_p(a), j, L, C.addressof(mesh), C.addressof(net)))
+
+
+def layer_mem(rec, j, mesh) -> int:
+    a = np.ascontiguousarray(rec).reshape(1)
+    return int(lib().autoddl_ref_layer_mem(_p(a), j, C.addressof(mesh)))
+
+
+# ---- the three steps ---------------------------------------------------------------------------
+def build_tables(layers: np.ndarray, mesh: RefMesh, net: RefNet):
+    """layers: LAYER_DTYPE [Bp, L] -> T int64 [Bp,L,K,K], node int64 [Bp,L,K], mask uint8 [Bp,L,K]"""
+    layers = np.ascontiguousarray(layers)
+    Bp, L = layers.shape
+    K = 6 ** mesh.ndim
+    T = np.empty((Bp, L, K, K), np.int64)
+    node = np.empty((Bp, L, K), np.int64)
+    mask = np.empty((Bp, L, K), np.uint8)
+    rc = lib().autoddl_ref_build_tables(_p(layers), Bp, L, C.addressof(mesh), C.addressof(net), _p(T), _p(node), _p(mask))
+    assert rc == 0, rc
+    return T, node, mask
+
+
+def chain_cost(T1: np.ndarray, s) -> int:
+    """T1: [L,K,K] of one problem"""
+    T1 = np.ascontiguousarray(T1, dtype=np.int64)
+    s = _st(s)
+    return int(lib().autoddl_ref_chain_cost(_p(T1), T1.shape[0], T1.shape[1], _p(s)))
+
+
+def chain_dp(T: np.ndarray):
+    T = np.ascontiguousarray(T, dtype=np.int64)
+    Bp, L, K, _ = T.shape
+    cost = np.empty(Bp, np.int64)
+    strat = np.empty((Bp, L), np.int32)
+    rc = lib().autoddl_ref_chain_dp(_p(T), Bp, L, K, _p(cost), _p(strat))
+    assert rc == 0, rc
+    return cost, strat
+
+
+def brute_force(T1: np.ndarray):
+    T1 = np.ascontiguousarray(T1, dtype=np.int64)
+    L, K, _ = T1.shape
+    cost = np.empty(1, np.int64)
+    strat = np.empty(L, np.int32)
+    rc = lib().autoddl_ref_brute_force(_p(T1), L, K, _p(cost), _p(strat))
+    assert rc == 0, rc
+    return int(cost[0]), strat
+
+
+def coord_descent(T: np.ndarray, init: np.ndarray, max_sweeps: int = 64, want_trace: bool = False):
+    T = np.ascontiguousarray(T, dtype=np.int64)
+    init = np.ascontiguousarray(init, dtype=np.int32)
+    Bp, L, K, _ = T.shape
+    S = init.shape[1]
+    assert init.shape == (Bp, S, L)
+    cost = np.empty((Bp, S), np.int64)
+    strat = np.empty((Bp, S, L), np.int32)
+    sweeps = np.empty((Bp, S), np.int32)
+    trace = np.full((Bp, S, max_sweeps, L), -1, np.int64) if want_trace else None
+    rc = lib().autoddl_ref_coord_descent(_p(T), Bp, L, K, _p(init), S, max_sweeps, _p(cost), _p(strat), _p(sweeps), _p(trace))
+    assert rc == 0, rc
+    if want_trace:
+        return cost, strat, sweeps, trace
+    return cost, strat, sweeps
