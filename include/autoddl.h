@@ -1,0 +1,125 @@
+/*
+ * include/autoddl.h -- C-ABI boundary of the B200-native AutoDDL strategy-search hot path.
+ *
+ * What it computes (citations are lines of the paper text PAPER.md, arxiv 2301.06813; the exact
+ * readings R1..R18 are listed in DESIGN.md section 3):
+ *   (a1) autoddl_build_tables   SBP cost tables: redistribution cost between every producer-output /
+ *        consumer-input signature pair (collectives of Table 2 PAPER.md:102-108,
+ *        intra/inter-node link rule PAPER.md:203) + weight-gradient all-reduce
+ *        + per-device memory feasibility.
+ *   (a2) autoddl_chain_dp       exact optimum over all K^L strategies of a chain (the result of the
+ *        paper's "exhaustive search") by min-plus dynamic programming.
+ *   (a3) autoddl_coord_descent  the paper's Coordinate Descent, many starts.
+ *
+ * Conventions
+ *   - All costs are int64 picoseconds.  PEN = 2^50 is added to every cell whose consumer signature
+ *     is infeasible; Cost < 2^50  <=>  strategy feasible.
+ *   - d_* arguments are DEVICE pointers owned by the caller, h_* are HOST pointers.  `mesh` and
+ *     `net` are host pointers, read before the call returns.  `stream` is a cudaStream_t (NULL =
+ *     default stream).  Calls taking only d_* pointers are asynchronous on `stream`; they allocate
+ *     nothing and never synchronise.  autoddl_search_host synchronises `stream` before returning.
+ *   - Layouts are dense row-major:  T[Bp][L][K][K] (i = producer signature = row, j = consumer
+ *     signature = column), node[Bp][L][K], mask[Bp][L][K], strategy[Bp][L], init[Bp][S][L],
+ *     cd_strategy[Bp][S][L], cd_cost[Bp][S], cd_sweeps[Bp][S].   K = 6^ndim.
+ *   - d_T must be 16-byte aligned; all other pointers naturally aligned.
+ *   - Return value: 0 success, AUTODDL_EINVAL (-1) bad argument, AUTODDL_ECUDA (-2) CUDA runtime
+ *     error, AUTODDL_EWORK (-3) workspace too small.  Text via autoddl_last_error() (thread-local).
+ *     There is no CPU fallback: without a CUDA device every compute entry point returns ECUDA.
+ */
+#ifndef AUTODDL_H
+#define AUTODDL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AUTODDL_OK      0
+#define AUTODDL_EINVAL (-1)
+#define AUTODDL_ECUDA  (-2)
+#define AUTODDL_EWORK  (-3)
+
+#define AUTODDL_PEN ((int64_t)1 << 50)
+
+/* layer kinds */
+#define AUTODDL_GEMM 0   /* O[M,N] = I[M,Kd] W[Kd,N] */
+#define AUTODDL_ATTN 1   /* weightless; partial-sum signatures are invalid                 */
+
+/* One layer of the chain, 64 bytes.  PAPER.md:189-193. */
+typedef struct {
+  int64_t M, Kd, N;          /* GEMM shape; ATTN: Kd = 0, N = hidden                                 */
+  int64_t in_rows, in_cols;  /* the activation that is redistributed INTO this layer (consumer side) */
+  int32_t kind;              /* AUTODDL_GEMM / AUTODDL_ATTN                                          */
+  int32_t act_bytes;         /* bytes per activation (and activation-gradient) element               */
+  int32_t wgrad_bytes;       /* bytes per weight-gradient element (the all-reduce message)           */
+  int32_t wstate_bytes;      /* resident bytes per weight element (weight + grad + optimiser state)  */
+  int32_t max_split_rows;    /* largest allowed total split of axis 0                 */
+  int32_t max_split_cols;    /* largest allowed total split of the output's axis 1                   */
+} autoddl_layer;
+
+/* Device mesh, level 0 outermost.  link[d]: 0 = intra-node (NVLink), 1 = inter-node. */
+typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } autoddl_mesh;
+
+/* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap. */
+typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; } autoddl_net;
+
+/* K = 6^ndim, or AUTODDL_EINVAL. Host only. */
+int autoddl_num_signatures(const autoddl_mesh* mesh);
+
+/* Bytes of device workspace that any entry point below may need for (Bp, L, S): the tables when
+ * d_T is NULL, DP back-pointers, and autoddl_search_host's staging.  Host only. */
+size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_mesh* mesh);
+
+/* (a1) Build T, node, mask for Bp chains of L layers.  d_node / d_mask may be NULL.
+ * Requires beta_ps_per_byte[c] * 2 * size[d] < 2^31 and alpha, beta >= 0. */
+int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
+                         const autoddl_mesh* mesh, const autoddl_net* net,
+                         int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* stream);
+
+/* (a2) f_0[j] = T[0][0][j]; f_l[j] = min_i f_{l-1}[i] + T[l][i][j]; smallest index wins every tie;
+ * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: tables are first built from d_layers
+ * into d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers.
+ * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
+int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
+                     const autoddl_mesh* mesh, const autoddl_net* net,
+                     const int64_t* d_T, void* d_work, size_t work_bytes,
+                     int64_t* d_opt_cost, int32_t* d_strategy, void* stream);
+
+/* (a3) Coordinate Descent from S starts per problem.  One sweep visits l = 0..L-1 in order and sets
+ * s_l to the smallest-index minimiser of T[l][s_{l-1}][c] + T[l+1][c][s_{l+1}] (s_{-1} = 0, last
+ * layer has no second term) using already-updated neighbours; stops after the first sweep that
+ * changes nothing or after max_sweeps.  d_sweeps counts sweeps including the final unchanged one.
+ * d_init entries must lie in [0, K).  d_T == NULL as in autoddl_chain_dp. */
+int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
+                          const autoddl_mesh* mesh, const autoddl_net* net,
+                          const int64_t* d_T, void* d_work, size_t work_bytes,
+                          const int32_t* d_init, int32_t S, int32_t max_sweeps,
+                          int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, void* stream);
+
+/* Whole path with HOST inputs and outputs (the end-to-end call): copies h_layers and h_init to the
+ * device, runs (a1) (a2) (a3) in d_work, copies the results back, synchronises `stream`.
+ * Any h_* output may be NULL to skip it; h_init NULL skips (a3). */
+int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
+                        const autoddl_mesh* mesh, const autoddl_net* net,
+                        const int32_t* h_init, int32_t S, int32_t max_sweeps,
+                        void* d_work, size_t work_bytes,
+                        int64_t* h_opt_cost, int32_t* h_strategy,
+                        int64_t* h_cd_cost, int32_t* h_cd_strategy, int32_t* h_cd_sweeps, void* stream);
+
+/* Plain device-to-device copy kernel (int4 grid-stride), used by bench.py to measure the HBM
+ * copy bandwidth in the same run as the kernels above.  bytes must be a multiple of 16. */
+int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream);
+
+/* Number of kernel launches issued by this library in the calling thread since load (for bench.py's
+ * gpu_launches). */
+int64_t autoddl_launch_count(void);
+
+/* Text of the last error in the calling thread ("" if none). */
+const char* autoddl_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,218 @@
+"""Thin ctypes binding over the C-ABI library (include/autoddl.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libautoddl.so.  torch is used for device memory
+and streams.  There is no CPU fallback: if the library is missing or there is no CUDA device the
+calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from .configs import LAYER_DTYPE, Workload
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libautoddl.so")
+
+EXPORTS = [
+    "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
+    "autoddl_coord_descent", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
+    "autoddl_last_error",
+]
+
+
+class AutoddlError(RuntimeError):
+    pass
+
+
+class CMesh(C.Structure):
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 3), ("link", C.c_int32 * 3)]
+
+
+class CNet(C.Structure):
+    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libautoddl.so; raises if it has not been built (python -m paper_2301_06813_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise AutoddlError(f"{LIB_PATH} not found: build it with `python paper_2301_06813_b200/build.py` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
+        L.autoddl_num_signatures.restype = C.c_int
+        L.autoddl_num_signatures.argtypes = [vp]
+        L.autoddl_workspace_bytes.restype = sz
+        L.autoddl_workspace_bytes.argtypes = [i32, i32, i32, vp]
+        L.autoddl_build_tables.restype = C.c_int
+        L.autoddl_build_tables.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.autoddl_chain_dp.restype = C.c_int
+        L.autoddl_chain_dp.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, vp, vp]
+        L.autoddl_coord_descent.restype = C.c_int
+        L.autoddl_coord_descent.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_search_host.restype = C.c_int
+        L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
+        L.autoddl_copy_probe.restype = C.c_int
+        L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
+        L.autoddl_launch_count.restype = i64
+        L.autoddl_launch_count.argtypes = []
+        L.autoddl_last_error.restype = C.c_char_p
+        L.autoddl_last_error.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise AutoddlError(f"autoddl error {rc}: {lib().autoddl_last_error().decode()}")
+
+
+def c_mesh(mesh) -> CMesh:
+    m = CMesh()
+    m.ndim = len(mesh.size)                       # ndim outside 1..3 is rejected by the library
+    for d in range(min(m.ndim, 3)):
+        m.size[d] = int(mesh.size[d])
+        m.link[d] = int(mesh.link[d])
+    return m
+
+
+def c_net(net) -> CNet:
+    n = CNet()
+    for c in range(2):
+        n.alpha_ps[c] = int(net.alpha_ps[c])
+        n.beta_ps_per_byte[c] = int(net.beta_ps_per_byte[c])
+    n.mem_cap_bytes = int(net.mem_cap_bytes)
+    return n
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def layers_to_device(layers: np.ndarray, device="cuda") -> torch.Tensor:
+    """LAYER_DTYPE [Bp, L] -> uint8 device tensor [Bp, L, 64]"""
+    assert layers.dtype == LAYER_DTYPE
+    raw = np.ascontiguousarray(layers).view(np.uint8).reshape(layers.shape + (64,))
+    return torch.from_numpy(raw).to(device)
+
+
+def num_signatures(mesh) -> int:
+    m = c_mesh(mesh)
+    k = lib().autoddl_num_signatures(C.addressof(m))
+    if k < 0:
+        _check(k)
+    return k
+
+
+def workspace_bytes(Bp: int, L: int, S: int, mesh) -> int:
+    m = c_mesh(mesh)
+    return int(lib().autoddl_workspace_bytes(Bp, L, S, C.addressof(m)))
+
+
+def build_tables(d_layers: torch.Tensor, mesh, net, want_node_mask: bool = True, out=None):
+    """(a1) -> T int64 [Bp,L,K,K], node int64 [Bp,L,K] | None, mask uint8 [Bp,L,K] | None (device tensors)"""
+    Bp, L = d_layers.shape[0], d_layers.shape[1]
+    K = 6 ** len(mesh.size)
+    dev = d_layers.device
+    T = out if out is not None else torch.empty((Bp, L, K, K), dtype=torch.int64, device=dev)
+    node = torch.empty((Bp, L, K), dtype=torch.int64, device=dev) if want_node_mask else None
+    mask = torch.empty((Bp, L, K), dtype=torch.uint8, device=dev) if want_node_mask else None
+    m, n = c_mesh(mesh), c_net(net)
+    _check(lib().autoddl_build_tables(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n), _ptr(T), _ptr(node),
+                                      _ptr(mask), _stream()))
+    return T, node, mask
+
+
+def chain_dp(T: torch.Tensor | None, mesh, net=None, d_layers=None, work: torch.Tensor | None = None, out=None):
+    """(a2) -> opt_cost int64 [Bp], strategy int32 [Bp, L] (device tensors)"""
+    if T is not None:
+        Bp, L = T.shape[0], T.shape[1]
+        dev = T.device
+    else:
+        Bp, L = d_layers.shape[0], d_layers.shape[1]
+        dev = d_layers.device
+    if work is None:
+        K = 6 ** len(mesh.size)
+        need = (0 if T is not None else Bp * L * K * K * 8 + 256) + (Bp * L * K + 256 if L * K > 16384 else 0)
+        work = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    if out is None:
+        cost = torch.empty(Bp, dtype=torch.int64, device=dev)
+        strat = torch.empty((Bp, L), dtype=torch.int32, device=dev)
+    else:
+        cost, strat = out
+    m = c_mesh(mesh)
+    n = c_net(net) if net is not None else None
+    _check(lib().autoddl_chain_dp(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
+                                  _ptr(T), _ptr(work), work.numel(), _ptr(cost), _ptr(strat), _stream()))
+    return cost, strat
+
+
+def coord_descent(T: torch.Tensor | None, init: torch.Tensor, mesh, max_sweeps: int = 64, net=None, d_layers=None,
+                  work: torch.Tensor | None = None, out=None):
+    """(a3) init int32 [Bp,S,L] -> cost int64 [Bp,S], strategy int32 [Bp,S,L], sweeps int32 [Bp,S]"""
+    Bp, S, L = init.shape
+    dev = init.device
+    if T is None and work is None:
+        K = 6 ** len(mesh.size)
+        work = torch.empty(Bp * L * K * K * 8 + 256, dtype=torch.uint8, device=dev)
+    if out is None:
+        cost = torch.empty((Bp, S), dtype=torch.int64, device=dev)
+        strat = torch.empty((Bp, S, L), dtype=torch.int32, device=dev)
+        sweeps = torch.empty((Bp, S), dtype=torch.int32, device=dev)
+    else:
+        cost, strat, sweeps = out
+    m = c_mesh(mesh)
+    n = c_net(net) if net is not None else None
+    _check(lib().autoddl_coord_descent(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
+                                       _ptr(T), _ptr(work), work.numel() if work is not None else 0, _ptr(init), S,
+                                       max_sweeps, _ptr(cost), _ptr(strat), _ptr(sweeps), _stream()))
+    return cost, strat, sweeps
+
+
+def search_host(w: Workload, init: np.ndarray | None, work: torch.Tensor, pinned=None):
+    """End-to-end call with HOST inputs/outputs (numpy or pinned torch CPU tensors).  Returns a dict of numpy arrays."""
+    layers = np.ascontiguousarray(w.layers)
+    Bp, L = layers.shape
+    S = 0 if init is None else init.shape[1]
+    if pinned is None:
+        pinned = alloc_host_outputs(Bp, L, S)
+    m, n = c_mesh(w.mesh), c_net(w.net)
+    ip = None if init is None else init.ctypes.data
+    _check(lib().autoddl_search_host(layers.ctypes.data, Bp, L, C.addressof(m), C.addressof(n), ip, S, w.max_sweeps,
+                                     work.data_ptr(), work.numel(),
+                                     pinned["opt_cost"].data_ptr(), pinned["strategy"].data_ptr(),
+                                     pinned["cd_cost"].data_ptr() if S else None,
+                                     pinned["cd_strategy"].data_ptr() if S else None,
+                                     pinned["cd_sweeps"].data_ptr() if S else None, _stream()))
+    return {k: v.numpy() for k, v in pinned.items()}
+
+
+def alloc_host_outputs(Bp: int, L: int, S: int, pin: bool = True):
+    pin = pin and torch.cuda.is_available()
+    mk = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=pin)
+    return {
+        "opt_cost": mk((Bp,), torch.int64), "strategy": mk((Bp, L), torch.int32),
+        "cd_cost": mk((Bp, max(S, 1)), torch.int64), "cd_strategy": mk((Bp, max(S, 1), L), torch.int32),
+        "cd_sweeps": mk((Bp, max(S, 1)), torch.int32),
+    }
+
+
+def copy_probe(src: torch.Tensor, dst: torch.Tensor):
+    nbytes = src.numel() * src.element_size()
+    _check(lib().autoddl_copy_probe(src.data_ptr(), dst.data_ptr(), nbytes, _stream()))
+
+
+def launch_count() -> int:
+    return int(lib().autoddl_launch_count())

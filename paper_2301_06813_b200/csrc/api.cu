@@ -1,0 +1,235 @@
+// C-ABI entry points (include/autoddl.h): argument validation, workspace carving, launches.
+#include <stdarg.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace autoddl {
+
+static thread_local char g_err[512] = "";
+static thread_local int64_t g_launches = 0;
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+void clear_error() { g_err[0] = 0; }
+void count_launch(int n) { g_launches += n; }
+
+int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshParams* out) {
+  ADL_REQUIRE(mesh != nullptr, "mesh is NULL");
+  ADL_REQUIRE(mesh->ndim >= 1 && mesh->ndim <= 3, "mesh.ndim = %d, must be 1..3", mesh->ndim);
+  for (int d = 0; d < mesh->ndim; ++d) {
+    ADL_REQUIRE(mesh->size[d] >= 1 && mesh->size[d] <= 65536, "mesh.size[%d] = %d out of range", d, mesh->size[d]);
+    ADL_REQUIRE(mesh->link[d] == 0 || mesh->link[d] == 1, "mesh.link[%d] = %d, must be 0 or 1", d, mesh->link[d]);
+  }
+  if (out) {
+    memset(out, 0, sizeof(*out));
+    out->ndim = mesh->ndim;
+    for (int d = 0; d < mesh->ndim; ++d) out->size[d] = mesh->size[d];
+  }
+  if (net) {
+    for (int c = 0; c < 2; ++c) {
+      ADL_REQUIRE(net->alpha_ps[c] >= 0 && net->alpha_ps[c] < ((int64_t)1 << 40), "net.alpha_ps[%d] out of range", c);
+      ADL_REQUIRE(net->beta_ps_per_byte[c] >= 0 && net->beta_ps_per_byte[c] < ((int64_t)1 << 20),
+                  "net.beta_ps_per_byte[%d] out of range", c);
+    }
+    ADL_REQUIRE(net->mem_cap_bytes >= 0, "net.mem_cap_bytes < 0");
+    if (out) {
+      for (int d = 0; d < mesh->ndim; ++d) {
+        out->alpha[d] = net->alpha_ps[mesh->link[d]];
+        out->beta[d] = net->beta_ps_per_byte[mesh->link[d]];
+      }
+      out->mem_cap = net->mem_cap_bytes;
+    }
+  }
+  return AUTODDL_OK;
+}
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline size_t table_bytes(int64_t Bp, int64_t L, int64_t K) { return align_up((size_t)Bp * L * K * K * 8, 256); }
+static inline bool bp_in_workspace(int64_t L, int64_t K) { return (size_t)L * K > 16 * 1024; }
+static inline size_t bp_bytes(int64_t Bp, int64_t L, int64_t K) {
+  return bp_in_workspace(L, K) ? align_up((size_t)Bp * L * K, 256) : 0;
+}
+
+static int check_device() {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n < 1) {
+    set_error("no CUDA device available (%s); this library has no CPU fallback", cudaGetErrorString(e));
+    cudaGetLastError();
+    return AUTODDL_ECUDA;
+  }
+  return AUTODDL_OK;
+}
+
+}  // namespace autoddl
+
+using namespace autoddl;
+
+extern "C" {
+
+int autoddl_num_signatures(const autoddl_mesh* mesh) {
+  clear_error();
+  int rc = validate_mesh_net(mesh, nullptr, nullptr);
+  if (rc) return rc;
+  return num_sigs(mesh->ndim);
+}
+
+size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_mesh* mesh) {
+  clear_error();
+  if (validate_mesh_net(mesh, nullptr, nullptr) || Bp < 1 || L < 1 || S < 0) return 0;
+  const int64_t K = num_sigs(mesh->ndim);
+  size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
+  // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
+  b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
+  b += align_up((size_t)Bp * S * L * 4, 256) * 2;
+  b += align_up((size_t)Bp * 8, 256) + align_up((size_t)Bp * L * 4, 256);
+  b += align_up((size_t)Bp * S * 8, 256) + align_up((size_t)Bp * S * 4, 256);
+  return b;
+}
+
+int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                         const autoddl_net* net, int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* stream) {
+  clear_error();
+  MeshParams mp;
+  ADL_REQUIRE(net != nullptr, "net is NULL");
+  int rc = validate_mesh_net(mesh, net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(d_layers != nullptr && d_T != nullptr, "d_layers / d_T is NULL");
+  ADL_REQUIRE(Bp >= 1 && L >= 1, "Bp = %d, L = %d must be >= 1", Bp, L);
+  ADL_REQUIRE(((uintptr_t)d_T & 15) == 0, "d_T must be 16-byte aligned");
+  ADL_REQUIRE(((uintptr_t)d_layers & 7) == 0 && ((uintptr_t)d_node & 7) == 0, "misaligned pointer");
+  if ((rc = check_device())) return rc;
+  return launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, (cudaStream_t)stream);
+}
+
+int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                     const autoddl_net* net, const int64_t* d_T, void* d_work, size_t work_bytes,
+                     int64_t* d_opt_cost, int32_t* d_strategy, void* stream) {
+  clear_error();
+  MeshParams mp;
+  int rc = validate_mesh_net(mesh, d_T ? nullptr : net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(Bp >= 1 && L >= 1, "Bp = %d, L = %d must be >= 1", Bp, L);
+  ADL_REQUIRE(d_opt_cost != nullptr && d_strategy != nullptr, "output pointer is NULL");
+  ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
+  ADL_REQUIRE(((uintptr_t)d_opt_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0, "misaligned output pointer");
+  const int K = num_sigs(mesh->ndim);
+  const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
+  if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
+    set_error("chain_dp: workspace of %zu bytes needed, %zu given", tb + bb, d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!d_T) {
+    ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
+    if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
+    d_T = (const int64_t*)d_work;
+  }
+  uint8_t* d_bp = bb ? (uint8_t*)d_work + tb : nullptr;
+  return launch_chain_dp(d_T, Bp, L, K, d_bp, d_opt_cost, d_strategy, st);
+}
+
+int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                          const autoddl_net* net, const int64_t* d_T, void* d_work, size_t work_bytes,
+                          const int32_t* d_init, int32_t S, int32_t max_sweeps, int64_t* d_cost,
+                          int32_t* d_strategy, int32_t* d_sweeps, void* stream) {
+  clear_error();
+  MeshParams mp;
+  int rc = validate_mesh_net(mesh, d_T ? nullptr : net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(Bp >= 1 && L >= 1 && S >= 1 && max_sweeps >= 1, "Bp, L, S, max_sweeps must be >= 1");
+  ADL_REQUIRE(d_init && d_cost && d_strategy && d_sweeps, "NULL pointer");
+  ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
+  ADL_REQUIRE(((uintptr_t)d_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0 && ((uintptr_t)d_init & 3) == 0 &&
+                  ((uintptr_t)d_sweeps & 3) == 0, "misaligned pointer");
+  const int K = num_sigs(mesh->ndim);
+  const size_t tb = d_T ? 0 : table_bytes(Bp, L, K);
+  if (tb > 0 && (d_work == nullptr || work_bytes < tb)) {
+    set_error("coord_descent: workspace of %zu bytes needed, %zu given", tb, d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!d_T) {
+    ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
+    if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
+    d_T = (const int64_t*)d_work;
+  }
+  return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+}
+
+int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                        const autoddl_net* net, const int32_t* h_init, int32_t S, int32_t max_sweeps,
+                        void* d_work, size_t work_bytes, int64_t* h_opt_cost, int32_t* h_strategy,
+                        int64_t* h_cd_cost, int32_t* h_cd_strategy, int32_t* h_cd_sweeps, void* stream) {
+  clear_error();
+  MeshParams mp;
+  ADL_REQUIRE(net != nullptr, "net is NULL");
+  int rc = validate_mesh_net(mesh, net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(h_layers != nullptr, "h_layers is NULL");
+  ADL_REQUIRE(Bp >= 1 && L >= 1, "Bp = %d, L = %d must be >= 1", Bp, L);
+  const bool do_cd = h_init != nullptr;
+  if (do_cd) ADL_REQUIRE(S >= 1 && max_sweeps >= 1, "S, max_sweeps must be >= 1");
+  if (!do_cd) S = 0;
+  ADL_REQUIRE(((uintptr_t)d_work & 255) == 0, "d_work must be 256-byte aligned");
+  const size_t need = autoddl_workspace_bytes(Bp, L, S, mesh);
+  if (d_work == nullptr || work_bytes < need) {
+    set_error("search_host: workspace of %zu bytes needed, %zu given", need, d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  if ((rc = check_device())) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int K = num_sigs(mesh->ndim);
+
+  unsigned char* w = (unsigned char*)d_work;
+  auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
+  int64_t* d_T = (int64_t*)carve(table_bytes(Bp, L, K));
+  uint8_t* d_bp = bp_bytes(Bp, L, K) ? (uint8_t*)carve(bp_bytes(Bp, L, K)) : nullptr;
+  autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));
+  int32_t* d_init = (int32_t*)carve((size_t)Bp * S * L * 4);
+  int32_t* d_cd_strategy = (int32_t*)carve((size_t)Bp * S * L * 4);
+  int64_t* d_opt = (int64_t*)carve((size_t)Bp * 8);
+  int32_t* d_strategy = (int32_t*)carve((size_t)Bp * L * 4);
+  int64_t* d_cd_cost = (int64_t*)carve((size_t)Bp * S * 8);
+  int32_t* d_cd_sweeps = (int32_t*)carve((size_t)Bp * S * 4);
+
+  ADL_CUDA_CHECK(cudaMemcpyAsync(d_layers, h_layers, (size_t)Bp * L * sizeof(autoddl_layer), cudaMemcpyHostToDevice, st));
+  if (do_cd) ADL_CUDA_CHECK(cudaMemcpyAsync(d_init, h_init, (size_t)Bp * S * L * 4, cudaMemcpyHostToDevice, st));
+  if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, nullptr, nullptr, st))) return rc;
+  if ((rc = launch_chain_dp(d_T, Bp, L, K, d_bp, d_opt, d_strategy, st))) return rc;
+  if (do_cd &&
+      (rc = launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
+    return rc;
+  if (h_opt_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_opt_cost, d_opt, (size_t)Bp * 8, cudaMemcpyDeviceToHost, st));
+  if (h_strategy) ADL_CUDA_CHECK(cudaMemcpyAsync(h_strategy, d_strategy, (size_t)Bp * L * 4, cudaMemcpyDeviceToHost, st));
+  if (do_cd) {
+    if (h_cd_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_cd_cost, d_cd_cost, (size_t)Bp * S * 8, cudaMemcpyDeviceToHost, st));
+    if (h_cd_strategy)
+      ADL_CUDA_CHECK(cudaMemcpyAsync(h_cd_strategy, d_cd_strategy, (size_t)Bp * S * L * 4, cudaMemcpyDeviceToHost, st));
+    if (h_cd_sweeps) ADL_CUDA_CHECK(cudaMemcpyAsync(h_cd_sweeps, d_cd_sweeps, (size_t)Bp * S * 4, cudaMemcpyDeviceToHost, st));
+  }
+  ADL_CUDA_CHECK(cudaStreamSynchronize(st));
+  return AUTODDL_OK;
+}
+
+int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {
+  clear_error();
+  ADL_REQUIRE(d_src && d_dst && bytes > 0 && bytes % 16 == 0, "copy_probe: bad arguments");
+  ADL_REQUIRE(((uintptr_t)d_src & 15) == 0 && ((uintptr_t)d_dst & 15) == 0, "copy_probe: misaligned");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_copy_probe(d_src, d_dst, bytes, (cudaStream_t)stream);
+}
+
+int64_t autoddl_launch_count(void) { return g_launches; }
+
+const char* autoddl_last_error(void) { return g_err; }
+
+}  // extern "C"

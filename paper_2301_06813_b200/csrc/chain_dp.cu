@@ -1,0 +1,228 @@
+// (a2) Exact min-plus chain DP for sm_100a.  DESIGN.md R9; the optimum equals the paper's exhaustive
+// search.
+//
+//   f_0[j] = T[0][0][j];  f_l[j] = min_i f_{l-1}[i] + T[l][i][j]  (smallest i on ties);  backtrack.
+//
+// One CTA per problem.  A producer warp streams the problem's tiles through a ring of shared-memory
+// stages with TMA bulk copies (cp.async.bulk + mbarrier complete_tx, L2 evict-first: every byte is read
+// once).  Consumer threads each own a pair of adjacent columns (one 16-byte shared load per row) and a
+// group of rows; f is broadcast from shared memory.  With one consumer warp (K = 36) a layer needs no
+// block barrier at all; with several row groups (K = 216) partial minima are merged through shared
+// memory with the lexicographic (value, row) order that keeps the lowest-index tie-break.
+#include "common.cuh"
+
+namespace autoddl {
+
+namespace {
+
+struct DpCfg {
+  int K;        // signatures
+  int RB;       // rows per stage
+  int STAGES;
+  int G;        // row groups (consumer threads = G * K/2, rounded up to warps)
+};
+
+template <int K, int RB, int STAGES, int G>
+struct DpLayout {
+  static constexpr int KH = K / 2;
+  static constexpr int NCONS = ((G * KH + 31) / 32) * 32;   // consumer threads
+  static constexpr int NT = NCONS + 32;                     // + producer warp
+  static constexpr int STAGE_BYTES = RB * K * 8;
+  static constexpr int NBLK = K / RB;                       // row blocks per tile
+  static_assert(K % RB == 0, "RB must divide K");
+  static_assert(RB % G == 0, "G must divide RB");
+  static_assert(STAGE_BYTES % 16 == 0, "bulk copy granularity");
+};
+
+__device__ __forceinline__ bool lex_less(int64_t v, int i, int64_t bv, int bi) {
+  return v < bv || (v == bv && i < bi);
+}
+
+template <int K, int RB, int STAGES, int G, bool BP_SMEM>
+__global__ void __launch_bounds__(DpLayout<K, RB, STAGES, G>::NT)
+chain_dp_kernel(const int64_t* __restrict__ T, int L, uint8_t* __restrict__ bp_glob,
+                int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy) {
+  using Lay = DpLayout<K, RB, STAGES, G>;
+  constexpr int KH = Lay::KH, NCONS = Lay::NCONS, NBLK = Lay::NBLK, SB = Lay::STAGE_BYTES;
+  constexpr int RPG = RB / G;                                // rows per group per stage
+
+  extern __shared__ __align__(128) unsigned char smem[];
+  // layout: stages | f[2][K] | part (G>1) | full[STAGES] empty[STAGES] | bp (optional) | strat
+  int64_t* stage0 = reinterpret_cast<int64_t*>(smem);
+  int64_t* fbuf = reinterpret_cast<int64_t*>(smem + (size_t)STAGES * SB);
+  int64_t* partv = fbuf + 2 * K;                             // [G][K] values
+  int32_t* parti = reinterpret_cast<int32_t*>(partv + (G > 1 ? G * K : 0));   // [G][K] rows
+  uint64_t* full = reinterpret_cast<uint64_t*>(parti + (G > 1 ? G * K : 0) + ((G > 1 ? G * K : 0) & 1));
+  uint64_t* empty = full + STAGES;
+  uint8_t* bp_s = reinterpret_cast<uint8_t*>(empty + STAGES);
+
+  const int tid = threadIdx.x;
+  const int p = blockIdx.x;
+  const int64_t* Tp = T + (size_t)p * L * K * K;
+  uint8_t* bp = BP_SMEM ? bp_s : bp_glob + (size_t)p * L * K;
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], NCONS / 32);                      // one arrive per consumer warp
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  const int nblocks = (L - 1) * NBLK;                        // tile 0 contributes only its row 0
+
+  if (tid >= NCONS) {
+    // ================= producer warp: one elected lane drives TMA =================
+    if (tid == NCONS) {
+      const uint64_t pol = policy_evict_first();
+      const unsigned char* src = reinterpret_cast<const unsigned char*>(Tp + (size_t)K * K);
+      for (int b = 0; b < nblocks; ++b) {
+        const int s = b % STAGES;
+        if (b >= STAGES) mbar_wait(&empty[s], ((b / STAGES) - 1) & 1);
+        mbar_arrive_expect_tx(&full[s], SB);
+        bulk_g2s(smem + (size_t)s * SB, src + (size_t)b * SB, SB, &full[s], pol);
+      }
+    }
+    return;
+  }
+
+  // ================= consumers =================
+  const int cp = tid % KH;                                   // column pair
+  const int g = tid / KH;                                    // row group (>= G: idle padding lanes)
+  const bool active = g < G;
+  const int lane = tid & 31;
+
+  // f_0 = row 0 of tile 0
+  for (int j = tid; j < K; j += NCONS) fbuf[j] = __ldg(Tp + j);
+  if (G > 1 || NCONS > 32) asm volatile("bar.sync 1, %0;" ::"n"(NCONS)); else __syncwarp();
+
+  int cur = 0;
+  int b = 0;
+  for (int l = 1; l < L; ++l) {
+    const int64_t* f = fbuf + cur * K;
+    int64_t best0 = INT64_MAX, best1 = INT64_MAX;     // cells < 2^62/L: the first row always wins
+    int a0 = 0, a1 = 0;
+    for (int rb = 0; rb < NBLK; ++rb, ++b) {
+      const int s = b % STAGES;
+      mbar_wait(&full[s], (b / STAGES) & 1);
+      if (active) {
+        const int64_t* tile = stage0 + (size_t)s * (SB / 8);
+#pragma unroll 6
+        for (int r = 0; r < RPG; ++r) {
+          const int rl = g * RPG + r;                        // row inside the stage
+          const int i = rb * RB + rl;
+          const int64_t fi = f[i];
+          const longlong2 t = *reinterpret_cast<const longlong2*>(tile + rl * K + 2 * cp);
+          const int64_t v0 = fi + t.x, v1 = fi + t.y;
+          if (v0 < best0) { best0 = v0; a0 = i; }
+          if (v1 < best1) { best1 = v1; a1 = i; }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);                 // this warp is done with the stage
+    }
+    int64_t* fn = fbuf + (cur ^ 1) * K;
+    if (G == 1) {
+      if (active) {
+        *reinterpret_cast<longlong2*>(fn + 2 * cp) = make_longlong2(best0, best1);
+        bp[(size_t)l * K + 2 * cp] = (uint8_t)a0;
+        bp[(size_t)l * K + 2 * cp + 1] = (uint8_t)a1;
+      }
+      if (NCONS > 32) asm volatile("bar.sync 1, %0;" ::"n"(NCONS)); else __syncwarp();
+    } else {
+      if (active) {
+        partv[g * K + 2 * cp] = best0;  parti[g * K + 2 * cp] = a0;
+        partv[g * K + 2 * cp + 1] = best1;  parti[g * K + 2 * cp + 1] = a1;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(NCONS));
+      for (int j = tid; j < K; j += NCONS) {
+        int64_t bv = partv[j];
+        int bi = parti[j];
+#pragma unroll
+        for (int gg = 1; gg < G; ++gg) {
+          const int64_t v = partv[gg * K + j];
+          const int i = parti[gg * K + j];
+          if (lex_less(v, i, bv, bi)) { bv = v; bi = i; }
+        }
+        fn[j] = bv;
+        bp[(size_t)l * K + j] = (uint8_t)bi;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(NCONS));
+    }
+    cur ^= 1;
+  }
+
+  // ---- smallest argmin of f_{L-1}, backtrack -------------------------------------------------------
+  if (tid < 32) {
+    const int64_t* f = fbuf + cur * K;
+    int64_t bv = 0;
+    int bi = -1;
+    for (int j = lane; j < K; j += 32) {
+      const int64_t v = f[j];
+      if (bi < 0 || v < bv) { bv = v; bi = j; }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (oi >= 0 && (bi < 0 || lex_less(ov, oi, bv, bi))) { bv = ov; bi = oi; }
+    }
+    int32_t* sp = strategy + (size_t)p * L;
+    if (lane == 0) {
+      opt_cost[p] = bv;
+      int s = bi;
+      sp[L - 1] = s;
+      for (int l = L - 1; l >= 1; --l) {
+        s = bp[(size_t)l * K + s];
+        sp[l - 1] = s;
+      }
+    }
+  }
+}
+
+template <int K, int RB, int STAGES, int G>
+size_t dp_smem_bytes(int L, bool bp_smem) {
+  using Lay = DpLayout<K, RB, STAGES, G>;
+  size_t b = (size_t)STAGES * Lay::STAGE_BYTES + 2 * K * 8;
+  if (G > 1) b += (size_t)G * K * 8 + (size_t)G * K * 4 + 8;
+  b += 2 * STAGES * 8;
+  if (bp_smem) b += (size_t)L * K;
+  return (b + 127) / 128 * 128;
+}
+
+template <int K, int RB, int STAGES, int G>
+int launch_cfg(const int64_t* d_T, int Bp, int L, uint8_t* d_bp, int64_t* d_opt, int32_t* d_strat, cudaStream_t st) {
+  using Lay = DpLayout<K, RB, STAGES, G>;
+  const bool bp_smem = (size_t)L * K <= 16 * 1024;
+  if (!bp_smem && d_bp == nullptr) { set_error("chain_dp: workspace for back-pointers missing"); return AUTODDL_EWORK; }
+  const size_t smem = dp_smem_bytes<K, RB, STAGES, G>(L, bp_smem);
+  if (smem > 227 * 1024) { set_error("chain_dp: %zu bytes of shared memory needed", smem); return AUTODDL_EINVAL; }
+  if (bp_smem) {
+    auto kern = chain_dp_kernel<K, RB, STAGES, G, true>;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<Bp, Lay::NT, smem, st>>>(d_T, L, d_bp, d_opt, d_strat);
+  } else {
+    auto kern = chain_dp_kernel<K, RB, STAGES, G, false>;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<Bp, Lay::NT, smem, st>>>(d_T, L, d_bp, d_opt, d_strat);
+  }
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+}  // namespace
+
+int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp, int64_t* d_opt_cost,
+                    int32_t* d_strategy, cudaStream_t st) {
+  switch (K) {
+    case 6:   return launch_cfg<6, 6, 4, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+    case 36:  return launch_cfg<36, 36, 3, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+    case 216: return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+  }
+  set_error("chain_dp: K must be 6, 36 or 216");
+  return AUTODDL_EINVAL;
+}
+
+}  // namespace autoddl

@@ -1,0 +1,128 @@
+// (a3) Multi-start Coordinate Descent (R10) for sm_100a.
+//
+// One block (one warp) per (problem, start).  A sweep visits l = 0..L-1 in order; the update of layer l
+//   s_l <- smallest-index argmin_c  T[l][s_{l-1}][c] + T[l+1][c][s_{l+1}]
+// reads one contiguous row and one strided column of the tables; lanes take candidates c, the minimum
+// and its lowest index are found with warp shuffles on the pair (cost, index).
+//
+// An update whose two neighbours have not changed since the layer was last updated would recompute the
+// same argmin (it is a deterministic function of (s_{l-1}, s_{l+1})), so it is skipped: a per-layer
+// dirty flag is set whenever a neighbour's signature changes.  The trajectory, the sweep count and the
+// result are identical to the plain algorithm; only redundant table reads disappear.
+#include "common.cuh"
+
+namespace autoddl {
+
+namespace {
+
+__device__ __forceinline__ void warp_argmin(int64_t& bv, int& bi) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+  }
+}
+
+template <int K>
+__global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int L, int S,
+                                                           const int32_t* __restrict__ init, int max_sweeps,
+                                                           int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
+                                                           int32_t* __restrict__ sweeps) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  int32_t* s = reinterpret_cast<int32_t*>(smem);            // [L]
+  uint8_t* dirty = reinterpret_cast<uint8_t*>(s + L);        // [L]
+
+  const int lane = threadIdx.x;
+  const size_t ps = blockIdx.x;
+  const size_t p = ps / S;
+  const int64_t* Tp = T + p * (size_t)L * K * K;
+
+  for (int l = lane; l < L; l += 32) {
+    s[l] = init[ps * L + l];
+    dirty[l] = 1;
+  }
+  __syncwarp();
+
+  int nsweeps = 0;
+  for (;;) {
+    bool changed = false;
+    for (int l = 0; l < L; ++l) {
+      if (!dirty[l]) continue;                               // warp-uniform
+      const int left = l > 0 ? s[l - 1] : 0;
+      const bool has_right = l < L - 1;
+      const int64_t* row = Tp + ((size_t)l * K + left) * K;
+      const int64_t* col = Tp + (size_t)(l + 1) * K * K + (has_right ? s[l + 1] : 0);
+      int64_t bv = INT64_MAX;
+      int bi = K;
+#pragma unroll
+      for (int c0 = 0; c0 < K; c0 += 32) {
+        const int c = c0 + lane;
+        if (c < K) {
+          int64_t g = __ldg(row + c);
+          if (has_right) g += __ldg(col + (size_t)c * K);
+          if (g < bv) { bv = g; bi = c; }
+        }
+      }
+      warp_argmin(bv, bi);
+      const int old = s[l];
+      __syncwarp();
+      if (lane == 0) {
+        dirty[l] = 0;
+        if (bi != old) {
+          s[l] = bi;
+          if (l > 0) dirty[l - 1] = 1;
+          if (has_right) dirty[l + 1] = 1;
+        }
+      }
+      changed |= (bi != old);
+      __syncwarp();
+    }
+    ++nsweeps;
+    if (!changed || nsweeps >= max_sweeps) break;
+  }
+
+  // Cost(s) = sum_l T[l][s_{l-1}][s_l]
+  int64_t acc = 0;
+  for (int l = lane; l < L; l += 32) {
+    const int left = l > 0 ? s[l - 1] : 0;
+    acc += __ldg(Tp + ((size_t)l * K + left) * K + s[l]);
+    strategy[ps * L + l] = s[l];
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+  if (lane == 0) {
+    cost[ps] = acc;
+    sweeps[ps] = nsweeps;
+  }
+}
+
+template <int K>
+int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
+             int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+  const size_t smem = ((size_t)L * 5 + 15) / 16 * 16;
+  if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
+  if (smem > 48 * 1024)
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int64_t nb = (int64_t)Bp * S;
+  if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
+  coord_descent_kernel<K><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+}  // namespace
+
+int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
+                         int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+  switch (K) {
+    case 6:   return launch_k<6>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 36:  return launch_k<36>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 216: return launch_k<216>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+  }
+  set_error("coord_descent: K must be 6, 36 or 216");
+  return AUTODDL_EINVAL;
+}
+
+}  // namespace autoddl

@@ -1,0 +1,234 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle: bit-exact, element by element.
+
+Run with `pytest -m gpu` on a B200.  All costs are int64, all indices int32/uint8: the bar is equality.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import ref
+from paper_2301_06813_b200 import configs as cf
+
+pytestmark = pytest.mark.gpu
+
+PEN = 1 << 50
+
+
+@pytest.fixture(scope="module")
+def adl():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (no CPU fallback exists)")
+    from paper_2301_06813_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _oracle_all(w, init):
+    T, node, mask = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+    dc, ds = ref.chain_dp(T)
+    cc, cs, sw = ref.coord_descent(T, init, w.max_sweeps)
+    return T, node, mask, dc, ds, cc, cs, sw
+
+
+def _gpu_all(adl, w, init):
+    d_layers = adl.layers_to_device(w.layers)
+    T, node, mask = adl.build_tables(d_layers, w.mesh, w.net)
+    dc, ds = adl.chain_dp(T, w.mesh)
+    cc, cs, sw = adl.coord_descent(T, torch.from_numpy(init).cuda(), w.mesh, w.max_sweeps)
+    torch.cuda.synchronize()
+    return [x.cpu().numpy() for x in (T, node, mask, dc, ds, cc, cs, sw)]
+
+
+def _assert_same(got, want, names=("T", "node", "mask", "dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps")):
+    for g, x, n in zip(got, want, names):
+        assert g.shape == x.shape and g.dtype == x.dtype, n
+        if not np.array_equal(g, x):
+            bad = np.argwhere(g != x)
+            raise AssertionError(f"{n}: {len(bad)} mismatches, first at {bad[0].tolist()}: got {g[tuple(bad[0])]} want {x[tuple(bad[0])]}")
+
+
+@pytest.mark.parametrize("k", [1, 2, 3])
+def test_configs_small_full(adl, k):
+    w = cf.CONFIGS[k]()
+    init = w.cd_init()
+    _assert_same(_gpu_all(adl, w, init), _oracle_all(w, init))
+
+
+def test_config5_k216(adl):
+    w = cf.config5_transformer96()
+    init = w.cd_init()[:, :96]                   # oracle CD: 1024 starts take ~4 s, 96 keep the suite short
+    _assert_same(_gpu_all(adl, w, init), _oracle_all(w, init))
+
+
+def test_config5_all_starts_properties(adl):
+    """all 1024 starts at full size: DP <= CD, cost == Cost(strategy), fixed point reached"""
+    w = cf.config5_transformer96()
+    init = torch.from_numpy(w.cd_init()).cuda()
+    T, _, _ = adl.build_tables(adl.layers_to_device(w.layers), w.mesh, w.net)
+    dc, ds = adl.chain_dp(T, w.mesh)
+    cc, cs, sw = adl.coord_descent(T, init, w.mesh, w.max_sweeps)
+    assert (cc >= dc[:, None]).all()
+    assert int(dc[0]) == 294_284_438_784         # tests/golden/survey_crosscheck.txt config5_dp
+    _check_costs(T, cs.reshape(1, -1, w.L), cc.reshape(1, -1))
+    _check_costs(T, ds.reshape(1, 1, w.L), dc.reshape(1, 1))
+
+
+def _check_costs(T, strat, cost):
+    """Cost(s) = sum_l T[l][s_{l-1}][s_l] recomputed with torch gathers for [Bp, S, L] strategies"""
+    Bp, S, L = strat.shape
+    K = T.shape[-1]
+    s = strat.long()
+    prev = torch.cat([torch.zeros_like(s[..., :1]), s[..., :-1]], dim=-1)
+    l = torch.arange(L, device=T.device).view(1, 1, L)
+    p = torch.arange(Bp, device=T.device).view(Bp, 1, 1)
+    flat = ((p * L + l) * K + prev) * K + s
+    tot = T.reshape(-1)[flat.reshape(-1)].reshape(Bp, S, L).sum(-1)
+    assert torch.equal(tot, cost)
+
+
+def test_config4_reduced_full_compare(adl):
+    w = cf.config4_batched(Bp=37, L=64)          # ragged: 37 problems
+    init = w.cd_init()
+    _assert_same(_gpu_all(adl, w, init), _oracle_all(w, init))
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 7])
+def test_config4_short_chains(adl, L):
+    w = cf.config4_batched(Bp=5, L=L, seed=3)
+    init = w.cd_init()
+    _assert_same(_gpu_all(adl, w, init), _oracle_all(w, init))
+
+
+def test_config4_full_size_sampled(adl):
+    """BASELINE.json configs[3] at full size (4096 x 64, the launch configuration bench.py times): the oracle
+    recomputes a sample of problems in full; properties are checked on all of them."""
+    w = cf.config4_batched()
+    init = w.cd_init()
+    d_layers = adl.layers_to_device(w.layers)
+    T, node, mask = adl.build_tables(d_layers, w.mesh, w.net)
+    dc, ds = adl.chain_dp(T, w.mesh)
+    cc, cs, sw = adl.coord_descent(T, torch.from_numpy(init).cuda(), w.mesh, w.max_sweeps)
+    torch.cuda.synchronize()
+    sample = [0, 1, 2, 147, 148, 1023, 2048, 3000, 4094, 4095] + np.random.default_rng(0).integers(0, 4096, 14).tolist()
+    mesh, net = ref.mesh_of(w), ref.net_of(w)
+    for p in sample:
+        oT, onode, omask = ref.build_tables(w.layers[p:p + 1], mesh, net)
+        odc, ods = ref.chain_dp(oT)
+        occ, ocs, osw = ref.coord_descent(oT, init[p:p + 1], w.max_sweeps)
+        got = [x[p:p + 1].cpu().numpy() for x in (T, node, mask, dc, ds, cc, cs, sw)]
+        _assert_same(got, (oT, onode, omask, odc, ods, occ, ocs, osw))
+    assert int(dc[0]) == 11_621_551_848          # tests/golden/survey_crosscheck.txt config4_problem0_dp
+    # properties at any size
+    _check_costs(T, ds.view(4096, 1, 64), dc.view(4096, 1))
+    _check_costs(T, cs, cc)
+    assert (cc >= dc[:, None]).all()
+    assert (dc < PEN).all()                      # no cap in config 4: always feasible
+    assert (sw >= 1).all() and (sw <= w.max_sweeps).all()
+
+
+def _random_tables(rng, Bp, L, K, hi):
+    T = rng.integers(0, hi, size=(Bp, L, K, K)).astype(np.int64)
+    T[rng.random(T.shape) < 0.08] += PEN
+    return T
+
+
+@pytest.mark.parametrize("K,L,Bp,hi", [(6, 1, 3, 10), (6, 9, 11, 4), (36, 2, 5, 3), (36, 65, 150, 7), (36, 33, 301, 10**9),
+                                        (216, 2, 2, 5), (216, 11, 3, 10**10), (216, 90, 1, 3)])
+def test_dp_cd_random_tables(adl, K, L, Bp, hi):
+    """generic tables with heavy ties and penalties; L*K > 16384 exercises back-pointers in the workspace"""
+    rng = np.random.default_rng(K * 1000 + L)
+    T = _random_tables(rng, Bp, L, K, hi)
+    S = 3
+    init = rng.integers(0, K, size=(Bp, S, L)).astype(np.int32)
+    mesh = cf.Mesh(tuple([2] * {6: 1, 36: 2, 216: 3}[K]), tuple([0] * {6: 1, 36: 2, 216: 3}[K]))
+    dT = torch.from_numpy(T).cuda()
+    dc, ds = adl.chain_dp(dT, mesh)
+    cc, cs, sw = adl.coord_descent(dT, torch.from_numpy(init).cuda(), mesh, 64)
+    odc, ods = ref.chain_dp(T)
+    occ, ocs, osw = ref.coord_descent(T, init, 64)
+    _assert_same([x.cpu().numpy() for x in (dc, ds, cc, cs, sw)], (odc, ods, occ, ocs, osw),
+                 names=("dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps"))
+
+
+def test_cd_sweep_cap(adl):
+    rng = np.random.default_rng(5)
+    T = _random_tables(rng, 4, 40, 36, 1000)
+    init = rng.integers(0, 36, size=(4, 6, 40)).astype(np.int32)
+    mesh = cf.Mesh((2, 2), (0, 0))
+    for cap in (1, 2, 3):
+        cc, cs, sw = adl.coord_descent(torch.from_numpy(T).cuda(), torch.from_numpy(init).cuda(), mesh, cap)
+        occ, ocs, osw = ref.coord_descent(T, init, cap)
+        _assert_same([x.cpu().numpy() for x in (cc, cs, sw)], (occ, ocs, osw), names=("cd_cost", "cd_strategy", "cd_sweeps"))
+
+
+def test_fused_build_paths_and_search_host(adl):
+    """d_T == NULL (tables built into the workspace) and the host-pointer end-to-end call"""
+    w = cf.config4_batched(Bp=9, L=17, seed=2)
+    init = w.cd_init()
+    want = _oracle_all(w, init)
+    d_layers = adl.layers_to_device(w.layers)
+    dc, ds = adl.chain_dp(None, w.mesh, net=w.net, d_layers=d_layers)
+    cc, cs, sw = adl.coord_descent(None, torch.from_numpy(init).cuda(), w.mesh, w.max_sweeps, net=w.net, d_layers=d_layers)
+    _assert_same([x.cpu().numpy() for x in (dc, ds, cc, cs, sw)], want[3:],
+                 names=("dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps"))
+    work = torch.empty(adl.workspace_bytes(w.Bp, w.L, w.S, w.mesh), dtype=torch.uint8, device="cuda")
+    out = adl.search_host(w, init, work)
+    _assert_same([out["opt_cost"], out["strategy"], out["cd_cost"], out["cd_strategy"], out["cd_sweeps"]], want[3:],
+                 names=("dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps"))
+    w5 = cf.config5_transformer96()               # back-pointers in the workspace, no CD
+    work = torch.empty(adl.workspace_bytes(w5.Bp, w5.L, 0, w5.mesh), dtype=torch.uint8, device="cuda")
+    out = adl.search_host(w5, None, work)
+    assert int(out["opt_cost"][0]) == 294_284_438_784
+
+
+def test_ragged_dims_and_mesh_with_unit_level(adl):
+    """non-divisible tensor dims (ceil shards), a level of size 1 and a 3-level odd mesh"""
+    rng = np.random.default_rng(9)
+    for sizes, links in [((3, 5), (1, 0)), ((1, 7), (1, 0)), ((2, 3, 5), (1, 1, 0)), ((4,), (1,))]:
+        L = 6
+        recs = []
+        for l in range(L):
+            M, Kd, N = (int(x) for x in rng.integers(1, 3000, 3))
+            if l % 3 == 1:
+                recs.append(cf.attn(M, N, int(rng.integers(1, 3000)), 2, int(rng.integers(1, 40)), int(rng.integers(1, 40))))
+            else:
+                recs.append(cf.gemm(M, Kd, N, 2, 4, 18, in_rows=int(rng.integers(1, 5000)), in_cols=int(rng.integers(1, 5000)),
+                                    max_rows=int(rng.integers(1, 64)), max_cols=int(rng.integers(1, 64))))
+        layers = np.zeros((1, L), dtype=cf.LAYER_DTYPE)
+        for l, r in enumerate(recs):
+            layers[0, l] = r
+        w = cf.Workload("ragged", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), 150_000 * L), S=4, seed=1)
+        init = w.cd_init()
+        _assert_same(_gpu_all(adl, w, init), _oracle_all(w, init))
+
+
+def test_large_dims_64bit(adl):
+    """dims beyond 32 bits in bytes (the paper's 2^20 x 8192 fp32 activation)"""
+    layers = np.zeros((1, 3), dtype=cf.LAYER_DTYPE)
+    for l in range(3):
+        layers[0, l] = cf.gemm(2**20, 8192, 8192 * 3, 4, 4, 16)
+    w = cf.Workload("big", layers, cf.Mesh((4, 16), (1, 1)), cf.Net((0, 0), (1, 1), 0), S=2)
+    init = w.cd_init()
+    got = _gpu_all(adl, w, init)
+    _assert_same(got, _oracle_all(w, init))
+    assert got[0][0, 1, 1, 1] - got[1][0, 1, 1] == 15 * 2**30     # (S0,S1)->(S0,B): the paper's 15 GB
+
+
+def test_errors(adl):
+    import ctypes as C
+    w = cf.config1_tiny()
+    d_layers = adl.layers_to_device(w.layers)
+    bad = cf.Mesh((2, 2, 2, 2), (0, 0, 0, 0))
+    with pytest.raises(Exception):
+        adl.num_signatures(bad)
+    T, _, _ = adl.build_tables(d_layers, w.mesh, w.net)
+    w5 = cf.config5_transformer96()
+    T5 = torch.zeros((1, 480, 216, 216), dtype=torch.int64, device="cuda")
+    with pytest.raises(adl.AutoddlError, match="workspace"):
+        adl.chain_dp(T5, w5.mesh, work=torch.empty(256, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(adl.AutoddlError):
+        adl.coord_descent(T, torch.zeros((1, 1, 4), dtype=torch.int32, device="cuda"), w.mesh, 0)
+    m, n = adl.c_mesh(w.mesh), adl.c_net(w.net)
+    rc = adl.lib().autoddl_build_tables(None, 1, 4, C.addressof(m), C.addressof(n), None, None, None, None)
+    assert rc == -1 and b"NULL" in adl.lib().autoddl_last_error()
