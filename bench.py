@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- AutoDDL strategy-search hot path on B200 (contract: see DESIGN.md section 8).
+
+One "step" = one pass of the whole hot path over one batch of synthetic input:
+  (a1) autoddl_build_tables -> (a2) autoddl_chain_dp -> (a3) autoddl_coord_descent
+on BASELINE.json configs[3] (4096 independent chains x 64 GEMM layers, mesh 4 x 4, K = 36), the
+configuration the metric is quoted on.  Inputs (layer records, CD starts) are resident in HBM for
+`value`; `e2e` goes through autoddl_search_host with pinned HOST buffers (H2D + D2H inside the timed
+region).  `--impl reference` times the CPU oracle (oracle/, plain single-threaded C++) instead.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...     (N > 1: one rank per GPU)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2301_06813_b200 import configs as cf  # noqa: E402
+
+METRIC = "SBP cost-table cells/s, min-plus DP cells/s, CD sweeps/s on 1 B200 vs HBM roofline"
+FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload_desc(w, extra=None):
+    d = {
+        "workload": "configs[3] batched random chains: %d problems x L=%d GEMM layers, dims log-uniform [256,16384], "
+                    "fp16 act / fp32 wgrad, mesh 4x4 (inter 25 GB/s, intra 300 GB/s), K=%d, 1 CD start per problem"
+                    % (w.Bp, w.L, w.K),
+        "Bp_per_gpu": w.Bp, "L": w.L, "K": w.K, "cd_starts": w.S, "seed": w.seed,
+        "cells_per_gpu": w.cells, "table_bytes_per_gpu": w.cells * 8,
+        "l2": "tables (2.7 GB) exceed the 126 MB L2, so every step streams them through HBM; no explicit flush",
+    }
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py may execute oracle/)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample_run(w, nprob, repeat=1):
+    """whole path of the oracle, as it stands, single thread, on the first nprob problems"""
+    from oracle import ref
+    mesh, net = ref.mesh_of(w), ref.net_of(w)
+    layers = np.ascontiguousarray(w.layers[:nprob])
+    init = np.ascontiguousarray(w.cd_init()[:nprob])
+    t = {"build": 0.0, "dp": 0.0, "cd": 0.0}
+    sweeps = 0
+    for _ in range(repeat):
+        t0 = time.perf_counter()
+        T, _, _ = ref.build_tables(layers, mesh, net)
+        t1 = time.perf_counter()
+        ref.chain_dp(T)
+        t2 = time.perf_counter()
+        _, _, sw = ref.coord_descent(T, init, w.max_sweeps)
+        t3 = time.perf_counter()
+        t["build"] += t1 - t0
+        t["dp"] += t2 - t1
+        t["cd"] += t3 - t2
+        sweeps += int(sw.sum())
+    cells = nprob * w.L * w.K * w.K * repeat
+    return cells, sweeps, t
+
+
+def cpu_baseline(w, nprob=1024):
+    cells, sweeps, t = oracle_sample_run(w, nprob)
+    tot = t["build"] + t["dp"] + t["cd"]
+    return {
+        "value": cells / tot, "unit": "cells/s", "cores": 1, "kind": "oracle",
+        "sample": "first %d of %d problems of the same workload, whole path (build + DP + CD), single-threaded "
+                  "g++ -O2 oracle, %.1f s" % (nprob, w.Bp, tot),
+        "parts": {"build_cells_per_s": cells / t["build"], "dp_cells_per_s": cells / t["dp"],
+                  "cd_sweeps_per_s": sweeps / t["cd"]},
+    }
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the box's host cores; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = cf.config4_batched()
+    nprob = max(4, min(48, 48 * 200 // max(args.steps, 1)))      # whole run stays within a few minutes
+    for _ in range(args.warmup):
+        oracle_sample_run(w, 4)
+    t0 = time.perf_counter()
+    cells = 0
+    parts = {"build": 0.0, "dp": 0.0, "cd": 0.0}
+    sweeps = 0
+    for _ in range(args.steps):
+        c, s, t = oracle_sample_run(w, nprob)
+        cells += c
+        sweeps += s
+        for k in parts:
+            parts[k] += t[k]
+    el = time.perf_counter() - t0
+    val = cells / el
+    sample = "each step = whole path on the first %d of %d problems, single-threaded oracle" % (nprob, w.Bp)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "cells/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int64", "data": "synthetic (seeded splitmix64)",
+        "config": workload_desc(w, {"sample": sample}),
+        "cpu_baseline": {"value": val, "unit": "cells/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "cells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "parts": {"build_cells_per_s": cells / parts["build"], "dp_cells_per_s": cells / parts["dp"],
+                  "cd_sweeps_per_s": sweeps / parts["cd"]},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback (use --impl reference for the oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2301_06813_b200 import binding as adl
+    adl.lib()
+
+    # weak scaling: every rank searches its own 4096 problems (seed = rank); no data-path collective
+    w = cf.config4_batched(seed=rank)
+    init_np = w.cd_init()
+    d_layers = adl.layers_to_device(w.layers)
+    d_init = torch.from_numpy(init_np).cuda()
+    K, L, Bp, S = w.K, w.L, w.Bp, w.S
+    T = torch.empty((Bp, L, K, K), dtype=torch.int64, device="cuda")
+    dp_out = (torch.empty(Bp, dtype=torch.int64, device="cuda"), torch.empty((Bp, L), dtype=torch.int32, device="cuda"))
+    cd_out = (torch.empty((Bp, S), dtype=torch.int64, device="cuda"), torch.empty((Bp, S, L), dtype=torch.int32, device="cuda"),
+              torch.empty((Bp, S), dtype=torch.int32, device="cuda"))
+
+    def step(evs=None):
+        if evs: evs[0].record()
+        adl.build_tables(d_layers, w.mesh, w.net, want_node_mask=False, out=T)
+        if evs: evs[1].record()
+        adl.chain_dp(T, w.mesh, out=dp_out)
+        if evs: evs[2].record()
+        adl.coord_descent(T, d_init, w.mesh, w.max_sweeps, out=cd_out)
+        if evs: evs[3].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    total_sweeps = int(cd_out[2].sum().item())
+
+    # ---- timed region: exactly K steps, CUDA events on the launching (current) stream ----------------
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = adl.launch_count()
+    barrier()
+    e_start.record()
+    for k in range(args.steps):
+        step(evs[k])
+    e_end.record()
+    barrier()
+    launches = adl.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    ms_total = e_start.elapsed_time(e_end)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms = {"build": 0.0, "dp": 0.0, "cd": 0.0}
+    for e in evs:
+        ms["build"] += e[0].elapsed_time(e[1]); ms["dp"] += e[1].elapsed_time(e[2]); ms["cd"] += e[2].elapsed_time(e[3])
+    for k in ms:
+        ms[k] /= args.steps
+    ms_step = ms_total / args.steps
+    cells = w.cells
+    value = world * cells / (ms_step * 1e-3)
+
+    # ---- HBM copy peak by our own copy kernel, in the same run -------------------------------------------
+    nb = 1 << 30
+    a = torch.empty(nb, dtype=torch.uint8, device="cuda").random_(0, 255)
+    b = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    best = 1e9
+    for i in range(13):
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(); adl.copy_probe(a, b); s1.record(); torch.cuda.synchronize()
+        if i >= 3:
+            best = min(best, s0.elapsed_time(s1))
+    copy_gbs = 2 * nb / (best * 1e-3) / 1e9
+    del a, b
+
+    # ---- end to end through the host-pointer C-ABI call (pinned host buffers, H2D + D2H timed) -----------
+    work = torch.empty(adl.workspace_bytes(Bp, L, S, w.mesh), dtype=torch.uint8, device="cuda")
+    pinned = adl.alloc_host_outputs(Bp, L, S)
+    h_layers = torch.from_numpy(np.ascontiguousarray(w.layers).view(np.uint8).reshape(Bp, L, 64).copy()).pin_memory()
+    h_init = torch.from_numpy(init_np.copy()).pin_memory()
+    w_host = cf.Workload(w.name, h_layers.numpy().view(cf.LAYER_DTYPE).reshape(Bp, L), w.mesh, w.net, S=S, seed=w.seed)
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(3):
+        adl.search_host(w_host, h_init.numpy(), work, pinned)
+    barrier()
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record()
+    for _ in range(e2e_steps):
+        adl.search_host(w_host, h_init.numpy(), work, pinned)
+    s1.record()
+    barrier()
+    e2e_ms = s0.elapsed_time(s1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_ms /= e2e_steps
+    h2d = h_layers.numel() + h_init.numel() * 4
+    d2h = sum(v.numel() * v.element_size() for v in pinned.values())
+    assert np.array_equal(pinned["opt_cost"].numpy(), dp_out[0].cpu().numpy())      # same answers through both routes
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        table_bytes = cells * 8
+        dp_bytes = (L - 1) * Bp * K * K * 8 + Bp * K * 8          # tile 0 contributes one row
+        cd_alg_bytes = total_sweeps * 16 * K * L
+        kernels = {
+            "build_tables": {"ms": ms["build"], "cells_per_s": cells / (ms["build"] * 1e-3),
+                             "alg_GBps": table_bytes / (ms["build"] * 1e-3) / 1e9, "bound": "hbm (write 8 B/cell)"},
+            "chain_dp": {"ms": ms["dp"], "cells_per_s": cells / (ms["dp"] * 1e-3),
+                         "alg_GBps": dp_bytes / (ms["dp"] * 1e-3) / 1e9, "bound": "hbm (read 8 B/cell)"},
+            "coord_descent": {"ms": ms["cd"], "sweeps_per_s": total_sweeps / (ms["cd"] * 1e-3), "sweeps": total_sweeps,
+                              "alg_GBps": cd_alg_bytes / (ms["cd"] * 1e-3) / 1e9, "bound": "latency / hbm (16*K*L B per sweep)"},
+        }
+        for k in kernels.values():
+            k["frac_of_peak"] = k["alg_GBps"] / peak
+        dom = max(("build_tables", "chain_dp", "coord_descent"), key=lambda n: kernels[n]["ms"])
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")          # per-launch DRAM bytes from the ncu --set full capture
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(dom)
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": value, "unit": "cells/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+            "data": "synthetic (seeded splitmix64; shapes of BASELINE.json configs[3])",
+            "config": workload_desc(w, {"parallelism": "problems sharded over %d GPU(s), no collective in the data path" % world}),
+            "parts": {"build_cells_per_s": world * kernels["build_tables"]["cells_per_s"],
+                      "dp_cells_per_s": world * kernels["chain_dp"]["cells_per_s"],
+                      "cd_sweeps_per_s": world * kernels["coord_descent"]["sweeps_per_s"]},
+            "kernels": kernels,
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
+                         "frac": kernels[dom]["alg_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+                         "copy_probe_GBps_same_run": copy_gbs},
+            "e2e": {"value": world * cells / (e2e_ms * 1e-3), "unit": "cells/s", "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+            "gpu_launches": launches,
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
