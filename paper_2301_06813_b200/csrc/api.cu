@@ -25,10 +25,23 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
     ADL_REQUIRE(mesh->size[d] >= 1 && mesh->size[d] <= 65536, "mesh.size[%d] = %d out of range", d, mesh->size[d]);
     ADL_REQUIRE(mesh->link[d] == 0 || mesh->link[d] == 1, "mesh.link[%d] = %d, must be 0 or 1", d, mesh->link[d]);
   }
+  int64_t prod = 1;
+  for (int d = 0; d < mesh->ndim; ++d) prod *= mesh->size[d];
+  ADL_REQUIRE(prod <= (1 << 20), "mesh has %lld devices, at most 2^20 supported", (long long)prod);
   if (out) {
     memset(out, 0, sizeof(*out));
     out->ndim = mesh->ndim;
-    for (int d = 0; d < mesh->ndim; ++d) out->size[d] = mesh->size[d];
+    for (int d = 0; d < mesh->ndim; ++d) {
+      out->size[d] = mesh->size[d];
+      out->magic_size[d] = (uint64_t)((((unsigned __int128)1 << 64) + mesh->size[d] - 1) / mesh->size[d]);
+    }
+    for (int m = 0; m < 8; ++m) {
+      int64_t f = 1;
+      for (int d = 0; d < mesh->ndim; ++d)
+        if (m >> d & 1) f *= mesh->size[d];
+      out->sub[m] = (int32_t)f;
+      out->magic_sub[m] = (uint64_t)((((unsigned __int128)1 << 64) + f - 1) / f);
+    }
   }
   if (net) {
     for (int c = 0; c < 2; ++c) {

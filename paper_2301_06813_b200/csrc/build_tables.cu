@@ -7,19 +7,21 @@
 //   V: all-reduce of the weight gradient on every level where W is replicated
 //   feasibility: split limits and per-device memory
 //
-// Design (differs from the plain per-cell evaluation on purpose):
-//   one CTA builds one K x K tile.  A redistribution moves every mesh level through the fixed
-//   state sequence  (start) -> after slice -> after reduce-scatter -> after all-to-all -> after
-//   all-gather, and that sequence depends only on the level's own (from,to) pair; levels interact
-//   only through the local tensor size at the moment a collective runs.  So per tile we compute
-//     1. ceil(rows/f0), ceil(cols/f1) for every subset of levels               (<= 16 divisions)
-//     2. CG[d][cfg], CA[d][cfg]: gather/scatter and all-to-all cost on level d when the levels are
-//        split as cfg (3^D configurations)                                     (<= 81 divisions)
-//     3. R[a][b] over the 4^D x 4^D state vectors: a sum of <= 3D table entries
-//     4. E[a][b] = R[a][b] + R[dual b][dual a]   (in place: the map is an involution)
-//     5. VP[j] = V + penalty, node, mask per consumer signature
-//     6. the K x K expansion: one shared-memory gather + one 64-bit add per cell, 16-byte stores.
-//   The kernel is then bound by the HBM write of 8 B per cell, not by integer arithmetic.
+// Design (differs from a per-cell evaluation on purpose).  A redistribution moves
+// every mesh level through a fixed sequence of states -- after the free slice, after reduce-scatter,
+// after all-to-all, after all-gather -- that depends only on the level's own (from, to) pair; levels
+// interact only through the local tensor size at the moment a collective runs.  Per K x K tile:
+//   1. Q[x][m] = ceil(x / prod(levels in m)) for the five extents and every level subset (magic-number
+//      division: divisors are fixed per launch)
+//   2. per level d and split configuration cfg (3^D of them): gather/scatter cost CG, all-to-all cost CA
+//      of the input tensor, all-reduce cost of the weight gradient, local sizes of W and O
+//   3. R[a][b] over the 4^D x 4^D state vectors = a sum of <= 3D table entries whose addresses do not
+//      depend on the tile (hoisted out of the persistent tile loop when one thread owns one entry);
+//      VP[j] = node cost + penalty per consumer signature from the step-2 tables
+//   4. only 4^D (+1) distinct rows exist: Erow[a][j] = R[a][b_j] + R[dual b_j][dual a] + VP[j]
+//      (forward leg + backward leg, b_j = I-state vector of consumer signature j)
+//   5. every output row is a copy of one Erow row: 16-byte shared loads, 16-byte streaming stores.
+// The kernel is then bound by the HBM write of 8 B per cell instead of integer arithmetic.
 #include "common.cuh"
 
 namespace autoddl {
@@ -28,256 +30,324 @@ namespace {
 
 constexpr int kS0 = 0, kS1 = 1, kB = 2, kP = 3;
 
-// per-level signature rows (PAPER.md:193 rows 0..2; replicate; partial pass-through), see DESIGN.md R1
+// per-level signature rows (PAPER.md:193 rows 0..2; replicate; partial pass-through), DESIGN.md R1
 __device__ __constant__ int8_t c_gemm_I[6] = {kS0, kB, kS1, kB, kP, kB};
 __device__ __constant__ int8_t c_gemm_W[6] = {kB, kS1, kS0, kB, kB, kP};
 __device__ __constant__ int8_t c_gemm_O[6] = {kS0, kS1, kP, kB, kP, kP};
 __device__ __constant__ int8_t c_attn_IO[6] = {kS0, kS1, -1, kB, -1, -1};
 
-__device__ __forceinline__ int64_t cdiv64(int64_t a, int64_t b) {
-  // operands are non-negative; most values fit 32 bits, where the division is ~5x cheaper
-  if (((uint64_t)a | (uint64_t)b) >> 32) return (a + b - 1) / b;
-  const uint32_t ua = (uint32_t)a, ub = (uint32_t)b;
-  const uint32_t q = ua / ub;
-  return (int64_t)(q + (q * ub != ua));
+// ---- one level's walk through a redistribution a -> b, packed ----------------------------------------
+// bits 0-1 / 2-3 / 4-5 / 6-7: split code (0 none, 1 rows, 2 cols) after slice / reduce-scatter / all-to-all /
+// all-gather; bit 8: reduce-scatter runs, bit 9: all-to-all runs, bit 10: all-gather runs.
+constexpr bool cx_split(int s) { return s == kS0 || s == kS1; }
+constexpr int cx_code(int s) { return s == kS0 ? 1 : (s == kS1 ? 2 : 0); }
+constexpr uint32_t cx_walk(int a, int b) {
+  const int s0 = (a == kB && cx_split(b)) ? b : a;                 // replicated -> split: keep own slice, free
+  const bool r1 = (s0 == kP && b != kP);                           // partial -> anything else: reduce-scatter
+  const int s1 = r1 ? (b == kB ? kS1 : b) : s0;
+  const bool r2 = cx_split(s1) && cx_split(b) && s1 != b;          // change of split axis: all-to-all
+  const int s2 = r2 ? b : s1;
+  const bool r3 = cx_split(s2) && b == kB;                         // split -> replicated: all-gather
+  const int s3 = r3 ? kB : s2;
+  return (uint32_t)(cx_code(s0) | cx_code(s1) << 2 | cx_code(s2) << 4 | cx_code(s3) << 6 | (r1 ? 256 : 0) |
+                    (r2 ? 512 : 0) | (r3 ? 1024 : 0));
 }
+struct WalkTable { uint32_t w[16]; };
+constexpr WalkTable make_walks() {
+  WalkTable t{};
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) t.w[a * 4 + b] = cx_walk(a, b);
+  return t;
+}
+__device__ __constant__ WalkTable c_walk = make_walks();
 
-__device__ __forceinline__ int split_code(int s) { return s == kS0 ? 1 : (s == kS1 ? 2 : 0); }
-__device__ __forceinline__ bool is_split(int s) { return s == kS0 || s == kS1; }
 __device__ __forceinline__ int dual_of(int s) { return s == kB ? kP : (s == kP ? kB : s); }
+
+// ceil(n / d) for n >= 0 with the launch-constant divisor d and M = ceil(2^64 / d): the multiply-high
+// quotient is exact for n < 2^64 / d (d <= 2^20 is enforced by the API, so n < 2^43 is safe).
+__device__ __forceinline__ int64_t cdiv_magic(int64_t n, uint32_t d, uint64_t M) {
+  if (d == 1) return n;
+  if ((uint64_t)n < (1ull << 43)) {
+    const uint64_t q = __umul64hi((uint64_t)n, M);
+    return (int64_t)(q + (q * d != (uint64_t)n));
+  }
+  return (n + d - 1) / d;
+}
 
 template <int D> struct Pow { };
 template <> struct Pow<1> { static constexpr int K = 6, NS = 4, NC = 3; };
 template <> struct Pow<2> { static constexpr int K = 36, NS = 16, NC = 9; };
 template <> struct Pow<3> { static constexpr int K = 216, NS = 64, NC = 27; };
 
-template <int D>
-struct TileSmem {
-  int64_t rowc[8];                        // ceil(in_rows / prod of the levels in the subset)
-  int64_t colc[8];
-  int64_t CG[D][Pow<D>::NC];              // all-gather == reduce-scatter cost on level d under split config
-  int64_t CA[D][Pow<D>::NC];              // all-to-all cost
-  int64_t VP[Pow<D>::K];                  // node cost + penalty per consumer signature
-  int16_t aidx[Pow<D>::K];                // producer signature -> O state-vector index (or -1)
-  int16_t bidx[Pow<D>::K];                // consumer signature -> I state-vector index (or -1)
-  int64_t E[Pow<D>::NS * Pow<D>::NS];     // R, then E in place
+// per (layer kind, signature) facts, built once per CTA
+struct SigInfo {
+  int16_t a_idx;      // O state-vector index, or NS (zero-edge row) when the signature is invalid for the kind
+  int16_t b_idx;      // I state-vector index, or -1
+  uint8_t cfgW, cfgO; // split configuration of W / of O
+  uint8_t mI0, mI1;   // level subsets splitting the input's rows / cols
+  uint8_t wB;         // levels on which W is replicated
+  uint8_t valid;
+  int32_t rowsplit, colsplit;
 };
 
 template <int D>
-__global__ void __launch_bounds__(256) build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles,
-                                                           int L, MeshParams mp, int64_t* __restrict__ T,
-                                                           int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
-  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
+struct TileSmem {
+  static constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
+  static constexpr bool kRows = (D <= 2);               // distinct-row expansion (steps 4/5)
+  SigInfo sig[2][K];
+  int64_t Q[5][8];                                      // M, Kd, N, in_rows, in_cols  x  level subset
+  int64_t CG[D][NC + 1];                                // [..][NC] = 0: the slot that does not run
+  int64_t CA[D][NC + 1];
+  int64_t WAR[D][NC];
+  int64_t locW[NC], locO[NC];
+  alignas(16) int64_t VP[K];
+  alignas(16) int64_t E[NS * NS];
+  alignas(16) int64_t Erow[kRows ? (NS + 1) * K : 1];
+};
+
+
+// split configuration index -> level subsets (rows, cols)
+template <int D>
+__device__ __forceinline__ void cfg_masks(int cfg, int& m0, int& m1) {
+  m0 = m1 = 0;
+#pragma unroll
+  for (int e = 0; e < D; ++e) {
+    const int sp = cfg % 3;
+    cfg /= 3;
+    if (sp == 1) m0 |= 1 << e;
+    if (sp == 2) m1 |= 1 << e;
+  }
+}
+
+// the <= 3D table entries whose sum is R[av][bv]; entries that do not run point at a zero slot
+template <int D>
+__device__ __forceinline__ void r_slots(int av, int bv, int (&idx)[3 * D]) {
+  constexpr int NC = Pow<D>::NC, STRIDE = NC + 1, CA_OFF = D * STRIDE, ZERO = NC;
+  int c0[D], c1[D], c2[D], c3[D];
+  bool r1[D], r2[D], r3[D];
+  int pw = 1;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    const int sh = 2 * (D - 1 - d);
+    const uint32_t w = c_walk.w[((av >> sh) & 3) * 4 + ((bv >> sh) & 3)];
+    c0[d] = (w & 3) * pw; c1[d] = (w >> 2 & 3) * pw; c2[d] = (w >> 4 & 3) * pw; c3[d] = (w >> 6 & 3) * pw;
+    r1[d] = w >> 8 & 1; r2[d] = w >> 9 & 1; r3[d] = w >> 10 & 1;
+    pw *= 3;
+  }
+  int n = 0;
+#pragma unroll
+  for (int d = D - 1; d >= 0; --d) {        // reduce-scatter, innermost level first; message = tensor before it
+    int cfg = 0;
+#pragma unroll
+    for (int e = 0; e < D; ++e) cfg += (e > d) ? c1[e] : (e < d ? c0[e] : 0);
+    idx[n++] = r1[d] ? d * STRIDE + cfg : ZERO;
+  }
+#pragma unroll
+  for (int d = D - 1; d >= 0; --d) {        // all-to-all, innermost first; message = tensor after it
+    int cfg = 0;
+#pragma unroll
+    for (int e = 0; e < D; ++e) cfg += (e > d) ? c2[e] : (e < d ? c1[e] : c2[e]);
+    idx[n++] = r2[d] ? CA_OFF + d * STRIDE + cfg : ZERO;
+  }
+#pragma unroll
+  for (int d = 0; d < D; ++d) {             // all-gather, outermost first; message = tensor after it
+    int cfg = 0;
+#pragma unroll
+    for (int e = 0; e < D; ++e) cfg += (e < d) ? c3[e] : (e > d ? c2[e] : 0);
+    idx[n++] = r3[d] ? d * STRIDE + cfg : ZERO;
+  }
+}
+
+template <int D>
+__device__ __forceinline__ int dual_vec(int v) {
+  int r = 0;
+#pragma unroll
+  for (int d = 0; d < D; ++d) r |= dual_of((v >> (2 * d)) & 3) << (2 * d);
+  return r;
+}
+
+template <int D>
+__global__ void __launch_bounds__(256, (D == 3) ? 1 : 4)
+build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
+                    int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  using SM = TileSmem<D>;
+  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2;
+  constexpr bool kHoist = (NS * NS <= NT);
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  TileSmem<D>& sm = *reinterpret_cast<TileSmem<D>*>(smem_raw);
-  const int tid = threadIdx.x, NT = blockDim.x;
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  const int tid = threadIdx.x;
+  const int64_t* tab = &sm.CG[0][0];                     // CG then CA, contiguous
+
+  // ---- once per CTA: facts per (kind, signature) -----------------------------------------------------
+  for (int x = tid; x < 2 * K; x += NT) {
+    const int kind = x / K, j = x % K;
+    int dig[D], r = j;
+#pragma unroll
+    for (int d = D - 1; d >= 0; --d) { dig[d] = r % 6; r /= 6; }
+    SigInfo si{};
+    int a = 0, b = 0, cw = 0, co = 0, pw = 1, rs = 1, cs = 1;
+    bool valid = true;
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      const int g = dig[d];
+      int sI, sO, sW;
+      if (kind == AUTODDL_GEMM) { sI = c_gemm_I[g]; sO = c_gemm_O[g]; sW = c_gemm_W[g]; }
+      else { sI = sO = c_attn_IO[g]; sW = kB; if (sI < 0) { valid = false; sI = sO = kB; } }
+      a = a * 4 + sO;
+      b = b * 4 + sI;
+      cw += (sW == kS0 ? 1 : sW == kS1 ? 2 : 0) * pw;
+      co += (sO == kS0 ? 1 : sO == kS1 ? 2 : 0) * pw;
+      pw *= 3;
+      if (sI == kS0) si.mI0 |= 1 << d;
+      if (sI == kS1) si.mI1 |= 1 << d;
+      if (sW == kB) si.wB |= 1 << d;
+      if (sI == kS0 || sO == kS0) rs *= mp.size[d];
+      if (sO == kS1) cs *= mp.size[d];
+    }
+    si.a_idx = valid ? a : NS;
+    si.b_idx = valid ? b : -1;
+    si.cfgW = cw; si.cfgO = co; si.valid = valid; si.rowsplit = rs; si.colsplit = cs;
+    sm.sig[kind][j] = si;
+  }
+  if (tid < D) { sm.CG[tid][NC] = 0; sm.CA[tid][NC] = 0; }
+
+  // tile-invariant roles of this thread
+  int slot[3 * D];
+  if (kHoist) {
+    if (tid < NS * NS) r_slots<D>(tid / NS, tid % NS, slot);
+    else {
+#pragma unroll
+      for (int k = 0; k < 3 * D; ++k) slot[k] = NC;
+    }
+  }
+  int roleA_m0 = 0, roleA_m1 = 0;
+  {
+    const int t = tid < 96 ? tid : (tid < 192 ? tid - 96 : tid - 192);
+    cfg_masks<D>(t % NC, roleA_m0, roleA_m1);
+  }
+  const int64_t cap_layer = mp.mem_cap / L;
+  __syncthreads();
 
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int l = tile % L;
     const autoddl_layer* cur = layers + tile;
-    // uniform per CTA: served by one broadcast transaction each
-    const int64_t in_rows = __ldg(&cur->in_rows), in_cols = __ldg(&cur->in_cols);
     const int kind = __ldg(&cur->kind);
-    const int64_t eb = __ldg(&cur->act_bytes);
     const int kind_prev = (l > 0) ? __ldg(&(cur - 1)->kind) : AUTODDL_GEMM;
+    const int64_t eb = __ldg(&cur->act_bytes);
 
-    // ---- 1. subset quotients ------------------------------------------------------------------
-    if (tid < 2 * (1 << D)) {
-      const int m = tid & ((1 << D) - 1);
-      int64_t f = 1;
-#pragma unroll
-      for (int d = 0; d < D; ++d)
-        if (m >> d & 1) f *= mp.size[d];
-      if (tid < (1 << D)) sm.rowc[m] = cdiv64(in_rows, f);
-      else                sm.colc[m] = cdiv64(in_cols, f);
+    // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
+    if (tid < 5 * (1 << D)) {
+      const int x = tid >> D, m = tid & ((1 << D) - 1);
+      const int64_t X = __ldg(reinterpret_cast<const int64_t*>(cur) + x);
+      sm.Q[x][m] = cdiv_magic(X, (uint32_t)mp.sub[m], mp.magic_sub[m]);
     }
-    // signature -> state-vector indices (base 4, level 0 most significant)
+    __syncthreads();
+
+    // ---- 2. tables per level and split configuration -------------------------------------------------------
+    if (tid < D * NC) {
+      if (l > 0) {                                           // input tensor: Table 2 rows 2 and 3
+        const int d = tid / NC;
+        const int64_t n = sm.Q[3][roleA_m0] * sm.Q[4][roleA_m1] * eb;
+        const int64_t p = mp.size[d];
+        int64_t cg = 0, ca = 0;
+        if (p > 1) {
+          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+        }
+        sm.CG[d][tid % NC] = cg;
+        sm.CA[d][tid % NC] = ca;
+      }
+    } else if (tid >= 96 && tid < 96 + D * NC) {
+      if (kind == AUTODDL_GEMM) {                            // weight gradient: AllReduce row
+        const int t = tid - 96, d = t / NC;
+        const int64_t n = sm.Q[1][roleA_m0] * sm.Q[2][roleA_m1] * (int64_t)__ldg(&cur->wgrad_bytes);
+        const int64_t p = mp.size[d];
+        sm.WAR[d][t % NC] =
+            p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
+      }
+    } else if (tid >= 192 && tid < 192 + NC) {
+      sm.locW[tid - 192] = sm.Q[1][roleA_m0] * sm.Q[2][roleA_m1];
+      sm.locO[tid - 192] = sm.Q[0][roleA_m0] * sm.Q[2][roleA_m1];
+    }
+    __syncthreads();
+
+    // ---- 3. VP[j] (node cost + penalty) and R[a][b] ------------------------------------------------------------
     for (int j = tid; j < K; j += NT) {
-      int a = 0, b = 0, r = j;
-      bool va = true, vb = true;
-      int dig[D];
+      const SigInfo si = sm.sig[kind][j];
+      int64_t v = 0, mem = 0;
+      if (si.valid) {
+        if (kind == AUTODDL_GEMM) {
 #pragma unroll
-      for (int d = D - 1; d >= 0; --d) { dig[d] = r % 6; r /= 6; }
-#pragma unroll
-      for (int d = 0; d < D; ++d) {
-        const int g = dig[d];
-        int so, si;
-        if (kind_prev == AUTODDL_GEMM) so = c_gemm_O[g]; else { so = c_attn_IO[g]; if (so < 0) { va = false; so = 0; } }
-        if (kind == AUTODDL_GEMM) si = c_gemm_I[g]; else { si = c_attn_IO[g]; if (si < 0) { vb = false; si = 0; } }
-        a = a * 4 + so;
-        b = b * 4 + si;
-      }
-      sm.aidx[j] = va ? (int16_t)a : (int16_t)-1;
-      sm.bidx[j] = vb ? (int16_t)b : (int16_t)-1;
-    }
-    __syncthreads();
-
-    // ---- 2. collective costs per level and split configuration ----------------------------------
-    if (l > 0 && tid < D * NC) {
-      const int d = tid / NC, cfg = tid % NC;
-      int m0 = 0, m1 = 0, r = cfg;
-#pragma unroll
-      for (int e = 0; e < D; ++e) {
-        const int sp = r % 3; r /= 3;
-        if (sp == 1) m0 |= 1 << e;
-        if (sp == 2) m1 |= 1 << e;
-      }
-      const int64_t n = sm.rowc[m0] * sm.colc[m1] * eb;          // bytes of the local tensor
-      const int64_t p = mp.size[d];
-      int64_t cg = 0, ca = 0;
-      if (p > 1) {                                                // Table 2
-        cg = (p - 1) * (mp.alpha[d] + cdiv64(n, p) * mp.beta[d]);
-        ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
-      }
-      sm.CG[d][cfg] = cg;
-      sm.CA[d][cfg] = ca;
-    }
-
-    // ---- 5. per consumer signature: node cost, feasibility (independent of steps 2-4) -------------
-    {
-      const int64_t Mo = __ldg(&cur->M), Kd = __ldg(&cur->Kd), No = __ldg(&cur->N);
-      const int64_t wgb = __ldg(&cur->wgrad_bytes), wsb = __ldg(&cur->wstate_bytes);
-      const int64_t maxr = __ldg(&cur->max_split_rows), maxc = __ldg(&cur->max_split_cols);
-      for (int j = tid; j < K; j += NT) {
-        int dig[D], r = j;
-#pragma unroll
-        for (int d = D - 1; d >= 0; --d) { dig[d] = r % 6; r /= 6; }
-        bool valid = true;
-        int mI0 = 0, mI1 = 0;                 // level subsets splitting I's rows / cols
-        int64_t fW0 = 1, fW1 = 1, fO0 = 1, fO1 = 1, rowsplit = 1, colsplit = 1;
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-          const int g = dig[d];
-          const int64_t p = mp.size[d];
-          int si, so, sw;
-          if (kind == AUTODDL_GEMM) { si = c_gemm_I[g]; so = c_gemm_O[g]; sw = c_gemm_W[g]; }
-          else { si = so = c_attn_IO[g]; sw = kB; if (si < 0) { valid = false; si = so = kB; } }
-          if (si == kS0) mI0 |= 1 << d;
-          if (si == kS1) mI1 |= 1 << d;
-          if (so == kS0) fO0 *= p;
-          if (so == kS1) { fO1 *= p; colsplit *= p; }
-          if (sw == kS0) fW0 *= p;
-          if (sw == kS1) fW1 *= p;
-          if (si == kS0 || so == kS0) rowsplit *= p;
+          for (int d = 0; d < D; ++d)
+            if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
+          mem = sm.locW[si.cfgW] * (int64_t)__ldg(&cur->wstate_bytes);
         }
-        int64_t v = 0, mem = 0;
-        if (valid) {
-          if (kind == AUTODDL_GEMM) {
-            const int64_t nw = cdiv64(Kd, fW0) * cdiv64(No, fW1);
-            const int64_t nbytes = nw * wgb;
-#pragma unroll
-            for (int d = 0; d < D; ++d) {
-              const int64_t p = mp.size[d];
-              if (c_gemm_W[dig[d]] == kB && p > 1)               // AllReduce row of Table 2
-                v += (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv64(nbytes, p) * mp.beta[d];
-            }
-            mem = nw * wsb;
-          }
-          mem += (sm.rowc[mI0] * sm.colc[mI1] + cdiv64(Mo, fO0) * cdiv64(No, fO1)) * eb;
-        }
-        const bool ok = valid && rowsplit <= maxr && colsplit <= maxc &&
-                        (mp.mem_cap == 0 || mem <= mp.mem_cap / L);
-        sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
-        if (node) node[(size_t)tile * K + j] = v;
-        if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
+        mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * eb;
       }
+      const bool ok = si.valid && si.rowsplit <= __ldg(&cur->max_split_rows) && si.colsplit <= __ldg(&cur->max_split_cols) &&
+                      (mp.mem_cap == 0 || mem <= cap_layer);
+      sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+      if (node) node[(size_t)tile * K + j] = v;
+      if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
     }
-    __syncthreads();
-
     if (l > 0) {
-      // ---- 3. R[a][b]: every level walks slice -> reduce-scatter -> all-to-all -> all-gather -----
-      for (int e = tid; e < NS * NS; e += NT) {
-        const int av = e / NS, bv = e % NS;
-        int pw3[D];
-        int c0[D], c1[D], c2[D], c3[D];   // split codes after slice / reduce / all-to-all / gather, times 3^level
-        bool act1[D], act2[D], act3[D];
-        {
-          int w = 1;
+      if (kHoist) {
+        if (tid < NS * NS) {
+          int64_t c = 0;
 #pragma unroll
-          for (int d = 0; d < D; ++d) { pw3[d] = w; w *= 3; }
+          for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
+          sm.E[tid] = c;
         }
+      } else {
+        for (int e = tid; e < NS * NS; e += NT) {
+          int idx[3 * D];
+          r_slots<D>(e / NS, e % NS, idx);
+          int64_t c = 0;
 #pragma unroll
-        for (int d = 0; d < D; ++d) {
-          const int a = (av >> (2 * (D - 1 - d))) & 3, b = (bv >> (2 * (D - 1 - d))) & 3;
-          const int s0 = (a == kB && is_split(b)) ? b : a;                 // keep own slice: free
-          act1[d] = (s0 == kP && b != kP);                                 // partial -> split
-          const int s1 = act1[d] ? (b == kB ? kS1 : b) : s0;
-          act2[d] = is_split(s1) && is_split(b) && s1 != b;                // change of split axis
-          const int s2 = act2[d] ? b : s1;
-          act3[d] = is_split(s2) && b == kB;                               // split -> replicated
-          const int s3 = act3[d] ? kB : s2;
-          c0[d] = split_code(s0) * pw3[d];
-          c1[d] = split_code(s1) * pw3[d];
-          c2[d] = split_code(s2) * pw3[d];
-          c3[d] = split_code(s3) * pw3[d];
-        }
-        int64_t cost = 0;
-        // reduce-scatter, innermost level first; message = local tensor before the scatter
-#pragma unroll
-        for (int d = D - 1; d >= 0; --d) {
-          int cfg = 0;
-#pragma unroll
-          for (int e2 = 0; e2 < D; ++e2) cfg += (e2 > d) ? c1[e2] : (e2 < d ? c0[e2] : 0);
-          if (act1[d]) cost += sm.CG[d][cfg];
-        }
-        // all-to-all, innermost first; message = local tensor after the exchange
-#pragma unroll
-        for (int d = D - 1; d >= 0; --d) {
-          int cfg = 0;
-#pragma unroll
-          for (int e2 = 0; e2 < D; ++e2) cfg += (e2 > d) ? c2[e2] : (e2 < d ? c1[e2] : c2[e2]);
-          if (act2[d]) cost += sm.CA[d][cfg];
-        }
-        // all-gather, outermost first; message = local tensor after the gather
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-          int cfg = 0;
-#pragma unroll
-          for (int e2 = 0; e2 < D; ++e2) cfg += (e2 < d) ? c3[e2] : (e2 > d ? c2[e2] : 0);
-          if (act3[d]) cost += sm.CG[d][cfg];
-        }
-        sm.E[e] = cost;
-      }
-      __syncthreads();
-
-      // ---- 4. E[a][b] = R[a][b] + R[dual b][dual a], in place ----------------------------------------
-      for (int e = tid; e < NS * NS; e += NT) {
-        const int av = e / NS, bv = e % NS;
-        int da = 0, db = 0;
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-          const int sh = 2 * (D - 1 - d);
-          da |= dual_of((av >> sh) & 3) << sh;
-          db |= dual_of((bv >> sh) & 3) << sh;
-        }
-        const int e2 = db * NS + da;                  // partner cell; (e2's partner is e)
-        if (e <= e2) {
-          const int64_t s = sm.E[e] + sm.E[e2];
-          sm.E[e] = s;
-          sm.E[e2] = s;
+          for (int k = 0; k < 3 * D; ++k) c += tab[idx[k]];
+          sm.E[e] = c;
         }
       }
-      __syncthreads();
     }
+    __syncthreads();
 
-    // ---- 6. expansion to K x K, two cells (16 bytes) per store -----------------------------------------
-    {
-      int64_t* out = T + (size_t)tile * K * K;
-      constexpr int KH = K / 2;
+    int64_t* out = T + (size_t)tile * K * K;
+    if (SM::kRows) {
+      // ---- 4. the NS + 1 distinct rows: Erow[a][j] = R[a][b_j] + R[dual b_j][dual a] + VP[j] ---------------------
+      for (int x = tid; x < (NS + 1) * K; x += NT) {
+        const int a = x / K, j = x % K;
+        const int b = sm.sig[kind][j].b_idx;
+        int64_t v = sm.VP[j];
+        if (l > 0 && a < NS && b >= 0) v += sm.E[a * NS + b] + sm.E[dual_vec<D>(b) * NS + dual_vec<D>(a)];
+        sm.Erow[x] = v;
+      }
+      __syncthreads();
+      // ---- 5. every output row copies one of them ---------------------------------------------------------------
+      constexpr int RG = NT / KH;                          // row groups
+      const int r = tid / KH, jp = tid % KH;
+      if (r < RG) {
+        for (int i = r; i < K; i += RG) {
+          const int a = (l > 0) ? sm.sig[kind_prev][i].a_idx : NS;
+          const longlong2 v = *reinterpret_cast<const longlong2*>(&sm.Erow[a * K + 2 * jp]);
+          __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + 2 * jp), v);
+        }
+      }
+    } else {
       for (int c = tid; c < K * KH; c += NT) {
         const int i = c / KH, j = (c % KH) * 2;
-        longlong2 v;
-        v.x = sm.VP[j];
-        v.y = sm.VP[j + 1];
+        longlong2 v = make_longlong2(sm.VP[j], sm.VP[j + 1]);
         if (l > 0) {
-          const int a = sm.aidx[i], b0 = sm.bidx[j], b1 = sm.bidx[j + 1];
-          if (a >= 0 && b0 >= 0) v.x += sm.E[a * NS + b0];
-          if (a >= 0 && b1 >= 0) v.y += sm.E[a * NS + b1];
+          const int a = sm.sig[kind_prev][i].a_idx, b0 = sm.sig[kind][j].b_idx, b1 = sm.sig[kind][j + 1].b_idx;
+          if (a < NS) {
+            const int da = dual_vec<D>(a);
+            if (b0 >= 0) v.x += sm.E[a * NS + b0] + sm.E[dual_vec<D>(b0) * NS + da];
+            if (b1 >= 0) v.y += sm.E[a * NS + b1] + sm.E[dual_vec<D>(b1) * NS + da];
+          }
         }
         __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
       }
+      __syncthreads();                                     // E is rewritten by the next tile's step 3
     }
-    __syncthreads();      // smem is reused by the next tile
   }
 }
 
@@ -290,7 +360,7 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   int dev = 0, sms = 148;
   ADL_CUDA_CHECK(cudaGetDevice(&dev));
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const int per_sm = (D == 3) ? 2 : 8;
+  const int per_sm = (D == 3) ? 1 : 4;
   const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;       // persistent, grid-stride over tiles
   build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();

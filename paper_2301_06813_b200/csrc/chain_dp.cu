@@ -9,6 +9,8 @@
 // group of rows; f is broadcast from shared memory.  With one consumer warp (K = 36) a layer needs no
 // block barrier at all; with several row groups (K = 216) partial minima are merged through shared
 // memory with the lexicographic (value, row) order that keeps the lowest-index tie-break.
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace autoddl {
@@ -181,6 +183,145 @@ chain_dp_kernel(const int64_t* __restrict__ T, int L, uint8_t* __restrict__ bp_g
   }
 }
 
+// ---- K = 36 (two mesh levels): one consumer warp with all 32 lanes busy --------------------------------
+// Columns 0..31: lane = h*16 + c owns columns (2c, 2c+1) and rows [18h, 18h+18): one 16-byte shared load per
+// row, the two halves merged with one shuffle step.  Columns 32..35: lane = g*4 + cc owns column 32+cc and
+// rows g, g+8, ..., merged over the 8 row groups with three shuffle steps.  Every merge compares
+// (value, row) lexicographically, so the smallest row wins ties exactly as in the sequential definition.
+template <int STAGES>
+__global__ void __launch_bounds__(64)
+chain_dp36_kernel(const int64_t* __restrict__ T, int L, int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy) {
+  constexpr int K = 36, SB = K * K * 8;
+  extern __shared__ __align__(128) unsigned char smem[];
+  int64_t* stage0 = reinterpret_cast<int64_t*>(smem);
+  int64_t* fbuf = reinterpret_cast<int64_t*>(smem + (size_t)STAGES * SB);      // [2][K]
+  uint64_t* full = reinterpret_cast<uint64_t*>(fbuf + 2 * K);
+  uint64_t* empty = full + STAGES;
+  uint8_t* bp = reinterpret_cast<uint8_t*>(empty + STAGES);                     // [L][K]
+
+  const int tid = threadIdx.x;
+  const int p = blockIdx.x;
+  const int64_t* Tp = T + (size_t)p * L * K * K;
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (tid >= 32) {                         // producer warp: one lane drives the TMA ring
+    if (tid == 32) {
+      const uint64_t pol = policy_evict_first();
+      const unsigned char* src = reinterpret_cast<const unsigned char*>(Tp + (size_t)K * K);
+      for (int b = 0; b < L - 1; ++b) {
+        const int s = b % STAGES;
+        if (b >= STAGES) mbar_wait(&empty[s], ((b / STAGES) - 1) & 1);
+        mbar_arrive_expect_tx(&full[s], SB);
+        bulk_g2s(smem + (size_t)s * SB, src + (size_t)b * SB, SB, &full[s], pol);
+      }
+    }
+    return;
+  }
+
+  const int lane = tid;
+  const int c = lane & 15, h = lane >> 4;          // main part
+  const int cc = lane & 3, g = lane >> 2;          // remainder part
+  for (int j = lane; j < K; j += 32) fbuf[j] = __ldg(Tp + j);     // f_0 = row 0 of tile 0
+  __syncwarp();
+
+  int cur = 0;
+  for (int l = 1; l < L; ++l) {
+    const int b = l - 1, s = b % STAGES;
+    const int64_t* f = fbuf + cur * K;
+    const int64_t* tile = stage0 + (size_t)s * (SB / 8);
+    mbar_wait(&full[s], (b / STAGES) & 1);
+
+    int64_t best0 = INT64_MAX, best1 = INT64_MAX, bestr = INT64_MAX;
+    int a0 = 0, a1 = 0, ar = 0;
+    const int64_t* trow = tile + (18 * h) * K + 2 * c;
+    const int64_t* frow = f + 18 * h;
+#pragma unroll 9
+    for (int r = 0; r < 18; ++r) {
+      const int64_t fi = frow[r];
+      const longlong2 t = *reinterpret_cast<const longlong2*>(trow + r * K);
+      const int64_t v0 = fi + t.x, v1 = fi + t.y;
+      if (v0 < best0) { best0 = v0; a0 = 18 * h + r; }
+      if (v1 < best1) { best1 = v1; a1 = 18 * h + r; }
+    }
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const int i = g + 8 * k;
+      if (i < K) {
+        const int64_t v = f[i] + tile[i * K + 32 + cc];
+        if (v < bestr) { bestr = v; ar = i; }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);           // stage consumed: the producer may refill it
+
+    {                                                // merge the two row halves
+      const int64_t o0 = __shfl_xor_sync(0xffffffffu, best0, 16), o1 = __shfl_xor_sync(0xffffffffu, best1, 16);
+      const int q0 = __shfl_xor_sync(0xffffffffu, a0, 16), q1 = __shfl_xor_sync(0xffffffffu, a1, 16);
+      if (lex_less(o0, q0, best0, a0)) { best0 = o0; a0 = q0; }
+      if (lex_less(o1, q1, best1, a1)) { best1 = o1; a1 = q1; }
+    }
+#pragma unroll
+    for (int off = 4; off <= 16; off <<= 1) {        // merge the eight row groups
+      const int64_t o = __shfl_xor_sync(0xffffffffu, bestr, off);
+      const int q = __shfl_xor_sync(0xffffffffu, ar, off);
+      if (lex_less(o, q, bestr, ar)) { bestr = o; ar = q; }
+    }
+    int64_t* fn = fbuf + (cur ^ 1) * K;
+    uint8_t* bpl = bp + (size_t)l * K;
+    if (lane < 16) {
+      *reinterpret_cast<longlong2*>(fn + 2 * c) = make_longlong2(best0, best1);
+      *reinterpret_cast<uint16_t*>(bpl + 2 * c) = (uint16_t)(a0 | a1 << 8);
+    }
+    if (lane < 4) {
+      fn[32 + cc] = bestr;
+      bpl[32 + cc] = (uint8_t)ar;
+    }
+    __syncwarp();
+    cur ^= 1;
+  }
+
+  // smallest argmin of f_{L-1}, then backtrack
+  const int64_t* f = fbuf + cur * K;
+  int64_t bv = f[lane];
+  int bi = lane;
+  if (lane < K - 32) {
+    const int64_t v = f[32 + lane];
+    if (v < bv) { bv = v; bi = 32 + lane; }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (lex_less(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+  }
+  int32_t* sp = strategy + (size_t)p * L;
+  if (lane == 0) {
+    opt_cost[p] = bv;
+    int sidx = bi;
+    sp[L - 1] = sidx;
+    for (int l = L - 1; l >= 1; --l) {
+      sidx = bp[(size_t)l * K + sidx];
+      sp[l - 1] = sidx;
+    }
+  }
+}
+
+template <int STAGES>
+int launch_dp36(const int64_t* d_T, int Bp, int L, int64_t* d_opt, int32_t* d_strat, cudaStream_t st) {
+  const size_t smem = ((size_t)STAGES * 36 * 36 * 8 + 2 * 36 * 8 + 2 * STAGES * 8 + (size_t)L * 36 + 127) / 128 * 128;
+  auto kern = chain_dp36_kernel<STAGES>;
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<Bp, 64, smem, st>>>(d_T, L, d_opt, d_strat);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
 template <int K, int RB, int STAGES, int G>
 size_t dp_smem_bytes(int L, bool bp_smem) {
   using Lay = DpLayout<K, RB, STAGES, G>;
@@ -218,7 +359,14 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
                     int32_t* d_strategy, cudaStream_t st) {
   switch (K) {
     case 6:   return launch_cfg<6, 6, 4, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
-    case 36:  return launch_cfg<36, 36, 3, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+    case 36:
+      if ((size_t)L * K <= 16 * 1024) {               // back-pointers fit in shared memory: the 32-lane kernel
+        static const int stages = [] { const char* e = getenv("AUTODDL_DP_STAGES"); return e ? atoi(e) : 3; }();
+        if (stages == 2) return launch_dp36<2>(d_T, Bp, L, d_opt_cost, d_strategy, st);
+        if (stages == 4) return launch_dp36<4>(d_T, Bp, L, d_opt_cost, d_strategy, st);
+        return launch_dp36<3>(d_T, Bp, L, d_opt_cost, d_strategy, st);
+      }
+      return launch_cfg<36, 36, 3, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
     case 216: return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
   }
   set_error("chain_dp: K must be 6, 36 or 216");

@@ -38,6 +38,9 @@ struct MeshParams {
   int64_t alpha[3];     // alpha of the level's link class
   int64_t beta[3];      // beta  of the level's link class
   int64_t mem_cap;      // 0 = none
+  int32_t sub[8];       // product of the sizes of the levels in subset m (bit e = level e)
+  uint64_t magic_sub[8];   // ceil(2^64 / sub[m])
+  uint64_t magic_size[3];  // ceil(2^64 / size[d])
 };
 
 int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshParams* out);
