@@ -83,6 +83,7 @@ template <> struct Pow<3> { static constexpr int K = 216, NS = 64, NC = 27; };
 struct SigInfo {
   int16_t a_idx;      // O state-vector index, or NS (zero-edge row) when the signature is invalid for the kind
   int16_t b_idx;      // I state-vector index, or -1
+  int16_t db_idx;     // index of the dual of the I state vector (B <-> P), or -1
   uint8_t cfgW, cfgO; // split configuration of W / of O
   uint8_t mI0, mI1;   // level subsets splitting the input's rows / cols
   uint8_t wB;         // levels on which W is replicated
@@ -166,17 +167,40 @@ __device__ __forceinline__ int dual_vec(int v) {
   return r;
 }
 
+// the per-tile scalars every thread needs, loaded one tile ahead so that no global latency is exposed
+struct TileRec {
+  int64_t X;                 // the extent this thread divides in step 1 (threads < 5 * 2^D)
+  int kind, kind_prev;
+  int eb, wgb, wsb, maxr, maxc;
+};
+
+template <int D>
+__device__ __forceinline__ TileRec load_rec(const autoddl_layer* layers, int tile, int l, int tid) {
+  TileRec r;
+  const autoddl_layer* cur = layers + tile;
+  const int2 ka = __ldg(reinterpret_cast<const int2*>(&cur->kind));           // kind, act_bytes
+  const int2 wg = __ldg(reinterpret_cast<const int2*>(&cur->wgrad_bytes));    // wgrad_bytes, wstate_bytes
+  const int2 mx = __ldg(reinterpret_cast<const int2*>(&cur->max_split_rows)); // max_split_rows, max_split_cols
+  r.kind = ka.x; r.eb = ka.y; r.wgb = wg.x; r.wsb = wg.y; r.maxr = mx.x; r.maxc = mx.y;
+  r.kind_prev = (l > 0) ? __ldg(&(cur - 1)->kind) : AUTODDL_GEMM;
+  r.X = (tid < 5 * (1 << D)) ? __ldg(reinterpret_cast<const int64_t*>(cur) + (tid >> D)) : 0;
+  return r;
+}
+
 template <int D>
 __global__ void __launch_bounds__(256, (D == 3) ? 1 : 4)
-build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
+build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, uint64_t magic_L, MeshParams mp,
                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
   using SM = TileSmem<D>;
   constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2;
-  constexpr bool kHoist = (NS * NS <= NT);
+  constexpr bool kHoist = SM::kRows;                       // D <= 2: every per-thread index is tile-invariant
+  constexpr int EPT = kHoist ? ((NS + 1) * K + NT - 1) / NT : 1;   // Erow entries per thread
+  constexpr int RG = NT / KH < K ? NT / KH : K;            // row groups of the copy-out
+  constexpr int RPT = (K + RG - 1) / RG;                   // rows per thread of the copy-out
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
   const int tid = threadIdx.x;
-  const int64_t* tab = &sm.CG[0][0];                     // CG then CA, contiguous
+  const int64_t* tab = &sm.CG[0][0];                       // CG then CA, contiguous
 
   // ---- once per CTA: facts per (kind, signature) -----------------------------------------------------
   for (int x = tid; x < 2 * K; x += NT) {
@@ -206,40 +230,59 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     }
     si.a_idx = valid ? a : NS;
     si.b_idx = valid ? b : -1;
+    si.db_idx = valid ? dual_vec<D>(b) : -1;
     si.cfgW = cw; si.cfgO = co; si.valid = valid; si.rowsplit = rs; si.colsplit = cs;
     sm.sig[kind][j] = si;
   }
   if (tid < D) { sm.CG[tid][NC] = 0; sm.CA[tid][NC] = 0; }
-
-  // tile-invariant roles of this thread
-  int slot[3 * D];
-  if (kHoist) {
-    if (tid < NS * NS) r_slots<D>(tid / NS, tid % NS, slot);
-    else {
-#pragma unroll
-      for (int k = 0; k < 3 * D; ++k) slot[k] = NC;
-    }
-  }
-  int roleA_m0 = 0, roleA_m1 = 0;
-  {
-    const int t = tid < 96 ? tid : (tid < 192 ? tid - 96 : tid - 192);
-    cfg_masks<D>(t % NC, roleA_m0, roleA_m1);
-  }
-  const int64_t cap_layer = mp.mem_cap / L;
   __syncthreads();
 
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const int l = tile % L;
-    const autoddl_layer* cur = layers + tile;
-    const int kind = __ldg(&cur->kind);
-    const int kind_prev = (l > 0) ? __ldg(&(cur - 1)->kind) : AUTODDL_GEMM;
-    const int64_t eb = __ldg(&cur->act_bytes);
+  // ---- tile-invariant roles of this thread ---------------------------------------------------------------
+  int slot[3 * D];                                         // step 3: the table entries summing to R[tid]
+  int er_a[EPT], er_j[EPT], er_da[EPT];                    // step 4: Erow entries x = tid + k * NT
+  int cp_a[RPT];                                           // step 5: O state index of row r + k * RG, per kind, packed
+  const int cp_r = tid / KH, cp_jp = tid % KH;
+  if (kHoist) {
+    if (tid < NS * NS) r_slots<D>(tid / NS, tid % NS, slot);
+#pragma unroll
+    for (int k = 0; k < EPT; ++k) {
+      const int x = tid + k * NT;
+      er_a[k] = x < (NS + 1) * K ? x / K : -1;
+      er_j[k] = x % K;
+      er_da[k] = (er_a[k] >= 0 && er_a[k] < NS) ? dual_vec<D>(er_a[k]) : 0;
+    }
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      const int i = cp_r + k * RG;
+      cp_a[k] = (cp_r < RG && i < K) ? (sm.sig[0][i].a_idx | sm.sig[1][i].a_idx << 8) : -1;
+    }
+  }
+  int role_m0 = 0, role_m1 = 0;
+  {
+    const int t = tid < 96 ? tid : (tid < 192 ? tid - 96 : tid - 192);
+    cfg_masks<D>(t % NC, role_m0, role_m1);
+  }
+  const int64_t cap_layer = mp.mem_cap / L;
+
+  int tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  int l = (L == 1) ? 0 : tile - (int)__umul64hi((uint64_t)tile, magic_L) * L;      // magic_L = ceil(2^64 / L)
+  TileRec rec = load_rec<D>(layers, tile, l, tid);
+
+  while (tile < ntiles) {
+    // prefetch the next tile's record; it is consumed one iteration later
+    const int tile_n = tile + gridDim.x;
+    const int tn = tile_n < ntiles ? tile_n : tile;
+    const int l_n = (L == 1) ? 0 : tn - (int)__umul64hi((uint64_t)tn, magic_L) * L;
+    const TileRec rec_n = load_rec<D>(layers, tn, l_n, tid);
+
+    const int kind = rec.kind, kind_prev = rec.kind_prev;
+    const int64_t eb = rec.eb;
 
     // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
     if (tid < 5 * (1 << D)) {
-      const int x = tid >> D, m = tid & ((1 << D) - 1);
-      const int64_t X = __ldg(reinterpret_cast<const int64_t*>(cur) + x);
-      sm.Q[x][m] = cdiv_magic(X, (uint32_t)mp.sub[m], mp.magic_sub[m]);
+      const int m = tid & ((1 << D) - 1);
+      sm.Q[tid >> D][m] = cdiv_magic(rec.X, (uint32_t)mp.sub[m], mp.magic_sub[m]);
     }
     __syncthreads();
 
@@ -247,7 +290,7 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     if (tid < D * NC) {
       if (l > 0) {                                           // input tensor: Table 2 rows 2 and 3
         const int d = tid / NC;
-        const int64_t n = sm.Q[3][roleA_m0] * sm.Q[4][roleA_m1] * eb;
+        const int64_t n = sm.Q[3][role_m0] * sm.Q[4][role_m1] * eb;
         const int64_t p = mp.size[d];
         int64_t cg = 0, ca = 0;
         if (p > 1) {
@@ -260,14 +303,14 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     } else if (tid >= 96 && tid < 96 + D * NC) {
       if (kind == AUTODDL_GEMM) {                            // weight gradient: AllReduce row
         const int t = tid - 96, d = t / NC;
-        const int64_t n = sm.Q[1][roleA_m0] * sm.Q[2][roleA_m1] * (int64_t)__ldg(&cur->wgrad_bytes);
+        const int64_t n = sm.Q[1][role_m0] * sm.Q[2][role_m1] * (int64_t)rec.wgb;
         const int64_t p = mp.size[d];
         sm.WAR[d][t % NC] =
             p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
       }
     } else if (tid >= 192 && tid < 192 + NC) {
-      sm.locW[tid - 192] = sm.Q[1][roleA_m0] * sm.Q[2][roleA_m1];
-      sm.locO[tid - 192] = sm.Q[0][roleA_m0] * sm.Q[2][roleA_m1];
+      sm.locW[tid - 192] = sm.Q[1][role_m0] * sm.Q[2][role_m1];
+      sm.locO[tid - 192] = sm.Q[0][role_m0] * sm.Q[2][role_m1];
     }
     __syncthreads();
 
@@ -280,12 +323,11 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 #pragma unroll
           for (int d = 0; d < D; ++d)
             if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
-          mem = sm.locW[si.cfgW] * (int64_t)__ldg(&cur->wstate_bytes);
+          mem = sm.locW[si.cfgW] * (int64_t)rec.wsb;
         }
         mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * eb;
       }
-      const bool ok = si.valid && si.rowsplit <= __ldg(&cur->max_split_rows) && si.colsplit <= __ldg(&cur->max_split_cols) &&
-                      (mp.mem_cap == 0 || mem <= cap_layer);
+      const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
       sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
       if (node) node[(size_t)tile * K + j] = v;
       if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
@@ -312,24 +354,29 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     __syncthreads();
 
     int64_t* out = T + (size_t)tile * K * K;
-    if (SM::kRows) {
+    if (kHoist) {
       // ---- 4. the NS + 1 distinct rows: Erow[a][j] = R[a][b_j] + R[dual b_j][dual a] + VP[j] ---------------------
-      for (int x = tid; x < (NS + 1) * K; x += NT) {
-        const int a = x / K, j = x % K;
-        const int b = sm.sig[kind][j].b_idx;
-        int64_t v = sm.VP[j];
-        if (l > 0 && a < NS && b >= 0) v += sm.E[a * NS + b] + sm.E[dual_vec<D>(b) * NS + dual_vec<D>(a)];
-        sm.Erow[x] = v;
+#pragma unroll
+      for (int k = 0; k < EPT; ++k) {
+        const int a = er_a[k], j = er_j[k];
+        if (a >= 0) {
+          int64_t v = sm.VP[j];
+          if (l > 0 && a < NS) {
+            const SigInfo& sj = sm.sig[kind][j];
+            const int b = sj.b_idx;
+            if (b >= 0) v += sm.E[a * NS + b] + sm.E[sj.db_idx * NS + er_da[k]];
+          }
+          sm.Erow[tid + k * NT] = v;
+        }
       }
       __syncthreads();
       // ---- 5. every output row copies one of them ---------------------------------------------------------------
-      constexpr int RG = NT / KH;                          // row groups
-      const int r = tid / KH, jp = tid % KH;
-      if (r < RG) {
-        for (int i = r; i < K; i += RG) {
-          const int a = (l > 0) ? sm.sig[kind_prev][i].a_idx : NS;
-          const longlong2 v = *reinterpret_cast<const longlong2*>(&sm.Erow[a * K + 2 * jp]);
-          __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + 2 * jp), v);
+#pragma unroll
+      for (int k = 0; k < RPT; ++k) {
+        if (cp_a[k] >= 0) {
+          const int a = (l > 0) ? ((cp_a[k] >> (8 * kind_prev)) & 0xff) : NS;
+          const longlong2 v = *reinterpret_cast<const longlong2*>(&sm.Erow[a * K + 2 * cp_jp]);
+          __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
         }
       }
     } else {
@@ -337,17 +384,22 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         const int i = c / KH, j = (c % KH) * 2;
         longlong2 v = make_longlong2(sm.VP[j], sm.VP[j + 1]);
         if (l > 0) {
-          const int a = sm.sig[kind_prev][i].a_idx, b0 = sm.sig[kind][j].b_idx, b1 = sm.sig[kind][j + 1].b_idx;
+          const int a = sm.sig[kind_prev][i].a_idx;
           if (a < NS) {
             const int da = dual_vec<D>(a);
-            if (b0 >= 0) v.x += sm.E[a * NS + b0] + sm.E[dual_vec<D>(b0) * NS + da];
-            if (b1 >= 0) v.y += sm.E[a * NS + b1] + sm.E[dual_vec<D>(b1) * NS + da];
+            const SigInfo& s0 = sm.sig[kind][j];
+            const SigInfo& s1 = sm.sig[kind][j + 1];
+            if (s0.b_idx >= 0) v.x += sm.E[a * NS + s0.b_idx] + sm.E[s0.db_idx * NS + da];
+            if (s1.b_idx >= 0) v.y += sm.E[a * NS + s1.b_idx] + sm.E[s1.db_idx * NS + da];
           }
         }
         __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
       }
       __syncthreads();                                     // E is rewritten by the next tile's step 3
     }
+    tile = tile_n;
+    l = l_n;
+    rec = rec_n;
   }
 }
 
@@ -362,7 +414,8 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int per_sm = (D == 3) ? 1 : 4;
   const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;       // persistent, grid-stride over tiles
-  build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
+  const uint64_t magic_L = (uint64_t)((((unsigned __int128)1 << 64) + L - 1) / L);   // tile / L by multiply-high, exact for tile < 2^31
+  build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, magic_L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
