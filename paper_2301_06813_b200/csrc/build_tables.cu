@@ -18,9 +18,9 @@
 //   3. R[a][b] over the 4^D x 4^D state vectors = a sum of <= 3D table entries whose addresses do not
 //      depend on the tile (hoisted out of the persistent tile loop when one thread owns one entry);
 //      VP[j] = node cost + penalty per consumer signature from the step-2 tables
-//   4. only 4^D (+1) distinct rows exist: Erow[a][j] = R[a][b_j] + R[dual b_j][dual a] + VP[j]
-//      (forward leg + backward leg, b_j = I-state vector of consumer signature j)
-//   5. every output row is a copy of one Erow row: 16-byte shared loads, 16-byte streaming stores.
+//   4. Esym[a][b] = R[a][b] + R[dual b][dual a]   (forward leg + backward leg)
+//   5. the K x K expansion T[i][j] = Esym[O-state(i)][I-state(j)] + VP[j]: one shared-memory gather and one
+//      64-bit add per cell, 16-byte streaming stores; all indices are hoisted out of the tile loop.
 // The kernel is then bound by the HBM write of 8 B per cell instead of integer arithmetic.
 #include "common.cuh"
 
@@ -79,6 +79,32 @@ template <> struct Pow<1> { static constexpr int K = 6, NS = 4, NC = 3; };
 template <> struct Pow<2> { static constexpr int K = 36, NS = 16, NC = 9; };
 template <> struct Pow<3> { static constexpr int K = 216, NS = 64, NC = 27; };
 
+// Layer records are staged one tile ahead with cp.async into a double buffer in shared memory (80 bytes:
+// the 64-byte record, then the previous layer's kind), so the tile loop never waits on a global load and
+// no register is held across an iteration for the prefetch.
+struct alignas(16) RecBuf {
+  int64_t X[5];              // M, Kd, N, in_rows, in_cols
+  int32_t kind, eb, wgb, wsb, maxr, maxc;
+  int32_t kind_prev;
+  int32_t pad[3];
+};
+static_assert(sizeof(RecBuf) == 80, "RecBuf mirrors autoddl_layer + 16 bytes");
+
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst_smem, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// threads 0..3 copy the record, thread 4 the previous layer's kind (layer 0: its own, unused)
+__device__ __forceinline__ void stage_rec(RecBuf* dst, const autoddl_layer* layers, int tile, int l, int tid) {
+  const autoddl_layer* cur = layers + tile;
+  if (tid < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * tid, reinterpret_cast<const unsigned char*>(cur) + 16 * tid);
+  else if (tid == 4) cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
+}
+
 // per (layer kind, signature) facts, built once per CTA
 struct SigInfo {
   int16_t a_idx;      // O state-vector index, or NS (zero-edge row) when the signature is invalid for the kind
@@ -94,7 +120,8 @@ struct SigInfo {
 template <int D>
 struct TileSmem {
   static constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
-  static constexpr bool kRows = (D <= 2);               // distinct-row expansion (steps 4/5)
+  static constexpr bool kRows = (D <= 2);               // one thread per state pair: hoisted fast path
+  RecBuf rec[2];
   SigInfo sig[2][K];
   int64_t Q[5][8];                                      // M, Kd, N, in_rows, in_cols  x  level subset
   int64_t CG[D][NC + 1];                                // [..][NC] = 0: the slot that does not run
@@ -103,7 +130,7 @@ struct TileSmem {
   int64_t locW[NC], locO[NC];
   alignas(16) int64_t VP[K];
   alignas(16) int64_t E[NS * NS];
-  alignas(16) int64_t Erow[kRows ? (NS + 1) * K : 1];
+  alignas(16) int64_t Esym[kRows ? (NS + 1) * (NS + 1) : 1];   // R[a][b] + R[dual b][dual a]; row NS and column NS are 0
 };
 
 
@@ -167,34 +194,13 @@ __device__ __forceinline__ int dual_vec(int v) {
   return r;
 }
 
-// the per-tile scalars every thread needs, loaded one tile ahead so that no global latency is exposed
-struct TileRec {
-  int64_t X;                 // the extent this thread divides in step 1 (threads < 5 * 2^D)
-  int kind, kind_prev;
-  int eb, wgb, wsb, maxr, maxc;
-};
-
-template <int D>
-__device__ __forceinline__ TileRec load_rec(const autoddl_layer* layers, int tile, int l, int tid) {
-  TileRec r;
-  const autoddl_layer* cur = layers + tile;
-  const int2 ka = __ldg(reinterpret_cast<const int2*>(&cur->kind));           // kind, act_bytes
-  const int2 wg = __ldg(reinterpret_cast<const int2*>(&cur->wgrad_bytes));    // wgrad_bytes, wstate_bytes
-  const int2 mx = __ldg(reinterpret_cast<const int2*>(&cur->max_split_rows)); // max_split_rows, max_split_cols
-  r.kind = ka.x; r.eb = ka.y; r.wgb = wg.x; r.wsb = wg.y; r.maxr = mx.x; r.maxc = mx.y;
-  r.kind_prev = (l > 0) ? __ldg(&(cur - 1)->kind) : AUTODDL_GEMM;
-  r.X = (tid < 5 * (1 << D)) ? __ldg(reinterpret_cast<const int64_t*>(cur) + (tid >> D)) : 0;
-  return r;
-}
-
 template <int D>
 __global__ void __launch_bounds__(256, (D == 3) ? 1 : 4)
-build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, uint64_t magic_L, MeshParams mp,
+build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
   using SM = TileSmem<D>;
   constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2;
   constexpr bool kHoist = SM::kRows;                       // D <= 2: every per-thread index is tile-invariant
-  constexpr int EPT = kHoist ? ((NS + 1) * K + NT - 1) / NT : 1;   // Erow entries per thread
   constexpr int RG = NT / KH < K ? NT / KH : K;            // row groups of the copy-out
   constexpr int RPT = (K + RG - 1) / RG;                   // rows per thread of the copy-out
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -239,23 +245,33 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 
   // ---- tile-invariant roles of this thread ---------------------------------------------------------------
   int slot[3 * D];                                         // step 3: the table entries summing to R[tid]
-  int er_a[EPT], er_j[EPT], er_da[EPT];                    // step 4: Erow entries x = tid + k * NT
-  int cp_a[RPT];                                           // step 5: O state index of row r + k * RG, per kind, packed
+  int partner = 0;                                         // step 4: index of R[dual b][dual a]
+  int cp_a[RPT];                                           // step 5: a_idx * NS of row r + k * RG for both producer kinds
+  int cp_b = 0;                                            // step 5: b_idx of columns 2jp, 2jp+1 for both consumer kinds
   const int cp_r = tid / KH, cp_jp = tid % KH;
   if (kHoist) {
-    if (tid < NS * NS) r_slots<D>(tid / NS, tid % NS, slot);
-#pragma unroll
-    for (int k = 0; k < EPT; ++k) {
-      const int x = tid + k * NT;
-      er_a[k] = x < (NS + 1) * K ? x / K : -1;
-      er_j[k] = x % K;
-      er_da[k] = (er_a[k] >= 0 && er_a[k] < NS) ? dual_vec<D>(er_a[k]) : 0;
+    if (tid < NS * NS) {
+      r_slots<D>(tid / NS, tid % NS, slot);
+      partner = dual_vec<D>(tid % NS) * NS + dual_vec<D>(tid / NS);
     }
 #pragma unroll
     for (int k = 0; k < RPT; ++k) {
       const int i = cp_r + k * RG;
-      cp_a[k] = (cp_r < RG && i < K) ? (sm.sig[0][i].a_idx | sm.sig[1][i].a_idx << 8) : -1;
+      if (cp_r < RG && i < K) {
+        const int a0 = sm.sig[0][i].a_idx, a1 = sm.sig[1][i].a_idx;       // NS = invalid -> the zero entry
+        cp_a[k] = (a0 * (NS + 1)) | (a1 * (NS + 1)) << 16;          // a = NS (invalid) selects the zero row
+      } else {
+        cp_a[k] = 0;
+      }
     }
+    if (cp_r < RG) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int b = sm.sig[q >> 1][2 * cp_jp + (q & 1)].b_idx;
+        cp_b |= (b >= 0 ? b : NS) << (8 * q);                  // b = NS (invalid) selects the zero column
+      }
+    }
+    for (int x = tid; x < (NS + 1) * (NS + 1); x += NT) sm.Esym[x] = 0;
   }
   int role_m0 = 0, role_m1 = 0;
   {
@@ -266,15 +282,22 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 
   int tile = blockIdx.x;
   if (tile >= ntiles) return;
-  int l = (L == 1) ? 0 : tile - (int)__umul64hi((uint64_t)tile, magic_L) * L;      // magic_L = ceil(2^64 / L)
-  TileRec rec = load_rec<D>(layers, tile, l, tid);
+  int l = tile % L;
+  const int l_step = gridDim.x % L;                        // l advances by gridDim.x mod L per iteration
+  int buf = 0;
+  stage_rec(&sm.rec[0], layers, tile, l, tid);
+  cp_async_wait_all();
+  __syncthreads();
 
   while (tile < ntiles) {
     // prefetch the next tile's record; it is consumed one iteration later
     const int tile_n = tile + gridDim.x;
     const int tn = tile_n < ntiles ? tile_n : tile;
-    const int l_n = (L == 1) ? 0 : tn - (int)__umul64hi((uint64_t)tn, magic_L) * L;
-    const TileRec rec_n = load_rec<D>(layers, tn, l_n, tid);
+    int l_n = l + l_step;
+    if (l_n >= L) l_n -= L;
+    if (tile_n >= ntiles) l_n = l;
+    stage_rec(&sm.rec[buf ^ 1], layers, tn, l_n, tid);
+    const RecBuf& rec = sm.rec[buf];
 
     const int kind = rec.kind, kind_prev = rec.kind_prev;
     const int64_t eb = rec.eb;
@@ -282,7 +305,7 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
     if (tid < 5 * (1 << D)) {
       const int m = tid & ((1 << D) - 1);
-      sm.Q[tid >> D][m] = cdiv_magic(rec.X, (uint32_t)mp.sub[m], mp.magic_sub[m]);
+      sm.Q[tid >> D][m] = cdiv_magic(rec.X[tid >> D], (uint32_t)mp.sub[m], mp.magic_sub[m]);
     }
     __syncthreads();
 
@@ -355,28 +378,24 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 
     int64_t* out = T + (size_t)tile * K * K;
     if (kHoist) {
-      // ---- 4. the NS + 1 distinct rows: Erow[a][j] = R[a][b_j] + R[dual b_j][dual a] + VP[j] ---------------------
-#pragma unroll
-      for (int k = 0; k < EPT; ++k) {
-        const int a = er_a[k], j = er_j[k];
-        if (a >= 0) {
-          int64_t v = sm.VP[j];
-          if (l > 0 && a < NS) {
-            const SigInfo& sj = sm.sig[kind][j];
-            const int b = sj.b_idx;
-            if (b >= 0) v += sm.E[a * NS + b] + sm.E[sj.db_idx * NS + er_da[k]];
-          }
-          sm.Erow[tid + k * NT] = v;
-        }
-      }
+      // ---- 4. Esym[a][b] = R[a][b] + R[dual b][dual a]: forward leg + backward leg ------------------------------
+      if (l > 0 && tid < NS * NS) sm.Esym[(tid / NS) * (NS + 1) + tid % NS] = sm.E[tid] + sm.E[partner];
+      if (tid < 5) cp_async_wait_all();                    // the next tile's record has landed; the barrier publishes it
       __syncthreads();
-      // ---- 5. every output row copies one of them ---------------------------------------------------------------
+      // ---- 5. K x K expansion: one gather + one add per cell, 16-byte streaming stores ---------------------------
+      if (cp_r < RG) {
+        const longlong2 vp = *reinterpret_cast<const longlong2*>(&sm.VP[2 * cp_jp]);
+        const int bb = cp_b >> (16 * kind);
+        const int b0 = bb & 0xff, b1 = (bb >> 8) & 0xff;
 #pragma unroll
-      for (int k = 0; k < RPT; ++k) {
-        if (cp_a[k] >= 0) {
-          const int a = (l > 0) ? ((cp_a[k] >> (8 * kind_prev)) & 0xff) : NS;
-          const longlong2 v = *reinterpret_cast<const longlong2*>(&sm.Erow[a * K + 2 * cp_jp]);
-          __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
+        for (int k = 0; k < RPT; ++k) {
+          if (cp_r + k * RG < K) {
+            const int ao = (l > 0) ? ((cp_a[k] >> (16 * kind_prev)) & 0xffff) : NS * (NS + 1);   // layer 0: zero row
+            longlong2 v;
+            v.x = vp.x + sm.Esym[ao + b0];
+            v.y = vp.y + sm.Esym[ao + b1];
+            __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
+          }
         }
       }
     } else {
@@ -395,11 +414,12 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         }
         __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
       }
-      __syncthreads();                                     // E is rewritten by the next tile's step 3
+      if (tid < 5) cp_async_wait_all();
+      __syncthreads();                                     // E is rewritten by the next tile's step 3; publishes the record
     }
     tile = tile_n;
     l = l_n;
-    rec = rec_n;
+    buf ^= 1;
   }
 }
 
@@ -414,8 +434,7 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int per_sm = (D == 3) ? 1 : 4;
   const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;       // persistent, grid-stride over tiles
-  const uint64_t magic_L = (uint64_t)((((unsigned __int128)1 << 64) + L - 1) / L);   // tile / L by multiply-high, exact for tile < 2^31
-  build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, magic_L, mp, d_T, d_node, d_mask);
+  build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
