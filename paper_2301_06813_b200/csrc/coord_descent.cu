@@ -24,6 +24,14 @@ __device__ __forceinline__ void warp_argmin(int64_t& bv, int& bi) {
   }
 }
 
+// 8-byte read-only load that asks L2 to fetch only a 64-byte granule (a column gather touches one element per
+// 288-byte row, so anything wider is wasted DRAM traffic)
+__device__ __forceinline__ int64_t ldg_narrow(const int64_t* p) {
+  int64_t v;
+  asm volatile("ld.global.nc.L2::64B.b64 %0, [%1];" : "=l"(v) : "l"(p));
+  return v;
+}
+
 template <int K>
 __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int L, int S,
                                                            const int32_t* __restrict__ init, int max_sweeps,
@@ -60,7 +68,7 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
         const int c = c0 + lane;
         if (c < K) {
           int64_t g = __ldg(row + c);
-          if (has_right) g += __ldg(col + (size_t)c * K);
+          if (has_right) g += ldg_narrow(col + (size_t)c * K);
           if (g < bv) { bv = g; bi = c; }
         }
       }
@@ -86,7 +94,7 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   int64_t acc = 0;
   for (int l = lane; l < L; l += 32) {
     const int left = l > 0 ? s[l - 1] : 0;
-    acc += __ldg(Tp + ((size_t)l * K + left) * K + s[l]);
+    acc += ldg_narrow(Tp + ((size_t)l * K + left) * K + s[l]);
     strategy[ps * L + l] = s[l];
   }
 #pragma unroll
