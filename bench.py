@@ -83,7 +83,7 @@ def oracle_sample_run(w, nprob, repeat=1):
     return cells, sweeps, t
 
 
-def cpu_baseline(w, nprob=1024):
+def cpu_baseline(w, nprob=2048):
     cells, sweeps, t = oracle_sample_run(w, nprob)
     tot = t["build"] + t["dp"] + t["cd"]
     return {
