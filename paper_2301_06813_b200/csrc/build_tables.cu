@@ -98,13 +98,6 @@ __device__ __forceinline__ void cp_async4(void* dst_smem, const void* src) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// threads 0..3 copy the record, thread 4 the previous layer's kind (layer 0: its own, unused)
-__device__ __forceinline__ void stage_rec(RecBuf* dst, const autoddl_layer* layers, int tile, int l, int tid) {
-  const autoddl_layer* cur = layers + tile;
-  if (tid < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * tid, reinterpret_cast<const unsigned char*>(cur) + 16 * tid);
-  else if (tid == 4) cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
-}
-
 // per (layer kind, signature) facts, built once per CTA
 struct SigInfo {
   int16_t a_idx;      // O state-vector index, or NS (zero-edge row) when the signature is invalid for the kind
@@ -121,16 +114,20 @@ template <int D>
 struct TileSmem {
   static constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
   static constexpr bool kRows = (D <= 2);               // one thread per state pair: hoisted fast path
-  RecBuf rec[2];
+  static constexpr int G = kRows ? 4 : 1;               // tiles processed together per loop iteration
+  struct PerTile {
+    int64_t Q[5][8];                                    // M, Kd, N, in_rows, in_cols  x  level subset
+    int64_t CG[D][NC + 1];                              // [..][NC] = 0: the slot that does not run
+    int64_t CA[D][NC + 1];
+    int64_t WAR[D][NC];
+    int64_t locW[NC], locO[NC];
+    alignas(16) int64_t VP[K];
+    alignas(16) int64_t E[NS * NS];
+    alignas(16) int64_t Esym[kRows ? (NS + 1) * (NS + 1) : 1];   // R[a][b] + R[dual b][dual a]; row NS, column NS = 0
+  };
+  RecBuf rec[2][G];
   SigInfo sig[2][K];
-  int64_t Q[5][8];                                      // M, Kd, N, in_rows, in_cols  x  level subset
-  int64_t CG[D][NC + 1];                                // [..][NC] = 0: the slot that does not run
-  int64_t CA[D][NC + 1];
-  int64_t WAR[D][NC];
-  int64_t locW[NC], locO[NC];
-  alignas(16) int64_t VP[K];
-  alignas(16) int64_t E[NS * NS];
-  alignas(16) int64_t Esym[kRows ? (NS + 1) * (NS + 1) : 1];   // R[a][b] + R[dual b][dual a]; row NS and column NS are 0
+  alignas(16) PerTile t[G];
 };
 
 
@@ -195,18 +192,19 @@ __device__ __forceinline__ int dual_vec(int v) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(256, (D == 3) ? 1 : 4)
+__global__ void __launch_bounds__(256, (D == 3) ? 1 : 3)
 build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
   using SM = TileSmem<D>;
-  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2;
+  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2, G = SM::G;
   constexpr bool kHoist = SM::kRows;                       // D <= 2: every per-thread index is tile-invariant
   constexpr int RG = NT / KH < K ? NT / KH : K;            // row groups of the copy-out
   constexpr int RPT = (K + RG - 1) / RG;                   // rows per thread of the copy-out
+  constexpr int STRIDE = NC + 1, TABN = 2 * D * STRIDE;    // CG then CA, contiguous per tile
+  static_assert(G * D * NC <= 96 && 192 + G * NC <= NT && G * 5 * (1 << D) <= NT, "role layout");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
   const int tid = threadIdx.x;
-  const int64_t* tab = &sm.CG[0][0];                       // CG then CA, contiguous
 
   // ---- once per CTA: facts per (kind, signature) -----------------------------------------------------
   for (int x = tid; x < 2 * K; x += NT) {
@@ -240,13 +238,13 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     si.cfgW = cw; si.cfgO = co; si.valid = valid; si.rowsplit = rs; si.colsplit = cs;
     sm.sig[kind][j] = si;
   }
-  if (tid < D) { sm.CG[tid][NC] = 0; sm.CA[tid][NC] = 0; }
+  for (int x = tid; x < G * D; x += NT) { sm.t[x / D].CG[x % D][NC] = 0; sm.t[x / D].CA[x % D][NC] = 0; }
   __syncthreads();
 
   // ---- tile-invariant roles of this thread ---------------------------------------------------------------
   int slot[3 * D];                                         // step 3: the table entries summing to R[tid]
   int partner = 0;                                         // step 4: index of R[dual b][dual a]
-  int cp_a[RPT];                                           // step 5: a_idx * NS of row r + k * RG for both producer kinds
+  int cp_a[RPT];                                           // step 5: a_idx * (NS+1) of row r + k * RG for both producer kinds
   int cp_b = 0;                                            // step 5: b_idx of columns 2jp, 2jp+1 for both consumer kinds
   const int cp_r = tid / KH, cp_jp = tid % KH;
   if (kHoist) {
@@ -258,8 +256,8 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     for (int k = 0; k < RPT; ++k) {
       const int i = cp_r + k * RG;
       if (cp_r < RG && i < K) {
-        const int a0 = sm.sig[0][i].a_idx, a1 = sm.sig[1][i].a_idx;       // NS = invalid -> the zero entry
-        cp_a[k] = (a0 * (NS + 1)) | (a1 * (NS + 1)) << 16;          // a = NS (invalid) selects the zero row
+        const int a0 = sm.sig[0][i].a_idx, a1 = sm.sig[1][i].a_idx;       // a = NS (invalid) selects the zero row
+        cp_a[k] = (a0 * (NS + 1)) | (a1 * (NS + 1)) << 16;
       } else {
         cp_a[k] = 0;
       }
@@ -271,154 +269,201 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         cp_b |= (b >= 0 ? b : NS) << (8 * q);                  // b = NS (invalid) selects the zero column
       }
     }
-    for (int x = tid; x < (NS + 1) * (NS + 1); x += NT) sm.Esym[x] = 0;
+    for (int x = tid; x < G * (NS + 1) * (NS + 1); x += NT) sm.t[x / ((NS + 1) * (NS + 1))].Esym[x % ((NS + 1) * (NS + 1))] = 0;
   }
+  // step 1 role: (tile in group, extent, level subset); step 2 roles: A [0,96) B [96,192) C [192,..)
+  const int q_t = tid / (5 << D), q_x = (tid % (5 << D)) >> D, q_m = tid & ((1 << D) - 1);
+  const int role_base = tid < 96 ? 0 : (tid < 192 ? 96 : 192);
+  const int role_i = tid - role_base;
+  const int role_t = role_base == 192 ? role_i / NC : role_i / (D * NC);      // tile in group
+  const int role_d = (role_i % (D * NC)) / NC;                                // level (roles A, B)
+  const int role_cfg = role_i % NC;
   int role_m0 = 0, role_m1 = 0;
-  {
-    const int t = tid < 96 ? tid : (tid < 192 ? tid - 96 : tid - 192);
-    cfg_masks<D>(t % NC, role_m0, role_m1);
-  }
+  cfg_masks<D>(role_cfg, role_m0, role_m1);
   const int64_t cap_layer = mp.mem_cap / L;
+  const int ngroups = (ntiles + G - 1) / G;
 
-  int tile = blockIdx.x;
-  if (tile >= ntiles) return;
-  int l = tile % L;
-  const int l_step = gridDim.x % L;                        // l advances by gridDim.x mod L per iteration
+  int grp = blockIdx.x;
+  if (grp >= ngroups) return;
+  int l0 = (int)(((int64_t)grp * G) % L);                  // layer index of the group's first tile
+  const int l_step = (int)(((int64_t)gridDim.x * G) % L);
   int buf = 0;
-  stage_rec(&sm.rec[0], layers, tile, l, tid);
+  // records: thread 5*t + part stages 16-byte part (or the previous kind) of tile t of the group
+  auto stage_group = [&](int b, int g, int lfirst) {
+    if (tid < 5 * G) {
+      const int t = tid / 5, part = tid % 5;
+      int tile = g * G + t;
+      if (tile >= ntiles) tile = ntiles - 1;                // ragged tail: restage a valid record, never used
+      int l = lfirst + t;
+      while (l >= L) l -= L;
+      const autoddl_layer* cur = layers + tile;
+      RecBuf* dst = &sm.rec[b][t];
+      if (part < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * part, reinterpret_cast<const unsigned char*>(cur) + 16 * part);
+      else cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
+    }
+  };
+  stage_group(0, grp, l0);
   cp_async_wait_all();
   __syncthreads();
 
-  while (tile < ntiles) {
-    // prefetch the next tile's record; it is consumed one iteration later
-    const int tile_n = tile + gridDim.x;
-    const int tn = tile_n < ntiles ? tile_n : tile;
-    int l_n = l + l_step;
-    if (l_n >= L) l_n -= L;
-    if (tile_n >= ntiles) l_n = l;
-    stage_rec(&sm.rec[buf ^ 1], layers, tn, l_n, tid);
-    const RecBuf& rec = sm.rec[buf];
-
-    const int kind = rec.kind, kind_prev = rec.kind_prev;
-    const int64_t eb = rec.eb;
+  while (grp < ngroups) {
+    const int grp_n = grp + gridDim.x;
+    int l0_n = l0 + l_step;
+    if (l0_n >= L) l0_n -= L;
+    stage_group(buf ^ 1, grp_n < ngroups ? grp_n : grp, grp_n < ngroups ? l0_n : l0);
+    const int tile0 = grp * G;
+    const int nt = ntiles - tile0 < G ? ntiles - tile0 : G;   // tiles of this group that exist
+    auto layer_of = [&](int t) { int l = l0 + t; while (l >= L) l -= L; return l; };
+    int kinds = 0;                                           // (kind, kind_prev) of every tile of the group, read before
+#pragma unroll                                               // the record buffer can be restaged by a faster thread
+    for (int t = 0; t < G; ++t) kinds |= (sm.rec[buf][t].kind | sm.rec[buf][t].kind_prev << 1) << (2 * t);
 
     // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
-    if (tid < 5 * (1 << D)) {
-      const int m = tid & ((1 << D) - 1);
-      sm.Q[tid >> D][m] = cdiv_magic(rec.X[tid >> D], (uint32_t)mp.sub[m], mp.magic_sub[m]);
-    }
+    if (tid < G * (5 << D) && q_t < nt)
+      sm.t[q_t].Q[q_x][q_m] = cdiv_magic(sm.rec[buf][q_t].X[q_x], (uint32_t)mp.sub[q_m], mp.magic_sub[q_m]);
     __syncthreads();
 
     // ---- 2. tables per level and split configuration -------------------------------------------------------
-    if (tid < D * NC) {
-      if (l > 0) {                                           // input tensor: Table 2 rows 2 and 3
-        const int d = tid / NC;
-        const int64_t n = sm.Q[3][role_m0] * sm.Q[4][role_m1] * eb;
-        const int64_t p = mp.size[d];
-        int64_t cg = 0, ca = 0;
-        if (p > 1) {
-          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+    if (role_t < nt) {
+      typename SM::PerTile& pt = sm.t[role_t];
+      const RecBuf& rec = sm.rec[buf][role_t];
+      if (role_base == 0 && role_i < G * D * NC) {
+        if (layer_of(role_t) > 0) {                          // input tensor: Table 2 rows 2 and 3
+          const int d = role_d;
+          const int64_t n = pt.Q[3][role_m0] * pt.Q[4][role_m1] * (int64_t)rec.eb;
+          const int64_t p = mp.size[d];
+          int64_t cg = 0, ca = 0;
+          if (p > 1) {
+            cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+            ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+          }
+          pt.CG[d][role_cfg] = cg;
+          pt.CA[d][role_cfg] = ca;
         }
-        sm.CG[d][tid % NC] = cg;
-        sm.CA[d][tid % NC] = ca;
+      } else if (role_base == 96 && role_i < G * D * NC) {
+        if (rec.kind == AUTODDL_GEMM) {                      // weight gradient: AllReduce row
+          const int d = role_d;
+          const int64_t n = pt.Q[1][role_m0] * pt.Q[2][role_m1] * (int64_t)rec.wgb;
+          const int64_t p = mp.size[d];
+          pt.WAR[d][role_cfg] =
+              p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
+        }
+      } else if (role_base == 192 && role_i < G * NC) {
+        pt.locW[role_cfg] = pt.Q[1][role_m0] * pt.Q[2][role_m1];
+        pt.locO[role_cfg] = pt.Q[0][role_m0] * pt.Q[2][role_m1];
       }
-    } else if (tid >= 96 && tid < 96 + D * NC) {
-      if (kind == AUTODDL_GEMM) {                            // weight gradient: AllReduce row
-        const int t = tid - 96, d = t / NC;
-        const int64_t n = sm.Q[1][role_m0] * sm.Q[2][role_m1] * (int64_t)rec.wgb;
-        const int64_t p = mp.size[d];
-        sm.WAR[d][t % NC] =
-            p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
-      }
-    } else if (tid >= 192 && tid < 192 + NC) {
-      sm.locW[tid - 192] = sm.Q[1][role_m0] * sm.Q[2][role_m1];
-      sm.locO[tid - 192] = sm.Q[0][role_m0] * sm.Q[2][role_m1];
     }
     __syncthreads();
 
     // ---- 3. VP[j] (node cost + penalty) and R[a][b] ------------------------------------------------------------
-    for (int j = tid; j < K; j += NT) {
-      const SigInfo si = sm.sig[kind][j];
+    for (int x = tid; x < nt * K; x += NT) {
+      const int t = x / K, j = x % K;
+      typename SM::PerTile& pt = sm.t[t];
+      const RecBuf& rec = sm.rec[buf][t];
+      const SigInfo si = sm.sig[rec.kind][j];
       int64_t v = 0, mem = 0;
       if (si.valid) {
-        if (kind == AUTODDL_GEMM) {
+        if (rec.kind == AUTODDL_GEMM) {
 #pragma unroll
           for (int d = 0; d < D; ++d)
-            if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
-          mem = sm.locW[si.cfgW] * (int64_t)rec.wsb;
+            if (si.wB >> d & 1) v += pt.WAR[d][si.cfgW];
+          mem = pt.locW[si.cfgW] * (int64_t)rec.wsb;
         }
-        mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * eb;
+        mem += (pt.Q[3][si.mI0] * pt.Q[4][si.mI1] + pt.locO[si.cfgO]) * (int64_t)rec.eb;
       }
       const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
-      sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
-      if (node) node[(size_t)tile * K + j] = v;
-      if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
+      pt.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+      const size_t o = (size_t)(tile0 + t) * K + j;
+      if (node) node[o] = v;
+      if (mask) mask[o] = ok ? 1 : 0;
     }
-    if (l > 0) {
-      if (kHoist) {
-        if (tid < NS * NS) {
-          int64_t c = 0;
+    if (kHoist) {
+      if (tid < NS * NS) {
 #pragma unroll
-          for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
-          sm.E[tid] = c;
+        for (int t = 0; t < G; ++t) {
+          if (t < nt && layer_of(t) > 0) {
+            const int64_t* tab = &sm.t[t].CG[0][0];
+            int64_t c = 0;
+#pragma unroll
+            for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
+            sm.t[t].E[tid] = c;
+          }
         }
-      } else {
+      }
+    } else {
+      if (layer_of(0) > 0) {
+        const int64_t* tab = &sm.t[0].CG[0][0];
         for (int e = tid; e < NS * NS; e += NT) {
           int idx[3 * D];
           r_slots<D>(e / NS, e % NS, idx);
           int64_t c = 0;
 #pragma unroll
           for (int k = 0; k < 3 * D; ++k) c += tab[idx[k]];
-          sm.E[e] = c;
+          sm.t[0].E[e] = c;
         }
       }
     }
     __syncthreads();
 
-    int64_t* out = T + (size_t)tile * K * K;
     if (kHoist) {
       // ---- 4. Esym[a][b] = R[a][b] + R[dual b][dual a]: forward leg + backward leg ------------------------------
-      if (l > 0 && tid < NS * NS) sm.Esym[(tid / NS) * (NS + 1) + tid % NS] = sm.E[tid] + sm.E[partner];
-      if (tid < 5) cp_async_wait_all();                    // the next tile's record has landed; the barrier publishes it
+      if (tid < NS * NS) {
+#pragma unroll
+        for (int t = 0; t < G; ++t)
+          if (t < nt && layer_of(t) > 0) sm.t[t].Esym[(tid / NS) * (NS + 1) + tid % NS] = sm.t[t].E[tid] + sm.t[t].E[partner];
+      }
+      if (tid < 5 * G) cp_async_wait_all();                // the next group's records have landed; the barrier publishes them
       __syncthreads();
       // ---- 5. K x K expansion: one gather + one add per cell, 16-byte streaming stores ---------------------------
       if (cp_r < RG) {
-        const longlong2 vp = *reinterpret_cast<const longlong2*>(&sm.VP[2 * cp_jp]);
-        const int bb = cp_b >> (16 * kind);
-        const int b0 = bb & 0xff, b1 = (bb >> 8) & 0xff;
 #pragma unroll
-        for (int k = 0; k < RPT; ++k) {
-          if (cp_r + k * RG < K) {
-            const int ao = (l > 0) ? ((cp_a[k] >> (16 * kind_prev)) & 0xffff) : NS * (NS + 1);   // layer 0: zero row
-            longlong2 v;
-            v.x = vp.x + sm.Esym[ao + b0];
-            v.y = vp.y + sm.Esym[ao + b1];
-            __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
+        for (int t = 0; t < G; ++t) {
+          if (t < nt) {
+            const typename SM::PerTile& pt = sm.t[t];
+            const int kind = (kinds >> (2 * t)) & 1, kind_prev = (kinds >> (2 * t + 1)) & 1;
+            const bool first = layer_of(t) == 0;
+            int64_t* out = T + (size_t)(tile0 + t) * K * K;
+            const longlong2 vp = *reinterpret_cast<const longlong2*>(&pt.VP[2 * cp_jp]);
+            const int bb = cp_b >> (16 * kind);
+            const int b0 = bb & 0xff, b1 = (bb >> 8) & 0xff;
+#pragma unroll
+            for (int k = 0; k < RPT; ++k) {
+              if (cp_r + k * RG < K) {
+                const int ao = first ? NS * (NS + 1) : ((cp_a[k] >> (16 * kind_prev)) & 0xffff);   // layer 0: zero row
+                longlong2 v;
+                v.x = vp.x + pt.Esym[ao + b0];
+                v.y = vp.y + pt.Esym[ao + b1];
+                __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
+              }
+            }
           }
         }
       }
     } else {
+      const typename SM::PerTile& pt = sm.t[0];
+      const RecBuf& rec = sm.rec[buf][0];
+      const int l = layer_of(0);
+      int64_t* out = T + (size_t)tile0 * K * K;
       for (int c = tid; c < K * KH; c += NT) {
         const int i = c / KH, j = (c % KH) * 2;
-        longlong2 v = make_longlong2(sm.VP[j], sm.VP[j + 1]);
+        longlong2 v = make_longlong2(pt.VP[j], pt.VP[j + 1]);
         if (l > 0) {
-          const int a = sm.sig[kind_prev][i].a_idx;
+          const int a = sm.sig[rec.kind_prev][i].a_idx;
           if (a < NS) {
             const int da = dual_vec<D>(a);
-            const SigInfo& s0 = sm.sig[kind][j];
-            const SigInfo& s1 = sm.sig[kind][j + 1];
-            if (s0.b_idx >= 0) v.x += sm.E[a * NS + s0.b_idx] + sm.E[s0.db_idx * NS + da];
-            if (s1.b_idx >= 0) v.y += sm.E[a * NS + s1.b_idx] + sm.E[s1.db_idx * NS + da];
+            const SigInfo& s0 = sm.sig[rec.kind][j];
+            const SigInfo& s1 = sm.sig[rec.kind][j + 1];
+            if (s0.b_idx >= 0) v.x += pt.E[a * NS + s0.b_idx] + pt.E[s0.db_idx * NS + da];
+            if (s1.b_idx >= 0) v.y += pt.E[a * NS + s1.b_idx] + pt.E[s1.db_idx * NS + da];
           }
         }
         __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
       }
-      if (tid < 5) cp_async_wait_all();
-      __syncthreads();                                     // E is rewritten by the next tile's step 3; publishes the record
+      if (tid < 5 * G) cp_async_wait_all();
+      __syncthreads();                                     // E is rewritten by the next group's step 3; publishes the records
     }
-    tile = tile_n;
-    l = l_n;
+    grp = grp_n;
+    l0 = l0_n;
     buf ^= 1;
   }
 }
@@ -432,8 +477,9 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   int dev = 0, sms = 148;
   ADL_CUDA_CHECK(cudaGetDevice(&dev));
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const int per_sm = (D == 3) ? 1 : 4;
-  const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;       // persistent, grid-stride over tiles
+  const int per_sm = (D == 3) ? 1 : 3;
+  const int ngroups = (ntiles + TileSmem<D>::G - 1) / TileSmem<D>::G;
+  const int grid = ngroups < sms * per_sm ? ngroups : sms * per_sm;     // persistent, grid-stride over tile groups
   build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
