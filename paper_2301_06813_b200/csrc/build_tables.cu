@@ -110,27 +110,6 @@ struct SigInfo {
   int32_t rowsplit, colsplit;
 };
 
-template <int D>
-struct TileSmem {
-  static constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
-  static constexpr bool kRows = (D <= 2);               // one thread per state pair: hoisted fast path
-  static constexpr int G = kRows ? 4 : 1;               // tiles processed together per loop iteration
-  struct PerTile {
-    int64_t Q[5][8];                                    // M, Kd, N, in_rows, in_cols  x  level subset
-    int64_t CG[D][NC + 1];                              // [..][NC] = 0: the slot that does not run
-    int64_t CA[D][NC + 1];
-    int64_t WAR[D][NC];
-    int64_t locW[NC], locO[NC];
-    alignas(16) int64_t VP[K];
-    alignas(16) int64_t E[NS * NS];
-    alignas(16) int64_t Esym[kRows ? (NS + 1) * (NS + 1) : 1];   // R[a][b] + R[dual b][dual a]; row NS, column NS = 0
-  };
-  RecBuf rec[2][G];
-  SigInfo sig[2][K];
-  alignas(16) PerTile t[G];
-};
-
-
 // split configuration index -> level subsets (rows, cols)
 template <int D>
 __device__ __forceinline__ void cfg_masks(int cfg, int& m0, int& m1) {
@@ -191,23 +170,11 @@ __device__ __forceinline__ int dual_vec(int v) {
   return r;
 }
 
+// facts per (layer kind, signature), built once per CTA
 template <int D>
-__global__ void __launch_bounds__(256, (D == 3) ? 1 : 3)
-build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
-                    int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
-  using SM = TileSmem<D>;
-  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2, G = SM::G;
-  constexpr bool kHoist = SM::kRows;                       // D <= 2: every per-thread index is tile-invariant
-  constexpr int RG = NT / KH < K ? NT / KH : K;            // row groups of the copy-out
-  constexpr int RPT = (K + RG - 1) / RG;                   // rows per thread of the copy-out
-  constexpr int STRIDE = NC + 1, TABN = 2 * D * STRIDE;    // CG then CA, contiguous per tile
-  static_assert(G * D * NC <= 96 && 192 + G * NC <= NT && G * 5 * (1 << D) <= NT, "role layout");
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  SM& sm = *reinterpret_cast<SM*>(smem_raw);
-  const int tid = threadIdx.x;
-
-  // ---- once per CTA: facts per (kind, signature) -----------------------------------------------------
-  for (int x = tid; x < 2 * K; x += NT) {
+__device__ __forceinline__ void fill_sig_table(SigInfo (*sig)[Pow<D>::K], const MeshParams& mp, int tid, int nthreads) {
+  constexpr int K = Pow<D>::K, NS = Pow<D>::NS;
+  for (int x = tid; x < 2 * K; x += nthreads) {
     const int kind = x / K, j = x % K;
     int dig[D], r = j;
 #pragma unroll
@@ -236,40 +203,225 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     si.b_idx = valid ? b : -1;
     si.db_idx = valid ? dual_vec<D>(b) : -1;
     si.cfgW = cw; si.cfgO = co; si.valid = valid; si.rowsplit = rs; si.colsplit = cs;
-    sm.sig[kind][j] = si;
+    sig[kind][j] = si;
   }
-  for (int x = tid; x < G * D; x += NT) { sm.t[x / D].CG[x % D][NC] = 0; sm.t[x / D].CA[x % D][NC] = 0; }
+}
+
+// ======================================================================================================
+// Generic kernel (any D; used for D = 1 and D = 3): one tile per loop iteration, direct 16-byte stores.
+// ======================================================================================================
+template <int D>
+struct TileSmem {
+  static constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC;
+  int64_t Q[5][8];                                      // M, Kd, N, in_rows, in_cols  x  level subset
+  int64_t CG[D][NC + 1];                                // [..][NC] = 0: the slot that does not run
+  int64_t CA[D][NC + 1];
+  int64_t WAR[D][NC];
+  int64_t locW[NC], locO[NC];
+  alignas(16) int64_t VP[K];
+  alignas(16) int64_t E[NS * NS];
+  RecBuf rec[2];
+  SigInfo sig[2][K];
+};
+
+template <int D>
+__global__ void __launch_bounds__(256)
+build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
+                    int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  using SM = TileSmem<D>;
+  constexpr int K = Pow<D>::K, NS = Pow<D>::NS, NC = Pow<D>::NC, NT = 256, KH = K / 2;
+  static_assert(D * NC <= 96 && 192 + NC <= NT && (5 << D) <= NT, "role layout");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  const int tid = threadIdx.x;
+
+  fill_sig_table<D>(sm.sig, mp, tid, NT);
+  if (tid < D) { sm.CG[tid][NC] = 0; sm.CA[tid][NC] = 0; }
+  __syncthreads();
+
+  // step 1 role: (extent, level subset); step 2 roles: A [0,96) B [96,192) C [192,..)
+  const int q_x = tid >> D, q_m = tid & ((1 << D) - 1);
+  const int role_base = tid < 96 ? 0 : (tid < 192 ? 96 : 192);
+  const int role_i = tid - role_base;
+  const int role_d = role_i / NC, role_cfg = role_i % NC;
+  int role_m0 = 0, role_m1 = 0;
+  cfg_masks<D>(role_cfg, role_m0, role_m1);
+  const int64_t cap_layer = mp.mem_cap / L;
+
+  int tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  auto stage = [&](int b, int tl) {                         // thread `part` stages 16-byte part (or the previous kind)
+    if (tid < 5) {
+      const autoddl_layer* cur = layers + tl;
+      RecBuf* dst = &sm.rec[b];
+      if (tid < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * tid, reinterpret_cast<const unsigned char*>(cur) + 16 * tid);
+      else cp_async4(&dst->kind_prev, &(tl % L > 0 ? cur - 1 : cur)->kind);
+    }
+  };
+  stage(0, tile);
+  cp_async_wait_all();
+  __syncthreads();
+  int buf = 0;
+
+  for (; tile < ntiles; tile += gridDim.x, buf ^= 1) {
+    const int tile_n = tile + gridDim.x;
+    stage(buf ^ 1, tile_n < ntiles ? tile_n : tile);
+    const int l = tile % L;
+    const RecBuf& rec = sm.rec[buf];
+
+    // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
+    if (tid < (5 << D)) sm.Q[q_x][q_m] = cdiv_magic(rec.X[q_x], (uint32_t)mp.sub[q_m], mp.magic_sub[q_m]);
+    __syncthreads();
+
+    // ---- 2. tables per level and split configuration -------------------------------------------------------
+    if (role_base == 0 && role_i < D * NC) {
+      if (l > 0) {                                           // input tensor: Table 2 rows 2 and 3
+        const int d = role_d;
+        const int64_t n = sm.Q[3][role_m0] * sm.Q[4][role_m1] * (int64_t)rec.eb;
+        const int64_t p = mp.size[d];
+        int64_t cg = 0, ca = 0;
+        if (p > 1) {
+          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+        }
+        sm.CG[d][role_cfg] = cg;
+        sm.CA[d][role_cfg] = ca;
+      }
+    } else if (role_base == 96 && role_i < D * NC) {
+      if (rec.kind == AUTODDL_GEMM) {                        // weight gradient: AllReduce row
+        const int d = role_d;
+        const int64_t n = sm.Q[1][role_m0] * sm.Q[2][role_m1] * (int64_t)rec.wgb;
+        const int64_t p = mp.size[d];
+        sm.WAR[d][role_cfg] =
+            p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
+      }
+    } else if (role_base == 192 && role_i < NC) {
+      sm.locW[role_cfg] = sm.Q[1][role_m0] * sm.Q[2][role_m1];
+      sm.locO[role_cfg] = sm.Q[0][role_m0] * sm.Q[2][role_m1];
+    }
+    __syncthreads();
+
+    // ---- 3. VP[j] (node cost + penalty) and R[a][b] ------------------------------------------------------------
+    for (int j = tid; j < K; j += NT) {
+      const SigInfo si = sm.sig[rec.kind][j];
+      int64_t v = 0, mem = 0;
+      if (si.valid) {
+        if (rec.kind == AUTODDL_GEMM) {
+#pragma unroll
+          for (int d = 0; d < D; ++d)
+            if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
+          mem = sm.locW[si.cfgW] * (int64_t)rec.wsb;
+        }
+        mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * (int64_t)rec.eb;
+      }
+      const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+      sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+      const size_t o = (size_t)tile * K + j;
+      if (node) node[o] = v;
+      if (mask) mask[o] = ok ? 1 : 0;
+    }
+    if (l > 0) {
+      const int64_t* tab = &sm.CG[0][0];
+      for (int e = tid; e < NS * NS; e += NT) {
+        int idx[3 * D];
+        r_slots<D>(e / NS, e % NS, idx);
+        int64_t c = 0;
+#pragma unroll
+        for (int k = 0; k < 3 * D; ++k) c += tab[idx[k]];
+        sm.E[e] = c;
+      }
+    }
+    __syncthreads();
+
+    // ---- 4. K x K expansion: forward leg R[a][b] + backward leg R[dual b][dual a] + VP[j] ---------------------
+    int64_t* out = T + (size_t)tile * K * K;
+    for (int c = tid; c < K * KH; c += NT) {
+      const int i = c / KH, j = (c % KH) * 2;
+      longlong2 v = make_longlong2(sm.VP[j], sm.VP[j + 1]);
+      if (l > 0) {
+        const int a = sm.sig[rec.kind_prev][i].a_idx;
+        if (a < NS) {
+          const int da = dual_vec<D>(a);
+          const SigInfo& s0 = sm.sig[rec.kind][j];
+          const SigInfo& s1 = sm.sig[rec.kind][j + 1];
+          if (s0.b_idx >= 0) v.x += sm.E[a * NS + s0.b_idx] + sm.E[s0.db_idx * NS + da];
+          if (s1.b_idx >= 0) v.y += sm.E[a * NS + s1.b_idx] + sm.E[s1.db_idx * NS + da];
+        }
+      }
+      __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
+    }
+    if (tid < 5) cp_async_wait_all();
+    __syncthreads();                                       // E is rewritten by the next tile's step 3; publishes the record
+  }
+}
+
+// ======================================================================================================
+// K = 36 kernel (two mesh levels): distinct rows in shared memory, TMA bulk stores to global.
+//
+// A tile has only 16 distinct rows: row i depends on i through the producer's output state vector a(i),
+// and the per-level output states of signatures 2, 4, 5 coincide (all P; for ATTN all invalid).  With
+// class(i0) = {0,1,2,3,2,2}[i0] over the level-0 digit, rows 6*i0 .. 6*i0+5 of the tile equal the block
+// EV[class(i0)][0..5][.] of 6 x 36 cells.  Per tile the CTA computes the 24 x 36 block rows
+//   EV[r][j] = VP[j] + R[a(r)][b(j)] + R[dual b(j)][dual a(r)]
+// in shared memory and one thread issues six 1,728-byte cp.async.bulk shared->global copies (SASS UBLKCP);
+// the store stream runs on the TMA engine while the CTA prepares the next group of tiles (EV is double
+// buffered; cp.async.bulk.wait_group.read guards its reuse).  G = 4 tiles share one barrier sequence.
+// ======================================================================================================
+struct Smem36 {
+  static constexpr int D = 2, K = 36, NS = 16, NC = 9, G = 4, ES = NS + 1, NROW = 24, STRIDE = NC + 1;
+  struct PerTile {
+    int64_t Q[5][4];                                    // M, Kd, N, in_rows, in_cols  x  level subset
+    int64_t TAB[2 * D * STRIDE];                        // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
+    int64_t WAR[D][NC];
+    int64_t locW[NC], locO[NC];
+    alignas(16) int64_t VP[K];
+    alignas(16) int64_t E[ES * ES];                     // R[a][b]; row NS and column NS stay 0
+  };
+  alignas(128) int64_t EV[2][G][NROW * K];
+  PerTile t[G];
+  RecBuf rec[2][G];
+  SigInfo sig[2][K];
+  int32_t meta[2];                                      // (kind | kind_prev << 1) of the group's tiles, 2 bits each
+};
+
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes)
+               : "memory");
+}
+
+__global__ void __launch_bounds__(256, 3)
+build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
+                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  using SM = Smem36;
+  constexpr int D = 2, K = SM::K, NS = SM::NS, NC = SM::NC, NT = 256, G = SM::G, ES = SM::ES, NROW = SM::NROW;
+  constexpr int STRIDE = SM::STRIDE;
+  constexpr int ISSUER = NT - 1;                           // idle in step 4 (252 threads fill EV)
+  static_assert(G * D * NC <= 96 && 192 + G * NC <= NT && G * 5 * (1 << D) <= NT && G * K <= NT, "role layout");
+  extern __shared__ __align__(128) unsigned char smem36_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem36_raw);
+  const int tid = threadIdx.x;
+
+  fill_sig_table<D>(sm.sig, mp, tid, NT);
+  for (int x = tid; x < G * ES * ES; x += NT) sm.t[x / (ES * ES)].E[x % (ES * ES)] = 0;
+  for (int x = tid; x < G * 2 * D; x += NT) sm.t[x / (2 * D)].TAB[(x % (2 * D)) * STRIDE + NC] = 0;
   __syncthreads();
 
   // ---- tile-invariant roles of this thread ---------------------------------------------------------------
-  int slot[3 * D];                                         // step 3: the table entries summing to R[tid]
-  int partner = 0;                                         // step 4: index of R[dual b][dual a]
-  int cp_a[RPT];                                           // step 5: a_idx * (NS+1) of row r + k * RG for both producer kinds
-  int cp_b = 0;                                            // step 5: b_idx of columns 2jp, 2jp+1 for both consumer kinds
-  const int cp_r = tid / KH, cp_jp = tid % KH;
-  if (kHoist) {
-    if (tid < NS * NS) {
-      r_slots<D>(tid / NS, tid % NS, slot);
-      partner = dual_vec<D>(tid % NS) * NS + dual_vec<D>(tid / NS);
-    }
+  // step 3: thread (a, b) sums the <= 6 table entries of R[a][b]
+  int slot[3 * D];
+  r_slots<D>(tid / NS, tid % NS, slot);
+  const int e_own = (tid / NS) * ES + tid % NS;
+  // step 4: thread (r0, j) fills EV rows r0, r0+7, r0+14, r0+21 of column j; indices for GEMM -> GEMM edges
+  const int ev_j = tid % K, ev_r0 = tid / K;               // ev_r0 = 7 for the last four threads: no rows
+  int ev_idx[4];
+  {
+    const int b = sm.sig[0][ev_j].b_idx, db = sm.sig[0][ev_j].db_idx;
 #pragma unroll
-    for (int k = 0; k < RPT; ++k) {
-      const int i = cp_r + k * RG;
-      if (cp_r < RG && i < K) {
-        const int a0 = sm.sig[0][i].a_idx, a1 = sm.sig[1][i].a_idx;       // a = NS (invalid) selects the zero row
-        cp_a[k] = (a0 * (NS + 1)) | (a1 * (NS + 1)) << 16;
-      } else {
-        cp_a[k] = 0;
-      }
+    for (int k = 0; k < 4; ++k) {
+      const int r = ev_r0 + 7 * k;
+      const int a = sm.sig[0][(r < NROW ? (r / 6) * 6 + r % 6 : 0)].a_idx;      // class representative i0 = r / 6
+      ev_idx[k] = (a * ES + b) | (db * ES + dual_vec<D>(a)) << 16;
     }
-    if (cp_r < RG) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int b = sm.sig[q >> 1][2 * cp_jp + (q & 1)].b_idx;
-        cp_b |= (b >= 0 ? b : NS) << (8 * q);                  // b = NS (invalid) selects the zero column
-      }
-    }
-    for (int x = tid; x < G * (NS + 1) * (NS + 1); x += NT) sm.t[x / ((NS + 1) * (NS + 1))].Esym[x % ((NS + 1) * (NS + 1))] = 0;
   }
   // step 1 role: (tile in group, extent, level subset); step 2 roles: A [0,96) B [96,192) C [192,..)
   const int q_t = tid / (5 << D), q_x = (tid % (5 << D)) >> D, q_m = tid & ((1 << D) - 1);
@@ -280,6 +432,7 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
   const int role_cfg = role_i % NC;
   int role_m0 = 0, role_m1 = 0;
   cfg_masks<D>(role_cfg, role_m0, role_m1);
+  const int vp_t = tid / K, vp_j = tid % K;                // step 3: VP role (tid < G * K)
   const int64_t cap_layer = mp.mem_cap / L;
   const int ngroups = (ntiles + G - 1) / G;
 
@@ -302,21 +455,34 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
       else cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
     }
   };
+  auto pack_meta = [&](int b) {                             // after the records of buffer b have landed and are published
+    int m = 0;
+#pragma unroll
+    for (int t = 0; t < G; ++t) m |= (sm.rec[b][t].kind | sm.rec[b][t].kind_prev << 1) << (2 * t);
+    sm.meta[b] = m;
+  };
   stage_group(0, grp, l0);
   cp_async_wait_all();
   __syncthreads();
+  if (tid == 0) pack_meta(0);
 
-  while (grp < ngroups) {
+  for (int it = 0; grp < ngroups; ++it) {
     const int grp_n = grp + gridDim.x;
     int l0_n = l0 + l_step;
     if (l0_n >= L) l0_n -= L;
     stage_group(buf ^ 1, grp_n < ngroups ? grp_n : grp, grp_n < ngroups ? l0_n : l0);
     const int tile0 = grp * G;
     const int nt = ntiles - tile0 < G ? ntiles - tile0 : G;   // tiles of this group that exist
-    auto layer_of = [&](int t) { int l = l0 + t; while (l >= L) l -= L; return l; };
-    int kinds = 0;                                           // (kind, kind_prev) of every tile of the group, read before
-#pragma unroll                                               // the record buffer can be restaged by a faster thread
-    for (int t = 0; t < G; ++t) kinds |= (sm.rec[buf][t].kind | sm.rec[buf][t].kind_prev << 1) << (2 * t);
+    int first = 0;                                            // bit t: tile t of the group is a chain's layer 0
+    {
+      int l = l0;
+#pragma unroll
+      for (int t = 0; t < G; ++t) {
+        first |= (l == 0) << t;
+        l = (l + 1 == L) ? 0 : l + 1;
+      }
+    }
+    const int eb = it & 1;
 
     // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
     if (tid < G * (5 << D) && q_t < nt)
@@ -325,10 +491,10 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 
     // ---- 2. tables per level and split configuration -------------------------------------------------------
     if (role_t < nt) {
-      typename SM::PerTile& pt = sm.t[role_t];
+      SM::PerTile& pt = sm.t[role_t];
       const RecBuf& rec = sm.rec[buf][role_t];
       if (role_base == 0 && role_i < G * D * NC) {
-        if (layer_of(role_t) > 0) {                          // input tensor: Table 2 rows 2 and 3
+        if (!(first >> role_t & 1)) {                        // input tensor: Table 2 rows 2 and 3
           const int d = role_d;
           const int64_t n = pt.Q[3][role_m0] * pt.Q[4][role_m1] * (int64_t)rec.eb;
           const int64_t p = mp.size[d];
@@ -337,8 +503,8 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
             cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
             ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
           }
-          pt.CG[d][role_cfg] = cg;
-          pt.CA[d][role_cfg] = ca;
+          pt.TAB[d * STRIDE + role_cfg] = cg;
+          pt.TAB[(D + d) * STRIDE + role_cfg] = ca;
         }
       } else if (role_base == 96 && role_i < G * D * NC) {
         if (rec.kind == AUTODDL_GEMM) {                      // weight gradient: AllReduce row
@@ -355,12 +521,11 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     }
     __syncthreads();
 
-    // ---- 3. VP[j] (node cost + penalty) and R[a][b] ------------------------------------------------------------
-    for (int x = tid; x < nt * K; x += NT) {
-      const int t = x / K, j = x % K;
-      typename SM::PerTile& pt = sm.t[t];
-      const RecBuf& rec = sm.rec[buf][t];
-      const SigInfo si = sm.sig[rec.kind][j];
+    // ---- 3. VP[j] (node cost + penalty) and R[a][b] (zero for a chain's first layer: no producer) -----------------
+    if (tid < G * K && vp_t < nt) {
+      SM::PerTile& pt = sm.t[vp_t];
+      const RecBuf& rec = sm.rec[buf][vp_t];
+      const SigInfo si = sm.sig[rec.kind][vp_j];
       int64_t v = 0, mem = 0;
       if (si.valid) {
         if (rec.kind == AUTODDL_GEMM) {
@@ -372,100 +537,79 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         mem += (pt.Q[3][si.mI0] * pt.Q[4][si.mI1] + pt.locO[si.cfgO]) * (int64_t)rec.eb;
       }
       const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
-      pt.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
-      const size_t o = (size_t)(tile0 + t) * K + j;
+      pt.VP[vp_j] = v + (ok ? 0 : AUTODDL_PEN);
+      const size_t o = (size_t)(tile0 + vp_t) * K + vp_j;
       if (node) node[o] = v;
       if (mask) mask[o] = ok ? 1 : 0;
     }
-    if (kHoist) {
-      if (tid < NS * NS) {
 #pragma unroll
-        for (int t = 0; t < G; ++t) {
-          if (t < nt && layer_of(t) > 0) {
-            const int64_t* tab = &sm.t[t].CG[0][0];
-            int64_t c = 0;
+    for (int t = 0; t < G; ++t) {
+      if (t < nt) {
+        const int64_t* tab = sm.t[t].TAB;
+        int64_t c = 0;
+        if (!(first >> t & 1)) {
 #pragma unroll
-            for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
-            sm.t[t].E[tid] = c;
-          }
+          for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
         }
-      }
-    } else {
-      if (layer_of(0) > 0) {
-        const int64_t* tab = &sm.t[0].CG[0][0];
-        for (int e = tid; e < NS * NS; e += NT) {
-          int idx[3 * D];
-          r_slots<D>(e / NS, e % NS, idx);
-          int64_t c = 0;
-#pragma unroll
-          for (int k = 0; k < 3 * D; ++k) c += tab[idx[k]];
-          sm.t[0].E[e] = c;
-        }
+        sm.t[t].E[e_own] = c;
       }
     }
     __syncthreads();
 
-    if (kHoist) {
-      // ---- 4. Esym[a][b] = R[a][b] + R[dual b][dual a]: forward leg + backward leg ------------------------------
-      if (tid < NS * NS) {
-#pragma unroll
-        for (int t = 0; t < G; ++t)
-          if (t < nt && layer_of(t) > 0) sm.t[t].Esym[(tid / NS) * (NS + 1) + tid % NS] = sm.t[t].E[tid] + sm.t[t].E[partner];
-      }
-      if (tid < 5 * G) cp_async_wait_all();                // the next group's records have landed; the barrier publishes them
-      __syncthreads();
-      // ---- 5. K x K expansion: one gather + one add per cell, 16-byte streaming stores ---------------------------
-      if (cp_r < RG) {
+    // ---- 4. EV[r][j] = VP[j] + R[a(r)][b(j)] + R[dual b(j)][dual a(r)]: the 24 block rows of every tile ---------------
+    const int meta = sm.meta[buf];
+    if (ev_r0 < 7) {
+      if (meta == 0) {                                       // every edge of the group is GEMM -> GEMM: hoisted indices
 #pragma unroll
         for (int t = 0; t < G; ++t) {
           if (t < nt) {
-            const typename SM::PerTile& pt = sm.t[t];
-            const int kind = (kinds >> (2 * t)) & 1, kind_prev = (kinds >> (2 * t + 1)) & 1;
-            const bool first = layer_of(t) == 0;
-            int64_t* out = T + (size_t)(tile0 + t) * K * K;
-            const longlong2 vp = *reinterpret_cast<const longlong2*>(&pt.VP[2 * cp_jp]);
-            const int bb = cp_b >> (16 * kind);
-            const int b0 = bb & 0xff, b1 = (bb >> 8) & 0xff;
+            const int64_t* E = sm.t[t].E;
+            const int64_t vp = sm.t[t].VP[ev_j];
+            int64_t* ev = &sm.EV[eb][t][ev_j];
 #pragma unroll
-            for (int k = 0; k < RPT; ++k) {
-              if (cp_r + k * RG < K) {
-                const int ao = first ? NS * (NS + 1) : ((cp_a[k] >> (16 * kind_prev)) & 0xffff);   // layer 0: zero row
-                longlong2 v;
-                v.x = vp.x + pt.Esym[ao + b0];
-                v.y = vp.y + pt.Esym[ao + b1];
-                __stcs(reinterpret_cast<longlong2*>(out + (size_t)(cp_r + k * RG) * K + 2 * cp_jp), v);
-              }
-            }
+            for (int k = 0; k < 4; ++k)
+              if (ev_r0 + 7 * k < NROW) ev[(ev_r0 + 7 * k) * K] = vp + E[ev_idx[k] & 0xffff] + E[ev_idx[k] >> 16];
+          }
+        }
+      } else {
+        for (int t = 0; t < nt; ++t) {
+          const int kind = (meta >> (2 * t)) & 1, kind_prev = (meta >> (2 * t + 1)) & 1;
+          const int64_t* E = sm.t[t].E;
+          const int64_t vp = sm.t[t].VP[ev_j];
+          int b = sm.sig[kind][ev_j].b_idx, db = sm.sig[kind][ev_j].db_idx;
+          if (b < 0) b = db = NS;                            // invalid consumer signature: zero column
+          for (int r = ev_r0; r < NROW; r += 7) {
+            const int a = sm.sig[kind_prev][r].a_idx;        // class representative: i0 = r / 6 in 0..3
+            const int da = a < NS ? dual_vec<D>(a) : NS;      // invalid producer signature: zero row
+            sm.EV[eb][t][r * K + ev_j] = vp + E[a * ES + b] + E[db * ES + da];
           }
         }
       }
-    } else {
-      const typename SM::PerTile& pt = sm.t[0];
-      const RecBuf& rec = sm.rec[buf][0];
-      const int l = layer_of(0);
-      int64_t* out = T + (size_t)tile0 * K * K;
-      for (int c = tid; c < K * KH; c += NT) {
-        const int i = c / KH, j = (c % KH) * 2;
-        longlong2 v = make_longlong2(pt.VP[j], pt.VP[j + 1]);
-        if (l > 0) {
-          const int a = sm.sig[rec.kind_prev][i].a_idx;
-          if (a < NS) {
-            const int da = dual_vec<D>(a);
-            const SigInfo& s0 = sm.sig[rec.kind][j];
-            const SigInfo& s1 = sm.sig[rec.kind][j + 1];
-            if (s0.b_idx >= 0) v.x += pt.E[a * NS + s0.b_idx] + pt.E[s0.db_idx * NS + da];
-            if (s1.b_idx >= 0) v.y += pt.E[a * NS + s1.b_idx] + pt.E[s1.db_idx * NS + da];
-          }
-        }
-        __stcs(reinterpret_cast<longlong2*>(out + (size_t)i * K + j), v);
-      }
-      if (tid < 5 * G) cp_async_wait_all();
-      __syncthreads();                                     // E is rewritten by the next group's step 3; publishes the records
     }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // EV written by the generic proxy, read by TMA
+    if (tid < 5 * G) cp_async_wait_all();                    // the next group's records have landed; the barrier publishes them
+    __syncthreads();
+
+    // ---- 5. six 1,728-byte bulk stores per tile; the copies run while the CTA prepares the next group -----------------
+    if (tid == ISSUER) {
+      for (int t = 0; t < nt; ++t) {
+        int64_t* out = T + (size_t)(tile0 + t) * K * K;
+        const int64_t* src = sm.EV[eb][t];
+#pragma unroll
+        for (int i0 = 0; i0 < 6; ++i0) {
+          const int cls = i0 < 4 ? i0 : 2;
+          bulk_s2g(out + i0 * 6 * K, src + cls * 6 * K, 6 * K * 8);
+        }
+      }
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the other EV buffer is free again
+    }
+    if (tid == 0) pack_meta(buf ^ 1);
     grp = grp_n;
     l0 = l0_n;
     buf ^= 1;
   }
+  if (tid == ISSUER) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 template <int D>
@@ -477,10 +621,24 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   int dev = 0, sms = 148;
   ADL_CUDA_CHECK(cudaGetDevice(&dev));
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const int per_sm = (D == 3) ? 1 : 3;
-  const int ngroups = (ntiles + TileSmem<D>::G - 1) / TileSmem<D>::G;
-  const int grid = ngroups < sms * per_sm ? ngroups : sms * per_sm;     // persistent, grid-stride over tile groups
+  const int per_sm = (D == 3) ? 1 : 4;
+  const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;     // persistent, grid-stride over tiles
   build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
+              int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
+  const size_t smem = sizeof(Smem36);
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(build_tables36_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int dev = 0, sms = 148;
+  ADL_CUDA_CHECK(cudaGetDevice(&dev));
+  ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int ngroups = (ntiles + Smem36::G - 1) / Smem36::G;
+  const int grid = ngroups < sms * 3 ? ngroups : sms * 3;             // persistent, grid-stride over tile groups
+  build_tables36_kernel<<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -494,7 +652,7 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
   if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   switch (mp.ndim) {
     case 1: return launch_d<1>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
-    case 2: return launch_d<2>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
+    case 2: return launch_36(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     case 3: return launch_d<3>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
   }
   set_error("ndim must be 1, 2 or 3");
