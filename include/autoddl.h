@@ -79,8 +79,10 @@ int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                          int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* stream);
 
 /* (a2) f_0[j] = T[0][0][j]; f_l[j] = min_i f_{l-1}[i] + T[l][i][j]; smallest index wins every tie;
- * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: tables are first built from d_layers
- * into d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers.
+ * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: the tables are computed from d_layers
+ * -- on a 2-level mesh (K = 36) inside the DP kernel itself, tile by tile in shared memory, never
+ * stored; otherwise they are first built into d_work.  d_work (>= autoddl_workspace_bytes) also
+ * holds back-pointers (fused kernel: of the chains in flight; separate kernel: when L * K > 16384).
  * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
 int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                      const autoddl_mesh* mesh, const autoddl_net* net,
@@ -97,6 +99,20 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                           const int64_t* d_T, void* d_work, size_t work_bytes,
                           const int32_t* d_init, int32_t S, int32_t max_sweeps,
                           int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, void* stream);
+
+/* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36)
+ * (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and
+ * consumed by the chain DP from shared memory, so the optimum costs no table read.  Other meshes run
+ * the three kernels back to back.  Results are identical to the three separate calls.
+ * d_T: [Bp][L][K][K] output, or NULL to keep the tables in d_work (any mesh) -- with d_init == NULL
+ * and K = 36 no table is materialised at all.  d_node / d_mask may be NULL.  d_init == NULL skips (a3).
+ * d_work: >= autoddl_workspace_bytes(Bp, L, S, mesh). */
+int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
+                   const autoddl_mesh* mesh, const autoddl_net* net,
+                   int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* d_work, size_t work_bytes,
+                   int64_t* d_opt_cost, int32_t* d_strategy,
+                   const int32_t* d_init, int32_t S, int32_t max_sweeps,
+                   int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, void* stream);
 
 /* Whole path with HOST inputs and outputs (the end-to-end call): copies h_layers and h_init to the
  * device, runs (a1) (a2) (a3) in d_work, copies the results back, synchronises `stream`.

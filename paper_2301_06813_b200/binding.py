@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -58,6 +58,8 @@ def lib():
         L.autoddl_chain_dp.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, vp, vp]
         L.autoddl_coord_descent.restype = C.c_int
         L.autoddl_coord_descent.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_search.restype = C.c_int
+        L.autoddl_search.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.autoddl_search_host.restype = C.c_int
         L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
         L.autoddl_copy_probe.restype = C.c_int
@@ -145,7 +147,10 @@ def chain_dp(T: torch.Tensor | None, mesh, net=None, d_layers=None, work: torch.
         dev = d_layers.device
     if work is None:
         K = 6 ** len(mesh.size)
-        need = (0 if T is not None else Bp * L * K * K * 8 + 256) + (Bp * L * K + 256 if L * K > 16384 else 0)
+        if T is None:
+            need = workspace_bytes(Bp, L, 0, mesh)
+        else:
+            need = Bp * L * K + 256 if L * K > 16384 else 0
         work = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     if out is None:
         cost = torch.empty(Bp, dtype=torch.int64, device=dev)
@@ -179,6 +184,40 @@ def coord_descent(T: torch.Tensor | None, init: torch.Tensor, mesh, max_sweeps: 
                                        _ptr(T), _ptr(work), work.numel() if work is not None else 0, _ptr(init), S,
                                        max_sweeps, _ptr(cost), _ptr(strat), _ptr(sweeps), _stream()))
     return cost, strat, sweeps
+
+
+def search(d_layers: torch.Tensor, mesh, net, init: torch.Tensor | None = None, max_sweeps: int = 64,
+           want_tables: bool = True, want_node_mask: bool = False, work: torch.Tensor | None = None, out=None):
+    """Whole path on device tensors in one call (autoddl_search).  Returns a dict with T (or None), node, mask,
+    opt_cost, strategy and, when init is given, cd_cost, cd_strategy, cd_sweeps."""
+    Bp, L = d_layers.shape[0], d_layers.shape[1]
+    K = 6 ** len(mesh.size)
+    dev = d_layers.device
+    o = dict(out) if out else {}
+    if want_tables and "T" not in o:
+        o["T"] = torch.empty((Bp, L, K, K), dtype=torch.int64, device=dev)
+    if want_node_mask:
+        o.setdefault("node", torch.empty((Bp, L, K), dtype=torch.int64, device=dev))
+        o.setdefault("mask", torch.empty((Bp, L, K), dtype=torch.uint8, device=dev))
+    o.setdefault("opt_cost", torch.empty(Bp, dtype=torch.int64, device=dev))
+    o.setdefault("strategy", torch.empty((Bp, L), dtype=torch.int32, device=dev))
+    S = 0
+    if init is not None:
+        S = init.shape[1]
+        o.setdefault("cd_cost", torch.empty((Bp, S), dtype=torch.int64, device=dev))
+        o.setdefault("cd_strategy", torch.empty((Bp, S, L), dtype=torch.int32, device=dev))
+        o.setdefault("cd_sweeps", torch.empty((Bp, S), dtype=torch.int32, device=dev))
+    if work is None:
+        need = workspace_bytes(Bp, L, S, mesh)
+        if o.get("T") is not None:
+            need -= Bp * L * K * K * 8                       # tables go to T, not to the workspace
+        work = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    m, n = c_mesh(mesh), c_net(net)
+    _check(lib().autoddl_search(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n), _ptr(o.get("T")), _ptr(o.get("node")),
+                                _ptr(o.get("mask")), _ptr(work), work.numel() if work is not None else 0,
+                                _ptr(o["opt_cost"]), _ptr(o["strategy"]), _ptr(init), S, max_sweeps,
+                                _ptr(o.get("cd_cost")), _ptr(o.get("cd_strategy")), _ptr(o.get("cd_sweeps")), _stream()))
+    return o
 
 
 def search_host(w: Workload, init: np.ndarray | None, work: torch.Tensor, pinned=None):

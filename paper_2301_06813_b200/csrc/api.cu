@@ -97,6 +97,7 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   if (validate_mesh_net(mesh, nullptr, nullptr) || Bp < 1 || L < 1 || S < 0) return 0;
   const int64_t K = num_sigs(mesh->ndim);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
+  if (mesh->ndim == 2) b += fused_bp_bytes(L);              // fused build + DP: back-pointers of the chains in flight
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
   b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
   b += align_up((size_t)Bp * S * L * 4, 256) * 2;
@@ -131,16 +132,24 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
   ADL_REQUIRE(d_opt_cost != nullptr && d_strategy != nullptr, "output pointer is NULL");
   ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
   ADL_REQUIRE(((uintptr_t)d_opt_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0, "misaligned output pointer");
+  if (!d_T) ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
   const int K = num_sigs(mesh->ndim);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!d_T && fused_build_dp_supported(mp, L)) {            // tables never leave shared memory
+    if (d_work == nullptr || work_bytes < fused_bp_bytes(L)) {
+      set_error("chain_dp: workspace of %zu bytes needed, %zu given", fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
+      return AUTODDL_EWORK;
+    }
+    if ((rc = check_device())) return rc;
+    return launch_build_dp_fused(d_layers, Bp, L, mp, nullptr, nullptr, nullptr, d_opt_cost, d_strategy, (uint8_t*)d_work, st);
+  }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
   if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
     set_error("chain_dp: workspace of %zu bytes needed, %zu given", tb + bb, d_work ? work_bytes : (size_t)0);
     return AUTODDL_EWORK;
   }
   if ((rc = check_device())) return rc;
-  cudaStream_t st = (cudaStream_t)stream;
   if (!d_T) {
-    ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
     d_T = (const int64_t*)d_work;
   }
@@ -177,6 +186,67 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
 }
 
+// (a1) -> (a2) -> (a3) on device pointers; tables go to d_T, or into d_work when d_T is NULL
+static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int K,
+                         int64_t* d_T, int64_t* d_node, uint8_t* d_mask, unsigned char* d_work, size_t work_bytes,
+                         int64_t* d_opt_cost, int32_t* d_strategy, const int32_t* d_init, int32_t S, int32_t max_sweeps,
+                         int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, cudaStream_t st) {
+  const bool do_cd = d_init != nullptr;
+  const bool fused = fused_build_dp_supported(mp, L);
+  const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
+  size_t used = 0;
+  int rc;
+  if (need_tables && !d_T && (do_cd || !fused)) {
+    used = table_bytes(Bp, L, K);
+    if (d_work == nullptr || work_bytes < used) {
+      set_error("search: workspace of %zu bytes needed for the tables, %zu given", used, d_work ? work_bytes : (size_t)0);
+      return AUTODDL_EWORK;
+    }
+    d_T = (int64_t*)d_work;
+  }
+  if (fused) {
+    if (d_work == nullptr || work_bytes < used + fused_bp_bytes(L)) {
+      set_error("search: workspace of %zu bytes needed, %zu given", used + fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
+      return AUTODDL_EWORK;
+    }
+    if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used, st))) return rc;
+  } else {
+    const size_t bb = bp_bytes(Bp, L, K);
+    if (bb && (d_work == nullptr || work_bytes < used + bb)) {
+      set_error("search: workspace of %zu bytes needed, %zu given", used + bb, d_work ? work_bytes : (size_t)0);
+      return AUTODDL_EWORK;
+    }
+    if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
+    if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + used : nullptr, d_opt_cost, d_strategy, st))) return rc;
+  }
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+  return AUTODDL_OK;
+}
+
+int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh, const autoddl_net* net,
+                   int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* d_work, size_t work_bytes, int64_t* d_opt_cost,
+                   int32_t* d_strategy, const int32_t* d_init, int32_t S, int32_t max_sweeps, int64_t* d_cd_cost,
+                   int32_t* d_cd_strategy, int32_t* d_cd_sweeps, void* stream) {
+  clear_error();
+  MeshParams mp;
+  ADL_REQUIRE(net != nullptr, "net is NULL");
+  int rc = validate_mesh_net(mesh, net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(d_layers != nullptr && d_opt_cost != nullptr && d_strategy != nullptr, "NULL pointer");
+  ADL_REQUIRE(Bp >= 1 && L >= 1, "Bp = %d, L = %d must be >= 1", Bp, L);
+  if (d_init) {
+    ADL_REQUIRE(S >= 1 && max_sweeps >= 1, "S, max_sweeps must be >= 1");
+    ADL_REQUIRE(d_cd_cost && d_cd_strategy && d_cd_sweeps, "NULL Coordinate Descent output");
+  }
+  ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
+  ADL_REQUIRE(((uintptr_t)d_layers & 7) == 0 && ((uintptr_t)d_node & 7) == 0 && ((uintptr_t)d_opt_cost & 7) == 0 &&
+                  ((uintptr_t)d_cd_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0 && ((uintptr_t)d_init & 3) == 0 &&
+                  ((uintptr_t)d_cd_strategy & 3) == 0 && ((uintptr_t)d_cd_sweeps & 3) == 0, "misaligned pointer");
+  if ((rc = check_device())) return rc;
+  return search_device(d_layers, Bp, L, mp, num_sigs(mesh->ndim), d_T, d_node, d_mask, (unsigned char*)d_work, work_bytes,
+                       d_opt_cost, d_strategy, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, (cudaStream_t)stream);
+}
+
 int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
                         const autoddl_net* net, const int32_t* h_init, int32_t S, int32_t max_sweeps,
                         void* d_work, size_t work_bytes, int64_t* h_opt_cost, int32_t* h_strategy,
@@ -203,8 +273,8 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
 
   unsigned char* w = (unsigned char*)d_work;
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
-  int64_t* d_T = (int64_t*)carve(table_bytes(Bp, L, K));
-  uint8_t* d_bp = bp_bytes(Bp, L, K) ? (uint8_t*)carve(bp_bytes(Bp, L, K)) : nullptr;
+  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) + (mesh->ndim == 2 ? fused_bp_bytes(L) : 0);
+  unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));
   int32_t* d_init = (int32_t*)carve((size_t)Bp * S * L * 4);
   int32_t* d_cd_strategy = (int32_t*)carve((size_t)Bp * S * L * 4);
@@ -215,10 +285,8 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
 
   ADL_CUDA_CHECK(cudaMemcpyAsync(d_layers, h_layers, (size_t)Bp * L * sizeof(autoddl_layer), cudaMemcpyHostToDevice, st));
   if (do_cd) ADL_CUDA_CHECK(cudaMemcpyAsync(d_init, h_init, (size_t)Bp * S * L * 4, cudaMemcpyHostToDevice, st));
-  if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, nullptr, nullptr, st))) return rc;
-  if ((rc = launch_chain_dp(d_T, Bp, L, K, d_bp, d_opt, d_strategy, st))) return rc;
-  if (do_cd &&
-      (rc = launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
+  if ((rc = search_device(d_layers, Bp, L, mp, K, nullptr, nullptr, nullptr, d_tables, tables_region,
+                          d_opt, d_strategy, do_cd ? d_init : nullptr, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
     return rc;
   if (h_opt_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_opt_cost, d_opt, (size_t)Bp * 8, cudaMemcpyDeviceToHost, st));
   if (h_strategy) ADL_CUDA_CHECK(cudaMemcpyAsync(h_strategy, d_strategy, (size_t)Bp * L * 4, cudaMemcpyDeviceToHost, st));

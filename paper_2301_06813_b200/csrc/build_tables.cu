@@ -22,6 +22,8 @@
 //   5. the K x K expansion T[i][j] = Esym[O-state(i)][I-state(j)] + VP[j]: one shared-memory gather and one
 //      64-bit add per cell, 16-byte streaming stores; all indices are hoisted out of the tile loop.
 // The kernel is then bound by the HBM write of 8 B per cell instead of integer arithmetic.
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace autoddl {
@@ -367,8 +369,9 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
 // the store stream runs on the TMA engine while the CTA prepares the next group of tiles (EV is double
 // buffered; cp.async.bulk.wait_group.read guards its reuse).  G = 4 tiles share one barrier sequence.
 // ======================================================================================================
+template <int G_>
 struct Smem36 {
-  static constexpr int D = 2, K = 36, NS = 16, NC = 9, G = 4, ES = NS + 1, NROW = 24, STRIDE = NC + 1;
+  static constexpr int D = 2, K = 36, NS = 16, NC = 9, G = G_, ES = NS + 1, NROW = 24, STRIDE = NC + 1;
   struct PerTile {
     int64_t Q[5][4];                                    // M, Kd, N, in_rows, in_cols  x  level subset
     int64_t TAB[2 * D * STRIDE];                        // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
@@ -382,6 +385,12 @@ struct Smem36 {
   RecBuf rec[2][G];
   SigInfo sig[2][K];
   int32_t meta[2];                                      // (kind | kind_prev << 1) of the group's tiles, 2 bits each
+  // fused chain DP only
+  alignas(16) int64_t f[2][K];                          // f_{l-1}, f_l
+  alignas(8) uint64_t full[2], freeb[2];                // mbarriers: EV buffer filled / consumed by the DP warp
+  int32_t dpmeta[2];                                    // meta of the group in EV[eb], handed over with full[eb]
+  uint8_t repcol[2][16];                                // per consumer kind: one representative column per input-state class
+  uint8_t repof[2][K];                                  //                    class of every column
 };
 
 __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
@@ -389,63 +398,258 @@ __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, u
                : "memory");
 }
 
-__global__ void __launch_bounds__(256, 3)
+// Work of one team (CTA): groups of up to G consecutive tiles.
+//   FUSE = false: groups blockIdx.x, blockIdx.x + gridDim.x, ... of the flat tile list (a group may straddle chains)
+//   FUSE = true : whole chains blockIdx.x, blockIdx.x + gridDim.x, ...; every chain starts a new group
+template <bool FUSE>
+struct GroupSched {
+  int tile0, l0, nt, p;      // first tile, its layer index, tiles in the group, chain (FUSE only)
+  bool valid;
+  int ntiles, L, Bp, step, l_step;
+  __device__ __forceinline__ void init(int ntiles_, int L_, int G) {
+    ntiles = ntiles_; L = L_; Bp = ntiles_ / L_; step = gridDim.x;
+    if (FUSE) {
+      p = blockIdx.x; l0 = 0; tile0 = p * L; valid = p < Bp; nt = L < G ? L : G;
+    } else {
+      p = 0; tile0 = blockIdx.x * G; valid = tile0 < ntiles;
+      l0 = (int)(((int64_t)blockIdx.x * G) % L);
+      l_step = (int)(((int64_t)gridDim.x * G) % L);
+      nt = ntiles - tile0 < G ? ntiles - tile0 : G;
+    }
+  }
+  __device__ __forceinline__ void advance(int G) {
+    if (FUSE) {
+      l0 += G;
+      if (l0 >= L) { l0 = 0; p += step; valid = p < Bp; }
+      tile0 = p * L + l0;
+      nt = L - l0 < G ? L - l0 : G;
+    } else {
+      tile0 += step * G;
+      valid = tile0 < ntiles;
+      l0 += l_step;
+      if (l0 >= L) l0 -= L;
+      nt = ntiles - tile0 < G ? ntiles - tile0 : G;
+    }
+  }
+};
+
+// block row of the tile that holds the row of producer signature i (class = {0,1,2,3,2,2} over the level-0 digit)
+__host__ __device__ constexpr int block_row_of(int i) { return (i / 6 < 4 ? i / 6 : 2) * 6 + i % 6; }
+
+// One chain-DP step on a tile held as 24 block rows in shared memory (R9), by one warp:
+//   fn[j] = min_i f[i] + EV[block_row_of(i)][j], smallest i on ties; bpl[j] = that i.
+// Columns whose consumer signatures share the input state vector b(j) differ only by a constant,
+//   EV[r][j] - EV[r][j'] = VP[j] - VP[j']  for every row r,
+// so they share the argmin and their minima differ by that constant: the recurrence runs on one representative
+// column per class (<= 16 of them), lane = (h, q): rows i = 18 h .. 18 h + 17 of representative q in ascending
+// order, the upper half merged into the lower with a strict '<' (smallest index wins), and the other columns
+// follow as fn[j] = fn[rep] + EV[0][j] - EV[0][rep].  Block rows: i for i < 24, i - 12 for 24..29, i - 18 for 30..35.
+__device__ __forceinline__ void dp36_step_blockrows(const int64_t* __restrict__ ev, const int64_t* __restrict__ f,
+                                                    int64_t* __restrict__ fn, uint8_t* __restrict__ bpl,
+                                                    const uint8_t* __restrict__ repcol, const uint8_t* __restrict__ repof,
+                                                    int lane) {
+  constexpr int K = 36;
+  const int q = lane & 15, h = lane >> 4;
+  const int col = repcol[q];                               // unused lanes (q >= number of classes) repeat column 0
+  const int64_t* fh = f + 18 * h;
+  const int64_t* e0 = ev + (18 * h) * K + col;             // r = 0..5
+  const int64_t* e1 = ev + (h ? 6 : 0) * K + col;          // r = 6..11:  h = 1 -> block rows 12..17
+  const int64_t* e2 = ev + col;                            // r = 12..17: h = 1 -> block rows 12..17
+  int64_t best = INT64_MAX;
+  int a = 0;
+#pragma unroll
+  for (int part = 0; part < 3; ++part) {
+    int64_t tv[6], fv[6];
+    const int64_t* e = part == 0 ? e0 : (part == 1 ? e1 : e2);
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {                          // loads first: six rows in flight
+      tv[r] = e[(6 * part + r) * K];
+      fv[r] = fh[6 * part + r];
+    }
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {
+      const int64_t v = fv[r] + tv[r];
+      if (v < best) { best = v; a = 6 * part + r; }
+    }
+  }
+  a += 18 * h;
+  {
+    const int64_t o = __shfl_down_sync(0xffffffffu, best, 16);
+    const int oa = __shfl_down_sync(0xffffffffu, a, 16);
+    if (o < best) { best = o; a = oa; }
+  }
+  // every column from its representative (lanes 0..15 hold them)
+#pragma unroll
+  for (int j0 = 0; j0 < 64; j0 += 32) {
+    const int j = j0 + lane;
+    const int rq = repof[j < K ? j : 0];
+    const int64_t rb = __shfl_sync(0xffffffffu, best, rq);
+    const int ra = __shfl_sync(0xffffffffu, a, rq);
+    if (j < K) {
+      fn[j] = rb + ev[j] - ev[repcol[rq]];
+      bpl[j] = (uint8_t)ra;
+    }
+  }
+}
+
+// NT builder threads, G tiles per group.  FUSE: one extra warp runs the chain DP (R9) on every tile
+// straight from shared memory while the tile is being stored, so the optimum costs no table read at all.
+template <int NT, int G, bool FUSE>
+__global__ void __launch_bounds__(FUSE ? NT + 32 : NT, FUSE ? 5 : 768 / NT)
 build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
-                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
-  using SM = Smem36;
-  constexpr int D = 2, K = SM::K, NS = SM::NS, NC = SM::NC, NT = 256, G = SM::G, ES = SM::ES, NROW = SM::NROW;
+                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
+                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob) {
+  using SM = Smem36<G>;
+  constexpr int D = 2, K = SM::K, NS = SM::NS, NC = SM::NC, ES = SM::ES, NROW = SM::NROW;
   constexpr int STRIDE = SM::STRIDE;
-  constexpr int ISSUER = NT - 1;                           // idle in step 4 (252 threads fill EV)
-  static_assert(G * D * NC <= 96 && 192 + G * NC <= NT && G * 5 * (1 << D) <= NT && G * K <= NT, "role layout");
+  constexpr int NR = NS * NS / NT;                         // R entries per thread
+  constexpr int RS = NT / K, EVN = (NROW + RS - 1) / RS;   // EV: row stride between a thread's rows, rows per thread
+  constexpr int ISSUER = NT - 1;                           // idle in step 4 (RS * K < NT threads fill EV)
+  constexpr int RA = G * D * NC;                           // threads of step-2 roles A and B; role C has G * NC
+  static_assert(NS * NS % NT == 0 && RS * K < NT, "thread layout");
+  static_assert(2 * RA + G * NC <= NT && G * 5 * (1 << D) <= NT && G * K <= NT && 5 * G <= NT, "role layout");
   extern __shared__ __align__(128) unsigned char smem36_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem36_raw);
+  // FUSE: back-pointers [L][K] of the chain in flight live in a per-CTA slice of the workspace (L2-resident)
+  uint8_t* bp = FUSE ? bp_glob + (size_t)blockIdx.x * L * K : nullptr;
   const int tid = threadIdx.x;
 
-  fill_sig_table<D>(sm.sig, mp, tid, NT);
-  for (int x = tid; x < G * ES * ES; x += NT) sm.t[x / (ES * ES)].E[x % (ES * ES)] = 0;
-  for (int x = tid; x < G * 2 * D; x += NT) sm.t[x / (2 * D)].TAB[(x % (2 * D)) * STRIDE + NC] = 0;
+  if (tid < NT) {
+    fill_sig_table<D>(sm.sig, mp, tid, NT);
+    for (int x = tid; x < G * ES * ES; x += NT) sm.t[x / (ES * ES)].E[x % (ES * ES)] = 0;
+    for (int x = tid; x < G * 2 * D; x += NT) sm.t[x / (2 * D)].TAB[(x % (2 * D)) * STRIDE + NC] = 0;
+  }
+  if (FUSE && tid == 0) {
+    for (int b = 0; b < 2; ++b) { mbar_init(&sm.full[b], 1); mbar_init(&sm.freeb[b], 1); }
+    mbar_fence_init();
+  }
   __syncthreads();
+  auto bsync = [&]() {                                      // barrier over the NT builder threads
+    if (FUSE) asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); else __syncthreads();
+  };
+
+  GroupSched<FUSE> sc;
+  sc.init(ntiles, L, G);
+
+  if (FUSE && tid >= NT) {
+    // =================== chain DP warp ===================
+    const int lane = tid & 31;
+    if (lane < 2) {                                        // classes of equal input state vector per consumer kind
+      const int kind = lane;
+      int n = 0;
+      for (int q = 0; q < 16; ++q) sm.repcol[kind][q] = 0;
+      for (int j = 0; j < K; ++j) {
+        int q = 0;
+        while (q < n && sm.sig[kind][sm.repcol[kind][q]].b_idx != sm.sig[kind][j].b_idx) ++q;
+        if (q == n) sm.repcol[kind][n++] = (uint8_t)j;
+        sm.repof[kind][j] = (uint8_t)q;
+      }
+    }
+    __syncwarp();
+    int cur = 0;
+    for (int it = 0; sc.valid; ++it, sc.advance(G)) {
+      const int eb = it & 1;
+      mbar_wait(&sm.full[eb], (it >> 1) & 1);
+      const int meta = sm.dpmeta[eb];
+      for (int t = 0; t < sc.nt; ++t) {
+        const int l = sc.l0 + t;
+        const int kind = (meta >> (2 * t)) & 1;
+        const int64_t* ev = sm.EV[eb][t];
+        int64_t* fn = sm.f[cur ^ 1];
+        if (l == 0) {                                      // f_0[j] = T[0][0][j]
+          for (int j = lane; j < K; j += 32) fn[j] = ev[j];
+        } else {
+          dp36_step_blockrows(ev, sm.f[cur], fn, bp + (size_t)l * K, sm.repcol[kind], sm.repof[kind], lane);
+        }
+        cur ^= 1;
+        __syncwarp();
+        if (l == L - 1) {                                  // smallest argmin of f_{L-1}, then backtrack
+          const int64_t* f = sm.f[cur];
+          int64_t bv = f[lane];
+          int bi = lane;
+          if (lane < K - 32) {
+            const int64_t v = f[32 + lane];
+            if (v < bv) { bv = v; bi = 32 + lane; }
+          }
+#pragma unroll
+          for (int off = 16; off > 0; off >>= 1) {
+            const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+            if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+          }
+          // the chain's back-pointers were written by this warp; pull them into L1 so that the dependent walk hits
+          __syncwarp();
+          {
+            int warm = 0;
+            for (int o = 16 * lane; o < L * K; o += 16 * 32) {
+              int4 x;
+              asm volatile("ld.global.ca.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(x.x), "=r"(x.y), "=r"(x.z), "=r"(x.w) : "l"(bp + o));
+              warm ^= x.x;
+            }
+            if (warm == 0x7fffffff) bi ^= 0;               // keep the loads
+          }
+          __syncwarp();
+          if (lane == 0) {
+            int32_t* sp = strategy + (size_t)sc.p * L;
+            opt_cost[sc.p] = bv;
+            int sidx = bi;
+            sp[L - 1] = sidx;
+            for (int ll = L - 1; ll >= 1; --ll) {
+              unsigned v;
+              asm volatile("ld.global.ca.u8 %0, [%1];" : "=r"(v) : "l"(bp + (size_t)ll * K + sidx));
+              sidx = (int)v;
+              sp[ll - 1] = sidx;
+            }
+          }
+          __syncwarp();
+        }
+      }
+      if (lane == 0) mbar_arrive(&sm.freeb[eb]);
+    }
+    return;
+  }
 
   // ---- tile-invariant roles of this thread ---------------------------------------------------------------
-  // step 3: thread (a, b) sums the <= 6 table entries of R[a][b]
-  int slot[3 * D];
-  r_slots<D>(tid / NS, tid % NS, slot);
-  const int e_own = (tid / NS) * ES + tid % NS;
-  // step 4: thread (r0, j) fills EV rows r0, r0+7, r0+14, r0+21 of column j; indices for GEMM -> GEMM edges
-  const int ev_j = tid % K, ev_r0 = tid / K;               // ev_r0 = 7 for the last four threads: no rows
-  int ev_idx[4];
+  // step 3: thread sums the <= 6 table entries of R[a][b] for NR state pairs (a, b) = tid + k * NT
+  int slot[NR][3 * D];
+  int e_own[NR];
+#pragma unroll
+  for (int k = 0; k < NR; ++k) {
+    const int e = tid + k * NT;
+    r_slots<D>(e / NS, e % NS, slot[k]);
+    e_own[k] = (e / NS) * ES + e % NS;
+  }
+  // step 4: thread (r0, j) fills EV rows r0, r0 + RS, ... of column j; indices for GEMM -> GEMM edges
+  const int ev_j = tid % K, ev_r0 = tid / K;               // ev_r0 >= RS: no rows
+  int ev_idx[EVN];
   {
     const int b = sm.sig[0][ev_j].b_idx, db = sm.sig[0][ev_j].db_idx;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int r = ev_r0 + 7 * k;
-      const int a = sm.sig[0][(r < NROW ? (r / 6) * 6 + r % 6 : 0)].a_idx;      // class representative i0 = r / 6
+    for (int k = 0; k < EVN; ++k) {
+      const int r = ev_r0 + RS * k;
+      const int a = sm.sig[0][r < NROW ? r : 0].a_idx;      // block row r = class representative i0 = r / 6, i1 = r % 6
       ev_idx[k] = (a * ES + b) | (db * ES + dual_vec<D>(a)) << 16;
     }
   }
-  // step 1 role: (tile in group, extent, level subset); step 2 roles: A [0,96) B [96,192) C [192,..)
+  // step 1 role: (tile in group, extent, level subset); step 2 roles: A [0,RA) B [RA,2RA) C [2RA,..)
   const int q_t = tid / (5 << D), q_x = (tid % (5 << D)) >> D, q_m = tid & ((1 << D) - 1);
-  const int role_base = tid < 96 ? 0 : (tid < 192 ? 96 : 192);
+  const int role_base = tid < RA ? 0 : (tid < 2 * RA ? RA : 2 * RA);
   const int role_i = tid - role_base;
-  const int role_t = role_base == 192 ? role_i / NC : role_i / (D * NC);      // tile in group
+  const int role_t = role_base == 2 * RA ? role_i / NC : role_i / (D * NC);   // tile in group
   const int role_d = (role_i % (D * NC)) / NC;                                // level (roles A, B)
   const int role_cfg = role_i % NC;
   int role_m0 = 0, role_m1 = 0;
   cfg_masks<D>(role_cfg, role_m0, role_m1);
   const int vp_t = tid / K, vp_j = tid % K;                // step 3: VP role (tid < G * K)
   const int64_t cap_layer = mp.mem_cap / L;
-  const int ngroups = (ntiles + G - 1) / G;
 
-  int grp = blockIdx.x;
-  if (grp >= ngroups) return;
-  int l0 = (int)(((int64_t)grp * G) % L);                  // layer index of the group's first tile
-  const int l_step = (int)(((int64_t)gridDim.x * G) % L);
+  if (!sc.valid) return;
   int buf = 0;
   // records: thread 5*t + part stages 16-byte part (or the previous kind) of tile t of the group
-  auto stage_group = [&](int b, int g, int lfirst) {
+  auto stage_group = [&](int b, int tile_first, int lfirst) {
     if (tid < 5 * G) {
       const int t = tid / 5, part = tid % 5;
-      int tile = g * G + t;
+      int tile = tile_first + t;
       if (tile >= ntiles) tile = ntiles - 1;                // ragged tail: restage a valid record, never used
       int l = lfirst + t;
       while (l >= L) l -= L;
@@ -461,18 +665,15 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
     for (int t = 0; t < G; ++t) m |= (sm.rec[b][t].kind | sm.rec[b][t].kind_prev << 1) << (2 * t);
     sm.meta[b] = m;
   };
-  stage_group(0, grp, l0);
+  stage_group(0, sc.tile0, sc.l0);
   cp_async_wait_all();
-  __syncthreads();
+  bsync();
   if (tid == 0) pack_meta(0);
 
-  for (int it = 0; grp < ngroups; ++it) {
-    const int grp_n = grp + gridDim.x;
-    int l0_n = l0 + l_step;
-    if (l0_n >= L) l0_n -= L;
-    stage_group(buf ^ 1, grp_n < ngroups ? grp_n : grp, grp_n < ngroups ? l0_n : l0);
-    const int tile0 = grp * G;
-    const int nt = ntiles - tile0 < G ? ntiles - tile0 : G;   // tiles of this group that exist
+  for (int it = 0; sc.valid; ++it) {
+    const int tile0 = sc.tile0, nt = sc.nt, l0 = sc.l0;
+    sc.advance(G);                                            // sc now describes the next group
+    stage_group(buf ^ 1, sc.valid ? sc.tile0 : tile0, sc.valid ? sc.l0 : l0);
     int first = 0;                                            // bit t: tile t of the group is a chain's layer 0
     {
       int l = l0;
@@ -487,13 +688,13 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
     // ---- 1. Q[x][m]: x = M, Kd, N, in_rows, in_cols (the record's first five int64) ---------------------
     if (tid < G * (5 << D) && q_t < nt)
       sm.t[q_t].Q[q_x][q_m] = cdiv_magic(sm.rec[buf][q_t].X[q_x], (uint32_t)mp.sub[q_m], mp.magic_sub[q_m]);
-    __syncthreads();
+    bsync();
 
     // ---- 2. tables per level and split configuration -------------------------------------------------------
     if (role_t < nt) {
-      SM::PerTile& pt = sm.t[role_t];
+      typename SM::PerTile& pt = sm.t[role_t];
       const RecBuf& rec = sm.rec[buf][role_t];
-      if (role_base == 0 && role_i < G * D * NC) {
+      if (role_base == 0) {
         if (!(first >> role_t & 1)) {                        // input tensor: Table 2 rows 2 and 3
           const int d = role_d;
           const int64_t n = pt.Q[3][role_m0] * pt.Q[4][role_m1] * (int64_t)rec.eb;
@@ -506,7 +707,7 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
           pt.TAB[d * STRIDE + role_cfg] = cg;
           pt.TAB[(D + d) * STRIDE + role_cfg] = ca;
         }
-      } else if (role_base == 96 && role_i < G * D * NC) {
+      } else if (role_base == RA) {
         if (rec.kind == AUTODDL_GEMM) {                      // weight gradient: AllReduce row
           const int d = role_d;
           const int64_t n = pt.Q[1][role_m0] * pt.Q[2][role_m1] * (int64_t)rec.wgb;
@@ -514,16 +715,16 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
           pt.WAR[d][role_cfg] =
               p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
         }
-      } else if (role_base == 192 && role_i < G * NC) {
+      } else if (role_i < G * NC) {
         pt.locW[role_cfg] = pt.Q[1][role_m0] * pt.Q[2][role_m1];
         pt.locO[role_cfg] = pt.Q[0][role_m0] * pt.Q[2][role_m1];
       }
     }
-    __syncthreads();
+    bsync();
 
     // ---- 3. VP[j] (node cost + penalty) and R[a][b] (zero for a chain's first layer: no producer) -----------------
     if (tid < G * K && vp_t < nt) {
-      SM::PerTile& pt = sm.t[vp_t];
+      typename SM::PerTile& pt = sm.t[vp_t];
       const RecBuf& rec = sm.rec[buf][vp_t];
       const SigInfo si = sm.sig[rec.kind][vp_j];
       int64_t v = 0, mem = 0;
@@ -546,19 +747,23 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
     for (int t = 0; t < G; ++t) {
       if (t < nt) {
         const int64_t* tab = sm.t[t].TAB;
-        int64_t c = 0;
-        if (!(first >> t & 1)) {
 #pragma unroll
-          for (int k = 0; k < 3 * D; ++k) c += tab[slot[k]];
+        for (int q = 0; q < NR; ++q) {
+          int64_t c = 0;
+          if (!(first >> t & 1)) {
+#pragma unroll
+            for (int k = 0; k < 3 * D; ++k) c += tab[slot[q][k]];
+          }
+          sm.t[t].E[e_own[q]] = c;
         }
-        sm.t[t].E[e_own] = c;
       }
     }
-    __syncthreads();
+    if (FUSE && tid == ISSUER && it >= 2) mbar_wait(&sm.freeb[eb], ((it >> 1) - 1) & 1);   // the DP warp is done with EV[eb]
+    bsync();
 
     // ---- 4. EV[r][j] = VP[j] + R[a(r)][b(j)] + R[dual b(j)][dual a(r)]: the 24 block rows of every tile ---------------
     const int meta = sm.meta[buf];
-    if (ev_r0 < 7) {
+    if (ev_r0 < RS) {
       if (meta == 0) {                                       // every edge of the group is GEMM -> GEMM: hoisted indices
 #pragma unroll
         for (int t = 0; t < G; ++t) {
@@ -567,8 +772,8 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
             const int64_t vp = sm.t[t].VP[ev_j];
             int64_t* ev = &sm.EV[eb][t][ev_j];
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-              if (ev_r0 + 7 * k < NROW) ev[(ev_r0 + 7 * k) * K] = vp + E[ev_idx[k] & 0xffff] + E[ev_idx[k] >> 16];
+            for (int k = 0; k < EVN; ++k)
+              if (ev_r0 + RS * k < NROW) ev[(ev_r0 + RS * k) * K] = vp + E[ev_idx[k] & 0xffff] + E[ev_idx[k] >> 16];
           }
         }
       } else {
@@ -578,7 +783,7 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
           const int64_t vp = sm.t[t].VP[ev_j];
           int b = sm.sig[kind][ev_j].b_idx, db = sm.sig[kind][ev_j].db_idx;
           if (b < 0) b = db = NS;                            // invalid consumer signature: zero column
-          for (int r = ev_r0; r < NROW; r += 7) {
+          for (int r = ev_r0; r < NROW; r += RS) {
             const int a = sm.sig[kind_prev][r].a_idx;        // class representative: i0 = r / 6 in 0..3
             const int da = a < NS ? dual_vec<D>(a) : NS;      // invalid producer signature: zero row
             sm.EV[eb][t][r * K + ev_j] = vp + E[a * ES + b] + E[db * ES + da];
@@ -586,12 +791,16 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
         }
       }
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // EV written by the generic proxy, read by TMA
+    if (T) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // EV written by the generic proxy, read by TMA
     if (tid < 5 * G) cp_async_wait_all();                    // the next group's records have landed; the barrier publishes them
-    __syncthreads();
+    bsync();
 
     // ---- 5. six 1,728-byte bulk stores per tile; the copies run while the CTA prepares the next group -----------------
-    if (tid == ISSUER) {
+    if (FUSE && tid == 0) {
+      sm.dpmeta[eb] = meta;
+      mbar_arrive(&sm.full[eb]);
+    }
+    if (T && tid == ISSUER) {
       for (int t = 0; t < nt; ++t) {
         int64_t* out = T + (size_t)(tile0 + t) * K * K;
         const int64_t* src = sm.EV[eb][t];
@@ -605,11 +814,9 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
       asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the other EV buffer is free again
     }
     if (tid == 0) pack_meta(buf ^ 1);
-    grp = grp_n;
-    l0 = l0_n;
     buf ^= 1;
   }
-  if (tid == ISSUER) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  if (T && tid == ISSUER) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 template <int D>
@@ -629,16 +836,31 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   return AUTODDL_OK;
 }
 
+constexpr int kNT = 256, kG = 4;                  // tables only: 3 CTAs of 256 threads per SM, 4 tiles per group
+constexpr int kFuseNT = 128, kFuseG = 2;           // fused with the chain DP: 6 CTAs of 128 + 32 threads per SM
+constexpr int kFusePerSM = 5;
+
 int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
-  const size_t smem = sizeof(Smem36);
-  ADL_CUDA_CHECK(cudaFuncSetAttribute(build_tables36_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (getenv("AUTODDL_BT_VARIANT")) {
+    auto kern = build_tables36_kernel<128, 2, false>;
+    const size_t smem = sizeof(Smem36<2>);
+    const int per = atoi(getenv("AUTODDL_BT_VARIANT"));
+    const int ngroups = (ntiles + 1) / 2;
+    const int grid = ngroups < 148 * per ? ngroups : 148 * per;
+    kern<<<grid, 128, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr);
+    count_launch();
+    return AUTODDL_OK;
+  }
+  auto kern = build_tables36_kernel<kNT, kG, false>;
+  const size_t smem = sizeof(Smem36<kG>);
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int dev = 0, sms = 148;
   ADL_CUDA_CHECK(cudaGetDevice(&dev));
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const int ngroups = (ntiles + Smem36::G - 1) / Smem36::G;
+  const int ngroups = (ntiles + kG - 1) / kG;
   const int grid = ngroups < sms * 3 ? ngroups : sms * 3;             // persistent, grid-stride over tile groups
-  build_tables36_kernel<<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
+  kern<<<grid, kNT, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -657,6 +879,40 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
   }
   set_error("ndim must be 1, 2 or 3");
   return AUTODDL_EINVAL;
+}
+
+// Fused (a1) + (a2) for K = 36: tables (d_T may be NULL: no table is written) and the chain DP in one kernel.
+// d_bp: fused_bp_bytes(L) of workspace for the back-pointers of the chains in flight (one slice per CTA).
+bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim == 2 && L >= 1; }
+
+static int fused_grid_limit() {
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
+  return sms * kFusePerSM;
+}
+
+size_t fused_bp_bytes(int32_t L) {
+  static const int limit = fused_grid_limit();             // host-only query, cached
+  return ((size_t)limit * L * 36 + 255) / 256 * 256 + 256;
+}
+
+int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
+                          int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
+                          cudaStream_t st) {
+  const int64_t nt = (int64_t)Bp * L;
+  if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  if (!fused_build_dp_supported(mp, L)) { set_error("fused build+DP needs a 2-level mesh"); return AUTODDL_EINVAL; }
+  if (d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
+  auto kern = build_tables36_kernel<kFuseNT, kFuseG, true>;
+  const size_t smem = sizeof(Smem36<kFuseG>);
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int limit = fused_grid_limit();
+  const int grid = Bp < limit ? Bp : limit;                            // persistent, grid-stride over chains
+  kern<<<grid, kFuseNT + 32, smem, st>>>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy,
+                                         (uint8_t*)(((uintptr_t)d_bp + 15) & ~(uintptr_t)15));
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
 }
 
 }  // namespace autoddl

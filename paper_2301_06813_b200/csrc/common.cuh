@@ -49,6 +49,11 @@ inline int num_sigs(int ndim) { return ndim == 1 ? 6 : ndim == 2 ? 36 : 216; }
 // ---- kernel launchers (defined in the .cu files) ----------------------------------------------------
 int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp,
                         int64_t* d_T, int64_t* d_node, uint8_t* d_mask, cudaStream_t st);
+bool fused_build_dp_supported(const MeshParams& mp, int32_t L);
+size_t fused_bp_bytes(int32_t L);
+int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
+                          int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
+                          cudaStream_t st);
 int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp,
                     int64_t* d_opt_cost, int32_t* d_strategy, cudaStream_t st);
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,

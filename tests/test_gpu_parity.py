@@ -182,6 +182,87 @@ def test_fused_build_paths_and_search_host(adl):
     assert int(out["opt_cost"][0]) == 294_284_438_784
 
 
+def _search_all(adl, w, init, **kw):
+    """the one-call path (autoddl_search): on 2-level meshes tables and chain DP run as one fused kernel"""
+    o = adl.search(adl.layers_to_device(w.layers), w.mesh, w.net, init=torch.from_numpy(init).cuda(), max_sweeps=w.max_sweeps,
+                   want_node_mask=True, **kw)
+    torch.cuda.synchronize()
+    return [o[k].cpu().numpy() for k in ("T", "node", "mask", "opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps")]
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 5])
+def test_search_one_call_configs(adl, k):
+    """configs 1-3 (K = 36: fused build + DP kernel, GEMM and ATTN edges) and 5 (K = 216: three kernels)"""
+    w = cf.CONFIGS[k]()
+    init = w.cd_init()[:, :8] if k == 5 else w.cd_init()
+    if k == 5:
+        T, node, mask = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+        dc, ds = ref.chain_dp(T)
+        cc, cs, sw = ref.coord_descent(T, init, w.max_sweeps)
+        want = (T, node, mask, dc, ds, cc, cs, sw)
+    else:
+        want = _oracle_all(w, init)
+    _assert_same(_search_all(adl, w, init), want)
+
+
+@pytest.mark.parametrize("Bp,L", [(1, 1), (3, 1), (5, 2), (7, 3), (5, 7), (1500, 3), (900, 5), (33, 64), (2, 300)])
+def test_search_fused_shapes(adl, Bp, L):
+    """fused kernel over ragged groups (L not a multiple of the group size), more chains than resident CTAs,
+    single-layer chains, and a chain longer than any shared-memory back-pointer table would allow"""
+    w = cf.config4_batched(Bp=Bp, L=L, seed=5)
+    init = w.cd_init()
+    nsamp = min(Bp, 40)
+    idx = np.unique(np.concatenate([np.arange(min(Bp, 6)), np.random.default_rng(1).integers(0, Bp, nsamp), [Bp - 1]]))
+    got = _search_all(adl, w, init)
+    ws = cf.Workload(w.name, np.ascontiguousarray(w.layers[idx]), w.mesh, w.net, S=w.S, seed=w.seed)
+    want = _oracle_all(ws, np.ascontiguousarray(init[idx]))
+    _assert_same([g[idx] for g in got], want)
+    # all chains: the fused DP equals the separate DP kernel on the same tables
+    d_layers = adl.layers_to_device(w.layers)
+    T, _, _ = adl.build_tables(d_layers, w.mesh, w.net)
+    dc, ds = adl.chain_dp(T, w.mesh)
+    assert np.array_equal(got[3], dc.cpu().numpy()) and np.array_equal(got[4], ds.cpu().numpy())
+    assert np.array_equal(got[0], T.cpu().numpy())
+
+
+def test_search_mixed_kinds_and_unit_level(adl):
+    """fused kernel with ATTN edges, ragged dims, split limits, a memory cap and a mesh level of size 1"""
+    rng = np.random.default_rng(11)
+    for sizes, links in [((3, 5), (1, 0)), ((1, 7), (1, 0)), ((8, 1), (1, 0))]:
+        Bp, L = 7, 9
+        layers = np.zeros((Bp, L), dtype=cf.LAYER_DTYPE)
+        for p in range(Bp):
+            for l in range(L):
+                M, Kd, N = (int(x) for x in rng.integers(1, 3000, 3))
+                if (l + p) % 3 == 1:
+                    layers[p, l] = cf.attn(M, N, int(rng.integers(1, 3000)), 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)))
+                else:
+                    layers[p, l] = cf.gemm(M, Kd, N, 2, 4, 18, in_rows=int(rng.integers(1, 5000)), in_cols=int(rng.integers(1, 5000)),
+                                           max_rows=int(rng.integers(1, 64)), max_cols=int(rng.integers(1, 64)))
+        w = cf.Workload("mixed", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), 150_000 * L), S=3, seed=2)
+        init = w.cd_init()
+        _assert_same(_search_all(adl, w, init), _oracle_all(w, init))
+
+
+def test_search_without_tables_and_full_size(adl):
+    """config 4 at full size through the fused kernel (the launch configuration bench.py times): DP results equal the
+    separate kernels' on every chain and the oracle's on a sample; with no table requested nothing is materialised"""
+    w = cf.config4_batched()
+    d_layers = adl.layers_to_device(w.layers)
+    o = adl.search(d_layers, w.mesh, w.net, want_tables=True)
+    dc2, ds2 = adl.chain_dp(None, w.mesh, net=w.net, d_layers=d_layers)       # fused, no table written
+    T, _, _ = adl.build_tables(d_layers, w.mesh, w.net)
+    dc, ds = adl.chain_dp(T, w.mesh)
+    torch.cuda.synchronize()
+    assert torch.equal(o["T"], T) and torch.equal(o["opt_cost"], dc) and torch.equal(o["strategy"], ds)
+    assert torch.equal(dc2, dc) and torch.equal(ds2, ds)
+    mesh, net = ref.mesh_of(w), ref.net_of(w)
+    for p in [0, 1, 739, 740, 2047, 4095]:
+        oT, _, _ = ref.build_tables(w.layers[p:p + 1], mesh, net)
+        odc, ods = ref.chain_dp(oT)
+        assert int(o["opt_cost"][p]) == int(odc[0]) and np.array_equal(o["strategy"][p].cpu().numpy(), ods[0])
+
+
 def test_ragged_dims_and_mesh_with_unit_level(adl):
     """non-divisible tensor dims (ceil shards), a level of size 1 and a 3-level odd mesh"""
     rng = np.random.default_rng(9)
