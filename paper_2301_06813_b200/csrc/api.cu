@@ -1,5 +1,6 @@
 // C-ABI entry points (include/autoddl.h): argument validation, workspace carving, launches.
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -192,7 +193,8 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
                          int64_t* d_opt_cost, int32_t* d_strategy, const int32_t* d_init, int32_t S, int32_t max_sweeps,
                          int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, cudaStream_t st) {
   const bool do_cd = d_init != nullptr;
-  const bool fused = fused_build_dp_supported(mp, L);
+  static const bool no_fuse = getenv("AUTODDL_NO_FUSE") != nullptr;   // debugging switch: three separate kernels
+  const bool fused = !no_fuse && fused_build_dp_supported(mp, L);
   const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
   size_t used = 0;
   int rc;
