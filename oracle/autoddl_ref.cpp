@@ -321,3 +321,80 @@ extern "C" int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L
   }
   return 0;
 }
+
+// ---- R19-R22: Metropolis-Hastings.  P(S) ~ exp(-beta Cost(S)), beta = 1 / tau; a proposal
+// changes the signature of one layer; it is accepted with probability min(1, P(S_new) / P(S_old)).
+extern "C" uint64_t autoddl_ref_rng(uint64_t seed, uint64_t n) {
+  uint64_t z = seed + n * 0x9E3779B97F4A7C15ull;                    // splitmix64: state after n increments
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// -ln(x / 2^32) in Q16, x in [1, 2^32].  log2(x) = n + frac: n = index of the top bit; the 16 fraction bits come
+// from squaring the mantissa m in [1, 2) sixteen times (m^2 >= 2 -> bit 1, halve), every product truncated to
+// Q62.  Then -ln = (32 - log2 x) * ln 2 with ln 2 = 744261117 / 2^30 (truncated).
+extern "C" int64_t autoddl_ref_neglog_q16(uint64_t x) {
+  if (x < 1 || x > (1ull << 32)) return -1;
+  int n = 0;
+  while ((x >> (n + 1)) != 0) ++n;
+  uint64_t m = x << (62 - n);                                        // Q62 in [2^62, 2^63)
+  uint64_t frac = 0;
+  for (int k = 0; k < 16; ++k) {
+    const unsigned __int128 sq = (unsigned __int128)m * m;           // Q124
+    m = (uint64_t)(sq >> 62);                                        // Q62 in [2^62, 2^64)
+    frac <<= 1;
+    if (m >= (1ull << 63)) { frac |= 1; m >>= 1; }
+  }
+  const int64_t log2_q16 = ((int64_t)n << 16) | (int64_t)frac;
+  const int64_t nlog2_q16 = ((int64_t)32 << 16) - log2_q16;          // >= 0
+  return (nlog2_q16 * 744261117ll) >> 30;
+}
+
+extern "C" int autoddl_ref_metropolis(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                                      const int32_t* init, int32_t S, int32_t nsteps, int64_t tau_ps, uint64_t seed,
+                                      int64_t* best_cost, int32_t* best_strategy, int64_t* final_cost,
+                                      int32_t* final_strategy, int32_t* accepted, int64_t* trace) {
+  if (!T || !init || !best_cost || !best_strategy || !final_cost || !final_strategy || !accepted) return -1;
+  if (Bp < 1 || L < 1 || K < 1 || S < 1 || nsteps < 0 || tau_ps < 0 || tau_ps >= ((int64_t)1 << 40)) return -1;
+  std::vector<int32_t> s(L), sbest(L);
+  for (int64_t p = 0; p < Bp; ++p) {
+    const int64_t* Tp = T + p * L * K * K;
+    for (int64_t r = 0; r < S; ++r) {
+      const uint64_t chain = (uint64_t)(p * S + r);
+      for (int l = 0; l < L; ++l) s[l] = init[(p * S + r) * L + l];
+      int64_t cur = autoddl_ref_chain_cost(Tp, L, K, s.data());
+      int64_t best = cur;
+      sbest = s;
+      int32_t nacc = 0;
+      for (int64_t t = 0; t < nsteps; ++t) {
+        const uint64_t base = ((chain << 32) + (uint64_t)t) * 4;
+        const int32_t l = (int32_t)(autoddl_ref_rng(seed, base + 1) % (uint64_t)L);
+        const int32_t c = (int32_t)(autoddl_ref_rng(seed, base + 2) % (uint64_t)K);
+        const uint64_t x = (autoddl_ref_rng(seed, base + 3) >> 32) + 1;
+        // Cost(S_new) - Cost(S_old): only the entries that touch layer l change
+        const int32_t left = (l > 0) ? s[l - 1] : 0;
+        int64_t d = Tp[((int64_t)l * K + left) * K + c] - Tp[((int64_t)l * K + left) * K + s[l]];
+        if (l < L - 1)
+          d += Tp[((int64_t)(l + 1) * K + c) * K + s[l + 1]] - Tp[((int64_t)(l + 1) * K + s[l]) * K + s[l + 1]];
+        bool acc = d <= 0;
+        if (!acc && d < ((int64_t)1 << 45)) acc = tau_ps * autoddl_ref_neglog_q16(x) >= (d << 16);
+        if (acc) {
+          s[l] = c;
+          cur += d;
+          ++nacc;
+          if (cur < best) { best = cur; sbest = s; }
+        }
+        if (trace) trace[(p * S + r) * (int64_t)nsteps + t] = cur;
+      }
+      best_cost[p * S + r] = best;
+      final_cost[p * S + r] = cur;
+      accepted[p * S + r] = nacc;
+      for (int l = 0; l < L; ++l) {
+        best_strategy[(p * S + r) * L + l] = sbest[l];
+        final_strategy[(p * S + r) * L + l] = s[l];
+      }
+    }
+  }
+  return 0;
+}

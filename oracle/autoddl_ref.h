@@ -17,6 +17,8 @@
  *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours)
  *   chain DP optimum (PAPER.md:225 exhaustive)     pinned  (brute force over K^L)
  *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
+ *   Metropolis-Hastings         pinned  (Boltzmann stationary law on enumerable chains, greedy and
+ *                                                  hot limits, integer -ln against libm, replay of a hand-checked chain)
  */
 #ifndef AUTODDL_REF_H
 #define AUTODDL_REF_H
@@ -91,6 +93,22 @@ int autoddl_ref_brute_force(const int64_t* T, int32_t L, int32_t K, int64_t* opt
 int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
                               const int32_t* init, int32_t S, int32_t max_sweeps,
                               int64_t* cost, int32_t* strategy, int32_t* sweeps, int64_t* trace);
+
+/* ---- Metropolis-Hastings sampler (R19-R22) --------------------------------
+ * n-th output (n >= 1) of splitmix64 started at `seed`: the counter-based generator both sides implement. */
+uint64_t autoddl_ref_rng(uint64_t seed, uint64_t n);
+/* floor-style fixed point -ln(x / 2^32) * 2^16 for x in [1, 2^32], by integer shift-and-square (R21) */
+int64_t autoddl_ref_neglog_q16(uint64_t x);
+/* One chain per (problem, start), nsteps proposals each.  Step t of chain c = p * S + r draws
+ *   l = rng(4 (c 2^32 + t) + 1) mod L,  s' = rng(.. + 2) mod K,  x = (rng(.. + 3) >> 32) + 1
+ * and accepts the move s_l <- s' iff dC <= 0 or (dC < 2^45 and tau * neglog_q16(x) >= dC * 2^16), i.e. with
+ * probability min(1, exp(-dC / tau)) = min(1, P(S_new) / P(S_old)) for P(S) ~ exp(-Cost(S) / tau).
+ * Outputs per chain: smallest cost seen (first time attained) and its strategy, the final strategy and cost,
+ * the number of accepted proposals.  trace (optional) [Bp][S][nsteps] = cost after every step. */
+int autoddl_ref_metropolis(const int64_t* T, int32_t Bp, int32_t L, int32_t K,
+                           const int32_t* init, int32_t S, int32_t nsteps, int64_t tau_ps, uint64_t seed,
+                           int64_t* best_cost, int32_t* best_strategy, int64_t* final_cost, int32_t* final_strategy,
+                           int32_t* accepted, int64_t* trace);
 
 #ifdef __cplusplus
 }

@@ -70,6 +70,12 @@ def lib():
         L.autoddl_ref_brute_force.argtypes = [vp, i32, i32, vp, vp]
         L.autoddl_ref_coord_descent.restype = C.c_int
         L.autoddl_ref_coord_descent.argtypes = [vp, i32, i32, i32, vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_ref_rng.restype = C.c_uint64
+        L.autoddl_ref_rng.argtypes = [C.c_uint64, C.c_uint64]
+        L.autoddl_ref_neglog_q16.restype = i64
+        L.autoddl_ref_neglog_q16.argtypes = [C.c_uint64]
+        L.autoddl_ref_metropolis.restype = C.c_int
+        L.autoddl_ref_metropolis.argtypes = [vp, i32, i32, i32, vp, i32, i32, i64, C.c_uint64, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -208,3 +214,30 @@ def coord_descent(T: np.ndarray, init: np.ndarray, max_sweeps: int = 64, want_tr
     if want_trace:
         return cost, strat, sweeps, trace
     return cost, strat, sweeps
+
+
+# ---- Metropolis-Hastings -------------------------------------------------------------
+def rng(seed: int, n: int) -> int:
+    return int(lib().autoddl_ref_rng(seed, n))
+
+
+def neglog_q16(x: int) -> int:
+    return int(lib().autoddl_ref_neglog_q16(x))
+
+
+def metropolis(T: np.ndarray, init: np.ndarray, nsteps: int, tau_ps: int, seed: int = 0, want_trace: bool = False):
+    """-> best_cost [Bp,S], best_strategy [Bp,S,L], final_cost [Bp,S], final_strategy [Bp,S,L], accepted [Bp,S] (, trace [Bp,S,nsteps])"""
+    T = np.ascontiguousarray(T, dtype=np.int64)
+    init = np.ascontiguousarray(init, dtype=np.int32)
+    Bp, L, K, _ = T.shape
+    S = init.shape[1]
+    assert init.shape == (Bp, S, L)
+    bc = np.empty((Bp, S), np.int64); fc = np.empty((Bp, S), np.int64)
+    bs = np.empty((Bp, S, L), np.int32); fs = np.empty((Bp, S, L), np.int32)
+    acc = np.empty((Bp, S), np.int32)
+    trace = np.empty((Bp, S, nsteps), np.int64) if want_trace else None
+    rc = lib().autoddl_ref_metropolis(_p(T), Bp, L, K, _p(init), S, nsteps, tau_ps, seed, _p(bc), _p(bs), _p(fc), _p(fs), _p(acc), _p(trace))
+    assert rc == 0, rc
+    if want_trace:
+        return bc, bs, fc, fs, acc, trace
+    return bc, bs, fc, fs, acc
