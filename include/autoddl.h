@@ -10,6 +10,7 @@
  *   (a2) autoddl_chain_dp       exact optimum over all K^L strategies of a chain (the result of the
  *        paper's "exhaustive search") by min-plus dynamic programming.
  *   (a3) autoddl_coord_descent  the paper's Coordinate Descent, many starts.
+ *   (f2) autoddl_metropolis     the paper's Metropolis-Hastings sampler, many chains.
  *
  * Conventions
  *   - All costs are int64 picoseconds.  PEN = 2^50 is added to every cell whose consumer signature
@@ -99,6 +100,22 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                           const int64_t* d_T, void* d_work, size_t work_bytes,
                           const int32_t* d_init, int32_t S, int32_t max_sweeps,
                           int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, void* stream);
+
+/* Metropolis-Hastings sampler on the tables (R19-R22): P(S) ~ exp(-Cost(S) / tau_ps).
+ * One chain per (problem, start), nsteps proposals each.  Step t of chain c = p * S + r draws, with rng(n) the
+ * n-th output of splitmix64 started at `seed`,
+ *   l = rng(4 (c 2^32 + t) + 1) mod L,   s' = rng(.. + 2) mod K,   x = (rng(.. + 3) >> 32) + 1  in [1, 2^32]
+ * and accepts s_l <- s' iff dC <= 0 or (dC < 2^45 and tau_ps * neglog_q16(x) >= dC * 2^16), dC = Cost(S_new) -
+ * Cost(S_old), neglog_q16(x) = -ln(x / 2^32) in Q16 by 16 shift-and-square steps on a Q62 mantissa, ln 2 =
+ * 744261117 / 2^30 (integer only: results are bit-exact).  That is acceptance with probability
+ * min(1, P(S_new) / P(S_old)).  Outputs per chain: d_best_cost [Bp][S] the smallest cost seen (start included) and
+ * d_best_strategy [Bp][S][L] the first strategy attaining it, d_final_cost / d_final_strategy the last state,
+ * d_accepted [Bp][S] the number of accepted proposals.  0 <= tau_ps < 2^40, nsteps >= 0, K <= 256,
+ * d_init entries in [0, K). */
+int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                       const int32_t* d_init, int32_t S, int32_t nsteps, int64_t tau_ps, uint64_t seed,
+                       int64_t* d_best_cost, int32_t* d_best_strategy, int64_t* d_final_cost,
+                       int32_t* d_final_strategy, int32_t* d_accepted, void* stream);
 
 /* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36)
  * (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and

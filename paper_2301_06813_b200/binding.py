@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -58,6 +58,8 @@ def lib():
         L.autoddl_chain_dp.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, vp, vp]
         L.autoddl_coord_descent.restype = C.c_int
         L.autoddl_coord_descent.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_metropolis.restype = C.c_int
+        L.autoddl_metropolis.argtypes = [vp, i32, i32, vp, vp, i32, i32, i64, C.c_uint64, vp, vp, vp, vp, vp, vp]
         L.autoddl_search.restype = C.c_int
         L.autoddl_search.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.autoddl_search_host.restype = C.c_int
@@ -184,6 +186,22 @@ def coord_descent(T: torch.Tensor | None, init: torch.Tensor, mesh, max_sweeps: 
                                        _ptr(T), _ptr(work), work.numel() if work is not None else 0, _ptr(init), S,
                                        max_sweeps, _ptr(cost), _ptr(strat), _ptr(sweeps), _stream()))
     return cost, strat, sweeps
+
+
+def metropolis(T: torch.Tensor, init: torch.Tensor, mesh, nsteps: int, tau_ps: int, seed: int = 0, out=None):
+    """Metropolis-Hastings chains on the tables -> best_cost [Bp,S], best_strategy [Bp,S,L], final_cost [Bp,S],
+    final_strategy [Bp,S,L], accepted [Bp,S] (device tensors)"""
+    Bp, S, L = init.shape
+    dev = init.device
+    if out is None:
+        out = (torch.empty((Bp, S), dtype=torch.int64, device=dev), torch.empty((Bp, S, L), dtype=torch.int32, device=dev),
+               torch.empty((Bp, S), dtype=torch.int64, device=dev), torch.empty((Bp, S, L), dtype=torch.int32, device=dev),
+               torch.empty((Bp, S), dtype=torch.int32, device=dev))
+    bc, bs, fc, fs, acc = out
+    m = c_mesh(mesh)
+    _check(lib().autoddl_metropolis(_ptr(T), Bp, L, C.addressof(m), _ptr(init), S, nsteps, tau_ps, seed, _ptr(bc), _ptr(bs),
+                                    _ptr(fc), _ptr(fs), _ptr(acc), _stream()))
+    return out
 
 
 def search(d_layers: torch.Tensor, mesh, net, init: torch.Tensor | None = None, max_sweeps: int = 64,

@@ -302,6 +302,24 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
   return AUTODDL_OK;
 }
 
+int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_mesh* mesh, const int32_t* d_init,
+                       int32_t S, int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost,
+                       int32_t* d_best_strategy, int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted,
+                       void* stream) {
+  clear_error();
+  int rc = validate_mesh_net(mesh, nullptr, nullptr);
+  if (rc) return rc;
+  ADL_REQUIRE(Bp >= 1 && L >= 1 && S >= 1 && nsteps >= 0, "Bp, L, S must be >= 1 and nsteps >= 0");
+  ADL_REQUIRE(tau_ps >= 0 && tau_ps < ((int64_t)1 << 40), "tau_ps must lie in [0, 2^40)");
+  ADL_REQUIRE(d_T && d_init && d_best_cost && d_best_strategy && d_final_cost && d_final_strategy && d_accepted, "NULL pointer");
+  ADL_REQUIRE(((uintptr_t)d_T & 7) == 0 && ((uintptr_t)d_best_cost & 7) == 0 && ((uintptr_t)d_final_cost & 7) == 0 &&
+                  ((uintptr_t)d_init & 3) == 0 && ((uintptr_t)d_best_strategy & 3) == 0 &&
+                  ((uintptr_t)d_final_strategy & 3) == 0 && ((uintptr_t)d_accepted & 3) == 0, "misaligned pointer");
+  if ((rc = check_device())) return rc;
+  return launch_metropolis(d_T, Bp, L, num_sigs(mesh->ndim), d_init, S, nsteps, tau_ps, seed, d_best_cost, d_best_strategy,
+                           d_final_cost, d_final_strategy, d_accepted, (cudaStream_t)stream);
+}
+
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {
   clear_error();
   ADL_REQUIRE(d_src && d_dst && bytes > 0 && bytes % 16 == 0, "copy_probe: bad arguments");

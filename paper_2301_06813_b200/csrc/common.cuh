@@ -59,6 +59,9 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
                          int32_t* d_sweeps, cudaStream_t st);
+int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
+                      int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost, int32_t* d_best_strategy,
+                      int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted, cudaStream_t st);
 int launch_copy_probe(const void* src, void* dst, size_t bytes, cudaStream_t st);
 
 // ---- device helpers ------------------------------------------------------------------------------------
