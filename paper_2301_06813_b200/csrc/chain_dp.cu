@@ -367,7 +367,16 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
         return launch_dp36<3>(d_T, Bp, L, d_opt_cost, d_strategy, st);
       }
       return launch_cfg<36, 36, 3, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
-    case 216: return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+    case 216: {
+      // few long chains: one 8-CTA cluster per chain (chain_dp_cluster.cu); many chains already fill the machine
+      static const bool no_cluster = getenv("AUTODDL_DP_NO_CLUSTER") != nullptr;
+      if (!no_cluster && Bp * 8 <= 148 && chain_dp_cluster_supported(K, L)) {
+        const int rc = launch_chain_dp_cluster(d_T, Bp, L, d_opt_cost, d_strategy, st);
+        if (rc == AUTODDL_OK) return rc;
+        cudaGetLastError();                                  // launch refused: fall back to one CTA per chain
+      }
+      return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
+    }
   }
   set_error("chain_dp: K must be 6, 36 or 216");
   return AUTODDL_EINVAL;

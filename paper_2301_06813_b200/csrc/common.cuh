@@ -56,6 +56,9 @@ int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
                           cudaStream_t st);
 int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp,
                     int64_t* d_opt_cost, int32_t* d_strategy, cudaStream_t st);
+bool chain_dp_cluster_supported(int32_t K, int32_t L);
+int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* d_opt_cost, int32_t* d_strategy,
+                            cudaStream_t st);
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
                          int32_t* d_sweeps, cudaStream_t st);

@@ -263,6 +263,20 @@ def test_search_without_tables_and_full_size(adl):
         assert int(o["opt_cost"][p]) == int(odc[0]) and np.array_equal(o["strategy"][p].cpu().numpy(), ods[0])
 
 
+@pytest.mark.parametrize("Bp,L,hi", [(1, 2, 5), (3, 7, 3), (2, 33, 10**9), (5, 100, 1000), (1, 864, 50), (1, 865, 50), (19, 5, 7)])
+def test_dp_k216_cluster_and_fallback(adl, Bp, L, hi):
+    """K = 216 chain DP: one 8-CTA cluster per chain (row blocks per CTA, partial minima exchanged over distributed
+    shared memory) for few chains and L <= 864, the one-CTA kernel otherwise; many exact ties (small hi)"""
+    rng = np.random.default_rng(Bp * 1000 + L)
+    T = rng.integers(0, hi, size=(Bp, L, 216, 216)).astype(np.int64)
+    T[:, 0] = T[:, 0, :1]
+    mesh = cf.Mesh((2, 2, 2), (0, 0, 0))
+    work = torch.empty(Bp * L * 216 + 4096, dtype=torch.uint8, device="cuda")
+    dc, ds = adl.chain_dp(torch.from_numpy(T).cuda(), mesh, work=work)
+    odc, ods = ref.chain_dp(T)
+    _assert_same([dc.cpu().numpy(), ds.cpu().numpy()], (odc, ods), names=("dp_cost", "dp_strategy"))
+
+
 def test_ragged_dims_and_mesh_with_unit_level(adl):
     """non-divisible tensor dims (ceil shards), a level of size 1 and a 3-level odd mesh"""
     rng = np.random.default_rng(9)
