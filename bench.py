@@ -369,6 +369,76 @@ def run_ours(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------------
+# --configs: one JSON line per BASELINE.json config (the small ones are launch-bound: absolute microseconds)
+# ---------------------------------------------------------------------------------------------------
+def run_configs(args):
+    """GPU kernel times and single-thread oracle times on configs 1, 2, 3, 5 (config 4 is the default run).  Also times
+    the Metropolis-Hastings kernel and, on config 4, reports its proposals/s."""
+    import torch
+    from oracle import ref
+    from paper_2301_06813_b200 import binding as adl
+    adl.lib()
+    torch.cuda.set_device(0)
+
+    def gpu_us(fn, n=30):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e3
+
+    for k in args.configs:
+        w = cf.CONFIGS[k]() if k != 4 else cf.config4_batched()
+        dl = adl.layers_to_device(w.layers)
+        init_np = w.cd_init()
+        init = torch.from_numpy(init_np).cuda()
+        T, _, _ = adl.build_tables(dl, w.mesh, w.net, want_node_mask=False)
+        work = torch.empty(adl.workspace_bytes(w.Bp, w.L, w.S, w.mesh), dtype=torch.uint8, device="cuda")
+        dp = adl.chain_dp(T, w.mesh, work=work)
+        cd = adl.coord_descent(T, init, w.mesh, w.max_sweeps)
+        nsteps = 4096
+        tau = 20_000_000
+        mh = adl.metropolis(T, init, w.mesh, nsteps, tau, seed=0)
+        one = adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out={"T": T})
+        torch.cuda.synchronize()
+        sweeps = int(cd[2].sum().item())
+        g = {
+            "build_us": gpu_us(lambda: adl.build_tables(dl, w.mesh, w.net, want_node_mask=False, out=T)),
+            "dp_us": gpu_us(lambda: adl.chain_dp(T, w.mesh, work=work, out=dp)),
+            "cd_us": gpu_us(lambda: adl.coord_descent(T, init, w.mesh, w.max_sweeps, out=cd)),
+            "search_us": gpu_us(lambda: adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out=one)),
+            "mh_us": gpu_us(lambda: adl.metropolis(T, init, w.mesh, nsteps, tau, seed=0, out=mh), n=5),
+        }
+        line = {"config": k, "name": w.name, "Bp": w.Bp, "L": w.L, "K": w.K, "S": w.S, "cells": w.cells, "cd_sweeps": sweeps,
+                "gpu": g,
+                "gpu_rates": {"build_cells_per_s": w.cells / g["build_us"] * 1e6, "dp_cells_per_s": w.cells / g["dp_us"] * 1e6,
+                              "cd_sweeps_per_s": sweeps / g["cd_us"] * 1e6,
+                              "mh_proposals_per_s": w.Bp * w.S * nsteps / g["mh_us"] * 1e6},
+                "dp_optimum_ps": int(dp[0][0]), "best_cd_over_dp": float(cd[0].min(dim=1).values.double().div(dp[0].double()).mean()),
+                "best_mh_over_dp": float(mh[0].min(dim=1).values.double().div(dp[0].double()).mean()),
+                "mh": {"nsteps": nsteps, "tau_ps": tau}}
+        if k != 4:                                           # oracle, one core (config 4's oracle numbers are in the default run)
+            mesh, net = ref.mesh_of(w), ref.net_of(w)
+            t0 = time.perf_counter(); oT, _, _ = ref.build_tables(w.layers, mesh, net)
+            t1 = time.perf_counter(); ref.chain_dp(oT)
+            t2 = time.perf_counter(); _, _, osw = ref.coord_descent(oT, init_np, w.max_sweeps)
+            t3 = time.perf_counter()
+            ms = min(nsteps, 256)
+            ref.metropolis(oT, init_np, ms, tau, seed=0)
+            t4 = time.perf_counter()
+            line["oracle_1core"] = {"build_cells_per_s": w.cells / (t1 - t0), "dp_cells_per_s": w.cells / (t2 - t1),
+                                    "cd_sweeps_per_s": int(osw.sum()) / (t3 - t2),
+                                    "mh_proposals_per_s": w.Bp * w.S * ms / (t4 - t3), "cores": 1}
+        print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -376,7 +446,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--configs", type=int, nargs="+", default=None,
+                    help="per-config report (kernel microseconds, oracle rates) instead of the bench line, e.g. --configs 1 2 3 5")
     args = ap.parse_args()
+    if args.configs:
+        return run_configs(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

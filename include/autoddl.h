@@ -81,8 +81,8 @@ int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
 
 /* (a2) f_0[j] = T[0][0][j]; f_l[j] = min_i f_{l-1}[i] + T[l][i][j]; smallest index wins every tie;
  * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: the tables are computed from d_layers
- * -- on a 2-level mesh (K = 36) inside the DP kernel itself, tile by tile in shared memory, never
- * stored; otherwise they are first built into d_work.  d_work (>= autoddl_workspace_bytes) also
+ * -- on a 2-level mesh (K = 36), for >= 296 chains or when d_work cannot hold the tables, inside the DP kernel
+ * itself, tile by tile in shared memory, never stored; otherwise they are first built into d_work.  d_work (>= autoddl_workspace_bytes) also
  * holds back-pointers (fused kernel: of the chains in flight; separate kernel: when L * K > 16384).
  * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
 int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
@@ -117,8 +117,8 @@ int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_
                        int64_t* d_best_cost, int32_t* d_best_strategy, int64_t* d_final_cost,
                        int32_t* d_final_strategy, int32_t* d_accepted, void* stream);
 
-/* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36)
- * (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and
+/* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36) with at least 296
+ * chains (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and
  * consumed by the chain DP from shared memory, so the optimum costs no table read.  Other meshes run
  * the three kernels back to back.  Results are identical to the three separate calls.
  * d_T: [Bp][L][K][K] output, or NULL to keep the tables in d_work (any mesh) -- with d_init == NULL

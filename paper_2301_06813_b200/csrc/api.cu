@@ -69,6 +69,10 @@ static inline size_t bp_bytes(int64_t Bp, int64_t L, int64_t K) {
   return bp_in_workspace(L, K) ? align_up((size_t)Bp * L * K, 256) : 0;
 }
 
+// the fused build + DP kernel runs one chain per CTA: below this many chains the separate kernels (which spread the
+// tiles of a chain over all SMs) are faster
+static constexpr int32_t kFusedMinChains = 296;
+
 static int check_device() {
   int n = 0;
   cudaError_t e = cudaGetDeviceCount(&n);
@@ -136,7 +140,10 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
   if (!d_T) ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
   const int K = num_sigs(mesh->ndim);
   cudaStream_t st = (cudaStream_t)stream;
-  if (!d_T && fused_build_dp_supported(mp, L)) {            // tables never leave shared memory
+  // many chains: the fused kernel (one chain per CTA, tables never leave shared memory); few chains: the fused kernel
+  // would serialise the tiles of a chain on one CTA, so the tables are built by all SMs first when d_work can hold them
+  if (!d_T && fused_build_dp_supported(mp, L) &&
+      (Bp >= kFusedMinChains || d_work == nullptr || work_bytes < table_bytes(Bp, L, K) + bp_bytes(Bp, L, K))) {
     if (d_work == nullptr || work_bytes < fused_bp_bytes(L)) {
       set_error("chain_dp: workspace of %zu bytes needed, %zu given", fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
       return AUTODDL_EWORK;
@@ -194,7 +201,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
                          int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, cudaStream_t st) {
   const bool do_cd = d_init != nullptr;
   static const bool no_fuse = getenv("AUTODDL_NO_FUSE") != nullptr;   // debugging switch: three separate kernels
-  const bool fused = !no_fuse && fused_build_dp_supported(mp, L);
+  const bool fused = !no_fuse && Bp >= kFusedMinChains && fused_build_dp_supported(mp, L);
   const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
   size_t used = 0;
   int rc;

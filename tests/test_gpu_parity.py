@@ -205,6 +205,17 @@ def test_search_one_call_configs(adl, k):
     _assert_same(_search_all(adl, w, init), want)
 
 
+def _fused_dp(adl, w):
+    """chain DP through the fused build + DP kernel whatever the number of chains: with a workspace too small for the
+    tables autoddl_chain_dp(d_T = NULL) has to run the tables through shared memory only"""
+    d_layers = adl.layers_to_device(w.layers)
+    small = torch.empty(148 * 8 * w.L * 36 + 4096, dtype=torch.uint8, device="cuda")
+    assert small.numel() < w.Bp * w.L * 36 * 36 * 8
+    dc, ds = adl.chain_dp(None, w.mesh, net=w.net, d_layers=d_layers, work=small)
+    torch.cuda.synchronize()
+    return dc.cpu().numpy(), ds.cpu().numpy()
+
+
 @pytest.mark.parametrize("Bp,L", [(1, 1), (3, 1), (5, 2), (7, 3), (5, 7), (1500, 3), (900, 5), (33, 64), (2, 300)])
 def test_search_fused_shapes(adl, Bp, L):
     """fused kernel over ragged groups (L not a multiple of the group size), more chains than resident CTAs,
@@ -213,23 +224,26 @@ def test_search_fused_shapes(adl, Bp, L):
     init = w.cd_init()
     nsamp = min(Bp, 40)
     idx = np.unique(np.concatenate([np.arange(min(Bp, 6)), np.random.default_rng(1).integers(0, Bp, nsamp), [Bp - 1]]))
-    got = _search_all(adl, w, init)
+    got = _search_all(adl, w, init)                              # fused for Bp >= 296, three kernels below
     ws = cf.Workload(w.name, np.ascontiguousarray(w.layers[idx]), w.mesh, w.net, S=w.S, seed=w.seed)
     want = _oracle_all(ws, np.ascontiguousarray(init[idx]))
     _assert_same([g[idx] for g in got], want)
-    # all chains: the fused DP equals the separate DP kernel on the same tables
+    # all chains: fused DP (forced) == one-call path == the separate DP kernel on the same tables
     d_layers = adl.layers_to_device(w.layers)
     T, _, _ = adl.build_tables(d_layers, w.mesh, w.net)
     dc, ds = adl.chain_dp(T, w.mesh)
     assert np.array_equal(got[3], dc.cpu().numpy()) and np.array_equal(got[4], ds.cpu().numpy())
     assert np.array_equal(got[0], T.cpu().numpy())
+    if Bp * L * 36 * 36 * 8 > 148 * 8 * L * 36 + 4096:
+        fc, fs = _fused_dp(adl, w)
+        assert np.array_equal(fc, dc.cpu().numpy()) and np.array_equal(fs, ds.cpu().numpy())
 
 
 def test_search_mixed_kinds_and_unit_level(adl):
     """fused kernel with ATTN edges, ragged dims, split limits, a memory cap and a mesh level of size 1"""
     rng = np.random.default_rng(11)
     for sizes, links in [((3, 5), (1, 0)), ((1, 7), (1, 0)), ((8, 1), (1, 0))]:
-        Bp, L = 7, 9
+        Bp, L = 310, 9
         layers = np.zeros((Bp, L), dtype=cf.LAYER_DTYPE)
         for p in range(Bp):
             for l in range(L):
@@ -239,9 +253,18 @@ def test_search_mixed_kinds_and_unit_level(adl):
                 else:
                     layers[p, l] = cf.gemm(M, Kd, N, 2, 4, 18, in_rows=int(rng.integers(1, 5000)), in_cols=int(rng.integers(1, 5000)),
                                            max_rows=int(rng.integers(1, 64)), max_cols=int(rng.integers(1, 64)))
-        w = cf.Workload("mixed", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), 150_000 * L), S=3, seed=2)
+        w = cf.Workload("mixed", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), 150_000 * L), S=2, seed=2)
         init = w.cd_init()
-        _assert_same(_search_all(adl, w, init), _oracle_all(w, init))
+        got = _search_all(adl, w, init)                          # 310 chains: the fused kernel
+        idx = np.arange(0, Bp, 9)
+        ws = cf.Workload(w.name, np.ascontiguousarray(w.layers[idx]), w.mesh, w.net, S=w.S, seed=w.seed)
+        _assert_same([g[idx] for g in got], _oracle_all(ws, np.ascontiguousarray(init[idx])))
+        fc, fs = _fused_dp(adl, w)
+        assert np.array_equal(fc, got[3]) and np.array_equal(fs, got[4])
+        d_layers = adl.layers_to_device(w.layers)
+        T, _, _ = adl.build_tables(d_layers, w.mesh, w.net)
+        dc, ds = adl.chain_dp(T, w.mesh)
+        assert np.array_equal(got[0], T.cpu().numpy()) and np.array_equal(got[3], dc.cpu().numpy()) and np.array_equal(got[4], ds.cpu().numpy())
 
 
 def test_search_without_tables_and_full_size(adl):
