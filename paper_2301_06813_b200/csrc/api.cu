@@ -149,7 +149,8 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
       return AUTODDL_EWORK;
     }
     if ((rc = check_device())) return rc;
-    return launch_build_dp_fused(d_layers, Bp, L, mp, nullptr, nullptr, nullptr, d_opt_cost, d_strategy, (uint8_t*)d_work, st);
+    return launch_build_dp_fused(d_layers, Bp, L, mp, nullptr, nullptr, nullptr, d_opt_cost, d_strategy, (uint8_t*)d_work,
+                                 nullptr, 0, nullptr, st);
   }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
   if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
@@ -205,6 +206,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
   size_t used = 0;
   int rc;
+  bool cd_resume = false;
   if (need_tables && !d_T && (do_cd || !fused)) {
     used = table_bytes(Bp, L, K);
     if (d_work == nullptr || work_bytes < used) {
@@ -218,7 +220,12 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
       set_error("search: workspace of %zu bytes needed, %zu given", used + fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
       return AUTODDL_EWORK;
     }
-    if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used, st))) return rc;
+    // the first CD sweep rides in the fused kernel (tiles are in shared memory there); the CD kernel resumes at sweep 2
+    static const bool no_cd_fuse = getenv("AUTODDL_NO_CD_FUSE") != nullptr;
+    cd_resume = do_cd && !no_cd_fuse && fused_cd_sweep_supported(L, S);
+    if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used,
+                                    cd_resume ? d_init : nullptr, S, cd_resume ? d_cd_strategy : nullptr, st)))
+      return rc;
   } else {
     const size_t bb = bp_bytes(Bp, L, K);
     if (bb && (d_work == nullptr || work_bytes < used + bb)) {
@@ -228,7 +235,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
     if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + used : nullptr, d_opt_cost, d_strategy, st))) return rc;
   }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume);
   return AUTODDL_OK;
 }
 

@@ -498,7 +498,8 @@ template <int NT, int G, bool FUSE>
 __global__ void __launch_bounds__(FUSE ? NT + 32 : NT, FUSE ? 5 : 768 / NT)
 build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
                       int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
-                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob) {
+                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
+                      const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1) {
   using SM = Smem36<G>;
   constexpr int D = 2, K = SM::K, NS = SM::NS, NC = SM::NC, ES = SM::ES, NROW = SM::NROW;
   constexpr int STRIDE = SM::STRIDE;
@@ -512,6 +513,7 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
   SM& sm = *reinterpret_cast<SM*>(smem36_raw);
   // FUSE: back-pointers [L][K] of the chain in flight live in a per-CTA slice of the workspace (L2-resident)
   uint8_t* bp = FUSE ? bp_glob + (size_t)blockIdx.x * L * K : nullptr;
+  uint8_t* cd_s = smem36_raw + sizeof(SM);                 // FUSE + CD: strategies of the chain's starts [cd_S][L]
   const int tid = threadIdx.x;
 
   if (tid < NT) {
@@ -547,6 +549,39 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
     }
     __syncwarp();
     int cur = 0;
+    const bool cd = cd_init != nullptr;
+    const int64_t* ev_prev = nullptr;                      // tile l - 1 of the chain (may live in the other EV buffer)
+    int pending_free = -1;                                 // EV buffer still needed for the CD update of its last tile
+    // first Coordinate Descent sweep (R10) of layer `l` of every start, from the tiles in shared memory:
+    //   s_l <- smallest-index argmin_c T[l][s_{l-1}][c] + T[l+1][c][s_{l+1}],  T[l][i][j] = EV_l[block_row_of(i)][j]
+    auto cd_update = [&](int l, const int64_t* ev_l, const int64_t* ev_r) {
+      for (int st = 0; st < cd_S; ++st) {
+        uint8_t* sv = cd_s + (size_t)st * L;
+        const int left = l > 0 ? sv[l - 1] : 0;
+        const int64_t* row = ev_l + block_row_of(left) * K;
+        const int right = ev_r ? sv[l + 1] : 0;
+        int64_t bv = INT64_MAX;
+        int bi = K;
+#pragma unroll
+        for (int c0 = 0; c0 < 64; c0 += 32) {
+          const int c = c0 + lane;
+          if (c < K) {
+            int64_t g = row[c];
+            if (ev_r) g += ev_r[(c < 24 ? c : (c < 30 ? c - 12 : c - 18)) * K + right];
+            if (g < bv) { bv = g; bi = c; }
+          }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+          const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+          const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+          if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        __syncwarp();
+        if (lane == 0) sv[l] = (uint8_t)bi;
+        __syncwarp();
+      }
+    };
     for (int it = 0; sc.valid; ++it, sc.advance(G)) {
       const int eb = it & 1;
       mbar_wait(&sm.full[eb], (it >> 1) & 1);
@@ -558,11 +593,26 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
         int64_t* fn = sm.f[cur ^ 1];
         if (l == 0) {                                      // f_0[j] = T[0][0][j]
           for (int j = lane; j < K; j += 32) fn[j] = ev[j];
+          if (cd) {                                        // the chain's starts
+            for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)sc.p * cd_S * L + x];
+          }
         } else {
           dp36_step_blockrows(ev, sm.f[cur], fn, bp + (size_t)l * K, sm.repcol[kind], sm.repof[kind], lane);
         }
         cur ^= 1;
         __syncwarp();
+        if (cd) {
+          if (l > 0) cd_update(l - 1, ev_prev, ev);
+          if (l == L - 1) {
+            cd_update(l, ev, nullptr);
+            for (int x = lane; x < cd_S * L; x += 32) cd_s1[(size_t)sc.p * cd_S * L + x] = cd_s[x];
+          }
+          ev_prev = ev;
+          if (t == 0 && pending_free >= 0) {               // the previous group's last tile has served its CD update
+            if (lane == 0) mbar_arrive(&sm.freeb[pending_free]);
+            pending_free = -1;
+          }
+        }
         if (l == L - 1) {                                  // smallest argmin of f_{L-1}, then backtrack
           const int64_t* f = sm.f[cur];
           int64_t bv = f[lane];
@@ -604,7 +654,12 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
           __syncwarp();
         }
       }
-      if (lane == 0) mbar_arrive(&sm.freeb[eb]);
+      __syncwarp();
+      if (cd && sc.l0 + sc.nt < L) {
+        pending_free = eb;                                 // its last tile is still needed: CD update of that layer
+      } else if (lane == 0) {
+        mbar_arrive(&sm.freeb[eb]);
+      }
     }
     return;
   }
@@ -848,7 +903,7 @@ int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams
     const int per = atoi(getenv("AUTODDL_BT_VARIANT"));
     const int ngroups = (ntiles + 1) / 2;
     const int grid = ngroups < 148 * per ? ngroups : 148 * per;
-    kern<<<grid, 128, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr);
+    kern<<<grid, 128, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr, nullptr, 0, nullptr);
     count_launch();
     return AUTODDL_OK;
   }
@@ -860,7 +915,7 @@ int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int ngroups = (ntiles + kG - 1) / kG;
   const int grid = ngroups < sms * 3 ? ngroups : sms * 3;             // persistent, grid-stride over tile groups
-  kern<<<grid, kNT, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr);
+  kern<<<grid, kNT, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr, nullptr, 0, nullptr);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -896,20 +951,24 @@ size_t fused_bp_bytes(int32_t L) {
   return ((size_t)limit * L * 36 + 255) / 256 * 256 + 256;
 }
 
+// largest S * L for which the first CD sweep rides in the fused kernel (strategies of a chain's starts in shared memory)
+bool fused_cd_sweep_supported(int32_t L, int32_t S) { return S >= 1 && (int64_t)S * L <= 4096; }
+
 int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
                           int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
-                          cudaStream_t st) {
+                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, cudaStream_t st) {
   const int64_t nt = (int64_t)Bp * L;
   if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   if (!fused_build_dp_supported(mp, L)) { set_error("fused build+DP needs a 2-level mesh"); return AUTODDL_EINVAL; }
   if (d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
   auto kern = build_tables36_kernel<kFuseNT, kFuseG, true>;
-  const size_t smem = sizeof(Smem36<kFuseG>);
+  if (d_cd_init && (!fused_cd_sweep_supported(L, S) || d_cd_s1 == nullptr)) { set_error("fused CD sweep: S * L too large"); return AUTODDL_EINVAL; }
+  const size_t smem = (sizeof(Smem36<kFuseG>) + (d_cd_init ? (size_t)S * L : 0) + 127) / 128 * 128;
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int limit = fused_grid_limit();
   const int grid = Bp < limit ? Bp : limit;                            // persistent, grid-stride over chains
   kern<<<grid, kFuseNT + 32, smem, st>>>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy,
-                                         (uint8_t*)(((uintptr_t)d_bp + 15) & ~(uintptr_t)15));
+                                         (uint8_t*)(((uintptr_t)d_bp + 15) & ~(uintptr_t)15), d_cd_init, S, d_cd_s1);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;

@@ -53,15 +53,17 @@ bool fused_build_dp_supported(const MeshParams& mp, int32_t L);
 size_t fused_bp_bytes(int32_t L);
 int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
                           int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
-                          cudaStream_t st);
+                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, cudaStream_t st);
+bool fused_cd_sweep_supported(int32_t L, int32_t S);
 int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp,
                     int64_t* d_opt_cost, int32_t* d_strategy, cudaStream_t st);
 bool chain_dp_cluster_supported(int32_t K, int32_t L);
 int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* d_opt_cost, int32_t* d_strategy,
                             cudaStream_t st);
+// resume: the first sweep has been done already (its result is in d_strategy); continue from sweep 2
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
-                         int32_t* d_sweeps, cudaStream_t st);
+                         int32_t* d_sweeps, cudaStream_t st, bool resume = false);
 int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                       int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost, int32_t* d_best_strategy,
                       int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted, cudaStream_t st);

@@ -32,7 +32,10 @@ __device__ __forceinline__ int64_t ldg_narrow(const int64_t* p) {
   return v;
 }
 
-template <int K>
+// RESUME: the first sweep was run elsewhere (the fused build + DP kernel does it from the tiles in shared memory) and
+// its result is in `strategy`; a layer is dirty iff its right neighbour changed in that sweep (changed = differs from
+// `init`: a layer is touched once per sweep), the sweep count starts at 1, and nothing changed <=> finished.
+template <int K, bool RESUME>
 __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int L, int S,
                                                            const int32_t* __restrict__ init, int max_sweeps,
                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
@@ -46,14 +49,26 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   const size_t p = ps / S;
   const int64_t* Tp = T + p * (size_t)L * K * K;
 
-  for (int l = lane; l < L; l += 32) {
-    s[l] = init[ps * L + l];
-    dirty[l] = 1;
+  int nsweeps = 0;
+  bool resume_done = false;
+  if (RESUME) {
+    bool any = false;
+    for (int l = lane; l < L; l += 32) {
+      s[l] = strategy[ps * L + l];
+      any |= s[l] != init[ps * L + l];
+      dirty[l] = (l + 1 < L && strategy[ps * L + l + 1] != init[ps * L + l + 1]) ? 1 : 0;
+    }
+    nsweeps = 1;
+    resume_done = !__any_sync(0xffffffffu, any) || max_sweeps <= 1;
+  } else {
+    for (int l = lane; l < L; l += 32) {
+      s[l] = init[ps * L + l];
+      dirty[l] = 1;
+    }
   }
   __syncwarp();
 
-  int nsweeps = 0;
-  for (;;) {
+  for (; !resume_done;) {
     bool changed = false;
     for (int l = 0; l < L; ++l) {
       if (!dirty[l]) continue;                               // warp-uniform
@@ -105,16 +120,16 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   }
 }
 
-template <int K>
+template <int K, bool RESUME>
 int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
              int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
   const size_t smem = ((size_t)L * 5 + 15) / 16 * 16;
   if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
   if (smem > 48 * 1024)
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K, RESUME>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t nb = (int64_t)Bp * S;
   if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
-  coord_descent_kernel<K><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
+  coord_descent_kernel<K, RESUME><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -123,11 +138,17 @@ int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, in
 }  // namespace
 
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
-                         int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+                         int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st,
+                         bool resume) {
+  if (resume) {
+    if (K == 36) return launch_k<36, true>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    set_error("coord_descent: resume mode exists for K = 36 only");
+    return AUTODDL_EINVAL;
+  }
   switch (K) {
-    case 6:   return launch_k<6>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
-    case 36:  return launch_k<36>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
-    case 216: return launch_k<216>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 6:   return launch_k<6, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 36:  return launch_k<36, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 216: return launch_k<216, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
   }
   set_error("coord_descent: K must be 6, 36 or 216");
   return AUTODDL_EINVAL;

@@ -279,6 +279,18 @@ def test_search_without_tables_and_full_size(adl):
     torch.cuda.synchronize()
     assert torch.equal(o["T"], T) and torch.equal(o["opt_cost"], dc) and torch.equal(o["strategy"], ds)
     assert torch.equal(dc2, dc) and torch.equal(ds2, ds)
+    # one call with CD: the first sweep runs inside the fused kernel, the CD kernel resumes at sweep 2
+    init = torch.from_numpy(w.cd_init()).cuda()
+    o3 = adl.search(d_layers, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps)
+    cc, cs, sw = adl.coord_descent(T, init, w.mesh, w.max_sweeps)
+    torch.cuda.synchronize()
+    assert torch.equal(o3["cd_cost"], cc) and torch.equal(o3["cd_strategy"], cs) and torch.equal(o3["cd_sweeps"], sw)
+    assert torch.equal(o3["opt_cost"], dc) and torch.equal(o3["T"], T)
+    for cap in (1, 2, 3):                                   # sweep cap below, at and above the resume point
+        o4 = adl.search(d_layers, w.mesh, w.net, init=init, max_sweeps=cap)
+        c4 = adl.coord_descent(T, init, w.mesh, cap)
+        torch.cuda.synchronize()
+        assert torch.equal(o4["cd_cost"], c4[0]) and torch.equal(o4["cd_strategy"], c4[1]) and torch.equal(o4["cd_sweeps"], c4[2])
     mesh, net = ref.mesh_of(w), ref.net_of(w)
     for p in [0, 1, 739, 740, 2047, 4095]:
         oT, _, _ = ref.build_tables(w.layers[p:p + 1], mesh, net)
