@@ -145,6 +145,11 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
  * copy bandwidth in the same run as the kernels above.  bytes must be a multiple of 16. */
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream);
 
+/* Profiling hook (used by bench.py for the per-kernel split of the one-call path): the next autoddl_search /
+ * autoddl_search_host call of this thread records `cuda_event` (a cudaEvent_t, NULL to cancel) on its stream after
+ * the tables + chain DP and before Coordinate Descent.  One shot. */
+int autoddl_profile_mark(void* cuda_event);
+
 /* Number of kernel launches issued by this library in the calling thread since load (for bench.py's
  * gpu_launches). */
 int64_t autoddl_launch_count(void);

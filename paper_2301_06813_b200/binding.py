@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -66,6 +66,8 @@ def lib():
         L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
         L.autoddl_copy_probe.restype = C.c_int
         L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
+        L.autoddl_profile_mark.restype = C.c_int
+        L.autoddl_profile_mark.argtypes = [vp]
         L.autoddl_launch_count.restype = i64
         L.autoddl_launch_count.argtypes = []
         L.autoddl_last_error.restype = C.c_char_p
@@ -202,6 +204,12 @@ def metropolis(T: torch.Tensor, init: torch.Tensor, mesh, nsteps: int, tau_ps: i
     _check(lib().autoddl_metropolis(_ptr(T), Bp, L, C.addressof(m), _ptr(init), S, nsteps, tau_ps, seed, _ptr(bc), _ptr(bs),
                                     _ptr(fc), _ptr(fs), _ptr(acc), _stream()))
     return out
+
+
+def profile_mark(event: "torch.cuda.Event | None"):
+    """the next search() records `event` between tables + DP and Coordinate Descent (the event must have been recorded
+    once before so that its handle exists)"""
+    _check(lib().autoddl_profile_mark(None if event is None else event.cuda_event))
 
 
 def search(d_layers: torch.Tensor, mesh, net, init: torch.Tensor | None = None, max_sweeps: int = 64,

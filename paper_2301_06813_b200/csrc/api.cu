@@ -9,6 +9,7 @@ namespace autoddl {
 
 static thread_local char g_err[512] = "";
 static thread_local int64_t g_launches = 0;
+static thread_local cudaEvent_t g_mark = nullptr;          // autoddl_profile_mark: one-shot event between the kernels of a search
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -235,6 +236,10 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
     if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + used : nullptr, d_opt_cost, d_strategy, st))) return rc;
   }
+  if (g_mark) {                                             // profiling hook: tables + DP done, CD not yet started
+    cudaEventRecord(g_mark, st);
+    g_mark = nullptr;
+  }
   if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume);
   return AUTODDL_OK;
 }
@@ -341,6 +346,11 @@ int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* strea
   int rc = check_device();
   if (rc) return rc;
   return launch_copy_probe(d_src, d_dst, bytes, (cudaStream_t)stream);
+}
+
+int autoddl_profile_mark(void* cuda_event) {
+  g_mark = (cudaEvent_t)cuda_event;
+  return AUTODDL_OK;
 }
 
 int64_t autoddl_launch_count(void) { return g_launches; }
