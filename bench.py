@@ -303,7 +303,7 @@ def run_ours(args):
     h_layers = torch.from_numpy(np.ascontiguousarray(w.layers).view(np.uint8).reshape(Bp, L, 64).copy()).pin_memory()
     h_init = torch.from_numpy(init_np.copy()).pin_memory()
     w_host = cf.Workload(w.name, h_layers.numpy().view(cf.LAYER_DTYPE).reshape(Bp, L), w.mesh, w.net, S=S, seed=w.seed)
-    e2e_steps = max(3, min(args.steps, 20))
+    e2e_steps = max(3, min(args.steps, 50))
     for _ in range(3):
         adl.search_host(w_host, h_init.numpy(), work, pinned)
     barrier()
