@@ -375,6 +375,7 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
                          "frac": kernels[dom]["alg_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
                          "copy_probe_GBps_same_run": copy_gbs,
+                         "frac_counting_only_bytes_that_must_reach_hbm": kernels[dom].get("hbm_min_frac_of_peak"),
                          "note": "algorithmic bytes by SURVEY 8(d) for the work the fused launch does (tables 8 B/cell + DP 8 B/cell "
                                  "+ one CD sweep per start); its HBM traffic is the table write only, see kernels[...].hbm_min_*"},
             "e2e": {"value": world * cells / (e2e_ms * 1e-3), "unit": "cells/s", "ms_per_step": e2e_ms,
