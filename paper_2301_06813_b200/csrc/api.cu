@@ -188,12 +188,13 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   }
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
+  const bool built_here = d_T == nullptr;                  // tables of this library's builder: identical rows per class
   if (!d_T) {
     ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
     d_T = (const int64_t*)d_work;
   }
-  return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+  return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, false, built_here);
 }
 
 // (a1) -> (a2) -> (a3) on device pointers; tables go to d_T, or into d_work when d_T is NULL
@@ -240,7 +241,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     cudaEventRecord(g_mark, st);
     g_mark = nullptr;
   }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume);
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, true);
   return AUTODDL_OK;
 }
 

@@ -61,9 +61,10 @@ bool chain_dp_cluster_supported(int32_t K, int32_t L);
 int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* d_opt_cost, int32_t* d_strategy,
                             cudaStream_t st);
 // resume: the first sweep has been done already (its result is in d_strategy); continue from sweep 2
+// sbp_rows: d_T was built by this library (identical rows per producer-signature class may be read through one row)
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
-                         int32_t* d_sweeps, cudaStream_t st, bool resume = false);
+                         int32_t* d_sweeps, cudaStream_t st, bool resume = false, bool sbp_rows = false);
 int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                       int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost, int32_t* d_best_strategy,
                       int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted, cudaStream_t st);

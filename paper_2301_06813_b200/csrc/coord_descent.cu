@@ -35,7 +35,11 @@ __device__ __forceinline__ int64_t ldg_narrow(const int64_t* p) {
 // RESUME: the first sweep was run elsewhere (the fused build + DP kernel does it from the tiles in shared memory) and
 // its result is in `strategy`; a layer is dirty iff its right neighbour changed in that sweep (changed = differs from
 // `init`: a layer is touched once per sweep), the sweep count starts at 1, and nothing changed <=> finished.
-template <int K, bool RESUME>
+// SBPROWS: the tables were built by this library (autoddl_search, or d_T == NULL), so rows of a tile whose producer
+// signatures agree up to the per-level classes {0}, {1}, {3}, {2, 4, 5} are identical (signatures 2, 4, 5 all output P,
+// or are all invalid for ATTN: DESIGN.md R1): the column gather reads the class representative's row, and candidates
+// of one class share one 64-byte granule -- 16 instead of 36 at K = 36.  Values, hence results, are unchanged.
+template <int K, bool RESUME, bool SBPROWS>
 __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int L, int S,
                                                            const int32_t* __restrict__ init, int max_sweeps,
                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
@@ -48,6 +52,24 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   const size_t ps = blockIdx.x;
   const size_t p = ps / S;
   const int64_t* Tp = T + p * (size_t)L * K * K;
+  constexpr int NCAND = (K + 31) / 32;
+  int rep[NCAND];                                          // row that holds candidate c's column value
+#pragma unroll
+  for (int q = 0; q < NCAND; ++q) {
+    const int c = 32 * q + lane;
+    int r = 0, pw = 1, x = c;
+    if (SBPROWS) {
+      for (int d = 0; d < 3 && pw < K; ++d) {              // base-6 digits, least significant first
+        const int dig = x % 6;
+        x /= 6;
+        r += (dig < 4 ? dig : 2) * pw;
+        pw *= 6;
+      }
+    } else {
+      r = c;
+    }
+    rep[q] = r;
+  }
 
   int nsweeps = 0;
   bool resume_done = false;
@@ -79,11 +101,11 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
       int64_t bv = INT64_MAX;
       int bi = K;
 #pragma unroll
-      for (int c0 = 0; c0 < K; c0 += 32) {
-        const int c = c0 + lane;
+      for (int q = 0; q < NCAND; ++q) {
+        const int c = 32 * q + lane;
         if (c < K) {
           int64_t g = __ldg(row + c);
-          if (has_right) g += ldg_narrow(col + (size_t)c * K);
+          if (has_right) g += ldg_narrow(col + (size_t)rep[q] * K);
           if (g < bv) { bv = g; bi = c; }
         }
       }
@@ -120,16 +142,16 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   }
 }
 
-template <int K, bool RESUME>
+template <int K, bool RESUME, bool SBPROWS>
 int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
              int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
   const size_t smem = ((size_t)L * 5 + 15) / 16 * 16;
   if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
   if (smem > 48 * 1024)
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K, RESUME>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K, RESUME, SBPROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t nb = (int64_t)Bp * S;
   if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
-  coord_descent_kernel<K, RESUME><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
+  coord_descent_kernel<K, RESUME, SBPROWS><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -139,17 +161,19 @@ int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, in
 
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                          int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st,
-                         bool resume) {
+                         bool resume, bool sbp_rows) {
+#define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
   if (resume) {
-    if (K == 36) return launch_k<36, true>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    if (K == 36) return sbp_rows ? ADL_CD(36, true, true) : ADL_CD(36, true, false);
     set_error("coord_descent: resume mode exists for K = 36 only");
     return AUTODDL_EINVAL;
   }
   switch (K) {
-    case 6:   return launch_k<6, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
-    case 36:  return launch_k<36, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
-    case 216: return launch_k<216, false>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    case 6:   return sbp_rows ? ADL_CD(6, false, true) : ADL_CD(6, false, false);
+    case 36:  return sbp_rows ? ADL_CD(36, false, true) : ADL_CD(36, false, false);
+    case 216: return sbp_rows ? ADL_CD(216, false, true) : ADL_CD(216, false, false);
   }
+#undef ADL_CD
   set_error("coord_descent: K must be 6, 36 or 216");
   return AUTODDL_EINVAL;
 }
