@@ -8,8 +8,8 @@
 //     with f read from the CTA's own 27-entry slice of f_{l-1};
 //   - the partial (value, row) of column j goes straight into the shared memory of the CTA that owns column j
 //     (j / 27) with st.async over DSMEM, which also completes the transaction count of that CTA's mbarrier;
-//   - 27 owner threads per CTA merge the 8 partials of their column in ascending row-block order (strict '<')
-//     and write f_l[27 q + c]: exactly the slice that CTA needs as f_{l-1}[i] for its rows of the next tile.
+//   - 8 lanes per owned column merge the 8 partials with three shuffle steps on (value, row) -- row blocks are
+//     disjoint, so the smaller row wins ties -- and write f_l[27 q + c]: exactly the slice that CTA needs as f_{l-1}[i] for its rows of the next tile.
 // One reduce-scatter per layer and no all-gather, no cluster-wide barrier inside the layer loop.  Back-pointers
 // stay in shared memory (27 per layer per CTA), are gathered into CTA 0 at the end and walked there.
 // Results are identical to the definition (R9): every comparison is on (value, smallest row).
@@ -121,34 +121,36 @@ chain_dp216_cluster_kernel(const int64_t* __restrict__ T, int L, int64_t* __rest
         const int64_t* f = sm.f[par ^ 1];
         int64_t best = INT64_MAX;
         int arg = 0;
+        int64_t tv[CR];
 #pragma unroll
-        for (int part = 0; part < 3; ++part) {
-          int64_t tv[9];
+        for (int k = 0; k < CR; ++k) tv[k] = tile[k * CK];  // all 27 rows in flight
 #pragma unroll
-          for (int k = 0; k < 9; ++k) tv[k] = tile[(9 * part + k) * CK];
-#pragma unroll
-          for (int k = 0; k < 9; ++k) {
-            const int64_t v = f[9 * part + k] + tv[k];
-            if (v < best) { best = v; arg = 9 * part + k; }
-          }
+        for (int k = 0; k < CR; ++k) {
+          const int64_t v = f[k] + tv[k];
+          if (v < best) { best = v; arg = k; }
         }
         st_async_v2(map_to_cta(&sm.slot[par][r][j - CR * owner][0], owner), best, (int64_t)(CR * r + arg),
                     map_to_cta(&sm.recv[par], owner));
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(&sm.empty[s]);            // this warp is done with the stage
-      if (tid < CR) {                                      // owner of column 27 r + tid: merge the 8 row blocks in order
+      {                                                    // 8 lanes per owned column merge the 8 row blocks
         while (!mbar_try_wait_cluster(&sm.recv[par], ((l - 1) >> 1) & 1)) {
         }
-        int64_t bv = sm.slot[par][0][tid][0];
-        int64_t bi = sm.slot[par][0][tid][1];
+        const int mc = tid >> 3, mq = tid & 7;             // owned column (< 27 for tid < 216), source CTA
+        const bool mine = tid < CR * CC;
+        int64_t bv = mine ? sm.slot[par][mq][mc][0] : INT64_MAX;
+        int64_t bi = mine ? sm.slot[par][mq][mc][1] : 0;
 #pragma unroll
-        for (int q = 1; q < CC; ++q) {
-          const int64_t v = sm.slot[par][q][tid][0];
-          if (v < bv) { bv = v; bi = sm.slot[par][q][tid][1]; }
+        for (int off = 1; off < 8; off <<= 1) {            // row blocks are disjoint: the smaller row wins ties
+          const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+          const int64_t oi = __shfl_xor_sync(0xffffffffu, bi, off);
+          if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
         }
-        sm.f[par][tid] = bv;
-        bp[(size_t)l * CR + tid] = (uint8_t)bi;
+        if (mine && mq == 0) {
+          sm.f[par][mc] = bv;
+          bp[(size_t)l * CR + mc] = (uint8_t)bi;
+        }
       }
       asm volatile("bar.sync 1, 224;" ::: "memory");       // f_l slice is complete for the next layer's scan
     }
