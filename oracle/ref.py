@@ -241,3 +241,20 @@ def metropolis(T: np.ndarray, init: np.ndarray, nsteps: int, tau_ps: int, seed: 
     if want_trace:
         return bc, bs, fc, fs, acc, trace
     return bc, bs, fc, fs, acc
+
+
+# ---- alpha-beta calibration (Table 2) ---------------------------------------
+def fit_design_matrix(kind: np.ndarray, p: np.ndarray, nbytes: np.ndarray) -> np.ndarray:
+    """rows (A_i, B_i) of the linear system t_i = A_i alpha + B_i beta, Table 2 as printed (real-valued (p-1)/p n):
+    AllGather / ReduceScatter: (p-1, (p-1)/p n); AllReduce: (2p-1, 2 (p-1)/p n); AlltoAll: (p-1, n)"""
+    kind = np.asarray(kind); p = np.asarray(p, dtype=np.float64); n = np.asarray(nbytes, dtype=np.float64)
+    A = np.where(kind == AR, 2 * p - 1, p - 1)
+    B = np.where(kind == AR, 2 * (p - 1) / p * n, np.where(kind == A2A, n, (p - 1) / p * n))
+    return np.stack([A, B], axis=1)
+
+
+def fit_alpha_beta(kind, p, nbytes, t):
+    """least-squares (alpha, beta) from timed collectives: the definition, solved by numpy.linalg.lstsq (SVD) in fp64"""
+    X = fit_design_matrix(kind, p, nbytes)
+    sol, *_ = np.linalg.lstsq(X, np.asarray(t, dtype=np.float64), rcond=None)
+    return float(sol[0]), float(sol[1])
