@@ -117,6 +117,16 @@ int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_
                        int64_t* d_best_cost, int32_t* d_best_strategy, int64_t* d_final_cost,
                        int32_t* d_final_strategy, int32_t* d_accepted, void* stream);
 
+/* alpha-beta calibration: least-squares (alpha, beta) of the linear system of Table 2
+ *   t_i = A_i alpha + B_i beta  over N timed collectives, d_kind[i] in {0 AllGather, 1 ReduceScatter,
+ * 2 AllReduce, 3 AlltoAll}, d_p[i] >= 2 participants, d_bytes[i] message bytes, d_time[i] measured time (any unit):
+ * (A, B) = (p-1, (p-1)/p n), (2p-1, 2 (p-1)/p n) for AllReduce, (p-1, n) for AlltoAll.  fp64; d_out[0] = alpha,
+ * d_out[1] = beta (time unit per byte).  d_work: >= autoddl_fit_workspace_bytes() bytes, 8-byte aligned.
+ * Deterministic (fixed grid and reduction order). */
+size_t autoddl_fit_workspace_bytes(void);
+int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64_t* d_bytes, const double* d_time,
+                           int64_t N, double* d_out, void* d_work, size_t work_bytes, void* stream);
+
 /* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36) with at least 296
  * chains (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and
  * consumed by the chain DP from shared memory, so the optimum costs no table read.  Other meshes run

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -66,6 +66,10 @@ def lib():
         L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
         L.autoddl_copy_probe.restype = C.c_int
         L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
+        L.autoddl_fit_workspace_bytes.restype = sz
+        L.autoddl_fit_workspace_bytes.argtypes = []
+        L.autoddl_fit_alpha_beta.restype = C.c_int
+        L.autoddl_fit_alpha_beta.argtypes = [vp, vp, vp, vp, i64, vp, vp, sz, vp]
         L.autoddl_profile_mark.restype = C.c_int
         L.autoddl_profile_mark.argtypes = [vp]
         L.autoddl_launch_count.restype = i64
@@ -203,6 +207,18 @@ def metropolis(T: torch.Tensor, init: torch.Tensor, mesh, nsteps: int, tau_ps: i
     m = c_mesh(mesh)
     _check(lib().autoddl_metropolis(_ptr(T), Bp, L, C.addressof(m), _ptr(init), S, nsteps, tau_ps, seed, _ptr(bc), _ptr(bs),
                                     _ptr(fc), _ptr(fs), _ptr(acc), _stream()))
+    return out
+
+
+def fit_alpha_beta(kind: torch.Tensor, p: torch.Tensor, nbytes: torch.Tensor, t: torch.Tensor, out=None, work=None):
+    """alpha-beta calibration: kind int32 [N], p int32 [N], nbytes int64 [N], t float64 [N] (device) -> float64 [2] (device)"""
+    N = kind.numel()
+    dev = kind.device
+    if out is None:
+        out = torch.empty(2, dtype=torch.float64, device=dev)
+    if work is None:
+        work = torch.empty(int(lib().autoddl_fit_workspace_bytes()), dtype=torch.uint8, device=dev)
+    _check(lib().autoddl_fit_alpha_beta(_ptr(kind), _ptr(p), _ptr(nbytes), _ptr(t), N, _ptr(out), _ptr(work), work.numel(), _stream()))
     return out
 
 

@@ -340,6 +340,24 @@ int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_
                            d_final_cost, d_final_strategy, d_accepted, (cudaStream_t)stream);
 }
 
+size_t autoddl_fit_workspace_bytes(void) { return fit_workspace_bytes(); }
+
+int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64_t* d_bytes, const double* d_time,
+                           int64_t N, double* d_out, void* d_work, size_t work_bytes, void* stream) {
+  clear_error();
+  ADL_REQUIRE(d_kind && d_p && d_bytes && d_time && d_out, "NULL pointer");
+  ADL_REQUIRE(N >= 1, "N must be >= 1");
+  ADL_REQUIRE(((uintptr_t)d_bytes & 7) == 0 && ((uintptr_t)d_time & 7) == 0 && ((uintptr_t)d_out & 7) == 0 &&
+                  ((uintptr_t)d_work & 7) == 0 && ((uintptr_t)d_kind & 3) == 0 && ((uintptr_t)d_p & 3) == 0, "misaligned pointer");
+  if (d_work == nullptr || work_bytes < fit_workspace_bytes()) {
+    set_error("fit_alpha_beta: workspace of %zu bytes needed, %zu given", fit_workspace_bytes(), d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_fit_alpha_beta(d_kind, d_p, d_bytes, d_time, N, d_out, (double*)d_work, (cudaStream_t)stream);
+}
+
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {
   clear_error();
   ADL_REQUIRE(d_src && d_dst && bytes > 0 && bytes % 16 == 0, "copy_probe: bad arguments");

@@ -68,6 +68,9 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
 int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                       int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost, int32_t* d_best_strategy,
                       int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted, cudaStream_t st);
+size_t fit_workspace_bytes();
+int launch_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64_t* d_bytes, const double* d_time,
+                          int64_t N, double* d_out, double* d_work, cudaStream_t st);
 int launch_copy_probe(const void* src, void* dst, size_t bytes, cudaStream_t st);
 
 // ---- device helpers ------------------------------------------------------------------------------------
