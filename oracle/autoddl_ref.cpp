@@ -106,7 +106,7 @@ extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
   for (int d = D - 1; d >= 0; --d)
     if (cur[d] == REF_P && b[d] != REF_P) {
       const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // RS input size (Table 2 caption)
-      const int c = mesh->link[d];
+      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)
       cost += autoddl_ref_collective(1, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
       cur[d] = (b[d] == REF_B) ? REF_S1 : b[d];
     }
@@ -118,7 +118,7 @@ extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
     if (cs && bs && cur[d] != b[d]) {
       cur[d] = b[d];
       const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // output size
-      const int c = mesh->link[d];
+      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)
       cost += autoddl_ref_collective(3, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
     }
   }
@@ -128,7 +128,7 @@ extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
     if ((cur[d] == REF_S0 || cur[d] == REF_S1) && b[d] == REF_B) {
       cur[d] = REF_B;
       const int64_t n = autoddl_ref_local_size(rows, cols, cur, mesh) * eb;   // output size
-      const int c = mesh->link[d];
+      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)
       cost += autoddl_ref_collective(0, n, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
     }
 
@@ -166,7 +166,7 @@ extern "C" int64_t autoddl_ref_node_cost(const ref_layer* cur, int j, const ref_
   int64_t v = 0;
   for (int d = 0; d < mesh->ndim; ++d)
     if (W[d] == REF_B) {
-      const int c = mesh->link[d];
+      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)
       v += autoddl_ref_collective(2, nw * cur->wgrad_bytes, mesh->size[d], net->alpha_ps[c], net->beta_ps_per_byte[c]);
     }
   return v;
@@ -187,6 +187,12 @@ extern "C" int64_t autoddl_ref_layer_mem(const ref_layer* cur, int j, const ref_
 extern "C" int autoddl_ref_feasible(const ref_layer* cur, int j, int32_t L, const ref_mesh* mesh, const ref_net* net) {
   int32_t I[3], W[3], O[3];
   if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
+  // R24: a level may restrict its signature rows (bits 8..13 of link[d], 0 = all six).  Rows {0,1,2} on every level
+  // of a mesh refined into prime sub-levels is the paper's own factorisation space.
+  for (int d = mesh->ndim - 1, r = j; d >= 0; --d, r /= 6) {
+    const int allow = (mesh->link[d] >> 8) & 0x3f;
+    if (allow != 0 && !((allow >> (r % 6)) & 1)) return 0;
+  }
   int64_t rowsplit = 1, colsplit = 1;
   for (int d = 0; d < mesh->ndim; ++d) {
     if (I[d] == REF_S0 || O[d] == REF_S0) rowsplit *= mesh->size[d];
