@@ -60,7 +60,12 @@ typedef struct {
   int32_t max_split_cols;    /* largest allowed total split of the output's axis 1                   */
 } autoddl_layer;
 
-/* Device mesh, level 0 outermost.  link[d]: 0 = intra-node (NVLink), 1 = inter-node. */
+/* Device mesh, level 0 outermost.  link[d] bit 0: 0 = intra-node (NVLink), 1 = inter-node.
+ * link[d] bits 8..13 (optional): the signature rows allowed on the level, bit g = row g of the per-level table
+ * (0 split rows, 1 split columns, 2 split the reduction dim, 3 replicate, 4 partial input, 5 partial weight); 0 = all
+ * six.  With 0x07 << 8 on every level of a mesh refined into prime sub-levels the feasible strategies are exactly the
+ * paper's SBP matmul factorisations I = (S0:p0, B:p1, S1:p2), W = (B, S1, S0), O = (S0, S1, P);
+ * disallowed signatures are infeasible (penalty 2^50, mask 0).  K stays 6^ndim. */
 typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } autoddl_mesh;
 
 /* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap. */

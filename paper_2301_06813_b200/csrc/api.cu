@@ -25,7 +25,7 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
   ADL_REQUIRE(mesh->ndim >= 1 && mesh->ndim <= 3, "mesh.ndim = %d, must be 1..3", mesh->ndim);
   for (int d = 0; d < mesh->ndim; ++d) {
     ADL_REQUIRE(mesh->size[d] >= 1 && mesh->size[d] <= 65536, "mesh.size[%d] = %d out of range", d, mesh->size[d]);
-    ADL_REQUIRE(mesh->link[d] == 0 || mesh->link[d] == 1, "mesh.link[%d] = %d, must be 0 or 1", d, mesh->link[d]);
+    ADL_REQUIRE((mesh->link[d] & ~0x3f01) == 0, "mesh.link[%d] = %d: bit 0 = link class, bits 8..13 = allowed rows", d, mesh->link[d]);
   }
   int64_t prod = 1;
   for (int d = 0; d < mesh->ndim; ++d) prod *= mesh->size[d];
@@ -35,6 +35,7 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
     out->ndim = mesh->ndim;
     for (int d = 0; d < mesh->ndim; ++d) {
       out->size[d] = mesh->size[d];
+      out->allow[d] = ((mesh->link[d] >> 8) & 0x3f) ? ((mesh->link[d] >> 8) & 0x3f) : 0x3f;
       out->magic_size[d] = (uint64_t)((((unsigned __int128)1 << 64) + mesh->size[d] - 1) / mesh->size[d]);
     }
     for (int m = 0; m < 8; ++m) {
@@ -54,8 +55,8 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
     ADL_REQUIRE(net->mem_cap_bytes >= 0, "net.mem_cap_bytes < 0");
     if (out) {
       for (int d = 0; d < mesh->ndim; ++d) {
-        out->alpha[d] = net->alpha_ps[mesh->link[d]];
-        out->beta[d] = net->beta_ps_per_byte[mesh->link[d]];
+        out->alpha[d] = net->alpha_ps[mesh->link[d] & 1];
+        out->beta[d] = net->beta_ps_per_byte[mesh->link[d] & 1];
       }
       out->mem_cap = net->mem_cap_bytes;
     }

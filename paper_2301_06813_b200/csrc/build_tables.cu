@@ -109,6 +109,7 @@ struct SigInfo {
   uint8_t mI0, mI1;   // level subsets splitting the input's rows / cols
   uint8_t wB;         // levels on which W is replicated
   uint8_t valid;
+  uint8_t allowed;    // every per-level row of the signature is in the level's allowed set (mesh.link bits 8..13)
   int32_t rowsplit, colsplit;
 };
 
@@ -183,10 +184,11 @@ __device__ __forceinline__ void fill_sig_table(SigInfo (*sig)[Pow<D>::K], const 
     for (int d = D - 1; d >= 0; --d) { dig[d] = r % 6; r /= 6; }
     SigInfo si{};
     int a = 0, b = 0, cw = 0, co = 0, pw = 1, rs = 1, cs = 1;
-    bool valid = true;
+    bool valid = true, allowed = true;
 #pragma unroll
     for (int d = 0; d < D; ++d) {
       const int g = dig[d];
+      allowed = allowed && ((mp.allow[d] >> g) & 1);
       int sI, sO, sW;
       if (kind == AUTODDL_GEMM) { sI = c_gemm_I[g]; sO = c_gemm_O[g]; sW = c_gemm_W[g]; }
       else { sI = sO = c_attn_IO[g]; sW = kB; if (sI < 0) { valid = false; sI = sO = kB; } }
@@ -204,7 +206,7 @@ __device__ __forceinline__ void fill_sig_table(SigInfo (*sig)[Pow<D>::K], const 
     si.a_idx = valid ? a : NS;
     si.b_idx = valid ? b : -1;
     si.db_idx = valid ? dual_vec<D>(b) : -1;
-    si.cfgW = cw; si.cfgO = co; si.valid = valid; si.rowsplit = rs; si.colsplit = cs;
+    si.cfgW = cw; si.cfgO = co; si.valid = valid; si.allowed = allowed; si.rowsplit = rs; si.colsplit = cs;
     sig[kind][j] = si;
   }
 }
@@ -316,7 +318,7 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         }
         mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * (int64_t)rec.eb;
       }
-      const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+      const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
       sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
       const size_t o = (size_t)tile * K + j;
       if (node) node[o] = v;
@@ -792,7 +794,7 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
         }
         mem += (pt.Q[3][si.mI0] * pt.Q[4][si.mI1] + pt.locO[si.cfgO]) * (int64_t)rec.eb;
       }
-      const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+      const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
       pt.VP[vp_j] = v + (ok ? 0 : AUTODDL_PEN);
       const size_t o = (size_t)(tile0 + vp_t) * K + vp_j;
       if (node) node[o] = v;

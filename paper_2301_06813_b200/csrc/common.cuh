@@ -35,6 +35,7 @@ void count_launch(int n = 1);
 struct MeshParams {
   int32_t ndim;
   int32_t size[3];
+  int32_t allow[3];     // signature rows allowed on the level (bit g = row g), 0x3f = all six
   int64_t alpha[3];     // alpha of the level's link class
   int64_t beta[3];      // beta  of the level's link class
   int64_t mem_cap;      // 0 = none
