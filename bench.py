@@ -445,6 +445,11 @@ def run_configs(args):
                 "dp_optimum_ps": int(dp[0][0]), "best_cd_over_dp": float(cd[0].min(dim=1).values.double().div(dp[0].double()).mean()),
                 "best_mh_over_dp": float(mh[0].min(dim=1).values.double().div(dp[0].double()).mean()),
                 "mh": {"nsteps": nsteps, "tau_ps": tau}}
+        if k == 6:                                           # the same chain on the unrestricted six-row space
+            wu = cf.config6_paper_space(restricted=False)
+            Tu, _, _ = adl.build_tables(dl, wu.mesh, wu.net, want_node_mask=False)
+            line["dp_optimum_unrestricted_ps"] = int(adl.chain_dp(Tu, wu.mesh, work=work)[0][0])
+            line["note"] = "rows {0,1,2} per prime sub-level: the paper's factorisation space (27 of 216 signatures)"
         if k != 4:                                           # oracle, one core (config 4's oracle numbers are in the default run)
             mesh, net = ref.mesh_of(w), ref.net_of(w)
             t0 = time.perf_counter(); oT, _, _ = ref.build_tables(w.layers, mesh, net)

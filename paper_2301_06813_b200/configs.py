@@ -221,10 +221,26 @@ def config5_transformer96() -> Workload:
                     Net(ALPHA_PS, (BETA_300, BETA_25), 80 * 10**9), S=1024)
 
 
+PAPER_ROWS = 0x07 << 8   # mesh.link bits 8..13: rows {0, 1, 2} = the paper's SBP matmul factors (R24)
+
+
+def config6_paper_space(restricted: bool = True) -> Workload:
+    """Not in BASELINE.json: the Transformer-24 chain on 4 nodes x 2 GPUs refined into prime sub-levels (2 . 2 | 2) with
+    the matmul rows only -- the paper's own factorisation space: 27 of the 216 signatures."""
+    M, H = 8 * 512, 1024
+    recs = []
+    for _ in range(24):
+        recs += _transformer_block(M, H, 4096, act=2, wgrad=4, wstate=18, attn_rows=8, attn_heads=16)
+    allow = PAPER_ROWS if restricted else 0
+    return Workload("paper-space", _stack(recs), Mesh((2, 2, 2), (INTER | allow, INTER | allow, INTRA | allow)),
+                    Net(ALPHA_PS, (BETA_300, BETA_25), 40 * 10**9), S=64)
+
+
 CONFIGS = {
     1: config1_tiny,
     2: config2_vgg16,
     3: config3_transformer24,
     4: config4_batched,
     5: config5_transformer96,
+    6: config6_paper_space,
 }
