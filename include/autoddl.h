@@ -2,7 +2,7 @@
  * include/autoddl.h -- C-ABI boundary of the B200-native AutoDDL strategy-search hot path.
  *
  * What it computes (citations are lines of the paper text PAPER.md, arxiv 2301.06813; the exact
- * readings R1..R18 are listed in DESIGN.md section 3):
+ * readings R1..R24 are listed in DESIGN.md section 3):
  *   (a1) autoddl_build_tables   SBP cost tables: redistribution cost between every producer-output /
  *        consumer-input signature pair (collectives of Table 2 PAPER.md:102-108,
  *        intra/inter-node link rule PAPER.md:203) + weight-gradient all-reduce
