@@ -457,8 +457,10 @@ __device__ __forceinline__ void dp36_step_blockrows(const int64_t* __restrict__ 
   const int64_t* e0 = ev + (18 * h) * K + col;             // r = 0..5
   const int64_t* e1 = ev + (h ? 6 : 0) * K + col;          // r = 6..11:  h = 1 -> block rows 12..17
   const int64_t* e2 = ev + col;                            // r = 12..17: h = 1 -> block rows 12..17
-  int64_t best = INT64_MAX;
-  int a = 0;
+  // three independent chains of six rows (instruction-level parallelism), merged in row order: strict '<' keeps the
+  // smallest index
+  int64_t pb[3];
+  int pa[3];
 #pragma unroll
   for (int part = 0; part < 3; ++part) {
     int64_t tv[6], fv[6];
@@ -468,12 +470,20 @@ __device__ __forceinline__ void dp36_step_blockrows(const int64_t* __restrict__ 
       tv[r] = e[(6 * part + r) * K];
       fv[r] = fh[6 * part + r];
     }
+    int64_t b = fv[0] + tv[0];
+    int ba = 6 * part;
 #pragma unroll
-    for (int r = 0; r < 6; ++r) {
+    for (int r = 1; r < 6; ++r) {
       const int64_t v = fv[r] + tv[r];
-      if (v < best) { best = v; a = 6 * part + r; }
+      if (v < b) { b = v; ba = 6 * part + r; }
     }
+    pb[part] = b;
+    pa[part] = ba;
   }
+  int64_t best = pb[0];
+  int a = pa[0];
+  if (pb[1] < best) { best = pb[1]; a = pa[1]; }
+  if (pb[2] < best) { best = pb[2]; a = pa[2]; }
   a += 18 * h;
   {
     const int64_t o = __shfl_down_sync(0xffffffffu, best, 16);
