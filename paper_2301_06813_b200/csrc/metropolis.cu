@@ -5,9 +5,11 @@
 // step t come from a counter-based generator (the n-th output of splitmix64), so they are known in advance.
 //
 // One warp per chain; the chain itself is sequential, but its proposals are not: lane k of the warp evaluates
-// step t + k against the state at the start of the window (4 scattered 8-byte loads per lane, all 128 in flight
-// at once), then the warp commits the steps in order: a step stays valid as long as no earlier step of the
-// window changed a layer within distance 1 of its own; the window is cut at the first invalidated step, which is
+// step t + k against the state at the start of the window (two scattered 8-byte loads per lane for the proposed
+// cells, all 64 in flight at once; the two cells of the current state come from a per-layer cache
+// e[l] = T[l][s_{l-1}][s_l] in shared memory, which a committed move refreshes from the cells it has just read), then
+// the warp commits the steps in order: a step stays valid as long as no earlier step of the window changed a layer
+// within distance 1 of its own; the window is cut at the first invalidated step, which is
 // re-evaluated in the next round.  The committed trajectory is exactly the sequential one.
 //
 // The acceptance test is integer only (bit-exact against the oracle): accept iff dC <= 0 or
@@ -60,7 +62,8 @@ metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int 
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int64_t chain = (int64_t)blockIdx.x * kWarps + wib;
   if (chain >= nchains) return;
-  uint8_t* s = smem + (size_t)wib * 2 * L;                 // current strategy [L]
+  int64_t* e = reinterpret_cast<int64_t*>(smem) + (size_t)wib * L;          // e[l] = T[l][s_{l-1}][s_l] of the current state
+  uint8_t* s = smem + (size_t)kWarps * L * 8 + (size_t)wib * 2 * L;         // current strategy [L]
   uint8_t* sb = s + L;                                     // best strategy [L]
   const int64_t* Tp = T + (chain / S) * (int64_t)L * K * K;
 
@@ -72,7 +75,10 @@ metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int 
     sb[l] = (uint8_t)v;
   }
   __syncwarp();
-  for (int l = lane; l < L; l += 32) part += ldg64(Tp + ((int64_t)l * K + (l > 0 ? s[l - 1] : 0)) * K + s[l]);
+  for (int l = lane; l < L; l += 32) {
+    e[l] = ldg64(Tp + ((int64_t)l * K + (l > 0 ? s[l - 1] : 0)) * K + s[l]);
+    part += e[l];
+  }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
   int64_t cur = part, best = part;
@@ -89,12 +95,10 @@ metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int 
     const uint64_t x = (splitmix_nth(seed, base + 3) >> 32) + 1;
     const int old = s[l];
     const int left = l > 0 ? s[l - 1] : 0;
-    const int64_t* row = Tp + ((int64_t)l * K + left) * K;
-    int64_t d = ldg64(row + c) - ldg64(row + old);
-    if (l < L - 1) {
-      const int64_t* nxt = Tp + (int64_t)(l + 1) * K * K + s[l + 1];
-      d += ldg64(nxt + (int64_t)c * K) - ldg64(nxt + (int64_t)old * K);
-    }
+    const int64_t n0 = ldg64(Tp + ((int64_t)l * K + left) * K + c);                       // T[l][s_{l-1}][s']
+    const int64_t n1 = l < L - 1 ? ldg64(Tp + ((int64_t)(l + 1) * K + c) * K + s[l + 1]) : 0;   // T[l+1][s'][s_{l+1}]
+    int64_t d = n0 - e[l];
+    if (l < L - 1) d += n1 - e[l + 1];
     bool acc = d <= 0;
     if (!acc && d < ((int64_t)1 << 45)) acc = tau * neglog_q16(x) >= (d << 16);
     acc = acc && live;
@@ -111,8 +115,13 @@ metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int 
       const int lj = __shfl_sync(0xffffffffu, l, j);
       const int cj = __shfl_sync(0xffffffffu, c, j);
       const int64_t dj = __shfl_sync(0xffffffffu, d, j);
+      const int64_t n0j = __shfl_sync(0xffffffffu, n0, j), n1j = __shfl_sync(0xffffffffu, n1, j);
       cur += dj;
-      if (lane == 0) s[lj] = (uint8_t)cj;
+      if (lane == 0) {
+        s[lj] = (uint8_t)cj;
+        e[lj] = n0j;
+        if (lj < L - 1) e[lj + 1] = n1j;
+      }
       __syncwarp();
       if (cur < best) {                                     // first time this cost is attained
         best = cur;
@@ -151,7 +160,7 @@ int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, cons
   const int64_t nchains = (int64_t)Bp * S;
   if (nchains > 0x3fffffff) { set_error("metropolis: Bp*S too large"); return AUTODDL_EINVAL; }
   if (K > 256) { set_error("metropolis: K must be <= 256"); return AUTODDL_EINVAL; }
-  const size_t smem = ((size_t)kWarps * 2 * L + 15) / 16 * 16;
+  const size_t smem = ((size_t)kWarps * (8 + 2) * L + 15) / 16 * 16;
   if (smem > 200 * 1024) { set_error("metropolis: L too large"); return AUTODDL_EINVAL; }
   if (smem > 48 * 1024)
     ADL_CUDA_CHECK(cudaFuncSetAttribute(metropolis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
