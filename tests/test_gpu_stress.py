@@ -1,0 +1,72 @@
+"""Randomised differential test (`pytest -m gpu`): the one-call path (fused kernel for >= 296 chains, CD resume, class
+representative rows) against the three separate kernels on ALL chains, and against the oracle on a sample, over random
+meshes (1-3 levels, sizes 1..8, random allowed-row masks), chain counts around the fused-kernel thresholds (295/296,
+739/740/741 = resident CTAs), chain lengths around the group size, mixed GEMM / ATTN kinds, split limits, memory caps,
+1-3 starts and sweep caps 1, 2, 3, 64.  Bit-exact.  (A 480-second run of the same generator, ~28,000 cases, is clean.)"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import ref
+from paper_2301_06813_b200 import configs as cf
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def adl():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (no CPU fallback exists)")
+    from paper_2301_06813_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+def test_random_cases(adl, seed):
+    rng = np.random.default_rng(seed)
+    for case in range(150):
+        D = int(rng.choice([1, 2, 2, 2, 3]))
+        sizes = tuple(int(x) for x in rng.choice([1, 2, 3, 4, 5, 8], D))
+        links = tuple(int(rng.integers(0, 2)) | (int(rng.choice([0, 0, 0x07, 0x0b, 0x3e, 0x15])) << 8) for _ in range(D))
+        Bp = int(rng.choice([1, 2, 17, 295, 296, 300, 739, 740, 741, 1481, 2000])) if D == 2 else int(rng.choice([1, 3, 9]))
+        L = int(rng.choice([1, 2, 3, 4, 5, 7, 8, 9, 16, 33, 63, 64, 65]))
+        if D == 3: L = min(L, 9)
+        if Bp * L > 60000: Bp = max(1, 60000 // L)
+        S = int(rng.choice([1, 1, 2, 3]))
+        layers = np.zeros((Bp, L), dtype=cf.LAYER_DTYPE)
+        base = cf.config4_batched(Bp=Bp, L=L, seed=int(rng.integers(0, 1000))).layers
+        layers[:] = base
+        pa = float(rng.choice([0.0, 0.0, 0.3]))
+        if pa > 0:
+            for p in range(min(Bp, 400)):
+                for l in range(L):
+                    if rng.random() < pa:
+                        layers[p, l] = cf.attn(int(layers[p, l]["M"]), int(layers[p, l]["N"]), int(rng.integers(1, 4000)), 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)))
+        if rng.random() < 0.3:
+            layers["max_split_rows"] = rng.integers(1, 40, size=layers.shape)
+            layers["max_split_cols"] = rng.integers(1, 40, size=layers.shape)
+        cap = int(rng.choice([0, 0, 10**7 * L, 10**9 * L]))
+        w = cf.Workload("stress", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), cap), S=S, seed=int(rng.integers(0, 1000)))
+        init = w.cd_init()
+        cap_sw = int(rng.choice([1, 2, 3, 64]))
+        dl = adl.layers_to_device(w.layers)
+        dinit = torch.from_numpy(init).cuda()
+        T, node, mask = adl.build_tables(dl, w.mesh, w.net)
+        work = torch.empty(adl.workspace_bytes(Bp, L, S, w.mesh), dtype=torch.uint8, device="cuda")
+        dc, ds = adl.chain_dp(T, w.mesh, work=work)
+        cc, cs, sw = adl.coord_descent(T, dinit, w.mesh, cap_sw)
+        o = adl.search(dl, w.mesh, w.net, init=dinit, max_sweeps=cap_sw, want_node_mask=True)
+        torch.cuda.synchronize()
+        ok = all(torch.equal(a, b) for a, b in ((o["T"], T), (o["node"], node), (o["mask"], mask), (o["opt_cost"], dc), (o["strategy"], ds),
+                                               (o["cd_cost"], cc), (o["cd_strategy"], cs), (o["cd_sweeps"], sw)))
+        idx = np.unique(rng.integers(0, Bp, min(Bp, 3)))
+        oT, on, om = ref.build_tables(np.ascontiguousarray(w.layers[idx]), ref.mesh_of(w), ref.net_of(w))
+        odc, ods = ref.chain_dp(oT)
+        occ, ocs, osw = ref.coord_descent(oT, np.ascontiguousarray(init[idx]), cap_sw)
+        ok2 = (np.array_equal(T[idx].cpu().numpy(), oT) and np.array_equal(mask[idx].cpu().numpy(), om) and np.array_equal(dc[idx].cpu().numpy(), odc)
+               and np.array_equal(ds[idx].cpu().numpy(), ods) and np.array_equal(cc[idx].cpu().numpy(), occ) and np.array_equal(cs[idx].cpu().numpy(), ocs)
+               and np.array_equal(sw[idx].cpu().numpy(), osw))
+        assert ok and ok2, dict(seed=seed, case=case, sizes=sizes, links=links, Bp=Bp, L=L, S=S, pa=pa, cap=cap, cap_sw=cap_sw,
+                                one_call_equals_separate=ok, separate_equals_oracle=ok2)
