@@ -236,17 +236,41 @@ chain_dp36_kernel(const int64_t* __restrict__ T, int L, int64_t* __restrict__ op
     const int64_t* tile = stage0 + (size_t)s * (SB / 8);
     mbar_wait(&full[s], (b / STAGES) & 1);
 
-    int64_t best0 = INT64_MAX, best1 = INT64_MAX, bestr = INT64_MAX;
-    int a0 = 0, a1 = 0, ar = 0;
+    int64_t best0, best1, bestr = INT64_MAX;
+    int a0, a1, ar = 0;
     const int64_t* trow = tile + (18 * h) * K + 2 * c;
     const int64_t* frow = f + 18 * h;
-#pragma unroll 9
-    for (int r = 0; r < 18; ++r) {
-      const int64_t fi = frow[r];
-      const longlong2 t = *reinterpret_cast<const longlong2*>(trow + r * K);
-      const int64_t v0 = fi + t.x, v1 = fi + t.y;
-      if (v0 < best0) { best0 = v0; a0 = 18 * h + r; }
-      if (v1 < best1) { best1 = v1; a1 = 18 * h + r; }
+    {
+      // three independent chains of six rows per column (instruction-level parallelism; one exposed chain of 18 is what
+      // a single long problem waits for), merged in row order: strict '<' keeps the smallest index
+      int64_t p0[3], p1[3];
+      int q0[3], q1[3];
+#pragma unroll
+      for (int part = 0; part < 3; ++part) {
+        longlong2 t[6];
+        int64_t fi[6];
+#pragma unroll
+        for (int r = 0; r < 6; ++r) {
+          t[r] = *reinterpret_cast<const longlong2*>(trow + (6 * part + r) * K);
+          fi[r] = frow[6 * part + r];
+        }
+        int64_t b0 = fi[0] + t[0].x, b1 = fi[0] + t[0].y;
+        int i0 = 6 * part, i1 = 6 * part;
+#pragma unroll
+        for (int r = 1; r < 6; ++r) {
+          const int64_t v0 = fi[r] + t[r].x, v1 = fi[r] + t[r].y;
+          if (v0 < b0) { b0 = v0; i0 = 6 * part + r; }
+          if (v1 < b1) { b1 = v1; i1 = 6 * part + r; }
+        }
+        p0[part] = b0; q0[part] = i0; p1[part] = b1; q1[part] = i1;
+      }
+      best0 = p0[0]; a0 = q0[0]; best1 = p1[0]; a1 = q1[0];
+      if (p0[1] < best0) { best0 = p0[1]; a0 = q0[1]; }
+      if (p0[2] < best0) { best0 = p0[2]; a0 = q0[2]; }
+      if (p1[1] < best1) { best1 = p1[1]; a1 = q1[1]; }
+      if (p1[2] < best1) { best1 = p1[2]; a1 = q1[2]; }
+      a0 += 18 * h;
+      a1 += 18 * h;
     }
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
