@@ -385,10 +385,11 @@ def run_ours(args):
         kernels["build_dp_cd1_fused"]["hbm_min_frac_of_peak"] = kernels["build_dp_cd1_fused"]["hbm_min_GBps"] / peak
         dom = max(("build_dp_cd1_fused", "coord_descent_resume"), key=lambda n: kernels[n]["ms"])
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")          # per-launch DRAM bytes from the ncu --set full capture
+        tpath = os.path.join(ROOT, "profiles", "traffic_r1.csv")       # per-launch DRAM bytes from the ncu --set full capture
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(dom)
+                rows = dict(l.strip().split(",") for l in open(tpath).read().splitlines()[1:] if l.strip())
+                traffic = float(rows[dom]) if dom in rows else None
             except Exception:
                 traffic = None
         line = {

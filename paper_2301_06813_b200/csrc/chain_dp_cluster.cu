@@ -9,7 +9,8 @@
 //   - the partial (value, row) of column j goes straight into the shared memory of the CTA that owns column j
 //     (j / 27) with st.async over DSMEM, which also completes the transaction count of that CTA's mbarrier;
 //   - 8 lanes per owned column merge the 8 partials with three shuffle steps on (value, row) -- row blocks are
-//     disjoint, so the smaller row wins ties -- and write f_l[27 q + c]: exactly the slice that CTA needs as f_{l-1}[i] for its rows of the next tile.
+//     disjoint, so the smaller row wins ties -- and write f_l[27 q + c]: exactly the slice that CTA needs as
+//     f_{l-1}[i] for its rows of the next tile.
 // One reduce-scatter per layer and no all-gather, no cluster-wide barrier inside the layer loop.  Back-pointers
 // stay in shared memory (27 per layer per CTA), are gathered into CTA 0 at the end and walked there.
 // Results are identical to the definition (R9): every comparison is on (value, smallest row).
