@@ -10,7 +10,8 @@ stand-alone kernels (autoddl_build_tables, autoddl_chain_dp, autoddl_coord_desce
 and reported under "kernels" / "parts" (the three numbers BASELINE.json's metric names).
 Workload: BASELINE.json configs[3] (4096 independent chains x 64 GEMM layers, mesh 4 x 4, K = 36), the
 configuration the metric is quoted on.  Inputs (layer records, CD starts) are resident in HBM for
-`value`; `e2e` goes through autoddl_search_host with pinned HOST buffers (H2D + D2H inside the timed
+`value`; `e2e` goes through autoddl_search_host with pinned HOST buffers (the kernels read the pinned inputs
+over PCIe, results are copied back: host-to-device and device-to-host traffic inside the timed
 region).  `--impl reference` times the CPU oracle (oracle/, plain single-threaded C++) instead.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]

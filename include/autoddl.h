@@ -146,8 +146,10 @@ int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                    const int32_t* d_init, int32_t S, int32_t max_sweeps,
                    int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, void* stream);
 
-/* Whole path with HOST inputs and outputs (the end-to-end call): copies h_layers and h_init to the
- * device, runs (a1) (a2) (a3) in d_work, copies the results back, synchronises `stream`.
+/* Whole path with HOST inputs and outputs (the end-to-end call): brings h_layers and h_init to the device -- inputs in
+ * pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister) are read by the kernels straight over PCIe, once,
+ * overlapped with the table stores; pageable inputs are copied first -- runs (a1) (a2) (a3) in d_work, copies the
+ * results back, synchronises `stream`.
  * Any h_* output may be NULL to skip it; h_init NULL skips (a3). */
 int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
                         const autoddl_mesh* mesh, const autoddl_net* net,

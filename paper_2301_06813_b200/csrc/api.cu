@@ -75,6 +75,17 @@ static inline size_t bp_bytes(int64_t Bp, int64_t L, int64_t K) {
 // tiles of a chain over all SMs) are faster
 static constexpr int32_t kFusedMinChains = 296;
 
+// device-side address of a host pointer that lies in pinned, device-mapped memory (cudaHostAlloc / cudaHostRegister,
+// e.g. a torch pin_memory() tensor); NULL for pageable memory
+static const void* mapped_host_pointer(const void* h) {
+  static const bool off = getenv("AUTODDL_NO_ZERO_COPY") != nullptr;
+  if (off || !h) return nullptr;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, h) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  if (a.type != cudaMemoryTypeHost || a.devicePointer == nullptr) return nullptr;
+  return a.devicePointer;
+}
+
 static int check_device() {
   int n = 0;
   cudaError_t e = cudaGetDeviceCount(&n);
@@ -306,10 +317,24 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
   int64_t* d_cd_cost = (int64_t*)carve((size_t)Bp * S * 8);
   int32_t* d_cd_sweeps = (int32_t*)carve((size_t)Bp * S * 4);
 
-  ADL_CUDA_CHECK(cudaMemcpyAsync(d_layers, h_layers, (size_t)Bp * L * sizeof(autoddl_layer), cudaMemcpyHostToDevice, st));
-  if (do_cd) ADL_CUDA_CHECK(cudaMemcpyAsync(d_init, h_init, (size_t)Bp * S * L * 4, cudaMemcpyHostToDevice, st));
-  if ((rc = search_device(d_layers, Bp, L, mp, K, nullptr, nullptr, nullptr, d_tables, tables_region,
-                          d_opt, d_strategy, do_cd ? d_init : nullptr, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
+  // Inputs in pinned (page-locked, device-mapped) host memory are read by the kernels straight over PCIe: every record
+  // and every start is read once, the reads overlap the table stores, and the explicit copy (0.3 ms for config 4)
+  // disappears.  Pageable inputs are copied first.
+  const autoddl_layer* k_layers = (const autoddl_layer*)mapped_host_pointer(h_layers);
+  if (!k_layers) {
+    ADL_CUDA_CHECK(cudaMemcpyAsync(d_layers, h_layers, (size_t)Bp * L * sizeof(autoddl_layer), cudaMemcpyHostToDevice, st));
+    k_layers = d_layers;
+  }
+  const int32_t* k_init = nullptr;
+  if (do_cd) {
+    k_init = (const int32_t*)mapped_host_pointer(h_init);
+    if (!k_init) {
+      ADL_CUDA_CHECK(cudaMemcpyAsync(d_init, h_init, (size_t)Bp * S * L * 4, cudaMemcpyHostToDevice, st));
+      k_init = d_init;
+    }
+  }
+  if ((rc = search_device(k_layers, Bp, L, mp, K, nullptr, nullptr, nullptr, d_tables, tables_region,
+                          d_opt, d_strategy, k_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
     return rc;
   if (h_opt_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_opt_cost, d_opt, (size_t)Bp * 8, cudaMemcpyDeviceToHost, st));
   if (h_strategy) ADL_CUDA_CHECK(cudaMemcpyAsync(h_strategy, d_strategy, (size_t)Bp * L * 4, cudaMemcpyDeviceToHost, st));

@@ -176,6 +176,22 @@ def test_fused_build_paths_and_search_host(adl):
     out = adl.search_host(w, init, work)
     _assert_same([out["opt_cost"], out["strategy"], out["cd_cost"], out["cd_strategy"], out["cd_sweeps"]], want[3:],
                  names=("dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps"))
+    # pinned (device-mapped) host inputs are read by the kernels straight over PCIe, pageable ones are copied: same results
+    for Bp2 in (9, 700):
+        w2 = cf.config4_batched(Bp=Bp2, L=17, seed=2)
+        init2 = w2.cd_init()
+        want2 = _oracle_all(cf.Workload(w2.name, w2.layers[:9], w2.mesh, w2.net, S=w2.S, seed=2), init2[:9])
+        h_layers = torch.from_numpy(np.ascontiguousarray(w2.layers).view(np.uint8).reshape(Bp2, 17, 64).copy()).pin_memory()
+        h_init = torch.from_numpy(init2.copy()).pin_memory()
+        w_pin = cf.Workload(w2.name, h_layers.numpy().view(cf.LAYER_DTYPE).reshape(Bp2, 17), w2.mesh, w2.net, S=w2.S, seed=2)
+        work2 = torch.empty(adl.workspace_bytes(Bp2, 17, w2.S, w2.mesh), dtype=torch.uint8, device="cuda")
+        pinned = adl.search_host(w_pin, h_init.numpy(), work2)
+        pinned = {k: v.copy() for k, v in pinned.items()}
+        pageable = adl.search_host(w2, init2, work2)
+        for k in pinned:
+            assert np.array_equal(pinned[k], pageable[k]), k
+        _assert_same([pinned[k][:9] for k in ("opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps")], want2[3:],
+                     names=("dp_cost", "dp_strategy", "cd_cost", "cd_strategy", "cd_sweeps"))
     w5 = cf.config5_transformer96()               # back-pointers in the workspace, no CD
     work = torch.empty(adl.workspace_bytes(w5.Bp, w5.L, 0, w5.mesh), dtype=torch.uint8, device="cuda")
     out = adl.search_host(w5, None, work)
