@@ -886,6 +886,177 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
   if (T && tid == ISSUER) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
+// ======================================================================================================
+// K = 216 kernel (three mesh levels): the same idea as the K = 36 kernel at one tile per iteration.
+// A tile has 64 distinct rows (producer classes {0},{1},{3},{2,4,5} per level); the CTA fills EV[64][216] in shared
+// memory (110 KB) and eight threads issue the 216 row copies of 1,728 bytes (cp.async.bulk shared -> global).  The
+// 4096 x 9 slot indices of R[a][b] are decoded once per CTA into a byte table, so the per-tile R step is nine
+// table reads per state pair.  The stores of a tile overlap steps 1-3 of the next one.
+// ======================================================================================================
+struct Smem216 {
+  static constexpr int D = 3, K = 216, NS = 64, NC = 27, ES = NS + 1, NROW = 64, STRIDE = NC + 1;
+  alignas(128) int64_t EV[NROW * K];
+  alignas(16) int64_t E[ES * ES];                       // R[a][b]; row NS and column NS stay 0
+  int64_t TAB[2 * D * STRIDE];                          // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
+  int64_t Q[5][8];
+  int64_t WAR[D][NC];
+  int64_t locW[NC], locO[NC];
+  alignas(16) int64_t VP[K];
+  RecBuf rec[2];
+  SigInfo sig[2][K];
+  int16_t a_rc[2][NROW], da_rc[2][NROW];                // per producer kind: state vector of a row class, and its dual
+  uint8_t slots[NS * NS][3 * D];                        // table entries whose sum is R[a][b]
+};
+
+__global__ void __launch_bounds__(256, 1)
+build_tables216_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
+                       int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  using SM = Smem216;
+  constexpr int D = 3, K = SM::K, NS = SM::NS, NC = SM::NC, ES = SM::ES, NROW = SM::NROW, STRIDE = SM::STRIDE, NT = 256;
+  constexpr int NISS = 8, ISS0 = NT - 32;                  // issuing threads: the first 8 lanes of the last warp
+  extern __shared__ __align__(128) unsigned char smem216_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem216_raw);
+  const int tid = threadIdx.x;
+
+  // ---- once per CTA --------------------------------------------------------------------------------------
+  fill_sig_table<D>(sm.sig, mp, tid, NT);
+  for (int x = tid; x < ES * ES; x += NT) sm.E[x] = 0;
+  if (tid < 2 * D) sm.TAB[tid * STRIDE + NC] = 0;
+  for (int e = tid; e < NS * NS; e += NT) {
+    int idx[3 * D];
+    r_slots<D>(e / NS, e % NS, idx);
+#pragma unroll
+    for (int k = 0; k < 3 * D; ++k) sm.slots[e][k] = (uint8_t)idx[k];
+  }
+  __syncthreads();
+  if (tid < 2 * NROW) {                                    // row class rc = (c0, c1, c2), representative digits = classes
+    const int kind = tid / NROW, rc = tid % NROW;
+    const int i = (rc >> 4) * 36 + ((rc >> 2) & 3) * 6 + (rc & 3);
+    const int a = sm.sig[kind][i].a_idx;
+    sm.a_rc[kind][rc] = (int16_t)a;
+    sm.da_rc[kind][rc] = (int16_t)(a < NS ? dual_vec<D>(a) : NS);
+  }
+  const int q_x = tid >> D, q_m = tid & ((1 << D) - 1);
+  const int role_base = tid < 96 ? 0 : (tid < 192 ? 96 : 192);
+  const int role_i = tid - role_base;
+  const int role_d = role_i / NC, role_cfg = role_i % NC;
+  int role_m0 = 0, role_m1 = 0;
+  cfg_masks<D>(role_cfg, role_m0, role_m1);
+  const int64_t cap_layer = mp.mem_cap / L;
+
+  int tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  auto stage = [&](int b, int tl) {
+    if (tid < 5) {
+      const autoddl_layer* cur = layers + tl;
+      RecBuf* dst = &sm.rec[b];
+      if (tid < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * tid, reinterpret_cast<const unsigned char*>(cur) + 16 * tid);
+      else cp_async4(&dst->kind_prev, &(tl % L > 0 ? cur - 1 : cur)->kind);
+    }
+  };
+  stage(0, tile);
+  cp_async_wait_all();
+  __syncthreads();
+  int buf = 0;
+
+  for (; tile < ntiles; tile += gridDim.x, buf ^= 1) {
+    const int tile_n = tile + gridDim.x;
+    stage(buf ^ 1, tile_n < ntiles ? tile_n : tile);
+    const int l = tile % L;
+    const RecBuf& rec = sm.rec[buf];
+
+    // ---- 1. Q[x][m] -----------------------------------------------------------------------------------------
+    if (tid < (5 << D)) sm.Q[q_x][q_m] = cdiv_magic(rec.X[q_x], (uint32_t)mp.sub[q_m], mp.magic_sub[q_m]);
+    __syncthreads();
+
+    // ---- 2. tables per level and split configuration -------------------------------------------------------
+    if (role_base == 0 && role_i < D * NC) {
+      if (l > 0) {
+        const int d = role_d;
+        const int64_t n = sm.Q[3][role_m0] * sm.Q[4][role_m1] * (int64_t)rec.eb;
+        const int64_t p = mp.size[d];
+        int64_t cg = 0, ca = 0;
+        if (p > 1) {
+          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+        }
+        sm.TAB[d * STRIDE + role_cfg] = cg;
+        sm.TAB[(D + d) * STRIDE + role_cfg] = ca;
+      }
+    } else if (role_base == 96 && role_i < D * NC) {
+      if (rec.kind == AUTODDL_GEMM) {
+        const int d = role_d;
+        const int64_t n = sm.Q[1][role_m0] * sm.Q[2][role_m1] * (int64_t)rec.wgb;
+        const int64_t p = mp.size[d];
+        sm.WAR[d][role_cfg] =
+            p > 1 ? (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d] : 0;
+      }
+    } else if (role_base == 192 && role_i < NC) {
+      sm.locW[role_cfg] = sm.Q[1][role_m0] * sm.Q[2][role_m1];
+      sm.locO[role_cfg] = sm.Q[0][role_m0] * sm.Q[2][role_m1];
+    }
+    __syncthreads();
+
+    // ---- 3. VP[j] and R[a][b] ---------------------------------------------------------------------------------
+    if (tid < K) {
+      const int j = tid;
+      const SigInfo si = sm.sig[rec.kind][j];
+      int64_t v = 0, mem = 0;
+      if (si.valid) {
+        if (rec.kind == AUTODDL_GEMM) {
+#pragma unroll
+          for (int d = 0; d < D; ++d)
+            if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
+          mem = sm.locW[si.cfgW] * (int64_t)rec.wsb;
+        }
+        mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * (int64_t)rec.eb;
+      }
+      const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+      sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+      const size_t o = (size_t)tile * K + j;
+      if (node) node[o] = v;
+      if (mask) mask[o] = ok ? 1 : 0;
+    }
+    for (int e = tid; e < NS * NS; e += NT) {
+      int64_t c = 0;
+      if (l > 0) {
+#pragma unroll
+        for (int k = 0; k < 3 * D; ++k) c += sm.TAB[sm.slots[e][k]];
+      }
+      sm.E[(e / NS) * ES + e % NS] = c;
+    }
+    if (tid >= ISS0 && tid < ISS0 + NISS) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // EV is free again
+    __syncthreads();
+
+    // ---- 4. EV[rc][j] = VP[j] + R[a(rc)][b(j)] + R[dual b(j)][dual a(rc)] ------------------------------------------
+    {
+      const int kind = rec.kind, kind_prev = rec.kind_prev;
+      for (int x = tid; x < NROW * K; x += NT) {
+        const int rc = x / K, j = x % K;
+        int b = sm.sig[kind][j].b_idx, db = sm.sig[kind][j].db_idx;
+        if (b < 0) b = db = NS;
+        const int a = sm.a_rc[kind_prev][rc], da = sm.da_rc[kind_prev][rc];
+        sm.EV[x] = sm.VP[j] + sm.E[a * ES + b] + sm.E[db * ES + da];
+      }
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (tid < 5) cp_async_wait_all();
+    __syncthreads();
+
+    // ---- 5. 216 row copies of 1,728 bytes, 27 per issuing thread ---------------------------------------------------
+    if (tid >= ISS0 && tid < ISS0 + NISS) {
+      int64_t* out = T + (size_t)tile * K * K;
+      for (int i = tid - ISS0; i < K; i += NISS) {
+        const int i0 = i / 36, i1 = (i / 6) % 6, i2 = i % 6;
+        const int rc = (i0 < 4 ? i0 : 2) * 16 + (i1 < 4 ? i1 : 2) * 4 + (i2 < 4 ? i2 : 2);
+        bulk_s2g(out + (size_t)i * K, sm.EV + rc * K, K * 8);
+      }
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+  }
+  if (tid >= ISS0 && tid < ISS0 + NISS) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
 template <int D>
 int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
              int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
@@ -898,6 +1069,20 @@ int launch_d(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams&
   const int per_sm = (D == 3) ? 1 : 4;
   const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;     // persistent, grid-stride over tiles
   build_tables_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+int launch_216(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
+               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
+  const size_t smem = sizeof(Smem216);
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(build_tables216_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int dev = 0, sms = 148;
+  ADL_CUDA_CHECK(cudaGetDevice(&dev));
+  ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int grid = ntiles < sms ? ntiles : sms;                        // persistent, one CTA per SM
+  build_tables216_kernel<<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -942,7 +1127,11 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
   switch (mp.ndim) {
     case 1: return launch_d<1>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     case 2: return launch_36(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
-    case 3: return launch_d<3>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
+    case 3: {
+      static const bool generic = getenv("AUTODDL_BT216_GENERIC") != nullptr;     // debugging switch
+      if (generic) return launch_d<3>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
+      return launch_216(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
+    }
   }
   set_error("ndim must be 1, 2 or 3");
   return AUTODDL_EINVAL;
