@@ -1029,14 +1029,17 @@ build_tables216_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int
     __syncthreads();
 
     // ---- 4. EV[rc][j] = VP[j] + R[a(rc)][b(j)] + R[dual b(j)][dual a(rc)] ------------------------------------------
-    {
-      const int kind = rec.kind, kind_prev = rec.kind_prev;
-      for (int x = tid; x < NROW * K; x += NT) {
-        const int rc = x / K, j = x % K;
-        int b = sm.sig[kind][j].b_idx, db = sm.sig[kind][j].db_idx;
-        if (b < 0) b = db = NS;
+    if (tid < K) {                                         // thread j fills column j of all 64 row classes
+      const int j = tid, kind_prev = rec.kind_prev;
+      int b = sm.sig[rec.kind][j].b_idx, db = sm.sig[rec.kind][j].db_idx;
+      if (b < 0) b = db = NS;                              // invalid consumer signature: zero column
+      const int64_t vp = sm.VP[j];
+      const int64_t* Eb = sm.E + b;
+      const int64_t* Ed = sm.E + db * ES;
+#pragma unroll 8
+      for (int rc = 0; rc < NROW; ++rc) {
         const int a = sm.a_rc[kind_prev][rc], da = sm.da_rc[kind_prev][rc];
-        sm.EV[x] = sm.VP[j] + sm.E[a * ES + b] + sm.E[db * ES + da];
+        sm.EV[rc * K + j] = vp + Eb[a * ES] + Ed[da];
       }
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
