@@ -1097,8 +1097,7 @@ constexpr int kFusePerSM = 5;
 
 int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
-  if (getenv("AUTODDL_BT_VARIANT")) {
-    auto kern = build_tables36_kernel<128, 2, false>;
+  auto kern = build_tables36_kernel<128, 2, false>;
     const size_t smem = sizeof(Smem36<2>);
     const int per = atoi(getenv("AUTODDL_BT_VARIANT"));
     const int ngroups = (ntiles + 1) / 2;
