@@ -1097,15 +1097,6 @@ constexpr int kFusePerSM = 5;
 
 int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
-  auto kern = build_tables36_kernel<128, 2, false>;
-    const size_t smem = sizeof(Smem36<2>);
-    const int per = atoi(getenv("AUTODDL_BT_VARIANT"));
-    const int ngroups = (ntiles + 1) / 2;
-    const int grid = ngroups < 148 * per ? ngroups : 148 * per;
-    kern<<<grid, 128, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr, nullptr, 0, nullptr);
-    count_launch();
-    return AUTODDL_OK;
-  }
   auto kern = build_tables36_kernel<kNT, kG, false>;
   const size_t smem = sizeof(Smem36<kG>);
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
