@@ -90,22 +90,58 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   }
   __syncwarp();
 
+  // The column T[l+1][.][s_{l+1}] of an update is known long before the update runs (s_{l+1} is not touched before
+  // layer l+1's own turn), the row T[l][s_{l-1}][.] only when layer l-1 is done.  So the column gather of the NEXT dirty
+  // layer is issued before the argmin of the current one and only the contiguous row read stays on the dependent
+  // chain.  If the current update changes its layer, layer l+1 becomes dirty and runs next: a prefetch made for a
+  // later layer is then dropped.  (Reading the next row speculatively as well was measured and costs more than it saves.)
+  auto next_dirty = [&](int from) {
+    int l = from;
+    while (l < L && !dirty[l]) ++l;
+    return l;
+  };
+  auto load_row = [&](int l, int64_t (&rv)[NCAND]) {
+    const int64_t* row = Tp + ((size_t)l * K + (l > 0 ? s[l - 1] : 0)) * K;
+#pragma unroll
+    for (int q = 0; q < NCAND; ++q) {
+      const int c = 32 * q + lane;
+      rv[q] = c < K ? __ldg(row + c) : 0;
+    }
+  };
+  auto load_col = [&](int l, int64_t (&cv)[NCAND]) {
+    const bool has_right = l < L - 1;
+    const int64_t* col = Tp + (size_t)(l + 1) * K * K + (has_right ? s[l + 1] : 0);
+#pragma unroll
+    for (int q = 0; q < NCAND; ++q) {
+      const int c = 32 * q + lane;
+      cv[q] = (has_right && c < K) ? ldg_narrow(col + (size_t)rep[q] * K) : 0;
+    }
+  };
   for (; !resume_done;) {
     bool changed = false;
-    for (int l = 0; l < L; ++l) {
-      if (!dirty[l]) continue;                               // warp-uniform
-      const int left = l > 0 ? s[l - 1] : 0;
-      const bool has_right = l < L - 1;
-      const int64_t* row = Tp + ((size_t)l * K + left) * K;
-      const int64_t* col = Tp + (size_t)(l + 1) * K * K + (has_right ? s[l + 1] : 0);
+    int l = next_dirty(0);
+    int64_t cvp[NCAND];                                      // prefetched column of layer pf
+    int pf = -1;
+    if (l < L) { load_col(l, cvp); pf = l; }
+    while (l < L) {
+      int64_t cv[NCAND], rv[NCAND];
+      if (pf == l) {
+#pragma unroll
+        for (int q = 0; q < NCAND; ++q) cv[q] = cvp[q];
+      } else {
+        load_col(l, cv);
+      }
+      load_row(l, rv);
+      int l2 = next_dirty(l + 1);
+      pf = -1;
+      if (l2 < L) { load_col(l2, cvp); pf = l2; }            // in flight during this layer's argmin
       int64_t bv = INT64_MAX;
       int bi = K;
 #pragma unroll
       for (int q = 0; q < NCAND; ++q) {
         const int c = 32 * q + lane;
         if (c < K) {
-          int64_t g = __ldg(row + c);
-          if (has_right) g += ldg_narrow(col + (size_t)rep[q] * K);
+          const int64_t g = rv[q] + cv[q];
           if (g < bv) { bv = g; bi = c; }
         }
       }
@@ -117,11 +153,15 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
         if (bi != old) {
           s[l] = bi;
           if (l > 0) dirty[l - 1] = 1;
-          if (has_right) dirty[l + 1] = 1;
+          if (l < L - 1) dirty[l + 1] = 1;
         }
       }
-      changed |= (bi != old);
       __syncwarp();
+      if (bi != old) {
+        changed = true;
+        if (l + 1 < L) l2 = l + 1;                           // now dirty: it runs next (its column prefetch exists iff pf == l + 1)
+      }
+      l = l2;
     }
     ++nsweeps;
     if (!changed || nsweeps >= max_sweeps) break;
