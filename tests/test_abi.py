@@ -99,3 +99,17 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".cpp", ".h")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "binding" not in text and "libautoddl.so" not in text and "include/autoddl.h" not in text, f
+
+
+def test_header_is_plain_c(tmp_path):
+    """the boundary is a C ABI: include/autoddl.h compiles as C99 with no torch / C++ types"""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "h.c"
+    src.write_text('#include "include/autoddl.h"\nint main(void) { return (int)sizeof(autoddl_layer) - 64; }\n')
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", ROOT, "-c", str(src), "-o", str(tmp_path / "h.o")],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
