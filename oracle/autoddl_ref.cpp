@@ -222,7 +222,9 @@ extern "C" int autoddl_ref_build_tables(const ref_layer* layers, int32_t Bp, int
         if (mask) mask[(p * L + l) * K + j] = (uint8_t)ok;
         for (int i = 0; i < K; ++i) {
           const int64_t e = prev ? autoddl_ref_edge_cost(prev, cur, i, j, mesh, net) : 0;
-          tile[(int64_t)i * K + j] = e + v + (ok ? 0 : REF_PEN);
+          // R25: redistributions once per micro-batch, weight-gradient synchronisation once per mini-batch
+          const int64_t m = net->micro_batches > 1 ? net->micro_batches : 1;
+          tile[(int64_t)i * K + j] = m * e + v + (ok ? 0 : REF_PEN);
         }
       }
     }

@@ -48,7 +48,9 @@ typedef struct {
 
 /* link[d]: bit 0 = 0 intra / 1 inter; bits 8..13 = allowed signature rows of the level (bit g = row g; 0 = all six) */
 typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } ref_mesh;
-typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; } ref_net;
+/* micro_batches: gradient accumulation: the activation redistributions run once per micro-batch,
+ * the weight-gradient synchronisation once per mini-batch; 0 or 1 = no accumulation (R25) */
+typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; int64_t micro_batches; } ref_net;
 
 #define REF_PEN ((int64_t)1 << 50)
 

@@ -30,7 +30,8 @@ class RefMesh(C.Structure):
 
 
 class RefNet(C.Structure):
-    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64)]
+    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64),
+                ("micro_batches", C.c_int64)]
 
 
 _lib = None
@@ -89,11 +90,12 @@ def make_mesh(size, link) -> RefMesh:
     return m
 
 
-def make_net(alpha_ps, beta_ps_per_byte, mem_cap_bytes=0) -> RefNet:
+def make_net(alpha_ps, beta_ps_per_byte, mem_cap_bytes=0, micro_batches=1) -> RefNet:
     n = RefNet()
     n.alpha_ps[0], n.alpha_ps[1] = int(alpha_ps[0]), int(alpha_ps[1])
     n.beta_ps_per_byte[0], n.beta_ps_per_byte[1] = int(beta_ps_per_byte[0]), int(beta_ps_per_byte[1])
     n.mem_cap_bytes = int(mem_cap_bytes)
+    n.micro_batches = int(micro_batches)
     return n
 
 
@@ -110,7 +112,7 @@ def mesh_of(w) -> RefMesh:
 
 
 def net_of(w) -> RefNet:
-    return make_net(w.net.alpha_ps, w.net.beta_ps_per_byte, w.net.mem_cap_bytes)
+    return make_net(w.net.alpha_ps, w.net.beta_ps_per_byte, w.net.mem_cap_bytes, getattr(w.net, "micro_batches", 1))
 
 
 # ---- scalar pieces (for the pins) -------------------------------------------------------------

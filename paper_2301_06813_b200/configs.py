@@ -81,6 +81,7 @@ class Net:
     alpha_ps: tuple = ALPHA_PS               # (intra, inter)
     beta_ps_per_byte: tuple = (BETA_300, BETA_25)
     mem_cap_bytes: int = 0                   # 0 = no cap
+    micro_batches: int = 1                   # gradient accumulation: redistributions per weight-gradient synchronisation
 
 
 @dataclass

@@ -15,7 +15,7 @@ DRIVER = r'''
 #include "autoddl_ref.h"
 int main() {
   ref_mesh mesh{3, {2, 3, 2}, {1, 1, 0}};
-  ref_net net{{5000000, 20000000}, {3, 40}, 3000000};
+  ref_net net{{5000000, 20000000}, {3, 40}, 3000000, 3};
   const int L = 3, Bp = 2, K = autoddl_ref_num_signatures(&mesh), S = 2;
   std::vector<ref_layer> layers(Bp * L);
   for (int i = 0; i < Bp * L; ++i) {
