@@ -2,7 +2,7 @@
  * include/autoddl.h -- C-ABI boundary of the B200-native AutoDDL strategy-search hot path.
  *
  * What it computes (citations are lines of the paper text PAPER.md, arxiv 2301.06813; the exact
- * readings R1..R24 are listed in DESIGN.md section 3):
+ * readings R1..R25 are listed in DESIGN.md section 3):
  *   (a1) autoddl_build_tables   SBP cost tables: redistribution cost between every producer-output /
  *        consumer-input signature pair (collectives of Table 2 PAPER.md:102-108,
  *        intra/inter-node link rule PAPER.md:203) + weight-gradient all-reduce
@@ -68,8 +68,11 @@ typedef struct {
  * disallowed signatures are infeasible (penalty 2^50, mask 0).  K stays 6^ndim. */
 typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } autoddl_mesh;
 
-/* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap. */
-typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; } autoddl_net;
+/* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap.
+ * micro_batches: gradient accumulation: the activation redistributions of a cell are paid once per
+ * micro-batch, the weight-gradient all-reduce once per mini-batch: T = m * edge + node + penalty; 0 or 1 = none.
+ * Must be < 2^20.  48 bytes. */
+typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; int64_t micro_batches; } autoddl_net;
 
 /* K = 6^ndim, or AUTODDL_EINVAL. Host only. */
 int autoddl_num_signatures(const autoddl_mesh* mesh);

@@ -33,7 +33,8 @@ class CMesh(C.Structure):
 
 
 class CNet(C.Structure):
-    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64)]
+    _fields_ = [("alpha_ps", C.c_int64 * 2), ("beta_ps_per_byte", C.c_int64 * 2), ("mem_cap_bytes", C.c_int64),
+                ("micro_batches", C.c_int64)]
 
 
 _lib = None
@@ -100,6 +101,7 @@ def c_net(net) -> CNet:
         n.alpha_ps[c] = int(net.alpha_ps[c])
         n.beta_ps_per_byte[c] = int(net.beta_ps_per_byte[c])
     n.mem_cap_bytes = int(net.mem_cap_bytes)
+    n.micro_batches = int(getattr(net, "micro_batches", 1))
     return n
 
 

@@ -53,12 +53,14 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
                   "net.beta_ps_per_byte[%d] out of range", c);
     }
     ADL_REQUIRE(net->mem_cap_bytes >= 0, "net.mem_cap_bytes < 0");
+    ADL_REQUIRE(net->micro_batches >= 0 && net->micro_batches < (1 << 20), "net.micro_batches out of range");
     if (out) {
       for (int d = 0; d < mesh->ndim; ++d) {
         out->alpha[d] = net->alpha_ps[mesh->link[d] & 1];
         out->beta[d] = net->beta_ps_per_byte[mesh->link[d] & 1];
       }
       out->mem_cap = net->mem_cap_bytes;
+      out->accum = net->micro_batches > 1 ? net->micro_batches : 1;
     }
   }
   return AUTODDL_OK;

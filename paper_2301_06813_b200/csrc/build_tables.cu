@@ -285,8 +285,8 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
         const int64_t p = mp.size[d];
         int64_t cg = 0, ca = 0;
         if (p > 1) {
-          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+          cg = mp.accum * ((p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]));
+          ca = mp.accum * ((p - 1) * mp.alpha[d] + n * mp.beta[d]);      // R25: once per micro-batch
         }
         sm.CG[d][role_cfg] = cg;
         sm.CA[d][role_cfg] = ca;
@@ -768,8 +768,8 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
           const int64_t p = mp.size[d];
           int64_t cg = 0, ca = 0;
           if (p > 1) {
-            cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-            ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+            cg = mp.accum * ((p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]));
+            ca = mp.accum * ((p - 1) * mp.alpha[d] + n * mp.beta[d]);      // R25: once per micro-batch
           }
           pt.TAB[d * STRIDE + role_cfg] = cg;
           pt.TAB[(D + d) * STRIDE + role_cfg] = ca;
@@ -977,8 +977,8 @@ build_tables216_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int
         const int64_t p = mp.size[d];
         int64_t cg = 0, ca = 0;
         if (p > 1) {
-          cg = (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-          ca = (p - 1) * mp.alpha[d] + n * mp.beta[d];
+          cg = mp.accum * ((p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]));
+          ca = mp.accum * ((p - 1) * mp.alpha[d] + n * mp.beta[d]);      // R25: once per micro-batch
         }
         sm.TAB[d * STRIDE + role_cfg] = cg;
         sm.TAB[(D + d) * STRIDE + role_cfg] = ca;

@@ -39,6 +39,7 @@ struct MeshParams {
   int64_t alpha[3];     // alpha of the level's link class
   int64_t beta[3];      // beta  of the level's link class
   int64_t mem_cap;      // 0 = none
+  int64_t accum;        // micro-batches per mini-batch (>= 1): multiplies the redistribution costs
   int32_t sub[8];       // product of the sizes of the levels in subset m (bit e = level e)
   uint64_t magic_sub[8];   // ceil(2^64 / sub[m])
   uint64_t magic_size[3];  // ceil(2^64 / size[d])
