@@ -2,7 +2,7 @@
 representative rows) against the three separate kernels on ALL chains, and against the oracle on a sample, over random
 meshes (1-3 levels, sizes 1..8, random allowed-row masks), chain counts around the fused-kernel thresholds (295/296,
 739/740/741 = resident CTAs), chain lengths around the group size, mixed GEMM / ATTN kinds, split limits, memory caps,
-1-3 starts and sweep caps 1, 2, 3, 64.  Bit-exact.  (A 480-second run of the same generator, ~28,000 cases, is clean.)"""
+1-3 starts, sweep caps 1, 2, 3, 64 and 0-17 micro-batches.  Bit-exact.  (A 480-second run of the same generator, ~28,000 cases, is clean.)"""
 import numpy as np
 import pytest
 
@@ -48,7 +48,7 @@ def test_random_cases(adl, seed):
             layers["max_split_rows"] = rng.integers(1, 40, size=layers.shape)
             layers["max_split_cols"] = rng.integers(1, 40, size=layers.shape)
         cap = int(rng.choice([0, 0, 10**7 * L, 10**9 * L]))
-        w = cf.Workload("stress", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), cap), S=S, seed=int(rng.integers(0, 1000)))
+        w = cf.Workload("stress", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), cap, micro_batches=int(rng.choice([0, 1, 1, 3, 17]))), S=S, seed=int(rng.integers(0, 1000)))
         init = w.cd_init()
         cap_sw = int(rng.choice([1, 2, 3, 64]))
         dl = adl.layers_to_device(w.layers)
