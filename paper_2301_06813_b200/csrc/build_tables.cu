@@ -506,7 +506,7 @@ __device__ __forceinline__ void dp36_step_blockrows(const int64_t* __restrict__ 
 
 // NT builder threads, G tiles per group.  FUSE: one extra warp runs the chain DP (R9) on every tile
 // straight from shared memory while the tile is being stored, so the optimum costs no table read at all.
-template <int NT, int G, bool FUSE>
+template <int NT, int G, bool FUSE, bool CD1 = false>
 __global__ void __launch_bounds__(FUSE ? NT + 32 : NT, FUSE ? 5 : 768 / NT)
 build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
                       int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
@@ -609,12 +609,37 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
             for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)sc.p * cd_S * L + x];
           }
         } else {
+          // CD1 (one start per chain): the argmin of layer l-1's update is independent of the DP step of tile l, so it
+          // is computed in the same straight-line code and its shuffle / compare chain interleaves with the DP scan
+          int64_t cbv = INT64_MAX;
+          int cbi = K;
+          if (CD1) {
+            const int left = l > 1 ? cd_s[l - 2] : 0, right = cd_s[l];
+            const int64_t* row = ev_prev + block_row_of(left) * K;
+#pragma unroll
+            for (int c0 = 0; c0 < 64; c0 += 32) {
+              const int c = c0 + lane;
+              if (c < K) {
+                const int64_t g = row[c] + ev[(c < 24 ? c : (c < 30 ? c - 12 : c - 18)) * K + right];
+                if (g < cbv) { cbv = g; cbi = c; }
+              }
+            }
+          }
           dp36_step_blockrows(ev, sm.f[cur], fn, bp + (size_t)l * K, sm.repcol[kind], sm.repof[kind], lane);
+          if (CD1) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+              const int64_t ov = __shfl_xor_sync(0xffffffffu, cbv, off);
+              const int oi = __shfl_xor_sync(0xffffffffu, cbi, off);
+              if (ov < cbv || (ov == cbv && oi < cbi)) { cbv = ov; cbi = oi; }
+            }
+            if (lane == 0) cd_s[l - 1] = (uint8_t)cbi;
+          }
         }
         cur ^= 1;
         __syncwarp();
         if (cd) {
-          if (l > 0) cd_update(l - 1, ev_prev, ev);
+          if (l > 0 && !CD1) cd_update(l - 1, ev_prev, ev);
           if (l == L - 1) {
             cd_update(l, ev, nullptr);
             for (int x = lane; x < cd_S * L; x += 32) cd_s1[(size_t)sc.p * cd_S * L + x] = cd_s[x];
@@ -1155,7 +1180,7 @@ int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   if (!fused_build_dp_supported(mp, L)) { set_error("fused build+DP needs a 2-level mesh"); return AUTODDL_EINVAL; }
   if (d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
-  auto kern = build_tables36_kernel<kFuseNT, kFuseG, true>;
+  auto kern = (d_cd_init && S == 1) ? build_tables36_kernel<kFuseNT, kFuseG, true, true> : build_tables36_kernel<kFuseNT, kFuseG, true, false>;
   if (d_cd_init && (!fused_cd_sweep_supported(L, S) || d_cd_s1 == nullptr)) { set_error("fused CD sweep: S * L too large"); return AUTODDL_EINVAL; }
   const size_t smem = (sizeof(Smem36<kFuseG>) + (d_cd_init ? (size_t)S * L : 0) + 127) / 128 * 128;
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
