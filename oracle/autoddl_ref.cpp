@@ -27,11 +27,37 @@ const int32_t ATTN_IO[6]    = {REF_S0, REF_S1, -1, REF_B, -1, -1};
 
 inline int ipow6(int d) { int k = 1; for (int t = 0; t < d; ++t) k *= 6; return k; }
 
-// digit of level d in signature index j, level 0 most significant
-inline int sig_digit(int j, int d, int D) {
+// rows a level admits: bits 8..13 of link[d], bit g = row g; 0 = all six (R24)
+inline int level_allow(const ref_mesh* mesh, int d) {
+  const int a = (mesh->link[d] >> 8) & 0x3f;
+  return a ? a : 0x3f;
+}
+inline int level_nrows(const ref_mesh* mesh, int d) {
+  int n = 0;
+  for (int g = 0; g < 6; ++g) n += (level_allow(mesh, d) >> g) & 1;
+  return n;
+}
+
+// per-level row of level d in signature index j, level 0 most significant.
+// ndim <= 3: j is a base-6 number over all six rows (a disallowed row makes the signature infeasible, R24).
+// ndim  > 3: j is a mixed-radix number over the ALLOWED rows only (R26): the digit x of level d is the x-th allowed
+//            row of that level in increasing order; the radix of level d is its number of allowed rows.
+inline int sig_digit(int j, int d, const ref_mesh* mesh) {
+  const int D = mesh->ndim;
+  if (D <= 3) {
+    int div = 1;
+    for (int t = 0; t < D - 1 - d; ++t) div *= 6;
+    return (j / div) % 6;
+  }
   int div = 1;
-  for (int t = 0; t < D - 1 - d; ++t) div *= 6;
-  return (j / div) % 6;
+  for (int t = d + 1; t < D; ++t) div *= level_nrows(mesh, t);
+  int x = (j / div) % level_nrows(mesh, d);
+  for (int g = 0; g < 6; ++g)
+    if ((level_allow(mesh, d) >> g) & 1) {
+      if (x == 0) return g;
+      --x;
+    }
+  return -1;                                  // not reached
 }
 
 inline int32_t dual_state(int32_t s) {   // R9: S0->S0, S1->S1, B->P, P->B
@@ -43,8 +69,11 @@ inline int32_t dual_state(int32_t s) {   // R9: S0->S0, S1->S1, B->P, P->B
 }  // namespace
 
 extern "C" int autoddl_ref_num_signatures(const ref_mesh* mesh) {
-  if (!mesh || mesh->ndim < 1 || mesh->ndim > 3) return -1;
-  return ipow6(mesh->ndim);
+  if (!mesh || mesh->ndim < 1 || mesh->ndim > REF_MAX_LEVELS) return -1;
+  if (mesh->ndim <= 3) return ipow6(mesh->ndim);
+  int64_t k = 1;                              // R26: product of the levels' allowed-row counts, at most 256
+  for (int d = 0; d < mesh->ndim; ++d) k *= level_nrows(mesh, d);
+  return k <= 256 ? (int)k : -1;
 }
 
 extern "C" int autoddl_ref_sig_states(int kind, int sig, const ref_mesh* mesh,
@@ -52,7 +81,7 @@ extern "C" int autoddl_ref_sig_states(int kind, int sig, const ref_mesh* mesh,
   const int D = mesh->ndim;
   int valid = 1;
   for (int d = 0; d < D; ++d) {
-    const int g = sig_digit(sig, d, D);
+    const int g = sig_digit(sig, d, mesh);
     if (kind == REF_GEMM) {
       I[d] = GEMM_I[g]; W[d] = GEMM_W[g]; O[d] = GEMM_O[g];
     } else {
@@ -94,7 +123,7 @@ extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
                                        const int32_t* a, const int32_t* b,
                                        const ref_mesh* mesh, const ref_net* net) {
   const int D = mesh->ndim;
-  int32_t cur[3];
+  int32_t cur[REF_MAX_LEVELS];
   for (int d = 0; d < D; ++d) cur[d] = a[d];
   int64_t cost = 0;
 
@@ -145,11 +174,11 @@ extern "C" int64_t autoddl_ref_reshard(int64_t rows, int64_t cols, int64_t eb,
 // "in both the forward path and the backward path").  The tensor is the consumer's input.
 extern "C" int64_t autoddl_ref_edge_cost(const ref_layer* prev, const ref_layer* cur, int i, int j,
                                          const ref_mesh* mesh, const ref_net* net) {
-  int32_t Ii[3], Wi[3], Oi[3], Ij[3], Wj[3], Oj[3];
+  int32_t Ii[REF_MAX_LEVELS], Wi[REF_MAX_LEVELS], Oi[REF_MAX_LEVELS], Ij[REF_MAX_LEVELS], Wj[REF_MAX_LEVELS], Oj[REF_MAX_LEVELS];
   const int vi = autoddl_ref_sig_states(prev->kind, i, mesh, Ii, Wi, Oi);
   const int vj = autoddl_ref_sig_states(cur->kind, j, mesh, Ij, Wj, Oj);
   if (!vi || !vj) return 0;
-  int32_t da[3], db[3];
+  int32_t da[REF_MAX_LEVELS], db[REF_MAX_LEVELS];
   for (int d = 0; d < mesh->ndim; ++d) { da[d] = dual_state(Oi[d]); db[d] = dual_state(Ij[d]); }
   const int64_t fwd = autoddl_ref_reshard(cur->in_rows, cur->in_cols, cur->act_bytes, Oi, Ij, mesh, net);
   const int64_t bwd = autoddl_ref_reshard(cur->in_rows, cur->in_cols, cur->act_bytes, db, da, mesh, net);
@@ -160,7 +189,7 @@ extern "C" int64_t autoddl_ref_edge_cost(const ref_layer* prev, const ref_layer*
 // replicated (B) all-reduces the local weight gradient.
 extern "C" int64_t autoddl_ref_node_cost(const ref_layer* cur, int j, const ref_mesh* mesh, const ref_net* net) {
   if (cur->kind != REF_GEMM) return 0;
-  int32_t I[3], W[3], O[3];
+  int32_t I[REF_MAX_LEVELS], W[REF_MAX_LEVELS], O[REF_MAX_LEVELS];
   if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
   const int64_t nw = autoddl_ref_local_size(cur->Kd, cur->N, W, mesh);
   int64_t v = 0;
@@ -175,7 +204,7 @@ extern "C" int64_t autoddl_ref_node_cost(const ref_layer* cur, int j, const ref_
 // ---- R7: per-device memory of one layer under signature j (PARITY UNPINNED: PAPER.md:221-223
 // uses a OneFlow CPU dry run and prints no formula; this one is ours).
 extern "C" int64_t autoddl_ref_layer_mem(const ref_layer* cur, int j, const ref_mesh* mesh) {
-  int32_t I[3], W[3], O[3];
+  int32_t I[REF_MAX_LEVELS], W[REF_MAX_LEVELS], O[REF_MAX_LEVELS];
   if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
   int64_t mem = 0;
   if (cur->kind == REF_GEMM) mem += autoddl_ref_local_size(cur->Kd, cur->N, W, mesh) * cur->wstate_bytes;
@@ -185,14 +214,13 @@ extern "C" int64_t autoddl_ref_layer_mem(const ref_layer* cur, int j, const ref_
 }
 
 extern "C" int autoddl_ref_feasible(const ref_layer* cur, int j, int32_t L, const ref_mesh* mesh, const ref_net* net) {
-  int32_t I[3], W[3], O[3];
+  int32_t I[REF_MAX_LEVELS], W[REF_MAX_LEVELS], O[REF_MAX_LEVELS];
   if (!autoddl_ref_sig_states(cur->kind, j, mesh, I, W, O)) return 0;
   // R24: a level may restrict its signature rows (bits 8..13 of link[d], 0 = all six).  Rows {0,1,2} on every level
   // of a mesh refined into prime sub-levels is the paper's own factorisation space.
-  for (int d = mesh->ndim - 1, r = j; d >= 0; --d, r /= 6) {
-    const int allow = (mesh->link[d] >> 8) & 0x3f;
-    if (allow != 0 && !((allow >> (r % 6)) & 1)) return 0;
-  }
+  // (with more than three levels the signature index runs over allowed rows only, R26: nothing to exclude)
+  for (int d = 0; d < mesh->ndim; ++d)
+    if (!((level_allow(mesh, d) >> sig_digit(j, d, mesh)) & 1)) return 0;
   int64_t rowsplit = 1, colsplit = 1;
   for (int d = 0; d < mesh->ndim; ++d) {
     if (I[d] == REF_S0 || O[d] == REF_S0) rowsplit *= mesh->size[d];

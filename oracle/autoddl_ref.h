@@ -17,6 +17,8 @@
  *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours)
  *   chain DP optimum (PAPER.md:225 exhaustive)     pinned  (brute force over K^L)
  *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
+ *   four / five mesh levels    pinned  (size-1 levels reproduce the three-level tables, decode order,
+ *                                                  data-parallel closed form, intra-node gather, brute force at K = 81)
  *   Metropolis-Hastings         pinned  (Boltzmann stationary law on enumerable chains, greedy and
  *                                                  hot limits, integer -ln against libm, replay of a hand-checked chain)
  */
@@ -47,14 +49,16 @@ typedef struct {
 } ref_layer;                 /* 64 bytes */
 
 /* link[d]: bit 0 = 0 intra / 1 inter; bits 8..13 = allowed signature rows of the level (bit g = row g; 0 = all six) */
-typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } ref_mesh;
+#define REF_MAX_LEVELS 5
+typedef struct { int32_t ndim; int32_t size[REF_MAX_LEVELS]; int32_t link[REF_MAX_LEVELS]; } ref_mesh;
 /* micro_batches: gradient accumulation: the activation redistributions run once per micro-batch,
  * the weight-gradient synchronisation once per mini-batch; 0 or 1 = no accumulation (R25) */
 typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; int64_t micro_batches; } ref_net;
 
 #define REF_PEN ((int64_t)1 << 50)
 
-/* 6^ndim signatures per layer */
+/* signatures per layer: 6^ndim for ndim <= 3; for ndim = 4, 5 the product of the levels' allowed-row counts
+ * (<= 256, else -1): there the signature index is a mixed-radix number over the allowed rows only (R26) */
 int autoddl_ref_num_signatures(const ref_mesh* mesh);
 
 /* Table 2. which: 0 AllGather, 1 ReduceScatter, 2 AllReduce, 3 AlltoAll */

@@ -26,7 +26,7 @@ def build(force: bool = False) -> str:
 
 
 class RefMesh(C.Structure):
-    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 3), ("link", C.c_int32 * 3)]
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 5), ("link", C.c_int32 * 5)]
 
 
 class RefNet(C.Structure):
@@ -119,6 +119,11 @@ def net_of(w) -> RefNet:
 AG, RS, AR, A2A = 0, 1, 2, 3
 
 
+def num_signatures(mesh: RefMesh) -> int:
+    """K: 6^ndim for ndim <= 3; the product of the levels' allowed-row counts for ndim = 4, 5 (R26)"""
+    return int(lib().autoddl_ref_num_signatures(C.addressof(mesh)))
+
+
 def collective(which, n, p, alpha, beta) -> int:
     return int(lib().autoddl_ref_collective(which, n, p, alpha, beta))
 
@@ -129,7 +134,7 @@ def local_size(R, Cc, st, mesh: RefMesh) -> int:
 
 
 def sig_states(kind, sig, mesh: RefMesh):
-    I = np.zeros(3, np.int32); W = np.zeros(3, np.int32); O = np.zeros(3, np.int32)
+    I = np.zeros(5, np.int32); W = np.zeros(5, np.int32); O = np.zeros(5, np.int32)
     v = lib().autoddl_ref_sig_states(kind, sig, C.addressof(mesh), _p(I), _p(W), _p(O))
     D = mesh.ndim
     return int(v), tuple(I[:D].tolist()), tuple(W[:D].tolist()), tuple(O[:D].tolist())
@@ -165,7 +170,7 @@ def build_tables(layers: np.ndarray, mesh: RefMesh, net: RefNet):
     """layers: LAYER_DTYPE [Bp, L] -> T int64 [Bp,L,K,K], node int64 [Bp,L,K], mask uint8 [Bp,L,K]"""
     layers = np.ascontiguousarray(layers)
     Bp, L = layers.shape
-    K = 6 ** mesh.ndim
+    K = num_signatures(mesh)
     T = np.empty((Bp, L, K, K), np.int64)
     node = np.empty((Bp, L, K), np.int64)
     mask = np.empty((Bp, L, K), np.uint8)
