@@ -21,7 +21,7 @@
  *     nothing and never synchronise.  autoddl_search_host synchronises `stream` before returning.
  *   - Layouts are dense row-major:  T[Bp][L][K][K] (i = producer signature = row, j = consumer
  *     signature = column), node[Bp][L][K], mask[Bp][L][K], strategy[Bp][L], init[Bp][S][L],
- *     cd_strategy[Bp][S][L], cd_cost[Bp][S], cd_sweeps[Bp][S].   K = 6^ndim.
+ *     cd_strategy[Bp][S][L], cd_cost[Bp][S], cd_sweeps[Bp][S].   K = autoddl_num_signatures(mesh).
  *   - d_T must be 16-byte aligned; all other pointers naturally aligned.
  *   - Return value: 0 success, AUTODDL_EINVAL (-1) bad argument, AUTODDL_ECUDA (-2) CUDA runtime
  *     error, AUTODDL_EWORK (-3) workspace too small.  Text via autoddl_last_error() (thread-local).
@@ -65,8 +65,13 @@ typedef struct {
  * (0 split rows, 1 split columns, 2 split the reduction dim, 3 replicate, 4 partial input, 5 partial weight); 0 = all
  * six.  With 0x07 << 8 on every level of a mesh refined into prime sub-levels the feasible strategies are exactly the
  * paper's SBP matmul factorisations I = (S0:p0, B:p1, S1:p2), W = (B, S1, S0), O = (S0, S1, P);
- * disallowed signatures are infeasible (penalty 2^50, mask 0).  K stays 6^ndim. */
-typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } autoddl_mesh;
+ * disallowed signatures are infeasible (penalty 2^50, mask 0).  For ndim <= 3, K stays 6^ndim.
+ * ndim = 4, 5 (R26; 2 nodes x 8 GPUs = 2 | 2.2.2, the paper's 2 x 16 GPUs = 2 | 2.2.2.2): the
+ * signature index runs over the ALLOWED rows only, a mixed-radix number with level 0 most significant whose digit x
+ * on level d names the x-th allowed row of that level in increasing order; K = product of the levels' allowed-row
+ * counts and must be <= 256 (81 / 243 with 0x07 << 8 on every level). */
+#define AUTODDL_MAX_LEVELS 5
+typedef struct { int32_t ndim; int32_t size[AUTODDL_MAX_LEVELS]; int32_t link[AUTODDL_MAX_LEVELS]; } autoddl_mesh;
 
 /* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap.
  * micro_batches: gradient accumulation: the activation redistributions of a cell are paid once per
@@ -74,7 +79,7 @@ typedef struct { int32_t ndim; int32_t size[3]; int32_t link[3]; } autoddl_mesh;
  * Must be < 2^20.  48 bytes. */
 typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; int64_t micro_batches; } autoddl_net;
 
-/* K = 6^ndim, or AUTODDL_EINVAL. Host only. */
+/* K = 6^ndim for ndim <= 3, the product of the allowed-row counts for ndim = 4, 5; or AUTODDL_EINVAL. Host only. */
 int autoddl_num_signatures(const autoddl_mesh* mesh);
 
 /* Bytes of device workspace that any entry point below may need for (Bp, L, S): the tables when

@@ -29,7 +29,7 @@ class AutoddlError(RuntimeError):
 
 
 class CMesh(C.Structure):
-    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 3), ("link", C.c_int32 * 3)]
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 5), ("link", C.c_int32 * 5)]
 
 
 class CNet(C.Structure):
@@ -88,8 +88,8 @@ def _check(rc: int):
 
 def c_mesh(mesh) -> CMesh:
     m = CMesh()
-    m.ndim = len(mesh.size)                       # ndim outside 1..3 is rejected by the library
-    for d in range(min(m.ndim, 3)):
+    m.ndim = len(mesh.size)                       # ndim outside 1..5 is rejected by the library
+    for d in range(min(m.ndim, 5)):
         m.size[d] = int(mesh.size[d])
         m.link[d] = int(mesh.link[d])
     return m
@@ -136,7 +136,7 @@ def workspace_bytes(Bp: int, L: int, S: int, mesh) -> int:
 def build_tables(d_layers: torch.Tensor, mesh, net, want_node_mask: bool = True, out=None):
     """(a1) -> T int64 [Bp,L,K,K], node int64 [Bp,L,K] | None, mask uint8 [Bp,L,K] | None (device tensors)"""
     Bp, L = d_layers.shape[0], d_layers.shape[1]
-    K = 6 ** len(mesh.size)
+    K = num_signatures(mesh)
     dev = d_layers.device
     T = out if out is not None else torch.empty((Bp, L, K, K), dtype=torch.int64, device=dev)
     node = torch.empty((Bp, L, K), dtype=torch.int64, device=dev) if want_node_mask else None
@@ -156,7 +156,7 @@ def chain_dp(T: torch.Tensor | None, mesh, net=None, d_layers=None, work: torch.
         Bp, L = d_layers.shape[0], d_layers.shape[1]
         dev = d_layers.device
     if work is None:
-        K = 6 ** len(mesh.size)
+        K = num_signatures(mesh)
         if T is None:
             need = workspace_bytes(Bp, L, 0, mesh)
         else:
@@ -180,7 +180,7 @@ def coord_descent(T: torch.Tensor | None, init: torch.Tensor, mesh, max_sweeps: 
     Bp, S, L = init.shape
     dev = init.device
     if T is None and work is None:
-        K = 6 ** len(mesh.size)
+        K = num_signatures(mesh)
         work = torch.empty(Bp * L * K * K * 8 + 256, dtype=torch.uint8, device=dev)
     if out is None:
         cost = torch.empty((Bp, S), dtype=torch.int64, device=dev)
@@ -235,7 +235,7 @@ def search(d_layers: torch.Tensor, mesh, net, init: torch.Tensor | None = None, 
     """Whole path on device tensors in one call (autoddl_search).  Returns a dict with T (or None), node, mask,
     opt_cost, strategy and, when init is given, cd_cost, cd_strategy, cd_sweeps."""
     Bp, L = d_layers.shape[0], d_layers.shape[1]
-    K = 6 ** len(mesh.size)
+    K = num_signatures(mesh)
     dev = d_layers.device
     o = dict(out) if out else {}
     if want_tables and "T" not in o:

@@ -73,7 +73,14 @@ class Mesh:
 
     @property
     def K(self) -> int:
-        return 6 ** self.ndim
+        """6^ndim for ndim <= 3; beyond, the signature index runs over the allowed rows only (R26)"""
+        if self.ndim <= 3:
+            return 6 ** self.ndim
+        k = 1
+        for l in self.link:
+            a = (l >> 8) & 0x3F
+            k *= bin(a).count("1") if a else 6
+        return k
 
 
 @dataclass
@@ -237,6 +244,21 @@ def config6_paper_space(restricted: bool = True) -> Workload:
                     Net(ALPHA_PS, (BETA_300, BETA_25), 40 * 10**9), S=64)
 
 
+def config7_two_nodes_sixteen_gpus() -> Workload:
+    """Not in BASELINE.json: the paper's Google Cloud machine, 2 nodes x 16 GPUs refined into prime
+    sub-levels 2 | 2.2.2.2, searched over the matmul rows {0,1,2} per sub-level (K = 3^5 = 243, R26), on the
+    shape of the paper's large Transformer (28 layers, model dimension 4,096, 32 heads, 2,048 sequences of
+    1,024 tokens per batch, run as 64 micro-batches of 32 sequences (PAPER.md:283 gradient accumulation, R25);
+    synthetic records, no weights).  Data parallelism does not fit the 40 GB cap, as in the paper."""
+    M, H = 32 * 1024, 4096
+    recs = []
+    for _ in range(28):
+        recs += _transformer_block(M, H, 4 * H, act=2, wgrad=4, wstate=18, attn_rows=32, attn_heads=32)
+    a = PAPER_ROWS
+    return Workload("two-nodes-x-16-gpus", _stack(recs), Mesh((2, 2, 2, 2, 2), (INTER | a, INTRA | a, INTRA | a, INTRA | a, INTRA | a)),
+                    Net(ALPHA_PS, (BETA_300, BETA_25), 40 * 10**9, micro_batches=64), S=64)
+
+
 CONFIGS = {
     1: config1_tiny,
     2: config2_vgg16,
@@ -244,4 +266,5 @@ CONFIGS = {
     4: config4_batched,
     5: config5_transformer96,
     6: config6_paper_space,
+    7: config7_two_nodes_sixteen_gpus,
 }

@@ -22,7 +22,7 @@ void count_launch(int n) { g_launches += n; }
 
 int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshParams* out) {
   ADL_REQUIRE(mesh != nullptr, "mesh is NULL");
-  ADL_REQUIRE(mesh->ndim >= 1 && mesh->ndim <= 3, "mesh.ndim = %d, must be 1..3", mesh->ndim);
+  ADL_REQUIRE(mesh->ndim >= 1 && mesh->ndim <= kMaxLevels, "mesh.ndim = %d, must be 1..%d", mesh->ndim, kMaxLevels);
   for (int d = 0; d < mesh->ndim; ++d) {
     ADL_REQUIRE(mesh->size[d] >= 1 && mesh->size[d] <= 65536, "mesh.size[%d] = %d out of range", d, mesh->size[d]);
     ADL_REQUIRE((mesh->link[d] & ~0x3f01) == 0, "mesh.link[%d] = %d: bit 0 = link class, bits 8..13 = allowed rows", d, mesh->link[d]);
@@ -30,15 +30,19 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
   int64_t prod = 1;
   for (int d = 0; d < mesh->ndim; ++d) prod *= mesh->size[d];
   ADL_REQUIRE(prod <= (1 << 20), "mesh has %lld devices, at most 2^20 supported", (long long)prod);
+  const int K = mesh_num_sigs(mesh);
+  ADL_REQUIRE(K <= 256, "mesh.ndim = %d with %d signatures per layer: more than three levels need K <= 256 "
+              "(restrict the rows per level, bits 8..13 of mesh.link)", mesh->ndim, K);
   if (out) {
     memset(out, 0, sizeof(*out));
     out->ndim = mesh->ndim;
+    out->K = K;
     for (int d = 0; d < mesh->ndim; ++d) {
       out->size[d] = mesh->size[d];
       out->allow[d] = ((mesh->link[d] >> 8) & 0x3f) ? ((mesh->link[d] >> 8) & 0x3f) : 0x3f;
       out->magic_size[d] = (uint64_t)((((unsigned __int128)1 << 64) + mesh->size[d] - 1) / mesh->size[d]);
     }
-    for (int m = 0; m < 8; ++m) {
+    for (int m = 0; m < (1 << kMaxLevels); ++m) {
       int64_t f = 1;
       for (int d = 0; d < mesh->ndim; ++d)
         if (m >> d & 1) f *= mesh->size[d];
@@ -64,6 +68,17 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
     }
   }
   return AUTODDL_OK;
+}
+
+// valid ndim assumed (1..kMaxLevels).  R26: beyond three levels the index runs over the allowed rows only
+int mesh_num_sigs(const autoddl_mesh* mesh) {
+  if (mesh->ndim <= 3) return mesh->ndim == 1 ? 6 : mesh->ndim == 2 ? 36 : 216;
+  int64_t k = 1;
+  for (int d = 0; d < mesh->ndim; ++d) {
+    const int a = (mesh->link[d] >> 8) & 0x3f;
+    k *= a ? __builtin_popcount(a) : 6;
+  }
+  return k > (1 << 20) ? (1 << 20) : (int)k;
 }
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -109,13 +124,13 @@ int autoddl_num_signatures(const autoddl_mesh* mesh) {
   clear_error();
   int rc = validate_mesh_net(mesh, nullptr, nullptr);
   if (rc) return rc;
-  return num_sigs(mesh->ndim);
+  return mesh_num_sigs(mesh);
 }
 
 size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_mesh* mesh) {
   clear_error();
   if (validate_mesh_net(mesh, nullptr, nullptr) || Bp < 1 || L < 1 || S < 0) return 0;
-  const int64_t K = num_sigs(mesh->ndim);
+  const int64_t K = mesh_num_sigs(mesh);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
   if (mesh->ndim == 2) b += fused_bp_bytes(L);              // fused build + DP: back-pointers of the chains in flight
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
@@ -153,7 +168,7 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
   ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
   ADL_REQUIRE(((uintptr_t)d_opt_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0, "misaligned output pointer");
   if (!d_T) ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
-  const int K = num_sigs(mesh->ndim);
+  const int K = mp.K;
   cudaStream_t st = (cudaStream_t)stream;
   // many chains: the fused kernel (one chain per CTA, tables never leave shared memory); few chains: the fused kernel
   // would serialise the tiles of a chain on one CTA, so the tables are built by all SMs first when d_work can hold them
@@ -194,7 +209,7 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   ADL_REQUIRE(((uintptr_t)d_T & 15) == 0 && ((uintptr_t)d_work & 255) == 0, "d_T must be 16-byte, d_work 256-byte aligned");
   ADL_REQUIRE(((uintptr_t)d_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0 && ((uintptr_t)d_init & 3) == 0 &&
                   ((uintptr_t)d_sweeps & 3) == 0, "misaligned pointer");
-  const int K = num_sigs(mesh->ndim);
+  const int K = mp.K;
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K);
   if (tb > 0 && (d_work == nullptr || work_bytes < tb)) {
     set_error("coord_descent: workspace of %zu bytes needed, %zu given", tb, d_work ? work_bytes : (size_t)0);
@@ -202,7 +217,7 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   }
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const bool built_here = d_T == nullptr;                  // tables of this library's builder: identical rows per class
+  const bool built_here = d_T == nullptr && mp.ndim <= 3;  // tables of this library's builder (base-6 index): identical rows per class
   if (!d_T) {
     ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
@@ -255,7 +270,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     cudaEventRecord(g_mark, st);
     g_mark = nullptr;
   }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, true);
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3);
   return AUTODDL_OK;
 }
 
@@ -279,7 +294,7 @@ int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const a
                   ((uintptr_t)d_cd_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0 && ((uintptr_t)d_init & 3) == 0 &&
                   ((uintptr_t)d_cd_strategy & 3) == 0 && ((uintptr_t)d_cd_sweeps & 3) == 0, "misaligned pointer");
   if ((rc = check_device())) return rc;
-  return search_device(d_layers, Bp, L, mp, num_sigs(mesh->ndim), d_T, d_node, d_mask, (unsigned char*)d_work, work_bytes,
+  return search_device(d_layers, Bp, L, mp, mp.K, d_T, d_node, d_mask, (unsigned char*)d_work, work_bytes,
                        d_opt_cost, d_strategy, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, (cudaStream_t)stream);
 }
 
@@ -305,7 +320,7 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
   }
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const int K = num_sigs(mesh->ndim);
+  const int K = mp.K;
 
   unsigned char* w = (unsigned char*)d_work;
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
@@ -364,7 +379,7 @@ int autoddl_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_
                   ((uintptr_t)d_init & 3) == 0 && ((uintptr_t)d_best_strategy & 3) == 0 &&
                   ((uintptr_t)d_final_strategy & 3) == 0 && ((uintptr_t)d_accepted & 3) == 0, "misaligned pointer");
   if ((rc = check_device())) return rc;
-  return launch_metropolis(d_T, Bp, L, num_sigs(mesh->ndim), d_init, S, nsteps, tau_ps, seed, d_best_cost, d_best_strategy,
+  return launch_metropolis(d_T, Bp, L, mesh_num_sigs(mesh), d_init, S, nsteps, tau_ps, seed, d_best_cost, d_best_strategy,
                            d_final_cost, d_final_strategy, d_accepted, (cudaStream_t)stream);
 }
 

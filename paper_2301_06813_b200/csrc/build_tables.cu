@@ -80,6 +80,9 @@ template <int D> struct Pow { };
 template <> struct Pow<1> { static constexpr int K = 6, NS = 4, NC = 3; };
 template <> struct Pow<2> { static constexpr int K = 36, NS = 16, NC = 9; };
 template <> struct Pow<3> { static constexpr int K = 216, NS = 64, NC = 27; };
+// four / five levels (R26): the signature index runs over the allowed rows only; K is a launch parameter <= 256
+template <> struct Pow<4> { static constexpr int K = 256, NS = 256, NC = 81; };
+template <> struct Pow<5> { static constexpr int K = 256, NS = 1024, NC = 243; };
 
 // Layer records are staged one tile ahead with cp.async into a double buffer in shared memory (80 bytes:
 // the 64-byte record, then the previous layer's kind), so the tile loop never waits on a global load and
@@ -128,7 +131,7 @@ __device__ __forceinline__ void cfg_masks(int cfg, int& m0, int& m1) {
 
 // the <= 3D table entries whose sum is R[av][bv]; entries that do not run point at a zero slot
 template <int D>
-__device__ __forceinline__ void r_slots(int av, int bv, int (&idx)[3 * D]) {
+__device__ __forceinline__ void r_slots(int av, int bv, int (&idx)[3 * D], const uint32_t* walk = c_walk.w) {
   constexpr int NC = Pow<D>::NC, STRIDE = NC + 1, CA_OFF = D * STRIDE, ZERO = NC;
   int c0[D], c1[D], c2[D], c3[D];
   bool r1[D], r2[D], r3[D];
@@ -136,7 +139,7 @@ __device__ __forceinline__ void r_slots(int av, int bv, int (&idx)[3 * D]) {
 #pragma unroll
   for (int d = 0; d < D; ++d) {
     const int sh = 2 * (D - 1 - d);
-    const uint32_t w = c_walk.w[((av >> sh) & 3) * 4 + ((bv >> sh) & 3)];
+    const uint32_t w = walk[((av >> sh) & 3) * 4 + ((bv >> sh) & 3)];
     c0[d] = (w & 3) * pw; c1[d] = (w >> 2 & 3) * pw; c2[d] = (w >> 4 & 3) * pw; c3[d] = (w >> 6 & 3) * pw;
     r1[d] = w >> 8 & 1; r2[d] = w >> 9 & 1; r3[d] = w >> 10 & 1;
     pw *= 3;
@@ -356,6 +359,189 @@ build_tables_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
     }
     if (tid < 5) cp_async_wait_all();
     __syncthreads();                                       // E is rewritten by the next tile's step 3; publishes the record
+  }
+}
+
+// ======================================================================================================
+// Four and five mesh levels (R26; 2 nodes x 16 GPUs = 2 | 2.2.2.2): K <= 256 signatures over
+// the allowed rows only.  The 4^D x 4^D state table of the kernels above no longer fits shared memory (8 MB at D = 5),
+// so every cell sums its <= 6D table entries itself:  T[i][j] = VP[j] + R[a(i)][b(j)] + R[dual b(j)][dual a(i)],
+// R = sum of the reduce-scatter / all-to-all / all-gather entries of steps 1-2 that the levels' walks select.
+// A work unit is a block of rows of one tile (a tile is split so that a single chain still fills the machine).
+// ======================================================================================================
+template <int D>
+struct DirectSmem {
+  static constexpr int NC = Pow<D>::NC;
+  int64_t Q[5][1 << D];
+  int64_t CG[D][NC + 1];                                // [..][NC] = 0: the slot that does not run
+  int64_t CA[D][NC + 1];
+  int64_t WAR[D][NC];
+  int64_t locW[NC], locO[NC];
+  int64_t VP[256];
+  RecBuf rec;
+  uint32_t walk[16];
+  SigInfo sig[2][256];
+};
+
+// facts per (layer kind, signature) with the mixed-radix index over the allowed rows
+template <int D>
+__device__ __forceinline__ void fill_sig_table_compact(SigInfo (*sig)[256], const MeshParams& mp, int K, int tid, int nthreads) {
+  constexpr int NS = Pow<D>::NS;
+  for (int x = tid; x < 2 * K; x += nthreads) {
+    const int kind = x / K, j = x % K;
+    int dig[D], r = j;
+#pragma unroll
+    for (int d = D - 1; d >= 0; --d) {                     // level 0 most significant; digit = rank among the allowed rows
+      const int nr = __popc(mp.allow[d]);
+      int xr = r % nr;
+      r /= nr;
+      int g = 0;
+      for (int t = 0; t < 6; ++t)
+        if ((mp.allow[d] >> t) & 1) {
+          if (xr == 0) { g = t; break; }
+          --xr;
+        }
+      dig[d] = g;
+    }
+    SigInfo si{};
+    int a = 0, b = 0, cw = 0, co = 0, pw = 1, rs = 1, cs = 1;
+    bool valid = true;
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      const int g = dig[d];
+      int sI, sO, sW;
+      if (kind == AUTODDL_GEMM) { sI = c_gemm_I[g]; sO = c_gemm_O[g]; sW = c_gemm_W[g]; }
+      else { sI = sO = c_attn_IO[g]; sW = kB; if (sI < 0) { valid = false; sI = sO = kB; } }
+      a = a * 4 + sO;
+      b = b * 4 + sI;
+      cw += (sW == kS0 ? 1 : sW == kS1 ? 2 : 0) * pw;
+      co += (sO == kS0 ? 1 : sO == kS1 ? 2 : 0) * pw;
+      pw *= 3;
+      if (sI == kS0) si.mI0 |= 1 << d;
+      if (sI == kS1) si.mI1 |= 1 << d;
+      if (sW == kB) si.wB |= 1 << d;
+      if (sI == kS0 || sO == kS0) rs *= mp.size[d];
+      if (sO == kS1) cs *= mp.size[d];
+    }
+    si.a_idx = valid ? a : NS;
+    si.b_idx = valid ? b : -1;
+    si.db_idx = valid ? dual_vec<D>(b) : -1;
+    si.cfgW = cw; si.cfgO = co; si.valid = valid; si.allowed = 1; si.rowsplit = rs; si.colsplit = cs;
+    sig[kind][j] = si;
+  }
+}
+
+constexpr int kDirectNT = 512;
+
+template <int D>
+__global__ void __launch_bounds__(kDirectNT)
+build_tables_direct_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, int K, int chunks, MeshParams mp,
+                           int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  using SM = DirectSmem<D>;
+  constexpr int NS = Pow<D>::NS, NC = Pow<D>::NC, NT = kDirectNT;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  const int tid = threadIdx.x;
+
+  fill_sig_table_compact<D>(sm.sig, mp, K, tid, NT);
+  if (tid < D) { sm.CG[tid][NC] = 0; sm.CA[tid][NC] = 0; }
+  if (tid < 16) sm.walk[tid] = c_walk.w[tid];
+  const int64_t cap_layer = mp.mem_cap / L;
+  const int rows_per_chunk = (K + chunks - 1) / chunks;
+  int last_tile = -1;
+
+  for (int unit = blockIdx.x; unit < ntiles * chunks; unit += gridDim.x) {
+    const int tile = unit / chunks, chunk = unit % chunks;
+    const int l = tile % L;
+    __syncthreads();                                         // previous unit's readers are done with the tables
+    if (tile != last_tile) {
+      last_tile = tile;
+      if (tid == 0) {
+        const autoddl_layer* cur = layers + tile;
+        RecBuf& r = sm.rec;
+        r.X[0] = cur->M; r.X[1] = cur->Kd; r.X[2] = cur->N; r.X[3] = cur->in_rows; r.X[4] = cur->in_cols;
+        r.kind = cur->kind; r.eb = cur->act_bytes; r.wgb = cur->wgrad_bytes; r.wsb = cur->wstate_bytes;
+        r.maxr = cur->max_split_rows; r.maxc = cur->max_split_cols;
+        r.kind_prev = l > 0 ? (cur - 1)->kind : cur->kind;
+      }
+      __syncthreads();
+      const RecBuf& rec = sm.rec;
+      // ---- 1. Q[x][m] ----------------------------------------------------------------------------------------
+      if (tid < (5 << D)) {
+        const int x = tid >> D, m = tid & ((1 << D) - 1);
+        sm.Q[x][m] = cdiv_magic(rec.X[x], (uint32_t)mp.sub[m], mp.magic_sub[m]);
+      }
+      __syncthreads();
+      // ---- 2. tables per level and split configuration (Table 2) ------------------------------
+      for (int e = tid; e < D * NC; e += NT) {
+        const int d = e / NC, cfg = e % NC;
+        int m0, m1;
+        cfg_masks<D>(cfg, m0, m1);
+        const int64_t p = mp.size[d];
+        int64_t cg = 0, ca = 0, war = 0;
+        if (p > 1) {
+          const int64_t n = sm.Q[3][m0] * sm.Q[4][m1] * (int64_t)rec.eb;
+          cg = mp.accum * ((p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]));
+          ca = mp.accum * ((p - 1) * mp.alpha[d] + n * mp.beta[d]);      // R25: once per micro-batch
+          const int64_t nw = sm.Q[1][m0] * sm.Q[2][m1] * (int64_t)rec.wgb;
+          war = (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(nw, (uint32_t)p, mp.magic_size[d]) * mp.beta[d];
+        }
+        sm.CG[d][cfg] = cg;
+        sm.CA[d][cfg] = ca;
+        sm.WAR[d][cfg] = war;
+        if (d == 0) {
+          sm.locW[cfg] = sm.Q[1][m0] * sm.Q[2][m1];
+          sm.locO[cfg] = sm.Q[0][m0] * sm.Q[2][m1];
+        }
+      }
+      __syncthreads();
+      // ---- 3. VP[j] = node cost + penalty ----------------------------------------------------------------------
+      for (int j = tid; j < K; j += NT) {
+        const SigInfo si = sm.sig[rec.kind][j];
+        int64_t v = 0, mem = 0;
+        if (si.valid) {
+          if (rec.kind == AUTODDL_GEMM) {
+#pragma unroll
+            for (int d = 0; d < D; ++d)
+              if (si.wB >> d & 1) v += sm.WAR[d][si.cfgW];
+            mem = sm.locW[si.cfgW] * (int64_t)rec.wsb;
+          }
+          mem += (sm.Q[3][si.mI0] * sm.Q[4][si.mI1] + sm.locO[si.cfgO]) * (int64_t)rec.eb;
+        }
+        const bool ok = si.valid && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+        sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+        if (chunk == 0) {                                      // one unit per tile reports the node costs and the mask
+          const size_t o = (size_t)tile * K + j;
+          if (node) node[o] = v;
+          if (mask) mask[o] = ok ? 1 : 0;
+        }
+      }
+      __syncthreads();
+    }
+    // ---- 4. the cells of this unit's rows ------------------------------------------------------------------------
+    const RecBuf& rec = sm.rec;
+    const int r0 = chunk * rows_per_chunk;
+    const int r1 = r0 + rows_per_chunk < K ? r0 + rows_per_chunk : K;
+    const int64_t* tab = &sm.CG[0][0];
+    int64_t* out = T + (size_t)tile * K * K;
+    for (int c = r0 * K + tid; c < r1 * K; c += NT) {
+      const int i = c / K, j = c - i * K;
+      int64_t v = sm.VP[j];
+      if (l > 0) {
+        const int a = sm.sig[rec.kind_prev][i].a_idx;
+        const SigInfo& sj = sm.sig[rec.kind][j];
+        if (a < NS && sj.b_idx >= 0) {
+          int idx[3 * D];
+          r_slots<D>(a, sj.b_idx, idx, sm.walk);               // forward leg
+#pragma unroll
+          for (int k = 0; k < 3 * D; ++k) v += tab[idx[k]];
+          r_slots<D>(sj.db_idx, dual_vec<D>(a), idx, sm.walk); // backward leg
+#pragma unroll
+          for (int k = 0; k < 3 * D; ++k) v += tab[idx[k]];
+        }
+      }
+      __stcs(out + c, v);
+    }
   }
 }
 
@@ -1136,6 +1322,28 @@ int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams
   return AUTODDL_OK;
 }
 
+template <int D>
+int launch_direct(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
+                  int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
+  auto kern = build_tables_direct_kernel<D>;
+  const size_t smem = sizeof(DirectSmem<D>);
+  if (smem > 48 * 1024) ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int dev = 0, sms = 148;
+  ADL_CUDA_CHECK(cudaGetDevice(&dev));
+  ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int slots = sms * 2;                                           // two CTAs of 512 threads per SM
+  int chunks = (2 * slots + ntiles - 1) / ntiles;                      // few tiles: split them into row blocks
+  if (chunks > 8) chunks = 8;
+  if (chunks > mp.K) chunks = mp.K;
+  if (chunks < 1) chunks = 1;
+  const int64_t units = (int64_t)ntiles * chunks;
+  const int grid = (int)(units < slots ? units : slots);
+  kern<<<grid, kDirectNT, smem, st>>>(d_layers, ntiles, L, mp.K, chunks, mp, d_T, d_node, d_mask);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
 }  // namespace
 
 int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
@@ -1150,8 +1358,10 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
       if (generic) return launch_d<3>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
       return launch_216(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     }
+    case 4: return launch_direct<4>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
+    case 5: return launch_direct<5>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
   }
-  set_error("ndim must be 1, 2 or 3");
+  set_error("ndim must be 1..5");
   return AUTODDL_EINVAL;
 }
 

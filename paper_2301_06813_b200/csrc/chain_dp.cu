@@ -377,6 +377,118 @@ int launch_cfg(const int64_t* d_T, int Bp, int L, uint8_t* d_bp, int64_t* d_opt,
   return AUTODDL_OK;
 }
 
+// ---- any K <= 256 (four / five mesh levels, R26: K = 81, 243, ... is odd, so neither the 16-byte column pairs nor
+// the 16-byte-aligned TMA row blocks of the kernels above apply).  One CTA of 1024 threads per problem: thread
+// (g, j) owns column j and the rows i = g, g + 4, ...; its loads do not depend on f, so eight of them are in flight
+// per thread (8-byte loads, coalesced over j); the four row groups are merged through shared memory in the
+// lexicographic (value, row) order.  Back-pointers live in shared memory when L * K fits, else in the workspace.
+constexpr int kAnyG = 4, kAnyCols = 256;
+
+template <bool BP_SMEM>
+__global__ void __launch_bounds__(kAnyG * kAnyCols)
+chain_dp_anyk_kernel(const int64_t* __restrict__ T, int L, int K, uint8_t* __restrict__ bp_glob,
+                     int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  int64_t* fbuf = reinterpret_cast<int64_t*>(smem);                  // [2][256]
+  int64_t* partv = fbuf + 2 * kAnyCols;                              // [G][256]
+  int32_t* parti = reinterpret_cast<int32_t*>(partv + kAnyG * kAnyCols);
+  uint8_t* bp_s = reinterpret_cast<uint8_t*>(parti + kAnyG * kAnyCols);
+  const int tid = threadIdx.x, j = tid % kAnyCols, g = tid / kAnyCols;
+  const int p = blockIdx.x;
+  const int64_t* Tp = T + (size_t)p * L * K * K;
+  uint8_t* bp = BP_SMEM ? bp_s : bp_glob + (size_t)p * L * K;
+  const bool active = j < K;
+
+  if (g == 0 && active) fbuf[j] = __ldg(Tp + j);                     // f_0 = row 0 of tile 0
+  __syncthreads();
+  int cur = 0;
+  for (int l = 1; l < L; ++l) {
+    const int64_t* f = fbuf + cur * kAnyCols;
+    const int64_t* tile = Tp + (size_t)l * K * K + j;
+    int64_t best = INT64_MAX;
+    int arg = 0;
+    if (active) {
+      int i = g;
+      for (; i + 7 * kAnyG < K; i += 8 * kAnyG) {
+        int64_t t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t[u] = __ldcs(tile + (size_t)(i + u * kAnyG) * K);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int64_t v = f[i + u * kAnyG] + t[u];
+          if (v < best) { best = v; arg = i + u * kAnyG; }
+        }
+      }
+      for (; i < K; i += kAnyG) {
+        const int64_t v = f[i] + __ldcs(tile + (size_t)i * K);
+        if (v < best) { best = v; arg = i; }
+      }
+      partv[g * kAnyCols + j] = best;
+      parti[g * kAnyCols + j] = arg;
+    }
+    __syncthreads();
+    if (g == 0 && active) {
+      int64_t bv = partv[j];
+      int bi = parti[j];
+#pragma unroll
+      for (int gg = 1; gg < kAnyG; ++gg) {
+        const int64_t v = partv[gg * kAnyCols + j];
+        const int i = parti[gg * kAnyCols + j];
+        if (v != INT64_MAX && lex_less(v, i, bv, bi)) { bv = v; bi = i; }     // a group with no row (K < 4) holds no candidate
+      }
+      fbuf[(cur ^ 1) * kAnyCols + j] = bv;
+      bp[(size_t)l * K + j] = (uint8_t)bi;
+    }
+    __syncthreads();
+    cur ^= 1;
+  }
+
+  if (tid < 32) {                                                    // smallest argmin of f_{L-1}, backtrack
+    const int lane = tid;
+    const int64_t* f = fbuf + cur * kAnyCols;
+    int64_t bv = 0;
+    int bi = -1;
+    for (int c = lane; c < K; c += 32) {
+      const int64_t v = f[c];
+      if (bi < 0 || v < bv) { bv = v; bi = c; }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (oi >= 0 && (bi < 0 || lex_less(ov, oi, bv, bi))) { bv = ov; bi = oi; }
+    }
+    int32_t* sp = strategy + (size_t)p * L;
+    if (lane == 0) {
+      opt_cost[p] = bv;
+      int s = bi;
+      sp[L - 1] = s;
+      for (int l = L - 1; l >= 1; --l) {
+        s = bp[(size_t)l * K + s];
+        sp[l - 1] = s;
+      }
+    }
+  }
+}
+
+int launch_anyk(const int64_t* d_T, int Bp, int L, int K, uint8_t* d_bp, int64_t* d_opt, int32_t* d_strat, cudaStream_t st) {
+  const size_t base = (size_t)2 * kAnyCols * 8 + (size_t)kAnyG * kAnyCols * 12;
+  const bool bp_smem = (size_t)L * K <= 16 * 1024;                  // same rule as the workspace sizing (api.cu)
+  if (!bp_smem && d_bp == nullptr) { set_error("chain_dp: workspace for back-pointers missing"); return AUTODDL_EWORK; }
+  const size_t smem = (base + (bp_smem ? (size_t)L * K : 0) + 127) / 128 * 128;
+  if (bp_smem) {
+    auto kern = chain_dp_anyk_kernel<true>;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<Bp, kAnyG * kAnyCols, smem, st>>>(d_T, L, K, d_bp, d_opt, d_strat);
+  } else {
+    auto kern = chain_dp_anyk_kernel<false>;
+    kern<<<Bp, kAnyG * kAnyCols, smem, st>>>(d_T, L, K, d_bp, d_opt, d_strat);
+  }
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
 }  // namespace
 
 int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp, int64_t* d_opt_cost,
@@ -402,7 +514,8 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
       return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
     }
   }
-  set_error("chain_dp: K must be 6, 36 or 216");
+  if (K >= 1 && K <= 256) return launch_anyk(d_T, Bp, L, K, d_bp, d_opt_cost, d_strategy, st);
+  set_error("chain_dp: K = %d not supported (at most 256)", K);
   return AUTODDL_EINVAL;
 }
 

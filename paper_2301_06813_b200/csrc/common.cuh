@@ -32,21 +32,24 @@ void count_launch(int n = 1);
   } while (0)
 
 // ---- mesh / net passed to kernels by value ----------------------------------------------------------
+constexpr int kMaxLevels = AUTODDL_MAX_LEVELS;
 struct MeshParams {
   int32_t ndim;
-  int32_t size[3];
-  int32_t allow[3];     // signature rows allowed on the level (bit g = row g), 0x3f = all six
-  int64_t alpha[3];     // alpha of the level's link class
-  int64_t beta[3];      // beta  of the level's link class
+  int32_t K;            // signatures per layer: 6^ndim (ndim <= 3), product of the allowed-row counts (ndim = 4, 5; R26)
+  int32_t size[kMaxLevels];
+  int32_t allow[kMaxLevels];     // signature rows allowed on the level (bit g = row g), 0x3f = all six
+  int64_t alpha[kMaxLevels];     // alpha of the level's link class
+  int64_t beta[kMaxLevels];      // beta  of the level's link class
   int64_t mem_cap;      // 0 = none
   int64_t accum;        // micro-batches per mini-batch (>= 1): multiplies the redistribution costs
-  int32_t sub[8];       // product of the sizes of the levels in subset m (bit e = level e)
-  uint64_t magic_sub[8];   // ceil(2^64 / sub[m])
-  uint64_t magic_size[3];  // ceil(2^64 / size[d])
+  int32_t sub[1 << kMaxLevels];       // product of the sizes of the levels in subset m (bit e = level e)
+  uint64_t magic_sub[1 << kMaxLevels];   // ceil(2^64 / sub[m])
+  uint64_t magic_size[kMaxLevels];  // ceil(2^64 / size[d])
 };
 
+// fills *out (may be NULL); returns AUTODDL_OK or AUTODDL_EINVAL.  K of a valid mesh: mesh_num_sigs()
 int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshParams* out);
-inline int num_sigs(int ndim) { return ndim == 1 ? 6 : ndim == 2 ? 36 : 216; }
+int mesh_num_sigs(const autoddl_mesh* mesh);
 
 // ---- kernel launchers (defined in the .cu files) ----------------------------------------------------
 int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp,

@@ -39,8 +39,9 @@ __device__ __forceinline__ int64_t ldg_narrow(const int64_t* p) {
 // signatures agree up to the per-level classes {0}, {1}, {3}, {2, 4, 5} are identical (signatures 2, 4, 5 all output P,
 // or are all invalid for ATTN: DESIGN.md R1): the column gather reads the class representative's row, and candidates
 // of one class share one 64-byte granule -- 16 instead of 36 at K = 36.  Values, hence results, are unchanged.
-template <int K, bool RESUME, bool SBPROWS>
-__global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int L, int S,
+// KT = 0: K is a launch parameter (any K <= 256: the mixed-radix signature spaces of four / five mesh levels, R26)
+template <int KT, bool RESUME, bool SBPROWS>
+__global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int Krt, int L, int S,
                                                            const int32_t* __restrict__ init, int max_sweeps,
                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
                                                            int32_t* __restrict__ sweeps) {
@@ -51,8 +52,9 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   const int lane = threadIdx.x;
   const size_t ps = blockIdx.x;
   const size_t p = ps / S;
+  const int K = KT ? KT : Krt;
   const int64_t* Tp = T + p * (size_t)L * K * K;
-  constexpr int NCAND = (K + 31) / 32;
+  constexpr int NCAND = KT ? (KT + 31) / 32 : 8;
   int rep[NCAND];                                          // row that holds candidate c's column value
 #pragma unroll
   for (int q = 0; q < NCAND; ++q) {
@@ -183,7 +185,7 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
 }
 
 template <int K, bool RESUME, bool SBPROWS>
-int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
+int launch_k(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
              int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
   const size_t smem = ((size_t)L * 5 + 15) / 16 * 16;
   if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
@@ -191,7 +193,7 @@ int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, in
     ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K, RESUME, SBPROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t nb = (int64_t)Bp * S;
   if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
-  coord_descent_kernel<K, RESUME, SBPROWS><<<(unsigned)nb, 32, smem, st>>>(d_T, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
+  coord_descent_kernel<K, RESUME, SBPROWS><<<(unsigned)nb, 32, smem, st>>>(d_T, Krt, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -202,7 +204,7 @@ int launch_k(const int64_t* d_T, int Bp, int L, const int32_t* d_init, int S, in
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                          int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st,
                          bool resume, bool sbp_rows) {
-#define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
+#define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
   if (resume) {
     if (K == 36) return sbp_rows ? ADL_CD(36, true, true) : ADL_CD(36, true, false);
     set_error("coord_descent: resume mode exists for K = 36 only");
@@ -213,8 +215,9 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
     case 36:  return sbp_rows ? ADL_CD(36, false, true) : ADL_CD(36, false, false);
     case 216: return sbp_rows ? ADL_CD(216, false, true) : ADL_CD(216, false, false);
   }
+  if (K >= 1 && K <= 256 && !sbp_rows) return ADL_CD(0, false, false);
 #undef ADL_CD
-  set_error("coord_descent: K must be 6, 36 or 216");
+  set_error("coord_descent: K = %d not supported (6, 36, 216, or any K <= 256 on caller-indexed tables)", K);
   return AUTODDL_EINVAL;
 }
 

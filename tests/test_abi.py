@@ -38,15 +38,19 @@ def test_struct_layouts_match_header(adl):
     assert cf.LAYER_DTYPE.itemsize == 64
     assert [cf.LAYER_DTYPE.fields[k][1] for k in ("M", "Kd", "N", "in_rows", "in_cols", "kind", "act_bytes",
             "wgrad_bytes", "wstate_bytes", "max_split_rows", "max_split_cols")] == [0, 8, 16, 24, 32, 40, 44, 48, 52, 56, 60]
-    assert C.sizeof(adl.CMesh) == 28 and C.sizeof(adl.CNet) == 48
+    assert C.sizeof(adl.CMesh) == 44 and C.sizeof(adl.CNet) == 48
 
 
 def test_host_only_calls(adl):
     assert adl.num_signatures(cf.Mesh((2, 2), (1, 0))) == 36
     assert adl.num_signatures(cf.Mesh((8, 8, 8), (1, 1, 0))) == 216
     assert adl.num_signatures(cf.Mesh((4,), (1,))) == 6
-    with pytest.raises(adl.AutoddlError, match="ndim"):
+    with pytest.raises(adl.AutoddlError, match="256"):                       # 6^4 signatures: rows must be restricted (R26)
         adl.num_signatures(cf.Mesh((2, 2, 2, 2), (0, 0, 0, 0)))
+    with pytest.raises(adl.AutoddlError, match="ndim"):
+        adl.num_signatures(cf.Mesh((2,) * 6, (0x07 << 8,) * 6))
+    assert adl.num_signatures(cf.Mesh((2, 2, 2, 2), (0x07 << 8,) * 4)) == 81
+    assert adl.num_signatures(cf.CONFIGS[7]().mesh) == 243 == cf.CONFIGS[7]().K
     w = cf.config4_batched(Bp=2)
     assert adl.workspace_bytes(4096, 64, 1, w.mesh) >= 4096 * 64 * 36 * 36 * 8 + 4096 * 64 * 64
     w5 = cf.config5_transformer96()
