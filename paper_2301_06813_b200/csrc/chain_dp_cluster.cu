@@ -197,6 +197,141 @@ chain_dp216_cluster_kernel(const int64_t* __restrict__ T, int L, int64_t* __rest
   }
 }
 
+// ---- any K <= 256 (four / five mesh levels, R26: K = 81, 243 are odd, so neither 16-byte-aligned TMA row blocks nor
+// column pairs exist).  Same decomposition over a cluster of 8 CTAs -- CTA r owns the rows and the columns
+// [CR r, CR r + CR) with CR = ceil(K / 8), the last CTAs may own fewer or none -- but the row block of a layer goes
+// from global memory straight into registers: thread j holds its column's <= 32 rows of layer l + 1 (8-byte loads,
+// coalesced over j, issued one layer ahead so that their latency hides behind layer l's exchange).
+constexpr int ACRMAX = 32, ANT = 256;                   // the kernel is instantiated for ACR = 8, 16, 24, 32 >= CR
+
+struct ClusterAnySmem {
+  alignas(16) int64_t slot[2][CC][ACRMAX][2];              // [layer parity][source CTA][owned column] = (value, row)
+  alignas(16) int64_t f[2][ACRMAX];
+  alignas(16) int64_t ffinal[256];
+  alignas(8) uint64_t recv[2];
+};
+
+template <int ACR>
+__global__ void __cluster_dims__(CC, 1, 1) __launch_bounds__(ANT, 1)
+chain_dp_cluster_anyk_kernel(const int64_t* __restrict__ T, int L, int K, int64_t* __restrict__ opt_cost,
+                             int32_t* __restrict__ strategy) {
+  extern __shared__ __align__(128) unsigned char smem_cl[];
+  ClusterAnySmem& sm = *reinterpret_cast<ClusterAnySmem*>(smem_cl);
+  uint8_t* bp = smem_cl + sizeof(ClusterAnySmem);          // [L][ACRMAX]: back-pointers of the columns this CTA owns
+  uint8_t* gath = bp + (size_t)L * ACRMAX;                 // CTA 0: [L][K] gathered back-pointers
+  const int tid = threadIdx.x, lane = tid & 31;
+  const uint32_t r = cluster_ctarank();
+  const int p = blockIdx.x / CC;
+  const int64_t* Tp = T + (size_t)p * L * K * K;
+  const int CR = (K + CC - 1) / CC;
+  const int r0 = CR * (int)r;
+  const int nr = K - r0 < 0 ? 0 : (K - r0 < CR ? K - r0 : CR);      // rows = owned columns of this CTA
+
+  if (tid == 0) {
+    mbar_init(&sm.recv[0], 1);
+    mbar_init(&sm.recv[1], 1);
+    mbar_fence_init();
+  }
+  if (tid < nr) sm.f[0][tid] = __ldg(Tp + r0 + tid);       // f_0[j] = T[0][0][j] for the owned columns
+  __syncthreads();
+  cluster_sync_all();                                      // every CTA's mbarriers exist before any remote store
+
+  const int j = tid;                                       // column
+  const bool col = j < K;
+  const uint32_t owner = col ? j / CR : 0;
+  int64_t tn[ACR];                                         // this column's rows of the NEXT layer
+  const int nrc = col ? nr : 0;
+  const int64_t* next = Tp + ((size_t)K + r0) * K + j;     // row r0 of layer 1, column j
+  auto load_rows = [&]() {
+    const int64_t* src = next;
+#pragma unroll
+    for (int k = 0; k < ACR; ++k) {
+      tn[k] = k < nrc ? __ldcs(src) : 0;
+      src += K;
+    }
+    next += (size_t)K * K;
+  };
+  if (L > 1) load_rows();
+  for (int l = 1; l < L; ++l) {
+    const int par = l & 1;
+    if (tid == 0) mbar_arrive_expect_tx(&sm.recv[par], (uint32_t)(CC * nr * 16));   // this layer's 8 x nr partials
+    int64_t tv[ACR];
+#pragma unroll
+    for (int k = 0; k < ACR; ++k) tv[k] = tn[k];
+    if (l + 1 < L) load_rows();                            // in flight during this layer's scan and exchange
+    if (col) {
+      const int64_t* f = sm.f[par ^ 1];
+      int64_t best = INT64_MAX;
+      int arg = 0;
+#pragma unroll
+      for (int k = 0; k < ACR; ++k)
+        if (k < nr) {
+          const int64_t v = f[k] + tv[k];
+          if (v < best) { best = v; arg = k; }
+        }
+      st_async_v2(map_to_cta(&sm.slot[par][r][j - CR * (int)owner][0], owner), best, (int64_t)(r0 + arg),
+                  map_to_cta(&sm.recv[par], owner));
+    }
+    if (nr > 0) {
+      while (!mbar_try_wait_cluster(&sm.recv[par], ((l - 1) >> 1) & 1)) {
+      }
+    }
+    {                                                      // 8 lanes per owned column merge the 8 row blocks
+      const int mc = tid >> 3, mq = tid & 7;
+      const bool mine = mc < nr;
+      int64_t bv = mine ? sm.slot[par][mq][mc][0] : INT64_MAX;
+      int64_t bi = mine ? sm.slot[par][mq][mc][1] : 0;
+#pragma unroll
+      for (int off = 1; off < 8; off <<= 1) {              // row blocks are disjoint: the smaller row wins ties
+        const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+        const int64_t oi = __shfl_xor_sync(0xffffffffu, bi, off);
+        if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+      }
+      if (mine && mq == 0) {
+        sm.f[par][mc] = bv;
+        bp[(size_t)l * ACRMAX + mc] = (uint8_t)bi;
+      }
+    }
+    __syncthreads();                                       // f_l slice is complete for the next layer's scan
+  }
+
+  // ---- gather f_{L-1} and all back-pointers into CTA 0, then walk back there --------------------------------
+  cluster_sync_all();
+  {
+    const int par = (L - 1) & 1;
+    if (tid < nr) st_cluster_b64(map_to_cta(&sm.ffinal[r0 + tid], 0), sm.f[par][tid]);
+    for (int x = tid; x < L * ACRMAX; x += ANT) {
+      const int l = x / ACRMAX, c = x % ACRMAX;
+      if (c < nr) st_cluster_u8(map_to_cta(gath + (size_t)l * K + r0 + c, 0), l >= 1 ? bp[x] : 0);
+    }
+  }
+  cluster_sync_all();
+  if (r == 0 && tid < 32) {
+    int64_t bv = INT64_MAX;
+    int bi = K;
+    for (int c = lane; c < K; c += 32) {
+      const int64_t v = sm.ffinal[c];
+      if (v < bv) { bv = v; bi = c; }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if (lane == 0) {
+      int32_t* sp = strategy + (size_t)p * L;
+      opt_cost[p] = bv;
+      int sidx = bi;
+      sp[L - 1] = sidx;
+      for (int l = L - 1; l >= 1; --l) {
+        sidx = gath[(size_t)l * K + sidx];
+        sp[l - 1] = sidx;
+      }
+    }
+  }
+}
+
 }  // namespace
 
 // One cluster of 8 CTAs per chain.  Supported for K = 216 and L <= 864 (the gathered back-pointers must fit the
@@ -209,6 +344,27 @@ int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* 
   if (smem > 227 * 1024) { set_error("chain_dp (cluster): %zu bytes of shared memory needed", smem); return AUTODDL_EINVAL; }
   ADL_CUDA_CHECK(cudaFuncSetAttribute(chain_dp216_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   chain_dp216_cluster_kernel<<<Bp * CC, CNT, smem, st>>>(d_T, L, d_opt_cost, d_strategy);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+static size_t cluster_anyk_smem(int32_t K, int32_t L) {
+  return (sizeof(ClusterAnySmem) + (size_t)L * ACRMAX + (size_t)L * K + 127) / 128 * 128;
+}
+// any 64 <= K <= 256: row blocks through registers; L limited by the back-pointers gathered in CTA 0
+bool chain_dp_cluster_anyk_supported(int32_t K, int32_t L) {
+  return K >= 64 && K <= 256 && L >= 2 && cluster_anyk_smem(K, L) <= 200 * 1024;
+}
+
+int launch_chain_dp_cluster_anyk(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, int64_t* d_opt_cost,
+                                 int32_t* d_strategy, cudaStream_t st) {
+  const size_t smem = cluster_anyk_smem(K, L);
+  const int CRk = (K + CC - 1) / CC;
+  auto kern = CRk <= 8 ? chain_dp_cluster_anyk_kernel<8> : CRk <= 16 ? chain_dp_cluster_anyk_kernel<16>
+            : CRk <= 24 ? chain_dp_cluster_anyk_kernel<24> : chain_dp_cluster_anyk_kernel<32>;
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<Bp * CC, ANT, smem, st>>>(d_T, L, K, d_opt_cost, d_strategy);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;

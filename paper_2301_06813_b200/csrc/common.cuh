@@ -65,6 +65,9 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
 bool chain_dp_cluster_supported(int32_t K, int32_t L);
 int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* d_opt_cost, int32_t* d_strategy,
                             cudaStream_t st);
+bool chain_dp_cluster_anyk_supported(int32_t K, int32_t L);
+int launch_chain_dp_cluster_anyk(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, int64_t* d_opt_cost,
+                                 int32_t* d_strategy, cudaStream_t st);
 // resume: the first sweep has been done already (its result is in d_strategy); continue from sweep 2
 // sbp_rows: d_T was built by this library (identical rows per producer-signature class may be read through one row)
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,

@@ -44,6 +44,8 @@ NAMES = ("T", "node", "mask", "dp_cost", "dp_strategy", "cd_cost", "cd_strategy"
 @pytest.mark.parametrize("sizes,links,Bp,L,cap,micro", [
     ((2, 2, 2, 2), (1 | PAPER, 0 | PAPER, 0 | PAPER, 0 | PAPER), 3, 6, 0, 1),                      # 2 x 8 GPUs, K = 81
     ((2, 2, 2, 2, 2), (1 | PAPER, 0 | PAPER, 0 | PAPER, 0 | PAPER, 0 | PAPER), 2, 5, 0, 1),       # 2 x 16 GPUs, K = 243
+    ((2, 2, 2, 2), (1 | PAPER, 1 | PAPER, 0 | PAPER, 0 | PAPER), 21, 4, 0, 1),                     # 21 chains: one CTA per chain
+    ((2, 2, 2, 2), (1 | (0x0f << 8), 0 | PAPER, 0 | PAPER, 0 | (0x03 << 8)), 2, 9, 0, 1),         # K = 72: last cluster CTA owns no row
     ((2, 2, 2, 2, 2), (1 | PAPER, 1 | PAPER, 0 | PAPER, 0 | PAPER, 0 | PAPER), 1, 7, 10**8, 4),   # 4 x 8, cap, accumulation
     ((3, 2, 2, 5), (1 | PAPER, 1 | (0x0b << 8), 0 | (0x30 << 8), 0 | (0x05 << 8)), 2, 6, 0, 1),    # unequal row sets: K = 36
     ((2, 3, 2, 2), (1 | (0x0f << 8), 0 | (0x0f << 8), 0 | (0x0f << 8), 1 | (0x0f << 8)), 1, 3, 0, 2),   # K = 256
