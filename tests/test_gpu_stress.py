@@ -2,7 +2,7 @@
 representative rows) against the three separate kernels on ALL chains, and against the oracle on a sample, over random
 meshes (1-3 levels, sizes 1..8, random allowed-row masks), chain counts around the fused-kernel thresholds (295/296,
 739/740/741 = resident CTAs), chain lengths around the group size, mixed GEMM / ATTN kinds, split limits, memory caps,
-1-3 starts, sweep caps 1, 2, 3, 64 and 0-17 micro-batches.  Bit-exact.  (A 480-second run of the same generator, ~28,000 cases, is clean.)"""
+1-3 starts, sweep caps 1, 2, 3, 64 and 0-17 micro-batches; a second generator covers four and five mesh levels.  Bit-exact.  (A 480-second run of the same generator, ~28,000 cases, is clean.)"""
 import numpy as np
 import pytest
 
@@ -69,4 +69,58 @@ def test_random_cases(adl, seed):
                and np.array_equal(ds[idx].cpu().numpy(), ods) and np.array_equal(cc[idx].cpu().numpy(), occ) and np.array_equal(cs[idx].cpu().numpy(), ocs)
                and np.array_equal(sw[idx].cpu().numpy(), osw))
         assert ok and ok2, dict(seed=seed, case=case, sizes=sizes, links=links, Bp=Bp, L=L, S=S, pa=pa, cap=cap, cap_sw=cap_sw,
+                                one_call_equals_separate=ok, separate_equals_oracle=ok2)
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_random_deep_meshes(adl, seed):
+    """four and five mesh levels (R26): random allowed-row sets with K <= 256, chain counts on both sides of the
+    cluster / one-CTA switch of the single-chain DP (Bp * 8 <= 148), back-pointers in shared memory and in the workspace"""
+    rng = np.random.default_rng(seed)
+    masks = [0x01, 0x03, 0x05, 0x06, 0x07, 0x0b, 0x0e, 0x15, 0x30, 0x0f, 0x38]
+    for case in range(40):
+        D = int(rng.choice([4, 5]))
+        while True:
+            allow = [int(rng.choice(masks)) for _ in range(D)]
+            K = int(np.prod([bin(a).count("1") for a in allow]))
+            if 2 <= K <= 256:
+                break
+        sizes = tuple(int(x) for x in rng.choice([1, 2, 2, 3, 4], D))
+        links = tuple(int(rng.integers(0, 2)) | (a << 8) for a in allow)
+        Bp = int(rng.choice([1, 2, 5, 18, 19, 40]))
+        L = int(rng.choice([1, 2, 3, 5, 9, 17, 70]))
+        if Bp * L * K * K > 3_000_000: Bp = max(1, 3_000_000 // (L * K * K))
+        S = int(rng.choice([1, 2, 3]))
+        layers = cf.config4_batched(Bp=Bp, L=L, seed=int(rng.integers(0, 1000))).layers.copy()
+        if rng.random() < 0.5:
+            for p in range(Bp):
+                for l in range(L):
+                    if rng.random() < 0.3:
+                        layers[p, l] = cf.attn(int(layers[p, l]["M"]), int(layers[p, l]["N"]), int(rng.integers(1, 4000)), 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)))
+        if rng.random() < 0.3:
+            layers["max_split_rows"] = rng.integers(1, 40, size=layers.shape)
+            layers["max_split_cols"] = rng.integers(1, 40, size=layers.shape)
+        cap = int(rng.choice([0, 0, 10**7 * L, 10**9 * L]))
+        w = cf.Workload("stress-deep", layers, cf.Mesh(sizes, links), cf.Net(cf.ALPHA_PS, (3, 40), cap, micro_batches=int(rng.choice([0, 1, 3]))), S=S, seed=int(rng.integers(0, 1000)))
+        assert w.K == K
+        init = w.cd_init()
+        cap_sw = int(rng.choice([1, 2, 64]))
+        dl = adl.layers_to_device(w.layers)
+        dinit = torch.from_numpy(init).cuda()
+        T, node, mask = adl.build_tables(dl, w.mesh, w.net)
+        work = torch.empty(adl.workspace_bytes(Bp, L, S, w.mesh), dtype=torch.uint8, device="cuda")
+        dc, ds = adl.chain_dp(T, w.mesh, work=work)
+        cc, cs, sw = adl.coord_descent(T, dinit, w.mesh, cap_sw)
+        o = adl.search(dl, w.mesh, w.net, init=dinit, max_sweeps=cap_sw, want_node_mask=True)
+        torch.cuda.synchronize()
+        ok = all(torch.equal(a, b) for a, b in ((o["T"], T), (o["node"], node), (o["mask"], mask), (o["opt_cost"], dc), (o["strategy"], ds),
+                                               (o["cd_cost"], cc), (o["cd_strategy"], cs), (o["cd_sweeps"], sw)))
+        idx = np.unique(rng.integers(0, Bp, min(Bp, 2)))
+        oT, on, om = ref.build_tables(np.ascontiguousarray(w.layers[idx]), ref.mesh_of(w), ref.net_of(w))
+        odc, ods = ref.chain_dp(oT)
+        occ, ocs, osw = ref.coord_descent(oT, np.ascontiguousarray(init[idx]), cap_sw)
+        ok2 = (np.array_equal(T[idx].cpu().numpy(), oT) and np.array_equal(node[idx].cpu().numpy(), on) and np.array_equal(mask[idx].cpu().numpy(), om)
+               and np.array_equal(dc[idx].cpu().numpy(), odc) and np.array_equal(ds[idx].cpu().numpy(), ods) and np.array_equal(cc[idx].cpu().numpy(), occ)
+               and np.array_equal(cs[idx].cpu().numpy(), ocs) and np.array_equal(sw[idx].cpu().numpy(), osw))
+        assert ok and ok2, dict(seed=seed, case=case, sizes=sizes, links=links, K=K, Bp=Bp, L=L, S=S, cap=cap, cap_sw=cap_sw,
                                 one_call_equals_separate=ok, separate_equals_oracle=ok2)
