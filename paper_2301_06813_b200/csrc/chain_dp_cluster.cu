@@ -201,7 +201,8 @@ chain_dp216_cluster_kernel(const int64_t* __restrict__ T, int L, int64_t* __rest
 // column pairs exist).  Same decomposition over a cluster of 8 CTAs -- CTA r owns the rows and the columns
 // [CR r, CR r + CR) with CR = ceil(K / 8), the last CTAs may own fewer or none -- but the row block of a layer goes
 // from global memory straight into registers: thread j holds its column's <= 32 rows of layer l + 1 (8-byte loads,
-// coalesced over j, issued one layer ahead so that their latency hides behind layer l's exchange).
+// coalesced over j, issued one layer ahead so that their latency hides behind layer l's exchange).  (1024 threads with
+// four row groups per column and a warp-wide merge of 32 partials was measured: 271 -> 384 us on config 7.)
 constexpr int ACRMAX = 32, ANT = 256;                   // the kernel is instantiated for ACR = 8, 16, 24, 32 >= CR
 
 struct ClusterAnySmem {
