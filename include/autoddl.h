@@ -157,7 +157,8 @@ int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
 /* Whole path with HOST inputs and outputs (the end-to-end call): brings h_layers and h_init to the device -- inputs in
  * pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister) are read by the kernels straight over PCIe, once,
  * overlapped with the table stores; pageable inputs are copied first -- runs (a1) (a2) (a3) in d_work, copies the
- * results back, synchronises `stream`.
+ * results back (the optimum and its strategy on an internal side stream while Coordinate Descent still runs),
+ * synchronises `stream`: all outputs are complete on return.
  * Any h_* output may be NULL to skip it; h_init NULL skips (a3). */
 int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
                         const autoddl_mesh* mesh, const autoddl_net* net,

@@ -10,6 +10,7 @@ namespace autoddl {
 static thread_local char g_err[512] = "";
 static thread_local int64_t g_launches = 0;
 static thread_local cudaEvent_t g_mark = nullptr;          // autoddl_profile_mark: one-shot event between the kernels of a search
+static thread_local cudaEvent_t g_dp_done = nullptr;       // autoddl_search_host: one-shot event after tables + DP (same place)
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -102,6 +103,32 @@ static const void* mapped_host_pointer(const void* h) {
   if (a.type != cudaMemoryTypeHost || a.devicePointer == nullptr) return nullptr;
   return a.devicePointer;
 }
+
+// Side stream of autoddl_search_host (per thread, per device): the optimum and its strategy are final when the chain DP
+// is done, so their device-to-host copy runs beside the Coordinate Descent kernel instead of after it.
+struct SideStream {
+  int dev = -1;
+  cudaStream_t stream = nullptr;
+  cudaEvent_t dp_done = nullptr, copied = nullptr;
+  bool ready() {
+    static const bool off = getenv("AUTODDL_NO_D2H_OVERLAP") != nullptr;
+    if (off) return false;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cur == dev && stream) return true;
+    if (stream) { cudaStreamDestroy(stream); cudaEventDestroy(dp_done); cudaEventDestroy(copied); stream = nullptr; }
+    if (cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&dp_done, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&copied, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      stream = nullptr;
+      return false;
+    }
+    dev = cur;
+    return true;
+  }
+};
+static thread_local SideStream g_side;
 
 static int check_device() {
   int n = 0;
@@ -270,6 +297,10 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     cudaEventRecord(g_mark, st);
     g_mark = nullptr;
   }
+  if (g_dp_done) {
+    cudaEventRecord(g_dp_done, st);
+    g_dp_done = nullptr;
+  }
   if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3);
   return AUTODDL_OK;
 }
@@ -350,11 +381,24 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
       k_init = d_init;
     }
   }
-  if ((rc = search_device(k_layers, Bp, L, mp, K, nullptr, nullptr, nullptr, d_tables, tables_region,
-                          d_opt, d_strategy, k_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st)))
-    return rc;
-  if (h_opt_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_opt_cost, d_opt, (size_t)Bp * 8, cudaMemcpyDeviceToHost, st));
-  if (h_strategy) ADL_CUDA_CHECK(cudaMemcpyAsync(h_strategy, d_strategy, (size_t)Bp * L * 4, cudaMemcpyDeviceToHost, st));
+  const bool overlap = do_cd && (h_opt_cost || h_strategy) && g_side.ready();
+  if (overlap) g_dp_done = g_side.dp_done;
+  rc = search_device(k_layers, Bp, L, mp, K, nullptr, nullptr, nullptr, d_tables, tables_region,
+                     d_opt, d_strategy, k_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+  const bool dp_recorded = overlap && g_dp_done == nullptr;
+  g_dp_done = nullptr;
+  if (rc) return rc;
+  cudaStream_t dp_st = st;
+  if (dp_recorded) {                                        // copy the DP results while Coordinate Descent runs
+    ADL_CUDA_CHECK(cudaStreamWaitEvent(g_side.stream, g_side.dp_done, 0));
+    dp_st = g_side.stream;
+  }
+  if (h_opt_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_opt_cost, d_opt, (size_t)Bp * 8, cudaMemcpyDeviceToHost, dp_st));
+  if (h_strategy) ADL_CUDA_CHECK(cudaMemcpyAsync(h_strategy, d_strategy, (size_t)Bp * L * 4, cudaMemcpyDeviceToHost, dp_st));
+  if (dp_recorded) {
+    ADL_CUDA_CHECK(cudaEventRecord(g_side.copied, g_side.stream));
+    ADL_CUDA_CHECK(cudaStreamWaitEvent(st, g_side.copied, 0));          // the final synchronise covers both streams
+  }
   if (do_cd) {
     if (h_cd_cost) ADL_CUDA_CHECK(cudaMemcpyAsync(h_cd_cost, d_cd_cost, (size_t)Bp * S * 8, cudaMemcpyDeviceToHost, st));
     if (h_cd_strategy)
