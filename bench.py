@@ -476,6 +476,9 @@ def run_configs(args):
                               "mh_proposals_per_s": w.Bp * w.S * nsteps / g["mh_us"] * 1e6},
                 "dp_optimum_ps": int(dp[0][0]), "best_cd_over_dp": float(cd[0].min(dim=1).values.double().div(dp[0].double()).mean()),
                 "best_mh_over_dp": float(mh[0].min(dim=1).values.double().div(dp[0].double()).mean()),
+                # random search with the same S samples (the starts themselves; zero proposals): PAPER.md Fig. 7's third arm
+                "best_random_over_dp": float(adl.metropolis(T, init, w.mesh, 0, tau, seed=0)[0].min(dim=1).values.double()
+                                             .div(dp[0].double()).mean()),
                 "mh": {"nsteps": nsteps, "tau_ps": tau}}
         if k == 6:                                           # the same chain on the unrestricted six-row space
             wu = cf.config6_paper_space(restricted=False)
