@@ -506,10 +506,6 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
     case 216: {
       // few long chains: one 8-CTA cluster per chain (chain_dp_cluster.cu); many chains already fill the machine
       static const bool no_cluster = getenv("AUTODDL_DP_NO_CLUSTER") != nullptr;
-      static const bool reg_cluster = getenv("AUTODDL_DP_REG_CLUSTER") != nullptr;   // debugging switch: rows through registers
-      if (reg_cluster && Bp * 8 <= 148 && chain_dp_cluster_anyk_supported(K, L) &&
-          launch_chain_dp_cluster_anyk(d_T, Bp, L, K, d_opt_cost, d_strategy, st) == AUTODDL_OK)
-        return AUTODDL_OK;
       if (!no_cluster && Bp * 8 <= 148 && chain_dp_cluster_supported(K, L)) {
         const int rc = launch_chain_dp_cluster(d_T, Bp, L, d_opt_cost, d_strategy, st);
         if (rc == AUTODDL_OK) return rc;

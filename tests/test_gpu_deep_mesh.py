@@ -117,3 +117,23 @@ def test_limits(adl):
     with pytest.raises(adl.AutoddlError, match="ndim"):
         adl.num_signatures(cf.Mesh((2,) * 6, (PAPER,) * 6))
     assert adl.num_signatures(cf.Mesh((2, 2, 2, 2), (0x0f << 8,) * 4)) == 256
+
+
+@pytest.mark.parametrize("K,L,Bp,sizes,links", [
+    (81, 400, 2, (2, 2, 2, 2), (PAPER,) * 4),                          # gathered back-pointers outgrow the stage memory
+    (243, 800, 1, (2, 2, 2, 2, 2), (PAPER,) * 5),                      # too long for the cluster kernel: one CTA, workspace
+    (100, 150, 3, (2, 2, 2, 2), (0x1f << 8, 0x1f << 8, 0x03 << 8, 0x03 << 8)),    # run-time K on the cluster kernel
+    (243, 33, 19, (2, 2, 2, 2, 2), (PAPER,) * 5),                      # 19 chains: one CTA per chain
+])
+def test_single_chain_dp_on_caller_tables(adl, K, L, Bp, sizes, links):
+    """(a2) alone on random tables with many exact ties (values in [0, 50)): every DP kernel for K <= 256 takes the same
+    smallest-index decisions as the definition"""
+    mesh = cf.Mesh(sizes, links)
+    assert adl.num_signatures(mesh) == K
+    rng = np.random.default_rng(K + L)
+    T = rng.integers(0, 50, size=(Bp, L, K, K)).astype(np.int64)
+    T[:, :, :, ::7] += 1 << 50                                          # infeasible columns
+    odc, ods = ref.chain_dp(T)
+    work = torch.empty(adl.workspace_bytes(Bp, L, 1, mesh), dtype=torch.uint8, device="cuda")
+    dc, ds = adl.chain_dp(torch.from_numpy(T).cuda(), mesh, work=work)
+    _same((dc, ds), (odc, ods), ("dp_cost", "dp_strategy"))
