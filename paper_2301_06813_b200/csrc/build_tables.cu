@@ -524,23 +524,23 @@ build_tables_direct_kernel(const autoddl_layer* __restrict__ layers, int ntiles,
     const int r1 = r0 + rows_per_chunk < K ? r0 + rows_per_chunk : K;
     const int64_t* tab = &sm.CG[0][0];
     int64_t* out = T + (size_t)tile * K * K;
-    for (int c = r0 * K + tid; c < r1 * K; c += NT) {
-      const int i = c / K, j = c - i * K;
-      int64_t v = sm.VP[j];
-      if (l > 0) {
-        const int a = sm.sig[rec.kind_prev][i].a_idx;
+    for (int i = r0 + (tid >> 5); i < r1; i += NT / 32) {   // one warp per row: no division, the row's state vector once
+      const int a = l > 0 ? sm.sig[rec.kind_prev][i].a_idx : NS;
+      const int da = dual_vec<D>(a & (NS - 1));
+      for (int j = tid & 31; j < K; j += 32) {
+        int64_t v = sm.VP[j];
         const SigInfo& sj = sm.sig[rec.kind][j];
         if (a < NS && sj.b_idx >= 0) {
           int idx[3 * D];
-          r_slots<D>(a, sj.b_idx, idx, sm.walk);               // forward leg
+          r_slots<D>(a, sj.b_idx, idx, sm.walk);             // forward leg
 #pragma unroll
           for (int k = 0; k < 3 * D; ++k) v += tab[idx[k]];
-          r_slots<D>(sj.db_idx, dual_vec<D>(a), idx, sm.walk); // backward leg
+          r_slots<D>(sj.db_idx, da, idx, sm.walk);           // backward leg
 #pragma unroll
           for (int k = 0; k < 3 * D; ++k) v += tab[idx[k]];
         }
+        __stcs(out + (size_t)i * K + j, v);
       }
-      __stcs(out + c, v);
     }
   }
 }

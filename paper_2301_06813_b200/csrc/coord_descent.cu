@@ -217,7 +217,11 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
     case 36:  return sbp_rows ? ADL_CD(36, false, true) : ADL_CD(36, false, false);
     case 216: return sbp_rows ? ADL_CD(216, false, true) : ADL_CD(216, false, false);
   }
-  if (K >= 1 && K <= 256 && !sbp_rows) return ADL_CD(0, false, false);
+  if (!sbp_rows) {                                         // four / five mesh levels (R26): the paper's rows, then any K
+    if (K == 81) return ADL_CD(81, false, false);
+    if (K == 243) return ADL_CD(243, false, false);
+    if (K >= 1 && K <= 256) return ADL_CD(0, false, false);
+  }
 #undef ADL_CD
   set_error("coord_descent: K = %d not supported (6, 36, 216, or any K <= 256 on caller-indexed tables)", K);
   return AUTODDL_EINVAL;
