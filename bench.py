@@ -391,6 +391,13 @@ def run_ours(args):
             try:
                 rows = dict(l.strip().split(",") for l in open(tpath).read().splitlines()[1:] if l.strip())
                 traffic = float(rows[dom]) if dom in rows else None
+                # next to the algorithmic GB/s, the DRAM GB/s actually moved (ncu bytes per launch of the committed
+                # capture / this run's launch time); for coord_descent the two differ by the 64-byte granules of the gather
+                for name, k in kernels.items():
+                    if name in rows:
+                        k["dram_bytes_per_launch_ncu"] = float(rows[name])
+                        k["dram_GBps"] = float(rows[name]) / (k["ms"] * 1e-3) / 1e9
+                        k["dram_frac_of_peak"] = k["dram_GBps"] / peak
             except Exception:
                 traffic = None
         line = {
