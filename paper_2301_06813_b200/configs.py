@@ -259,6 +259,21 @@ def config7_two_nodes_sixteen_gpus() -> Workload:
                     Net(ALPHA_PS, (BETA_300, BETA_25), 40 * 10**9, micro_batches=64), S=64)
 
 
+def config8_vgg13_32_nodes() -> Workload:
+    """Not in BASELINE.json: the setting of the paper's Fig. 8: VGG13 on 32 single-GPU nodes of Piz Daint
+    (batch = 8 x nodes, fp32, 16 GB), the nodes refined into prime sub-levels 2.2.2.2.2 and searched over
+    the matmul rows (K = 243, R26).  Convolutions as im2col GEMMs as in config 2; synthetic records."""
+    B = 8 * 32
+    convs = [(3, 64, 224), (64, 64, 224), (64, 128, 112), (128, 128, 112), (128, 256, 56), (256, 256, 56),
+             (256, 512, 28), (512, 512, 28), (512, 512, 14), (512, 512, 14)]
+    recs = [gemm(B * h * h, 9 * cin, cout, act=4, wgrad=4, wstate=12, in_rows=B * h * h, in_cols=cin)
+            for (cin, cout, h) in convs]
+    for (kd, n) in [(25088, 4096), (4096, 4096), (4096, 1000)]:
+        recs.append(gemm(B, kd, n, act=4, wgrad=4, wstate=12))
+    return Workload("vgg13-32-nodes", _stack(recs), Mesh((2, 2, 2, 2, 2), (INTER | PAPER_ROWS,) * 5),
+                    Net(ALPHA_PS, (BETA_300, BETA_12_5), 16 * 10**9), S=64)
+
+
 CONFIGS = {
     1: config1_tiny,
     2: config2_vgg16,
@@ -267,4 +282,5 @@ CONFIGS = {
     5: config5_transformer96,
     6: config6_paper_space,
     7: config7_two_nodes_sixteen_gpus,
+    8: config8_vgg13_32_nodes,
 }

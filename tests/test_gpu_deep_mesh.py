@@ -109,6 +109,23 @@ def test_config7_full_size(adl):
     _same([host[k] for k in ("opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps")], (odc, ods, occ, ocs, osw), NAMES[3:])
 
 
+def test_config8_vgg13_on_32_nodes(adl):
+    """the setting of the paper's Fig. 8 (configs.config8): every output against the oracle; the optimum the GPU returns
+    keeps the dense layers' weights un-replicated"""
+    w = cf.CONFIGS[8]()
+    init = w.cd_init()
+    oT, onode, omask = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+    odc, ods = ref.chain_dp(oT)
+    occ, ocs, osw = ref.coord_descent(oT, init, w.max_sweeps)
+    one = adl.search(adl.layers_to_device(w.layers), w.mesh, w.net, init=torch.from_numpy(init).cuda(), max_sweeps=w.max_sweeps,
+                     want_node_mask=True)
+    _same([one[k] for k in ("T", "node", "mask", "opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps")],
+          (oT, onode, omask, odc, ods, occ, ocs, osw), NAMES)
+    strat = one["strategy"][0].tolist()
+    for l in (10, 11, 12):
+        assert int(one["node"][0, l, strat[l]]) == 0            # no weight-gradient all-reduce on the dense layers
+
+
 def test_limits(adl):
     with pytest.raises(adl.AutoddlError, match="256"):
         adl.num_signatures(cf.Mesh((2, 2, 2, 2), (0, 0, 0, 0)))                       # 6^4 signatures

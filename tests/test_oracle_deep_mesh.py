@@ -11,6 +11,9 @@ only (K = 3^4 = 81, 3^5 = 243), level 0 most significant.  No GPU.
       over the network only
   D5  exhaustive search over K^L strategies equals the DP on an 81-signature chain
   D6  K is bounded: more than 256 signatures, or more than five levels, is refused
+  D7  the qualitative result the paper reports for VGG13 on 32 GPUs (Fig. 8): the optimum keeps the weight
+      matrices of the three dense layers un-replicated (no B state: zero weight-gradient synchronisation) and runs the early
+      convolutions purely data parallel, (S0: p) in and out
 """
 import itertools
 
@@ -163,3 +166,27 @@ def test_k_is_bounded():
     m = ref.make_mesh((2, 2, 2, 2, 2), [ROWS012] * 5)
     m.ndim = 6
     assert ref.num_signatures(m) == -1
+
+
+# ---- D7 ---------------------------------------------------------------------------------------------------
+def test_vgg13_on_32_nodes_has_the_structure_of_fig8():
+    w = cf.CONFIGS[8]()
+    mesh, net = ref.mesh_of(w), ref.net_of(w)
+    assert ref.num_signatures(mesh) == 243 and w.L == 13
+    T, node, mask = ref.build_tables(w.layers, mesh, net)
+    dc, ds = ref.chain_dp(T)
+    assert dc[0] < (1 << 50)
+    strat = ds[0].tolist()
+    for l in (10, 11, 12):                                       # dense layers: "W1, W2, and W3 are not replicated"
+        _, I, W, O = ref.sig_states(0, strat[l], mesh)
+        assert B not in W, (l, W)
+        assert node[0, l, strat[l]] == 0                         # "zero weight gradient synchronization overhead"
+    for l in range(6):                                           # convolutions: "(S0: p) for input and output tensors"
+        assert strat[l] == 0
+        _, I, W, O = ref.sig_states(0, 0, mesh)
+        assert set(I) == {S0} and set(O) == {S0} and set(W) == {B}
+    # data parallelism throughout is not even feasible here (the first dense layer's replicated weight state alone
+    # exceeds the per-layer share of 16 GB) and the best 1-opt strategies CD finds are no better than the optimum
+    assert ref.chain_cost(T[0], [0] * w.L) >= (1 << 50)
+    cc, cs, _ = ref.coord_descent(T, w.cd_init(), w.max_sweeps)
+    assert (cc >= dc[0]).all() and cc.min() < (1 << 50)
