@@ -384,10 +384,12 @@ int launch_cfg(const int64_t* d_T, int Bp, int L, uint8_t* d_bp, int64_t* d_opt,
 // lexicographic (value, row) order.  Back-pointers live in shared memory when L * K fits, else in the workspace.
 constexpr int kAnyG = 4, kAnyCols = 256;
 
-template <bool BP_SMEM>
+// KT = 81, 243 (the paper's rows on four / five levels): K at compile time, row offsets become immediates; KT = 0: any K
+template <int KT, bool BP_SMEM>
 __global__ void __launch_bounds__(kAnyG * kAnyCols)
-chain_dp_anyk_kernel(const int64_t* __restrict__ T, int L, int K, uint8_t* __restrict__ bp_glob,
+chain_dp_anyk_kernel(const int64_t* __restrict__ T, int L, int Krt, uint8_t* __restrict__ bp_glob,
                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy) {
+  const int K = KT ? KT : Krt;
   extern __shared__ __align__(16) unsigned char smem[];
   int64_t* fbuf = reinterpret_cast<int64_t*>(smem);                  // [2][256]
   int64_t* partv = fbuf + 2 * kAnyCols;                              // [G][256]
@@ -477,11 +479,11 @@ int launch_anyk(const int64_t* d_T, int Bp, int L, int K, uint8_t* d_bp, int64_t
   if (!bp_smem && d_bp == nullptr) { set_error("chain_dp: workspace for back-pointers missing"); return AUTODDL_EWORK; }
   const size_t smem = (base + (bp_smem ? (size_t)L * K : 0) + 127) / 128 * 128;
   if (bp_smem) {
-    auto kern = chain_dp_anyk_kernel<true>;
+    auto kern = K == 243 ? chain_dp_anyk_kernel<243, true> : K == 81 ? chain_dp_anyk_kernel<81, true> : chain_dp_anyk_kernel<0, true>;
     ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<Bp, kAnyG * kAnyCols, smem, st>>>(d_T, L, K, d_bp, d_opt, d_strat);
   } else {
-    auto kern = chain_dp_anyk_kernel<false>;
+    auto kern = K == 243 ? chain_dp_anyk_kernel<243, false> : K == 81 ? chain_dp_anyk_kernel<81, false> : chain_dp_anyk_kernel<0, false>;
     kern<<<Bp, kAnyG * kAnyCols, smem, st>>>(d_T, L, K, d_bp, d_opt, d_strat);
   }
   count_launch();
