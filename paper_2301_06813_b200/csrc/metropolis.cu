@@ -45,6 +45,15 @@ __device__ __forceinline__ int64_t neglog_q16(uint64_t x) {
   return (nlog2_q16 * 744261117ll) >> 30;                  // ln 2 = 744261117 / 2^30, truncated
 }
 
+// x mod d for any 64-bit x with the launch constant M = floor(2^64 / d): the multiply-high quotient is short by at most
+// two, so two conditional subtractions make the remainder exact (a run-time 64-bit division costs ~5x as much)
+__device__ __forceinline__ uint32_t mod_magic(uint64_t x, uint32_t d, uint64_t M) {
+  uint64_t r = x - __umul64hi(x, M) * d;
+  if (r >= d) r -= d;
+  if (r >= d) r -= d;
+  return (uint32_t)r;
+}
+
 __device__ __forceinline__ int64_t ldg64(const int64_t* p) {
   int64_t v;
   asm volatile("ld.global.nc.L2::64B.b64 %0, [%1];" : "=l"(v) : "l"(p));
@@ -55,7 +64,7 @@ constexpr int kWarps = 4;                                  // chains per block
 
 __global__ void __launch_bounds__(kWarps * 32)
 metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int S, const int32_t* __restrict__ init,
-                  int nsteps, int64_t tau, uint64_t seed, int64_t* __restrict__ best_cost,
+                  int nsteps, int64_t tau, uint64_t seed, uint64_t magicL, uint64_t magicK, int64_t* __restrict__ best_cost,
                   int32_t* __restrict__ best_strategy, int64_t* __restrict__ final_cost,
                   int32_t* __restrict__ final_strategy, int32_t* __restrict__ accepted) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -90,8 +99,8 @@ metropolis_kernel(const int64_t* __restrict__ T, int nchains, int L, int K, int 
     const int tk = t + lane;
     const bool live = tk < nsteps;
     const uint64_t base = (((uint64_t)chain << 32) + (uint64_t)(live ? tk : 0)) * 4;
-    const int l = (int)(splitmix_nth(seed, base + 1) % (uint64_t)L);
-    const int c = (int)(splitmix_nth(seed, base + 2) % (uint64_t)K);
+    const int l = (int)mod_magic(splitmix_nth(seed, base + 1), (uint32_t)L, magicL);
+    const int c = (int)mod_magic(splitmix_nth(seed, base + 2), (uint32_t)K, magicK);
     const uint64_t x = (splitmix_nth(seed, base + 3) >> 32) + 1;
     const int old = s[l];
     const int left = l > 0 ? s[l - 1] : 0;
@@ -165,7 +174,11 @@ int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, cons
   if (smem > 48 * 1024)
     ADL_CUDA_CHECK(cudaFuncSetAttribute(metropolis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const unsigned grid = (unsigned)((nchains + kWarps - 1) / kWarps);
-  metropolis_kernel<<<grid, kWarps * 32, smem, st>>>(d_T, (int)nchains, L, K, S, d_init, nsteps, tau_ps, seed, d_best_cost,
+  // floor(2^64 / d); d = 1 would need 2^64: every x mod 1 is 0, which M = 0 also yields (r = x, two subtractions of 1 are
+  // not enough), so d = 1 uses M = 2^64 - 1: quotient x - 1 for x >= 1, remainder 1 -> corrected to 0
+  auto magic = [](uint32_t d) { return d == 1 ? ~(uint64_t)0 : (uint64_t)((((unsigned __int128)1) << 64) / d); };
+  metropolis_kernel<<<grid, kWarps * 32, smem, st>>>(d_T, (int)nchains, L, K, S, d_init, nsteps, tau_ps, seed,
+                                                     magic((uint32_t)L), magic((uint32_t)K), d_best_cost,
                                                      d_best_strategy, d_final_cost, d_final_strategy, d_accepted);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
