@@ -112,3 +112,19 @@ def test_config4_full_size_sampled(adl):
         re = T[ar, lidx, prev, s].sum(1)
         assert torch.equal(re, cost[:, 0])
     assert (bc[:, 0] >= dc).all() and (bc <= fc).all() and (acc >= 0).all() and (acc <= nsteps).all()
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 31, 97, 1000, 4099])
+@pytest.mark.parametrize("sizes,links", [((4,), (1,)), ((2, 2, 2, 2), (0x03 << 8,) * 4), ((2, 2, 2, 2, 2), (0x07 << 8,) * 5)])
+def test_draw_reduction_for_odd_lengths_and_k(adl, L, sizes, links):
+    """the layer and signature draws are reduced modulo L and K by a multiply-high remainder in the kernel and by `%` in the
+    oracle: chain lengths 1, primes, a value above 2^12, and K = 6, 16, 243 on random tables"""
+    mesh = cf.Mesh(sizes, links)
+    K = adl.num_signatures(mesh)
+    L = min(L, 60_000_000 // (K * K))                            # K = 243: at most 1016 layers (480 MB of tables)
+    rng = np.random.default_rng(L + K)
+    T = rng.integers(0, 1000, size=(1, L, K, K)).astype(np.int64)
+    init = rng.integers(0, K, size=(1, 5, L)).astype(np.int32)
+    want = ref.metropolis(T, init, 3000, 400, seed=L)
+    got = adl.metropolis(torch.from_numpy(T).cuda(), torch.from_numpy(init).cuda(), mesh, 3000, 400, seed=L)
+    _same(got, want)
