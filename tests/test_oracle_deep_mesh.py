@@ -190,3 +190,15 @@ def test_vgg13_on_32_nodes_has_the_structure_of_fig8():
     assert ref.chain_cost(T[0], [0] * w.L) >= (1 << 50)
     cc, cs, _ = ref.coord_descent(T, w.cd_init(), w.max_sweeps)
     assert (cc >= dc[0]).all() and cc.min() < (1 << 50)
+
+
+# ---- stored optima of the extra configs (regression values written by tests/golden/make_extra_config_optima.py) ----------
+@pytest.mark.parametrize("k", [6, 7, 8])
+def test_stored_optima_of_the_extra_configs(k):
+    from tests.conftest import read_golden
+    g = read_golden("extra_config_optima.txt")
+    w = cf.CONFIGS[k]()
+    T, _, _ = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+    dc, ds = ref.chain_dp(T)
+    assert int(dc[0]) == g["config%d_dp" % k]
+    assert sum((l + 1) * int(s) for l, s in enumerate(ds[0])) == g["config%d_strategy_sum" % k]
