@@ -65,8 +65,8 @@ def test_random_cases(adl, seed):
         oT, on, om = ref.build_tables(np.ascontiguousarray(w.layers[idx]), ref.mesh_of(w), ref.net_of(w))
         odc, ods = ref.chain_dp(oT)
         occ, ocs, osw = ref.coord_descent(oT, np.ascontiguousarray(init[idx]), cap_sw)
-        ok2 = (np.array_equal(T[idx].cpu().numpy(), oT) and np.array_equal(mask[idx].cpu().numpy(), om) and np.array_equal(dc[idx].cpu().numpy(), odc)
-               and np.array_equal(ds[idx].cpu().numpy(), ods) and np.array_equal(cc[idx].cpu().numpy(), occ) and np.array_equal(cs[idx].cpu().numpy(), ocs)
+        ok2 = (np.array_equal(T[idx].cpu().numpy(), oT) and np.array_equal(node[idx].cpu().numpy(), on) and np.array_equal(mask[idx].cpu().numpy(), om)
+               and np.array_equal(dc[idx].cpu().numpy(), odc) and np.array_equal(ds[idx].cpu().numpy(), ods) and np.array_equal(cc[idx].cpu().numpy(), occ) and np.array_equal(cs[idx].cpu().numpy(), ocs)
                and np.array_equal(sw[idx].cpu().numpy(), osw))
         assert ok and ok2, dict(seed=seed, case=case, sizes=sizes, links=links, Bp=Bp, L=L, S=S, pa=pa, cap=cap, cap_sw=cap_sw,
                                 one_call_equals_separate=ok, separate_equals_oracle=ok2)
