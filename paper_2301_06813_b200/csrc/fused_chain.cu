@@ -1,0 +1,481 @@
+// Fused (a1) + (a2) + first sweep of (a3) on two mesh levels (K = 36): ONE WARP PER CHAIN, no block barrier.
+//
+// A warp walks its chain layer by layer.  Per layer it evaluates the cost model in FACTOR form:
+//   T[l][i][j] = VP[j] + Esym[A(i)][B(j)]
+//     VP[j]      = weight-gradient all-reduce of consumer signature j + 2^50 if j is infeasible
+//     Esym[a][b] = R[a][b] + R[dual b][dual a]: forward + backward redistribution (Table 2 :102-108)
+//                  between the producer's output state vector a and the consumer's input state vector b
+//     A(i), B(j) = state-vector index of producer signature i / consumer signature j (16 = invalid for the layer kind:
+//                  zero edge), so a tile holds 36 + 17 x 17 numbers of information
+// and then, from those 2.6 KB in shared memory,
+//   * writes the 36 x 36 tile to HBM with coalesced 16-byte streaming stores (skipped when no table is wanted),
+//   * advances the chain DP  f_l[j] = VP[j] + min_i f_{l-1}[i] + Esym[A(i)][B(j)]  (smallest i on ties, R9): 16 input
+//     state classes x 2 row halves on the 32 lanes, columns follow their class,
+//   * runs the first Coordinate Descent sweep of the chain's starts (R10): the update of layer l-1 needs the row
+//     T[l-1][s_{l-2}][.] (stashed in registers one layer earlier) and the column T[l][.][s_l] = Esym_l[A(.)][B(s_l)] + const.
+// Nothing is exchanged between warps: no mbarrier, no bar.sync, no TMA hand-off in the layer loop -- the warps of an SM
+// (14-16 of them, one CTA per SM) hide each other's latencies.  After the last layer lane 0 back-tracks the chain from
+// byte back-pointers in the warp's shared memory (or in a workspace slice for very long chains).
+#include "sbp_builder.cuh"
+
+namespace autoddl {
+
+namespace {
+
+constexpr int FK = 36, FD = 2, FNS = 16, FNC = 9, FES = 17, FSTRIDE = FNC + 1, FCELLS = FK * FK;
+constexpr int kMaxFusedStarts = 8;                        // CD starts per chain whose first sweep rides along
+
+struct CtaShared {
+  SigInfo sig[2][FK];
+  uint16_t aoff[2][FK];                                   // per producer kind: A(i) * 17
+  uint8_t bcls[2][FK];                                    // per consumer kind: B(j) in 0..16
+  // step 3, state pair e = lane + 32 k: the <= 6 table entries whose sum is R[a][b] (6 bits each: five in slot_lo, the
+  // sixth in bits 26.. of sym) and the two entries (9 bits each) whose sum is Esym of the pair
+  uint32_t slot_lo[8][32], sym[8][32];
+};
+
+struct alignas(16) WarpShared {
+  int64_t Q[5][4];                                        // M, Kd, N, in_rows, in_cols  x  level subset
+  int64_t TAB[2 * FD * FSTRIDE];                          // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
+  int64_t WAR[FD][FNC];
+  int64_t locW[FNC], locO[FNC];
+  alignas(16) int64_t VP[FK];
+  int64_t Esym[FES * FES];                                // R[a][b], then symmetrised in place; row / column 16 stay 0
+  alignas(16) int64_t f[2][FK];
+  RecBuf rec[2];
+};
+
+__device__ __forceinline__ void lexmin_xor(int64_t& bv, int& bi) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+  }
+}
+
+// smallest (value, index) over the warp for 0 <= value and index < 64.  Fast path when every value is below 2^57: the
+// key value * 64 + index is reduced as two 32-bit halves with redux.sync (the low half only among the lanes that hold
+// the smallest high half); otherwise the shuffle butterfly.  Both are exact.
+__device__ __forceinline__ void warp_argmin64(int64_t& bv, int& bi) {
+  if (__all_sync(0xffffffffu, (uint64_t)bv < (1ull << 57))) {
+    const uint64_t key = ((uint64_t)bv << 6) | (uint32_t)bi;
+    const uint32_t hi = (uint32_t)(key >> 32), lo = (uint32_t)key;
+    const uint32_t mh = __reduce_min_sync(0xffffffffu, hi);
+    const uint32_t ml = __reduce_min_sync(0xffffffffu, hi == mh ? lo : 0xffffffffu);
+    const uint64_t m = ((uint64_t)mh << 32) | ml;
+    bv = (int64_t)(m >> 6);
+    bi = (int)(m & 63);
+  } else {
+    lexmin_xor(bv, bi);
+  }
+}
+
+__global__ void __launch_bounds__(896, 1)
+fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, MeshParams mp,
+                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
+                     int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
+                     const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1, int per_warp_bytes) {
+  extern __shared__ __align__(128) unsigned char fsm_raw[];
+  CtaShared& cs = *reinterpret_cast<CtaShared*>(fsm_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+  unsigned char* wbase = fsm_raw + ((sizeof(CtaShared) + 127) & ~(size_t)127) + (size_t)warp * per_warp_bytes;
+  WarpShared& ws = *reinterpret_cast<WarpShared*>(wbase);
+  // CD only: row stash [cd_S][36] int64, then the strategies of the chain's starts [cd_S][L]; then the back-pointers
+  int64_t* cd_stash = reinterpret_cast<int64_t*>(wbase + sizeof(WarpShared));
+  uint8_t* cd_s = wbase + sizeof(WarpShared) + (cd_init ? (size_t)cd_S * FK * 8 : 0);
+  const size_t cd_bytes = cd_init ? (((size_t)cd_S * L + 15) & ~(size_t)15) : 0;
+  uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
+
+  // ---- once per CTA: facts per (layer kind, signature) -----------------------------------------------------------
+  fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
+  __syncthreads();
+  for (int x = tid; x < 2 * FK; x += blockDim.x) {
+    const SigInfo& si = cs.sig[x / FK][x % FK];
+    cs.aoff[x / FK][x % FK] = (uint16_t)(si.a_idx * FES);  // a_idx = 16 for an invalid signature: the zero row
+    cs.bcls[x / FK][x % FK] = (uint8_t)(si.b_idx >= 0 ? si.b_idx : FNS);
+  }
+  for (int e = tid; e < FNS * FNS; e += blockDim.x) {
+    const int a = e / FNS, b = e % FNS;
+    int idx[3 * FD];
+    r_slots<FD>(a, b, idx);
+    cs.slot_lo[e >> 5][e & 31] = idx[0] | idx[1] << 6 | idx[2] << 12 | idx[3] << 18 | idx[4] << 24;
+    cs.sym[e >> 5][e & 31] = (a * FES + b) | (dual_vec<FD>(b) * FES + dual_vec<FD>(a)) << 9 | idx[5] << 26;
+  }
+  __syncthreads();
+
+  // ---- once per warp: tile-invariant roles of this lane ---------------------------------------------------------
+  for (int x = lane; x < FES * FES; x += 32) ws.Esym[x] = 0;
+  if (lane < 2 * FD) ws.TAB[lane * FSTRIDE + FNC] = 0;
+  // step 1: lane (x, m) for lane < 20
+  const int q_x = lane >> 2, q_m = lane & 3;
+  const uint32_t q_sub = (uint32_t)mp.sub[q_m];
+  const uint64_t q_magic = mp.magic_sub[q_m];
+  // step 2: lanes 0..17 = (level, split configuration) for the input tensor and the weight gradient; lanes 18..26 = local sizes
+  const int role_i = lane < 18 ? lane : lane - 18;
+  const int role_d = lane < 18 ? role_i / FNC : 0, role_cfg = role_i % FNC;
+  int role_m0 = 0, role_m1 = 0;
+  cfg_masks<FD>(role_cfg, role_m0, role_m1);
+  const int64_t r_p = mp.size[role_d], r_alpha = mp.alpha[role_d], r_beta = mp.beta[role_d];
+  const uint64_t r_magic = mp.magic_size[role_d];
+  const int64_t cap_layer = mp.mem_cap / L;
+  // chain DP: lane (b, half)
+  const int dp_b = lane & 15, dp_h = lane >> 4;
+
+  const int nslots = gridDim.x * W;
+  for (int p = warp * gridDim.x + blockIdx.x; p < Bp; p += nslots) {
+    const autoddl_layer* chain = layers + (size_t)p * L;
+    auto stage = [&](int b, int l) {                        // lanes 0..3: the 64-byte record; lane 4: the previous kind
+      if (lane < 5) {
+        const autoddl_layer* cur = chain + l;
+        RecBuf* dst = &ws.rec[b];
+        if (lane < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * lane, reinterpret_cast<const unsigned char*>(cur) + 16 * lane);
+        else cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
+      }
+    };
+    stage(0, 0);
+    const bool cd = cd_init != nullptr;
+    if (cd) {
+      for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)p * cd_S * L + x];
+    }
+    int cur = 0;
+
+    for (int l = 0; l < L; ++l) {
+      if (lane < 5) cp_async_wait_all();
+      __syncwarp();
+      if (l + 1 < L) stage((l + 1) & 1, l + 1);
+      const RecBuf& rec = ws.rec[l & 1];
+      const int kind = rec.kind, kind_prev = rec.kind_prev;
+      const size_t tile = (size_t)p * L + l;
+
+      // ---- 1. Q[x][m] = ceil(extent x / product of the levels in m) -------------------------------------------------
+      if (lane < 20) ws.Q[q_x][q_m] = cdiv_magic(rec.X[q_x], q_sub, q_magic);
+      __syncwarp();
+
+      // ---- 2. Table 2 per level and split configuration -------------------------------------------
+      if (lane < 18) {
+        if (l > 0) {                                         // the layer's input tensor: gather / scatter and all-to-all
+          const int64_t n = ws.Q[3][role_m0] * ws.Q[4][role_m1] * (int64_t)rec.eb;
+          int64_t cg = 0, ca = 0;
+          if (r_p > 1) {
+            cg = mp.accum * ((r_p - 1) * (r_alpha + cdiv_magic(n, (uint32_t)r_p, r_magic) * r_beta));
+            ca = mp.accum * ((r_p - 1) * r_alpha + n * r_beta);          // R25: once per micro-batch
+          }
+          ws.TAB[role_d * FSTRIDE + role_cfg] = cg;
+          ws.TAB[(FD + role_d) * FSTRIDE + role_cfg] = ca;
+        }
+        if (kind == AUTODDL_GEMM) {                          // weight gradient: the AllReduce row
+          const int64_t n = ws.Q[1][role_m0] * ws.Q[2][role_m1] * (int64_t)rec.wgb;
+          ws.WAR[role_d][role_cfg] =
+              r_p > 1 ? (2 * r_p - 1) * r_alpha + 2 * (r_p - 1) * cdiv_magic(n, (uint32_t)r_p, r_magic) * r_beta : 0;
+        }
+      } else if (lane < 27) {
+        ws.locW[role_cfg] = ws.Q[1][role_m0] * ws.Q[2][role_m1];
+        ws.locO[role_cfg] = ws.Q[0][role_m0] * ws.Q[2][role_m1];
+      }
+      __syncwarp();
+
+      // ---- 3. VP[j] (node cost + penalty) and R[a][b] (zero for the first layer: no producer) -------------------------
+#pragma unroll
+      for (int j0 = 0; j0 < 64; j0 += 32) {
+        const int j = j0 + lane;
+        if (j < FK) {
+          const SigInfo si = cs.sig[kind][j];
+          int64_t v = 0, mem = 0;
+          if (si.valid) {
+            if (kind == AUTODDL_GEMM) {
+#pragma unroll
+              for (int d = 0; d < FD; ++d)
+                if (si.wB >> d & 1) v += ws.WAR[d][si.cfgW];
+              mem = ws.locW[si.cfgW] * (int64_t)rec.wsb;
+            }
+            mem += (ws.Q[3][si.mI0] * ws.Q[4][si.mI1] + ws.locO[si.cfgO]) * (int64_t)rec.eb;
+          }
+          const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc &&
+                          (mp.mem_cap == 0 || mem <= cap_layer);
+          ws.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+          if (node) node[tile * FK + j] = v;
+          if (mask) mask[tile * FK + j] = ok ? 1 : 0;
+        }
+      }
+      {
+        uint32_t sy[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) sy[k] = cs.sym[k][lane];
+        if (l > 0) {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const uint32_t lo = cs.slot_lo[k][lane];
+            ws.Esym[sy[k] & 511] = ws.TAB[lo & 63] + ws.TAB[lo >> 6 & 63] + ws.TAB[lo >> 12 & 63] + ws.TAB[lo >> 18 & 63] +
+                                   ws.TAB[lo >> 24 & 63] + ws.TAB[sy[k] >> 26];
+          }
+          __syncwarp();
+          int64_t es[8];                                     // forward leg + backward leg, in place: reads, then writes
+#pragma unroll
+          for (int k = 0; k < 8; ++k) es[k] = ws.Esym[sy[k] & 511] + ws.Esym[sy[k] >> 9 & 511];
+          __syncwarp();
+#pragma unroll
+          for (int k = 0; k < 8; ++k) ws.Esym[sy[k] & 511] = es[k];
+        } else {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) ws.Esym[sy[k] & 511] = 0;
+        }
+      }
+      __syncwarp();
+
+      // ---- 4. the tile: T[i][j] = VP[j] + Esym[A(i)][B(j)], 16-byte streaming stores --------------------------------------
+      // Columns 0..31: lane (h, pc) owns the column pair (2 pc, 2 pc + 1) -- its VP pair and B classes stay in registers --
+      // and the rows whose level-1 digit is 3 h + t, t = 0..2.  Rows whose digits agree up to the classes {0},{1},{3},
+      // {2,4,5} are identical (signatures 2, 4, 5 all output P, or are all invalid for ATTN), so a value pair is computed
+      // once per class row and stored to its 1 or 3 member rows: 12 gathers for 18 stores per lane; a half-warp store
+      // covers 256 contiguous bytes.  Columns 32..35: one lane per row, 32 contiguous bytes each.
+      if (T) {
+        int64_t* out = T + tile * FCELLS;
+        const uint16_t* aok = cs.aoff[kind_prev];
+        {
+          const int pc = lane & 15, h = lane >> 4;
+          const longlong2 vp = *reinterpret_cast<const longlong2*>(&ws.VP[2 * pc]);
+          const uint32_t bb = *reinterpret_cast<const uint16_t*>(&cs.bcls[kind][2 * pc]);
+          const int b0 = bb & 255, b1 = bb >> 8;
+          int64_t* o = out + (3 * h) * FK + 2 * pc;
+#pragma unroll
+          for (int c0 = 0; c0 < 4; ++c0) {
+            const int r0 = c0 < 2 ? c0 : (c0 == 2 ? 3 : 2);  // representative level-0 digit: 0, 1, 3, 2 (= 4 = 5)
+#pragma unroll
+            for (int t = 0; t < 3; ++t) {
+              const int ao = aok[r0 * 6 + 3 * h + t];
+              const longlong2 v = make_longlong2(vp.x + ws.Esym[ao + b0], vp.y + ws.Esym[ao + b1]);
+              __stcs(reinterpret_cast<longlong2*>(o + (r0 * 6 + t) * FK), v);
+              if (c0 == 3) {
+                __stcs(reinterpret_cast<longlong2*>(o + (4 * 6 + t) * FK), v);
+                __stcs(reinterpret_cast<longlong2*>(o + (5 * 6 + t) * FK), v);
+              }
+            }
+          }
+        }
+        {
+          const longlong2 vpa = *reinterpret_cast<const longlong2*>(&ws.VP[32]);
+          const longlong2 vpb = *reinterpret_cast<const longlong2*>(&ws.VP[34]);
+          const uint32_t bb = *reinterpret_cast<const uint32_t*>(&cs.bcls[kind][32]);
+#pragma unroll
+          for (int i0 = 0; i0 < 64; i0 += 32) {
+            const int i = i0 + lane;
+            if (i < FK) {
+              const int64_t* er = ws.Esym + aok[i];
+              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 32), make_longlong2(vpa.x + er[bb & 255], vpa.y + er[bb >> 8 & 255]));
+              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 34), make_longlong2(vpb.x + er[bb >> 16 & 255], vpb.y + er[bb >> 24]));
+            }
+          }
+        }
+      }
+
+      // ---- 5. chain DP (R9): f_l[j] = VP[j] + min_i f_{l-1}[i] + Esym[A(i)][B(j)], smallest i on ties -----------------
+      int64_t* fn = ws.f[cur ^ 1];
+      if (l == 0) {
+        for (int j = lane; j < FK; j += 32) fn[j] = ws.VP[j];            // f_0[j] = T[0][0][j]
+      } else {
+        const int64_t* f = ws.f[cur];
+        const uint16_t* ao = cs.aoff[kind_prev] + 18 * dp_h;
+        const int64_t* fh = f + 18 * dp_h;
+        int64_t pb[3];
+        int pa[3];
+#pragma unroll
+        for (int part = 0; part < 3; ++part) {             // three independent chains of six rows, merged in row order
+          int64_t tv[6], fv[6];
+#pragma unroll
+          for (int r = 0; r < 6; ++r) tv[r] = ws.Esym[ao[6 * part + r] + dp_b];
+#pragma unroll
+          for (int r = 0; r < 6; r += 2) {
+            const longlong2 f2 = *reinterpret_cast<const longlong2*>(fh + 6 * part + r);
+            fv[r] = f2.x;
+            fv[r + 1] = f2.y;
+          }
+          int64_t b = fv[0] + tv[0];
+          int ba = 6 * part;
+#pragma unroll
+          for (int r = 1; r < 6; ++r) {
+            const int64_t v = fv[r] + tv[r];
+            if (v < b) { b = v; ba = 6 * part + r; }
+          }
+          pb[part] = b;
+          pa[part] = ba;
+        }
+        int64_t best = pb[0];
+        int a = pa[0];
+        if (pb[1] < best) { best = pb[1]; a = pa[1]; }
+        if (pb[2] < best) { best = pb[2]; a = pa[2]; }
+        a += 18 * dp_h;
+        {
+          const int64_t o = __shfl_down_sync(0xffffffffu, best, 16);
+          const int oa = __shfl_down_sync(0xffffffffu, a, 16);
+          if (o < best) { best = o; a = oa; }              // rows 18..35 into rows 0..17: strict '<'
+        }
+        // consumer signatures that are invalid for the layer kind (class 16) have a zero edge: min_i f[i], smallest i
+        int64_t h16 = 0;
+        int a16 = 0;
+        if (kind != AUTODDL_GEMM) {
+          h16 = f[lane];
+          a16 = lane;
+          if (lane < FK - 32) {
+            const int64_t v = f[32 + lane];
+            if (v < h16) { h16 = v; a16 = 32 + lane; }
+          }
+          warp_argmin64(h16, a16);
+        }
+#pragma unroll
+        for (int j0 = 0; j0 < 64; j0 += 32) {
+          const int j = j0 + lane;
+          const int bj = cs.bcls[kind][j < FK ? j : 0];
+          int64_t hb = __shfl_sync(0xffffffffu, best, bj & 15);
+          int ha = __shfl_sync(0xffffffffu, a, bj & 15);
+          if (bj == FNS) { hb = h16; ha = a16; }
+          if (j < FK) {
+            fn[j] = ws.VP[j] + hb;
+            bp[(size_t)l * FK + j] = (uint8_t)ha;
+          }
+        }
+      }
+      cur ^= 1;
+
+      // ---- 6. first Coordinate Descent sweep (R10) of every start ------------------------------------------------------
+      if (cd) {
+        __syncwarp();
+        for (int st = 0; st < cd_S; ++st) {
+          {
+            uint8_t* sv = cd_s + (size_t)st * L;
+            int64_t* stash = cd_stash + st * FK;             // T[l][s_{l-1}][.] of this start, for the next layer's update
+            if (l > 0) {                                     // update of layer l-1: row stashed, column from this tile
+              const int right = sv[l];
+              const int bright = cs.bcls[kind][right];
+              int64_t bv = INT64_MAX;
+              int bi = FK;
+#pragma unroll
+              for (int q = 0; q < 2; ++q) {
+                const int c = 32 * q + lane;
+                if (c < FK) {
+                  const int64_t g = stash[c] + ws.Esym[cs.aoff[kind_prev][c] + bright];
+                  if (g < bv) { bv = g; bi = c; }
+                }
+              }
+              warp_argmin64(bv, bi);
+              if (lane == 0) sv[l - 1] = (uint8_t)bi;
+              __syncwarp();
+            }
+            // row T[l][s_{l-1}][.] for the update of layer l (s_{-1} := 0; E(0) = 0 whatever the row)
+            const int left = l > 0 ? sv[l - 1] : 0;
+            const int aleft = cs.aoff[kind_prev][left];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const int c = 32 * q + lane;
+              if (c < FK) stash[c] = ws.VP[c] + ws.Esym[aleft + cs.bcls[kind][c]];
+            }
+            __syncwarp();
+            if (l == L - 1) {                                // last layer: no right neighbour
+              int64_t bv = INT64_MAX;
+              int bi = FK;
+#pragma unroll
+              for (int q = 0; q < 2; ++q) {
+                const int c = 32 * q + lane;
+                if (c < FK && stash[c] < bv) { bv = stash[c]; bi = c; }
+              }
+              warp_argmin64(bv, bi);
+              if (lane == 0) sv[l] = (uint8_t)bi;
+              __syncwarp();
+            }
+          }
+        }
+      }
+      __syncwarp();
+    }
+
+    // ---- end of the chain: smallest argmin of f_{L-1}, back-track, results --------------------------------------------
+    {
+      const int64_t* f = ws.f[cur];
+      int64_t bv = f[lane];
+      int bi = lane;
+      if (lane < FK - 32) {
+        const int64_t v = f[32 + lane];
+        if (v < bv) { bv = v; bi = 32 + lane; }
+      }
+      warp_argmin64(bv, bi);
+      if (lane == 0) {
+        int32_t* sp = strategy + (size_t)p * L;
+        opt_cost[p] = bv;
+        int sidx = bi;
+        sp[L - 1] = sidx;
+        for (int ll = L - 1; ll >= 1; --ll) {
+          sidx = bp[(size_t)ll * FK + sidx];
+          sp[ll - 1] = sidx;
+        }
+      }
+      if (cd) {
+        for (int x = lane; x < cd_S * L; x += 32) cd_s1[(size_t)p * cd_S * L + x] = cd_s[x];
+      }
+      __syncwarp();
+    }
+  }
+}
+
+int fused_sm_count() {
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
+  return sms;
+}
+
+constexpr int kMaxWarps = 28;
+constexpr size_t kSmemBudget = 224 * 1024;
+
+// back-pointers [L][36] of the chain a warp has in flight: in its shared memory when they fit, else in the workspace
+size_t warp_bytes(int32_t L, int32_t S, bool bp_smem) {
+  const size_t cd = S > 0 ? (((size_t)S * L + 15) & ~(size_t)15) + (size_t)S * FK * 8 : 0;
+  return (sizeof(WarpShared) + cd + (bp_smem ? (size_t)L * FK : 0) + 127) & ~(size_t)127;
+}
+bool bp_fits_smem(int32_t L, int32_t S) { return 8 * warp_bytes(L, S, true) + sizeof(CtaShared) + 128 <= kSmemBudget; }
+
+}  // namespace
+
+bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim == 2 && L >= 1; }
+
+// largest S for which the first CD sweep rides in the fused kernel (one row stash of two registers per start and lane)
+bool fused_cd_sweep_supported(int32_t L, int32_t S) { return S >= 1 && S <= kMaxFusedStarts && (int64_t)S * L <= 8192; }
+
+size_t fused_bp_bytes(int32_t L) {
+  static const int sms = fused_sm_count();                 // host-only query, cached
+  if (bp_fits_smem(L, kMaxFusedStarts)) return 256;
+  return ((size_t)sms * kMaxWarps * L * FK + 255) / 256 * 256 + 256;
+}
+
+// Fused (a1) + (a2) for K = 36: tables (d_T may be NULL: no table is written) and the chain DP in one kernel, plus the
+// first CD sweep of S <= 4 starts per chain.  d_bp: fused_bp_bytes(L) of workspace (back-pointers of very long chains).
+int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
+                          int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
+                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, cudaStream_t st) {
+  if ((int64_t)Bp * L > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  if (!fused_build_dp_supported(mp, L)) { set_error("fused build+DP needs a 2-level mesh"); return AUTODDL_EINVAL; }
+  if (d_cd_init && (!fused_cd_sweep_supported(L, S) || d_cd_s1 == nullptr)) { set_error("fused CD sweep: too many starts"); return AUTODDL_EINVAL; }
+  const int cdS = d_cd_init ? S : 0;
+  const bool bp_smem = bp_fits_smem(L, cdS);
+  if (!bp_smem && d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
+  const size_t per_warp = warp_bytes(L, cdS, bp_smem);
+  const size_t fixed = ((sizeof(CtaShared) + 127) & ~(size_t)127);
+  int wmax = (int)((kSmemBudget - fixed) / per_warp);
+  if (wmax > kMaxWarps) wmax = kMaxWarps;
+  if (wmax < 1) { set_error("fused build+DP: chain too long for shared memory"); return AUTODDL_EINVAL; }
+  const int sms = fused_sm_count();
+  // warps per CTA (one CTA per SM): the fewest that reach the minimal number of rounds of chains per warp
+  const int rounds = (Bp + sms * wmax - 1) / (sms * wmax);
+  int W = (Bp + sms * rounds - 1) / (sms * rounds);
+  if (W < 4) W = Bp < 4 * sms ? (Bp + sms - 1) / sms : 4;
+  if (W > wmax) W = wmax;
+  if (W < 1) W = 1;
+  const int grid = Bp < sms * W ? (Bp + W - 1) / W : sms;
+  const size_t smem = fixed + (size_t)W * per_warp;
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(fused_chain36_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  fused_chain36_kernel<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy,
+                                                   bp_smem ? nullptr : d_bp, d_cd_init, cdS, d_cd_s1, (int)per_warp);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+}  // namespace autoddl
