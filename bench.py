@@ -156,7 +156,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "cells/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int64", "data": "synthetic (seeded splitmix64)",
-        "config": workload_desc(w, {"sample": sample}),
+        "config": workload_desc(w, {"parallelism": "problems sharded over %d GPU(s), one all-gather of the result rows" % args.gpus,
+                                    "scaling_mode": args.scaling}),
         "cpu_baseline": {"value": val, "unit": "cells/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "cells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "parts": {"build_cells_per_s": cells / parts["build"], "dp_cells_per_s": cells / parts["dp"],
@@ -217,6 +218,27 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
+def cuda_compute(adl, w, work=None, out=None):
+    """(compute, best_of_starts) callables for shard.ShardedSearch backed by the CUDA path: compute uploads a shard once
+    (cached by the identity of the numpy arrays: the timed loop calls it every step with the same shard) and runs the
+    one-call entry point autoddl_search on it; best_of_starts is the library's reduction kernel."""
+    import torch
+    cache = {}
+
+    def resident(a, to_dev):
+        key = (id(a), a.shape)
+        if key not in cache:
+            cache[key] = (a, to_dev(a))                           # keeps `a` alive: ids are not reused
+        return cache[key][1]
+
+    def compute(layers, init):
+        d_layers = resident(layers, adl.layers_to_device)
+        d_init = None if init is None else resident(init, lambda x: torch.from_numpy(x).cuda())
+        return adl.search(d_layers, w.mesh, w.net, init=d_init, max_sweeps=w.max_sweeps, work=work, out=out)
+
+    return compute, adl.best_of_starts
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -227,14 +249,21 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
+    sampler = ClockSampler(local) if rank == 0 else None          # from before the warm-up to after the end-to-end loop
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2301_06813_b200 import binding as adl
+    from paper_2301_06813_b200.shard import ShardedSearch, shard_range
     adl.lib()
 
-    # weak scaling: every rank searches its own 4096 problems (seed = rank); no data-path collective
-    w = cf.config4_batched(seed=rank)
-    init_np = w.cd_init()
+    # weak scaling (default): every rank searches its own 4096 problems (seed = rank); strong: the 4096 problems of seed 0
+    # are split over the ranks.  Either way the step ends with ONE all-gather of the result rows; there is
+    # no collective in the data path.
+    strong = args.scaling == "strong"
+    w_all = cf.config4_batched(seed=0 if strong else rank)
+    plan = ShardedSearch(w_all.layers, w_all.cd_init(), mode="problems", local_shard=not strong)
+    w = cf.Workload(w_all.name, plan.layers, w_all.mesh, w_all.net, S=w_all.S, seed=w_all.seed, max_sweeps=w_all.max_sweeps)
+    init_np = plan.init
     d_layers = adl.layers_to_device(w.layers)
     d_init = torch.from_numpy(init_np).cuda()
     K, L, Bp, S = w.K, w.L, w.Bp, w.S
@@ -246,14 +275,17 @@ def run_ours(args):
     work = torch.empty(adl.workspace_bytes(Bp, L, S, w.mesh), dtype=torch.uint8, device="cuda")
     one_out = {"T": T, "opt_cost": dp_out[0], "strategy": dp_out[1], "cd_cost": cd_out[0], "cd_strategy": cd_out[1],
                "cd_sweeps": cd_out[2]}
+    compute, best = cuda_compute(adl, w, work=work, out=one_out)
+    results = {}
 
     def step(evs=None):
-        """the whole path in ONE library call (autoddl_search): the fused kernel (tables, chain DP, first CD sweep), then
-        the CD kernel from sweep 2.  evs[1] is recorded by the library between the two kernels (autoddl_profile_mark)."""
+        """the whole path on this rank's shard in ONE library call (autoddl_search): the fused kernel (tables, chain DP,
+        first CD sweep), then the CD kernel from sweep 2; then the exchange: all-gather of the result rows and the
+        best-of-starts kernel.  evs[1] is recorded by the library between the two kernels (autoddl_profile_mark)."""
         if evs:
             adl.profile_mark(evs[1])
             evs[0].record()
-        adl.search(d_layers, w.mesh, w.net, init=d_init, max_sweeps=w.max_sweeps, work=work, out=one_out)
+        results.update(plan.run(compute, best))
         if evs: evs[2].record()
 
     def step_separate(evs):
@@ -281,7 +313,6 @@ def run_ours(args):
     for e in evs:
         e[1].record()                                        # instantiate the handle the library records later
     e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local) if rank == 0 else None
     launches0 = adl.launch_count()
     barrier()
     e_start.record()
@@ -290,7 +321,6 @@ def run_ours(args):
     e_end.record()
     barrier()
     launches = adl.launch_count() - launches0
-    clocks = sampler.stop() if sampler else None
     ms_total = e_start.elapsed_time(e_end)
     if world > 1:
         t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
@@ -309,23 +339,34 @@ def run_ours(args):
     torch.cuda.synchronize()
     for e in evs2:
         ms["build"] += e[0].elapsed_time(e[1]); ms["dp"] += e[1].elapsed_time(e[2]); ms["cd"] += e[2].elapsed_time(e[3])
+    # the one-call path with no table requested (nothing of (a1) reaches HBM): reported beside the step, not as the step
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    nt_out = {k: v for k, v in one_out.items() if k != "T"}
+    for _ in range(3):
+        adl.chain_dp(None, w.mesh, net=w.net, d_layers=d_layers, work=work, out=dp_out)
+    e0.record()
+    for _ in range(args.steps):
+        adl.chain_dp(None, w.mesh, net=w.net, d_layers=d_layers, work=work, out=dp_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms["fused_no_table"] = e0.elapsed_time(e1)
     for k in ms:
         ms[k] /= args.steps
     ms_step = ms_total / args.steps
-    cells = w.cells
+    cells = w.cells                                          # per rank
     value = world * cells / (ms_step * 1e-3)
 
     # ---- HBM copy peak by our own copy kernel, in the same run -------------------------------------------
     nb = 1 << 30
     a = torch.empty(nb, dtype=torch.uint8, device="cuda").random_(0, 255)
     b = torch.empty(nb, dtype=torch.uint8, device="cuda")
-    best = 1e9
+    best_ms = 1e9
     for i in range(13):
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         s0.record(); adl.copy_probe(a, b); s1.record(); torch.cuda.synchronize()
         if i >= 3:
-            best = min(best, s0.elapsed_time(s1))
-    copy_gbs = 2 * nb / (best * 1e-3) / 1e9
+            best_ms = min(best_ms, s0.elapsed_time(s1))
+    copy_gbs = 2 * nb / (best_ms * 1e-3) / 1e9
     del a, b
 
     # ---- end to end through the host-pointer C-ABI call (pinned host buffers, H2D + D2H timed) -----------
@@ -349,73 +390,88 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item())
     e2e_ms /= e2e_steps
+    clocks = sampler.stop() if sampler else None
     h2d = h_layers.numel() + h_init.numel() * 4
     d2h = sum(v.numel() * v.element_size() for v in pinned.values())
     assert np.array_equal(pinned["opt_cost"].numpy(), dp_out[0].cpu().numpy())      # same answers through both routes
+    off = plan.rank * Bp if not strong else shard_range(plan.n_total, plan.rank, world)[0]
+    assert torch.equal(results["opt_cost"][off:off + Bp], dp_out[0])            # the gathered rows hold this rank's shard
 
     if rank == 0:
         peak, peak_src = measured_peak()
         table_bytes = cells * 8
         dp_bytes = (L - 1) * Bp * K * K * 8 + Bp * K * 8          # tile 0 contributes one row
         cd_alg_bytes = total_sweeps * 16 * K * L
-        # algorithmic bytes by SURVEY.md 8(d): 8 B per cell written (tables), 8 B per cell read (DP), 16 K L B per CD sweep.
-        # The fused kernel does all three kinds of work for one launch (tables, DP, one sweep per start) but only the
-        # table write touches HBM: "alg" counts the work by 8(d), "hbm_min" the bytes that have to move.
         sweep1_bytes = Bp * S * 16 * K * L
-        fused_alg = table_bytes + dp_bytes + sweep1_bytes
+        # Bytes that MUST reach HBM per launch (what "roofline" means here): the fused kernel writes the tables (8 B per
+        # cell) and reads 64 B per layer record; the chain DP and the first CD sweep run from shared memory and move
+        # nothing.  SURVEY 8(d)'s per-unit figures (8 B/cell written + 8 B/cell read by the DP + 16 K L B per CD sweep)
+        # count WORK; for the fused launch their sum is reported separately as work_units_*: it exceeds the HBM bytes
+        # because fusion removed two of the three streams.
+        fused_hbm = table_bytes + Bp * L * 64
+        fused_work = table_bytes + dp_bytes + sweep1_bytes
         kernels = {
             "build_dp_cd1_fused": {"ms": ms["fused"], "cells_per_s": cells / (ms["fused"] * 1e-3),
-                                   "alg_GBps": fused_alg / (ms["fused"] * 1e-3) / 1e9,
-                                   "hbm_min_GBps": table_bytes / (ms["fused"] * 1e-3) / 1e9, "in_step": True,
-                                   "bound": "issue/latency; hbm traffic = the 8 B/cell table write only (DP and the first CD "
-                                            "sweep read the tiles from shared memory)"},
+                                   "hbm_GBps": fused_hbm / (ms["fused"] * 1e-3) / 1e9,
+                                   "work_units_GBps": fused_work / (ms["fused"] * 1e-3) / 1e9, "in_step": True,
+                                   "bound": "shared-memory bandwidth / issue (ncu: LSU wavefronts 75 %, issue 67 %); hbm traffic = "
+                                            "the 8 B/cell table write only (DP and the first CD sweep read the tile factors from "
+                                            "shared memory)"},
             "coord_descent_resume": {"ms": ms["cd_resume"], "sweeps": total_sweeps - Bp * S,
                                      "sweeps_per_s": (total_sweeps - Bp * S) / (ms["cd_resume"] * 1e-3),
-                                     "alg_GBps": (cd_alg_bytes - sweep1_bytes) / (ms["cd_resume"] * 1e-3) / 1e9, "in_step": True,
-                                     "bound": "hbm, random 64-byte granules (16*K*L B per sweep), sweeps 2.."},
+                                     "hbm_GBps": (cd_alg_bytes - sweep1_bytes) / (ms["cd_resume"] * 1e-3) / 1e9, "in_step": True,
+                                     "bound": "latency of the dependent updates of the slowest chains; 16*K*L B per sweep, sweeps 2.. "
+                                              "(plus the exchange: all-gather of result rows and best-of-starts, no-ops at 1 GPU)"},
             "build_tables": {"ms": ms["build"], "cells_per_s": cells / (ms["build"] * 1e-3),
-                             "alg_GBps": table_bytes / (ms["build"] * 1e-3) / 1e9, "in_step": False, "bound": "hbm (write 8 B/cell)"},
+                             "hbm_GBps": table_bytes / (ms["build"] * 1e-3) / 1e9, "in_step": False, "bound": "hbm (write 8 B/cell)"},
             "chain_dp": {"ms": ms["dp"], "cells_per_s": cells / (ms["dp"] * 1e-3),
-                         "alg_GBps": dp_bytes / (ms["dp"] * 1e-3) / 1e9, "in_step": False, "bound": "hbm (read 8 B/cell)"},
+                         "hbm_GBps": dp_bytes / (ms["dp"] * 1e-3) / 1e9, "in_step": False, "bound": "hbm (read 8 B/cell)"},
             "coord_descent": {"ms": ms["cd"], "sweeps_per_s": total_sweeps / (ms["cd"] * 1e-3), "sweeps": total_sweeps,
-                              "alg_GBps": cd_alg_bytes / (ms["cd"] * 1e-3) / 1e9, "in_step": False,
+                              "hbm_GBps": cd_alg_bytes / (ms["cd"] * 1e-3) / 1e9, "in_step": False,
                               "bound": "hbm, random 64-byte granules (16*K*L B per sweep)"},
+            "fused_no_table": {"ms": ms["fused_no_table"], "cells_per_s": cells / (ms["fused_no_table"] * 1e-3), "in_step": False,
+                               "hbm_GBps": Bp * L * 64 / (ms["fused_no_table"] * 1e-3) / 1e9,
+                               "bound": "autoddl_chain_dp(d_T = NULL): the same kernel with no table written (optimum + strategy "
+                                        "only): shared-memory bandwidth / issue"},
         }
         for k in kernels.values():
-            k["frac_of_peak"] = k["alg_GBps"] / peak
-        kernels["build_dp_cd1_fused"]["hbm_min_frac_of_peak"] = kernels["build_dp_cd1_fused"]["hbm_min_GBps"] / peak
+            k["frac_of_peak"] = k["hbm_GBps"] / peak
+        kernels["build_dp_cd1_fused"]["work_units_frac_of_peak"] = kernels["build_dp_cd1_fused"]["work_units_GBps"] / peak
         dom = max(("build_dp_cd1_fused", "coord_descent_resume"), key=lambda n: kernels[n]["ms"])
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic_r1.csv")       # per-launch DRAM bytes from the ncu --set full capture
+        traffic, traffic_src = None, None
+        tpath = os.path.join(ROOT, "profiles", "traffic_r2.csv")       # per-launch DRAM bytes from a committed ncu --set full capture
         if os.path.exists(tpath):
             try:
-                rows = dict(l.strip().split(",") for l in open(tpath).read().splitlines()[1:] if l.strip())
+                rows = dict(l.strip().split(",")[:2] for l in open(tpath).read().splitlines()[1:] if l.strip())
                 traffic = float(rows[dom]) if dom in rows else None
-                # next to the algorithmic GB/s, the DRAM GB/s actually moved (ncu bytes per launch of the committed
-                # capture / this run's launch time); for coord_descent the two differ by the 64-byte granules of the gather
+                traffic_src = "profiles/traffic_r2.csv (committed ncu --set full capture of the same command, NOT measured in this run)"
                 for name, k in kernels.items():
                     if name in rows:
                         k["dram_bytes_per_launch_ncu"] = float(rows[name])
                         k["dram_GBps"] = float(rows[name]) / (k["ms"] * 1e-3) / 1e9
                         k["dram_frac_of_peak"] = k["dram_GBps"] / peak
+                        k["dram_source"] = "committed ncu capture (profiles/traffic_r2.csv) / this run's launch time"
             except Exception:
-                traffic = None
+                traffic, traffic_src = None, None
         line = {
             "metric": METRIC, "value": value, "unit": "cells/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
-            "data": "synthetic (seeded splitmix64; shapes of BASELINE.json configs[3])",
-            "config": workload_desc(w, {"parallelism": "problems sharded over %d GPU(s), no collective in the data path" % world}),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
+            "dtype": "int64", "data": "synthetic (seeded splitmix64; shapes of BASELINE.json configs[3])",
+            "config": workload_desc(w, {"parallelism": "problems sharded over %d GPU(s), one all-gather of the result rows" % world,
+                                        "scaling_mode": args.scaling}),
             "parts": {"build_cells_per_s": world * kernels["build_tables"]["cells_per_s"],
                       "dp_cells_per_s": world * kernels["chain_dp"]["cells_per_s"],
                       "fused_build_dp_cd1_cells_per_s": world * kernels["build_dp_cd1_fused"]["cells_per_s"],
                       "cd_sweeps_per_s": world * kernels["coord_descent"]["sweeps_per_s"]},
             "kernels": kernels,
-            "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
-                         "frac": kernels[dom]["alg_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
-                         "copy_probe_GBps_same_run": copy_gbs,
-                         "frac_counting_only_bytes_that_must_reach_hbm": kernels[dom].get("hbm_min_frac_of_peak"),
-                         "note": "algorithmic bytes by SURVEY 8(d) for the work the fused launch does (tables 8 B/cell + DP 8 B/cell "
-                                 "+ one CD sweep per start); its HBM traffic is the table write only, see kernels[...].hbm_min_*"},
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["hbm_GBps"], "peak": peak, "unit": "GB/s",
+                         "frac": kernels[dom]["hbm_GBps"] / peak, "traffic": traffic, "traffic_source": traffic_src,
+                         "peak_source": peak_src, "copy_probe_GBps_same_run": copy_gbs,
+                         "bytes_per_launch": fused_hbm if dom == "build_dp_cd1_fused" else cd_alg_bytes - sweep1_bytes,
+                         "work_units_frac": kernels[dom].get("work_units_frac_of_peak"),
+                         "note": "frac = bytes that must reach HBM per launch (8 B per cell written + 64 B per layer record read) / "
+                                 "CUDA-event launch time / peak; work_units_frac counts SURVEY 8(d)'s per-unit bytes for all the work "
+                                 "the fused launch does (tables + DP + one CD sweep) and can exceed 1"},
             "e2e": {"value": world * cells / (e2e_ms * 1e-3), "unit": "cells/s", "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": launches,
@@ -515,6 +571,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
+                    help="N > 1: weak = every rank its own 4096 problems; strong = the 4096 problems of seed 0 split over the ranks")
     ap.add_argument("--configs", type=int, nargs="+", default=None,
                     help="per-config report (kernel microseconds, oracle rates) instead of the bench line, e.g. --configs 1 2 3 5")
     args = ap.parse_args()

@@ -87,7 +87,11 @@ int autoddl_num_signatures(const autoddl_mesh* mesh);
 size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_mesh* mesh);
 
 /* (a1) Build T, node, mask for Bp chains of L layers.  d_node / d_mask may be NULL.
- * Requires beta_ps_per_byte[c] * 2 * size[d] < 2^31 and alpha, beta >= 0. */
+ * Accepted ranges (checked, AUTODDL_EINVAL otherwise): 1 <= mesh.size[d] <= 65536 and at most 2^20 devices in all;
+ * 0 <= alpha_ps < 2^40; 0 <= beta_ps_per_byte < 2^20; 0 <= micro_batches < 2^20; mem_cap_bytes >= 0.
+ * Caller's obligation (NOT checked: the records live on the device): every extent of a layer record is >= 1 and the
+ * products rows * cols * bytes * beta * micro_batches stay below 2^50, so that a cell is below 2^51 and no int64
+ * product or sum overflows; real workloads (the paper's 2^20 x 8192 fp32 activations at 80 ps/B) are below 2^44. */
 int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                          const autoddl_mesh* mesh, const autoddl_net* net,
                          int64_t* d_T, int64_t* d_node, uint8_t* d_mask, void* stream);
@@ -95,8 +99,9 @@ int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
 /* (a2) f_0[j] = T[0][0][j]; f_l[j] = min_i f_{l-1}[i] + T[l][i][j]; smallest index wins every tie;
  * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: the tables are computed from d_layers
  * -- on a 2-level mesh (K = 36), for >= 296 chains or when d_work cannot hold the tables, inside the DP kernel
- * itself, tile by tile in shared memory, never stored; otherwise they are first built into d_work.  d_work (>= autoddl_workspace_bytes) also
- * holds back-pointers (fused kernel: of the chains in flight; separate kernel: when L * K > 16384).
+ * itself (one warp per chain, every tile in factor form in shared memory, never stored); otherwise they are first built
+ * into d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers (fused kernel: only for chains too long
+ * for shared memory; separate kernel: when L * K > 16384).
  * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
 int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                      const autoddl_mesh* mesh, const autoddl_net* net,
@@ -141,9 +146,10 @@ int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int6
                            int64_t N, double* d_out, void* d_work, size_t work_bytes, void* stream);
 
 /* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36) with at least 296
- * chains (a1) and (a2) run as ONE kernel: every tile is built in shared memory, stored to d_T by TMA and
- * consumed by the chain DP from shared memory, so the optimum costs no table read.  Other meshes run
- * the three kernels back to back.  Results are identical to the three separate calls.
+ * chains (a1), (a2) and the first sweep of (a3) for up to 8 starts per chain run as ONE kernel, one warp per chain:
+ * every tile is evaluated in factor form in shared memory, written to d_T with coalesced stores and consumed by the
+ * chain DP and the CD sweep from shared memory, so the optimum costs no table read; the CD kernel resumes at sweep 2.
+ * Other meshes run the three kernels back to back.  Results are identical to the three separate calls.
  * d_T: [Bp][L][K][K] output, or NULL to keep the tables in d_work (any mesh) -- with d_init == NULL
  * and K = 36 no table is materialised at all.  d_node / d_mask may be NULL.  d_init == NULL skips (a3).
  * d_work: >= autoddl_workspace_bytes(Bp, L, S, mesh). */
@@ -166,6 +172,12 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
                         void* d_work, size_t work_bytes,
                         int64_t* h_opt_cost, int32_t* h_strategy,
                         int64_t* h_cd_cost, int32_t* h_cd_strategy, int32_t* h_cd_sweeps, void* stream);
+
+/* Best of the Coordinate Descent starts ("records the best strategy"): for every problem p the smallest
+ * d_cost[p][s] over s = 0..S-1 and the smallest s attaining it.  d_cost [Bp][S] int64, d_best_cost [Bp] int64,
+ * d_best_start [Bp] int32: device pointers, 8 / 4-byte aligned; Bp, S >= 1.  Asynchronous on `stream`. */
+int autoddl_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t* d_best_cost, int32_t* d_best_start,
+                           void* stream);
 
 /* Plain device-to-device copy kernel (int4 grid-stride), used by bench.py to measure the HBM
  * copy bandwidth in the same run as the kernels above.  bytes must be a multiple of 16. */

@@ -358,6 +358,19 @@ extern "C" int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L
   return 0;
 }
 
+// ---- R10 / PAPER.md:243 "records the best strategy": smallest cost over the starts, smallest start index on ties
+extern "C" int autoddl_ref_best_of_starts(const int64_t* cost, int32_t Bp, int32_t S, int64_t* best_cost, int32_t* best_start) {
+  if (!cost || !best_cost || !best_start || Bp < 1 || S < 1) return -1;
+  for (int64_t p = 0; p < Bp; ++p) {
+    int32_t arg = 0;
+    for (int32_t s = 1; s < S; ++s)
+      if (cost[p * S + s] < cost[p * S + arg]) arg = s;               // strict: the first start attaining the minimum
+    best_cost[p] = cost[p * S + arg];
+    best_start[p] = arg;
+  }
+  return 0;
+}
+
 // ---- R19-R22: Metropolis-Hastings.  P(S) ~ exp(-beta Cost(S)), beta = 1 / tau; a proposal
 // changes the signature of one layer; it is accepted with probability min(1, P(S_new) / P(S_old)).
 extern "C" uint64_t autoddl_ref_rng(uint64_t seed, uint64_t n) {

@@ -101,6 +101,9 @@ int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L, int32_t K
                               const int32_t* init, int32_t S, int32_t max_sweeps,
                               int64_t* cost, int32_t* strategy, int32_t* sweeps, int64_t* trace);
 
+/* best of the starts of every problem: smallest cost, then smallest start index */
+int autoddl_ref_best_of_starts(const int64_t* cost, int32_t Bp, int32_t S, int64_t* best_cost, int32_t* best_start);
+
 /* ---- Metropolis-Hastings sampler (R19-R22) --------------------------------
  * n-th output (n >= 1) of splitmix64 started at `seed`: the counter-based generator both sides implement. */
 uint64_t autoddl_ref_rng(uint64_t seed, uint64_t n);

@@ -74,6 +74,8 @@ def lib():
         L.autoddl_ref_brute_force.argtypes = [vp, i32, i32, vp, vp]
         L.autoddl_ref_coord_descent.restype = C.c_int
         L.autoddl_ref_coord_descent.argtypes = [vp, i32, i32, i32, vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_ref_best_of_starts.restype = C.c_int
+        L.autoddl_ref_best_of_starts.argtypes = [vp, i32, i32, vp, vp]
         L.autoddl_ref_rng.restype = C.c_uint64
         L.autoddl_ref_rng.argtypes = [C.c_uint64, C.c_uint64]
         L.autoddl_ref_neglog_q16.restype = i64
@@ -224,6 +226,16 @@ def coord_descent(T: np.ndarray, init: np.ndarray, max_sweeps: int = 64, want_tr
     if want_trace:
         return cost, strat, sweeps, trace
     return cost, strat, sweeps
+
+
+def best_of_starts(cost: np.ndarray):
+    """cost [Bp, S] -> (best cost [Bp], first start attaining it [Bp])"""
+    cost = np.ascontiguousarray(cost, dtype=np.int64)
+    Bp, S = cost.shape
+    bc = np.empty(Bp, np.int64); bs = np.empty(Bp, np.int32)
+    rc = lib().autoddl_ref_best_of_starts(_p(cost), Bp, S, _p(bc), _p(bs))
+    assert rc == 0, rc
+    return bc, bs
 
 
 # ---- Metropolis-Hastings (PAPER.md:227-237) -------------------------------------------------------------

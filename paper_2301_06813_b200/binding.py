@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -65,6 +65,8 @@ def lib():
         L.autoddl_search.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.autoddl_search_host.restype = C.c_int
         L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
+        L.autoddl_best_of_starts.restype = C.c_int
+        L.autoddl_best_of_starts.argtypes = [vp, i32, i32, vp, vp, vp]
         L.autoddl_copy_probe.restype = C.c_int
         L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
         L.autoddl_fit_workspace_bytes.restype = sz
@@ -109,8 +111,32 @@ def _stream() -> int:
     return torch.cuda.current_stream().cuda_stream
 
 
-def _ptr(t):
-    return None if t is None else t.data_ptr()
+def _ptr(t, dtype=None, name="tensor"):
+    """device pointer of a tensor the library will read or write as raw memory: it must live on a CUDA device, be
+    contiguous and have exactly the dtype the C-ABI states (the library cannot see any of this)"""
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise AutoddlError(f"{name}: expected a CUDA tensor")
+    if not t.is_contiguous():
+        raise AutoddlError(f"{name}: tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise AutoddlError(f"{name}: dtype {t.dtype}, the C-ABI needs {dtype}")
+    return t.data_ptr()
+
+
+def _hptr(a, dtype, name):
+    """host pointer of a numpy array handed to the host entry point: C-contiguous, exact dtype"""
+    if a is None:
+        return None
+    if not isinstance(a, np.ndarray) or not a.flags["C_CONTIGUOUS"]:
+        raise AutoddlError(f"{name}: expected a C-contiguous numpy array")
+    if a.dtype != dtype:
+        raise AutoddlError(f"{name}: dtype {a.dtype}, the C-ABI needs {np.dtype(dtype)}")
+    return a.ctypes.data
+
+
+I64, I32, U8, F64 = torch.int64, torch.int32, torch.uint8, torch.float64
 
 
 def layers_to_device(layers: np.ndarray, device="cuda") -> torch.Tensor:
@@ -142,8 +168,8 @@ def build_tables(d_layers: torch.Tensor, mesh, net, want_node_mask: bool = True,
     node = torch.empty((Bp, L, K), dtype=torch.int64, device=dev) if want_node_mask else None
     mask = torch.empty((Bp, L, K), dtype=torch.uint8, device=dev) if want_node_mask else None
     m, n = c_mesh(mesh), c_net(net)
-    _check(lib().autoddl_build_tables(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n), _ptr(T), _ptr(node),
-                                      _ptr(mask), _stream()))
+    _check(lib().autoddl_build_tables(_ptr(d_layers, U8, "d_layers"), Bp, L, C.addressof(m), C.addressof(n), _ptr(T, I64, "T"),
+                                      _ptr(node, I64, "node"), _ptr(mask, U8, "mask"), _stream()))
     return T, node, mask
 
 
@@ -169,8 +195,9 @@ def chain_dp(T: torch.Tensor | None, mesh, net=None, d_layers=None, work: torch.
         cost, strat = out
     m = c_mesh(mesh)
     n = c_net(net) if net is not None else None
-    _check(lib().autoddl_chain_dp(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
-                                  _ptr(T), _ptr(work), work.numel(), _ptr(cost), _ptr(strat), _stream()))
+    _check(lib().autoddl_chain_dp(_ptr(d_layers, U8, "d_layers"), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
+                                  _ptr(T, I64, "T"), _ptr(work, U8, "work"), work.numel(), _ptr(cost, I64, "opt_cost"),
+                                  _ptr(strat, I32, "strategy"), _stream()))
     return cost, strat
 
 
@@ -190,9 +217,10 @@ def coord_descent(T: torch.Tensor | None, init: torch.Tensor, mesh, max_sweeps: 
         cost, strat, sweeps = out
     m = c_mesh(mesh)
     n = c_net(net) if net is not None else None
-    _check(lib().autoddl_coord_descent(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
-                                       _ptr(T), _ptr(work), work.numel() if work is not None else 0, _ptr(init), S,
-                                       max_sweeps, _ptr(cost), _ptr(strat), _ptr(sweeps), _stream()))
+    _check(lib().autoddl_coord_descent(_ptr(d_layers, U8, "d_layers"), Bp, L, C.addressof(m), C.addressof(n) if n is not None else None,
+                                       _ptr(T, I64, "T"), _ptr(work, U8, "work"), work.numel() if work is not None else 0,
+                                       _ptr(init, I32, "init"), S, max_sweeps, _ptr(cost, I64, "cost"), _ptr(strat, I32, "strategy"),
+                                       _ptr(sweeps, I32, "sweeps"), _stream()))
     return cost, strat, sweeps
 
 
@@ -207,8 +235,9 @@ def metropolis(T: torch.Tensor, init: torch.Tensor, mesh, nsteps: int, tau_ps: i
                torch.empty((Bp, S), dtype=torch.int32, device=dev))
     bc, bs, fc, fs, acc = out
     m = c_mesh(mesh)
-    _check(lib().autoddl_metropolis(_ptr(T), Bp, L, C.addressof(m), _ptr(init), S, nsteps, tau_ps, seed, _ptr(bc), _ptr(bs),
-                                    _ptr(fc), _ptr(fs), _ptr(acc), _stream()))
+    _check(lib().autoddl_metropolis(_ptr(T, I64, "T"), Bp, L, C.addressof(m), _ptr(init, I32, "init"), S, nsteps, tau_ps, seed,
+                                    _ptr(bc, I64, "best_cost"), _ptr(bs, I32, "best_strategy"), _ptr(fc, I64, "final_cost"),
+                                    _ptr(fs, I32, "final_strategy"), _ptr(acc, I32, "accepted"), _stream()))
     return out
 
 
@@ -220,7 +249,17 @@ def fit_alpha_beta(kind: torch.Tensor, p: torch.Tensor, nbytes: torch.Tensor, t:
         out = torch.empty(2, dtype=torch.float64, device=dev)
     if work is None:
         work = torch.empty(int(lib().autoddl_fit_workspace_bytes()), dtype=torch.uint8, device=dev)
-    _check(lib().autoddl_fit_alpha_beta(_ptr(kind), _ptr(p), _ptr(nbytes), _ptr(t), N, _ptr(out), _ptr(work), work.numel(), _stream()))
+    _check(lib().autoddl_fit_alpha_beta(_ptr(kind, I32, "kind"), _ptr(p, I32, "p"), _ptr(nbytes, I64, "nbytes"), _ptr(t, F64, "t"), N,
+                                        _ptr(out, F64, "out"), _ptr(work, U8, "work"), work.numel(), _stream()))
+    return out
+
+
+def best_of_starts(cost: torch.Tensor, out=None):
+    """cost int64 [Bp, S] (device) -> best_cost int64 [Bp], best_start int32 [Bp]: smallest cost, smallest start on ties"""
+    Bp, S = cost.shape
+    if out is None:
+        out = (torch.empty(Bp, dtype=torch.int64, device=cost.device), torch.empty(Bp, dtype=torch.int32, device=cost.device))
+    _check(lib().autoddl_best_of_starts(_ptr(cost, I64, "cost"), Bp, S, _ptr(out[0], I64, "best_cost"), _ptr(out[1], I32, "best_start"), _stream()))
     return out
 
 
@@ -257,10 +296,12 @@ def search(d_layers: torch.Tensor, mesh, net, init: torch.Tensor | None = None, 
             need -= Bp * L * K * K * 8                       # tables go to T, not to the workspace
         work = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
     m, n = c_mesh(mesh), c_net(net)
-    _check(lib().autoddl_search(_ptr(d_layers), Bp, L, C.addressof(m), C.addressof(n), _ptr(o.get("T")), _ptr(o.get("node")),
-                                _ptr(o.get("mask")), _ptr(work), work.numel() if work is not None else 0,
-                                _ptr(o["opt_cost"]), _ptr(o["strategy"]), _ptr(init), S, max_sweeps,
-                                _ptr(o.get("cd_cost")), _ptr(o.get("cd_strategy")), _ptr(o.get("cd_sweeps")), _stream()))
+    _check(lib().autoddl_search(_ptr(d_layers, U8, "d_layers"), Bp, L, C.addressof(m), C.addressof(n), _ptr(o.get("T"), I64, "T"),
+                                _ptr(o.get("node"), I64, "node"), _ptr(o.get("mask"), U8, "mask"), _ptr(work, U8, "work"),
+                                work.numel() if work is not None else 0, _ptr(o["opt_cost"], I64, "opt_cost"),
+                                _ptr(o["strategy"], I32, "strategy"), _ptr(init, I32, "init"), S, max_sweeps,
+                                _ptr(o.get("cd_cost"), I64, "cd_cost"), _ptr(o.get("cd_strategy"), I32, "cd_strategy"),
+                                _ptr(o.get("cd_sweeps"), I32, "cd_sweeps"), _stream()))
     return o
 
 
@@ -272,14 +313,15 @@ def search_host(w: Workload, init: np.ndarray | None, work: torch.Tensor, pinned
     if pinned is None:
         pinned = alloc_host_outputs(Bp, L, S)
     m, n = c_mesh(w.mesh), c_net(w.net)
-    ip = None if init is None else init.ctypes.data
-    _check(lib().autoddl_search_host(layers.ctypes.data, Bp, L, C.addressof(m), C.addressof(n), ip, S, w.max_sweeps,
-                                     work.data_ptr(), work.numel(),
+    ip = _hptr(init, np.int32, "init")
+    _check(lib().autoddl_search_host(_hptr(layers, LAYER_DTYPE, "layers"), Bp, L, C.addressof(m), C.addressof(n), ip, S, w.max_sweeps,
+                                     _ptr(work, U8, "work"), work.numel(),
                                      pinned["opt_cost"].data_ptr(), pinned["strategy"].data_ptr(),
                                      pinned["cd_cost"].data_ptr() if S else None,
                                      pinned["cd_strategy"].data_ptr() if S else None,
                                      pinned["cd_sweeps"].data_ptr() if S else None, _stream()))
-    return {k: v.numpy() for k, v in pinned.items()}
+    keys = ("opt_cost", "strategy") + (("cd_cost", "cd_strategy", "cd_sweeps") if S else ())
+    return {k: pinned[k].numpy() for k in keys}         # no Coordinate Descent: no cd_* keys (nothing was written there)
 
 
 def alloc_host_outputs(Bp: int, L: int, S: int, pin: bool = True):

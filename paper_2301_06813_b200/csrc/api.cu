@@ -1,6 +1,5 @@
 // C-ABI entry points (include/autoddl.h): argument validation, workspace carving, launches.
 #include <stdarg.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -96,7 +95,7 @@ static constexpr int32_t kFusedMinChains = 296;
 // device-side address of a host pointer that lies in pinned, device-mapped memory (cudaHostAlloc / cudaHostRegister,
 // e.g. a torch pin_memory() tensor); NULL for pageable memory
 static const void* mapped_host_pointer(const void* h) {
-  static const bool off = getenv("AUTODDL_NO_ZERO_COPY") != nullptr;
+  static const bool off = ADL_DEBUG_ENV("AUTODDL_NO_ZERO_COPY");
   if (off || !h) return nullptr;
   cudaPointerAttributes a;
   if (cudaPointerGetAttributes(&a, h) != cudaSuccess) { cudaGetLastError(); return nullptr; }
@@ -111,7 +110,7 @@ struct SideStream {
   cudaStream_t stream = nullptr;
   cudaEvent_t dp_done = nullptr, copied = nullptr;
   bool ready() {
-    static const bool off = getenv("AUTODDL_NO_D2H_OVERLAP") != nullptr;
+    static const bool off = ADL_DEBUG_ENV("AUTODDL_NO_D2H_OVERLAP");
     if (off) return false;
     int cur = -1;
     if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -129,6 +128,15 @@ struct SideStream {
   }
 };
 static thread_local SideStream g_side;
+
+int device_sm_count() {
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError();
+    sms = 148;
+  }
+  return sms;
+}
 
 static int check_device() {
   int n = 0;
@@ -259,7 +267,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
                          int64_t* d_opt_cost, int32_t* d_strategy, const int32_t* d_init, int32_t S, int32_t max_sweeps,
                          int64_t* d_cd_cost, int32_t* d_cd_strategy, int32_t* d_cd_sweeps, cudaStream_t st) {
   const bool do_cd = d_init != nullptr;
-  static const bool no_fuse = getenv("AUTODDL_NO_FUSE") != nullptr;   // debugging switch: three separate kernels
+  static const bool no_fuse = ADL_DEBUG_ENV("AUTODDL_NO_FUSE");         // debug builds only: three separate kernels
   const bool fused = !no_fuse && Bp >= kFusedMinChains && fused_build_dp_supported(mp, L);
   const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
   size_t used = 0;
@@ -279,7 +287,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
       return AUTODDL_EWORK;
     }
     // the first CD sweep rides in the fused kernel (tiles are in shared memory there); the CD kernel resumes at sweep 2
-    static const bool no_cd_fuse = getenv("AUTODDL_NO_CD_FUSE") != nullptr;
+    static const bool no_cd_fuse = ADL_DEBUG_ENV("AUTODDL_NO_CD_FUSE");
     cd_resume = do_cd && !no_cd_fuse && fused_cd_sweep_supported(L, S);
     if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used,
                                     cd_resume ? d_init : nullptr, S, cd_resume ? d_cd_strategy : nullptr, st)))
@@ -443,6 +451,17 @@ int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int6
   int rc = check_device();
   if (rc) return rc;
   return launch_fit_alpha_beta(d_kind, d_p, d_bytes, d_time, N, d_out, (double*)d_work, (cudaStream_t)stream);
+}
+
+int autoddl_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t* d_best_cost, int32_t* d_best_start,
+                           void* stream) {
+  clear_error();
+  ADL_REQUIRE(d_cost && d_best_cost && d_best_start, "NULL pointer");
+  ADL_REQUIRE(Bp >= 1 && S >= 1, "Bp, S must be >= 1");
+  ADL_REQUIRE(((uintptr_t)d_cost & 7) == 0 && ((uintptr_t)d_best_cost & 7) == 0 && ((uintptr_t)d_best_start & 3) == 0, "misaligned pointer");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_best_of_starts(d_cost, Bp, S, d_best_cost, d_best_start, (cudaStream_t)stream);
 }
 
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {

@@ -22,8 +22,6 @@
 //   5. the K x K expansion T[i][j] = Esym[O-state(i)][I-state(j)] + VP[j]: one shared-memory gather and one
 //      64-bit add per cell, 16-byte streaming stores; all indices are hoisted out of the tile loop.
 // The kernel is then bound by the HBM write of 8 B per cell instead of integer arithmetic.
-#include <stdlib.h>
-
 #include "sbp_builder.cuh"
 
 namespace autoddl {
@@ -389,12 +387,6 @@ struct Smem36 {
   RecBuf rec[2][G];
   SigInfo sig[2][K];
   int32_t meta[2];                                      // (kind | kind_prev << 1) of the group's tiles, 2 bits each
-  // fused chain DP only
-  alignas(16) int64_t f[2][K];                          // f_{l-1}, f_l
-  alignas(8) uint64_t full[2], freeb[2];                // mbarriers: EV buffer filled / consumed by the DP warp
-  int32_t dpmeta[2];                                    // meta of the group in EV[eb], handed over with full[eb]
-  uint8_t repcol[2][16];                                // per consumer kind: one representative column per input-state class
-  uint8_t repof[2][K];                                  //                    class of every column
 };
 
 __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
@@ -402,118 +394,33 @@ __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, u
                : "memory");
 }
 
-// Work of one team (CTA): groups of up to G consecutive tiles.
-//   FUSE = false: groups blockIdx.x, blockIdx.x + gridDim.x, ... of the flat tile list (a group may straddle chains)
-//   FUSE = true : whole chains blockIdx.x, blockIdx.x + gridDim.x, ...; every chain starts a new group
-template <bool FUSE>
+// Work of one team (CTA): groups blockIdx.x, blockIdx.x + gridDim.x, ... of up to G consecutive tiles of the flat tile
+// list (a group may straddle chains)
 struct GroupSched {
-  int tile0, l0, nt, p;      // first tile, its layer index, tiles in the group, chain (FUSE only)
+  int tile0, l0, nt;         // first tile, its layer index, tiles in the group
   bool valid;
-  int ntiles, L, Bp, step, l_step;
+  int ntiles, L, step, l_step;
   __device__ __forceinline__ void init(int ntiles_, int L_, int G) {
-    ntiles = ntiles_; L = L_; Bp = ntiles_ / L_; step = gridDim.x;
-    if (FUSE) {
-      p = blockIdx.x; l0 = 0; tile0 = p * L; valid = p < Bp; nt = L < G ? L : G;
-    } else {
-      p = 0; tile0 = blockIdx.x * G; valid = tile0 < ntiles;
-      l0 = (int)(((int64_t)blockIdx.x * G) % L);
-      l_step = (int)(((int64_t)gridDim.x * G) % L);
-      nt = ntiles - tile0 < G ? ntiles - tile0 : G;
-    }
+    ntiles = ntiles_; L = L_; step = gridDim.x;
+    tile0 = blockIdx.x * G; valid = tile0 < ntiles;
+    l0 = (int)(((int64_t)blockIdx.x * G) % L);
+    l_step = (int)(((int64_t)gridDim.x * G) % L);
+    nt = ntiles - tile0 < G ? ntiles - tile0 : G;
   }
   __device__ __forceinline__ void advance(int G) {
-    if (FUSE) {
-      l0 += G;
-      if (l0 >= L) { l0 = 0; p += step; valid = p < Bp; }
-      tile0 = p * L + l0;
-      nt = L - l0 < G ? L - l0 : G;
-    } else {
-      tile0 += step * G;
-      valid = tile0 < ntiles;
-      l0 += l_step;
-      if (l0 >= L) l0 -= L;
-      nt = ntiles - tile0 < G ? ntiles - tile0 : G;
-    }
+    tile0 += step * G;
+    valid = tile0 < ntiles;
+    l0 += l_step;
+    if (l0 >= L) l0 -= L;
+    nt = ntiles - tile0 < G ? ntiles - tile0 : G;
   }
 };
 
-// block row of the tile that holds the row of producer signature i (class = {0,1,2,3,2,2} over the level-0 digit)
-__host__ __device__ constexpr int block_row_of(int i) { return (i / 6 < 4 ? i / 6 : 2) * 6 + i % 6; }
-
-// One chain-DP step on a tile held as 24 block rows in shared memory (R9), by one warp:
-//   fn[j] = min_i f[i] + EV[block_row_of(i)][j], smallest i on ties; bpl[j] = that i.
-// Columns whose consumer signatures share the input state vector b(j) differ only by a constant,
-//   EV[r][j] - EV[r][j'] = VP[j] - VP[j']  for every row r,
-// so they share the argmin and their minima differ by that constant: the recurrence runs on one representative
-// column per class (<= 16 of them), lane = (h, q): rows i = 18 h .. 18 h + 17 of representative q in ascending
-// order, the upper half merged into the lower with a strict '<' (smallest index wins), and the other columns
-// follow as fn[j] = fn[rep] + EV[0][j] - EV[0][rep].  Block rows: i for i < 24, i - 12 for 24..29, i - 18 for 30..35.
-__device__ __forceinline__ void dp36_step_blockrows(const int64_t* __restrict__ ev, const int64_t* __restrict__ f,
-                                                    int64_t* __restrict__ fn, uint8_t* __restrict__ bpl,
-                                                    const uint8_t* __restrict__ repcol, const uint8_t* __restrict__ repof,
-                                                    int lane) {
-  constexpr int K = 36;
-  const int q = lane & 15, h = lane >> 4;
-  const int col = repcol[q];                               // unused lanes (q >= number of classes) repeat column 0
-  const int64_t* fh = f + 18 * h;
-  const int64_t* e0 = ev + (18 * h) * K + col;             // r = 0..5
-  const int64_t* e1 = ev + (h ? 6 : 0) * K + col;          // r = 6..11:  h = 1 -> block rows 12..17
-  const int64_t* e2 = ev + col;                            // r = 12..17: h = 1 -> block rows 12..17
-  // three independent chains of six rows (instruction-level parallelism), merged in row order: strict '<' keeps the
-  // smallest index
-  int64_t pb[3];
-  int pa[3];
-#pragma unroll
-  for (int part = 0; part < 3; ++part) {
-    int64_t tv[6], fv[6];
-    const int64_t* e = part == 0 ? e0 : (part == 1 ? e1 : e2);
-#pragma unroll
-    for (int r = 0; r < 6; ++r) {                          // loads first: six rows in flight
-      tv[r] = e[(6 * part + r) * K];
-      fv[r] = fh[6 * part + r];
-    }
-    int64_t b = fv[0] + tv[0];
-    int ba = 6 * part;
-#pragma unroll
-    for (int r = 1; r < 6; ++r) {
-      const int64_t v = fv[r] + tv[r];
-      if (v < b) { b = v; ba = 6 * part + r; }
-    }
-    pb[part] = b;
-    pa[part] = ba;
-  }
-  int64_t best = pb[0];
-  int a = pa[0];
-  if (pb[1] < best) { best = pb[1]; a = pa[1]; }
-  if (pb[2] < best) { best = pb[2]; a = pa[2]; }
-  a += 18 * h;
-  {
-    const int64_t o = __shfl_down_sync(0xffffffffu, best, 16);
-    const int oa = __shfl_down_sync(0xffffffffu, a, 16);
-    if (o < best) { best = o; a = oa; }
-  }
-  // every column from its representative (lanes 0..15 hold them)
-#pragma unroll
-  for (int j0 = 0; j0 < 64; j0 += 32) {
-    const int j = j0 + lane;
-    const int rq = repof[j < K ? j : 0];
-    const int64_t rb = __shfl_sync(0xffffffffu, best, rq);
-    const int ra = __shfl_sync(0xffffffffu, a, rq);
-    if (j < K) {
-      fn[j] = rb + ev[j] - ev[repcol[rq]];
-      bpl[j] = (uint8_t)ra;
-    }
-  }
-}
-
-// NT builder threads, G tiles per group.  FUSE: one extra warp runs the chain DP (R9) on every tile
-// straight from shared memory while the tile is being stored, so the optimum costs no table read at all.
-template <int NT, int G, bool FUSE, bool CD1 = false>
-__global__ void __launch_bounds__(FUSE ? NT + 32 : NT, FUSE ? 5 : 768 / NT)
+// NT builder threads, G tiles per group.
+template <int NT, int G>
+__global__ void __launch_bounds__(NT, 768 / NT)
 build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L, MeshParams mp,
-                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
-                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
-                      const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1) {
+                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
   using SM = Smem36<G>;
   constexpr int D = 2, K = SM::K, NS = SM::NS, NC = SM::NC, ES = SM::ES, NROW = SM::NROW;
   constexpr int STRIDE = SM::STRIDE;
@@ -525,183 +432,18 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
   static_assert(2 * RA + G * NC <= NT && G * 5 * (1 << D) <= NT && G * K <= NT && 5 * G <= NT, "role layout");
   extern __shared__ __align__(128) unsigned char smem36_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem36_raw);
-  // FUSE: back-pointers [L][K] of the chain in flight live in a per-CTA slice of the workspace (L2-resident)
-  uint8_t* bp = FUSE ? bp_glob + (size_t)blockIdx.x * L * K : nullptr;
-  uint8_t* cd_s = smem36_raw + sizeof(SM);                 // FUSE + CD: strategies of the chain's starts [cd_S][L]
   const int tid = threadIdx.x;
 
-  if (tid < NT) {
+  {
     fill_sig_table<D>(sm.sig, mp, tid, NT);
     for (int x = tid; x < G * ES * ES; x += NT) sm.t[x / (ES * ES)].E[x % (ES * ES)] = 0;
     for (int x = tid; x < G * 2 * D; x += NT) sm.t[x / (2 * D)].TAB[(x % (2 * D)) * STRIDE + NC] = 0;
   }
-  if (FUSE && tid == 0) {
-    for (int b = 0; b < 2; ++b) { mbar_init(&sm.full[b], 1); mbar_init(&sm.freeb[b], 1); }
-    mbar_fence_init();
-  }
   __syncthreads();
-  auto bsync = [&]() {                                      // barrier over the NT builder threads
-    if (FUSE) asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); else __syncthreads();
-  };
+  auto bsync = [&]() { __syncthreads(); };
 
-  GroupSched<FUSE> sc;
+  GroupSched sc;
   sc.init(ntiles, L, G);
-
-  if (FUSE && tid >= NT) {
-    // =================== chain DP warp ===================
-    const int lane = tid & 31;
-    if (lane < 2) {                                        // classes of equal input state vector per consumer kind
-      const int kind = lane;
-      int n = 0;
-      for (int q = 0; q < 16; ++q) sm.repcol[kind][q] = 0;
-      for (int j = 0; j < K; ++j) {
-        int q = 0;
-        while (q < n && sm.sig[kind][sm.repcol[kind][q]].b_idx != sm.sig[kind][j].b_idx) ++q;
-        if (q == n) sm.repcol[kind][n++] = (uint8_t)j;
-        sm.repof[kind][j] = (uint8_t)q;
-      }
-    }
-    __syncwarp();
-    int cur = 0;
-    const bool cd = cd_init != nullptr;
-    const int64_t* ev_prev = nullptr;                      // tile l - 1 of the chain (may live in the other EV buffer)
-    int pending_free = -1;                                 // EV buffer still needed for the CD update of its last tile
-    // first Coordinate Descent sweep (R10) of layer `l` of every start, from the tiles in shared memory:
-    //   s_l <- smallest-index argmin_c T[l][s_{l-1}][c] + T[l+1][c][s_{l+1}],  T[l][i][j] = EV_l[block_row_of(i)][j]
-    auto cd_update = [&](int l, const int64_t* ev_l, const int64_t* ev_r) {
-      for (int st = 0; st < cd_S; ++st) {
-        uint8_t* sv = cd_s + (size_t)st * L;
-        const int left = l > 0 ? sv[l - 1] : 0;
-        const int64_t* row = ev_l + block_row_of(left) * K;
-        const int right = ev_r ? sv[l + 1] : 0;
-        int64_t bv = INT64_MAX;
-        int bi = K;
-#pragma unroll
-        for (int c0 = 0; c0 < 64; c0 += 32) {
-          const int c = c0 + lane;
-          if (c < K) {
-            int64_t g = row[c];
-            if (ev_r) g += ev_r[(c < 24 ? c : (c < 30 ? c - 12 : c - 18)) * K + right];
-            if (g < bv) { bv = g; bi = c; }
-          }
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-          const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
-          const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-          if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-        }
-        __syncwarp();
-        if (lane == 0) sv[l] = (uint8_t)bi;
-        __syncwarp();
-      }
-    };
-    for (int it = 0; sc.valid; ++it, sc.advance(G)) {
-      const int eb = it & 1;
-      mbar_wait(&sm.full[eb], (it >> 1) & 1);
-      const int meta = sm.dpmeta[eb];
-      for (int t = 0; t < sc.nt; ++t) {
-        const int l = sc.l0 + t;
-        const int kind = (meta >> (2 * t)) & 1;
-        const int64_t* ev = sm.EV[eb][t];
-        int64_t* fn = sm.f[cur ^ 1];
-        if (l == 0) {                                      // f_0[j] = T[0][0][j]
-          for (int j = lane; j < K; j += 32) fn[j] = ev[j];
-          if (cd) {                                        // the chain's starts
-            for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)sc.p * cd_S * L + x];
-          }
-        } else {
-          // CD1 (one start per chain): the argmin of layer l-1's update is independent of the DP step of tile l, so it
-          // is computed in the same straight-line code and its shuffle / compare chain interleaves with the DP scan
-          int64_t cbv = INT64_MAX;
-          int cbi = K;
-          if (CD1) {
-            const int left = l > 1 ? cd_s[l - 2] : 0, right = cd_s[l];
-            const int64_t* row = ev_prev + block_row_of(left) * K;
-#pragma unroll
-            for (int c0 = 0; c0 < 64; c0 += 32) {
-              const int c = c0 + lane;
-              if (c < K) {
-                const int64_t g = row[c] + ev[(c < 24 ? c : (c < 30 ? c - 12 : c - 18)) * K + right];
-                if (g < cbv) { cbv = g; cbi = c; }
-              }
-            }
-          }
-          dp36_step_blockrows(ev, sm.f[cur], fn, bp + (size_t)l * K, sm.repcol[kind], sm.repof[kind], lane);
-          if (CD1) {
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-              const int64_t ov = __shfl_xor_sync(0xffffffffu, cbv, off);
-              const int oi = __shfl_xor_sync(0xffffffffu, cbi, off);
-              if (ov < cbv || (ov == cbv && oi < cbi)) { cbv = ov; cbi = oi; }
-            }
-            if (lane == 0) cd_s[l - 1] = (uint8_t)cbi;
-          }
-        }
-        cur ^= 1;
-        __syncwarp();
-        if (cd) {
-          if (l > 0 && !CD1) cd_update(l - 1, ev_prev, ev);
-          if (l == L - 1) {
-            cd_update(l, ev, nullptr);
-            for (int x = lane; x < cd_S * L; x += 32) cd_s1[(size_t)sc.p * cd_S * L + x] = cd_s[x];
-          }
-          ev_prev = ev;
-          if (t == 0 && pending_free >= 0) {               // the previous group's last tile has served its CD update
-            if (lane == 0) mbar_arrive(&sm.freeb[pending_free]);
-            pending_free = -1;
-          }
-        }
-        if (l == L - 1) {                                  // smallest argmin of f_{L-1}, then backtrack
-          const int64_t* f = sm.f[cur];
-          int64_t bv = f[lane];
-          int bi = lane;
-          if (lane < K - 32) {
-            const int64_t v = f[32 + lane];
-            if (v < bv) { bv = v; bi = 32 + lane; }
-          }
-#pragma unroll
-          for (int off = 16; off > 0; off >>= 1) {
-            const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-            if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-          }
-          // the chain's back-pointers were written by this warp; pull them into L1 so that the dependent walk hits
-          __syncwarp();
-          {
-            int warm = 0;
-            for (int o = 16 * lane; o < L * K; o += 16 * 32) {
-              int4 x;
-              asm volatile("ld.global.ca.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(x.x), "=r"(x.y), "=r"(x.z), "=r"(x.w) : "l"(bp + o));
-              warm ^= x.x;
-            }
-            if (warm == 0x7fffffff) bi ^= 0;               // keep the loads
-          }
-          __syncwarp();
-          if (lane == 0) {
-            int32_t* sp = strategy + (size_t)sc.p * L;
-            opt_cost[sc.p] = bv;
-            int sidx = bi;
-            sp[L - 1] = sidx;
-            for (int ll = L - 1; ll >= 1; --ll) {
-              unsigned v;
-              asm volatile("ld.global.ca.u8 %0, [%1];" : "=r"(v) : "l"(bp + (size_t)ll * K + sidx));
-              sidx = (int)v;
-              sp[ll - 1] = sidx;
-            }
-          }
-          __syncwarp();
-        }
-      }
-      __syncwarp();
-      if (cd && sc.l0 + sc.nt < L) {
-        pending_free = eb;                                 // its last tile is still needed: CD update of that layer
-      } else if (lane == 0) {
-        mbar_arrive(&sm.freeb[eb]);
-      }
-    }
-    return;
-  }
 
   // ---- tile-invariant roles of this thread ---------------------------------------------------------------
   // step 3: thread sums the <= 6 table entries of R[a][b] for NR state pairs (a, b) = tid + k * NT
@@ -852,7 +594,6 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
         }
       }
     }
-    if (FUSE && tid == ISSUER && it >= 2) mbar_wait(&sm.freeb[eb], ((it >> 1) - 1) & 1);   // the DP warp is done with EV[eb]
     bsync();
 
     // ---- 4. EV[r][j] = VP[j] + R[a(r)][b(j)] + R[dual b(j)][dual a(r)]: the 24 block rows of every tile ---------------
@@ -890,10 +631,6 @@ build_tables36_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int 
     bsync();
 
     // ---- 5. six 1,728-byte bulk stores per tile; the copies run while the CTA prepares the next group -----------------
-    if (FUSE && tid == 0) {
-      sm.dpmeta[eb] = meta;
-      mbar_arrive(&sm.full[eb]);
-    }
     if (T && tid == ISSUER) {
       for (int t = 0; t < nt; ++t) {
         int64_t* out = T + (size_t)(tile0 + t) * K * K;
@@ -1119,12 +856,10 @@ int launch_216(const autoddl_layer* d_layers, int ntiles, int L, const MeshParam
 }
 
 constexpr int kNT = 256, kG = 4;                  // tables only: 3 CTAs of 256 threads per SM, 4 tiles per group
-constexpr int kFuseNT = 128, kFuseG = 2;           // fused with the chain DP: 6 CTAs of 128 + 32 threads per SM
-constexpr int kFusePerSM = 5;
 
 int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams& mp, int64_t* d_T,
               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
-  auto kern = build_tables36_kernel<kNT, kG, false>;
+  auto kern = build_tables36_kernel<kNT, kG>;
   const size_t smem = sizeof(Smem36<kG>);
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int dev = 0, sms = 148;
@@ -1132,7 +867,7 @@ int launch_36(const autoddl_layer* d_layers, int ntiles, int L, const MeshParams
   ADL_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int ngroups = (ntiles + kG - 1) / kG;
   const int grid = ngroups < sms * 3 ? ngroups : sms * 3;             // persistent, grid-stride over tile groups
-  kern<<<grid, kNT, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask, nullptr, nullptr, nullptr, nullptr, 0, nullptr);
+  kern<<<grid, kNT, smem, st>>>(d_layers, ntiles, L, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -1170,7 +905,7 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
     case 1: return launch_d<1>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     case 2: return launch_36(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     case 3: {
-      static const bool generic = getenv("AUTODDL_BT216_GENERIC") != nullptr;     // debugging switch
+      static const bool generic = ADL_DEBUG_ENV("AUTODDL_BT216_GENERIC");          // debug builds only
       if (generic) return launch_d<3>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
       return launch_216(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     }

@@ -9,7 +9,6 @@
 // group of rows; f is broadcast from shared memory.  With one consumer warp (K = 36) a layer needs no
 // block barrier at all; with several row groups (K = 216) partial minima are merged through shared
 // memory with the lexicographic (value, row) order that keeps the lowest-index tie-break.
-#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -499,7 +498,7 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
     case 6:   return launch_cfg<6, 6, 4, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
     case 36:
       if ((size_t)L * K <= 16 * 1024) {               // back-pointers fit in shared memory: the 32-lane kernel
-        static const int stages = [] { const char* e = getenv("AUTODDL_DP_STAGES"); return e ? atoi(e) : 3; }();
+        static const int stages = ADL_DEBUG_ENV_INT("AUTODDL_DP_STAGES", 3);
         if (stages == 2) return launch_dp36<2>(d_T, Bp, L, d_opt_cost, d_strategy, st);
         if (stages == 4) return launch_dp36<4>(d_T, Bp, L, d_opt_cost, d_strategy, st);
         return launch_dp36<3>(d_T, Bp, L, d_opt_cost, d_strategy, st);
@@ -507,21 +506,23 @@ int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_
       return launch_cfg<36, 36, 3, 1>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
     case 216: {
       // few long chains: one 8-CTA cluster per chain (chain_dp_cluster.cu); many chains already fill the machine
-      static const bool no_cluster = getenv("AUTODDL_DP_NO_CLUSTER") != nullptr;
-      if (!no_cluster && Bp * 8 <= 148 && chain_dp_cluster_supported(K, L)) {
+      static const bool no_cluster = ADL_DEBUG_ENV("AUTODDL_DP_NO_CLUSTER");
+      if (!no_cluster && Bp * 8 <= device_sm_count() && chain_dp_cluster_supported(K, L)) {
         const int rc = launch_chain_dp_cluster(d_T, Bp, L, d_opt_cost, d_strategy, st);
         if (rc == AUTODDL_OK) return rc;
         cudaGetLastError();                                  // launch refused: fall back to one CTA per chain
+        clear_error();
       }
       return launch_cfg<216, 24, 4, 8>(d_T, Bp, L, d_bp, d_opt_cost, d_strategy, st);
     }
   }
   if (K >= 1 && K <= 256) {
-    static const bool no_cluster = getenv("AUTODDL_DP_NO_CLUSTER") != nullptr;
-    if (!no_cluster && Bp * 8 <= 148 && chain_dp_cluster_anyk_supported(K, L)) {
+    static const bool no_cluster = ADL_DEBUG_ENV("AUTODDL_DP_NO_CLUSTER");
+    if (!no_cluster && Bp * 8 <= device_sm_count() && chain_dp_cluster_anyk_supported(K, L)) {
       const int rc = launch_chain_dp_cluster_anyk(d_T, Bp, L, K, d_opt_cost, d_strategy, st);
       if (rc == AUTODDL_OK) return rc;
       cudaGetLastError();                                    // launch refused: fall back to one CTA per chain
+      clear_error();
     }
     return launch_anyk(d_T, Bp, L, K, d_bp, d_opt_cost, d_strategy, st);
   }

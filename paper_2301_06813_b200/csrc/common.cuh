@@ -23,6 +23,17 @@ void count_launch(int n = 1);
     }                                                                                    \
   } while (0)
 
+// Debugging switches (they select between kernels that are all held to the same bit-exact parity) exist only in builds
+// with -DAUTODDL_DEBUG_SWITCHES: the dispatch of the shipped library never depends on the caller's environment.
+#ifdef AUTODDL_DEBUG_SWITCHES
+#include <stdlib.h>
+#define ADL_DEBUG_ENV(name) (getenv(name) != nullptr)
+#define ADL_DEBUG_ENV_INT(name, dflt) (getenv(name) ? atoi(getenv(name)) : (dflt))
+#else
+#define ADL_DEBUG_ENV(name) false
+#define ADL_DEBUG_ENV_INT(name, dflt) (dflt)
+#endif
+
 #define ADL_REQUIRE(cond, ...)                  \
   do {                                          \
     if (!(cond)) {                              \
@@ -80,6 +91,9 @@ size_t fit_workspace_bytes();
 int launch_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64_t* d_bytes, const double* d_time,
                           int64_t N, double* d_out, double* d_work, cudaStream_t st);
 int launch_copy_probe(const void* src, void* dst, size_t bytes, cudaStream_t st);
+int launch_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t* d_best_cost, int32_t* d_best_start,
+                          cudaStream_t st);
+int device_sm_count();                                     // multiprocessors of the current device (148 if the query fails)
 
 // ---- device helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {

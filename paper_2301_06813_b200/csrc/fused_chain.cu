@@ -34,6 +34,12 @@ struct CtaShared {
   uint32_t slot_lo[8][32], sym[8][32];
 };
 
+struct alignas(16) Rec64 {                                 // byte image of autoddl_layer
+  int64_t X[5];                                           // M, Kd, N, in_rows, in_cols
+  int32_t kind, eb, wgb, wsb, maxr, maxc;
+};
+static_assert(sizeof(Rec64) == sizeof(autoddl_layer), "Rec64 mirrors autoddl_layer");
+
 struct alignas(16) WarpShared {
   int64_t Q[5][4];                                        // M, Kd, N, in_rows, in_cols  x  level subset
   int64_t TAB[2 * FD * FSTRIDE];                          // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
@@ -42,7 +48,7 @@ struct alignas(16) WarpShared {
   alignas(16) int64_t VP[FK];
   int64_t Esym[FES * FES];                                // R[a][b], then symmetrised in place; row / column 16 stay 0
   alignas(16) int64_t f[2][FK];
-  RecBuf rec[2];
+  Rec64 rec[8];                                           // ring of layer records, fetched four at a time
 };
 
 __device__ __forceinline__ void lexmin_xor(int64_t& bv, int& bi) {
@@ -125,15 +131,17 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   const int nslots = gridDim.x * W;
   for (int p = warp * gridDim.x + blockIdx.x; p < Bp; p += nslots) {
     const autoddl_layer* chain = layers + (size_t)p * L;
-    auto stage = [&](int b, int l) {                        // lanes 0..3: the 64-byte record; lane 4: the previous kind
-      if (lane < 5) {
-        const autoddl_layer* cur = chain + l;
-        RecBuf* dst = &ws.rec[b];
-        if (lane < 4) cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * lane, reinterpret_cast<const unsigned char*>(cur) + 16 * lane);
-        else cp_async4(&dst->kind_prev, &(l > 0 ? cur - 1 : cur)->kind);
-      }
+    // Layer records: 256-byte groups of four consecutive records per request (16 lanes x 16 bytes; host-mapped inputs are
+    // read over PCIe, where small requests are what costs), into a ring of eight, one group (four layers) ahead.
+    auto stage4 = [&](int l4) {                              // records l4 .. l4 + 3 -> slots (l4 .. l4 + 3) & 7
+      const int l = l4 + (lane >> 2);
+      if (lane < 16 && l < L)
+        cp_async16(reinterpret_cast<unsigned char*>(&ws.rec[l & 7]) + 16 * (lane & 3),
+                   reinterpret_cast<const unsigned char*>(chain + l) + 16 * (lane & 3));
     };
-    stage(0, 0);
+    stage4(0);
+    stage4(4);
+    int kind_prev = 0;
     const bool cd = cd_init != nullptr;
     if (cd) {
       for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)p * cd_S * L + x];
@@ -141,11 +149,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     int cur = 0;
 
     for (int l = 0; l < L; ++l) {
-      if (lane < 5) cp_async_wait_all();
-      __syncwarp();
-      if (l + 1 < L) stage((l + 1) & 1, l + 1);
-      const RecBuf& rec = ws.rec[l & 1];
-      const int kind = rec.kind, kind_prev = rec.kind_prev;
+      if ((l & 3) == 0) {
+        if (lane < 16) cp_async_wait_all();                  // the group of this layer has landed
+        __syncwarp();
+        if (l >= 4) stage4(l + 4);                           // its slots held layers l-4 .. l-1: done
+      }
+      const Rec64& rec = ws.rec[l & 7];
+      const int kind = rec.kind;
+      if (l == 0) kind_prev = kind;                          // no producer: any valid kind (E(0) = 0)
       const size_t tile = (size_t)p * L + l;
 
       // ---- 1. Q[x][m] = ceil(extent x / product of the levels in m) -------------------------------------------------
@@ -386,6 +397,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         }
       }
       __syncwarp();
+      kind_prev = kind;
     }
 
     // ---- end of the chain: smallest argmin of f_{L-1}, back-track, results --------------------------------------------
