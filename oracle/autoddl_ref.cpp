@@ -8,6 +8,8 @@
 // Build: g++ -O2 -std=c++17 -shared -fPIC oracle/autoddl_ref.cpp -o oracle/libautoddl_ref.so
 #include "autoddl_ref.h"
 
+#include <cstdint>
+#include <climits>
 #include <vector>
 
 namespace {
@@ -367,6 +369,122 @@ extern "C" int autoddl_ref_best_of_starts(const int64_t* cost, int32_t Bp, int32
       if (cost[p * S + s] < cost[p * S + arg]) arg = s;               // strict: the first start attaining the minimum
     best_cost[p] = cost[p * S + arg];
     best_start[p] = arg;
+  }
+  return 0;
+}
+
+// ---- R27: pipeline stages ("consecutive layers form a pipeline stage", 1F1B) -----------
+// A stage is a contiguous segment [a, b) of the chain on its own sub-mesh; T / node / mask are the tables of the chain
+// ON THAT SUB-MESH.  The first layer of a segment has no producer inside the stage (its input arrives from the previous
+// stage by point-to-point transfer, already in the layout it needs), so only its node cost and penalty count:
+//   f_a[j] = node[a][j] + PEN * [mask[a][j] == 0];  f_l[j] = min_i f_{l-1}[i] + T[l][i][j]  (a < l < b);
+//   C(a, b) = min_j f_{b-1}[j]   -- the optimum of the segment over all K^(b-a) strategies.
+// tri[a * (L + 1) + b] = C(a, b) for 0 <= a < b <= L, -1 elsewhere.
+extern "C" int autoddl_ref_segment_optima(const int64_t* T, const int64_t* node, const uint8_t* mask, int32_t L, int32_t K,
+                                          int64_t* tri) {
+  if (!T || !node || !mask || !tri || L < 1 || K < 1) return -1;
+  for (int64_t x = 0; x < (int64_t)L * (L + 1); ++x) tri[x] = -1;
+  std::vector<int64_t> f(K), g(K);
+  for (int32_t a = 0; a < L; ++a) {
+    for (int j = 0; j < K; ++j) f[j] = node[(int64_t)a * K + j] + (mask[(int64_t)a * K + j] ? 0 : REF_PEN);
+    for (int32_t b = a + 1; b <= L; ++b) {                           // segment [a, b): last layer b - 1
+      if (b - 1 > a) {
+        const int64_t* tile = T + (int64_t)(b - 1) * K * K;
+        for (int j = 0; j < K; ++j) {
+          int64_t best = f[0] + tile[j];
+          for (int i = 1; i < K; ++i) {
+            const int64_t v = f[i] + tile[(int64_t)i * K + j];
+            if (v < best) best = v;
+          }
+          g[j] = best;
+        }
+        f.swap(g);
+      }
+      int64_t m = f[0];
+      for (int j = 1; j < K; ++j) if (f[j] < m) m = f[j];
+      tri[(int64_t)a * (L + 1) + b] = m;
+    }
+  }
+  return 0;
+}
+
+// Point-to-point transfer at a stage boundary in front of layer b (a message of n bytes takes
+// alpha + n beta; "point-to-point communications for transferring intermediate results between stages"):
+// the input tensor of layer b, split evenly over the q devices of a stage, crosses the inter-node network once forward
+// (activations) and once backward (their gradients) per micro-batch:
+//   X(b) = 2 m (alpha_inter + ceil(in_rows_b in_cols_b act_bytes_b / q) beta_inter),   X(0) = 0.
+extern "C" int autoddl_ref_stage_transfer(const ref_layer* layers, int32_t L, const ref_mesh* mesh, const ref_net* net,
+                                          int64_t* xfer) {
+  if (!layers || !mesh || !net || !xfer || L < 1) return -1;
+  int64_t q = 1;
+  for (int d = 0; d < mesh->ndim; ++d) q *= mesh->size[d];
+  const int64_t m = net->micro_batches > 1 ? net->micro_batches : 1;
+  xfer[0] = 0;
+  for (int32_t b = 1; b < L; ++b) {
+    const int64_t bytes = layers[b].in_rows * layers[b].in_cols * layers[b].act_bytes;
+    xfer[b] = 2 * m * (net->alpha_ps[1] + ceil_div(bytes, q) * net->beta_ps_per_byte[1]);
+  }
+  return 0;
+}
+
+// Partition of the chain into `stages` contiguous non-empty segments.  Cost of a stage [a, b): its segment optimum plus
+// the transfers at both of its boundaries, c(a, b) = C(a, b) + X(a) + [b < L] X(b).  objective 0: the SUM of the stage
+// costs (total communication); objective 1: the MAX (the slowest stage sets the pace of a 1F1B pipeline).  Plain DP over
+// the cuts: g_1[b] = c(0, b); g_k[b] = min_{a} comb(g_{k-1}[a], c(a, b)), smallest a on ties; cuts by back-tracking
+// from g_stages[L].  cuts[0] = 0 < cuts[1] < ... < cuts[stages] = L.
+extern "C" int autoddl_ref_pipeline_partition(const int64_t* tri, const int64_t* xfer, int32_t L, int32_t stages,
+                                              int32_t objective, int64_t* value, int32_t* cuts) {
+  if (!tri || !xfer || !value || !cuts || L < 1 || stages < 1 || stages > L || objective < 0 || objective > 1) return -1;
+  const int64_t INF = INT64_MAX;
+  std::vector<int64_t> g((size_t)(stages + 1) * (L + 1), INF);
+  std::vector<int32_t> arg((size_t)(stages + 1) * (L + 1), -1);
+  auto c = [&](int a, int b) { return tri[(int64_t)a * (L + 1) + b] + xfer[a] + (b < L ? xfer[b] : 0); };
+  for (int b = 1; b <= L; ++b) { g[(size_t)1 * (L + 1) + b] = c(0, b); arg[(size_t)1 * (L + 1) + b] = 0; }
+  for (int k = 2; k <= stages; ++k)
+    for (int b = k; b <= L; ++b)
+      for (int a = k - 1; a < b; ++a) {
+        const int64_t prev = g[(size_t)(k - 1) * (L + 1) + a];
+        if (prev == INF) continue;
+        const int64_t cs = c(a, b);
+        const int64_t v = objective == 0 ? prev + cs : (prev > cs ? prev : cs);
+        if (v < g[(size_t)k * (L + 1) + b]) { g[(size_t)k * (L + 1) + b] = v; arg[(size_t)k * (L + 1) + b] = a; }
+      }
+  *value = g[(size_t)stages * (L + 1) + L];
+  cuts[stages] = L;
+  for (int k = stages; k >= 1; --k) cuts[k - 1] = arg[(size_t)k * (L + 1) + cuts[k]];
+  return 0;
+}
+
+// Strategy of the whole chain under given cuts: every segment's optimum by the DP above with back-pointers (smallest
+// index on ties, smallest end state), concatenated; seg_cost[k] = C(cuts[k], cuts[k+1]).
+extern "C" int autoddl_ref_segment_strategies(const int64_t* T, const int64_t* node, const uint8_t* mask, int32_t L, int32_t K,
+                                              const int32_t* cuts, int32_t stages, int64_t* seg_cost, int32_t* strategy) {
+  if (!T || !node || !mask || !cuts || !seg_cost || !strategy || L < 1 || K < 1 || stages < 1) return -1;
+  std::vector<int64_t> f(K), g(K);
+  std::vector<int32_t> bp((size_t)L * K);
+  for (int k = 0; k < stages; ++k) {
+    const int a = cuts[k], b = cuts[k + 1];
+    if (a < 0 || b > L || a >= b) return -1;
+    for (int j = 0; j < K; ++j) f[j] = node[(int64_t)a * K + j] + (mask[(int64_t)a * K + j] ? 0 : REF_PEN);
+    for (int l = a + 1; l < b; ++l) {
+      const int64_t* tile = T + (int64_t)l * K * K;
+      for (int j = 0; j < K; ++j) {
+        int64_t best = f[0] + tile[j];
+        int32_t ar = 0;
+        for (int i = 1; i < K; ++i) {
+          const int64_t v = f[i] + tile[(int64_t)i * K + j];
+          if (v < best) { best = v; ar = i; }
+        }
+        g[j] = best;
+        bp[(size_t)l * K + j] = ar;
+      }
+      f.swap(g);
+    }
+    int js = 0;
+    for (int j = 1; j < K; ++j) if (f[j] < f[js]) js = j;
+    seg_cost[k] = f[js];
+    strategy[b - 1] = js;
+    for (int l = b - 1; l > a; --l) strategy[l - 1] = bp[(size_t)l * K + strategy[l]];
   }
   return 0;
 }

@@ -19,6 +19,9 @@
  *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
  *   four / five mesh levels    pinned  (size-1 levels reproduce the three-level tables, decode order,
  *                                                  data-parallel closed form, intra-node gather, brute force at K = 81)
+ *   pipeline stages         segment optima and the partition pinned (one stage = the chain DP,
+ *                                                  brute force over strategies and over cut sets); the stage COST MODEL
+ *                                                  (transfer term, sum / max objective) is PARITY UNPINNED: the paper prints none
  *   Metropolis-Hastings         pinned  (Boltzmann stationary law on enumerable chains, greedy and
  *                                                  hot limits, integer -ln against libm, replay of a hand-checked chain)
  */
@@ -103,6 +106,18 @@ int autoddl_ref_coord_descent(const int64_t* T, int32_t Bp, int32_t L, int32_t K
 
 /* best of the starts of every problem: smallest cost, then smallest start index */
 int autoddl_ref_best_of_starts(const int64_t* cost, int32_t Bp, int32_t S, int64_t* best_cost, int32_t* best_start);
+
+/* ---- pipeline stages (R27) ------------------------------------------------------------
+ * tri[a * (L + 1) + b] = optimum of the segment [a, b) as its own chain whose first layer has no producer (-1 elsewhere) */
+int autoddl_ref_segment_optima(const int64_t* T, const int64_t* node, const uint8_t* mask, int32_t L, int32_t K, int64_t* tri);
+/* xfer[b] = 2 m (alpha_inter + ceil(bytes of layer b's input / devices of the mesh) beta_inter), xfer[0] = 0 */
+int autoddl_ref_stage_transfer(const ref_layer* layers, int32_t L, const ref_mesh* mesh, const ref_net* net, int64_t* xfer);
+/* best `stages` contiguous segments; objective 0 = sum of the stage costs, 1 = max; cuts[stages + 1] */
+int autoddl_ref_pipeline_partition(const int64_t* tri, const int64_t* xfer, int32_t L, int32_t stages, int32_t objective,
+                                   int64_t* value, int32_t* cuts);
+/* per-segment optimum strategies under given cuts: seg_cost[stages], strategy[L] */
+int autoddl_ref_segment_strategies(const int64_t* T, const int64_t* node, const uint8_t* mask, int32_t L, int32_t K,
+                                   const int32_t* cuts, int32_t stages, int64_t* seg_cost, int32_t* strategy);
 
 /* ---- Metropolis-Hastings sampler (R19-R22) --------------------------------
  * n-th output (n >= 1) of splitmix64 started at `seed`: the counter-based generator both sides implement. */

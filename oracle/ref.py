@@ -76,6 +76,14 @@ def lib():
         L.autoddl_ref_coord_descent.argtypes = [vp, i32, i32, i32, vp, i32, i32, vp, vp, vp, vp]
         L.autoddl_ref_best_of_starts.restype = C.c_int
         L.autoddl_ref_best_of_starts.argtypes = [vp, i32, i32, vp, vp]
+        L.autoddl_ref_segment_optima.restype = C.c_int
+        L.autoddl_ref_segment_optima.argtypes = [vp, vp, vp, i32, i32, vp]
+        L.autoddl_ref_stage_transfer.restype = C.c_int
+        L.autoddl_ref_stage_transfer.argtypes = [vp, i32, vp, vp, vp]
+        L.autoddl_ref_pipeline_partition.restype = C.c_int
+        L.autoddl_ref_pipeline_partition.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+        L.autoddl_ref_segment_strategies.restype = C.c_int
+        L.autoddl_ref_segment_strategies.argtypes = [vp, vp, vp, i32, i32, vp, i32, vp, vp]
         L.autoddl_ref_rng.restype = C.c_uint64
         L.autoddl_ref_rng.argtypes = [C.c_uint64, C.c_uint64]
         L.autoddl_ref_neglog_q16.restype = i64
@@ -236,6 +244,47 @@ def best_of_starts(cost: np.ndarray):
     rc = lib().autoddl_ref_best_of_starts(_p(cost), Bp, S, _p(bc), _p(bs))
     assert rc == 0, rc
     return bc, bs
+
+
+# ---- pipeline stages (R27) ----------------------------------------------------------
+def segment_optima(T1: np.ndarray, node1: np.ndarray, mask1: np.ndarray) -> np.ndarray:
+    """one problem: T1 [L,K,K], node1 [L,K], mask1 [L,K] -> tri [L, L+1] (C(a,b) for a < b, -1 elsewhere)"""
+    T1 = np.ascontiguousarray(T1, dtype=np.int64); node1 = np.ascontiguousarray(node1, dtype=np.int64)
+    mask1 = np.ascontiguousarray(mask1, dtype=np.uint8)
+    L, K, _ = T1.shape
+    tri = np.empty((L, L + 1), np.int64)
+    rc = lib().autoddl_ref_segment_optima(_p(T1), _p(node1), _p(mask1), L, K, _p(tri))
+    assert rc == 0, rc
+    return tri
+
+
+def stage_transfer(layers1: np.ndarray, mesh: RefMesh, net: RefNet) -> np.ndarray:
+    layers1 = np.ascontiguousarray(layers1)
+    L = layers1.shape[0]
+    x = np.empty(L, np.int64)
+    rc = lib().autoddl_ref_stage_transfer(_p(layers1), L, C.addressof(mesh), C.addressof(net), _p(x))
+    assert rc == 0, rc
+    return x
+
+
+def pipeline_partition(tri: np.ndarray, xfer: np.ndarray, stages: int, objective: int):
+    tri = np.ascontiguousarray(tri, dtype=np.int64); xfer = np.ascontiguousarray(xfer, dtype=np.int64)
+    L = tri.shape[0]
+    val = np.empty(1, np.int64); cuts = np.empty(stages + 1, np.int32)
+    rc = lib().autoddl_ref_pipeline_partition(_p(tri), _p(xfer), L, stages, objective, _p(val), _p(cuts))
+    assert rc == 0, rc
+    return int(val[0]), cuts
+
+
+def segment_strategies(T1, node1, mask1, cuts):
+    T1 = np.ascontiguousarray(T1, dtype=np.int64); node1 = np.ascontiguousarray(node1, dtype=np.int64)
+    mask1 = np.ascontiguousarray(mask1, dtype=np.uint8); cuts = np.ascontiguousarray(cuts, dtype=np.int32)
+    L, K, _ = T1.shape
+    stages = len(cuts) - 1
+    sc = np.empty(stages, np.int64); st = np.empty(L, np.int32)
+    rc = lib().autoddl_ref_segment_strategies(_p(T1), _p(node1), _p(mask1), L, K, _p(cuts), stages, _p(sc), _p(st))
+    assert rc == 0, rc
+    return sc, st
 
 
 # ---- Metropolis-Hastings (PAPER.md:227-237) -------------------------------------------------------------

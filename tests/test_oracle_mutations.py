@@ -17,7 +17,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, "oracle", "autoddl_ref.cpp")
 PIN_FILES = ["tests/test_oracle_pins.py", "tests/test_oracle_ragged_pins.py", "tests/test_oracle_mh.py",
-             "tests/test_oracle_accum.py", "tests/test_oracle_paper_space.py", "tests/test_oracle_pipeline.py"]
+             "tests/test_oracle_accum.py", "tests/test_oracle_paper_space.py", "tests/test_oracle_pipeline.py",
+             "tests/test_shard_gloo.py::test_oracle_best_of_starts_lowest_index"]
 DESELECT = "not survey_crosscheck and not brute_force_config1"
 
 # (name, old text, new text, which occurrence of `old` (0-based; None = it must be unique))
@@ -59,7 +60,8 @@ MUTANTS = [
     ("M17 floor instead of ceil", "return (a + b - 1) / b;", "return a / b;", None),
     ("M18 local size with the axes swapped", "return ceil_div(R, f0) * ceil_div(C, f1);", "return ceil_div(R, f1) * ceil_div(C, f0);", None),
     ("M19 DP keeps the last minimiser", "if (v < best) { best = v; arg = i; }", "if (v <= best) { best = v; arg = i; }", None),
-    ("M20 DP end state keeps the last minimiser", "if (f[j] < f[js]) js = j;", "if (f[j] <= f[js]) js = j;", None),
+    ("M20 DP end state keeps the last minimiser", "if (f[j] < f[js]) js = j;", "if (f[j] <= f[js]) js = j;", 0),
+    ("M48 segment end state keeps the last minimiser", "if (f[j] < f[js]) js = j;", "if (f[j] <= f[js]) js = j;", 1),
     ("M21 CD keeps the last minimiser", "if (arg < 0 || g < best) { best = g; arg = c; }", "if (arg < 0 || g <= best) { best = g; arg = c; }", None),
     ("M22 CD ignores the right neighbour", "if (l < L - 1) g += Tp[((int64_t)(l + 1) * K + c) * K + s[l + 1]];",
      "if (l < L - 2) g += Tp[((int64_t)(l + 1) * K + c) * K + s[l + 1]];", None),
@@ -84,6 +86,17 @@ MUTANTS = [
     ("M37 weight-gradient all-reduce charged on P levels", "    if (W[d] == REF_B) {\n      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)\n      v +=",
      "    if (W[d] == REF_B || W[d] == REF_P) {\n      const int c = mesh->link[d] & 1;                 // bit 0: link class; bits 8..13: allowed rows (R24)\n      v +=", None),
     ("M38 memory counts resident weight with the gradient element size", "W, mesh) * cur->wstate_bytes;", "W, mesh) * cur->wgrad_bytes;", None),
+    ("M40 a segment's first layer pays the redistribution from the previous stage",
+     "for (int j = 0; j < K; ++j) f[j] = node[(int64_t)a * K + j] + (mask[(int64_t)a * K + j] ? 0 : REF_PEN);\n    for (int32_t b = a + 1; b <= L; ++b) {",
+     "for (int j = 0; j < K; ++j) f[j] = T[(int64_t)a * K * K + j];\n    for (int32_t b = a + 1; b <= L; ++b) {", None),
+    ("M41 partition forgets the transfer at a stage's right boundary", "+ xfer[a] + (b < L ? xfer[b] : 0); };", "+ xfer[a]; };", None),
+    ("M42 bottleneck objective takes the faster stage", "objective == 0 ? prev + cs : (prev > cs ? prev : cs);", "objective == 0 ? prev + cs : (prev < cs ? prev : cs);", None),
+    ("M43 partition keeps the last start attaining the minimum", "if (v < g[(size_t)k * (L + 1) + b]) {", "if (v <= g[(size_t)k * (L + 1) + b]) {", None),
+    ("M44 stage transfer paid in one direction only", "xfer[b] = 2 * m * (net->alpha_ps[1]", "xfer[b] = m * (net->alpha_ps[1]", None),
+    ("M45 stage transfer over the intra-node link", "xfer[b] = 2 * m * (net->alpha_ps[1] + ceil_div(bytes, q) * net->beta_ps_per_byte[1]);",
+     "xfer[b] = 2 * m * (net->alpha_ps[0] + ceil_div(bytes, q) * net->beta_ps_per_byte[0]);", None),
+    ("M46 segment strategies keep the last minimiser", "if (v < best) { best = v; ar = i; }", "if (v <= best) { best = v; ar = i; }", None),
+    ("M47 best of starts keeps the last start", "if (cost[p * S + s] < cost[p * S + arg]) arg = s;", "if (cost[p * S + s] <= cost[p * S + arg]) arg = s;", None),
 ]
 
 
@@ -103,7 +116,7 @@ def _kill(args):
         f.write(mutated)
     subprocess.check_call(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", "-I", os.path.join(ROOT, "oracle"), cpp, "-o", so])
     env = dict(os.environ, AUTODDL_REF_SO=so)
-    files = [f for f in PIN_FILES if os.path.exists(os.path.join(ROOT, f))]
+    files = [f for f in PIN_FILES if os.path.exists(os.path.join(ROOT, f.split("::")[0]))]
     r = subprocess.run([sys.executable, "-m", "pytest", *files, "-x", "-q", "-k", DESELECT, "-p", "no:cacheprovider"],
                        cwd=ROOT, env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     return name, r.returncode, r.stdout[-400:]
@@ -113,7 +126,7 @@ def test_unmutated_oracle_passes_the_same_selection(tmp_path):
     """the selection used against the mutants is green on the real oracle (otherwise every mutant dies trivially)"""
     so = os.path.join(str(tmp_path), "clean.so")
     subprocess.check_call(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", SRC, "-o", so])
-    files = [f for f in PIN_FILES if os.path.exists(os.path.join(ROOT, f))]
+    files = [f for f in PIN_FILES if os.path.exists(os.path.join(ROOT, f.split("::")[0]))]
     r = subprocess.run([sys.executable, "-m", "pytest", *files, "-x", "-q", "-k", DESELECT, "-p", "no:cacheprovider"],
                        cwd=ROOT, env=dict(os.environ, AUTODDL_REF_SO=so), stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     assert r.returncode == 0, r.stdout[-2000:]
