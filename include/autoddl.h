@@ -179,6 +179,38 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
 int autoddl_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t* d_best_cost, int32_t* d_best_start,
                            void* stream);
 
+/* ---- Pipeline stages ("consecutive layers form a pipeline stage", 1F1B, Table 3 "Opt.
+ * Stages"; R27).  ONE chain of L layers.  A stage is a contiguous segment [a, b) of the chain on its own
+ * sub-mesh (the mesh with 1 / stages of the nodes); d_T / d_node / d_mask are the outputs of autoddl_build_tables for the
+ * chain ON THAT SUB-MESH.  The stage COST MODEL below is this library's reading: the paper prints none.
+ *
+ * autoddl_segment_optima: d_tri [L][L + 1] int64, d_tri[a][b] = C(a, b) = the optimum over all K^(b-a) strategies of the
+ *   segment [a, b) as a chain of its own whose first layer has no producer (f_a[j] = node[a][j] + 2^50 [mask[a][j] == 0]);
+ *   -1 for a >= b.  One pass over the tables for all L (L + 1) / 2 segments (min-plus products of 16 starts at a time).
+ * autoddl_stage_transfer: d_xfer [L] int64, d_xfer[b] = 2 m (alpha_inter + ceil(in_rows_b in_cols_b act_bytes_b / q)
+ *   beta_inter): the input of layer b, split over the q devices of the sub-mesh, crosses the network point to point
+ *    forward and backward once per micro-batch (m = net.micro_batches); d_xfer[0] = 0.
+ * autoddl_pipeline_partition: the best `stages` contiguous non-empty segments; stage cost c(a, b) = C(a, b) + xfer[a] +
+ *   [b < L] xfer[b]; objective 0 = sum of the stage costs, 1 = max (the slowest stage paces a 1F1B pipeline).
+ *   g_1[b] = c(0, b); g_k[b] = min_a comb(g_{k-1}[a], c(a, b)), smallest a on ties; d_value [1] = g_stages[L];
+ *   d_cuts [stages + 1] by back-tracking (d_cuts[0] = 0, d_cuts[stages] = L).  d_work >= autoddl_pipeline_workspace_bytes.
+ * autoddl_segment_strategies: per stage k the optimum strategy of [d_cuts[k], d_cuts[k + 1]) (smallest index on every
+ *   tie, as autoddl_chain_dp): d_seg_cost [stages] = C(.,.), d_strategy [L].  d_cuts is read on the device: no host
+ *   synchronisation between the partition and the strategies.  d_work >= autoddl_pipeline_workspace_bytes.
+ * All pointers are device pointers (8-byte aligned for int64, 4 for int32, d_work 256); asynchronous on `stream`.
+ * The outer enumeration over stage counts (build the tables on every candidate sub-mesh, partition, compare) is the
+ * caller's loop. */
+size_t autoddl_pipeline_workspace_bytes(int32_t L, int32_t K, int32_t stages);
+int autoddl_segment_optima(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L,
+                           const autoddl_mesh* mesh, int64_t* d_tri, void* stream);
+int autoddl_stage_transfer(const autoddl_layer* d_layers, int32_t L, const autoddl_mesh* mesh, const autoddl_net* net,
+                           int64_t* d_xfer, void* stream);
+int autoddl_pipeline_partition(const int64_t* d_tri, const int64_t* d_xfer, int32_t L, int32_t stages, int32_t objective,
+                               void* d_work, size_t work_bytes, int64_t* d_value, int32_t* d_cuts, void* stream);
+int autoddl_segment_strategies(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L,
+                               const autoddl_mesh* mesh, const int32_t* d_cuts, int32_t stages, void* d_work, size_t work_bytes,
+                               int64_t* d_seg_cost, int32_t* d_strategy, void* stream);
+
 /* Plain device-to-device copy kernel (int4 grid-stride), used by bench.py to measure the HBM
  * copy bandwidth in the same run as the kernels above.  bytes must be a multiple of 16. */
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream);

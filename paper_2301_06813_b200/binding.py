@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
+    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_pipeline_workspace_bytes", "autoddl_segment_optima", "autoddl_stage_transfer",
+    "autoddl_pipeline_partition", "autoddl_segment_strategies", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -67,6 +68,16 @@ def lib():
         L.autoddl_search_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp, sz, vp, vp, vp, vp, vp, vp]
         L.autoddl_best_of_starts.restype = C.c_int
         L.autoddl_best_of_starts.argtypes = [vp, i32, i32, vp, vp, vp]
+        L.autoddl_pipeline_workspace_bytes.restype = sz
+        L.autoddl_pipeline_workspace_bytes.argtypes = [i32, i32, i32]
+        L.autoddl_segment_optima.restype = C.c_int
+        L.autoddl_segment_optima.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+        L.autoddl_stage_transfer.restype = C.c_int
+        L.autoddl_stage_transfer.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.autoddl_pipeline_partition.restype = C.c_int
+        L.autoddl_pipeline_partition.argtypes = [vp, vp, i32, i32, i32, vp, sz, vp, vp, vp]
+        L.autoddl_segment_strategies.restype = C.c_int
+        L.autoddl_segment_strategies.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, sz, vp, vp, vp]
         L.autoddl_copy_probe.restype = C.c_int
         L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
         L.autoddl_fit_workspace_bytes.restype = sz
@@ -261,6 +272,31 @@ def best_of_starts(cost: torch.Tensor, out=None):
         out = (torch.empty(Bp, dtype=torch.int64, device=cost.device), torch.empty(Bp, dtype=torch.int32, device=cost.device))
     _check(lib().autoddl_best_of_starts(_ptr(cost, I64, "cost"), Bp, S, _ptr(out[0], I64, "best_cost"), _ptr(out[1], I32, "best_start"), _stream()))
     return out
+
+
+def pipeline_stages(d_layers1: torch.Tensor, T1: torch.Tensor, node1: torch.Tensor, mask1: torch.Tensor, mesh, net, stages: int,
+                    objective: int = 1):
+    """Pipeline-stage enumeration of ONE chain whose tables (T1 [L,K,K], node1 [L,K], mask1 [L,K]; d_layers1 [L,64]) were
+    built on the stage sub-mesh `mesh`: -> dict(tri [L, L+1], xfer [L], value [1], cuts [stages+1], seg_cost [stages],
+    strategy [L]) -- four kernels, no host synchronisation in between."""
+    L, K = T1.shape[0], T1.shape[1]
+    dev = T1.device
+    m, n = c_mesh(mesh), c_net(net)
+    tri = torch.empty((L, L + 1), dtype=torch.int64, device=dev)
+    xfer = torch.empty(L, dtype=torch.int64, device=dev)
+    value = torch.empty(1, dtype=torch.int64, device=dev)
+    cuts = torch.empty(stages + 1, dtype=torch.int32, device=dev)
+    seg_cost = torch.empty(stages, dtype=torch.int64, device=dev)
+    strategy = torch.empty(L, dtype=torch.int32, device=dev)
+    work = torch.empty(int(lib().autoddl_pipeline_workspace_bytes(L, K, stages)), dtype=torch.uint8, device=dev)
+    _check(lib().autoddl_segment_optima(_ptr(T1, I64, "T"), _ptr(node1, I64, "node"), _ptr(mask1, U8, "mask"), L, C.addressof(m),
+                                        _ptr(tri), _stream()))
+    _check(lib().autoddl_stage_transfer(_ptr(d_layers1, U8, "d_layers"), L, C.addressof(m), C.addressof(n), _ptr(xfer), _stream()))
+    _check(lib().autoddl_pipeline_partition(_ptr(tri), _ptr(xfer), L, stages, objective, _ptr(work), work.numel(), _ptr(value),
+                                            _ptr(cuts), _stream()))
+    _check(lib().autoddl_segment_strategies(_ptr(T1, I64, "T"), _ptr(node1, I64, "node"), _ptr(mask1, U8, "mask"), L, C.addressof(m),
+                                            _ptr(cuts), stages, _ptr(work), work.numel(), _ptr(seg_cost), _ptr(strategy), _stream()))
+    return dict(tri=tri, xfer=xfer, value=value, cuts=cuts, seg_cost=seg_cost, strategy=strategy)
 
 
 def profile_mark(event: "torch.cuda.Event | None"):

@@ -464,6 +464,75 @@ int autoddl_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t
   return launch_best_of_starts(d_cost, Bp, S, d_best_cost, d_best_start, (cudaStream_t)stream);
 }
 
+size_t autoddl_pipeline_workspace_bytes(int32_t L, int32_t K, int32_t stages) {
+  if (L < 1 || K < 1 || stages < 1) return 0;
+  const size_t a = partition_workspace_bytes(L, stages), b = align_up((size_t)L * K, 256) + 256;
+  return a > b ? a : b;
+}
+
+int autoddl_segment_optima(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, const autoddl_mesh* mesh,
+                           int64_t* d_tri, void* stream) {
+  clear_error();
+  int rc = validate_mesh_net(mesh, nullptr, nullptr);
+  if (rc) return rc;
+  ADL_REQUIRE(d_T && d_node && d_mask && d_tri, "NULL pointer");
+  ADL_REQUIRE(L >= 1, "L must be >= 1");
+  ADL_REQUIRE(((uintptr_t)d_T & 7) == 0 && ((uintptr_t)d_node & 7) == 0 && ((uintptr_t)d_tri & 7) == 0, "misaligned pointer");
+  if ((rc = check_device())) return rc;
+  return launch_segment_optima(d_T, d_node, d_mask, L, mesh_num_sigs(mesh), d_tri, (cudaStream_t)stream);
+}
+
+int autoddl_stage_transfer(const autoddl_layer* d_layers, int32_t L, const autoddl_mesh* mesh, const autoddl_net* net,
+                           int64_t* d_xfer, void* stream) {
+  clear_error();
+  MeshParams mp;
+  ADL_REQUIRE(net != nullptr, "net is NULL");
+  int rc = validate_mesh_net(mesh, net, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(d_layers && d_xfer, "NULL pointer");
+  ADL_REQUIRE(L >= 1, "L must be >= 1");
+  ADL_REQUIRE(((uintptr_t)d_layers & 7) == 0 && ((uintptr_t)d_xfer & 7) == 0, "misaligned pointer");
+  if ((rc = check_device())) return rc;
+  int64_t q = 1;
+  for (int d = 0; d < mesh->ndim; ++d) q *= mesh->size[d];
+  return launch_stage_transfer(d_layers, L, q, mp.accum, net->alpha_ps[1], net->beta_ps_per_byte[1], d_xfer, (cudaStream_t)stream);
+}
+
+int autoddl_pipeline_partition(const int64_t* d_tri, const int64_t* d_xfer, int32_t L, int32_t stages, int32_t objective,
+                               void* d_work, size_t work_bytes, int64_t* d_value, int32_t* d_cuts, void* stream) {
+  clear_error();
+  ADL_REQUIRE(d_tri && d_xfer && d_value && d_cuts, "NULL pointer");
+  ADL_REQUIRE(L >= 1 && stages >= 1 && stages <= L, "need 1 <= stages <= L");
+  ADL_REQUIRE(objective == 0 || objective == 1, "objective: 0 = sum of the stage costs, 1 = max");
+  ADL_REQUIRE(((uintptr_t)d_tri & 7) == 0 && ((uintptr_t)d_xfer & 7) == 0 && ((uintptr_t)d_value & 7) == 0 &&
+                  ((uintptr_t)d_cuts & 3) == 0 && ((uintptr_t)d_work & 255) == 0, "misaligned pointer");
+  if (d_work == nullptr || work_bytes < partition_workspace_bytes(L, stages)) {
+    set_error("pipeline_partition: workspace of %zu bytes needed, %zu given", partition_workspace_bytes(L, stages), d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_partition(d_tri, d_xfer, L, stages, objective, d_work, d_value, d_cuts, (cudaStream_t)stream);
+}
+
+int autoddl_segment_strategies(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L,
+                               const autoddl_mesh* mesh, const int32_t* d_cuts, int32_t stages, void* d_work, size_t work_bytes,
+                               int64_t* d_seg_cost, int32_t* d_strategy, void* stream) {
+  clear_error();
+  int rc = validate_mesh_net(mesh, nullptr, nullptr);
+  if (rc) return rc;
+  ADL_REQUIRE(d_T && d_node && d_mask && d_cuts && d_seg_cost && d_strategy, "NULL pointer");
+  ADL_REQUIRE(L >= 1 && stages >= 1 && stages <= L, "need 1 <= stages <= L");
+  const int K = mesh_num_sigs(mesh);
+  if (d_work == nullptr || work_bytes < (size_t)L * K) {
+    set_error("segment_strategies: workspace of %zu bytes needed, %zu given", (size_t)L * K, d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
+  }
+  if ((rc = check_device())) return rc;
+  return launch_segment_strategies(d_T, d_node, d_mask, L, K, d_cuts, stages, (uint8_t*)d_work, d_seg_cost, d_strategy,
+                                   (cudaStream_t)stream);
+}
+
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {
   clear_error();
   ADL_REQUIRE(d_src && d_dst && bytes > 0 && bytes % 16 == 0, "copy_probe: bad arguments");

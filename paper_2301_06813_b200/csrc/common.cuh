@@ -93,6 +93,16 @@ int launch_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64
 int launch_copy_probe(const void* src, void* dst, size_t bytes, cudaStream_t st);
 int launch_best_of_starts(const int64_t* d_cost, int32_t Bp, int32_t S, int64_t* d_best_cost, int32_t* d_best_start,
                           cudaStream_t st);
+int launch_segment_optima(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, int32_t K,
+                          int64_t* d_tri, cudaStream_t st);
+int launch_stage_transfer(const autoddl_layer* d_layers, int32_t L, int64_t q, int64_t m, int64_t alpha, int64_t beta,
+                          int64_t* d_xfer, cudaStream_t st);
+size_t partition_workspace_bytes(int32_t L, int32_t stages);
+int launch_partition(const int64_t* d_tri, const int64_t* d_xfer, int32_t L, int32_t stages, int32_t objective, void* d_work,
+                     int64_t* d_value, int32_t* d_cuts, cudaStream_t st);
+int launch_segment_strategies(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, int32_t K,
+                              const int32_t* d_cuts, int32_t stages, uint8_t* d_bp, int64_t* d_seg_cost, int32_t* d_strategy,
+                              cudaStream_t st);
 int device_sm_count();                                     // multiprocessors of the current device (148 if the query fails)
 
 // ---- device helpers ------------------------------------------------------------------------------------
