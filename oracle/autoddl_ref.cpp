@@ -40,12 +40,50 @@ inline int level_nrows(const ref_mesh* mesh, int d) {
   return n;
 }
 
+inline bool folded(const ref_mesh* mesh) { return (mesh->link[0] & REF_FOLD) != 0; }
+
+// R28: groups of the folded space = maximal runs of consecutive levels with equal size and link class.  Returns the
+// number of groups; first[g] = first level of group g, len[g] = its number of levels.
+inline int fold_groups(const ref_mesh* mesh, int* first, int* len) {
+  int ng = 0;
+  for (int d = 0; d < mesh->ndim; ++d) {
+    if (d > 0 && mesh->size[d] == mesh->size[d - 1] && (mesh->link[d] & 1) == (mesh->link[d - 1] & 1)) {
+      ++len[ng - 1];
+    } else {
+      first[ng] = d;
+      len[ng] = 1;
+      ++ng;
+    }
+  }
+  return ng;
+}
+inline int fold_radix(int n) { return (n + 2) * (n + 1) / 2; }       // sorted strings of length n over {0,1,2}
+
 // per-level row of level d in signature index j, level 0 most significant.
 // ndim <= 3: j is a base-6 number over all six rows (a disallowed row makes the signature infeasible, R24).
 // ndim  > 3: j is a mixed-radix number over the ALLOWED rows only (R26): the digit x of level d is the x-th allowed
 //            row of that level in increasing order; the radix of level d is its number of allowed rows.
+// folded (R28): j is a mixed-radix number over the groups (group 0 most significant); the digit x of a group of n levels
+//            names the x-th sorted string 0^n0 1^n1 2^n2 (n0 + n1 + n2 = n) in increasing lexicographic order, i.e.
+//            n0 = n, n-1, .. and, for equal n0, n1 descending; level t of the group has row 0 / 1 / 2 accordingly.
 inline int sig_digit(int j, int d, const ref_mesh* mesh) {
   const int D = mesh->ndim;
+  if (folded(mesh)) {
+    int first[REF_MAX_LEVELS], len[REF_MAX_LEVELS];
+    const int ng = fold_groups(mesh, first, len);
+    int g = 0;
+    while (g + 1 < ng && first[g + 1] <= d) ++g;                     // the group of level d
+    int div = 1;
+    for (int t = g + 1; t < ng; ++t) div *= fold_radix(len[t]);
+    int x = (j / div) % fold_radix(len[g]);
+    const int n = len[g], t = d - first[g];
+    for (int n0 = n; n0 >= 0; --n0)
+      for (int n1 = n - n0; n1 >= 0; --n1) {
+        if (x == 0) return t < n0 ? 0 : (t < n0 + n1 ? 1 : 2);
+        --x;
+      }
+    return -1;                                // not reached
+  }
   if (D <= 3) {
     int div = 1;
     for (int t = 0; t < D - 1 - d; ++t) div *= 6;
@@ -72,6 +110,14 @@ inline int32_t dual_state(int32_t s) {   // R9: S0->S0, S1->S1, B->P, P->B
 
 extern "C" int autoddl_ref_num_signatures(const ref_mesh* mesh) {
   if (!mesh || mesh->ndim < 1 || mesh->ndim > REF_MAX_LEVELS) return -1;
+  if (folded(mesh)) {                           // R28: product over the groups of the number of ordered factorisations
+    int first[REF_MAX_LEVELS], len[REF_MAX_LEVELS];
+    const int ng = fold_groups(mesh, first, len);
+    int64_t k = 1;
+    for (int g = 0; g < ng; ++g) k *= fold_radix(len[g]);
+    return k <= 256 ? (int)k : -1;
+  }
+  if (mesh->ndim > 5) return -1;                // more than five levels only in the folded space
   if (mesh->ndim <= 3) return ipow6(mesh->ndim);
   int64_t k = 1;                              // R26: product of the levels' allowed-row counts, at most 256
   for (int d = 0; d < mesh->ndim; ++d) k *= level_nrows(mesh, d);
@@ -222,7 +268,7 @@ extern "C" int autoddl_ref_feasible(const ref_layer* cur, int j, int32_t L, cons
   // of a mesh refined into prime sub-levels is the paper's own factorisation space.
   // (with more than three levels the signature index runs over allowed rows only, R26: nothing to exclude)
   for (int d = 0; d < mesh->ndim; ++d)
-    if (!((level_allow(mesh, d) >> sig_digit(j, d, mesh)) & 1)) return 0;
+    if (!folded(mesh) && !((level_allow(mesh, d) >> sig_digit(j, d, mesh)) & 1)) return 0;   // (folded: rows 0..2 by construction)
   int64_t rowsplit = 1, colsplit = 1;
   for (int d = 0; d < mesh->ndim; ++d) {
     if (I[d] == REF_S0 || O[d] == REF_S0) rowsplit *= mesh->size[d];

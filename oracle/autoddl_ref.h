@@ -17,6 +17,9 @@
  *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours)
  *   chain DP optimum (PAPER.md:225 exhaustive)     pinned  (brute force over K^L)
  *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
+ *   folded factorisation space pinned  (equal, cell by cell, to the canonical signatures of the prime-
+ *                                                  sub-level encoding on every machine both express; decode order by
+ *                                                  enumeration; data-parallel closed form on 2^6 .. 2^8 nodes)
  *   four / five mesh levels    pinned  (size-1 levels reproduce the three-level tables, decode order,
  *                                                  data-parallel closed form, intra-node gather, brute force at K = 81)
  *   pipeline stages         segment optima and the partition pinned (one stage = the chain DP,
@@ -51,8 +54,12 @@ typedef struct {
   int32_t max_split_cols;
 } ref_layer;                 /* 64 bytes */
 
-/* link[d]: bit 0 = 0 intra / 1 inter; bits 8..13 = allowed signature rows of the level (bit g = row g; 0 = all six) */
-#define REF_MAX_LEVELS 5
+/* link[d]: bit 0 = 0 intra / 1 inter; bits 8..13 = allowed signature rows of the level (bit g = row g; 0 = all six);
+ * bit 14 of link[0] = FOLDED factorisation space (R28): rows {0,1,2} on every level, and inside every group of
+ * consecutive levels with equal size and link class only the sorted digit strings 0..0 1..1 2..2 are signatures -- the
+ * paper's ordered factorisations p = p0 p1 p2 with (nodes, GPUs) tuples.  ndim up to 8 when folded. */
+#define REF_MAX_LEVELS 8
+#define REF_FOLD 0x4000
 typedef struct { int32_t ndim; int32_t size[REF_MAX_LEVELS]; int32_t link[REF_MAX_LEVELS]; } ref_mesh;
 /* micro_batches: gradient accumulation: the activation redistributions run once per micro-batch,
  * the weight-gradient synchronisation once per mini-batch; 0 or 1 = no accumulation (R25) */
@@ -61,7 +68,9 @@ typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_c
 #define REF_PEN ((int64_t)1 << 50)
 
 /* signatures per layer: 6^ndim for ndim <= 3; for ndim = 4, 5 the product of the levels' allowed-row counts
- * (<= 256, else -1): there the signature index is a mixed-radix number over the allowed rows only (R26) */
+ * (<= 256, else -1): there the signature index is a mixed-radix number over the allowed rows only (R26);
+ * folded (R28): the product over the groups of equal levels of C(n_g + 2, 2) (<= 256), group 0 most significant, inside
+ * a group the sorted strings in increasing lexicographic order */
 int autoddl_ref_num_signatures(const ref_mesh* mesh);
 
 /* Table 2. which: 0 AllGather, 1 ReduceScatter, 2 AllReduce, 3 AlltoAll */

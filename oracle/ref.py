@@ -29,7 +29,7 @@ def build(force: bool = False) -> str:
 
 
 class RefMesh(C.Structure):
-    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 5), ("link", C.c_int32 * 5)]
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 8), ("link", C.c_int32 * 8)]
 
 
 class RefNet(C.Structure):
@@ -147,7 +147,7 @@ def local_size(R, Cc, st, mesh: RefMesh) -> int:
 
 
 def sig_states(kind, sig, mesh: RefMesh):
-    I = np.zeros(5, np.int32); W = np.zeros(5, np.int32); O = np.zeros(5, np.int32)
+    I = np.zeros(8, np.int32); W = np.zeros(8, np.int32); O = np.zeros(8, np.int32)
     v = lib().autoddl_ref_sig_states(kind, sig, C.addressof(mesh), _p(I), _p(W), _p(O))
     D = mesh.ndim
     return int(v), tuple(I[:D].tolist()), tuple(W[:D].tolist()), tuple(O[:D].tolist())

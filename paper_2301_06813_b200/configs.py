@@ -29,6 +29,7 @@ assert LAYER_DTYPE.itemsize == 64
 
 GEMM, ATTN = 0, 1
 INTRA, INTER = 0, 1
+FOLD = 0x4000            # bit 14 of mesh.link[0]: the folded factorisation space (R28)
 
 # picoseconds; 5 us intra-node, 20 us inter-node (BASELINE.json configs[0])
 ALPHA_PS = (5_000_000, 20_000_000)
@@ -73,7 +74,17 @@ class Mesh:
 
     @property
     def K(self) -> int:
-        """6^ndim for ndim <= 3; beyond, the signature index runs over the allowed rows only (R26)"""
+        """6^ndim for ndim <= 3; beyond, the signature index runs over the allowed rows only (R26); folded
+        (bit 14 of link[0], R28): the product over the groups of equal levels of the number of ordered factorisations"""
+        if self.link[0] & FOLD:
+            k, d = 1, 0
+            while d < self.ndim:
+                n = 1
+                while d + n < self.ndim and self.size[d + n] == self.size[d] and (self.link[d + n] & 1) == (self.link[d] & 1):
+                    n += 1
+                k *= (n + 2) * (n + 1) // 2
+                d += n
+            return k
         if self.ndim <= 3:
             return 6 ** self.ndim
         k = 1
@@ -274,6 +285,22 @@ def config8_vgg13_32_nodes() -> Workload:
                     Net(ALPHA_PS, (BETA_300, BETA_12_5), 16 * 10**9), S=64)
 
 
+def config9_piz_daint_transformer(nodes: int = 64) -> Workload:
+    """Not in BASELINE.json: the paper's Piz Daint Transformer runs (model dimension 8,192, 64 heads of 128,
+    8 / 20 / 44 layers on 64 / 128 / 256 single-GPU P100 nodes, batch 1,024 sequences of 1,024 tokens, fp32), searched in
+    the FOLDED factorisation space (R28): the nodes as 6 / 7 / 8 equal prime sub-levels of size 2, one signature
+    per ordered factorisation p = p0 p1 p2 (K = 28 / 36 / 45).  The batch runs as 64 micro-batches of 16 sequences
+    (R25).  Synthetic records, no weights."""
+    n = {64: 6, 128: 7, 256: 8}[nodes]
+    layers = {64: 8, 128: 20, 256: 44}[nodes]
+    M, H = 16 * 1024, 8192
+    recs = []
+    for _ in range(layers):
+        recs += _transformer_block(M, H, 4 * H, act=4, wgrad=4, wstate=16, attn_rows=16, attn_heads=64)
+    return Workload("piz-daint-transformer-%d-nodes" % nodes, _stack(recs), Mesh((2,) * n, (INTER | FOLD,) + (INTER,) * (n - 1)),
+                    Net(ALPHA_PS, (BETA_300, BETA_12_5), 16 * 10**9, micro_batches=64), S=64)
+
+
 CONFIGS = {
     1: config1_tiny,
     2: config2_vgg16,
@@ -283,4 +310,7 @@ CONFIGS = {
     6: config6_paper_space,
     7: config7_two_nodes_sixteen_gpus,
     8: config8_vgg13_32_nodes,
+    9: config9_piz_daint_transformer,
+    10: lambda: config9_piz_daint_transformer(128),
+    11: lambda: config9_piz_daint_transformer(256),
 }

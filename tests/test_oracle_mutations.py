@@ -17,7 +17,7 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, "oracle", "autoddl_ref.cpp")
 PIN_FILES = ["tests/test_oracle_pins.py", "tests/test_oracle_ragged_pins.py", "tests/test_oracle_mh.py",
-             "tests/test_oracle_accum.py", "tests/test_oracle_paper_space.py", "tests/test_oracle_pipeline.py",
+             "tests/test_oracle_accum.py", "tests/test_oracle_paper_space.py", "tests/test_oracle_pipeline.py", "tests/test_oracle_folded.py",
              "tests/test_shard_gloo.py::test_oracle_best_of_starts_lowest_index"]
 DESELECT = "not survey_crosscheck and not brute_force_config1"
 
@@ -96,6 +96,9 @@ MUTANTS = [
     ("M45 stage transfer over the intra-node link", "xfer[b] = 2 * m * (net->alpha_ps[1] + ceil_div(bytes, q) * net->beta_ps_per_byte[1]);",
      "xfer[b] = 2 * m * (net->alpha_ps[0] + ceil_div(bytes, q) * net->beta_ps_per_byte[0]);", None),
     ("M46 segment strategies keep the last minimiser", "if (v < best) { best = v; ar = i; }", "if (v <= best) { best = v; ar = i; }", None),
+    ("M50 folded space enumerates p1 upwards", "for (int n1 = n - n0; n1 >= 0; --n1) {", "for (int n1 = 0; n1 <= n - n0; ++n1) {", None),
+    ("M51 folded groups ignore the link class", "mesh->size[d] == mesh->size[d - 1] && (mesh->link[d] & 1) == (mesh->link[d - 1] & 1)",
+     "mesh->size[d] == mesh->size[d - 1]", None),
     ("M47 best of starts keeps the last start", "if (cost[p * S + s] < cost[p * S + arg]) arg = s;", "if (cost[p * S + s] <= cost[p * S + arg]) arg = s;", None),
 ]
 
