@@ -70,7 +70,16 @@ typedef struct {
  * signature index runs over the ALLOWED rows only, a mixed-radix number with level 0 most significant whose digit x
  * on level d names the x-th allowed row of that level in increasing order; K = product of the levels' allowed-row
  * counts and must be <= 256 (81 / 243 with 0x07 << 8 on every level). */
-#define AUTODDL_MAX_LEVELS 5
+/* FOLDED factorisation space (R28): bit 14 (AUTODDL_FOLD) of link[0].  Rows {0,1,2} on every level (bits 8..13
+ * are ignored), ndim up to 8, and inside every group of consecutive levels with equal size and link class only the
+ * sorted digit strings 0..0 1..1 2..2 are signatures: one signature per ordered factorisation p = p0 p1 p2 of the group
+ * -- with an inter-node group followed by an intra-node group these are the paper's (nodes, GPUs) tuples per SBP
+ * dimension.  The index is a mixed-radix number over the groups, group 0 most significant; the digit
+ * of a group of n levels enumerates its (n + 2)(n + 1) / 2 strings in increasing lexicographic order (p0 descending,
+ * then p1 descending); K = the product over the groups, <= 256 (28 / 36 / 45 for 2^6 / 2^7 / 2^8 single-GPU nodes).
+ * Costs are those of the same digit strings in the per-level encoding above. */
+#define AUTODDL_MAX_LEVELS 8
+#define AUTODDL_FOLD 0x4000
 typedef struct { int32_t ndim; int32_t size[AUTODDL_MAX_LEVELS]; int32_t link[AUTODDL_MAX_LEVELS]; } autoddl_mesh;
 
 /* alpha-beta parameters per link class; mem_cap_bytes 0 = no cap.
@@ -79,7 +88,8 @@ typedef struct { int32_t ndim; int32_t size[AUTODDL_MAX_LEVELS]; int32_t link[AU
  * Must be < 2^20.  48 bytes. */
 typedef struct { int64_t alpha_ps[2]; int64_t beta_ps_per_byte[2]; int64_t mem_cap_bytes; int64_t micro_batches; } autoddl_net;
 
-/* K = 6^ndim for ndim <= 3, the product of the allowed-row counts for ndim = 4, 5; or AUTODDL_EINVAL. Host only. */
+/* K = 6^ndim for ndim <= 3, the product of the allowed-row counts for ndim = 4, 5, the number of ordered factorisations
+ * in the folded space; or AUTODDL_EINVAL. Host only. */
 int autoddl_num_signatures(const autoddl_mesh* mesh);
 
 /* Bytes of device workspace that any entry point below may need for (Bp, L, S): the tables when

@@ -30,7 +30,7 @@ class AutoddlError(RuntimeError):
 
 
 class CMesh(C.Structure):
-    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 5), ("link", C.c_int32 * 5)]
+    _fields_ = [("ndim", C.c_int32), ("size", C.c_int32 * 8), ("link", C.c_int32 * 8)]
 
 
 class CNet(C.Structure):
@@ -101,8 +101,8 @@ def _check(rc: int):
 
 def c_mesh(mesh) -> CMesh:
     m = CMesh()
-    m.ndim = len(mesh.size)                       # ndim outside 1..5 is rejected by the library
-    for d in range(min(m.ndim, 5)):
+    m.ndim = len(mesh.size)                       # ndim outside 1..8 is rejected by the library
+    for d in range(min(m.ndim, 8)):
         m.size[d] = int(mesh.size[d])
         m.link[d] = int(mesh.link[d])
     return m

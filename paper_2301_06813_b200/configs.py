@@ -289,16 +289,17 @@ def config9_piz_daint_transformer(nodes: int = 64) -> Workload:
     """Not in BASELINE.json: the paper's Piz Daint Transformer runs (model dimension 8,192, 64 heads of 128,
     8 / 20 / 44 layers on 64 / 128 / 256 single-GPU P100 nodes, batch 1,024 sequences of 1,024 tokens, fp32), searched in
     the FOLDED factorisation space (R28): the nodes as 6 / 7 / 8 equal prime sub-levels of size 2, one signature
-    per ordered factorisation p = p0 p1 p2 (K = 28 / 36 / 45).  The batch runs as 64 micro-batches of 16 sequences
-    (R25).  Synthetic records, no weights."""
+    per ordered factorisation p = p0 p1 p2 (K = 28 / 36 / 45).  The batch runs as 256 micro-batches of 4 sequences
+    (R25), which keeps a feasible strategy under the per-layer memory budget of R7 at every size.
+    Synthetic records, no weights."""
     n = {64: 6, 128: 7, 256: 8}[nodes]
     layers = {64: 8, 128: 20, 256: 44}[nodes]
-    M, H = 16 * 1024, 8192
+    M, H = 4 * 1024, 8192
     recs = []
     for _ in range(layers):
-        recs += _transformer_block(M, H, 4 * H, act=4, wgrad=4, wstate=16, attn_rows=16, attn_heads=64)
+        recs += _transformer_block(M, H, 4 * H, act=4, wgrad=4, wstate=16, attn_rows=4, attn_heads=64)
     return Workload("piz-daint-transformer-%d-nodes" % nodes, _stack(recs), Mesh((2,) * n, (INTER | FOLD,) + (INTER,) * (n - 1)),
-                    Net(ALPHA_PS, (BETA_300, BETA_12_5), 16 * 10**9, micro_batches=64), S=64)
+                    Net(ALPHA_PS, (BETA_300, BETA_12_5), 16 * 10**9, micro_batches=256), S=64)
 
 
 CONFIGS = {

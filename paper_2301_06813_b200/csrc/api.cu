@@ -20,12 +20,32 @@ void set_error(const char* fmt, ...) {
 void clear_error() { g_err[0] = 0; }
 void count_launch(int n) { g_launches += n; }
 
+static inline bool mesh_folded(const autoddl_mesh* mesh) { return (mesh->link[0] & AUTODDL_FOLD) != 0; }
+
+// R28: groups = maximal runs of consecutive levels with equal size and link class
+static int fold_groups(const autoddl_mesh* mesh, int32_t* first, int32_t* len) {
+  int ng = 0;
+  for (int d = 0; d < mesh->ndim; ++d) {
+    if (d > 0 && mesh->size[d] == mesh->size[d - 1] && ((mesh->link[d] ^ mesh->link[d - 1]) & 1) == 0) {
+      ++len[ng - 1];
+    } else {
+      first[ng] = d;
+      len[ng++] = 1;
+    }
+  }
+  return ng;
+}
+
 int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshParams* out) {
   ADL_REQUIRE(mesh != nullptr, "mesh is NULL");
   ADL_REQUIRE(mesh->ndim >= 1 && mesh->ndim <= kMaxLevels, "mesh.ndim = %d, must be 1..%d", mesh->ndim, kMaxLevels);
+  const bool fold = mesh_folded(mesh);
+  ADL_REQUIRE(fold || mesh->ndim <= kTabLevels, "mesh.ndim = %d: more than %d levels exist only in the folded space "
+              "(AUTODDL_FOLD in mesh.link[0])", mesh->ndim, kTabLevels);
   for (int d = 0; d < mesh->ndim; ++d) {
     ADL_REQUIRE(mesh->size[d] >= 1 && mesh->size[d] <= 65536, "mesh.size[%d] = %d out of range", d, mesh->size[d]);
-    ADL_REQUIRE((mesh->link[d] & ~0x3f01) == 0, "mesh.link[%d] = %d: bit 0 = link class, bits 8..13 = allowed rows", d, mesh->link[d]);
+    ADL_REQUIRE((mesh->link[d] & ~(0x3f01 | (d == 0 ? AUTODDL_FOLD : 0))) == 0,
+                "mesh.link[%d] = %d: bit 0 = link class, bits 8..13 = allowed rows, bit 14 of link[0] = folded space", d, mesh->link[d]);
   }
   int64_t prod = 1;
   for (int d = 0; d < mesh->ndim; ++d) prod *= mesh->size[d];
@@ -37,14 +57,16 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
     memset(out, 0, sizeof(*out));
     out->ndim = mesh->ndim;
     out->K = K;
+    out->fold = fold ? 1 : 0;
+    if (fold) out->ngroups = fold_groups(mesh, out->gfirst, out->glen);
     for (int d = 0; d < mesh->ndim; ++d) {
       out->size[d] = mesh->size[d];
-      out->allow[d] = ((mesh->link[d] >> 8) & 0x3f) ? ((mesh->link[d] >> 8) & 0x3f) : 0x3f;
+      out->allow[d] = fold ? 0x07 : (((mesh->link[d] >> 8) & 0x3f) ? ((mesh->link[d] >> 8) & 0x3f) : 0x3f);
       out->magic_size[d] = (uint64_t)((((unsigned __int128)1 << 64) + mesh->size[d] - 1) / mesh->size[d]);
     }
-    for (int m = 0; m < (1 << kMaxLevels); ++m) {
+    for (int m = 0; m < (1 << kTabLevels); ++m) {
       int64_t f = 1;
-      for (int d = 0; d < mesh->ndim; ++d)
+      for (int d = 0; d < mesh->ndim && d < kTabLevels; ++d)
         if (m >> d & 1) f *= mesh->size[d];
       out->sub[m] = (int32_t)f;
       out->magic_sub[m] = (uint64_t)((((unsigned __int128)1 << 64) + f - 1) / f);
@@ -72,6 +94,13 @@ int validate_mesh_net(const autoddl_mesh* mesh, const autoddl_net* net, MeshPara
 
 // valid ndim assumed (1..kMaxLevels).  R26: beyond three levels the index runs over the allowed rows only
 int mesh_num_sigs(const autoddl_mesh* mesh) {
+  if (mesh_folded(mesh)) {                                 // R28: ordered factorisations per group of equal levels
+    int32_t first[kMaxLevels], len[kMaxLevels];
+    const int ng = fold_groups(mesh, first, len);
+    int64_t k = 1;
+    for (int g = 0; g < ng; ++g) k *= (int64_t)(len[g] + 2) * (len[g] + 1) / 2;
+    return k > (1 << 20) ? (1 << 20) : (int)k;
+  }
   if (mesh->ndim <= 3) return mesh->ndim == 1 ? 6 : mesh->ndim == 2 ? 36 : 216;
   int64_t k = 1;
   for (int d = 0; d < mesh->ndim; ++d) {
@@ -252,7 +281,7 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   }
   if ((rc = check_device())) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const bool built_here = d_T == nullptr && mp.ndim <= 3;  // tables of this library's builder (base-6 index): identical rows per class
+  const bool built_here = d_T == nullptr && mp.ndim <= 3 && !mp.fold;  // tables of this library's builder (base-6 index): identical rows per class
   if (!d_T) {
     ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
@@ -309,7 +338,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     cudaEventRecord(g_dp_done, st);
     g_dp_done = nullptr;
   }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3);
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3 && !mp.fold);
   return AUTODDL_OK;
 }
 

@@ -901,6 +901,7 @@ int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, co
                         int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
   const int64_t nt = (int64_t)Bp * L;
   if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  if (mp.fold) return launch_build_tables_folded(d_layers, Bp, L, mp, d_T, d_node, d_mask, st);
   switch (mp.ndim) {
     case 1: return launch_d<1>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);
     case 2: return launch_36(d_layers, (int)nt, L, mp, d_T, d_node, d_mask, st);

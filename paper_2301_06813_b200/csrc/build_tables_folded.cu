@@ -1,0 +1,198 @@
+// (a1) for the FOLDED factorisation space (R28; PAPER.md:193 p = p0 p1 p2, :201 (nodes, GPUs) tuples): up to
+// eight mesh levels, one signature per ordered factorisation of every group of equal levels (K <= 256; 28 / 36 / 45 on
+// 2^6 / 2^7 / 2^8 single-GPU nodes).  The 3^D split-configuration tables of the other builders do not exist at D = 8,
+// so a cell walks its redistribution itself -- but on bit masks: a tensor state is (m0, m1) = the sets of levels that
+// split its rows / columns, the local size is Q_rows[m0] * Q_cols[m1] with Q[x][m] = ceil(extent x / product of the levels
+// in m) tabulated once per tile for all 2^D subsets (no division in the walk), and a level's state is two bits of a
+// packed word.  One CTA per tile (grid-stride), one thread per cell.
+#include "sbp_builder.cuh"
+
+namespace autoddl {
+
+namespace {
+
+constexpr int kFoldNT = 256;
+
+struct FoldSmem {
+  int64_t Q[5][256];                                     // M, Kd, N, in_rows, in_cols  x  level subset
+  int64_t VP[256];
+  uint16_t dig[256];                                     // per signature: row (0, 1, 2) of level d at bits 2d
+  RecBuf rec;
+};
+
+// packed per-level states (two bits per level) of a signature's digits for a layer kind; false if invalid for the kind
+__device__ __forceinline__ bool fold_states(int kind, uint32_t dig, int D, uint32_t& sI, uint32_t& sW, uint32_t& sO) {
+  sI = sW = sO = 0;
+  bool valid = true;
+  for (int d = 0; d < D; ++d) {
+    const int g = dig >> (2 * d) & 3;
+    int i, w, o;
+    if (kind == AUTODDL_GEMM) { i = c_gemm_I[g]; w = c_gemm_W[g]; o = c_gemm_O[g]; }
+    else { i = o = c_attn_IO[g]; w = kB; if (i < 0) { valid = false; i = o = kB; } }
+    sI |= i << (2 * d); sW |= w << (2 * d); sO |= o << (2 * d);
+  }
+  return valid;
+}
+
+__device__ __forceinline__ uint32_t fold_dual(uint32_t s, int D) {
+  uint32_t r = 0;
+  for (int d = 0; d < D; ++d) r |= (uint32_t)dual_of(s >> (2 * d) & 3) << (2 * d);
+  return r;
+}
+
+// forward redistribution a -> b of the layer's input tensor (R4): slice, reduce-scatter (innermost level
+// first, message = tensor before), all-to-all (innermost first, message = tensor after), all-gather (outermost first,
+// message = tensor after); Table 2 with the level's size and link parameters
+__device__ int64_t fold_walk(uint32_t a, uint32_t b, int D, const int64_t* __restrict__ Qr, const int64_t* __restrict__ Qc,
+                             int64_t eb, const MeshParams& mp) {
+  uint32_t m0 = 0, m1 = 0, mP = 0;                       // levels whose current state is S0 / S1 / P
+  for (int d = 0; d < D; ++d) {
+    int c = a >> (2 * d) & 3;
+    const int t = b >> (2 * d) & 3;
+    if (c == kB && (t == kS0 || t == kS1)) c = t;        // replicated -> split: keep the own slice, free
+    if (c == kS0) m0 |= 1u << d;
+    if (c == kS1) m1 |= 1u << d;
+    if (c == kP) mP |= 1u << d;
+  }
+  int64_t cost = 0;
+  for (int d = D - 1; d >= 0; --d) {                     // partial sums: reduce-scatter
+    const int t = b >> (2 * d) & 3;
+    if ((mP >> d & 1) && t != kP) {
+      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
+      if (p > 1) cost += (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+      mP &= ~(1u << d);
+      if (t == kS0) m0 |= 1u << d; else m1 |= 1u << d;   // P -> B scatters on axis 1 and gathers later
+    }
+  }
+  for (int d = D - 1; d >= 0; --d) {                     // change of split axis: all-to-all
+    const int t = b >> (2 * d) & 3;
+    const bool c0 = m0 >> d & 1, c1 = m1 >> d & 1;
+    if ((c0 && t == kS1) || (c1 && t == kS0)) {
+      m0 ^= 1u << d; m1 ^= 1u << d;
+      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
+      if (p > 1) cost += (p - 1) * mp.alpha[d] + n * mp.beta[d];
+    }
+  }
+  for (int d = 0; d < D; ++d) {                          // split -> replicated: all-gather
+    const int t = b >> (2 * d) & 3;
+    if (((m0 | m1) >> d & 1) && t == kB) {
+      m0 &= ~(1u << d); m1 &= ~(1u << d);
+      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
+      if (p > 1) cost += (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
+    }
+  }
+  return cost;                                           // (-> P is a zero fill, free)
+}
+
+__global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
+                                                                      MeshParams mp, int64_t* __restrict__ T,
+                                                                      int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
+  __shared__ FoldSmem sm;
+  const int tid = threadIdx.x, D = mp.ndim, K = mp.K;
+  // signature index -> digits: mixed radix over the groups (group 0 most significant); inside a group of n levels the
+  // x-th sorted string 0^n0 1^n1 2^n2 in increasing lexicographic order (n0 descending, then n1 descending)
+  for (int j = tid; j < K; j += kFoldNT) {
+    uint32_t dg = 0;
+    int r = j;
+    for (int g = mp.ngroups - 1; g >= 0; --g) {
+      const int n = mp.glen[g], radix = (n + 2) * (n + 1) / 2;
+      int x = r % radix;
+      r /= radix;
+      int n0 = n, n1 = 0;
+      while (x > n - n0) { x -= n - n0 + 1; --n0; }      // n0 = n has 1 string, n0 = n - 1 has 2, ...
+      n1 = n - n0 - x;
+      for (int t = 0; t < n; ++t) dg |= (uint32_t)(t < n0 ? 0 : (t < n0 + n1 ? 1 : 2)) << (2 * (mp.gfirst[g] + t));
+    }
+    sm.dig[j] = (uint16_t)dg;
+  }
+  const int64_t cap_layer = mp.mem_cap / L;
+
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int l = tile % L;
+    __syncthreads();                                     // the previous tile's readers are done
+    if (tid == 0) {
+      const autoddl_layer* cur = layers + tile;
+      RecBuf& r = sm.rec;
+      r.X[0] = cur->M; r.X[1] = cur->Kd; r.X[2] = cur->N; r.X[3] = cur->in_rows; r.X[4] = cur->in_cols;
+      r.kind = cur->kind; r.eb = cur->act_bytes; r.wgb = cur->wgrad_bytes; r.wsb = cur->wstate_bytes;
+      r.maxr = cur->max_split_rows; r.maxc = cur->max_split_cols;
+      r.kind_prev = l > 0 ? (cur - 1)->kind : cur->kind;
+    }
+    __syncthreads();
+    const RecBuf& rec = sm.rec;
+    // ---- 1. Q[x][m] for every subset m of the levels ------------------------------------------------------------------
+    for (int e = tid; e < 5 << D; e += kFoldNT) {
+      const int x = e >> D, m = e & ((1 << D) - 1);
+      int64_t f = 1;
+      for (int d = 0; d < D; ++d)
+        if (m >> d & 1) f *= mp.size[d];
+      sm.Q[x][m] = (rec.X[x] + f - 1) / f;
+    }
+    __syncthreads();
+    // ---- 2. VP[j] = weight-gradient all-reduce + penalty ------------------------------------------------
+    for (int j = tid; j < K; j += kFoldNT) {
+      uint32_t sI, sW, sO;
+      const bool valid = fold_states(rec.kind, sm.dig[j], D, sI, sW, sO);
+      int64_t v = 0, mem = 0, rs = 1, cs = 1;
+      if (valid) {
+        uint32_t w0 = 0, w1 = 0, i0 = 0, i1 = 0, o0 = 0, o1 = 0;
+        for (int d = 0; d < D; ++d) {
+          const int w = sW >> (2 * d) & 3, i = sI >> (2 * d) & 3, o = sO >> (2 * d) & 3;
+          if (w == kS0) w0 |= 1u << d;
+          if (w == kS1) w1 |= 1u << d;
+          if (i == kS0) i0 |= 1u << d;
+          if (i == kS1) i1 |= 1u << d;
+          if (o == kS0) o0 |= 1u << d;
+          if (o == kS1) o1 |= 1u << d;
+          if (i == kS0 || o == kS0) rs *= mp.size[d];
+          if (o == kS1) cs *= mp.size[d];
+        }
+        if (rec.kind == AUTODDL_GEMM) {
+          const int64_t nw = sm.Q[1][w0] * sm.Q[2][w1];
+          for (int d = 0; d < D; ++d)
+            if ((sW >> (2 * d) & 3) == kB) {
+              const int64_t p = mp.size[d], n = nw * (int64_t)rec.wgb;
+              if (p > 1) v += (2 * p - 1) * mp.alpha[d] + 2 * (p - 1) * cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d];
+            }
+          mem = nw * (int64_t)rec.wsb;
+        }
+        mem += (sm.Q[3][i0] * sm.Q[4][i1] + sm.Q[0][o0] * sm.Q[2][o1]) * (int64_t)rec.eb;
+      }
+      const bool ok = valid && rs <= rec.maxr && cs <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
+      sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+      if (node) node[(size_t)tile * K + j] = v;
+      if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
+    }
+    __syncthreads();
+    // ---- 3. the cells: forward + backward redistribution (R5), once per micro-batch (R25) -------------------------------------
+    int64_t* out = T + (size_t)tile * K * K;
+    for (int c = tid; c < K * K; c += kFoldNT) {
+      const int i = c / K, j = c % K;
+      int64_t e = 0;
+      if (l > 0) {
+        uint32_t aI, aW, aO, bI, bW, bO;
+        const bool vi = fold_states(rec.kind_prev, sm.dig[i], D, aI, aW, aO);
+        const bool vj = fold_states(rec.kind, sm.dig[j], D, bI, bW, bO);
+        if (vi && vj)
+          e = fold_walk(aO, bI, D, sm.Q[3], sm.Q[4], rec.eb, mp) + fold_walk(fold_dual(bI, D), fold_dual(aO, D), D, sm.Q[3], sm.Q[4], rec.eb, mp);
+      }
+      out[c] = mp.accum * e + sm.VP[j];
+    }
+  }
+}
+
+}  // namespace
+
+int launch_build_tables_folded(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
+                               int64_t* d_node, uint8_t* d_mask, cudaStream_t st) {
+  const int64_t nt = (int64_t)Bp * L;
+  if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  const int slots = device_sm_count() * 4;
+  const int grid = (int)(nt < slots ? nt : slots);
+  build_tables_folded_kernel<<<grid, kFoldNT, 0, st>>>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+}  // namespace autoddl

@@ -44,6 +44,7 @@ void count_launch(int n = 1);
 
 // ---- mesh / net passed to kernels by value ----------------------------------------------------------
 constexpr int kMaxLevels = AUTODDL_MAX_LEVELS;
+constexpr int kTabLevels = 5;                              // the table-factorised builders handle up to five levels
 struct MeshParams {
   int32_t ndim;
   int32_t K;            // signatures per layer: 6^ndim (ndim <= 3), product of the allowed-row counts (ndim = 4, 5; R26)
@@ -53,9 +54,11 @@ struct MeshParams {
   int64_t beta[kMaxLevels];      // beta  of the level's link class
   int64_t mem_cap;      // 0 = none
   int64_t accum;        // micro-batches per mini-batch (>= 1): multiplies the redistribution costs
-  int32_t sub[1 << kMaxLevels];       // product of the sizes of the levels in subset m (bit e = level e)
-  uint64_t magic_sub[1 << kMaxLevels];   // ceil(2^64 / sub[m])
+  int32_t sub[1 << kTabLevels];       // product of the sizes of the levels in subset m (bit e = level e), levels 0..4
+  uint64_t magic_sub[1 << kTabLevels];   // ceil(2^64 / sub[m])
   uint64_t magic_size[kMaxLevels];  // ceil(2^64 / size[d])
+  int32_t fold;                     // folded factorisation space (R28): groups of equal levels
+  int32_t ngroups, gfirst[kMaxLevels], glen[kMaxLevels];
 };
 
 // fills *out (may be NULL); returns AUTODDL_OK or AUTODDL_EINVAL.  K of a valid mesh: mesh_num_sigs()
@@ -65,6 +68,8 @@ int mesh_num_sigs(const autoddl_mesh* mesh);
 // ---- kernel launchers (defined in the .cu files) ----------------------------------------------------
 int launch_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp,
                         int64_t* d_T, int64_t* d_node, uint8_t* d_mask, cudaStream_t st);
+int launch_build_tables_folded(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp,
+                               int64_t* d_T, int64_t* d_node, uint8_t* d_mask, cudaStream_t st);
 bool fused_build_dp_supported(const MeshParams& mp, int32_t L);
 size_t fused_bp_bytes(int32_t L);
 int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,

@@ -446,7 +446,7 @@ bool bp_fits_smem(int32_t L, int32_t S) { return 8 * warp_bytes(L, S, true) + si
 
 }  // namespace
 
-bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim == 2 && L >= 1; }
+bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim == 2 && !mp.fold && L >= 1; }
 
 // largest S for which the first CD sweep rides in the fused kernel (one row stash of two registers per start and lane)
 bool fused_cd_sweep_supported(int32_t L, int32_t S) { return S >= 1 && S <= kMaxFusedStarts && (int64_t)S * L <= 8192; }

@@ -38,7 +38,7 @@ def test_struct_layouts_match_header(adl):
     assert cf.LAYER_DTYPE.itemsize == 64
     assert [cf.LAYER_DTYPE.fields[k][1] for k in ("M", "Kd", "N", "in_rows", "in_cols", "kind", "act_bytes",
             "wgrad_bytes", "wstate_bytes", "max_split_rows", "max_split_cols")] == [0, 8, 16, 24, 32, 40, 44, 48, 52, 56, 60]
-    assert C.sizeof(adl.CMesh) == 44 and C.sizeof(adl.CNet) == 48
+    assert C.sizeof(adl.CMesh) == 68 and C.sizeof(adl.CNet) == 48
 
 
 def test_host_only_calls(adl):

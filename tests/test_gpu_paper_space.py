@@ -87,6 +87,6 @@ def test_fused_kernel_on_the_paper_space(adl):
 
 def test_bad_link_bits_rejected(adl):
     with pytest.raises(adl.AutoddlError, match="link"):
-        adl.num_signatures(cf.Mesh((2, 2), (1 | (1 << 14), 0)))
+        adl.num_signatures(cf.Mesh((2, 2), (1 | (1 << 15), 0)))
     with pytest.raises(adl.AutoddlError, match="link"):
         adl.num_signatures(cf.Mesh((2, 2), (2, 0)))
