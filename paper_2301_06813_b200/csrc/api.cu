@@ -193,9 +193,11 @@ int autoddl_num_signatures(const autoddl_mesh* mesh) {
 
 size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_mesh* mesh) {
   clear_error();
-  if (validate_mesh_net(mesh, nullptr, nullptr) || Bp < 1 || L < 1 || S < 0) return 0;
+  MeshParams mp;
+  if (validate_mesh_net(mesh, nullptr, &mp) || Bp < 1 || L < 1 || S < 0) return 0;
   const int64_t K = mesh_num_sigs(mesh);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
+  if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L);   // many starts: factors + best responses
   if (mesh->ndim == 2) b += fused_bp_bytes(L);              // fused build + DP: back-pointers of the chains in flight
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
   b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
@@ -274,13 +276,24 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   ADL_REQUIRE(((uintptr_t)d_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0 && ((uintptr_t)d_init & 3) == 0 &&
                   ((uintptr_t)d_sweeps & 3) == 0, "misaligned pointer");
   const int K = mp.K;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!d_T && cd_lookup_supported(mp, L, S)) {
+    // many starts on library-built tables: no K x K table at all (factors -> best responses -> look-up sweeps)
+    ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
+    const size_t need = cd_lookup_workspace_bytes(mp, Bp, L);
+    if (d_work == nullptr || work_bytes < need) {
+      set_error("coord_descent: workspace of %zu bytes needed, %zu given", need, d_work ? work_bytes : (size_t)0);
+      return AUTODDL_EWORK;
+    }
+    if ((rc = check_device())) return rc;
+    return launch_cd_lookup(d_layers, Bp, L, mp, d_work, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+  }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K);
   if (tb > 0 && (d_work == nullptr || work_bytes < tb)) {
     set_error("coord_descent: workspace of %zu bytes needed, %zu given", tb, d_work ? work_bytes : (size_t)0);
     return AUTODDL_EWORK;
   }
   if ((rc = check_device())) return rc;
-  cudaStream_t st = (cudaStream_t)stream;
   const bool built_here = d_T == nullptr && mp.ndim <= 3 && !mp.fold;  // tables of this library's builder (base-6 index): identical rows per class
   if (!d_T) {
     ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
@@ -338,6 +351,13 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     cudaEventRecord(g_dp_done, st);
     g_dp_done = nullptr;
   }
+  if (do_cd && !cd_resume && cd_lookup_supported(mp, L, S)) {
+    // many starts per problem: best-response look-ups on the factors instead of gathers on the K x K tables
+    const size_t off = (used + (fused ? fused_bp_bytes(L) : bp_bytes(Bp, L, K)) + 255) / 256 * 256;
+    const size_t need = off + cd_lookup_workspace_bytes(mp, Bp, L);
+    if (d_work != nullptr && work_bytes >= need)
+      return launch_cd_lookup(d_layers, Bp, L, mp, d_work + off, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+  }
   if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3 && !mp.fold);
   return AUTODDL_OK;
 }
@@ -392,7 +412,8 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
 
   unsigned char* w = (unsigned char*)d_work;
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
-  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) + (mesh->ndim == 2 ? fused_bp_bytes(L) : 0);
+  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) + (mesh->ndim == 2 ? fused_bp_bytes(L) : 0) +
+                               (do_cd && cd_lookup_supported(mp, L, S) ? cd_lookup_workspace_bytes(mp, Bp, L) + 512 : 0);
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));
   int32_t* d_init = (int32_t*)carve((size_t)Bp * S * L * 4);

@@ -474,13 +474,12 @@ int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   if (wmax > kMaxWarps) wmax = kMaxWarps;
   if (wmax < 1) { set_error("fused build+DP: chain too long for shared memory"); return AUTODDL_EINVAL; }
   const int sms = fused_sm_count();
-  // warps per CTA (one CTA per SM): the fewest that reach the minimal number of rounds of chains per warp
-  const int rounds = (Bp + sms * wmax - 1) / (sms * wmax);
-  int W = (Bp + sms * rounds - 1) / (sms * rounds);
-  if (W < 4) W = Bp < 4 * sms ? (Bp + sms - 1) / sms : 4;
+  // one CTA per SM on every SM; warps per CTA: the fewest that reach the minimal number of rounds of chains per warp
+  const int grid = Bp < sms ? Bp : sms;
+  const int rounds = (Bp + grid * wmax - 1) / (grid * wmax);
+  int W = (Bp + grid * rounds - 1) / (grid * rounds);
   if (W > wmax) W = wmax;
   if (W < 1) W = 1;
-  const int grid = Bp < sms * W ? (Bp + W - 1) / W : sms;
   const size_t smem = fixed + (size_t)W * per_warp;
   ADL_CUDA_CHECK(cudaFuncSetAttribute(fused_chain36_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   fused_chain36_kernel<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy,
