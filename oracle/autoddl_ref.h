@@ -12,9 +12,10 @@
  *
  * Parity status (see DESIGN.md section 4 "Pins"):
  *   collectives (Table 2)        pinned  (hand values, identities)
- *   reshard path                pinned  (paper's 15 GB example, hand cell, symmetry)
- *   weight-gradient sync        pinned  (data-parallel closed form)
- *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours)
+ *   reshard path                pinned  (paper's 15 GB example, hand cells on divisible AND ragged dims:
+ *                                                  level order, message size before / after, scatter axis, fwd != bwd)
+ *   weight-gradient sync        pinned  (data-parallel closed form, ragged local weight by hand)
+ *   memory feasibility          PARITY UNPINNED (paper gives no formula; ours: hand value + boundaries)
  *   chain DP optimum (PAPER.md:225 exhaustive)     pinned  (brute force over K^L)
  *   coordinate descent          pinned by properties (1-opt, monotone, DP <= CD)
  *   folded factorisation space pinned  (equal, cell by cell, to the canonical signatures of the prime-
