@@ -198,7 +198,7 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   const int64_t K = mesh_num_sigs(mesh);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
   if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L);   // many starts: factors + best responses
-  if (mesh->ndim == 2) b += fused_bp_bytes(L);              // fused build + DP: back-pointers of the chains in flight
+  if (mesh->ndim == 2) b += fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256;   // fused kernel: back-pointers, strategies after sweep 1
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
   b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
   b += align_up((size_t)Bp * S * L * 4, 256) * 2;
@@ -246,7 +246,7 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
     }
     if ((rc = check_device())) return rc;
     return launch_build_dp_fused(d_layers, Bp, L, mp, nullptr, nullptr, nullptr, d_opt_cost, d_strategy, (uint8_t*)d_work,
-                                 nullptr, 0, nullptr, st);
+                                 nullptr, 0, nullptr, nullptr, st);
   }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
   if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
@@ -315,6 +315,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   size_t used = 0;
   int rc;
   bool cd_resume = false;
+  int32_t* d_cd_prev = nullptr;                             // strategies after sweep 1 when two sweeps were fused
   if (need_tables && !d_T && (do_cd || !fused)) {
     used = table_bytes(Bp, L, K);
     if (d_work == nullptr || work_bytes < used) {
@@ -328,11 +329,15 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
       set_error("search: workspace of %zu bytes needed, %zu given", used + fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
       return AUTODDL_EWORK;
     }
-    // the first CD sweep rides in the fused kernel (tiles are in shared memory there); the CD kernel resumes at sweep 2
+    // the first two CD sweeps ride in the fused kernel (the tile factors are in shared memory there); the CD kernel resumes
+    // at sweep 3.  The strategies after sweep 1 go to a workspace slice behind the back-pointers.
     static const bool no_cd_fuse = ADL_DEBUG_ENV("AUTODDL_NO_CD_FUSE");
     cd_resume = do_cd && !no_cd_fuse && fused_cd_sweep_supported(L, S);
+    const size_t s1_off = (used + fused_bp_bytes(L) + 255) / 256 * 256;
+    if (cd_resume && work_bytes >= s1_off + (size_t)Bp * S * L * 4) d_cd_prev = (int32_t*)(d_work + s1_off);
     if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used,
-                                    cd_resume ? d_init : nullptr, S, cd_resume ? d_cd_strategy : nullptr, st)))
+                                    cd_resume ? d_init : nullptr, S, cd_resume ? (d_cd_prev ? d_cd_prev : d_cd_strategy) : nullptr,
+                                    cd_resume && d_cd_prev ? d_cd_strategy : nullptr, st)))
       return rc;
   } else {
     const size_t bb = bp_bytes(Bp, L, K);
@@ -358,7 +363,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     if (d_work != nullptr && work_bytes >= need)
       return launch_cd_lookup(d_layers, Bp, L, mp, d_work + off, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
   }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3 && !mp.fold);
+  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3 && !mp.fold, d_cd_prev);
   return AUTODDL_OK;
 }
 
@@ -412,7 +417,8 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
 
   unsigned char* w = (unsigned char*)d_work;
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
-  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) + (mesh->ndim == 2 ? fused_bp_bytes(L) : 0) +
+  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) +
+                               (mesh->ndim == 2 ? fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256 : 0) +
                                (do_cd && cd_lookup_supported(mp, L, S) ? cd_lookup_workspace_bytes(mp, Bp, L) + 512 : 0);
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));

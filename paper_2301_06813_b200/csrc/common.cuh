@@ -74,7 +74,7 @@ bool fused_build_dp_supported(const MeshParams& mp, int32_t L);
 size_t fused_bp_bytes(int32_t L);
 int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
                           int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
-                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, cudaStream_t st);
+                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, int32_t* d_cd_s2, cudaStream_t st);
 bool fused_cd_sweep_supported(int32_t L, int32_t S);
 int launch_chain_dp(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, uint8_t* d_bp,
                     int64_t* d_opt_cost, int32_t* d_strategy, cudaStream_t st);
@@ -84,11 +84,13 @@ int launch_chain_dp_cluster(const int64_t* d_T, int32_t Bp, int32_t L, int64_t* 
 bool chain_dp_cluster_anyk_supported(int32_t K, int32_t L);
 int launch_chain_dp_cluster_anyk(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, int64_t* d_opt_cost,
                                  int32_t* d_strategy, cudaStream_t st);
-// resume: the first sweep has been done already (its result is in d_strategy); continue from sweep 2
+// resume: the first sweep (d_prev == NULL) or the first two sweeps (d_prev = the strategies after sweep 1) have been done
+// already and their result is in d_strategy; continue from there
 // sbp_rows: d_T was built by this library (identical rows per producer-signature class may be read through one row)
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init,
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
-                         int32_t* d_sweeps, cudaStream_t st, bool resume = false, bool sbp_rows = false);
+                         int32_t* d_sweeps, cudaStream_t st, bool resume = false, bool sbp_rows = false,
+                         const int32_t* d_prev = nullptr);
 // many starts per problem on library-built tables (K = 36, 216): factors -> best responses -> look-up sweeps (factors.cu)
 bool cd_lookup_supported(const MeshParams& mp, int32_t L, int32_t S);
 size_t cd_lookup_workspace_bytes(const MeshParams& mp, int32_t Bp, int32_t L);

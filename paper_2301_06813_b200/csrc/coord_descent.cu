@@ -32,9 +32,11 @@ __device__ __forceinline__ int64_t ldg_narrow(const int64_t* p) {
   return v;
 }
 
-// RESUME: the first sweep was run elsewhere (the fused build + DP kernel does it from the tiles in shared memory) and
-// its result is in `strategy`; a layer is dirty iff its right neighbour changed in that sweep (changed = differs from
-// `init`: a layer is touched once per sweep), the sweep count starts at 1, and nothing changed <=> finished.
+// RESUME: the first sweep -- or the first two (prev != NULL: the strategies after sweep 1) -- were run elsewhere (the fused
+// kernel does them from the tile factors in shared memory) and the result of the last one is in `strategy`.  A layer is
+// dirty iff its right neighbour changed in the last sweep done (a layer is touched once per sweep and sees its left
+// neighbour's new value); the sweep count starts at 1 or 2; a sweep that changed nothing ends the descent -- so if sweep 1
+// changed nothing the answer is its result with a count of 1, whatever was run after it.
 // SBPROWS: the tables were built by this library (autoddl_search, or d_T == NULL), so rows of a tile whose producer
 // signatures agree up to the per-level classes {0}, {1}, {3}, {2, 4, 5} are identical (signatures 2, 4, 5 all output P,
 // or are all invalid for ATTN: DESIGN.md R1): the column gather reads the class representative's row, and candidates
@@ -44,7 +46,7 @@ template <int KT, bool RESUME, bool SBPROWS>
 __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __restrict__ T, int Krt, int L, int S,
                                                            const int32_t* __restrict__ init, int max_sweeps,
                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
-                                                           int32_t* __restrict__ sweeps) {
+                                                           int32_t* __restrict__ sweeps, const int32_t* __restrict__ prev) {
   extern __shared__ __align__(16) unsigned char smem[];
   int32_t* s = reinterpret_cast<int32_t*>(smem);            // [L]
   uint8_t* dirty = reinterpret_cast<uint8_t*>(s + L);        // [L]
@@ -76,14 +78,23 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   int nsweeps = 0;
   bool resume_done = false;
   if (RESUME) {
-    bool any = false;
+    bool any1 = false, any2 = false;                       // sweep 1 / sweep 2 changed something
     for (int l = lane; l < L; l += 32) {
-      s[l] = strategy[ps * L + l];
-      any |= s[l] != init[ps * L + l];
-      dirty[l] = (l + 1 < L && strategy[ps * L + l + 1] != init[ps * L + l + 1]) ? 1 : 0;
+      const int s0 = init[ps * L + l], s1 = prev ? prev[ps * L + l] : strategy[ps * L + l];
+      any1 |= s1 != s0;
+      if (prev) any2 |= strategy[ps * L + l] != s1;
     }
-    nsweeps = 1;
-    resume_done = !__any_sync(0xffffffffu, any) || max_sweeps <= 1;
+    any1 = __any_sync(0xffffffffu, any1);
+    any2 = __any_sync(0xffffffffu, any2);
+    const bool two = prev != nullptr && any1 && max_sweeps > 1;     // sweep 2 counts
+    for (int l = lane; l < L; l += 32) {
+      const int32_t* last = two || !prev ? strategy : prev;         // the state the descent stands at
+      const int32_t* before = two ? prev : init;                    // the state one sweep earlier
+      s[l] = last[ps * L + l];
+      dirty[l] = (l + 1 < L && last[ps * L + l + 1] != before[ps * L + l + 1]) ? 1 : 0;
+    }
+    nsweeps = two ? 2 : 1;
+    resume_done = !any1 || max_sweeps <= 1 || (two && (!any2 || max_sweeps <= 2));
   } else {
     for (int l = lane; l < L; l += 32) {
       s[l] = init[ps * L + l];
@@ -188,14 +199,14 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
 
 template <int K, bool RESUME, bool SBPROWS>
 int launch_k(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
-             int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+             int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st, const int32_t* d_prev = nullptr) {
   const size_t smem = ((size_t)L * 5 + 15) / 16 * 16;
   if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
   if (smem > 48 * 1024)
     ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_kernel<K, RESUME, SBPROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int64_t nb = (int64_t)Bp * S;
   if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
-  coord_descent_kernel<K, RESUME, SBPROWS><<<(unsigned)nb, 32, smem, st>>>(d_T, Krt, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps);
+  coord_descent_kernel<K, RESUME, SBPROWS><<<(unsigned)nb, 32, smem, st>>>(d_T, Krt, L, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps, d_prev);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -205,8 +216,8 @@ int launch_k(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, 
 
 int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                          int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st,
-                         bool resume, bool sbp_rows) {
-#define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
+                         bool resume, bool sbp_rows, const int32_t* d_prev) {
+#define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, d_prev)
   if (resume) {
     if (K == 36) return sbp_rows ? ADL_CD(36, true, true) : ADL_CD(36, true, false);
     set_error("coord_descent: resume mode exists for K = 36 only");

@@ -40,13 +40,14 @@ struct alignas(16) Rec64 {                                 // byte image of auto
 };
 static_assert(sizeof(Rec64) == sizeof(autoddl_layer), "Rec64 mirrors autoddl_layer");
 
+template <int NB>                                          // NB = 2: the previous layer's factors stay (second CD sweep)
 struct alignas(16) WarpShared {
   int64_t Q[5][4];                                        // M, Kd, N, in_rows, in_cols  x  level subset
   int64_t TAB[2 * FD * FSTRIDE];                          // CG[D][NC+1] then CA[D][NC+1]; [..][NC] = 0
   int64_t WAR[FD][FNC];
   int64_t locW[FNC], locO[FNC];
-  alignas(16) int64_t VP[FK];
-  int64_t Esym[FES * FES];                                // R[a][b], then symmetrised in place; row / column 16 stay 0
+  alignas(16) int64_t VP[NB][FK];                         // layer l in buffer l & (NB - 1)
+  int64_t Esym[NB][FES * FES];                             // R[a][b], then symmetrised in place; row / column 16 stay 0
   alignas(16) int64_t f[2][FK];
   Rec64 rec[8];                                           // ring of layer records, fetched four at a time
 };
@@ -77,21 +78,32 @@ __device__ __forceinline__ void warp_argmin64(int64_t& bv, int& bi) {
   }
 }
 
+template <int NB>
 __global__ void __launch_bounds__(896, 1)
 fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, MeshParams mp,
                      int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
                      int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
-                     const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1, int per_warp_bytes) {
+                     const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1, int32_t* __restrict__ cd_s2,
+                     int per_warp_bytes) {
   extern __shared__ __align__(128) unsigned char fsm_raw[];
   CtaShared& cs = *reinterpret_cast<CtaShared*>(fsm_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
   unsigned char* wbase = fsm_raw + ((sizeof(CtaShared) + 127) & ~(size_t)127) + (size_t)warp * per_warp_bytes;
-  WarpShared& ws = *reinterpret_cast<WarpShared*>(wbase);
-  // CD only: row stash [cd_S][36] int64, then the strategies of the chain's starts [cd_S][L]; then the back-pointers
-  int64_t* cd_stash = reinterpret_cast<int64_t*>(wbase + sizeof(WarpShared));
-  uint8_t* cd_s = wbase + sizeof(WarpShared) + (cd_init ? (size_t)cd_S * FK * 8 : 0);
-  const size_t cd_bytes = cd_init ? (((size_t)cd_S * L + 15) & ~(size_t)15) : 0;
+  using WS = WarpShared<NB>;
+  WS& ws = *reinterpret_cast<WS*>(wbase);
+  // CD only: the row stashes of the two sweeps [2][cd_S][36] int64, then the strategies of the chain's starts after
+  // sweep 1 and sweep 2 [2][cd_S][L] bytes; then the back-pointers [L][K] (or a workspace slice: bp_glob)
+  int64_t* cd_stash = reinterpret_cast<int64_t*>(wbase + sizeof(WS));
+  int64_t* cd_stash2 = cd_stash + (size_t)cd_S * FK;
+  uint8_t* cd_s = wbase + sizeof(WS) + (cd_init ? (size_t)2 * cd_S * FK * 8 : 0);
+  uint8_t* cd_t = cd_s + (size_t)cd_S * L;
+  const size_t cd_bytes = cd_init ? (((size_t)2 * cd_S * L + 15) & ~(size_t)15) : 0;
   uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
+#ifdef ADL_EXP_NO_SWEEP2
+  const bool two = false;
+#else
+  const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well
+#endif
 
   // ---- once per CTA: facts per (layer kind, signature) -----------------------------------------------------------
   fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
@@ -111,7 +123,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   __syncthreads();
 
   // ---- once per warp: tile-invariant roles of this lane ---------------------------------------------------------
-  for (int x = lane; x < FES * FES; x += 32) ws.Esym[x] = 0;
+  for (int x = lane; x < NB * FES * FES; x += 32) (&ws.Esym[0][0])[x] = 0;
   if (lane < 2 * FD) ws.TAB[lane * FSTRIDE + FNC] = 0;
   // step 1: lane (x, m) for lane < 20
   const int q_x = lane >> 2, q_m = lane & 3;
@@ -141,7 +153,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     };
     stage4(0);
     stage4(4);
-    int kind_prev = 0;
+    int kind_prev = 0, kind_pp = 0;                          // kinds of layers l - 1 and l - 2
     const bool cd = cd_init != nullptr;
     if (cd) {
       for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)p * cd_S * L + x];
@@ -158,6 +170,10 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       const int kind = rec.kind;
       if (l == 0) kind_prev = kind;                          // no producer: any valid kind (E(0) = 0)
       const size_t tile = (size_t)p * L + l;
+      int64_t* const Ecur = ws.Esym[l & (NB - 1)];
+      int64_t* const VPc = ws.VP[l & (NB - 1)];
+      const int64_t* const Eprv = ws.Esym[(l & (NB - 1)) ^ (NB - 1)];   // layer l - 1 (NB = 2)
+      const int64_t* const VPp = ws.VP[(l & (NB - 1)) ^ (NB - 1)];
 
       // ---- 1. Q[x][m] = ceil(extent x / product of the levels in m) -------------------------------------------------
       if (lane < 20) ws.Q[q_x][q_m] = cdiv_magic(rec.X[q_x], q_sub, q_magic);
@@ -204,7 +220,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           }
           const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc &&
                           (mp.mem_cap == 0 || mem <= cap_layer);
-          ws.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
+          VPc[j] = v + (ok ? 0 : AUTODDL_PEN);
           if (node) node[tile * FK + j] = v;
           if (mask) mask[tile * FK + j] = ok ? 1 : 0;
         }
@@ -217,19 +233,19 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
             const uint32_t lo = cs.slot_lo[k][lane];
-            ws.Esym[sy[k] & 511] = ws.TAB[lo & 63] + ws.TAB[lo >> 6 & 63] + ws.TAB[lo >> 12 & 63] + ws.TAB[lo >> 18 & 63] +
+            Ecur[sy[k] & 511] = ws.TAB[lo & 63] + ws.TAB[lo >> 6 & 63] + ws.TAB[lo >> 12 & 63] + ws.TAB[lo >> 18 & 63] +
                                    ws.TAB[lo >> 24 & 63] + ws.TAB[sy[k] >> 26];
           }
           __syncwarp();
           int64_t es[8];                                     // forward leg + backward leg, in place: reads, then writes
 #pragma unroll
-          for (int k = 0; k < 8; ++k) es[k] = ws.Esym[sy[k] & 511] + ws.Esym[sy[k] >> 9 & 511];
+          for (int k = 0; k < 8; ++k) es[k] = Ecur[sy[k] & 511] + Ecur[sy[k] >> 9 & 511];
           __syncwarp();
 #pragma unroll
-          for (int k = 0; k < 8; ++k) ws.Esym[sy[k] & 511] = es[k];
+          for (int k = 0; k < 8; ++k) Ecur[sy[k] & 511] = es[k];
         } else {
 #pragma unroll
-          for (int k = 0; k < 8; ++k) ws.Esym[sy[k] & 511] = 0;
+          for (int k = 0; k < 8; ++k) Ecur[sy[k] & 511] = 0;
         }
       }
       __syncwarp();
@@ -245,7 +261,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         const uint16_t* aok = cs.aoff[kind_prev];
         {
           const int pc = lane & 15, h = lane >> 4;
-          const longlong2 vp = *reinterpret_cast<const longlong2*>(&ws.VP[2 * pc]);
+          const longlong2 vp = *reinterpret_cast<const longlong2*>(&VPc[2 * pc]);
           const uint32_t bb = *reinterpret_cast<const uint16_t*>(&cs.bcls[kind][2 * pc]);
           const int b0 = bb & 255, b1 = bb >> 8;
           int64_t* o = out + (3 * h) * FK + 2 * pc;
@@ -255,7 +271,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
 #pragma unroll
             for (int t = 0; t < 3; ++t) {
               const int ao = aok[r0 * 6 + 3 * h + t];
-              const longlong2 v = make_longlong2(vp.x + ws.Esym[ao + b0], vp.y + ws.Esym[ao + b1]);
+              const longlong2 v = make_longlong2(vp.x + Ecur[ao + b0], vp.y + Ecur[ao + b1]);
               __stcs(reinterpret_cast<longlong2*>(o + (r0 * 6 + t) * FK), v);
               if (c0 == 3) {
                 __stcs(reinterpret_cast<longlong2*>(o + (4 * 6 + t) * FK), v);
@@ -265,14 +281,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           }
         }
         {
-          const longlong2 vpa = *reinterpret_cast<const longlong2*>(&ws.VP[32]);
-          const longlong2 vpb = *reinterpret_cast<const longlong2*>(&ws.VP[34]);
+          const longlong2 vpa = *reinterpret_cast<const longlong2*>(&VPc[32]);
+          const longlong2 vpb = *reinterpret_cast<const longlong2*>(&VPc[34]);
           const uint32_t bb = *reinterpret_cast<const uint32_t*>(&cs.bcls[kind][32]);
 #pragma unroll
           for (int i0 = 0; i0 < 64; i0 += 32) {
             const int i = i0 + lane;
             if (i < FK) {
-              const int64_t* er = ws.Esym + aok[i];
+              const int64_t* er = Ecur + aok[i];
               __stcs(reinterpret_cast<longlong2*>(out + i * FK + 32), make_longlong2(vpa.x + er[bb & 255], vpa.y + er[bb >> 8 & 255]));
               __stcs(reinterpret_cast<longlong2*>(out + i * FK + 34), make_longlong2(vpb.x + er[bb >> 16 & 255], vpb.y + er[bb >> 24]));
             }
@@ -283,7 +299,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       // ---- 5. chain DP (R9): f_l[j] = VP[j] + min_i f_{l-1}[i] + Esym[A(i)][B(j)], smallest i on ties -----------------
       int64_t* fn = ws.f[cur ^ 1];
       if (l == 0) {
-        for (int j = lane; j < FK; j += 32) fn[j] = ws.VP[j];            // f_0[j] = T[0][0][j]
+        for (int j = lane; j < FK; j += 32) fn[j] = VPc[j];            // f_0[j] = T[0][0][j]
       } else {
         const int64_t* f = ws.f[cur];
         const uint16_t* ao = cs.aoff[kind_prev] + 18 * dp_h;
@@ -294,7 +310,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         for (int part = 0; part < 3; ++part) {             // three independent chains of six rows, merged in row order
           int64_t tv[6], fv[6];
 #pragma unroll
-          for (int r = 0; r < 6; ++r) tv[r] = ws.Esym[ao[6 * part + r] + dp_b];
+          for (int r = 0; r < 6; ++r) tv[r] = Ecur[ao[6 * part + r] + dp_b];
 #pragma unroll
           for (int r = 0; r < 6; r += 2) {
             const longlong2 f2 = *reinterpret_cast<const longlong2*>(fh + 6 * part + r);
@@ -341,62 +357,119 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           int ha = __shfl_sync(0xffffffffu, a, bj & 15);
           if (bj == FNS) { hb = h16; ha = a16; }
           if (j < FK) {
-            fn[j] = ws.VP[j] + hb;
+            fn[j] = VPc[j] + hb;
             bp[(size_t)l * FK + j] = (uint8_t)ha;
           }
         }
       }
       cur ^= 1;
 
-      // ---- 6. first Coordinate Descent sweep (R10) of every start ------------------------------------------------------
+      // ---- 6. Coordinate Descent (R10): sweep 1 of layer l-1 and, trailing it by one layer, sweep 2 of layer l-2 --------------
+      // Sweep 2's update of layer m needs the row T[m][s2_{m-1}][.] (stashed at tile m+1 from the previous layer's
+      // factors) and the column T[m+1][.][s1_{m+1}], whose s1_{m+1} is final once sweep 1 has passed layer m+1: at tile
+      // m+2, with tile m+1's Esym still in the other buffer.  Every layer is re-evaluated in sweep 2: the update of a
+      // clean layer returns the value it has, so the result is that of the plain algorithm (61 of the 64 layers of a
+      // config-4 chain change in sweep 1: sweep 2 would re-evaluate them all anyway).
       if (cd) {
         __syncwarp();
         for (int st = 0; st < cd_S; ++st) {
-          {
-            uint8_t* sv = cd_s + (size_t)st * L;
-            int64_t* stash = cd_stash + st * FK;             // T[l][s_{l-1}][.] of this start, for the next layer's update
-            if (l > 0) {                                     // update of layer l-1: row stashed, column from this tile
-              const int right = sv[l];
-              const int bright = cs.bcls[kind][right];
-              int64_t bv = INT64_MAX;
-              int bi = FK;
+          uint8_t* sv = cd_s + (size_t)st * L;               // after sweep 1 (starts as the initial strategy)
+          uint8_t* tv = cd_t + (size_t)st * L;               // after sweep 2
+          int64_t* stash = cd_stash + st * FK;               // T[l][s1_{l-1}][.]: row of sweep 1's next update
+          int64_t* stash2 = cd_stash2 + st * FK;             // T[l-1][s2_{l-2}][.]: row of sweep 2's next update
+          if (l > 0) {                                       // sweep 1, layer l-1: row stashed, column from this tile
+            const int bright = cs.bcls[kind][sv[l]];
+            int64_t bv = INT64_MAX;
+            int bi = FK;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const int c = 32 * q + lane;
+              if (c < FK) {
+                const int64_t g = stash[c] + Ecur[cs.aoff[kind_prev][c] + bright];
+                if (g < bv) { bv = g; bi = c; }
+              }
+            }
+            warp_argmin64(bv, bi);
+            if (lane == 0) sv[l - 1] = (uint8_t)bi;
+            __syncwarp();
+          }
+          if (two && l > 1) {                                // sweep 2, layer l-2: column from tile l-1 given s1_{l-1}
+            const int bright = cs.bcls[kind_prev][sv[l - 1]];
+            int64_t bv = INT64_MAX;
+            int bi = FK;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const int c = 32 * q + lane;
+              if (c < FK) {
+                const int64_t g = stash2[c] + Eprv[cs.aoff[kind_pp][c] + bright];
+                if (g < bv) { bv = g; bi = c; }
+              }
+            }
+            warp_argmin64(bv, bi);
+            if (lane == 0) tv[l - 2] = (uint8_t)bi;
+            __syncwarp();
+          }
+          {                                                  // rows for the next updates (s_{-1} := 0; E(0) = 0 whatever the row)
+            const int aleft = cs.aoff[kind_prev][l > 0 ? sv[l - 1] : 0];
+            const int aleft2 = cs.aoff[kind_pp][l > 1 ? tv[l - 2] : 0];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const int c = 32 * q + lane;
+              if (c < FK) {
+                stash[c] = VPc[c] + Ecur[aleft + cs.bcls[kind][c]];
+                if (two && l > 0) stash2[c] = VPp[c] + Eprv[aleft2 + cs.bcls[kind_prev][c]];
+              }
+            }
+            __syncwarp();
+          }
+          if (l == L - 1) {                                  // the chain ends: the updates that have no later tile
+            int64_t bv = INT64_MAX;
+            int bi = FK;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {                    // sweep 1, last layer: no right neighbour
+              const int c = 32 * q + lane;
+              if (c < FK && stash[c] < bv) { bv = stash[c]; bi = c; }
+            }
+            warp_argmin64(bv, bi);
+            if (lane == 0) sv[l] = (uint8_t)bi;
+            __syncwarp();
+            if (two) {
+              if (l > 0) {                                   // sweep 2, layer L-2: column from this (last) tile given s1_{L-1}
+                const int bright = cs.bcls[kind][sv[l]];
+                bv = INT64_MAX;
+                bi = FK;
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                  const int c = 32 * q + lane;
+                  if (c < FK) {
+                    const int64_t g = stash2[c] + Ecur[cs.aoff[kind_prev][c] + bright];
+                    if (g < bv) { bv = g; bi = c; }
+                  }
+                }
+                warp_argmin64(bv, bi);
+                if (lane == 0) tv[l - 1] = (uint8_t)bi;
+                __syncwarp();
+              }
+              const int aleft2 = cs.aoff[kind_prev][l > 0 ? tv[l - 1] : 0];   // sweep 2, last layer
+              bv = INT64_MAX;
+              bi = FK;
 #pragma unroll
               for (int q = 0; q < 2; ++q) {
                 const int c = 32 * q + lane;
                 if (c < FK) {
-                  const int64_t g = stash[c] + ws.Esym[cs.aoff[kind_prev][c] + bright];
+                  const int64_t g = VPc[c] + Ecur[aleft2 + cs.bcls[kind][c]];
                   if (g < bv) { bv = g; bi = c; }
                 }
               }
               warp_argmin64(bv, bi);
-              if (lane == 0) sv[l - 1] = (uint8_t)bi;
-              __syncwarp();
-            }
-            // row T[l][s_{l-1}][.] for the update of layer l (s_{-1} := 0; E(0) = 0 whatever the row)
-            const int left = l > 0 ? sv[l - 1] : 0;
-            const int aleft = cs.aoff[kind_prev][left];
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-              const int c = 32 * q + lane;
-              if (c < FK) stash[c] = ws.VP[c] + ws.Esym[aleft + cs.bcls[kind][c]];
-            }
-            __syncwarp();
-            if (l == L - 1) {                                // last layer: no right neighbour
-              int64_t bv = INT64_MAX;
-              int bi = FK;
-#pragma unroll
-              for (int q = 0; q < 2; ++q) {
-                const int c = 32 * q + lane;
-                if (c < FK && stash[c] < bv) { bv = stash[c]; bi = c; }
-              }
-              warp_argmin64(bv, bi);
-              if (lane == 0) sv[l] = (uint8_t)bi;
+              if (lane == 0) tv[l] = (uint8_t)bi;
               __syncwarp();
             }
           }
         }
       }
       __syncwarp();
+      kind_pp = kind_prev;
       kind_prev = kind;
     }
 
@@ -410,18 +483,50 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         if (v < bv) { bv = v; bi = 32 + lane; }
       }
       warp_argmin64(bv, bi);
+      // back-pointers in the workspace: pull the chain's L x 36 bytes into the (now free) Esym buffers first, so that
+      // the dependent walk reads shared memory
+      const uint8_t* bw = bp;
+      __syncwarp();
+      if (bp_glob && (size_t)L * FK <= sizeof(ws.Esym)) {
+        uint8_t* scratch = reinterpret_cast<uint8_t*>(&ws.Esym[0][0]);
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(bp);       // L * 36 bytes: a multiple of 4, slices 4-byte aligned
+        uint32_t* dst = reinterpret_cast<uint32_t*>(scratch);
+        const int n4 = L * FK / 4;
+        for (int x0 = 0; x0 < n4; x0 += 32 * 8) {                          // eight independent loads in flight per lane
+          uint32_t v[8];
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const int x = x0 + 32 * q + lane;
+            v[q] = x < n4 ? __ldcg(src + x) : 0;
+          }
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const int x = x0 + 32 * q + lane;
+            if (x < n4) dst[x] = v[q];
+          }
+        }
+        __syncwarp();
+        bw = scratch;
+      }
       if (lane == 0) {
         int32_t* sp = strategy + (size_t)p * L;
         opt_cost[p] = bv;
         int sidx = bi;
         sp[L - 1] = sidx;
         for (int ll = L - 1; ll >= 1; --ll) {
-          sidx = bp[(size_t)ll * FK + sidx];
+          sidx = bw[(size_t)ll * FK + sidx];
           sp[ll - 1] = sidx;
         }
       }
+      __syncwarp();
+      if (bw != bp) {                                      // the next chain expects zero borders in the Esym buffers
+        for (int x = lane; x < NB * FES * FES; x += 32) (&ws.Esym[0][0])[x] = 0;
+      }
       if (cd) {
-        for (int x = lane; x < cd_S * L; x += 32) cd_s1[(size_t)p * cd_S * L + x] = cd_s[x];
+        for (int x = lane; x < cd_S * L; x += 32) {
+          cd_s1[(size_t)p * cd_S * L + x] = cd_s[x];
+          if (two) cd_s2[(size_t)p * cd_S * L + x] = cd_t[x];
+        }
       }
       __syncwarp();
     }
@@ -435,55 +540,61 @@ int fused_sm_count() {
 }
 
 constexpr int kMaxWarps = 28;
-constexpr size_t kSmemBudget = 224 * 1024;
+constexpr size_t kSmemBudget = 226 * 1024;
 
-// back-pointers [L][36] of the chain a warp has in flight: in its shared memory when they fit, else in the workspace
-size_t warp_bytes(int32_t L, int32_t S, bool bp_smem) {
-  const size_t cd = S > 0 ? (((size_t)S * L + 15) & ~(size_t)15) + (size_t)S * FK * 8 : 0;
-  return (sizeof(WarpShared) + cd + (bp_smem ? (size_t)L * FK : 0) + 127) & ~(size_t)127;
+// per-warp shared memory: tile factors, DP state, (CD) row stashes and strategies of two sweeps, (optionally) back-pointers
+size_t warp_bytes(int32_t L, int32_t S, bool bp_smem, bool two = true) {
+  const size_t cd = S > 0 ? (((size_t)2 * S * L + 15) & ~(size_t)15) + (size_t)2 * S * FK * 8 : 0;
+  return ((two ? sizeof(WarpShared<2>) : sizeof(WarpShared<1>)) + cd + (bp_smem ? (size_t)L * FK : 0) + 127) & ~(size_t)127;
 }
-bool bp_fits_smem(int32_t L, int32_t S) { return 8 * warp_bytes(L, S, true) + sizeof(CtaShared) + 128 <= kSmemBudget; }
+size_t fixed_bytes() { return (sizeof(CtaShared) + 127) & ~(size_t)127; }
 
 }  // namespace
 
 bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim == 2 && !mp.fold && L >= 1; }
 
-// largest S for which the first CD sweep rides in the fused kernel (one row stash of two registers per start and lane)
-bool fused_cd_sweep_supported(int32_t L, int32_t S) { return S >= 1 && S <= kMaxFusedStarts && (int64_t)S * L <= 8192; }
+// largest S for which the first two CD sweeps ride in the fused kernel (row stashes and strategies in shared memory)
+bool fused_cd_sweep_supported(int32_t L, int32_t S) {
+  return S >= 1 && S <= kMaxFusedStarts && fixed_bytes() + 4 * warp_bytes(L, S, false, true) <= kSmemBudget;
+}
 
+// workspace for the back-pointers [L][36] of the chains in flight (one slice per warp) when they do not fit beside the
+// warps' shared memory
 size_t fused_bp_bytes(int32_t L) {
   static const int sms = fused_sm_count();                 // host-only query, cached
-  if (bp_fits_smem(L, kMaxFusedStarts)) return 256;
   return ((size_t)sms * kMaxWarps * L * FK + 255) / 256 * 256 + 256;
 }
 
 // Fused (a1) + (a2) for K = 36: tables (d_T may be NULL: no table is written) and the chain DP in one kernel, plus the
-// first CD sweep of S <= 4 starts per chain.  d_bp: fused_bp_bytes(L) of workspace (back-pointers of very long chains).
+// first two CD sweeps of S <= 8 starts per chain (d_cd_s1 / d_cd_s2: strategies after sweep 1 / sweep 2; d_cd_s2 NULL:
+// one sweep).  d_bp: fused_bp_bytes(L) of workspace.
 int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_T,
                           int64_t* d_node, uint8_t* d_mask, int64_t* d_opt_cost, int32_t* d_strategy, uint8_t* d_bp,
-                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, cudaStream_t st) {
+                          const int32_t* d_cd_init, int32_t S, int32_t* d_cd_s1, int32_t* d_cd_s2, cudaStream_t st) {
   if ((int64_t)Bp * L > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   if (!fused_build_dp_supported(mp, L)) { set_error("fused build+DP needs a 2-level mesh"); return AUTODDL_EINVAL; }
   if (d_cd_init && (!fused_cd_sweep_supported(L, S) || d_cd_s1 == nullptr)) { set_error("fused CD sweep: too many starts"); return AUTODDL_EINVAL; }
   const int cdS = d_cd_init ? S : 0;
-  const bool bp_smem = bp_fits_smem(L, cdS);
-  if (!bp_smem && d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
-  const size_t per_warp = warp_bytes(L, cdS, bp_smem);
-  const size_t fixed = ((sizeof(CtaShared) + 127) & ~(size_t)127);
-  int wmax = (int)((kSmemBudget - fixed) / per_warp);
-  if (wmax > kMaxWarps) wmax = kMaxWarps;
-  if (wmax < 1) { set_error("fused build+DP: chain too long for shared memory"); return AUTODDL_EINVAL; }
+  const bool two = d_cd_init != nullptr && d_cd_s2 != nullptr;        // two CD sweeps: the previous layer's factors stay
   const int sms = fused_sm_count();
+  const size_t fixed = fixed_bytes();
   // one CTA per SM on every SM; warps per CTA: the fewest that reach the minimal number of rounds of chains per warp
   const int grid = Bp < sms ? Bp : sms;
+  int wmax = (int)((kSmemBudget - fixed) / warp_bytes(L, cdS, false, two));
+  if (wmax > kMaxWarps) wmax = kMaxWarps;
+  if (wmax < 1) { set_error("fused build+DP: chain too long for shared memory"); return AUTODDL_EINVAL; }
   const int rounds = (Bp + grid * wmax - 1) / (grid * wmax);
   int W = (Bp + grid * rounds - 1) / (grid * rounds);
   if (W > wmax) W = wmax;
   if (W < 1) W = 1;
+  const bool bp_smem = fixed + (size_t)W * warp_bytes(L, cdS, true, two) <= kSmemBudget;   // else a workspace slice per warp
+  if (!bp_smem && d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
+  const size_t per_warp = warp_bytes(L, cdS, bp_smem, two);
   const size_t smem = fixed + (size_t)W * per_warp;
-  ADL_CUDA_CHECK(cudaFuncSetAttribute(fused_chain36_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  fused_chain36_kernel<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy,
-                                                   bp_smem ? nullptr : d_bp, d_cd_init, cdS, d_cd_s1, (int)per_warp);
+  auto kern = two ? fused_chain36_kernel<2> : fused_chain36_kernel<1>;
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, bp_smem ? nullptr : d_bp,
+                                   d_cd_init, cdS, d_cd_s1, two ? d_cd_s2 : nullptr, (int)per_warp);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
