@@ -197,7 +197,7 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   if (validate_mesh_net(mesh, nullptr, &mp) || Bp < 1 || L < 1 || S < 0) return 0;
   const int64_t K = mesh_num_sigs(mesh);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
-  if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L);   // many starts: factors + best responses
+  if (cd_lookup_supported(mp, L, S)) b += factors_bytes(mp, Bp, L) + cd_lookup_workspace_bytes(mp, Bp, L) + 256;   // many starts: factors, best responses
   if (mesh->ndim == 2) b += fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256;   // fused kernel: back-pointers, strategies after sweep 1
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
   b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
@@ -280,13 +280,15 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   if (!d_T && cd_lookup_supported(mp, L, S)) {
     // many starts on library-built tables: no K x K table at all (factors -> best responses -> look-up sweeps)
     ADL_REQUIRE(d_layers != nullptr && net != nullptr, "d_T is NULL and no layers / net given");
-    const size_t need = cd_lookup_workspace_bytes(mp, Bp, L);
+    const size_t fbytes = factors_bytes(mp, Bp, L), need = fbytes + cd_lookup_workspace_bytes(mp, Bp, L);
     if (d_work == nullptr || work_bytes < need) {
       set_error("coord_descent: workspace of %zu bytes needed, %zu given", need, d_work ? work_bytes : (size_t)0);
       return AUTODDL_EWORK;
     }
     if ((rc = check_device())) return rc;
-    return launch_cd_lookup(d_layers, Bp, L, mp, d_work, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+    if ((rc = launch_build_factors(d_layers, Bp, L, mp, (int64_t*)d_work, st))) return rc;
+    return launch_cd_lookup((const int64_t*)d_work, Bp, L, mp, (unsigned char*)d_work + fbytes, d_init, S, max_sweeps, d_cost,
+                            d_strategy, d_sweeps, st);
   }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K);
   if (tb > 0 && (d_work == nullptr || work_bytes < tb)) {
@@ -311,20 +313,18 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   const bool do_cd = d_init != nullptr;
   static const bool no_fuse = ADL_DEBUG_ENV("AUTODDL_NO_FUSE");         // debug builds only: three separate kernels
   const bool fused = !no_fuse && Bp >= kFusedMinChains && fused_build_dp_supported(mp, L);
-  const bool need_tables = do_cd || !fused || d_T != nullptr || d_node != nullptr || d_mask != nullptr;
-  size_t used = 0;
   int rc;
-  bool cd_resume = false;
-  int32_t* d_cd_prev = nullptr;                             // strategies after sweep 1 when two sweeps were fused
-  if (need_tables && !d_T && (do_cd || !fused)) {
-    used = table_bytes(Bp, L, K);
-    if (d_work == nullptr || work_bytes < used) {
-      set_error("search: workspace of %zu bytes needed for the tables, %zu given", used, d_work ? work_bytes : (size_t)0);
-      return AUTODDL_EWORK;
-    }
-    d_T = (int64_t*)d_work;
-  }
   if (fused) {
+    // ---- many chains on a two-level mesh: ONE kernel for tables + DP + the first two CD sweeps -----------------------------
+    size_t used = 0;
+    if (!d_T && do_cd) {                                    // the CD kernel that resumes reads the tables: keep them in d_work
+      used = table_bytes(Bp, L, K);
+      if (d_work == nullptr || work_bytes < used) {
+        set_error("search: workspace of %zu bytes needed for the tables, %zu given", used, d_work ? work_bytes : (size_t)0);
+        return AUTODDL_EWORK;
+      }
+      d_T = (int64_t*)d_work;
+    }
     if (d_work == nullptr || work_bytes < used + fused_bp_bytes(L)) {
       set_error("search: workspace of %zu bytes needed, %zu given", used + fused_bp_bytes(L), d_work ? work_bytes : (size_t)0);
       return AUTODDL_EWORK;
@@ -332,39 +332,50 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     // the first two CD sweeps ride in the fused kernel (the tile factors are in shared memory there); the CD kernel resumes
     // at sweep 3.  The strategies after sweep 1 go to a workspace slice behind the back-pointers.
     static const bool no_cd_fuse = ADL_DEBUG_ENV("AUTODDL_NO_CD_FUSE");
-    cd_resume = do_cd && !no_cd_fuse && fused_cd_sweep_supported(L, S);
+    const bool cd_resume = do_cd && !no_cd_fuse && fused_cd_sweep_supported(L, S);
+    int32_t* d_cd_prev = nullptr;                           // strategies after sweep 1 when two sweeps were fused
     const size_t s1_off = (used + fused_bp_bytes(L) + 255) / 256 * 256;
     if (cd_resume && work_bytes >= s1_off + (size_t)Bp * S * L * 4) d_cd_prev = (int32_t*)(d_work + s1_off);
     if ((rc = launch_build_dp_fused(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, d_work + used,
                                     cd_resume ? d_init : nullptr, S, cd_resume ? (d_cd_prev ? d_cd_prev : d_cd_strategy) : nullptr,
                                     cd_resume && d_cd_prev ? d_cd_strategy : nullptr, st)))
       return rc;
-  } else {
-    const size_t bb = bp_bytes(Bp, L, K);
-    if (bb && (d_work == nullptr || work_bytes < used + bb)) {
-      set_error("search: workspace of %zu bytes needed, %zu given", used + bb, d_work ? work_bytes : (size_t)0);
-      return AUTODDL_EWORK;
+    if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }   // profiling hook: tables + DP done, CD kernel not yet started
+    if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
+    if (!do_cd) return AUTODDL_OK;
+    if (!cd_resume && cd_lookup_supported(mp, L, S)) {      // many starts per chain: best-response look-ups on the factors
+      const size_t off = s1_off, fbytes = factors_bytes(mp, Bp, L);
+      if (work_bytes >= off + fbytes + cd_lookup_workspace_bytes(mp, Bp, L)) {
+        if ((rc = launch_build_factors(d_layers, Bp, L, mp, (int64_t*)(d_work + off), st))) return rc;
+        return launch_cd_lookup((const int64_t*)(d_work + off), Bp, L, mp, d_work + off + fbytes, d_init, S, max_sweeps, d_cd_cost,
+                                d_cd_strategy, d_cd_sweeps, st);
+      }
     }
-    if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
-    if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + used : nullptr, d_opt_cost, d_strategy, st))) return rc;
+    return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, true, d_cd_prev);
   }
-  if (g_mark) {                                             // profiling hook: tables + DP done, CD not yet started
-    cudaEventRecord(g_mark, st);
-    g_mark = nullptr;
+
+  // ---- few chains, or another mesh: separate kernels.  The DP reads the K x K tables; CD from >= 32 starts on two / three
+  // mesh levels runs on the factors and their best-response tables instead (no table gather).
+  const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
+  if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
+    set_error("search: workspace of %zu bytes needed, %zu given", tb + bb, d_work ? work_bytes : (size_t)0);
+    return AUTODDL_EWORK;
   }
-  if (g_dp_done) {
-    cudaEventRecord(g_dp_done, st);
-    g_dp_done = nullptr;
+  if (!d_T) d_T = (int64_t*)d_work;
+  if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
+  if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + tb : nullptr, d_opt_cost, d_strategy, st))) return rc;
+  if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
+  if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
+  if (!do_cd) return AUTODDL_OK;
+  if (cd_lookup_supported(mp, L, S)) {
+    const size_t off = align_up(tb + bb, 256), fbytes = factors_bytes(mp, Bp, L);
+    if (work_bytes >= off + fbytes + cd_lookup_workspace_bytes(mp, Bp, L)) {
+      if ((rc = launch_build_factors(d_layers, Bp, L, mp, (int64_t*)(d_work + off), st))) return rc;
+      return launch_cd_lookup((const int64_t*)(d_work + off), Bp, L, mp, d_work + off + fbytes, d_init, S, max_sweeps, d_cd_cost,
+                              d_cd_strategy, d_cd_sweeps, st);
+    }
   }
-  if (do_cd && !cd_resume && cd_lookup_supported(mp, L, S)) {
-    // many starts per problem: best-response look-ups on the factors instead of gathers on the K x K tables
-    const size_t off = (used + (fused ? fused_bp_bytes(L) : bp_bytes(Bp, L, K)) + 255) / 256 * 256;
-    const size_t need = off + cd_lookup_workspace_bytes(mp, Bp, L);
-    if (d_work != nullptr && work_bytes >= need)
-      return launch_cd_lookup(d_layers, Bp, L, mp, d_work + off, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
-  }
-  if (do_cd) return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, mp.ndim <= 3 && !mp.fold, d_cd_prev);
-  return AUTODDL_OK;
+  return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, false, mp.ndim <= 3 && !mp.fold);
 }
 
 int autoddl_search(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const autoddl_mesh* mesh, const autoddl_net* net,
@@ -417,9 +428,9 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
 
   unsigned char* w = (unsigned char*)d_work;
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
-  const size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) +
-                               (mesh->ndim == 2 ? fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256 : 0) +
-                               (do_cd && cd_lookup_supported(mp, L, S) ? cd_lookup_workspace_bytes(mp, Bp, L) + 512 : 0);
+  size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) +
+                         (mesh->ndim == 2 ? fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256 : 0);
+  if (do_cd && cd_lookup_supported(mp, L, S)) tables_region += factors_bytes(mp, Bp, L) + cd_lookup_workspace_bytes(mp, Bp, L) + 512;
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));
   int32_t* d_init = (int32_t*)carve((size_t)Bp * S * L * 4);

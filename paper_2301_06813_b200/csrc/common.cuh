@@ -91,12 +91,15 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
                          int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
                          int32_t* d_sweeps, cudaStream_t st, bool resume = false, bool sbp_rows = false,
                          const int32_t* d_prev = nullptr);
-// many starts per problem on library-built tables (K = 36, 216): factors -> best responses -> look-up sweeps (factors.cu)
+// library-built tables of two / three mesh levels in factor form (factors.cu): the factors, the chain DP on them, and
+// Coordinate Descent from many starts by best-response look-ups
+bool factors_supported(const MeshParams& mp);
+size_t factors_bytes(const MeshParams& mp, int32_t Bp, int32_t L);
+int launch_build_factors(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_F, cudaStream_t st);
 bool cd_lookup_supported(const MeshParams& mp, int32_t L, int32_t S);
 size_t cd_lookup_workspace_bytes(const MeshParams& mp, int32_t Bp, int32_t L);
-int launch_cd_lookup(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, void* d_work,
-                     const int32_t* d_init, int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
-                     int32_t* d_sweeps, cudaStream_t st);
+int launch_cd_lookup(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams& mp, void* d_work, const int32_t* d_init, int32_t S,
+                     int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st);
 int launch_metropolis(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, const int32_t* d_init, int32_t S,
                       int32_t nsteps, int64_t tau_ps, uint64_t seed, int64_t* d_best_cost, int32_t* d_best_strategy,
                       int64_t* d_final_cost, int32_t* d_final_strategy, int32_t* d_accepted, cudaStream_t st);

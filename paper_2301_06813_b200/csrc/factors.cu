@@ -412,22 +412,26 @@ __global__ void __launch_bounds__(128) cd_lookup_kernel(const int64_t* __restric
 }
 
 template <int D>
-int launch_lookup_d(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_F, uint8_t* d_BR,
+int launch_factors_d(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_F, cudaStream_t st) {
+  const int ntiles = Bp * L, sms = device_sm_count();
+  const size_t smem = sizeof(FacSmem<D>);
+  ADL_CUDA_CHECK(cudaFuncSetAttribute(build_factors_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int per_sm = D == 3 ? 2 : 4;
+  const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;
+  build_factors_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_F);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
+template <int D>
+int launch_lookup_d(int32_t Bp, int32_t L, const MeshParams& mp, const int64_t* d_F, uint8_t* d_BR,
                     const int32_t* d_init, int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps,
                     cudaStream_t st) {
   using F = Fac<D>;
   const int64_t nt64 = (int64_t)Bp * L;
   if (nt64 > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   const int ntiles = (int)nt64, sms = device_sm_count();
-  {
-    const size_t smem = sizeof(FacSmem<D>);
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(build_factors_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int per_sm = D == 3 ? 2 : 4;
-    const int grid = ntiles < sms * per_sm ? ntiles : sms * per_sm;
-    build_factors_kernel<D><<<grid, 256, smem, st>>>(d_layers, ntiles, L, mp, d_F);
-    count_launch();
-    ADL_CUDA_CHECK(cudaGetLastError());
-  }
   {
     const size_t smem = sizeof(BrSmem<D>);
     ADL_CUDA_CHECK(cudaFuncSetAttribute(best_response_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -455,27 +459,34 @@ int launch_lookup_d(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const 
 
 }  // namespace
 
-// many starts per problem on library-built tables of two or three mesh levels
-bool cd_lookup_supported(const MeshParams& mp, int32_t L, int32_t S) {
-  return (mp.ndim == 2 || mp.ndim == 3) && !mp.fold && S >= 32 && L <= 16384;
+// library-built tables of two or three mesh levels have the factor form these kernels work on
+bool factors_supported(const MeshParams& mp) { return (mp.ndim == 2 || mp.ndim == 3) && !mp.fold; }
+
+size_t factors_bytes(const MeshParams& mp, int32_t Bp, int32_t L) {
+  const size_t fb = mp.ndim == 2 ? Fac<2>::FB : Fac<3>::FB;
+  return ((size_t)Bp * L * fb * 8 + 255) / 256 * 256;
 }
 
+int launch_build_factors(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_F, cudaStream_t st) {
+  if ((int64_t)Bp * L > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  return mp.ndim == 2 ? launch_factors_d<2>(d_layers, Bp, L, mp, d_F, st) : launch_factors_d<3>(d_layers, Bp, L, mp, d_F, st);
+}
+
+// many starts per problem: best-response look-ups on the factors
+bool cd_lookup_supported(const MeshParams& mp, int32_t L, int32_t S) { return factors_supported(mp) && S >= 32 && L <= 16384; }
+
+// bytes of the best-response tables (the factors are counted by factors_bytes)
 size_t cd_lookup_workspace_bytes(const MeshParams& mp, int32_t Bp, int32_t L) {
   const size_t nt = (size_t)Bp * L;
-  const size_t fb = mp.ndim == 2 ? Fac<2>::FB : Fac<3>::FB, es = mp.ndim == 2 ? Fac<2>::ES : Fac<3>::ES,
-               cs = mp.ndim == 2 ? Fac<2>::CS : Fac<3>::CS;
-  return (nt * fb * 8 + 255) / 256 * 256 + (nt * es * cs + 255) / 256 * 256 + 256;
+  const size_t es = mp.ndim == 2 ? Fac<2>::ES : Fac<3>::ES, cs = mp.ndim == 2 ? Fac<2>::CS : Fac<3>::CS;
+  return (nt * es * cs + 255) / 256 * 256 + 256;
 }
 
-int launch_cd_lookup(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, void* d_work,
-                     const int32_t* d_init, int32_t S, int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy,
-                     int32_t* d_sweeps, cudaStream_t st) {
-  const size_t nt = (size_t)Bp * L;
-  const size_t fb = mp.ndim == 2 ? Fac<2>::FB : Fac<3>::FB;
-  int64_t* d_F = (int64_t*)d_work;
-  uint8_t* d_BR = (uint8_t*)d_work + (nt * fb * 8 + 255) / 256 * 256;
-  if (mp.ndim == 2) return launch_lookup_d<2>(d_layers, Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
-  return launch_lookup_d<3>(d_layers, Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+int launch_cd_lookup(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams& mp, void* d_work, const int32_t* d_init, int32_t S,
+                     int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+  uint8_t* d_BR = (uint8_t*)d_work;
+  if (mp.ndim == 2) return launch_lookup_d<2>(Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+  return launch_lookup_d<3>(Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
 }
 
 }  // namespace autoddl

@@ -99,11 +99,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   uint8_t* cd_t = cd_s + (size_t)cd_S * L;
   const size_t cd_bytes = cd_init ? (((size_t)2 * cd_S * L + 15) & ~(size_t)15) : 0;
   uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
-#ifdef ADL_EXP_NO_SWEEP2
-  const bool two = false;
-#else
   const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well
-#endif
 
   // ---- once per CTA: facts per (layer kind, signature) -----------------------------------------------------------
   fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
