@@ -22,16 +22,29 @@ namespace autoddl {
 
 namespace {
 
-constexpr int FK = 36, FD = 2, FNS = 16, FNC = 9, FES = 17, FSTRIDE = FNC + 1, FCELLS = FK * FK;
-constexpr int kMaxFusedStarts = 8;                        // CD starts per chain whose first sweep rides along
+constexpr int FK = 36, FD = 2, FNS = 16, FNC = 9, FSTRIDE = FNC + 1, FCELLS = FK * FK;
+constexpr int FNU = 10;                                   // classes of a level's (output state, input state) pair, see below
+constexpr int FGZ = 100, FG = 104;                        // G[FGZ] = 0: the edge of an invalid signature / of the first layer
+constexpr int kMaxFusedStarts = 8;                        // CD starts per chain whose first sweeps ride along
 
+// Esym[a][b] = R[a][b] + R[dual b][dual a] takes only 10 x 10 distinct values on two mesh levels: a level's pair of states
+// (a_d, b_d) enters R only through its walk (slice / reduce-scatter / all-to-all / all-gather steps and the split codes
+// between them, sbp_builder.cuh) forward and backward, and the 16 pairs fall into FNU = 10 classes of equal (forward walk,
+// backward walk).  A tile therefore carries G[u0][u1]: 9 of the 100 entries are zero (no collective on either level),
+// 36 are the sum of two entries of the per-level Table-2 values TAB, 42 of four, 12 of six, 1 of eight.  They are laid out
+// by ascending number of summands so that a round of 32 lanes loads only what its entries need; the consumers (tile
+// expansion, DP, CD) reach G through byte index tables built once per CTA.
 struct CtaShared {
   SigInfo sig[2][FK];
-  uint16_t aoff[2][FK];                                   // per producer kind: A(i) * 17
-  uint8_t bcls[2][FK];                                    // per consumer kind: B(j) in 0..16
-  // step 3, state pair e = lane + 32 k: the <= 6 table entries whose sum is R[a][b] (6 bits each: five in slot_lo, the
-  // sixth in bits 26.. of sym) and the two entries (9 bits each) whose sum is Esym of the pair
-  uint32_t slot_lo[8][32], sym[8][32];
+  uint8_t bcls[2][FK];                                    // per consumer kind: B(j) in 0..16 (16 = invalid for the kind)
+  uint8_t ucls[16];                                       // class of a level's (a_d, b_d)
+  uint8_t nnz[FNU * FNU], gpos[FNU * FNU];                // per (u0, u1): number of summands, position in G
+  int32_t nl, nh;                                         // entries of <= 4 summands (positions 0..nl-1), of more (nl..nl+nh-1)
+  uint32_t lslot[3][32];                                  // position 32 k + lane: four 6-bit TAB slots
+  uint32_t hslot[2][32];                                  // position nl + lane: eight
+  alignas(16) uint8_t DPI[2][2][16][16];                  // [producer kind][row half][input class b][part * 4 + q]: DP rows
+  uint32_t XI[2][2][6][32];                               // [producer kind][kind][word][lane]: the 24 cells of the lane's class rows
+  alignas(4) uint8_t GI[2][2][FK][FK];                    // [producer kind][kind][i][j]: position of Esym[A(i)][B(j)] in G
 };
 
 struct alignas(16) Rec64 {                                 // byte image of autoddl_layer
@@ -47,7 +60,7 @@ struct alignas(16) WarpShared {
   int64_t WAR[FD][FNC];
   int64_t locW[FNC], locO[FNC];
   alignas(16) int64_t VP[NB][FK];                         // layer l in buffer l & (NB - 1)
-  int64_t Esym[NB][FES * FES];                             // R[a][b], then symmetrised in place; row / column 16 stay 0
+  int64_t G[NB][FG];                                      // the distinct values of Esym; [FGZ] = 0
   alignas(16) int64_t f[2][FK];
   Rec64 rec[8];                                           // ring of layer records, fetched four at a time
 };
@@ -101,26 +114,119 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
   const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well
 
-  // ---- once per CTA: facts per (layer kind, signature) -----------------------------------------------------------
+  // ---- once per CTA: facts per (layer kind, signature), the layout of G, the index tables ---------------------------
   fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
+  if (tid < 16) {                                          // class of (a_d, b_d) = rank of its (forward, backward) walk pair
+    auto key = [](int x) { return c_walk.w[x] | c_walk.w[dual_of(x & 3) * 4 + dual_of(x >> 2)] << 11; };
+    const uint32_t mine = key(tid);
+    int rep = tid, id = 0;
+    for (int y = tid - 1; y >= 0; --y)
+      if (key(y) == mine) rep = y;
+    for (int y = 0; y < rep; ++y) {
+      bool first = true;
+      for (int z = 0; z < y; ++z) first = first && key(z) != key(y);
+      id += first;
+    }
+    cs.ucls[tid] = (uint8_t)id;
+  }
+  for (int x = tid; x < 5 * 32; x += blockDim.x) (&cs.lslot[0][0])[x] = FNC | FNC << 6 | FNC << 12 | FNC << 18;   // zero slots (lslot, hslot)
   __syncthreads();
+  constexpr uint32_t kNoSlots = FNC | FNC << 6 | FNC << 12 | FNC << 18;
+  // the summands of entry e = (u0, u1), 6 bits each in w0 (first four) and w1; returns their number
+  auto entry_slots = [&](int e, uint32_t& w0, uint32_t& w1) -> int {
+    w0 = w1 = kNoSlots;
+    int n = 0, p0 = -1, p1 = -1;                           // a representative state pair per level
+    for (int x = 15; x >= 0; --x) {
+      if (cs.ucls[x] == e / FNU) p0 = x;
+      if (cs.ucls[x] == e % FNU) p1 = x;
+    }
+    if (p0 < 0 || p1 < 0) return 0;
+    const int a = (p0 >> 2) << 2 | (p1 >> 2), b = (p0 & 3) << 2 | (p1 & 3);
+    int idx[3 * FD];
+    auto take = [&]() {
+#pragma unroll
+      for (int q = 0; q < 3 * FD; ++q)
+        if (idx[q] != FNC) {
+          if (n < 4) w0 ^= (uint32_t)(FNC ^ idx[q]) << (6 * n);
+          else if (n < 8) w1 ^= (uint32_t)(FNC ^ idx[q]) << (6 * (n - 4));
+          else __trap();
+          ++n;
+        }
+    };
+    r_slots<FD>(a, b, idx);
+    take();
+    r_slots<FD>(dual_vec<FD>(b), dual_vec<FD>(a), idx);
+    take();
+    return n;
+  };
+  for (int e = tid; e < FNU * FNU; e += blockDim.x) {
+    uint32_t w0, w1;
+    cs.nnz[e] = (uint8_t)entry_slots(e, w0, w1);
+  }
+  __syncthreads();
+  for (int e = tid; e < FNU * FNU; e += blockDim.x) {      // positions: ascending number of summands, then (u0, u1)
+    uint32_t w0, w1;
+    const int my_n = entry_slots(e, w0, w1);
+    int pos = 0, nl = 0, nh = 0;
+    for (int o = 0; o < FNU * FNU; ++o) {
+      const int n = cs.nnz[o];
+      if (n >= 1 && n <= 4) ++nl;
+      if (n > 4) ++nh;
+      if (n >= 1 && (n < my_n || (n == my_n && o < e))) ++pos;
+    }
+    if (my_n == 0) pos = FGZ;
+    cs.gpos[e] = (uint8_t)pos;
+    if (e == 0) { cs.nl = nl; cs.nh = nh; }
+    if (my_n >= 1 && my_n <= 4) {
+      if (pos >= 96 || (pos < 32 && my_n > 2)) __trap();   // (the layout the rounds below rely on; holds for this walk table)
+      cs.lslot[pos >> 5][pos & 31] = w0;
+    } else if (my_n > 4) {
+      if (pos - nl >= 32) __trap();
+      cs.hslot[0][pos - nl] = w0;
+      cs.hslot[1][pos - nl] = w1;
+    }
+  }
   for (int x = tid; x < 2 * FK; x += blockDim.x) {
     const SigInfo& si = cs.sig[x / FK][x % FK];
-    cs.aoff[x / FK][x % FK] = (uint16_t)(si.a_idx * FES);  // a_idx = 16 for an invalid signature: the zero row
     cs.bcls[x / FK][x % FK] = (uint8_t)(si.b_idx >= 0 ? si.b_idx : FNS);
   }
-  for (int e = tid; e < FNS * FNS; e += blockDim.x) {
-    const int a = e / FNS, b = e % FNS;
-    int idx[3 * FD];
-    r_slots<FD>(a, b, idx);
-    cs.slot_lo[e >> 5][e & 31] = idx[0] | idx[1] << 6 | idx[2] << 12 | idx[3] << 18 | idx[4] << 24;
-    cs.sym[e >> 5][e & 31] = (a * FES + b) | (dual_vec<FD>(b) * FES + dual_vec<FD>(a)) << 9 | idx[5] << 26;
+  __syncthreads();
+  auto gp = [&](int a, int b) -> int {                     // position of Esym[a][b]; a = 16 / b < 0: invalid signature, zero
+    if (a >= FNS || b < 0 || b >= FNS) return FGZ;
+    return cs.gpos[cs.ucls[(a >> 2) << 2 | (b >> 2)] * FNU + cs.ucls[(a & 3) << 2 | (b & 3)]];
+  };
+  for (int x = tid; x < 4 * FCELLS; x += blockDim.x) {
+    const int kk = x / FCELLS, i = x % FCELLS / FK, j = x % FK;
+    cs.GI[kk >> 1][kk & 1][i][j] = (uint8_t)gp(cs.sig[kk >> 1][i].a_idx, cs.sig[kk & 1][j].b_idx);
+  }
+  for (int x = tid; x < 2 * 2 * 16 * 16; x += blockDim.x) {
+    // DP: lane (b, half) scans rows 18 half + 6 part + r; rows whose level-1 digit r is 2, 4 or 5 share their edge (all
+    // output P, or all invalid), so a part has four distinct values q = 0..3 for r = 0, 1, 3, 2
+    const int kp = x >> 9, half = x >> 8 & 1, bcl = x >> 4 & 15, part = (x & 15) >> 2, q = x & 3;
+    const int row = 18 * half + 6 * part + (q < 2 ? q : (q == 2 ? 3 : 2));
+    cs.DPI[kp][half][bcl][x & 15] = (uint8_t)(part < 3 ? gp(cs.sig[kp][row].a_idx, bcl) : FGZ);
   }
   __syncthreads();
+  for (int x = tid; x < 4 * 6 * 32; x += blockDim.x) {
+    // tile expansion: lane (h, pc), class row n = 3 c0 + t -> row (rep(c0), 3 h + t); bytes 2 n, 2 n + 1 = its two columns
+    const int kk = x / 192, w = x % 192 / 32, ln = x % 32, pc = ln & 15, h = ln >> 4;
+    uint32_t word = 0;
+    for (int by = 0; by < 4; ++by) {
+      const int n = (4 * w + by) >> 1, col = 2 * pc + ((4 * w + by) & 1), c0 = n / 3, t = n % 3;
+      const int r0 = c0 < 2 ? c0 : (c0 == 2 ? 3 : 2);
+      word |= (uint32_t)cs.GI[kk >> 1][kk & 1][r0 * 6 + 3 * h + t][col] << (8 * by);
+    }
+    cs.XI[kk >> 1][kk & 1][w][ln] = word;
+  }
+  __syncthreads();
+  const int g_nl = cs.nl, g_nh = cs.nh;
 
   // ---- once per warp: tile-invariant roles of this lane ---------------------------------------------------------
-  for (int x = lane; x < NB * FES * FES; x += 32) (&ws.Esym[0][0])[x] = 0;
-  if (lane < 2 * FD) ws.TAB[lane * FSTRIDE + FNC] = 0;
+  auto warp_init = [&]() {                                 // zero slots of TAB, zero entry (and first-layer state) of G
+    for (int x = lane; x < NB * FG; x += 32) (&ws.G[0][0])[x] = 0;
+    if (lane < 2 * FD) ws.TAB[lane * FSTRIDE + FNC] = 0;
+  };
+  warp_init();
   // step 1: lane (x, m) for lane < 20
   const int q_x = lane >> 2, q_m = lane & 3;
   const uint32_t q_sub = (uint32_t)mp.sub[q_m];
@@ -166,9 +272,9 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       const int kind = rec.kind;
       if (l == 0) kind_prev = kind;                          // no producer: any valid kind (E(0) = 0)
       const size_t tile = (size_t)p * L + l;
-      int64_t* const Ecur = ws.Esym[l & (NB - 1)];
+      int64_t* const Gc = ws.G[l & (NB - 1)];
       int64_t* const VPc = ws.VP[l & (NB - 1)];
-      const int64_t* const Eprv = ws.Esym[(l & (NB - 1)) ^ (NB - 1)];   // layer l - 1 (NB = 2)
+      const int64_t* const Gp = ws.G[(l & (NB - 1)) ^ (NB - 1)];          // layer l - 1 (NB = 2)
       const int64_t* const VPp = ws.VP[(l & (NB - 1)) ^ (NB - 1)];
 
       // ---- 1. Q[x][m] = ceil(extent x / product of the levels in m) -------------------------------------------------
@@ -221,28 +327,25 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           if (mask) mask[tile * FK + j] = ok ? 1 : 0;
         }
       }
-      {
-        uint32_t sy[8];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) sy[k] = cs.sym[k][lane];
-        if (l > 0) {
-#pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            const uint32_t lo = cs.slot_lo[k][lane];
-            Ecur[sy[k] & 511] = ws.TAB[lo & 63] + ws.TAB[lo >> 6 & 63] + ws.TAB[lo >> 12 & 63] + ws.TAB[lo >> 18 & 63] +
-                                   ws.TAB[lo >> 24 & 63] + ws.TAB[sy[k] >> 26];
-          }
-          __syncwarp();
-          int64_t es[8];                                     // forward leg + backward leg, in place: reads, then writes
-#pragma unroll
-          for (int k = 0; k < 8; ++k) es[k] = Ecur[sy[k] & 511] + Ecur[sy[k] >> 9 & 511];
-          __syncwarp();
-#pragma unroll
-          for (int k = 0; k < 8; ++k) Ecur[sy[k] & 511] = es[k];
-        } else {
-#pragma unroll
-          for (int k = 0; k < 8; ++k) Ecur[sy[k] & 511] = 0;
+      // G: positions 0..31 are sums of two TAB entries, 32..nl-1 of at most four, nl..nl+nh-1 (<= 32 of them) of at most eight
+      if (l > 0) {
+        {
+          const uint32_t w = cs.lslot[0][lane];
+          Gc[lane] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63];
         }
+#pragma unroll
+        for (int k = 1; k < 3; ++k) {
+          const uint32_t w = cs.lslot[k][lane];
+          const int64_t v = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63] + ws.TAB[w >> 12 & 63] + ws.TAB[w >> 18 & 63];
+          if (32 * k + lane < g_nl) Gc[32 * k + lane] = v;
+        }
+        if (lane < g_nh) {
+          const uint32_t w = cs.hslot[0][lane], x = cs.hslot[1][lane];
+          Gc[g_nl + lane] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63] + ws.TAB[w >> 12 & 63] + ws.TAB[w >> 18 & 63] +
+                            ws.TAB[x & 63] + ws.TAB[x >> 6 & 63] + ws.TAB[x >> 12 & 63] + ws.TAB[x >> 18 & 63];
+        }
+      } else {
+        for (int x = lane; x < FGZ; x += 32) Gc[x] = 0;       // the first layer has no producer
       }
       __syncwarp();
 
@@ -254,20 +357,22 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       // covers 256 contiguous bytes.  Columns 32..35: one lane per row, 32 contiguous bytes each.
       if (T) {
         int64_t* out = T + tile * FCELLS;
-        const uint16_t* aok = cs.aoff[kind_prev];
         {
           const int pc = lane & 15, h = lane >> 4;
           const longlong2 vp = *reinterpret_cast<const longlong2*>(&VPc[2 * pc]);
-          const uint32_t bb = *reinterpret_cast<const uint16_t*>(&cs.bcls[kind][2 * pc]);
-          const int b0 = bb & 255, b1 = bb >> 8;
+          const uint32_t* xi = &cs.XI[kind_prev][kind][0][lane];
+          uint32_t xw[6];
+#pragma unroll
+          for (int w = 0; w < 6; ++w) xw[w] = xi[32 * w];
           int64_t* o = out + (3 * h) * FK + 2 * pc;
 #pragma unroll
           for (int c0 = 0; c0 < 4; ++c0) {
             const int r0 = c0 < 2 ? c0 : (c0 == 2 ? 3 : 2);  // representative level-0 digit: 0, 1, 3, 2 (= 4 = 5)
 #pragma unroll
             for (int t = 0; t < 3; ++t) {
-              const int ao = aok[r0 * 6 + 3 * h + t];
-              const longlong2 v = make_longlong2(vp.x + Ecur[ao + b0], vp.y + Ecur[ao + b1]);
+              const int n = 3 * c0 + t;
+              const uint32_t pr = xw[n >> 1] >> (16 * (n & 1));
+              const longlong2 v = make_longlong2(vp.x + Gc[pr & 255], vp.y + Gc[pr >> 8 & 255]);
               __stcs(reinterpret_cast<longlong2*>(o + (r0 * 6 + t) * FK), v);
               if (c0 == 3) {
                 __stcs(reinterpret_cast<longlong2*>(o + (4 * 6 + t) * FK), v);
@@ -279,14 +384,13 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         {
           const longlong2 vpa = *reinterpret_cast<const longlong2*>(&VPc[32]);
           const longlong2 vpb = *reinterpret_cast<const longlong2*>(&VPc[34]);
-          const uint32_t bb = *reinterpret_cast<const uint32_t*>(&cs.bcls[kind][32]);
 #pragma unroll
           for (int i0 = 0; i0 < 64; i0 += 32) {
             const int i = i0 + lane;
             if (i < FK) {
-              const int64_t* er = Ecur + aok[i];
-              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 32), make_longlong2(vpa.x + er[bb & 255], vpa.y + er[bb >> 8 & 255]));
-              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 34), make_longlong2(vpb.x + er[bb >> 16 & 255], vpb.y + er[bb >> 24]));
+              const uint32_t gi = *reinterpret_cast<const uint32_t*>(&cs.GI[kind_prev][kind][i][32]);
+              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 32), make_longlong2(vpa.x + Gc[gi & 255], vpa.y + Gc[gi >> 8 & 255]));
+              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 34), make_longlong2(vpb.x + Gc[gi >> 16 & 255], vpb.y + Gc[gi >> 24]));
             }
           }
         }
@@ -298,15 +402,18 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         for (int j = lane; j < FK; j += 32) fn[j] = VPc[j];            // f_0[j] = T[0][0][j]
       } else {
         const int64_t* f = ws.f[cur];
-        const uint16_t* ao = cs.aoff[kind_prev] + 18 * dp_h;
+        const uint4 dq = *reinterpret_cast<const uint4*>(&cs.DPI[kind_prev][dp_h][dp_b][0]);
         const int64_t* fh = f + 18 * dp_h;
         int64_t pb[3];
         int pa[3];
 #pragma unroll
         for (int part = 0; part < 3; ++part) {             // three independent chains of six rows, merged in row order
+          const uint32_t dw = part == 0 ? dq.x : (part == 1 ? dq.y : dq.z);
           int64_t tv[6], fv[6];
-#pragma unroll
-          for (int r = 0; r < 6; ++r) tv[r] = Ecur[ao[6 * part + r] + dp_b];
+          tv[0] = Gc[dw & 255];
+          tv[1] = Gc[dw >> 8 & 255];
+          tv[3] = Gc[dw >> 16 & 255];
+          tv[2] = tv[4] = tv[5] = Gc[dw >> 24];            // level-1 digits 2, 4, 5: the same edge
 #pragma unroll
           for (int r = 0; r < 6; r += 2) {
             const longlong2 f2 = *reinterpret_cast<const longlong2*>(fh + 6 * part + r);
@@ -374,14 +481,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           int64_t* stash = cd_stash + st * FK;               // T[l][s1_{l-1}][.]: row of sweep 1's next update
           int64_t* stash2 = cd_stash2 + st * FK;             // T[l-1][s2_{l-2}][.]: row of sweep 2's next update
           if (l > 0) {                                       // sweep 1, layer l-1: row stashed, column from this tile
-            const int bright = cs.bcls[kind][sv[l]];
+            const uint8_t* gcol = &cs.GI[kind_prev][kind][0][sv[l]];           // column s1_l of this tile
             int64_t bv = INT64_MAX;
             int bi = FK;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const int c = 32 * q + lane;
               if (c < FK) {
-                const int64_t g = stash[c] + Ecur[cs.aoff[kind_prev][c] + bright];
+                const int64_t g = stash[c] + Gc[gcol[c * FK]];
                 if (g < bv) { bv = g; bi = c; }
               }
             }
@@ -390,14 +497,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
             __syncwarp();
           }
           if (two && l > 1) {                                // sweep 2, layer l-2: column from tile l-1 given s1_{l-1}
-            const int bright = cs.bcls[kind_prev][sv[l - 1]];
+            const uint8_t* gcol = &cs.GI[kind_pp][kind_prev][0][sv[l - 1]];    // column s1_{l-1} of tile l-1
             int64_t bv = INT64_MAX;
             int bi = FK;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const int c = 32 * q + lane;
               if (c < FK) {
-                const int64_t g = stash2[c] + Eprv[cs.aoff[kind_pp][c] + bright];
+                const int64_t g = stash2[c] + Gp[gcol[c * FK]];
                 if (g < bv) { bv = g; bi = c; }
               }
             }
@@ -406,14 +513,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
             __syncwarp();
           }
           {                                                  // rows for the next updates (s_{-1} := 0; E(0) = 0 whatever the row)
-            const int aleft = cs.aoff[kind_prev][l > 0 ? sv[l - 1] : 0];
-            const int aleft2 = cs.aoff[kind_pp][l > 1 ? tv[l - 2] : 0];
+            const uint8_t* grow = cs.GI[kind_prev][kind][l > 0 ? sv[l - 1] : 0];
+            const uint8_t* grow2 = cs.GI[kind_pp][kind_prev][l > 1 ? tv[l - 2] : 0];
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const int c = 32 * q + lane;
               if (c < FK) {
-                stash[c] = VPc[c] + Ecur[aleft + cs.bcls[kind][c]];
-                if (two && l > 0) stash2[c] = VPp[c] + Eprv[aleft2 + cs.bcls[kind_prev][c]];
+                stash[c] = VPc[c] + Gc[grow[c]];
+                if (two && l > 0) stash2[c] = VPp[c] + Gp[grow2[c]];
               }
             }
             __syncwarp();
@@ -431,14 +538,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
             __syncwarp();
             if (two) {
               if (l > 0) {                                   // sweep 2, layer L-2: column from this (last) tile given s1_{L-1}
-                const int bright = cs.bcls[kind][sv[l]];
+                const uint8_t* gcol = &cs.GI[kind_prev][kind][0][sv[l]];
                 bv = INT64_MAX;
                 bi = FK;
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                   const int c = 32 * q + lane;
                   if (c < FK) {
-                    const int64_t g = stash2[c] + Ecur[cs.aoff[kind_prev][c] + bright];
+                    const int64_t g = stash2[c] + Gc[gcol[c * FK]];
                     if (g < bv) { bv = g; bi = c; }
                   }
                 }
@@ -446,14 +553,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
                 if (lane == 0) tv[l - 1] = (uint8_t)bi;
                 __syncwarp();
               }
-              const int aleft2 = cs.aoff[kind_prev][l > 0 ? tv[l - 1] : 0];   // sweep 2, last layer
+              const uint8_t* grow2 = cs.GI[kind_prev][kind][l > 0 ? tv[l - 1] : 0];   // sweep 2, last layer
               bv = INT64_MAX;
               bi = FK;
 #pragma unroll
               for (int q = 0; q < 2; ++q) {
                 const int c = 32 * q + lane;
                 if (c < FK) {
-                  const int64_t g = VPc[c] + Ecur[aleft2 + cs.bcls[kind][c]];
+                  const int64_t g = VPc[c] + Gc[grow2[c]];
                   if (g < bv) { bv = g; bi = c; }
                 }
               }
@@ -479,12 +586,12 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         if (v < bv) { bv = v; bi = 32 + lane; }
       }
       warp_argmin64(bv, bi);
-      // back-pointers in the workspace: pull the chain's L x 36 bytes into the (now free) Esym buffers first, so that
-      // the dependent walk reads shared memory
+      // back-pointers in the workspace: pull the chain's L x 36 bytes into the warp's (now free) tile state first, so
+      // that the dependent walk reads shared memory
       const uint8_t* bw = bp;
       __syncwarp();
-      if (bp_glob && (size_t)L * FK <= sizeof(ws.Esym)) {
-        uint8_t* scratch = reinterpret_cast<uint8_t*>(&ws.Esym[0][0]);
+      if (bp_glob && (size_t)L * FK <= offsetof(WS, rec)) {
+        uint8_t* scratch = reinterpret_cast<uint8_t*>(&ws);
         const uint32_t* src = reinterpret_cast<const uint32_t*>(bp);       // L * 36 bytes: a multiple of 4, slices 4-byte aligned
         uint32_t* dst = reinterpret_cast<uint32_t*>(scratch);
         const int n4 = L * FK / 4;
@@ -515,9 +622,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         }
       }
       __syncwarp();
-      if (bw != bp) {                                      // the next chain expects zero borders in the Esym buffers
-        for (int x = lane; x < NB * FES * FES; x += 32) (&ws.Esym[0][0])[x] = 0;
-      }
+      if (bw != bp) warp_init();                           // the next chain expects the zero entries of TAB and G
       if (cd) {
         for (int x = lane; x < cd_S * L; x += 32) {
           cd_s1[(size_t)p * cd_S * L + x] = cd_s[x];
