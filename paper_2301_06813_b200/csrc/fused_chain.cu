@@ -24,24 +24,31 @@ namespace {
 
 constexpr int FK = 36, FD = 2, FNS = 16, FNC = 9, FSTRIDE = FNC + 1, FCELLS = FK * FK;
 constexpr int FNU = 10;                                   // classes of a level's (output state, input state) pair, see below
-constexpr int FGZ = 100, FG = 104;                        // G[FGZ] = 0: the edge of an invalid signature / of the first layer
+constexpr int FGZ = 143, FG = 144;                        // G[FGZ] = 0: the edge of an invalid signature / of the first layer
 constexpr int kMaxFusedStarts = 8;                        // CD starts per chain whose first sweeps ride along
 
 // Esym[a][b] = R[a][b] + R[dual b][dual a] takes only 10 x 10 distinct values on two mesh levels: a level's pair of states
 // (a_d, b_d) enters R only through its walk (slice / reduce-scatter / all-to-all / all-gather steps and the split codes
 // between them, sbp_builder.cuh) forward and backward, and the 16 pairs fall into FNU = 10 classes of equal (forward walk,
 // backward walk).  A tile therefore carries G[u0][u1]: 9 of the 100 entries are zero (no collective on either level),
-// 36 are the sum of two entries of the per-level Table-2 values TAB, 42 of four, 12 of six, 1 of eight.  They are laid out
-// by ascending number of summands so that a round of 32 lanes loads only what its entries need; the consumers (tile
-// expansion, DP, CD) reach G through byte index tables built once per CTA.
+// 36 are the sum of two entries of the per-level Table-2 values TAB, 42 of four, 12 of six, 1 of eight.  They are computed
+// in order of ascending number of summands, so that a round of 32 lanes loads only what its entries need; the consumers
+// (tile expansion, DP, CD) reach G through byte index tables built once per CTA.
+// Where an entry lives: position 16 (3 hi(u0) + hi(u1)) + 4 col(u0) + col(u1).  col is a 4-colouring of the classes in
+// which the classes (a_d, .) of one producer state differ and so do the classes (., b_d) of one consumer state: the 16
+// entries a consumer reads along a row of the tile (fixed a, all b) or along a column lie in 16 different 8-byte bank
+// slots.  (Performance only: any injective (col, hi) gives the same results.)
+__device__ __constant__ uint8_t c_ucol[FNU] = {0, 2, 1, 3, 1, 0, 2, 1, 0, 3};
+__device__ __constant__ uint8_t c_uhi[FNU] = {0, 0, 0, 0, 1, 1, 1, 2, 2, 1};
 struct CtaShared {
   SigInfo sig[2][FK];
   uint8_t bcls[2][FK];                                    // per consumer kind: B(j) in 0..16 (16 = invalid for the kind)
   uint8_t ucls[16];                                       // class of a level's (a_d, b_d)
-  uint8_t nnz[FNU * FNU], gpos[FNU * FNU];                // per (u0, u1): number of summands, position in G
-  int32_t nl, nh;                                         // entries of <= 4 summands (positions 0..nl-1), of more (nl..nl+nh-1)
-  uint32_t lslot[3][32];                                  // position 32 k + lane: four 6-bit TAB slots
-  uint32_t hslot[2][32];                                  // position nl + lane: eight
+  uint8_t nnz[FNU * FNU];                                 // per (u0, u1): number of summands
+  uint32_t ew[2][FNU * FNU];                              // (set-up scratch: its summand words)
+  int32_t nl, nh;                                         // entries of 1..4 summands (ranks 0..nl-1), of more (nl..nl+nh-1)
+  uint32_t lslot[3][32];                                  // rank 32 k + lane: four 6-bit TAB slots, position in bits 24..31
+  uint32_t hslot[2][32];                                  // rank nl + lane: eight slots, position in bits 24..31 of [1]
   alignas(16) uint8_t DPI[2][2][16][16];                  // [producer kind][row half][input class b][part * 4 + q]: DP rows
   uint32_t XI[2][2][6][32];                               // [producer kind][kind][word][lane]: the 24 cells of the lane's class rows
   alignas(4) uint8_t GI[2][2][FK][FK];                    // [producer kind][kind][i][j]: position of Esym[A(i)][B(j)] in G
@@ -61,7 +68,7 @@ struct alignas(16) WarpShared {
   int64_t locW[FNC], locO[FNC];
   alignas(16) int64_t VP[NB][FK];                         // layer l in buffer l & (NB - 1)
   int64_t G[NB][FG];                                      // the distinct values of Esym; [FGZ] = 0
-  alignas(16) int64_t f[2][FK];
+  alignas(16) int64_t f[FK];
   Rec64 rec[8];                                           // ring of layer records, fetched four at a time
 };
 
@@ -104,15 +111,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   unsigned char* wbase = fsm_raw + ((sizeof(CtaShared) + 127) & ~(size_t)127) + (size_t)warp * per_warp_bytes;
   using WS = WarpShared<NB>;
   WS& ws = *reinterpret_cast<WS*>(wbase);
-  // CD only: the row stashes of the two sweeps [2][cd_S][36] int64, then the strategies of the chain's starts after
-  // sweep 1 and sweep 2 [2][cd_S][L] bytes; then the back-pointers [L][K] (or a workspace slice: bp_glob)
-  int64_t* cd_stash = reinterpret_cast<int64_t*>(wbase + sizeof(WS));
-  int64_t* cd_stash2 = cd_stash + (size_t)cd_S * FK;
-  uint8_t* cd_s = wbase + sizeof(WS) + (cd_init ? (size_t)2 * cd_S * FK * 8 : 0);
+  // CD only: the row stash of sweep 2 [cd_S][36] int64, then the strategies of the chain's starts after sweep 1 and
+  // sweep 2 [2][cd_S][L] bytes; then the back-pointers [L][K] (or a workspace slice: bp_glob)
+  int64_t* cd_stash2 = reinterpret_cast<int64_t*>(wbase + sizeof(WS));
+  uint8_t* cd_s = wbase + sizeof(WS) + (cd_init ? (size_t)cd_S * FK * 8 : 0);
   uint8_t* cd_t = cd_s + (size_t)cd_S * L;
   const size_t cd_bytes = cd_init ? (((size_t)2 * cd_S * L + 15) & ~(size_t)15) : 0;
   uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
-  const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well
+  const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well (NB = 2 whenever CD rides along)
 
   // ---- once per CTA: facts per (layer kind, signature), the layout of G, the index tables ---------------------------
   fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
@@ -162,38 +168,17 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   for (int e = tid; e < FNU * FNU; e += blockDim.x) {
     uint32_t w0, w1;
     cs.nnz[e] = (uint8_t)entry_slots(e, w0, w1);
-  }
-  __syncthreads();
-  for (int e = tid; e < FNU * FNU; e += blockDim.x) {      // positions: ascending number of summands, then (u0, u1)
-    uint32_t w0, w1;
-    const int my_n = entry_slots(e, w0, w1);
-    int pos = 0, nl = 0, nh = 0;
-    for (int o = 0; o < FNU * FNU; ++o) {
-      const int n = cs.nnz[o];
-      if (n >= 1 && n <= 4) ++nl;
-      if (n > 4) ++nh;
-      if (n >= 1 && (n < my_n || (n == my_n && o < e))) ++pos;
-    }
-    if (my_n == 0) pos = FGZ;
-    cs.gpos[e] = (uint8_t)pos;
-    if (e == 0) { cs.nl = nl; cs.nh = nh; }
-    if (my_n >= 1 && my_n <= 4) {
-      if (pos >= 96 || (pos < 32 && my_n > 2)) __trap();   // (the layout the rounds below rely on; holds for this walk table)
-      cs.lslot[pos >> 5][pos & 31] = w0;
-    } else if (my_n > 4) {
-      if (pos - nl >= 32) __trap();
-      cs.hslot[0][pos - nl] = w0;
-      cs.hslot[1][pos - nl] = w1;
-    }
+    cs.ew[0][e] = w0;
+    cs.ew[1][e] = w1;
   }
   for (int x = tid; x < 2 * FK; x += blockDim.x) {
     const SigInfo& si = cs.sig[x / FK][x % FK];
     cs.bcls[x / FK][x % FK] = (uint8_t)(si.b_idx >= 0 ? si.b_idx : FNS);
   }
-  __syncthreads();
+  auto upos = [&](int u0, int u1) -> int { return 16 * (3 * c_uhi[u0] + c_uhi[u1]) + 4 * c_ucol[u0] + c_ucol[u1]; };
   auto gp = [&](int a, int b) -> int {                     // position of Esym[a][b]; a = 16 / b < 0: invalid signature, zero
     if (a >= FNS || b < 0 || b >= FNS) return FGZ;
-    return cs.gpos[cs.ucls[(a >> 2) << 2 | (b >> 2)] * FNU + cs.ucls[(a & 3) << 2 | (b & 3)]];
+    return upos(cs.ucls[(a >> 2) << 2 | (b >> 2)], cs.ucls[(a & 3) << 2 | (b & 3)]);
   };
   for (int x = tid; x < 4 * FCELLS; x += blockDim.x) {
     const int kk = x / FCELLS, i = x % FCELLS / FK, j = x % FK;
@@ -207,6 +192,26 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     cs.DPI[kp][half][bcl][x & 15] = (uint8_t)(part < 3 ? gp(cs.sig[kp][row].a_idx, bcl) : FGZ);
   }
   __syncthreads();
+  for (int e = tid; e < FNU * FNU; e += blockDim.x) {      // computed in order of ascending number of summands, then (u0, u1)
+    const int my_n = cs.nnz[e];
+    int rank = 0, nl = 0, nh = 0;
+    for (int o = 0; o < FNU * FNU; ++o) {
+      const int n = cs.nnz[o];
+      if (n >= 1 && n <= 4) ++nl;
+      if (n > 4) ++nh;
+      if (n >= 1 && (n < my_n || (n == my_n && o < e))) ++rank;
+    }
+    const uint32_t pos = upos(e / FNU, e % FNU);           // (an entry without summands is never written: it stays 0)
+    if (e == 0) { cs.nl = nl; cs.nh = nh; }
+    if (my_n >= 1 && my_n <= 4) {
+      if (rank >= 96 || (rank < 32 && my_n > 2)) __trap();   // (what the rounds below rely on; holds for this walk table)
+      cs.lslot[rank >> 5][rank & 31] = cs.ew[0][e] | pos << 24;
+    } else if (my_n > 4) {
+      if (rank - nl >= 32) __trap();
+      cs.hslot[0][rank - nl] = cs.ew[0][e];
+      cs.hslot[1][rank - nl] = cs.ew[1][e] | pos << 24;
+    }
+  }
   for (int x = tid; x < 4 * 6 * 32; x += blockDim.x) {
     // tile expansion: lane (h, pc), class row n = 3 c0 + t -> row (rep(c0), 3 h + t); bytes 2 n, 2 n + 1 = its two columns
     const int kk = x / 192, w = x % 192 / 32, ln = x % 32, pc = ln & 15, h = ln >> 4;
@@ -260,7 +265,6 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     if (cd) {
       for (int x = lane; x < cd_S * L; x += 32) cd_s[x] = (uint8_t)cd_init[(size_t)p * cd_S * L + x];
     }
-    int cur = 0;
 
     for (int l = 0; l < L; ++l) {
       if ((l & 3) == 0) {
@@ -327,25 +331,25 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           if (mask) mask[tile * FK + j] = ok ? 1 : 0;
         }
       }
-      // G: positions 0..31 are sums of two TAB entries, 32..nl-1 of at most four, nl..nl+nh-1 (<= 32 of them) of at most eight
+      // G: ranks 0..31 are sums of two TAB entries, 32..nl-1 of at most four, nl..nl+nh-1 (<= 32 of them) of at most eight
       if (l > 0) {
         {
           const uint32_t w = cs.lslot[0][lane];
-          Gc[lane] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63];
+          Gc[w >> 24] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63];
         }
 #pragma unroll
         for (int k = 1; k < 3; ++k) {
           const uint32_t w = cs.lslot[k][lane];
           const int64_t v = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63] + ws.TAB[w >> 12 & 63] + ws.TAB[w >> 18 & 63];
-          if (32 * k + lane < g_nl) Gc[32 * k + lane] = v;
+          if (32 * k + lane < g_nl) Gc[w >> 24] = v;
         }
         if (lane < g_nh) {
           const uint32_t w = cs.hslot[0][lane], x = cs.hslot[1][lane];
-          Gc[g_nl + lane] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63] + ws.TAB[w >> 12 & 63] + ws.TAB[w >> 18 & 63] +
-                            ws.TAB[x & 63] + ws.TAB[x >> 6 & 63] + ws.TAB[x >> 12 & 63] + ws.TAB[x >> 18 & 63];
+          Gc[x >> 24] = ws.TAB[w & 63] + ws.TAB[w >> 6 & 63] + ws.TAB[w >> 12 & 63] + ws.TAB[w >> 18 & 63] +
+                        ws.TAB[x & 63] + ws.TAB[x >> 6 & 63] + ws.TAB[x >> 12 & 63] + ws.TAB[x >> 18 & 63];
         }
       } else {
-        for (int x = lane; x < FGZ; x += 32) Gc[x] = 0;       // the first layer has no producer
+        for (int x = lane; x < FG; x += 32) Gc[x] = 0;        // the first layer has no producer
       }
       __syncwarp();
 
@@ -397,11 +401,11 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       }
 
       // ---- 5. chain DP (R9): f_l[j] = VP[j] + min_i f_{l-1}[i] + Esym[A(i)][B(j)], smallest i on ties -----------------
-      int64_t* fn = ws.f[cur ^ 1];
+      int64_t* fn = ws.f;
       if (l == 0) {
         for (int j = lane; j < FK; j += 32) fn[j] = VPc[j];            // f_0[j] = T[0][0][j]
       } else {
-        const int64_t* f = ws.f[cur];
+        const int64_t* f = ws.f;
         const uint4 dq = *reinterpret_cast<const uint4*>(&cs.DPI[kind_prev][dp_h][dp_b][0]);
         const int64_t* fh = f + 18 * dp_h;
         int64_t pb[3];
@@ -452,6 +456,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           }
           warp_argmin64(h16, a16);
         }
+        __syncwarp();                                        // f_{l-1} has been read by every lane: f_l goes in its place
 #pragma unroll
         for (int j0 = 0; j0 < 64; j0 += 32) {
           const int j = j0 + lane;
@@ -465,39 +470,41 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           }
         }
       }
-      cur ^= 1;
 
       // ---- 6. Coordinate Descent (R10): sweep 1 of layer l-1 and, trailing it by one layer, sweep 2 of layer l-2 --------------
-      // Sweep 2's update of layer m needs the row T[m][s2_{m-1}][.] (stashed at tile m+1 from the previous layer's
-      // factors) and the column T[m+1][.][s1_{m+1}], whose s1_{m+1} is final once sweep 1 has passed layer m+1: at tile
-      // m+2, with tile m+1's Esym still in the other buffer.  Every layer is re-evaluated in sweep 2: the update of a
-      // clean layer returns the value it has, so the result is that of the plain algorithm (61 of the 64 layers of a
-      // config-4 chain change in sweep 1: sweep 2 would re-evaluate them all anyway).
-      if (cd) {
+      // Sweep 1's update of layer l-1 takes its row T[l-1][s1_{l-2}][.] from the previous tile's factors (still in the other
+      // buffer) and its column T[l][.][s_l] from this tile's.  Sweep 2's update of layer m needs the row T[m][s2_{m-1}][.]
+      // (stashed at tile m+1, from the previous layer's factors) and the column T[m+1][.][s1_{m+1}], whose s1_{m+1} is final
+      // once sweep 1 has passed layer m+1: at tile m+2, with tile m+1's factors still in the other buffer.  Every layer is
+      // re-evaluated in sweep 2: the update of a clean layer returns the value it has, so the result is that of the plain
+      // algorithm (61 of the 64 layers of a config-4 chain change in sweep 1: sweep 2 would re-evaluate them all anyway).
+      // Lane c (and c + 32) owns candidate c: it alone reads and writes stash2[c], so the stash needs no barrier.
+      if (NB == 2 && cd) {
         __syncwarp();
         for (int st = 0; st < cd_S; ++st) {
           uint8_t* sv = cd_s + (size_t)st * L;               // after sweep 1 (starts as the initial strategy)
           uint8_t* tv = cd_t + (size_t)st * L;               // after sweep 2
-          int64_t* stash = cd_stash + st * FK;               // T[l][s1_{l-1}][.]: row of sweep 1's next update
           int64_t* stash2 = cd_stash2 + st * FK;             // T[l-1][s2_{l-2}][.]: row of sweep 2's next update
-          if (l > 0) {                                       // sweep 1, layer l-1: row stashed, column from this tile
-            const uint8_t* gcol = &cs.GI[kind_prev][kind][0][sv[l]];           // column s1_l of this tile
+          int s1 = 0, s2 = 0;                                // s1_{l-1}, s2_{l-2} as updated at this tile (s_{-1} := 0)
+          if (l > 0) {                                       // sweep 1, layer l-1
+            const uint8_t* grow = cs.GI[kind_pp][kind_prev][l > 1 ? sv[l - 2] : 0];   // (tile 0's G is zero whatever the row)
+            const uint8_t* gcol = &cs.GI[kind_prev][kind][0][sv[l]];                  // column s_l of this tile
             int64_t bv = INT64_MAX;
             int bi = FK;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const int c = 32 * q + lane;
               if (c < FK) {
-                const int64_t g = stash[c] + Gc[gcol[c * FK]];
+                const int64_t g = VPp[c] + Gp[grow[c]] + Gc[gcol[c * FK]];
                 if (g < bv) { bv = g; bi = c; }
               }
             }
             warp_argmin64(bv, bi);
             if (lane == 0) sv[l - 1] = (uint8_t)bi;
-            __syncwarp();
+            s1 = bi;
           }
           if (two && l > 1) {                                // sweep 2, layer l-2: column from tile l-1 given s1_{l-1}
-            const uint8_t* gcol = &cs.GI[kind_pp][kind_prev][0][sv[l - 1]];    // column s1_{l-1} of tile l-1
+            const uint8_t* gcol = &cs.GI[kind_pp][kind_prev][0][s1];
             int64_t bv = INT64_MAX;
             int bi = FK;
 #pragma unroll
@@ -510,35 +517,34 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
             }
             warp_argmin64(bv, bi);
             if (lane == 0) tv[l - 2] = (uint8_t)bi;
-            __syncwarp();
+            s2 = bi;
           }
-          {                                                  // rows for the next updates (s_{-1} := 0; E(0) = 0 whatever the row)
-            const uint8_t* grow = cs.GI[kind_prev][kind][l > 0 ? sv[l - 1] : 0];
-            const uint8_t* grow2 = cs.GI[kind_pp][kind_prev][l > 1 ? tv[l - 2] : 0];
+          if (two && l > 0) {                                // sweep 2's next row: T[l-1][s2_{l-2}][.]
+            const uint8_t* grow2 = cs.GI[kind_pp][kind_prev][s2];
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const int c = 32 * q + lane;
-              if (c < FK) {
-                stash[c] = VPc[c] + Gc[grow[c]];
-                if (two && l > 0) stash2[c] = VPp[c] + Gp[grow2[c]];
-              }
+              if (c < FK) stash2[c] = VPp[c] + Gp[grow2[c]];
             }
-            __syncwarp();
           }
           if (l == L - 1) {                                  // the chain ends: the updates that have no later tile
+            const uint8_t* grow = cs.GI[kind_prev][kind][s1];
             int64_t bv = INT64_MAX;
             int bi = FK;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {                    // sweep 1, last layer: no right neighbour
               const int c = 32 * q + lane;
-              if (c < FK && stash[c] < bv) { bv = stash[c]; bi = c; }
+              if (c < FK) {
+                const int64_t g = VPc[c] + Gc[grow[c]];
+                if (g < bv) { bv = g; bi = c; }
+              }
             }
             warp_argmin64(bv, bi);
             if (lane == 0) sv[l] = (uint8_t)bi;
-            __syncwarp();
             if (two) {
+              int s2m = 0;                                   // s2_{L-2}
               if (l > 0) {                                   // sweep 2, layer L-2: column from this (last) tile given s1_{L-1}
-                const uint8_t* gcol = &cs.GI[kind_prev][kind][0][sv[l]];
+                const uint8_t* gcol = &cs.GI[kind_prev][kind][0][bi];
                 bv = INT64_MAX;
                 bi = FK;
 #pragma unroll
@@ -551,9 +557,9 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
                 }
                 warp_argmin64(bv, bi);
                 if (lane == 0) tv[l - 1] = (uint8_t)bi;
-                __syncwarp();
+                s2m = bi;
               }
-              const uint8_t* grow2 = cs.GI[kind_prev][kind][l > 0 ? tv[l - 1] : 0];   // sweep 2, last layer
+              const uint8_t* grow2 = cs.GI[kind_prev][kind][s2m];   // sweep 2, last layer
               bv = INT64_MAX;
               bi = FK;
 #pragma unroll
@@ -566,7 +572,6 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
               }
               warp_argmin64(bv, bi);
               if (lane == 0) tv[l] = (uint8_t)bi;
-              __syncwarp();
             }
           }
         }
@@ -578,7 +583,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
 
     // ---- end of the chain: smallest argmin of f_{L-1}, back-track, results --------------------------------------------
     {
-      const int64_t* f = ws.f[cur];
+      const int64_t* f = ws.f;
       int64_t bv = f[lane];
       int bi = lane;
       if (lane < FK - 32) {
@@ -644,9 +649,9 @@ constexpr int kMaxWarps = 28;
 constexpr size_t kSmemBudget = 226 * 1024;
 
 // per-warp shared memory: tile factors, DP state, (CD) row stashes and strategies of two sweeps, (optionally) back-pointers
-size_t warp_bytes(int32_t L, int32_t S, bool bp_smem, bool two = true) {
-  const size_t cd = S > 0 ? (((size_t)2 * S * L + 15) & ~(size_t)15) + (size_t)2 * S * FK * 8 : 0;
-  return ((two ? sizeof(WarpShared<2>) : sizeof(WarpShared<1>)) + cd + (bp_smem ? (size_t)L * FK : 0) + 127) & ~(size_t)127;
+size_t warp_bytes(int32_t L, int32_t S, bool bp_smem) {
+  const size_t cd = S > 0 ? (((size_t)2 * S * L + 15) & ~(size_t)15) + (size_t)S * FK * 8 : 0;
+  return ((S > 0 ? sizeof(WarpShared<2>) : sizeof(WarpShared<1>)) + cd + (bp_smem ? (size_t)L * FK : 0) + 127) & ~(size_t)127;
 }
 size_t fixed_bytes() { return (sizeof(CtaShared) + 127) & ~(size_t)127; }
 
@@ -656,7 +661,7 @@ bool fused_build_dp_supported(const MeshParams& mp, int32_t L) { return mp.ndim 
 
 // largest S for which the first two CD sweeps ride in the fused kernel (row stashes and strategies in shared memory)
 bool fused_cd_sweep_supported(int32_t L, int32_t S) {
-  return S >= 1 && S <= kMaxFusedStarts && fixed_bytes() + 4 * warp_bytes(L, S, false, true) <= kSmemBudget;
+  return S >= 1 && S <= kMaxFusedStarts && fixed_bytes() + 4 * warp_bytes(L, S, false) <= kSmemBudget;
 }
 
 // workspace for the back-pointers [L][36] of the chains in flight (one slice per warp) when they do not fit beside the
@@ -681,18 +686,18 @@ int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   const size_t fixed = fixed_bytes();
   // one CTA per SM on every SM; warps per CTA: the fewest that reach the minimal number of rounds of chains per warp
   const int grid = Bp < sms ? Bp : sms;
-  int wmax = (int)((kSmemBudget - fixed) / warp_bytes(L, cdS, false, two));
+  int wmax = (int)((kSmemBudget - fixed) / warp_bytes(L, cdS, false));
   if (wmax > kMaxWarps) wmax = kMaxWarps;
   if (wmax < 1) { set_error("fused build+DP: chain too long for shared memory"); return AUTODDL_EINVAL; }
   const int rounds = (Bp + grid * wmax - 1) / (grid * wmax);
   int W = (Bp + grid * rounds - 1) / (grid * rounds);
   if (W > wmax) W = wmax;
   if (W < 1) W = 1;
-  const bool bp_smem = fixed + (size_t)W * warp_bytes(L, cdS, true, two) <= kSmemBudget;   // else a workspace slice per warp
+  const bool bp_smem = fixed + (size_t)W * warp_bytes(L, cdS, true) <= kSmemBudget;   // else a workspace slice per warp
   if (!bp_smem && d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
-  const size_t per_warp = warp_bytes(L, cdS, bp_smem, two);
+  const size_t per_warp = warp_bytes(L, cdS, bp_smem);
   const size_t smem = fixed + (size_t)W * per_warp;
-  auto kern = two ? fused_chain36_kernel<2> : fused_chain36_kernel<1>;
+  auto kern = cdS > 0 ? fused_chain36_kernel<2> : fused_chain36_kernel<1>;   // CD reads the previous layer's factors
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, bp_smem ? nullptr : d_bp,
                                    d_cd_init, cdS, d_cd_s1, two ? d_cd_s2 : nullptr, (int)per_warp);
