@@ -244,6 +244,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   const int64_t r_p = mp.size[role_d], r_alpha = mp.alpha[role_d], r_beta = mp.beta[role_d];
   const uint64_t r_magic = mp.magic_size[role_d];
   const int64_t cap_layer = mp.mem_cap / L;
+  const bool capped = mp.mem_cap != 0;                     // no cap: the memory model is not evaluated
   // chain DP: lane (b, half)
   const int dp_b = lane & 15, dp_h = lane >> 4;
 
@@ -302,7 +303,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           ws.WAR[role_d][role_cfg] =
               r_p > 1 ? (2 * r_p - 1) * r_alpha + 2 * (r_p - 1) * cdiv_magic(n, (uint32_t)r_p, r_magic) * r_beta : 0;
         }
-      } else if (lane < 27) {
+      } else if (lane < 27 && capped) {                      // local sizes of W and O: the memory model only
         ws.locW[role_cfg] = ws.Q[1][role_m0] * ws.Q[2][role_m1];
         ws.locO[role_cfg] = ws.Q[0][role_m0] * ws.Q[2][role_m1];
       }
@@ -320,12 +321,14 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
 #pragma unroll
               for (int d = 0; d < FD; ++d)
                 if (si.wB >> d & 1) v += ws.WAR[d][si.cfgW];
-              mem = ws.locW[si.cfgW] * (int64_t)rec.wsb;
             }
-            mem += (ws.Q[3][si.mI0] * ws.Q[4][si.mI1] + ws.locO[si.cfgO]) * (int64_t)rec.eb;
+            if (capped) {                                    // R6: weight state + input + output of the layer
+              if (kind == AUTODDL_GEMM) mem = ws.locW[si.cfgW] * (int64_t)rec.wsb;
+              mem += (ws.Q[3][si.mI0] * ws.Q[4][si.mI1] + ws.locO[si.cfgO]) * (int64_t)rec.eb;
+            }
           }
           const bool ok = si.valid && si.allowed && si.rowsplit <= rec.maxr && si.colsplit <= rec.maxc &&
-                          (mp.mem_cap == 0 || mem <= cap_layer);
+                          (!capped || mem <= cap_layer);
           VPc[j] = v + (ok ? 0 : AUTODDL_PEN);
           if (node) node[tile * FK + j] = v;
           if (mask) mask[tile * FK + j] = ok ? 1 : 0;
