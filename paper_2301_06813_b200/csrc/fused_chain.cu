@@ -44,6 +44,8 @@ struct CtaShared {
   SigInfo sig[2][FK];
   uint8_t bcls[2][FK];                                    // per consumer kind: B(j) in 0..16 (16 = invalid for the kind)
   uint8_t ucls[16];                                       // class of a level's (a_d, b_d)
+  uint8_t ucol[FNU], uhi[FNU];                            // (copies of c_ucol, c_uhi, c_walk: per-thread indices are slow
+  uint32_t walk[16];                                      //  in constant memory)
   uint8_t nnz[FNU * FNU];                                 // per (u0, u1): number of summands
   uint32_t ew[2][FNU * FNU];                              // (set-up scratch: its summand words)
   int32_t nl, nh;                                         // entries of 1..4 summands (ranks 0..nl-1), of more (nl..nl+nh-1)
@@ -122,18 +124,20 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
 
   // ---- once per CTA: facts per (layer kind, signature), the layout of G, the index tables ---------------------------
   fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
-  if (tid < 16) {                                          // class of (a_d, b_d) = rank of its (forward, backward) walk pair
-    auto key = [](int x) { return c_walk.w[x] | c_walk.w[dual_of(x & 3) * 4 + dual_of(x >> 2)] << 11; };
-    const uint32_t mine = key(tid);
-    int rep = tid, id = 0;
-    for (int y = tid - 1; y >= 0; --y)
-      if (key(y) == mine) rep = y;
-    for (int y = 0; y < rep; ++y) {
-      bool first = true;
-      for (int z = 0; z < y; ++z) first = first && key(z) != key(y);
-      id += first;
-    }
-    cs.ucls[tid] = (uint8_t)id;
+  if (tid >= 32 && tid < 48) cs.walk[tid - 32] = c_walk.w[tid - 32];
+  if (tid >= 64 && tid < 64 + FNU) { cs.ucol[tid - 64] = c_ucol[tid - 64]; cs.uhi[tid - 64] = c_uhi[tid - 64]; }
+  if (blockDim.x < 96 && tid < 16) {                       // (a CTA of one or two warps)
+    cs.walk[tid] = c_walk.w[tid];
+    if (tid < FNU) { cs.ucol[tid] = c_ucol[tid]; cs.uhi[tid] = c_uhi[tid]; }
+  }
+  if (tid < 32) {                                          // class of (a_d, b_d) = rank of its (forward, backward) walk pair
+    const int x = tid & 15;
+    const uint32_t key = c_walk.w[x] | c_walk.w[dual_of(x & 3) * 4 + dual_of(x >> 2)] << 11;
+    int rep = x;                                           // first pair with the same walks
+    for (int y = 15; y >= 0; --y)
+      if (__shfl_sync(0xffffffffu, key, y) == key) rep = y;
+    const uint32_t firsts = __ballot_sync(0xffffffffu, tid < 16 && rep == x);
+    if (tid < 16) cs.ucls[x] = (uint8_t)__popc(firsts & ((1u << rep) - 1));
   }
   for (int x = tid; x < 5 * 32; x += blockDim.x) (&cs.lslot[0][0])[x] = FNC | FNC << 6 | FNC << 12 | FNC << 18;   // zero slots (lslot, hslot)
   __syncthreads();
@@ -159,9 +163,9 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           ++n;
         }
     };
-    r_slots<FD>(a, b, idx);
+    r_slots<FD>(a, b, idx, cs.walk);
     take();
-    r_slots<FD>(dual_vec<FD>(b), dual_vec<FD>(a), idx);
+    r_slots<FD>(dual_vec<FD>(b), dual_vec<FD>(a), idx, cs.walk);
     take();
     return n;
   };
@@ -175,7 +179,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     const SigInfo& si = cs.sig[x / FK][x % FK];
     cs.bcls[x / FK][x % FK] = (uint8_t)(si.b_idx >= 0 ? si.b_idx : FNS);
   }
-  auto upos = [&](int u0, int u1) -> int { return 16 * (3 * c_uhi[u0] + c_uhi[u1]) + 4 * c_ucol[u0] + c_ucol[u1]; };
+  auto upos = [&](int u0, int u1) -> int { return 16 * (3 * cs.uhi[u0] + cs.uhi[u1]) + 4 * cs.ucol[u0] + cs.ucol[u1]; };
   auto gp = [&](int a, int b) -> int {                     // position of Esym[a][b]; a = 16 / b < 0: invalid signature, zero
     if (a >= FNS || b < 0 || b >= FNS) return FGZ;
     return upos(cs.ucls[(a >> 2) << 2 | (b >> 2)], cs.ucls[(a & 3) << 2 | (b & 3)]);
