@@ -238,15 +238,22 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
   warp_init();
   // step 1: lane (x, m) for lane < 20
   const int q_x = lane >> 2, q_m = lane & 3;
-  const uint32_t q_sub = (uint32_t)mp.sub[q_m];
-  const uint64_t q_magic = mp.magic_sub[q_m];
+  // (selects between statically indexed parameters: a per-lane index into the parameter space costs a load per use)
+  const uint32_t q_sub = (uint32_t)(q_m == 0 ? mp.sub[0] : (q_m == 1 ? mp.sub[1] : (q_m == 2 ? mp.sub[2] : mp.sub[3])));
+  const uint64_t q_magic = q_m == 0 ? mp.magic_sub[0] : (q_m == 1 ? mp.magic_sub[1] : (q_m == 2 ? mp.magic_sub[2] : mp.magic_sub[3]));
+  // every level size a power of two (the usual machine): ceil(n / d) is an add and a shift
+  const bool pow2 = ((mp.size[0] & (mp.size[0] - 1)) | (mp.size[1] & (mp.size[1] - 1))) == 0;
+  const int q_sh = 31 - __clz((int)q_sub);
   // step 2: lanes 0..17 = (level, split configuration) for the input tensor and the weight gradient; lanes 18..26 = local sizes
   const int role_i = lane < 18 ? lane : lane - 18;
   const int role_d = lane < 18 ? role_i / FNC : 0, role_cfg = role_i % FNC;
   int role_m0 = 0, role_m1 = 0;
   cfg_masks<FD>(role_cfg, role_m0, role_m1);
-  const int64_t r_p = mp.size[role_d], r_alpha = mp.alpha[role_d], r_beta = mp.beta[role_d];
-  const uint64_t r_magic = mp.magic_size[role_d];
+  const int64_t r_p = role_d ? mp.size[1] : mp.size[0], r_alpha = role_d ? mp.alpha[1] : mp.alpha[0],
+                r_beta = role_d ? mp.beta[1] : mp.beta[0];
+  const uint64_t r_magic = role_d ? mp.magic_size[1] : mp.magic_size[0];
+  const int r_sh = 31 - __clz((int)r_p);
+  auto cdiv_p = [&](int64_t n) -> int64_t { return pow2 ? (n + r_p - 1) >> r_sh : cdiv_magic(n, (uint32_t)r_p, r_magic); };
   const int64_t cap_layer = mp.mem_cap / L;
   const bool capped = mp.mem_cap != 0;                     // no cap: the memory model is not evaluated
   // chain DP: lane (b, half)
@@ -287,7 +294,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       const int64_t* const VPp = ws.VP[(l & (NB - 1)) ^ (NB - 1)];
 
       // ---- 1. Q[x][m] = ceil(extent x / product of the levels in m) -------------------------------------------------
-      if (lane < 20) ws.Q[q_x][q_m] = cdiv_magic(rec.X[q_x], q_sub, q_magic);
+      if (lane < 20) ws.Q[q_x][q_m] = pow2 ? (rec.X[q_x] + q_sub - 1) >> q_sh : cdiv_magic(rec.X[q_x], q_sub, q_magic);
       __syncwarp();
 
       // ---- 2. Table 2 per level and split configuration -------------------------------------------
@@ -296,7 +303,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           const int64_t n = ws.Q[3][role_m0] * ws.Q[4][role_m1] * (int64_t)rec.eb;
           int64_t cg = 0, ca = 0;
           if (r_p > 1) {
-            cg = mp.accum * ((r_p - 1) * (r_alpha + cdiv_magic(n, (uint32_t)r_p, r_magic) * r_beta));
+            cg = mp.accum * ((r_p - 1) * (r_alpha + cdiv_p(n) * r_beta));
             ca = mp.accum * ((r_p - 1) * r_alpha + n * r_beta);          // R25: once per micro-batch
           }
           ws.TAB[role_d * FSTRIDE + role_cfg] = cg;
@@ -305,7 +312,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
         if (kind == AUTODDL_GEMM) {                          // weight gradient: the AllReduce row
           const int64_t n = ws.Q[1][role_m0] * ws.Q[2][role_m1] * (int64_t)rec.wgb;
           ws.WAR[role_d][role_cfg] =
-              r_p > 1 ? (2 * r_p - 1) * r_alpha + 2 * (r_p - 1) * cdiv_magic(n, (uint32_t)r_p, r_magic) * r_beta : 0;
+              r_p > 1 ? (2 * r_p - 1) * r_alpha + 2 * (r_p - 1) * cdiv_p(n) * r_beta : 0;
         }
       } else if (lane < 27 && capped) {                      // local sizes of W and O: the memory model only
         ws.locW[role_cfg] = ws.Q[1][role_m0] * ws.Q[2][role_m1];
@@ -393,15 +400,20 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
           }
         }
         {
-          const longlong2 vpa = *reinterpret_cast<const longlong2*>(&VPc[32]);
-          const longlong2 vpb = *reinterpret_cast<const longlong2*>(&VPc[34]);
+          // columns 32..35: lane (class row (c0, c1), column pair) computes its 16 bytes once and stores them to the 1, 3
+          // or 9 rows of the class
+          const int c0 = lane >> 3, c1 = lane >> 1 & 3, cp = 32 + 2 * (lane & 1);
+          const int d0 = c0 < 2 ? c0 : (c0 == 2 ? 3 : 2), d1 = c1 < 2 ? c1 : (c1 == 2 ? 3 : 2);
+          const longlong2 vp = *reinterpret_cast<const longlong2*>(&VPc[cp]);
+          const uint32_t gi = *reinterpret_cast<const uint16_t*>(&cs.GI[kind_prev][kind][d0 * 6 + d1][cp]);
+          const longlong2 v = make_longlong2(vp.x + Gc[gi & 255], vp.y + Gc[gi >> 8]);
+          int64_t* o = out + cp;
 #pragma unroll
-          for (int i0 = 0; i0 < 64; i0 += 32) {
-            const int i = i0 + lane;
-            if (i < FK) {
-              const uint32_t gi = *reinterpret_cast<const uint32_t*>(&cs.GI[kind_prev][kind][i][32]);
-              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 32), make_longlong2(vpa.x + Gc[gi & 255], vpa.y + Gc[gi >> 8 & 255]));
-              __stcs(reinterpret_cast<longlong2*>(out + i * FK + 34), make_longlong2(vpb.x + Gc[gi >> 16 & 255], vpb.y + Gc[gi >> 24]));
+          for (int m0 = 0; m0 < 3; ++m0) {
+#pragma unroll
+            for (int m1 = 0; m1 < 3; ++m1) {
+              const int r0 = m0 == 0 ? d0 : 3 + m0, r1 = m1 == 0 ? d1 : 3 + m1;          // class 3 = digits 2, 4, 5
+              if ((m0 == 0 || c0 == 3) && (m1 == 0 || c1 == 3)) __stcs(reinterpret_cast<longlong2*>(o + (r0 * 6 + r1) * FK), v);
             }
           }
         }
