@@ -3,9 +3,9 @@
 
 One "step" = one pass of the whole hot path over one batch of synthetic input:
   (a1) cost tables -> (a2) chain DP -> (a3) coordinate descent
-run through the library's one-call entry point autoddl_search: (a1) + (a2) + the first sweep of (a3) as ONE fused
-kernel (tiles built in shared memory, TMA-stored to HBM, consumed by the DP and the CD sweep from shared memory),
-then the CD kernel from sweep 3.  The three
+run through the library's one-call entry point autoddl_search: (a1) + (a2) + the first two sweeps of (a3) as ONE
+fused kernel (one warp per chain: a tile's factors are evaluated in shared memory, expanded to HBM with 16-byte
+streaming stores, and consumed by the DP and the CD sweeps from shared memory), then the CD kernel from sweep 3.  The three
 stand-alone kernels (autoddl_build_tables, autoddl_chain_dp, autoddl_coord_descent) are timed in the same run
 and reported under "kernels" / "parts" (the three numbers BASELINE.json's metric names).
 Workload: BASELINE.json configs[3] (4096 independent chains x 64 GEMM layers, mesh 4 x 4, K = 36), the
@@ -405,7 +405,7 @@ def run_ours(args):
         cd_alg_bytes = total_sweeps * 16 * K * L
         sweep1_bytes = fused_sweeps * 16 * K * L             # CD work done inside the fused launch (sweeps 1 and 2)
         # Bytes that MUST reach HBM per launch (what "roofline" means here): the fused kernel writes the tables (8 B per
-        # cell) and reads 64 B per layer record; the chain DP and the first CD sweep run from shared memory and move
+        # cell) and reads 64 B per layer record; the chain DP and the first two CD sweeps run from shared memory and move
         # nothing.  SURVEY 8(d)'s per-unit figures (8 B/cell written + 8 B/cell read by the DP + 16 K L B per CD sweep)
         # count WORK; for the fused launch their sum is reported separately as work_units_*: it exceeds the HBM bytes
         # because fusion removed two of the three streams.
@@ -415,9 +415,9 @@ def run_ours(args):
             "build_dp_cd1_fused": {"ms": ms["fused"], "cells_per_s": cells / (ms["fused"] * 1e-3),
                                    "hbm_GBps": fused_hbm / (ms["fused"] * 1e-3) / 1e9,
                                    "work_units_GBps": fused_work / (ms["fused"] * 1e-3) / 1e9, "in_step": True,
-                                   "bound": "shared-memory bandwidth / issue (ncu: LSU wavefronts 75 %, issue 67 %); hbm traffic = "
-                                            "the 8 B/cell table write only (DP and the first CD sweep read the tile factors from "
-                                            "shared memory)"},
+                                   "bound": "LSU data pipe (shared-memory loads + the global stores: ncu 81 %) / issue (67 %); hbm traffic "
+                                            "= the 8 B/cell table write only (DP and the first two CD sweeps read the tile factors "
+                                            "from shared memory)"},
             "coord_descent_resume": {"ms": ms["cd_resume"], "sweeps": total_sweeps - fused_sweeps,
                                      "sweeps_per_s": (total_sweeps - fused_sweeps) / (ms["cd_resume"] * 1e-3),
                                      "hbm_GBps": (cd_alg_bytes - sweep1_bytes) / (ms["cd_resume"] * 1e-3) / 1e9, "in_step": True,
@@ -472,7 +472,7 @@ def run_ours(args):
                          "work_units_frac": kernels[dom].get("work_units_frac_of_peak"),
                          "note": "frac = bytes that must reach HBM per launch (8 B per cell written + 64 B per layer record read) / "
                                  "CUDA-event launch time / peak; work_units_frac counts SURVEY 8(d)'s per-unit bytes for all the work "
-                                 "the fused launch does (tables + DP + one CD sweep) and can exceed 1"},
+                                 "the fused launch does (tables + DP + two CD sweeps) and can exceed 1"},
             "e2e": {"value": world * cells / (e2e_ms * 1e-3), "unit": "cells/s", "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": launches,
