@@ -180,9 +180,8 @@ template <int D>
 struct BrSmem {
   using F = Fac<D>;
   alignas(16) int64_t VP[F::K];
-  alignas(16) int64_t El[F::ES * F::ES + 1];               // Esym of layer l (overwritten by the class minima W)
+  alignas(16) int64_t El[F::ES * F::ES + 1];               // Esym of layer l (overwritten by the class minima W, as keys)
   alignas(16) int64_t Er[F::ES * F::ES + 1];               // Esym of layer l + 1
-  uint8_t Wc[F::ES * F::ES];                               // candidate attaining W[a][alpha]
   SigInfo sig[2][F::K];
   uint8_t acls[2][F::K], bcls[2][F::K];
   uint8_t mstart[2][F::ES + 1], mlist[2][F::K];            // per kind: the candidates of every producer class alpha, ascending
@@ -199,6 +198,7 @@ __global__ void __launch_bounds__(512) best_response_kernel(const int64_t* __res
   using F = Fac<D>;
   constexpr int K = F::K, ES = F::ES, CS = F::CS, NT = 512, NW = (ES * ES + NT - 1) / NT;
   constexpr int64_t kNone = (int64_t)1 << 61;             // no candidate in the class (real sums stay below 2^53)
+  constexpr int64_t kNoneKey = (int64_t)1 << 62;
   extern __shared__ __align__(16) unsigned char br_raw[];
   BrSmem<D>& sm = *reinterpret_cast<BrSmem<D>*>(br_raw);
   const int tid = threadIdx.x;
@@ -206,11 +206,13 @@ __global__ void __launch_bounds__(512) best_response_kernel(const int64_t* __res
   __syncthreads();
   fill_classes<D>(sm.acls, sm.bcls, sm.sig, tid, NT);
   __syncthreads();
-  if (tid < 2 * ES) {                                      // candidates per producer class, ascending: count, prefix, fill
-    const int kind = tid / ES, al = tid % ES;
+  // candidates per producer class, ascending: count, prefix, fill -- a warp per (kind, class), 32 candidates per ballot
+  const int lane = tid & 31, warp = tid >> 5;
+  for (int pr = warp; pr < 2 * ES; pr += NT / 32) {
+    const int kind = pr / ES, al = pr % ES;
     int n = 0;
-    for (int c = 0; c < K; ++c) n += sm.acls[kind][c] == al;
-    sm.mstart[kind][al + 1] = (uint8_t)n;                  // (counts for now)
+    for (int c0 = 0; c0 < K; c0 += 32) n += __popc(__ballot_sync(0xffffffffu, c0 + lane < K && sm.acls[kind][c0 + lane] == al));
+    if (lane == 0) sm.mstart[kind][al + 1] = (uint8_t)n;   // (counts for now)
   }
   __syncthreads();
   if (tid < 2) {
@@ -219,11 +221,15 @@ __global__ void __launch_bounds__(512) best_response_kernel(const int64_t* __res
     for (int al = 0; al < ES; ++al) { n += sm.mstart[tid][al + 1]; sm.mstart[tid][al + 1] = (uint8_t)n; }
   }
   __syncthreads();
-  if (tid < 2 * ES) {
-    const int kind = tid / ES, al = tid % ES;
+  for (int pr = warp; pr < 2 * ES; pr += NT / 32) {
+    const int kind = pr / ES, al = pr % ES;
     int n = sm.mstart[kind][al];
-    for (int c = 0; c < K; ++c)
-      if (sm.acls[kind][c] == al) sm.mlist[kind][n++] = (uint8_t)c;
+    for (int c0 = 0; c0 < K; c0 += 32) {
+      const bool mine = c0 + lane < K && sm.acls[kind][c0 + lane] == al;
+      const uint32_t m = __ballot_sync(0xffffffffu, mine);
+      if (mine) sm.mlist[kind][n + __popc(m & ((1u << lane) - 1))] = (uint8_t)(c0 + lane);
+      n += __popc(m);
+    }
   }
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int l = tile % L;
@@ -244,49 +250,81 @@ __global__ void __launch_bounds__(512) best_response_kernel(const int64_t* __res
     const uint8_t* bc = sm.bcls[kind];                     // tile l and A(c) as producers of tile l + 1
     const uint8_t* ms = sm.mstart[kind];
     const uint8_t* ml = sm.mlist[kind];
-    // W[a][alpha] into registers (the rows of El are still being read), then over El
-    int64_t wv[NW];
-    uint8_t wc[NW];
+    // W[a][alpha] = min over the candidates c of producer class alpha of VP[c] + El[a][B(c)], smallest c on ties, as the key
+    // W * 256 + c (sums stay below 2^53) -- into registers (the rows of El are still being read), then over El.  A warp
+    // takes one class alpha and 32 rows a: its lanes walk the same candidate list.  The candidates that are invalid for
+    // the kind (class ES - 1) all carry 2^50 and the zero edge: the first one wins.
+    int64_t wk[NW];
 #pragma unroll
     for (int q = 0; q < NW; ++q) {
       const int x = tid + q * NT;
-      wv[q] = kNone;
-      wc[q] = 255;
+      wk[q] = kNoneKey;
       if (x < ES * ES) {
-        const int a = x / ES, al = x % ES;
+        const int al = x / ES, a = x % ES;
         const int64_t* row = sm.El + a * ES;
-        for (int m = ms[al]; m < ms[al + 1]; ++m) {
+        const int m0 = ms[al], m1 = al == ES - 1 ? (ms[al + 1] > m0 ? m0 + 1 : m0) : ms[al + 1];
+        int64_t wv = kNone;
+        int wc = 255;
+        for (int m = m0; m < m1; ++m) {
           const int c = ml[m];
           const int64_t g = sm.VP[c] + row[bc[c]];
-          if (g < wv[q]) { wv[q] = g; wc[q] = (uint8_t)c; }
+          if (g < wv) { wv = g; wc = c; }
         }
+        if (wc != 255) wk[q] = wv << 8 | wc;
       }
     }
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < NW; ++q) {
       const int x = tid + q * NT;
-      if (x < ES * ES) { sm.El[x] = wv[q]; sm.Wc[x] = wc[q]; }
+      if (x < ES * ES) {
+        sm.El[x % ES * ES + x / ES] = wk[q];
+        sm.Er[x] <<= 8;                                    // the right edge in key units
+      }
     }
     __syncthreads();
+    // BR[a][b] = argmin over alpha of W[a][alpha] + Er[alpha][b]: (value, candidate) lexicographic = plain min of the keys
+    // (an empty class carries 2^62: it never wins).  Thread (ta, tb) owns the R x R outputs (ta + T i, tb + T j): R loads
+    // of W and R of Er per alpha for R^2 sums; lanes run along b: the Er loads are conflict-free, the W loads broadcasts.
     const uint8_t* ac = sm.acls[kind];
     uint8_t* out = BRt + (size_t)tile * ES * CS;
-    for (int x = tid; x < ES * ES; x += NT) {
-      const int a = x / ES, b = x % ES;                    // consecutive b: W[a][.] is a broadcast, Er[.][b] conflict-free
-      const int64_t* w = sm.El + a * ES;
-      const uint8_t* wcand = sm.Wc + a * ES;
-      const int64_t* col = sm.Er + b;
-      int64_t best = INT64_MAX;
-      int arg = 255;
+    constexpr int R = D == 3 ? 3 : 1, T = (ES + R - 1) / R;
+    static_assert(T * T <= NT, "one pass");
+    if (tid < T * T) {
+      const int ta = tid / T, tb = tid % T;
+      int64_t best[R][R];
+      int ao[R], bo[R];
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        ao[i] = (ta + T * i < ES ? ta + T * i : ES - 1) * ES;        // (clamped: the value is dropped below)
+        bo[i] = tb + T * i < ES ? tb + T * i : ES - 1;
+#pragma unroll
+        for (int j = 0; j < R; ++j) best[i][j] = INT64_MAX;
+      }
+#pragma unroll 5
       for (int al = 0; al < ES; ++al) {
-        const int64_t g = w[al] + col[al * ES];            // (an empty class carries 2^61: it never wins)
-        if (g <= best) {
-          const int c = wcand[al];
-          if (g < best || c < arg) { best = g; arg = c; }
-        }
+        int64_t wv[R], cv[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) { wv[i] = sm.El[ao[i] + al]; cv[i] = sm.Er[al * ES + bo[i]]; }
+#pragma unroll
+        for (int i = 0; i < R; ++i)
+#pragma unroll
+          for (int j = 0; j < R; ++j) {
+            const int64_t g = wv[i] + cv[j];
+            best[i][j] = g < best[i][j] ? g : best[i][j];
+          }
       }
       // the entry: the candidate and the producer class it presents to layer l + 1 (the next look-up's row)
-      reinterpret_cast<uint16_t*>(out + b * CS)[a] = (uint16_t)(arg | ac[arg] << 8);
+#pragma unroll
+      for (int i = 0; i < R; ++i)
+#pragma unroll
+        for (int j = 0; j < R; ++j) {
+          const int a = ta + T * i, b2 = tb + T * j;
+          if (a < ES && b2 < ES) {
+            const int arg = (int)(best[i][j] & 255);
+            reinterpret_cast<uint16_t*>(out + b2 * CS)[a] = (uint16_t)(arg | ac[arg] << 8);
+          }
+        }
     }
   }
 }
