@@ -197,7 +197,10 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   if (validate_mesh_net(mesh, nullptr, &mp) || Bp < 1 || L < 1 || S < 0) return 0;
   const int64_t K = mesh_num_sigs(mesh);
   size_t b = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K);
-  if (cd_lookup_supported(mp, L, S)) b += factors_bytes(mp, Bp, L) + cd_lookup_workspace_bytes(mp, Bp, L) + 256;   // many starts: factors, best responses
+  const bool scan = chain_dp_scan_supported(mp, Bp, L);
+  if (scan || cd_lookup_supported(mp, L, S)) b += factors_bytes(mp, Bp, L) + 256;
+  if (scan) b += chain_dp_scan_bytes(mp, Bp, L);           // few long chains: the DP in class space, parallel over the layers
+  if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L) + 256;   // many starts: best responses
   if (mesh->ndim == 2) b += fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256;   // fused kernel: back-pointers, strategies after sweep 1
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
   b += align_up((size_t)Bp * L * sizeof(autoddl_layer), 256);
@@ -247,6 +250,15 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
     if ((rc = check_device())) return rc;
     return launch_build_dp_fused(d_layers, Bp, L, mp, nullptr, nullptr, nullptr, d_opt_cost, d_strategy, (uint8_t*)d_work,
                                  nullptr, 0, nullptr, nullptr, st);
+  }
+  if (!d_T && chain_dp_scan_supported(mp, Bp, L)) {
+    // few long chains, no table wanted: the factors (2.6 / 35.6 KB per layer) and the DP in class space on them
+    const size_t fbytes = factors_bytes(mp, Bp, L);
+    if (d_work != nullptr && work_bytes >= fbytes + chain_dp_scan_bytes(mp, Bp, L)) {
+      if ((rc = check_device())) return rc;
+      if ((rc = launch_build_factors(d_layers, Bp, L, mp, (int64_t*)d_work, st))) return rc;
+      return launch_chain_dp_scan((const int64_t*)d_work, Bp, L, mp, (unsigned char*)d_work + fbytes, d_opt_cost, d_strategy, st);
+    }
   }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
   if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
@@ -354,8 +366,31 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, cd_resume, true, d_cd_prev);
   }
 
-  // ---- few chains, or another mesh: separate kernels.  The DP reads the K x K tables; CD from >= 32 starts on two / three
-  // mesh levels runs on the factors and their best-response tables instead (no table gather).
+  // ---- few chains, or another mesh: separate kernels.  Few long chains on two / three mesh levels take the DP in class space
+  // on the factors (parallel over the layers); CD from >= 32 starts runs on the factors and their best-response tables.  A
+  // K x K table is built only when the caller wants it (d_T, d_node, d_mask) or a kernel that reads it runs.
+  const bool lookup = do_cd && cd_lookup_supported(mp, L, S);
+  {
+    const bool want_T = d_T != nullptr || d_node != nullptr || d_mask != nullptr || (do_cd && !lookup);
+    const size_t tb = want_T && !d_T ? table_bytes(Bp, L, K) : 0, fbytes = factors_bytes(mp, Bp, L);
+    const size_t sb = chain_dp_scan_supported(mp, Bp, L) ? chain_dp_scan_bytes(mp, Bp, L) : 0;
+    const size_t brb = lookup ? cd_lookup_workspace_bytes(mp, Bp, L) : 0;
+    if (sb && d_work != nullptr && work_bytes >= tb + fbytes + sb + brb) {
+      int64_t* d_F = (int64_t*)(d_work + tb);
+      if (want_T) {
+        if (!d_T) d_T = (int64_t*)d_work;
+        if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
+      }
+      if ((rc = launch_build_factors(d_layers, Bp, L, mp, d_F, st))) return rc;
+      if ((rc = launch_chain_dp_scan(d_F, Bp, L, mp, d_work + tb + fbytes, d_opt_cost, d_strategy, st))) return rc;
+      if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
+      if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
+      if (!do_cd) return AUTODDL_OK;
+      if (lookup)
+        return launch_cd_lookup(d_F, Bp, L, mp, d_work + tb + fbytes + sb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+      return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, false, true);
+    }
+  }
   const size_t tb = d_T ? 0 : table_bytes(Bp, L, K), bb = bp_bytes(Bp, L, K);
   if (tb + bb > 0 && (d_work == nullptr || work_bytes < tb + bb)) {
     set_error("search: workspace of %zu bytes needed, %zu given", tb + bb, d_work ? work_bytes : (size_t)0);
@@ -367,7 +402,7 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
   if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
   if (!do_cd) return AUTODDL_OK;
-  if (cd_lookup_supported(mp, L, S)) {
+  if (lookup) {
     const size_t off = align_up(tb + bb, 256), fbytes = factors_bytes(mp, Bp, L);
     if (work_bytes >= off + fbytes + cd_lookup_workspace_bytes(mp, Bp, L)) {
       if ((rc = launch_build_factors(d_layers, Bp, L, mp, (int64_t*)(d_work + off), st))) return rc;
@@ -430,7 +465,9 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
   auto carve = [&](size_t bytes) { unsigned char* p = w; w += align_up(bytes, 256); return p; };
   size_t tables_region = table_bytes(Bp, L, K) + bp_bytes(Bp, L, K) +
                          (mesh->ndim == 2 ? fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256 : 0);
-  if (do_cd && cd_lookup_supported(mp, L, S)) tables_region += factors_bytes(mp, Bp, L) + cd_lookup_workspace_bytes(mp, Bp, L) + 512;
+  if (chain_dp_scan_supported(mp, Bp, L) || (do_cd && cd_lookup_supported(mp, L, S))) tables_region += factors_bytes(mp, Bp, L) + 256;
+  if (chain_dp_scan_supported(mp, Bp, L)) tables_region += chain_dp_scan_bytes(mp, Bp, L);
+  if (do_cd && cd_lookup_supported(mp, L, S)) tables_region += cd_lookup_workspace_bytes(mp, Bp, L) + 512;
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));
   int32_t* d_init = (int32_t*)carve((size_t)Bp * S * L * 4);
