@@ -31,6 +31,7 @@ template <int D> struct Fac {
   static constexpr int FB = (HDR + K + ES * ES + 1) / 2 * 2;   // int64 words per tile (16-byte multiple)
   static constexpr int CS = (2 * ES + 15) / 16 * 16;       // bytes per best-response column of ES 16-bit entries (16-byte multiple)
   static constexpr int N2P = (ES * ES + 1) / 2 * 2;        // words between two ES x ES class matrices (16-byte multiple)
+  static constexpr int SQ = (ES + 7) / 16 * 16 + 8;        // row stride of a chunk product Q: = 8 mod 16, see chunk_prefix_kernel
 };
 
 template <int D>
@@ -562,99 +563,118 @@ __global__ void __launch_bounds__(512) class_matrix_kernel(const int64_t* __rest
   }
 }
 
-// C = A (x) B on ES x ES min-plus matrices in shared memory: thread (ta, tb) owns the R x R outputs (ta + T i, tb + T j)
-template <int D, int NT>
-__device__ __forceinline__ void minplus_tile(const int64_t* __restrict__ A, const int64_t* __restrict__ B, int tid,
-                                             int64_t (&best)[D == 3 ? 3 : 1][D == 3 ? 3 : 1]) {
-  constexpr int ES = Fac<D>::ES, R = D == 3 ? 3 : 1, T = (ES + R - 1) / R;
-  static_assert(T * T <= NT, "one pass");
-  const int ta = tid / T, tb = tid % T;
-  int ao[R], bo[R];
-#pragma unroll
-  for (int i = 0; i < R; ++i) {
-    ao[i] = (ta + T * i < ES ? ta + T * i : ES - 1) * ES;  // (clamped: the value is dropped by the caller)
-    bo[i] = tb + T * i < ES ? tb + T * i : ES - 1;
-#pragma unroll
-    for (int j = 0; j < R; ++j) best[i][j] = INT64_MAX;
-  }
-  if (tid >= T * T) return;
-#pragma unroll 5
-  for (int k = 0; k < ES; ++k) {
-    int64_t av[R], bv[R];
-#pragma unroll
-    for (int i = 0; i < R; ++i) { av[i] = A[ao[i] + k]; bv[i] = B[k * ES + bo[i]]; }
-#pragma unroll
-    for (int i = 0; i < R; ++i)
-#pragma unroll
-      for (int j = 0; j < R; ++j) {
-        const int64_t g = av[i] + bv[j];
-        best[i][j] = g < best[i][j] ? g : best[i][j];
-      }
-  }
-}
-
-// 2. Q[p][c] = M_{t_c + 1} (x) ... (x) M_{t_c + len} for c = 0 .. C - 2 (grid.x = C - 1, grid.y = Bp); one TMA bulk copy per matrix
+// 2. Q[p][c] = M_{t_c + 1} (x) ... (x) M_{t_c + len} for c = 0 .. C - 2, evaluated from the right: a CTA owns a group of W
+// columns of the result, X = M_{t_c + len}[., cols], X <- M_k (x) X for k = t_c + len - 1 .. t_c + 1 -- the column groups of a
+// chunk never talk to each other (grid.x = C - 1, grid.y = Bp, grid.z = groups).  One TMA bulk copy per matrix, two in flight.
 template <int D>
-__global__ void __launch_bounds__(512) chunk_product_kernel(const int64_t* __restrict__ M, int L, int len, int64_t* __restrict__ Q) {
+struct ProdCfg {
+  static constexpr int ES = Fac<D>::ES;
+  static constexpr int NG = D == 3 ? 5 : 1;                // column groups
+  static constexpr int W = (ES + NG - 1) / NG;             // 13 / 17 columns each
+  static constexpr int RA = D == 3 ? 3 : 1, RJ = 1;        // outputs per thread: rows a + TA i, columns j + TJ k.  The loop
+  static constexpr int TA = (ES + RA - 1) / RA;            // is bound by shared-memory loads (RA + RJ per RA RJ sums) and by the
+  static constexpr int TJ = (W + RJ - 1) / RJ;             // 64-bit min (6 instructions); 3 x 1 measured best (3 x 3: too few
+  static constexpr int NT = (TA * TJ + 31) / 32 * 32;      // warps on the SM, 1 x 1: twice the loads): 288 / 320 threads
+};
+
+template <int D>
+__global__ void __launch_bounds__(ProdCfg<D>::NT) chunk_product_kernel(const int64_t* __restrict__ M, int L, int len, int64_t* __restrict__ Q) {
   using F = Fac<D>;
-  constexpr int ES = F::ES, NT = 512, R = D == 3 ? 3 : 1, T = (ES + R - 1) / R, N2 = ES * ES, N2P = F::N2P;
+  using PC = ProdCfg<D>;
+  constexpr int ES = F::ES, N2P = F::N2P, W = PC::W, RA = PC::RA, RJ = PC::RJ, TA = PC::TA, TJ = PC::TJ, NT = PC::NT;
   extern __shared__ __align__(128) unsigned char cp_raw[];
-  int64_t* A = reinterpret_cast<int64_t*>(cp_raw);         // [N2P], then two buffers for the right factor
-  int64_t* Bb = A + N2P;
-  __shared__ uint64_t bar[3];                              // A, B[0], B[1]
-  const int tid = threadIdx.x, c = blockIdx.x, p = blockIdx.y;
-  const int64_t* Mp = M + ((size_t)p * L + (size_t)c * len + 1) * N2P;     // M_{t_c + 1}
+  int64_t* Ab = reinterpret_cast<int64_t*>(cp_raw);        // two matrix buffers [N2P], then X [2][ES][W]
+  int64_t* X = Ab + 2 * N2P;
+  __shared__ uint64_t bar[2];
+  const int tid = threadIdx.x, c = blockIdx.x, p = blockIdx.y, col0 = blockIdx.z * W;
+  const int ncol = col0 + W <= ES ? W : ES - col0;
+  const int64_t* Mp = M + ((size_t)p * L + (size_t)c * len) * N2P;         // M_{t_c}; M_{t_c + k} = Mp + k N2P
   if (tid == 0) {
-    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1);
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1);
     mbar_fence_init();
   }
   __syncthreads();
   const uint64_t pol = policy_evict_first();
-  auto fetch = [&](int k) {                                // M_{t_c + 1 + k} into buffer k & 1 (thread 0)
-    mbar_arrive_expect_tx(&bar[1 + (k & 1)], N2P * 8);
-    bulk_g2s(Bb + (k & 1) * N2P, Mp + (size_t)k * N2P, N2P * 8, &bar[1 + (k & 1)], pol);
-  };
-  if (tid == 0) {
-    mbar_arrive_expect_tx(&bar[0], N2P * 8);
-    bulk_g2s(A, Mp, N2P * 8, &bar[0], pol);
-    if (len > 1) fetch(1);
-    if (len > 2) fetch(2);
-  }
-  mbar_wait(&bar[0], 0);
-  for (int k = 1; k < len; ++k) {
-    mbar_wait(&bar[1 + (k & 1)], ((k - 1) >> 1) & 1);      // the ((k - 1) / 2 + 1)-th use of the buffer
-    int64_t best[R][R];
-    minplus_tile<D, NT>(A, Bb + (k & 1) * N2P, tid, best);
-    __syncthreads();                                       // A and the buffer have been read by everyone
-    if (tid == 0 && k + 2 < len) fetch(k + 2);
-    if (tid < T * T) {
-      const int ta = tid / T, tb = tid % T;
-#pragma unroll
-      for (int i = 0; i < R; ++i)
-#pragma unroll
-        for (int j = 0; j < R; ++j)
-          if (ta + T * i < ES && tb + T * j < ES) A[(ta + T * i) * ES + tb + T * j] = best[i][j] < kInfCls ? best[i][j] : kInfCls;
+  // use u = 0, 1, ..: matrix k = len - u into buffer u & 1
+  auto fetch = [&](int u) {                                // thread 0
+    if (u < len) {
+      mbar_arrive_expect_tx(&bar[u & 1], N2P * 8);
+      bulk_g2s(Ab + (u & 1) * N2P, Mp + (size_t)(len - u) * N2P, N2P * 8, &bar[u & 1], pol);
     }
-    __syncthreads();
+  };
+  if (tid == 0) { fetch(0); fetch(1); }
+  mbar_wait(&bar[0], 0);
+  for (int x = tid; x < ES * W; x += NT) {                 // X = the CTA's columns of M_{t_c + len}
+    const int m = x / W, j = x % W;
+    X[x] = j < ncol ? Ab[m * ES + col0 + j] : kInfCls;
   }
-  int64_t* out = Q + ((size_t)p * gridDim.x + c) * N2P;
-  for (int x = tid; x < N2; x += NT) out[x] = A[x];
+  __syncthreads();
+  if (tid == 0) fetch(2);
+  const int ta = tid / TJ, tj = tid % TJ;
+  int cur = 0;
+  for (int u = 1; u < len; ++u) {
+    mbar_wait(&bar[u & 1], (u >> 1) & 1);
+    const int64_t* A = Ab + (u & 1) * N2P;
+    const int64_t* Xc = X + cur * ES * W;
+    int64_t* Xn = X + (cur ^ 1) * ES * W;
+    if (ta < TA) {
+      int ao[RA], jo[RJ];
+      int64_t best[RA][RJ];
+#pragma unroll
+      for (int i = 0; i < RA; ++i) {
+        ao[i] = (ta + TA * i < ES ? ta + TA * i : ES - 1) * ES;        // (clamped: dropped below)
+#pragma unroll
+        for (int k = 0; k < RJ; ++k) best[i][k] = INT64_MAX;
+      }
+#pragma unroll
+      for (int k = 0; k < RJ; ++k) jo[k] = tj + TJ * k < W ? tj + TJ * k : W - 1;
+#pragma unroll 5
+      for (int m = 0; m < ES; ++m) {
+        int64_t av[RA], xv[RJ];
+#pragma unroll
+        for (int i = 0; i < RA; ++i) av[i] = A[ao[i] + m];
+#pragma unroll
+        for (int k = 0; k < RJ; ++k) xv[k] = Xc[m * W + jo[k]];
+#pragma unroll
+        for (int i = 0; i < RA; ++i)
+#pragma unroll
+          for (int k = 0; k < RJ; ++k) {
+            const int64_t g = av[i] + xv[k];
+            best[i][k] = g < best[i][k] ? g : best[i][k];
+          }
+      }
+#pragma unroll
+      for (int i = 0; i < RA; ++i)
+#pragma unroll
+        for (int k = 0; k < RJ; ++k)
+          if (ta + TA * i < ES && tj + TJ * k < W) Xn[(ta + TA * i) * W + tj + TJ * k] = best[i][k] < kInfCls ? best[i][k] : kInfCls;
+    }
+    cur ^= 1;
+    __syncthreads();                                       // the matrix buffer has been read, the new X is complete
+    if (tid == 0) fetch(u + 2);
+  }
+  int64_t* out = Q + ((size_t)p * gridDim.x + c) * (ES * F::SQ) + col0;    // rows SQ words apart
+  const int64_t* Xc = X + cur * ES * W;
+  for (int x = tid; x < ES * W; x += NT)
+    if (x % W < ncol) out[x / W * F::SQ + x % W] = Xc[x];
 }
 
-// 3. V[p][0] = g_0 (any row of M_0), V[p][c + 1] = V[p][c] (x) Q[p][c]   (one CTA per chain; nq = C - 1 matrices, TMA ring)
+// 3. V[p][0] = g_0 (any row of M_0), V[p][c + 1] = V[p][c] (x) Q[p][c]   (one CTA per chain; nq = C - 1 matrices, TMA ring).
+// The steps are sequential and short: thread (b, part) of 4 parts per output b takes every fourth a; with rows SQ = 8 mod 16
+// words apart the 32 lanes of a load (8 outputs x 4 parts) hit 32 different 8-byte bank slots.
 template <int D>
-__global__ void __launch_bounds__(Fac<D>::ES * 8 / 32 * 32 + 32) chunk_prefix_kernel(const int64_t* __restrict__ M, int L,
-                                                                                   const int64_t* __restrict__ Q, int nq,
-                                                                                   int64_t* __restrict__ V) {
+__global__ void __launch_bounds__((Fac<D>::ES * 4 + 31) / 32 * 32) chunk_prefix_kernel(const int64_t* __restrict__ M, int L,
+                                                                                    const int64_t* __restrict__ Q, int nq,
+                                                                                    int64_t* __restrict__ V) {
   using F = Fac<D>;
-  constexpr int ES = F::ES, N2P = F::N2P, PARTS = 8, ST = 4, NA = (ES + PARTS - 1) / PARTS;
+  constexpr int ES = F::ES, SQ = F::SQ, QW = ES * SQ, PARTS = 4, ST = 4, NA = (ES + PARTS - 1) / PARTS;
   extern __shared__ __align__(128) unsigned char pf_raw[];
   int64_t* ring = reinterpret_cast<int64_t*>(pf_raw);      // ST matrices
   __shared__ int64_t v[2][ES];
   __shared__ uint64_t full[ST];
   const int tid = threadIdx.x, p = blockIdx.x;
   const int b = tid / PARTS, part = tid % PARTS;
-  const int64_t* Qp = Q + (size_t)p * nq * N2P;
+  const int64_t* Qp = Q + (size_t)p * nq * QW;
   if (tid == 0) {
     for (int s2 = 0; s2 < ST; ++s2) mbar_init(&full[s2], 1);
     mbar_fence_init();
@@ -663,33 +683,31 @@ __global__ void __launch_bounds__(Fac<D>::ES * 8 / 32 * 32 + 32) chunk_prefix_ke
   const uint64_t pol = policy_evict_first();
   auto fetch = [&](int c) {                                // thread 0
     if (c < nq) {
-      mbar_arrive_expect_tx(&full[c % ST], N2P * 8);
-      bulk_g2s(ring + (size_t)(c % ST) * N2P, Qp + (size_t)c * N2P, N2P * 8, &full[c % ST], pol);
+      mbar_arrive_expect_tx(&full[c % ST], QW * 8);
+      bulk_g2s(ring + (size_t)(c % ST) * QW, Qp + (size_t)c * QW, QW * 8, &full[c % ST], pol);
     }
   };
   if (tid == 0)
     for (int s2 = 0; s2 < ST; ++s2) fetch(s2);
   if (tid < ES) {
-    const int64_t g0 = M[(size_t)p * L * N2P + tid];
+    const int64_t g0 = M[(size_t)p * L * F::N2P + tid];
     v[0][tid] = g0;
     V[(size_t)p * (nq + 1) * ES + tid] = g0;
   }
   __syncthreads();
   for (int c = 0; c < nq; ++c) {
     mbar_wait(&full[c % ST], (c / ST) & 1);
-    const int64_t* Qc = ring + (size_t)(c % ST) * N2P;
+    const int64_t* Qc = ring + (size_t)(c % ST) * QW + (b < ES ? b : 0);
     const int64_t* vin = v[c & 1];
-    int64_t best = kInfCls;
-    if (b < ES) {
-      int64_t t[NA];
+    int64_t t[NA];
 #pragma unroll
-      for (int q = 0; q < NA; ++q) {
-        const int a = part + q * PARTS;
-        t[q] = a < ES ? vin[a] + Qc[a * ES + b] : kInfCls;
-      }
-#pragma unroll
-      for (int q = 0; q < NA; ++q) best = t[q] < best ? t[q] : best;
+    for (int q = 0; q < NA; ++q) {
+      const int a = part + q * PARTS;
+      t[q] = a < ES ? vin[a] + Qc[a * SQ] : kInfCls;
     }
+    int64_t best = kInfCls;
+#pragma unroll
+    for (int q = 0; q < NA; ++q) best = t[q] < best ? t[q] : best;
 #pragma unroll
     for (int off = 1; off < PARTS; off <<= 1) {
       const int64_t o = __shfl_xor_sync(0xffffffffu, best, off);
@@ -926,21 +944,20 @@ int launch_lookup_d(int32_t Bp, int32_t L, const MeshParams& mp, const int64_t* 
 
 }  // namespace
 
+// layers per chunk: the chunk products and the per-chunk DP grow with it, the serial prefix pass shrinks
+static inline int scan_chunk_len(int ndim, int L) { return ndim == 3 && L >= 256 ? 16 : 8; }
+
 template <int D>
 int launch_dp_scan_d(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams& mp, unsigned char* d_work, int64_t* d_opt_cost,
                      int32_t* d_strategy, cudaStream_t st) {
   using F = Fac<D>;
   constexpr int ES = F::ES, N2 = F::N2P, K = F::K;        // (matrices N2P words apart)
-#ifdef ADL_DBG_LEN
-  const int len = ADL_DBG_LEN, C = (L - 2 + len - 1) / len;
-#else
-  const int len = D == 3 ? 4 : 8, C = (L - 2 + len - 1) / len;
-#endif
+  const int len = scan_chunk_len(D, L), C = (L - 2 + len - 1) / len;
   const int sms = device_sm_count();
-  // workspace: M [Bp][L][N2P], Q [Bp][C-1][N2P], V [Bp][C][ES] (int64), last signature [Bp] (int32), back-pointers [Bp][bp_stride]
+  // workspace: M [Bp][L][N2P], Q [Bp][C-1][ES][SQ], V [Bp][C][ES] (int64), last signature [Bp] (int32), back-pointers [Bp][bp_stride]
   int64_t* d_M = reinterpret_cast<int64_t*>(d_work);
   int64_t* d_Q = d_M + (size_t)Bp * L * N2;
-  int64_t* d_V = d_Q + (size_t)Bp * (C > 1 ? C - 1 : 1) * N2;
+  int64_t* d_V = d_Q + (size_t)Bp * (C > 1 ? C - 1 : 1) * (ES * F::SQ);
   auto up256 = [](void* q) { return reinterpret_cast<unsigned char*>(((uintptr_t)q + 255) & ~(uintptr_t)255); };
   int32_t* d_last = reinterpret_cast<int32_t*>(up256(d_V + (size_t)Bp * C * ES));
   uint8_t* d_bp = up256(d_last + Bp);                      // (bulk copies want 16-byte aligned sources)
@@ -955,17 +972,18 @@ int launch_dp_scan_d(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams
     ADL_CUDA_CHECK(cudaGetLastError());
   }
   if (C > 1) {
-    const size_t smem = (size_t)3 * N2 * 8;
+    using PC = ProdCfg<D>;
+    const size_t smem = ((size_t)2 * N2 + 2 * ES * PC::W) * 8;
     ADL_CUDA_CHECK(cudaFuncSetAttribute(chunk_product_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    chunk_product_kernel<D><<<dim3(C - 1, Bp), 512, smem, st>>>(d_M, L, len, d_Q);
+    chunk_product_kernel<D><<<dim3(C - 1, Bp, PC::NG), PC::NT, smem, st>>>(d_M, L, len, d_Q);
     count_launch();
     ADL_CUDA_CHECK(cudaGetLastError());
   }
   const int nt8 = (ES * 8 + 31) / 32 * 32;
   {
-    const size_t smem = (size_t)4 * N2 * 8;
+    const size_t smem = (size_t)4 * ES * F::SQ * 8;
     ADL_CUDA_CHECK(cudaFuncSetAttribute(chunk_prefix_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    chunk_prefix_kernel<D><<<Bp, nt8, smem, st>>>(d_M, L, d_Q, C - 1, d_V);
+    chunk_prefix_kernel<D><<<Bp, (ES * 4 + 31) / 32 * 32, smem, st>>>(d_M, L, d_Q, C - 1, d_V);
     count_launch();
     ADL_CUDA_CHECK(cudaGetLastError());
   }
@@ -977,11 +995,7 @@ int launch_dp_scan_d(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams
     ADL_CUDA_CHECK(cudaGetLastError());
   }
   {
-#ifdef ADL_DBG_NOSTAGE
-    const int staged = 0;
-#else
     const int staged = bp_stride <= 200 * 1024;
-#endif
     const size_t smem = staged ? bp_stride : 16;
     ADL_CUDA_CHECK(cudaFuncSetAttribute(chain_walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     chain_walk_kernel<<<Bp, 32, smem, st>>>(d_bp, bp_stride, L, K, d_last, d_strategy, staged);
@@ -1025,9 +1039,10 @@ int launch_cd_lookup(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams
 bool chain_dp_scan_supported(const MeshParams& mp, int32_t Bp, int32_t L) { return factors_supported(mp) && L >= 32 && Bp <= 64; }
 
 size_t chain_dp_scan_bytes(const MeshParams& mp, int32_t Bp, int32_t L) {
-  const int es = mp.ndim == 2 ? Fac<2>::ES : Fac<3>::ES, k = mp.ndim == 2 ? Fac<2>::K : Fac<3>::K, len = mp.ndim == 3 ? 4 : 8;
+  const int es = mp.ndim == 2 ? Fac<2>::ES : Fac<3>::ES, k = mp.ndim == 2 ? Fac<2>::K : Fac<3>::K, len = scan_chunk_len(mp.ndim, L);
   const size_t n2 = mp.ndim == 2 ? Fac<2>::N2P : Fac<3>::N2P, c = (L - 2 + len - 1) / len;
-  const size_t b = ((size_t)Bp * L * n2 + (size_t)Bp * (c > 1 ? c - 1 : 1) * n2 + (size_t)Bp * c * es) * 8 +
+  const size_t qw = (size_t)es * (mp.ndim == 2 ? Fac<2>::SQ : Fac<3>::SQ);
+  const size_t b = ((size_t)Bp * L * n2 + (size_t)Bp * (c > 1 ? c - 1 : 1) * qw + (size_t)Bp * c * es) * 8 +
                    (((size_t)Bp * 4 + 255) & ~(size_t)255) + (size_t)Bp * (((size_t)L * k + 15) & ~(size_t)15);
   return (b + 255) / 256 * 256 + 768;                      // (+ the alignment gaps of the carve-up)
 }
