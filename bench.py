@@ -524,7 +524,10 @@ def run_configs(args):
         tau = 20_000_000
         mh = adl.metropolis(T, init, w.mesh, nsteps, tau, seed=0)
         one = adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out={"T": T})
+        one_nt = adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, want_tables=False, work=work)
         torch.cuda.synchronize()
+        for key in ("opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps"):
+            assert torch.equal(one[key], one_nt[key]), key
         sweeps = int(cd[2].sum().item())
         g = {
             "build_us": gpu_us(lambda: adl.build_tables(dl, w.mesh, w.net, want_node_mask=False, out=T)),
@@ -533,6 +536,10 @@ def run_configs(args):
             # d_T = NULL: no K x K table; with >= 32 starts per problem on 2 / 3 mesh levels factors -> best responses -> look-ups
             "cd_no_table_us": gpu_us(lambda: adl.coord_descent(None, init, w.mesh, w.max_sweeps, net=w.net, d_layers=dl, work=work, out=cd)),
             "search_us": gpu_us(lambda: adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out=one)),
+            # the same with no table asked for (optimum, strategies and CD results only): long chains take the DP in class space
+            "dp_no_table_us": gpu_us(lambda: adl.chain_dp(None, w.mesh, net=w.net, d_layers=dl, work=work, out=dp)),
+            "search_no_table_us": gpu_us(lambda: adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, want_tables=False,
+                                                            work=work, out=one_nt)),
             "mh_us": gpu_us(lambda: adl.metropolis(T, init, w.mesh, nsteps, tau, seed=0, out=mh), n=5),
         }
         line = {"config": k, "name": w.name, "Bp": w.Bp, "L": w.L, "K": w.K, "S": w.S, "cells": w.cells, "cd_sweeps": sweeps,

@@ -109,9 +109,12 @@ int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
 /* (a2) f_0[j] = T[0][0][j]; f_l[j] = min_i f_{l-1}[i] + T[l][i][j]; smallest index wins every tie;
  * backtrack from the smallest argmin of f_{L-1}.  d_T == NULL: the tables are computed from d_layers
  * -- on a 2-level mesh (K = 36), for >= 296 chains or when d_work cannot hold the tables, inside the DP kernel
- * itself (one warp per chain, every tile in factor form in shared memory, never stored); otherwise they are first built
- * into d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers (fused kernel: only for chains too long
- * for shared memory; separate kernel: when L * K > 16384).
+ * itself (one warp per chain, every tile in factor form in shared memory, never stored); at most 64 chains of at least
+ * 32 layers on a 2- or 3-level mesh are solved in class space, parallel over the layers, from the tiles' factors alone
+ * (no K x K table is formed; same optimum, same tie-break); otherwise the tables are first built into
+ * d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers (fused kernel: only for chains too long for
+ * shared memory; separate kernel: when L * K > 16384) and the class matrices of that path; with less workspace than a
+ * path needs the next one is taken, AUTODDL_EWORK if none fits.
  * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
 int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                      const autoddl_mesh* mesh, const autoddl_net* net,
