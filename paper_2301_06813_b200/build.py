@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libautoddl.so")
-SOURCES = ["api.cu", "build_tables.cu", "build_tables_folded.cu", "fused_chain.cu", "chain_dp.cu", "chain_dp_cluster.cu", "coord_descent.cu", "factors.cu", "metropolis.cu", "fit_alpha_beta.cu", "copy_probe.cu", "best_of_starts.cu", "pipeline.cu"]
+SOURCES = ["api.cu", "build_tables.cu", "build_tables_folded.cu", "fused_chain.cu", "chain_dp.cu", "chain_dp_cluster.cu", "coord_descent.cu", "factors.cu", "chain_dp_scan.cu", "metropolis.cu", "fit_alpha_beta.cu", "copy_probe.cu", "best_of_starts.cu", "pipeline.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "--use_fast_math",

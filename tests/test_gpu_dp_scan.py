@@ -1,4 +1,4 @@
-"""Chain DP of few long chains in class space, parallel over the layers (csrc/factors.cu: class matrices, chunk products,
+"""Chain DP of few long chains in class space, parallel over the layers (csrc/chain_dp_scan.cu: class matrices, chunk products,
 prefix vectors, per-chunk DP, walk) against the oracle's sequential DP (PAPER.md:225 exhaustive optimum,
 R9 tie-break): optimum AND strategy bit-exact at chain lengths around every chunk boundary, on two and three mesh levels,
 with attention layers (the invalid class), split limits, a memory cap (2^50 penalties in the sums) and several chains."""
