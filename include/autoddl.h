@@ -114,7 +114,8 @@ int autoddl_build_tables(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
  * (no K x K table is formed; same optimum, same tie-break); otherwise the tables are first built into
  * d_work.  d_work (>= autoddl_workspace_bytes) also holds back-pointers (fused kernel: only for chains too long for
  * shared memory; separate kernel: when L * K > 16384) and the class matrices of that path; with less workspace than a
- * path needs the next one is taken, AUTODDL_EWORK if none fits.
+ * path needs the next one is taken, AUTODDL_EWORK if none fits.  Tables with K <= 64 (given or built) of at most 64 chains
+ * of at least 32 layers take the same layer-parallel scheme on the tiles themselves.
  * Cells must lie in [0, 2^62 / L) so that sums cannot overflow. */
 int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                      const autoddl_mesh* mesh, const autoddl_net* net,

@@ -200,6 +200,7 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   const bool scan = chain_dp_scan_supported(mp, Bp, L);
   if (scan || cd_lookup_supported(mp, L, S)) b += factors_bytes(mp, Bp, L) + 256;
   if (scan) b += chain_dp_scan_bytes(mp, Bp, L);           // few long chains: the DP in class space, parallel over the layers
+  if (chain_dp_scan_tab_supported((int32_t)K, Bp, L)) b += chain_dp_scan_tab_bytes((int32_t)K, Bp, L);   // the same on small tables
   if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L) + 256;   // many starts: best responses
   if (mesh->ndim == 2) b += fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256;   // fused kernel: back-pointers, strategies after sweep 1
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
@@ -270,6 +271,9 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
     d_T = (const int64_t*)d_work;
   }
+  // few long chains on small tables (K <= 64): chunk products, prefix vectors, per-chunk DP -- parallel over the layers
+  if (chain_dp_scan_tab_supported(K, Bp, L) && d_work != nullptr && work_bytes >= tb + chain_dp_scan_tab_bytes(K, Bp, L))
+    return launch_chain_dp_scan_tab(d_T, Bp, L, K, (unsigned char*)d_work + tb, d_opt_cost, d_strategy, st);
   uint8_t* d_bp = bb ? (uint8_t*)d_work + tb : nullptr;
   return launch_chain_dp(d_T, Bp, L, K, d_bp, d_opt_cost, d_strategy, st);
 }
@@ -398,7 +402,10 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   }
   if (!d_T) d_T = (int64_t*)d_work;
   if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
-  if ((rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + tb : nullptr, d_opt_cost, d_strategy, st))) return rc;
+  const bool scan_tab = chain_dp_scan_tab_supported((int32_t)K, Bp, L) && work_bytes >= tb + chain_dp_scan_tab_bytes((int32_t)K, Bp, L);
+  if (scan_tab) rc = launch_chain_dp_scan_tab(d_T, Bp, L, (int32_t)K, d_work + tb, d_opt_cost, d_strategy, st);
+  else rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + tb : nullptr, d_opt_cost, d_strategy, st);
+  if (rc) return rc;
   if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
   if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
   if (!do_cd) return AUTODDL_OK;
@@ -467,6 +474,7 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
                          (mesh->ndim == 2 ? fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256 : 0);
   if (chain_dp_scan_supported(mp, Bp, L) || (do_cd && cd_lookup_supported(mp, L, S))) tables_region += factors_bytes(mp, Bp, L) + 256;
   if (chain_dp_scan_supported(mp, Bp, L)) tables_region += chain_dp_scan_bytes(mp, Bp, L);
+  if (chain_dp_scan_tab_supported((int32_t)K, Bp, L)) tables_region += chain_dp_scan_tab_bytes((int32_t)K, Bp, L);
   if (do_cd && cd_lookup_supported(mp, L, S)) tables_region += cd_lookup_workspace_bytes(mp, Bp, L) + 512;
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));

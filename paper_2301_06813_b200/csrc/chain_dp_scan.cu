@@ -418,6 +418,224 @@ __global__ void __launch_bounds__(32) chain_walk_kernel(const uint8_t* __restric
   }
 }
 
+// ---- the same scheme on K x K TABLES (caller-supplied, or built for a mesh without the factor form), K <= 64 -------------
+// Without classes the state is f_l itself and the matrices are the tiles: Q_c = T_{t_c+1} (x) ... (x) T_{t_c+len}, V_0 = f_0 =
+// T[0][0][.], V_{c+1} = V_c (x) Q_c = f_{t_{c+1}}, and the CTA of chunk c runs the ordinary DP over layers t_c+1 .. t_c+len
+// from f_{t_c} (smallest i on ties: the sequential DP on its chunk).  K^3 <= 2.6e5 operations per product: a CTA per chunk.
+__device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// one K x K tile global -> shared by all threads of the CTA (tiles of an odd K are only 8-byte aligned); one commit group
+__device__ __forceinline__ void tile_g2s(int64_t* dst, const int64_t* src, int K, int tid, int nt) {
+  const int n = K * K;
+  if ((K & 1) == 0)
+    for (int x = tid; x < n / 2; x += nt) cp_async16(dst + 2 * x, src + 2 * x);
+  else
+    for (int x = tid; x < n; x += nt) cp_async8(dst + x, src + x);
+  cp_async_commit();
+}
+
+// Q[p][c] = T_{t_c + 1} (x) ... (x) T_{t_c + len} for c = 0 .. C - 2 (grid.x = C - 1, grid.y = Bp); matrices QS words apart
+__global__ void __launch_bounds__(512) chunk_product_tab_kernel(const int64_t* __restrict__ T, int L, int K, int len,
+                                                                int64_t* __restrict__ Q, int QS) {
+  constexpr int NT = 512, MAXO = 8;                        // outputs per thread: 64 x 64 / 512
+  extern __shared__ __align__(128) unsigned char tp_raw[];
+  const int n = K * K, nb = (n + 1) & ~1;
+  int64_t* A = reinterpret_cast<int64_t*>(tp_raw);
+  int64_t* Bb = A + nb;
+  const int tid = threadIdx.x, c = blockIdx.x, p = blockIdx.y;
+  const int64_t* T1 = T + ((size_t)p * L + (size_t)c * len + 1) * n;       // T_{t_c + 1}
+  tile_g2s(A, T1, K, tid, NT);
+  if (len > 1) tile_g2s(Bb + nb, T1 + n, K, tid, NT);      // T_{t_c + 1 + k} -> buffer k & 1
+  for (int k = 1; k < len; ++k) {
+    if (k + 1 < len) { tile_g2s(Bb + ((k + 1) & 1) * nb, T1 + (size_t)(k + 1) * n, K, tid, NT); cp_async_wait_group<1>(); }
+    else cp_async_wait_group<0>();
+    __syncthreads();
+    const int64_t* B = Bb + (k & 1) * nb;
+    int64_t best[MAXO];
+#pragma unroll
+    for (int q = 0; q < MAXO; ++q) {
+      const int o = tid + q * NT;
+      best[q] = INT64_MAX;
+      if (o < n) {
+        const int64_t* a = A + o / K * K;
+        const int64_t* b = B + o % K;
+        int64_t bv = INT64_MAX;
+        for (int m = 0; m < K; ++m) {
+          const int64_t g = a[m] + b[m * K];
+          bv = g < bv ? g : bv;
+        }
+        best[q] = bv;
+      }
+    }
+    __syncthreads();                                       // A and the buffer have been read by everyone
+#pragma unroll
+    for (int q = 0; q < MAXO; ++q)
+      if (tid + q * NT < n) A[tid + q * NT] = best[q];
+  }
+  if (len == 1) cp_async_wait_group<0>();
+  __syncthreads();
+  int64_t* out = Q + ((size_t)p * gridDim.x + c) * QS;
+  for (int x = tid; x < n; x += NT) out[x] = A[x];
+}
+
+// V[p][0] = f_0 = T[p][0][0][.], V[p][c + 1] = V[p][c] (x) Q[p][c]   (one CTA per chain, 4 threads per output, TMA ring)
+__global__ void __launch_bounds__(256) chunk_prefix_tab_kernel(const int64_t* __restrict__ T, int L, int K, const int64_t* __restrict__ Q,
+                                                               int QS, int nq, int64_t* __restrict__ V) {
+  constexpr int PARTS = 4, ST = 4;
+  extern __shared__ __align__(128) unsigned char tf_raw[];
+  int64_t* ring = reinterpret_cast<int64_t*>(tf_raw);      // ST matrices
+  __shared__ int64_t v[2][64];
+  __shared__ uint64_t full[ST];
+  const int tid = threadIdx.x, p = blockIdx.x;
+  const int b = tid / PARTS, part = tid % PARTS;
+  const int64_t* Qp = Q + (size_t)p * nq * QS;
+  if (tid == 0) {
+    for (int s2 = 0; s2 < ST; ++s2) mbar_init(&full[s2], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  const uint64_t pol = policy_evict_first();
+  auto fetch = [&](int c) {                                // thread 0
+    if (c < nq) {
+      mbar_arrive_expect_tx(&full[c % ST], QS * 8);
+      bulk_g2s(ring + (size_t)(c % ST) * QS, Qp + (size_t)c * QS, QS * 8, &full[c % ST], pol);
+    }
+  };
+  if (tid == 0)
+    for (int s2 = 0; s2 < ST; ++s2) fetch(s2);
+  if (tid < K) {
+    const int64_t f0 = T[(size_t)p * L * K * K + tid];
+    v[0][tid] = f0;
+    V[(size_t)p * (nq + 1) * K + tid] = f0;
+  }
+  __syncthreads();
+  for (int c = 0; c < nq; ++c) {
+    mbar_wait(&full[c % ST], (c / ST) & 1);
+    const int64_t* Qc = ring + (size_t)(c % ST) * QS + (b < K ? b : 0);
+    const int64_t* vin = v[c & 1];
+    int64_t best = INT64_MAX;
+    for (int a = part; a < K; a += PARTS) {
+      const int64_t g = vin[a] + Qc[a * K];
+      best = g < best ? g : best;
+    }
+#pragma unroll
+    for (int off = 1; off < PARTS; off <<= 1) {
+      const int64_t o = __shfl_xor_sync(0xffffffffu, best, off);
+      best = o < best ? o : best;
+    }
+    if (b < K && part == 0) {
+      v[(c & 1) ^ 1][b] = best;
+      V[((size_t)p * (nq + 1) + c + 1) * K + b] = best;
+    }
+    __syncthreads();
+    if (tid == 0) fetch(c + ST);
+  }
+}
+
+// the DP of chunk c of chain p over layers t_c + 1 .. min(t_c + len, L - 1), from V[p][c] = f_{t_c} (grid.x = C, grid.y = Bp)
+__global__ void __launch_bounds__(512) chunk_dp_tab_kernel(const int64_t* __restrict__ T, int L, int K, int len,
+                                                           const int64_t* __restrict__ V, uint8_t* __restrict__ bp, size_t bp_stride,
+                                                           int64_t* __restrict__ opt_cost, int32_t* __restrict__ last_sig) {
+  constexpr int NT = 512, PARTS = 8;
+  extern __shared__ __align__(128) unsigned char td_raw[];
+  const int n = K * K, nb = (n + 1) & ~1;
+  int64_t* tiles = reinterpret_cast<int64_t*>(td_raw);     // two buffers
+  __shared__ int64_t f[64];
+  const int tid = threadIdx.x, c = blockIdx.x, C = gridDim.x, p = blockIdx.y;
+  const int j = tid / PARTS, part = tid % PARTS;
+  const int l0 = c * len + 1, l1 = (l0 + len - 1 < L - 1 && c + 1 < C) ? l0 + len - 1 : L - 1;
+  const int64_t* Tp = T + (size_t)p * L * n;
+  uint8_t* bpp = bp + (size_t)p * bp_stride;
+  tile_g2s(tiles, Tp + (size_t)l0 * n, K, tid, NT);
+  if (tid < K) f[tid] = V[((size_t)p * C + c) * K + tid];
+  for (int l = l0; l <= l1; ++l) {
+    if (l + 1 <= l1) { tile_g2s(tiles + ((l + 1 - l0) & 1) * nb, Tp + (size_t)(l + 1) * n, K, tid, NT); cp_async_wait_group<1>(); }
+    else cp_async_wait_group<0>();
+    __syncthreads();
+    const int64_t* tl = tiles + ((l - l0) & 1) * nb + (j < K ? j : 0);
+    int64_t bv = INT64_MAX;
+    int bi = 1 << 30;
+    if (j < K)
+      for (int i = part; i < K; i += PARTS) {              // increasing i and strict '<': the thread keeps its smallest i
+        const int64_t g = f[i] + tl[i * K];
+        if (g < bv) { bv = g; bi = i; }
+      }
+#pragma unroll
+    for (int off = 1; off < PARTS; off <<= 1) {
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    __syncthreads();                                       // f_{l-1} and the tile have been read by everyone
+    if (j < K && part == 0) {
+      f[j] = bv;
+      bpp[(size_t)l * K + j] = (uint8_t)bi;
+    }
+  }
+  __syncthreads();
+  if (l1 == L - 1 && tid < 32) {                           // the chain's optimum: smallest argmin of f_{L-1}
+    int64_t bv = INT64_MAX;
+    int bi = 1 << 30;
+    for (int a = tid; a < K; a += 32)
+      if (f[a] < bv) { bv = f[a]; bi = a; }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if (tid == 0) { opt_cost[p] = bv; last_sig[p] = bi; }
+  }
+}
+
+constexpr int kTabScanLen = 8, kTabScanMaxK = 64;
+
+int launch_dp_scan_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, unsigned char* d_work, int64_t* d_opt_cost,
+                       int32_t* d_strategy, cudaStream_t st) {
+  const int len = kTabScanLen, C = (L - 1 + len - 1) / len, n = K * K, QS = (n + 1) & ~1;
+  // workspace: Q [Bp][C-1][QS], V [Bp][C][K] (int64), last signature [Bp] (int32), back-pointers [Bp][bp_stride]
+  auto up256 = [](void* q) { return reinterpret_cast<unsigned char*>(((uintptr_t)q + 255) & ~(uintptr_t)255); };
+  int64_t* d_Q = reinterpret_cast<int64_t*>(d_work);
+  int64_t* d_V = d_Q + (size_t)Bp * (C > 1 ? C - 1 : 1) * QS;
+  int32_t* d_last = reinterpret_cast<int32_t*>(up256(d_V + (size_t)Bp * C * K));
+  uint8_t* d_bp = up256(d_last + Bp);
+  const size_t bp_stride = ((size_t)L * K + 15) & ~(size_t)15;
+  if (C > 1) {
+    const size_t smem = (size_t)3 * QS * 8;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(chunk_product_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    chunk_product_tab_kernel<<<dim3(C - 1, Bp), 512, smem, st>>>(d_T, L, K, len, d_Q, QS);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  {
+    const size_t smem = (size_t)4 * QS * 8;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(chunk_prefix_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    chunk_prefix_tab_kernel<<<Bp, 256, smem, st>>>(d_T, L, K, d_Q, QS, C - 1, d_V);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  {
+    const size_t smem = (size_t)2 * QS * 8;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(chunk_dp_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    chunk_dp_tab_kernel<<<dim3(C, Bp), 512, smem, st>>>(d_T, L, K, len, d_V, d_bp, bp_stride, d_opt_cost, d_last);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  {
+    const int staged = bp_stride <= 200 * 1024;
+    const size_t smem = staged ? bp_stride : 16;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(chain_walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    chain_walk_kernel<<<Bp, 32, smem, st>>>(d_bp, bp_stride, L, K, d_last, d_strategy, staged);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  return AUTODDL_OK;
+}
+
 // layers per chunk: the chunk products and the per-chunk DP grow with it, the serial prefix pass shrinks
 static inline int scan_chunk_len(int ndim, int L) { return ndim == 3 && L >= 256 ? 16 : 8; }
 
@@ -499,4 +717,19 @@ int launch_chain_dp_scan(const int64_t* d_F, int32_t Bp, int32_t L, const MeshPa
                       : launch_dp_scan_d<3>(d_F, Bp, L, mp, (unsigned char*)d_work, d_opt_cost, d_strategy, st);
 }
 
+
+// the same on K x K tables: any mesh, K <= 64, L >= 32, Bp <= 64
+bool chain_dp_scan_tab_supported(int32_t K, int32_t Bp, int32_t L) { return K <= kTabScanMaxK && L >= 32 && Bp <= 64; }
+
+size_t chain_dp_scan_tab_bytes(int32_t K, int32_t Bp, int32_t L) {
+  const size_t c = (L - 1 + kTabScanLen - 1) / kTabScanLen, qs = ((size_t)K * K + 1) & ~(size_t)1;
+  const size_t b = ((size_t)Bp * (c > 1 ? c - 1 : 1) * qs + (size_t)Bp * c * K) * 8 + (((size_t)Bp * 4 + 255) & ~(size_t)255) +
+                   (size_t)Bp * (((size_t)L * K + 15) & ~(size_t)15);
+  return (b + 255) / 256 * 256 + 768;
+}
+
+int launch_chain_dp_scan_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* d_work, int64_t* d_opt_cost,
+                             int32_t* d_strategy, cudaStream_t st) {
+  return launch_dp_scan_tab(d_T, Bp, L, K, (unsigned char*)d_work, d_opt_cost, d_strategy, st);
+}
 }  // namespace autoddl

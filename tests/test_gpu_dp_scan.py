@@ -79,3 +79,41 @@ def test_scan_dp_many_chains_and_fallbacks(adl):
         w = cf.Workload("scan-many", _chains(rng, Bp, L, ragged=True), cf.Mesh((2, 2, 2), (cf.INTER, cf.INTER, cf.INTRA)),
                         cf.Net(cf.ALPHA_PS, (cf.BETA_300, cf.BETA_25), 0), S=1, seed=1)
         _check(adl, w)
+
+
+# ---- the same scheme on K x K tables (any mesh, K <= 64): caller-supplied tables, so random ones with MANY ties --------------
+def _mesh_with_k(K):
+    """a mesh whose signature count is K (the tables themselves are random)"""
+    if K == 36:
+        return cf.Mesh((4, 4), (cf.INTER, cf.INTRA))
+    if K == 16:                                              # four levels, two allowed rows each (R24, R26)
+        return cf.Mesh((2, 2, 2, 2), tuple(l | (0x03 << 8) for l in (cf.INTER, cf.INTER, cf.INTRA, cf.INTRA)))
+    if K == 64:                                              # four levels, 4 . 4 . 2 . 2 allowed rows
+        return cf.Mesh((2, 2, 2, 2), (cf.INTER | (0x0f << 8), cf.INTER | (0x0f << 8), cf.INTRA | (0x03 << 8), cf.INTRA | (0x03 << 8)))
+    if K in (28, 45):                                        # folded: six / eight equal levels (R28)
+        n = 6 if K == 28 else 8
+        return cf.Mesh((2,) * n, (cf.INTER | cf.FOLD,) + (cf.INTER,) * (n - 1))
+    raise ValueError(K)
+
+
+@pytest.mark.parametrize("K,L,Bp,hi", [(36, 32, 1, 4), (36, 33, 3, 1 << 40), (16, 41, 2, 3), (28, 40, 1, 5), (45, 57, 2, 1 << 45),
+                                       (45, 220, 1, 7), (64, 49, 2, 4), (64, 130, 1, 1 << 50), (36, 64, 64, 6)])
+def test_scan_dp_on_tables(adl, K, L, Bp, hi):
+    """random tables; with cells in [0, hi) for a small hi nearly every minimum is tied: the back-pointers must be the
+    sequential DP's (smallest i), chunk by chunk"""
+    mesh = _mesh_with_k(K)
+    assert adl.num_signatures(mesh) == K
+    rng = np.random.default_rng(K * 1000 + L)
+    T = rng.integers(0, hi, size=(Bp, L, K, K), dtype=np.int64)
+    want_c, want_s = ref.chain_dp(T)
+    d_T = torch.from_numpy(T).cuda()
+    work = torch.empty(adl.workspace_bytes(Bp, L, 0, mesh), dtype=torch.uint8, device="cuda")
+    work.fill_(0xA5)
+    got_c, got_s = adl.chain_dp(d_T, mesh, work=work)
+    torch.cuda.synchronize()
+    assert np.array_equal(got_c.cpu().numpy(), want_c)
+    assert np.array_equal(got_s.cpu().numpy(), want_s)
+    # the kernel that runs when the workspace is too small for this path gives the same
+    small = torch.empty(Bp * L * K + 4096, dtype=torch.uint8, device="cuda")
+    c2, s2 = adl.chain_dp(d_T, mesh, work=small)
+    assert torch.equal(c2, got_c) and torch.equal(s2, got_s)
