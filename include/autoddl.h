@@ -126,7 +126,10 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
  * s_l to the smallest-index minimiser of T[l][s_{l-1}][c] + T[l+1][c][s_{l+1}] (s_{-1} = 0, last
  * layer has no second term) using already-updated neighbours; stops after the first sweep that
  * changes nothing or after max_sweeps.  d_sweeps counts sweeps including the final unchanged one.
- * d_init entries must lie in [0, K).  d_T == NULL as in autoddl_chain_dp. */
+ * d_init entries must lie in [0, K).  d_T == NULL as in autoddl_chain_dp.  With S >= 32 starts the update of a layer is
+ * tabulated once per (left, right) neighbour (from the tiles' factors on 2- / 3-level meshes with d_T == NULL, from the
+ * tiles themselves when K <= 64 and d_work holds autoddl_workspace_bytes) and a sweep is one look-up per layer: same
+ * trajectory, sweep count and result. */
 int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                           const autoddl_mesh* mesh, const autoddl_net* net,
                           const int64_t* d_T, void* d_work, size_t work_bytes,

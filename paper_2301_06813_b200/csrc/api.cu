@@ -201,6 +201,7 @@ size_t autoddl_workspace_bytes(int32_t Bp, int32_t L, int32_t S, const autoddl_m
   if (scan || cd_lookup_supported(mp, L, S)) b += factors_bytes(mp, Bp, L) + 256;
   if (scan) b += chain_dp_scan_bytes(mp, Bp, L);           // few long chains: the DP in class space, parallel over the layers
   if (chain_dp_scan_tab_supported((int32_t)K, Bp, L)) b += chain_dp_scan_tab_bytes((int32_t)K, Bp, L);   // the same on small tables
+  if (cd_lookup_tab_supported((int32_t)K, L, S)) b += cd_lookup_tab_workspace_bytes((int32_t)K, Bp, L);   // best responses from small tables
   if (cd_lookup_supported(mp, L, S)) b += cd_lookup_workspace_bytes(mp, Bp, L) + 256;   // many starts: best responses
   if (mesh->ndim == 2) b += fused_bp_bytes(L) + align_up((size_t)Bp * S * L * 4, 256) + 256;   // fused kernel: back-pointers, strategies after sweep 1
   // autoddl_search_host staging: layers, init, opt_cost, strategy, cd_cost, cd_strategy, cd_sweeps
@@ -318,6 +319,9 @@ int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
     if ((rc = launch_build_tables(d_layers, Bp, L, mp, (int64_t*)d_work, nullptr, nullptr, st))) return rc;
     d_T = (const int64_t*)d_work;
   }
+  // many starts on small tables (K <= 64): best responses from the tiles, then look-up sweeps
+  if (cd_lookup_tab_supported(K, L, S) && d_work != nullptr && work_bytes >= tb + cd_lookup_tab_workspace_bytes(K, Bp, L))
+    return launch_cd_lookup_tab(d_T, Bp, L, K, (unsigned char*)d_work + tb, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
   return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, false, built_here);
 }
 
@@ -417,6 +421,8 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
                               d_cd_strategy, d_cd_sweeps, st);
     }
   }
+  if (cd_lookup_tab_supported((int32_t)K, L, S) && work_bytes >= tb + cd_lookup_tab_workspace_bytes((int32_t)K, Bp, L))
+    return launch_cd_lookup_tab(d_T, Bp, L, (int32_t)K, d_work + tb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
   return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, false, mp.ndim <= 3 && !mp.fold);
 }
 
@@ -475,6 +481,7 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L, co
   if (chain_dp_scan_supported(mp, Bp, L) || (do_cd && cd_lookup_supported(mp, L, S))) tables_region += factors_bytes(mp, Bp, L) + 256;
   if (chain_dp_scan_supported(mp, Bp, L)) tables_region += chain_dp_scan_bytes(mp, Bp, L);
   if (chain_dp_scan_tab_supported((int32_t)K, Bp, L)) tables_region += chain_dp_scan_tab_bytes((int32_t)K, Bp, L);
+  if (do_cd && cd_lookup_tab_supported((int32_t)K, L, S)) tables_region += cd_lookup_tab_workspace_bytes((int32_t)K, Bp, L);
   if (do_cd && cd_lookup_supported(mp, L, S)) tables_region += cd_lookup_workspace_bytes(mp, Bp, L) + 512;
   unsigned char* d_tables = carve(tables_region);                                   // tables, then back-pointers
   autoddl_layer* d_layers = (autoddl_layer*)carve((size_t)Bp * L * sizeof(autoddl_layer));

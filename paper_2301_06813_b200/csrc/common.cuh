@@ -100,6 +100,10 @@ bool chain_dp_scan_supported(const MeshParams& mp, int32_t Bp, int32_t L);
 size_t chain_dp_scan_bytes(const MeshParams& mp, int32_t Bp, int32_t L);
 int launch_chain_dp_scan(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams& mp, void* d_work, int64_t* d_opt_cost,
                          int32_t* d_strategy, cudaStream_t st);
+bool cd_lookup_tab_supported(int32_t K, int32_t L, int32_t S);
+size_t cd_lookup_tab_workspace_bytes(int32_t K, int32_t Bp, int32_t L);
+int launch_cd_lookup_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* d_work, const int32_t* d_init, int32_t S,
+                         int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st);
 bool chain_dp_scan_tab_supported(int32_t K, int32_t Bp, int32_t L);
 size_t chain_dp_scan_tab_bytes(int32_t K, int32_t Bp, int32_t L);
 int launch_chain_dp_scan_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* d_work, int64_t* d_opt_cost,

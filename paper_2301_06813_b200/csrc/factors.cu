@@ -406,6 +406,136 @@ __global__ void __launch_bounds__(128) cd_lookup_kernel(const int64_t* __restric
   }
 }
 
+// ---- the same look-up scheme on K x K TABLES, K <= 64 (caller-supplied tables, meshes without the factor form) -----------
+// Without classes the neighbours enter the update of layer l as themselves: BRt[l][j'][i] = smallest-index argmin_c
+// T[l][i][c] + T[l+1][c][j']  (K^3 operations per layer; layer 0's row is T[0][0][.], the last layer has no right term and
+// only its column 0 is used).  The 16-bit entry is (c, c), so the walk below is the walk of cd_lookup_kernel.
+__global__ void __launch_bounds__(512) best_response_tab_kernel(const int64_t* __restrict__ T, int ntiles, int L, int K, int CS,
+                                                                uint8_t* __restrict__ BRt) {
+  constexpr int NT = 512;
+  extern __shared__ __align__(16) unsigned char brt_raw[];
+  const int n = K * K, tid = threadIdx.x;
+  int64_t* Tl = reinterpret_cast<int64_t*>(brt_raw);
+  int64_t* Tr = Tl + n;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int l = tile % L;
+    const bool has_right = l < L - 1;
+    const int64_t* tl = T + (size_t)tile * n;
+    __syncthreads();
+    for (int x = tid; x < n; x += NT) {
+      Tl[x] = __ldg(tl + (l == 0 ? x % K : x));            // (layer 0: every row is row 0, s_{-1} := 0)
+      Tr[x] = has_right ? __ldg(tl + n + x) : 0;
+    }
+    __syncthreads();
+    uint8_t* out = BRt + (size_t)tile * K * CS;
+    const int ncol = has_right ? K : 1;
+    for (int o = tid; o < K * ncol; o += NT) {
+      const int i = o / ncol, jr = o % ncol;
+      const int64_t* a = Tl + i * K;
+      const int64_t* b = Tr + jr;
+      int64_t best = INT64_MAX;
+      int arg = 0;
+      for (int c = 0; c < K; ++c) {
+        const int64_t g = a[c] + b[c * K];
+        if (g < best) { best = g; arg = c; }               // increasing c, strict '<': the smallest index
+      }
+      reinterpret_cast<uint16_t*>(out + (size_t)jr * CS)[i] = (uint16_t)(arg | arg << 8);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(128) cd_lookup_tab_kernel(const int64_t* __restrict__ T, const uint8_t* __restrict__ BRt, int Bp, int L,
+                                                            int K, int CS, int S, const int32_t* __restrict__ init, int max_sweeps,
+                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
+                                                            int32_t* __restrict__ sweeps, int per_warp_bytes) {
+  extern __shared__ __align__(16) unsigned char cdt_raw[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+  const size_t ps = (size_t)blockIdx.x * W + warp;
+  if (ps >= (size_t)Bp * S) return;
+  const size_t p = ps / S;
+  unsigned char* wb = cdt_raw + (size_t)warp * per_warp_bytes;
+  uint8_t* chunk = wb;                                     // [2][32][CS] best-response columns of 32 layers, double buffered
+  uint8_t* s = chunk + 2 * 32 * CS;                        // [L] strategy
+  uint8_t* dirty = s + L;                                  // [L]
+  const uint8_t* Bp_ = BRt + p * (size_t)L * K * CS;
+  for (int l = lane; l < L; l += 32) {
+    s[l] = (uint8_t)init[ps * L + l];
+    dirty[l] = 1;
+  }
+  __syncwarp();
+  // column of layer l for the CURRENT right neighbour (old s_{l+1}: it is not touched before layer l + 1's own turn)
+  auto fetch = [&](int l0, int b) {                        // lane i -> layer l0 + i -> chunk[b][i][0 .. CS), asynchronously
+    const int l = l0 + lane;
+    if (l < L) {
+      const int right = l < L - 1 ? s[l + 1] : 0;
+      const unsigned char* src = Bp_ + ((size_t)l * K + right) * CS;
+      unsigned char* dst = chunk + ((size_t)b * 32 + lane) * CS;
+      for (int q = 0; q < CS / 16; ++q) cp_async16(dst + 16 * q, src + 16 * q);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  int nsweeps = 0;
+  for (;;) {                                               // (the sweep of cd_lookup_kernel with identity classes)
+    bool changed = false, carry = false, have = false;
+    int aprev = 0, cb = 0;
+    for (int l0 = 0; l0 < L; l0 += 32) {
+      const int n = L - l0 < 32 ? L - l0 : 32;
+      int sreg = lane < n ? s[l0 + lane] : 0;
+      const unsigned dmask = __ballot_sync(0xffffffffu, lane < n && dirty[l0 + lane]);
+      if (dmask == 0 && !carry) {
+        aprev = __shfl_sync(0xffffffffu, sreg, n - 1);
+        if (have) asm volatile("cp.async.wait_group 0;" ::: "memory");
+        have = false;
+        continue;
+      }
+      if (!have) fetch(l0, cb);
+      const bool ahead = l0 + 32 < L;
+      if (ahead) fetch(l0 + 32, cb ^ 1);
+      if (ahead) asm volatile("cp.async.wait_group 1;" ::: "memory"); else asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+      const uint16_t* colb = reinterpret_cast<const uint16_t*>(chunk + (size_t)cb * 32 * CS);
+      const int i0 = carry ? 0 : __ffs(dmask) - 1;
+      if (i0 > 0) aprev = __shfl_sync(0xffffffffu, sreg, i0 - 1);
+      int mine = sreg;
+      for (int i = i0; i < n; ++i) {
+        const int e = colb[i * (CS / 2) + aprev] & 255;
+        if (lane == i) mine = e;
+        aprev = e;
+      }
+      const unsigned chm = __ballot_sync(0xffffffffu, lane < n && mine != sreg);
+      if (chm) changed = true;
+      carry = chm >> (n - 1) & 1;
+      const unsigned dnext = chm >> 1;
+      if ((chm & 1) && l0 > 0 && lane == 0) dirty[l0 - 1] = 1;
+      sreg = mine;
+      if (lane < n) {
+        s[l0 + lane] = (uint8_t)sreg;
+        dirty[l0 + lane] = dnext >> lane & 1;
+      }
+      __syncwarp();
+      cb ^= 1;
+      have = l0 + 32 < L;
+    }
+    ++nsweeps;
+    if (!changed || nsweeps >= max_sweeps) break;
+    __syncwarp();
+  }
+  __syncwarp();
+  const int64_t* Tp = T + p * (size_t)L * K * K;           // Cost(s) = sum_l T[l][s_{l-1}][s_l]   (s_{-1} := 0)
+  int64_t acc = 0;
+  for (int l = lane; l < L; l += 32) {
+    const int sl = s[l], sp = l > 0 ? s[l - 1] : 0;
+    acc += __ldg(Tp + ((size_t)l * K + sp) * K + sl);
+    strategy[ps * L + l] = sl;
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+  if (lane == 0) {
+    cost[ps] = acc;
+    sweeps[ps] = nsweeps;
+  }
+}
+
 template <int D>
 int launch_factors_d(const autoddl_layer* d_layers, int32_t Bp, int32_t L, const MeshParams& mp, int64_t* d_F, cudaStream_t st) {
   const int ntiles = Bp * L, sms = device_sm_count();
@@ -482,6 +612,44 @@ int launch_cd_lookup(const int64_t* d_F, int32_t Bp, int32_t L, const MeshParams
   uint8_t* d_BR = (uint8_t*)d_work;
   if (mp.ndim == 2) return launch_lookup_d<2>(Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
   return launch_lookup_d<3>(Bp, L, mp, d_F, d_BR, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st);
+}
+
+// best-response look-ups on K x K tables: any mesh, K <= 64, >= 32 starts per problem
+bool cd_lookup_tab_supported(int32_t K, int32_t L, int32_t S) { return K <= 64 && S >= 32 && L <= 16384; }
+
+static inline size_t tab_cs(int32_t K) { return ((size_t)2 * K + 15) / 16 * 16; }
+
+size_t cd_lookup_tab_workspace_bytes(int32_t K, int32_t Bp, int32_t L) { return ((size_t)Bp * L * K * tab_cs(K) + 255) / 256 * 256 + 256; }
+
+int launch_cd_lookup_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* d_work, const int32_t* d_init, int32_t S,
+                         int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+  uint8_t* d_BR = (uint8_t*)d_work;
+  const int CS = (int)tab_cs(K);
+  const int64_t nt64 = (int64_t)Bp * L;
+  if (nt64 > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
+  const int ntiles = (int)nt64, sms = device_sm_count();
+  {
+    const size_t smem = (size_t)2 * K * K * 8;
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(best_response_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int grid = ntiles < sms * 2 ? ntiles : sms * 2;
+    best_response_tab_kernel<<<grid, 512, smem, st>>>(d_T, ntiles, L, K, CS, d_BR);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  {
+    const int W = 4;
+    const size_t per_warp = ((size_t)2 * 32 * CS + 2 * (size_t)L + 15) & ~(size_t)15;
+    const size_t smem = W * per_warp;
+    if (smem > 200 * 1024) { set_error("coord_descent: L too large"); return AUTODDL_EINVAL; }
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(cd_lookup_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t nb = ((int64_t)Bp * S + W - 1) / W;
+    if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
+    cd_lookup_tab_kernel<<<(unsigned)nb, W * 32, smem, st>>>(d_T, d_BR, Bp, L, K, CS, S, d_init, max_sweeps, d_cost, d_strategy, d_sweeps,
+                                                             (int)per_warp);
+    count_launch();
+    ADL_CUDA_CHECK(cudaGetLastError());
+  }
+  return AUTODDL_OK;
 }
 
 }  // namespace autoddl

@@ -83,3 +83,38 @@ def test_random_workloads_both_routes(adl):
                            ("search.cost", o["cd_cost"], occ), ("search.strategy", o["cd_strategy"], ocs), ("search.sweeps", o["cd_sweeps"], osw),
                            ("gather.cost", b[0], occ), ("gather.strategy", b[1], ocs), ("gather.sweeps", b[2], osw), ("T", o["T"], oT)):
             assert np.array_equal(g.cpu().numpy(), x), (name, info)
+
+
+# ---- the same look-up scheme on K x K tables (K <= 64): caller-supplied tables, random ones with many ties -----------------
+def _mesh_with_k(K):
+    if K == 36:
+        return cf.Mesh((4, 4), (cf.INTER, cf.INTRA))
+    if K == 16:
+        return cf.Mesh((2, 2, 2, 2), tuple(l | (0x03 << 8) for l in (cf.INTER, cf.INTER, cf.INTRA, cf.INTRA)))
+    if K == 64:
+        return cf.Mesh((2, 2, 2, 2), (cf.INTER | (0x0f << 8), cf.INTER | (0x0f << 8), cf.INTRA | (0x03 << 8), cf.INTRA | (0x03 << 8)))
+    n = 6 if K == 28 else 8
+    return cf.Mesh((2,) * n, (cf.INTER | cf.FOLD,) + (cf.INTER,) * (n - 1))
+
+
+@pytest.mark.parametrize("K,L,Bp,S,hi,cap", [(36, 1, 2, 32, 5, 64), (36, 2, 3, 33, 1 << 40, 64), (16, 31, 2, 40, 3, 64), (28, 32, 1, 64, 4, 64),
+                                             (45, 33, 2, 32, 6, 64), (45, 97, 1, 50, 1 << 45, 3), (64, 64, 2, 32, 4, 64),
+                                             (64, 130, 1, 100, 9, 64), (36, 65, 5, 64, 3, 1)])
+def test_lookup_cd_on_tables(adl, K, L, Bp, S, hi, cap):
+    """trajectory, sweep count and result of the plain algorithm (R10: smallest-index argmin, Gauss-Seidel order, dirty
+    layers) on random tables -- cells in [0, hi) for a small hi tie nearly every update --, also with a sweep cap"""
+    mesh = _mesh_with_k(K)
+    assert adl.num_signatures(mesh) == K
+    rng = np.random.default_rng(K * 977 + L)
+    T = rng.integers(0, hi, size=(Bp, L, K, K), dtype=np.int64)
+    init = rng.integers(0, K, size=(Bp, S, L), dtype=np.int32)
+    want = ref.coord_descent(T, init, cap)
+    d_T, d_init = torch.from_numpy(T).cuda(), torch.from_numpy(init).cuda()
+    work = torch.empty(adl.workspace_bytes(Bp, L, S, mesh), dtype=torch.uint8, device="cuda")
+    work.fill_(0xC3)
+    got = adl.coord_descent(d_T, d_init, mesh, cap, work=work)          # best responses from the tiles + look-up sweeps
+    plain = adl.coord_descent(d_T, d_init, mesh, cap)                   # no workspace: the gather kernel
+    torch.cuda.synchronize()
+    for name, g, q, x in zip(("cd_cost", "cd_strategy", "cd_sweeps"), got, plain, want):
+        assert np.array_equal(g.cpu().numpy(), x), name
+        assert np.array_equal(q.cpu().numpy(), x), name + " (gather kernel)"
