@@ -532,7 +532,9 @@ def run_configs(args):
         g = {
             "build_us": gpu_us(lambda: adl.build_tables(dl, w.mesh, w.net, want_node_mask=False, out=T)),
             "dp_us": gpu_us(lambda: adl.chain_dp(T, w.mesh, work=work, out=dp)),
-            "cd_us": gpu_us(lambda: adl.coord_descent(T, init, w.mesh, w.max_sweeps, out=cd)),
+            "cd_us": gpu_us(lambda: adl.coord_descent(T, init, w.mesh, w.max_sweeps, out=cd)),          # no workspace: the gather kernel
+            # with a workspace: K <= 64 and >= 32 starts take best responses from the tiles + look-up sweeps
+            "cd_work_us": gpu_us(lambda: adl.coord_descent(T, init, w.mesh, w.max_sweeps, work=work, out=cd)),
             # d_T = NULL: no K x K table; with >= 32 starts per problem on 2 / 3 mesh levels factors -> best responses -> look-ups
             "cd_no_table_us": gpu_us(lambda: adl.coord_descent(None, init, w.mesh, w.max_sweeps, net=w.net, d_layers=dl, work=work, out=cd)),
             "search_us": gpu_us(lambda: adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out=one)),
