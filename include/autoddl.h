@@ -190,6 +190,23 @@ int autoddl_search_host(const autoddl_layer* h_layers, int32_t Bp, int32_t L,
                         int64_t* h_opt_cost, int32_t* h_strategy,
                         int64_t* h_cd_cost, int32_t* h_cd_strategy, int32_t* h_cd_sweeps, void* stream);
 
+/* (a2) on caller-supplied tables WITHOUT any allocation and without a workspace argument, for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the layer-parallel chain DP
+ * of autoddl_chain_dp for K <= 64 with its scratch -- chunk products, prefix vectors,
+ * back-pointers -- in a static device array of AUTODDL_STATIC_SCRATCH_BYTES that every GPU loading the library holds until
+ * exit.  Same results as autoddl_chain_dp (same optimum, smallest index on every tie).
+ * d_T [Bp][L][K][K] int64 (8-byte aligned), d_opt_cost [Bp] int64, d_strategy [Bp][L] int32: device pointers, owned by
+ * the caller.  Accepted: K <= 64, 1 <= Bp <= 64, L >= 32 (AUTODDL_EINVAL otherwise), and
+ * autoddl_chain_dp_static_bytes(Bp, L, mesh) <= AUTODDL_STATIC_SCRATCH_BYTES (AUTODDL_EWORK otherwise: use
+ * autoddl_chain_dp with a workspace).  Calls no cudaMalloc / cudaFree / allocating routine; asynchronous on `stream`.
+ * ALL calls on a device share the one array, which keeps the last call's contents (nothing needs to start at zero):
+ * calls that overlap on the GPU -- two streams, two host threads -- race; serialise them. */
+#define AUTODDL_STATIC_SCRATCH_BYTES (8u << 20)
+int autoddl_chain_dp_static(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_mesh* mesh,
+                            int64_t* d_opt_cost, int32_t* d_strategy, void* stream);
+/* Bytes of the static array a call with (Bp, L, mesh) uses; 0 if the arguments are outside the accepted ranges. Host only. */
+size_t autoddl_chain_dp_static_bytes(int32_t Bp, int32_t L, const autoddl_mesh* mesh);
+
 /* Best of the Coordinate Descent starts ("records the best strategy"): for every problem p the smallest
  * d_cost[p][s] over s = 0..S-1 and the smallest s attaining it.  d_cost [Bp][S] int64, d_best_cost [Bp] int64,
  * d_best_start [Bp] int32: device pointers, 8 / 4-byte aligned; Bp, S >= 1.  Asynchronous on `stream`. */

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
-    "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_pipeline_workspace_bytes", "autoddl_segment_optima", "autoddl_stage_transfer",
+    "autoddl_chain_dp_static", "autoddl_chain_dp_static_bytes", "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_pipeline_workspace_bytes", "autoddl_segment_optima", "autoddl_stage_transfer",
     "autoddl_pipeline_partition", "autoddl_segment_strategies", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
@@ -58,6 +58,10 @@ def lib():
         L.autoddl_build_tables.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp]
         L.autoddl_chain_dp.restype = C.c_int
         L.autoddl_chain_dp.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, vp, vp]
+        L.autoddl_chain_dp_static.restype = C.c_int
+        L.autoddl_chain_dp_static.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+        L.autoddl_chain_dp_static_bytes.restype = sz
+        L.autoddl_chain_dp_static_bytes.argtypes = [i32, i32, vp]
         L.autoddl_coord_descent.restype = C.c_int
         L.autoddl_coord_descent.argtypes = [vp, i32, i32, vp, vp, vp, vp, sz, vp, i32, i32, vp, vp, vp, vp]
         L.autoddl_metropolis.restype = C.c_int
@@ -262,6 +266,24 @@ def fit_alpha_beta(kind: torch.Tensor, p: torch.Tensor, nbytes: torch.Tensor, t:
         work = torch.empty(int(lib().autoddl_fit_workspace_bytes()), dtype=torch.uint8, device=dev)
     _check(lib().autoddl_fit_alpha_beta(_ptr(kind, I32, "kind"), _ptr(p, I32, "p"), _ptr(nbytes, I64, "nbytes"), _ptr(t, F64, "t"), N,
                                         _ptr(out, F64, "out"), _ptr(work, U8, "work"), work.numel(), _stream()))
+    return out
+
+
+STATIC_SCRATCH_BYTES = 8 << 20   # AUTODDL_STATIC_SCRATCH_BYTES
+
+
+def chain_dp_static_bytes(Bp: int, L: int, mesh) -> int:
+    m = c_mesh(mesh)
+    return int(lib().autoddl_chain_dp_static_bytes(Bp, L, C.addressof(m)))
+
+
+def chain_dp_static(T: torch.Tensor, mesh, out):
+    """(a2) on tables with K <= 64 with the scratch in the library's static device array (autoddl_chain_dp_static): no
+    allocation here or in the library -- `out` = (opt_cost int64 [Bp], strategy int32 [Bp, L]) is the caller's."""
+    Bp, L = T.shape[0], T.shape[1]
+    m = c_mesh(mesh)
+    _check(lib().autoddl_chain_dp_static(_ptr(T, I64, "T"), Bp, L, C.addressof(m), _ptr(out[0], I64, "opt_cost"),
+                                         _ptr(out[1], I32, "strategy"), _stream()))
     return out
 
 

@@ -733,3 +733,75 @@ int launch_chain_dp_scan_tab(const int64_t* d_T, int32_t Bp, int32_t L, int32_t 
   return launch_dp_scan_tab(d_T, Bp, L, K, (unsigned char*)d_work, d_opt_cost, d_strategy, st);
 }
 }  // namespace autoddl
+
+// ---- autoddl_chain_dp_static: the layer-parallel chain DP on K x K tables with its scratch in a STATIC device array ----------
+// For callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
+// the chunk products Q, the prefix vectors V, the last signatures and the back-pointers of launch_dp_scan_tab live in a
+// file-scope array of AUTODDL_STATIC_SCRATCH_BYTES; every GPU that loads the library holds it until exit.  In host code
+// the array's name is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress, once per
+// device, with that device current.  No cudaMalloc / cudaFree / allocating library routine is called here or in the
+// launcher.  Nothing has to start at zero: every word a kernel of the call reads was written by an earlier kernel of the same
+// call (the array keeps the last call's contents; tests poison it).  All calls share the array: calls that overlap on the
+// GPU (two streams, two host threads) race.
+namespace autoddl {
+namespace {
+
+static __device__ __align__(256) unsigned char g_static_scratch[AUTODDL_STATIC_SCRATCH_BYTES];
+
+constexpr int kMaxDevices = 64;
+void* g_static_ptr[kMaxDevices];                           // device address of g_static_scratch per device (NULL: not asked yet)
+
+// device address of the array on the CURRENT device; AUTODDL_OK or AUTODDL_ECUDA
+int static_scratch_address(void** out) {
+  int dev = -1;
+  ADL_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) { set_error("chain_dp_static: device %d out of range", dev); return AUTODDL_ECUDA; }
+  void* p = __atomic_load_n(&g_static_ptr[dev], __ATOMIC_ACQUIRE);
+  if (p == nullptr) {
+    ADL_CUDA_CHECK(cudaGetSymbolAddress(&p, g_static_scratch));      // (the same value whichever thread asks first)
+    if (p == nullptr) { set_error("chain_dp_static: cudaGetSymbolAddress returned NULL"); return AUTODDL_ECUDA; }
+    __atomic_store_n(&g_static_ptr[dev], p, __ATOMIC_RELEASE);
+  }
+  *out = p;
+  return AUTODDL_OK;
+}
+
+}  // namespace
+}  // namespace autoddl
+
+extern "C" {
+
+size_t autoddl_chain_dp_static_bytes(int32_t Bp, int32_t L, const autoddl_mesh* mesh) {
+  using namespace autoddl;
+  clear_error();
+  MeshParams mp;
+  if (validate_mesh_net(mesh, nullptr, &mp) || Bp < 1 || L < 1) return 0;
+  if (!chain_dp_scan_tab_supported(mp.K, Bp, L)) return 0;
+  return chain_dp_scan_tab_bytes(mp.K, Bp, L);
+}
+
+int autoddl_chain_dp_static(const int64_t* d_T, int32_t Bp, int32_t L, const autoddl_mesh* mesh, int64_t* d_opt_cost,
+                            int32_t* d_strategy, void* stream) {
+  using namespace autoddl;
+  clear_error();
+  MeshParams mp;
+  int rc = validate_mesh_net(mesh, nullptr, &mp);
+  if (rc) return rc;
+  ADL_REQUIRE(d_T != nullptr && d_opt_cost != nullptr && d_strategy != nullptr, "NULL pointer");
+  ADL_REQUIRE(((uintptr_t)d_T & 7) == 0 && ((uintptr_t)d_opt_cost & 7) == 0 && ((uintptr_t)d_strategy & 3) == 0, "misaligned pointer");
+  ADL_REQUIRE(Bp >= 1 && L >= 1, "Bp = %d, L = %d must be >= 1", Bp, L);
+  const int K = mp.K;
+  ADL_REQUIRE(chain_dp_scan_tab_supported(K, Bp, L),
+              "chain_dp_static: K = %d, Bp = %d, L = %d outside K <= 64, Bp <= 64, L >= 32 (use autoddl_chain_dp)", K, Bp, L);
+  const size_t need = chain_dp_scan_tab_bytes(K, Bp, L);
+  if (need > (size_t)AUTODDL_STATIC_SCRATCH_BYTES) {
+    set_error("chain_dp_static: %zu bytes of scratch needed, the static array holds %zu (use autoddl_chain_dp with a workspace)",
+              need, (size_t)AUTODDL_STATIC_SCRATCH_BYTES);
+    return AUTODDL_EWORK;
+  }
+  void* scratch = nullptr;
+  if ((rc = static_scratch_address(&scratch))) return rc;
+  return launch_chain_dp_scan_tab(d_T, Bp, L, K, scratch, d_opt_cost, d_strategy, (cudaStream_t)stream);
+}
+
+}  // extern "C"
