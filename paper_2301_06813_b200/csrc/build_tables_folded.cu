@@ -17,6 +17,9 @@ struct FoldSmem {
   int64_t Q[5][256];                                     // M, Kd, N, in_rows, in_cols  x  level subset
   int64_t VP[256];
   uint16_t dig[256];                                     // per signature: row (0, 1, 2) of level d at bits 2d
+  // per (layer kind, signature), once per CTA: packed output states, input states and their duals (two bits per level);
+  // bit 31 of stO = invalid for the kind
+  uint32_t stO[2][256], stI[2][256], duO[2][256], duI[2][256];
   RecBuf rec;
 };
 
@@ -85,7 +88,7 @@ __device__ int64_t fold_walk(uint32_t a, uint32_t b, int D, const int64_t* __res
 }
 
 __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const autoddl_layer* __restrict__ layers, int ntiles, int L,
-                                                                      MeshParams mp, int64_t* __restrict__ T,
+                                                                      int chunks, MeshParams mp, int64_t* __restrict__ T,
                                                                       int64_t* __restrict__ node, uint8_t* __restrict__ mask) {
   __shared__ FoldSmem sm;
   const int tid = threadIdx.x, D = mp.ndim, K = mp.K;
@@ -105,9 +108,22 @@ __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const auto
     }
     sm.dig[j] = (uint16_t)dg;
   }
+  __syncthreads();
+  for (int x = tid; x < 2 * K; x += kFoldNT) {
+    const int kind = x / K, j = x % K;
+    uint32_t sI, sW, sO;
+    const bool valid = fold_states(kind, sm.dig[j], D, sI, sW, sO);
+    sm.stO[kind][j] = sO | (valid ? 0u : 1u << 31);
+    sm.stI[kind][j] = sI;
+    sm.duO[kind][j] = fold_dual(sO, D);
+    sm.duI[kind][j] = fold_dual(sI, D);
+  }
   const int64_t cap_layer = mp.mem_cap / L;
 
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  // a unit = (tile, chunk of its cells): few tiles (one model) are split so that every SM holds several CTAs -- the walk of
+  // a cell is a long dependent chain, and occupancy is what hides it; Q and VP are recomputed per unit (cheap next to the cells)
+  for (int unit = blockIdx.x; unit < ntiles * chunks; unit += gridDim.x) {
+    const int tile = unit / chunks, chunk = unit % chunks;
     const int l = tile % L;
     __syncthreads();                                     // the previous tile's readers are done
     if (tid == 0) {
@@ -126,7 +142,8 @@ __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const auto
       int64_t f = 1;
       for (int d = 0; d < D; ++d)
         if (m >> d & 1) f *= mp.size[d];
-      sm.Q[x][m] = (rec.X[x] + f - 1) / f;
+      // (f <= 2^20; a power of two on the usual machines: an add and a shift instead of a 64-bit division)
+      sm.Q[x][m] = (f & (f - 1)) == 0 ? (rec.X[x] + f - 1) >> (63 - __clzll(f)) : (rec.X[x] + f - 1) / f;
     }
     __syncthreads();
     // ---- 2. VP[j] = weight-gradient all-reduce + penalty ------------------------------------------------
@@ -160,21 +177,21 @@ __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const auto
       }
       const bool ok = valid && rs <= rec.maxr && cs <= rec.maxc && (mp.mem_cap == 0 || mem <= cap_layer);
       sm.VP[j] = v + (ok ? 0 : AUTODDL_PEN);
-      if (node) node[(size_t)tile * K + j] = v;
-      if (mask) mask[(size_t)tile * K + j] = ok ? 1 : 0;
+      if (node && chunk == 0) node[(size_t)tile * K + j] = v;
+      if (mask && chunk == 0) mask[(size_t)tile * K + j] = ok ? 1 : 0;
     }
     __syncthreads();
     // ---- 3. the cells: forward + backward redistribution (R5), once per micro-batch (R25) -------------------------------------
     int64_t* out = T + (size_t)tile * K * K;
-    for (int c = tid; c < K * K; c += kFoldNT) {
+    const int per = (K * K + chunks - 1) / chunks, c_end = (chunk + 1) * per < K * K ? (chunk + 1) * per : K * K;
+    for (int c = chunk * per + tid; c < c_end; c += kFoldNT) {
       const int i = c / K, j = c % K;
       int64_t e = 0;
       if (l > 0) {
-        uint32_t aI, aW, aO, bI, bW, bO;
-        const bool vi = fold_states(rec.kind_prev, sm.dig[i], D, aI, aW, aO);
-        const bool vj = fold_states(rec.kind, sm.dig[j], D, bI, bW, bO);
-        if (vi && vj)
-          e = fold_walk(aO, bI, D, sm.Q[3], sm.Q[4], rec.eb, mp) + fold_walk(fold_dual(bI, D), fold_dual(aO, D), D, sm.Q[3], sm.Q[4], rec.eb, mp);
+        const uint32_t aO = sm.stO[rec.kind_prev][i], vj = sm.stO[rec.kind][j];
+        if (!((aO | vj) >> 31))
+          e = fold_walk(aO, sm.stI[rec.kind][j], D, sm.Q[3], sm.Q[4], rec.eb, mp) +
+              fold_walk(sm.duI[rec.kind][j], sm.duO[rec.kind_prev][i], D, sm.Q[3], sm.Q[4], rec.eb, mp);
       }
       out[c] = mp.accum * e + sm.VP[j];
     }
@@ -188,8 +205,14 @@ int launch_build_tables_folded(const autoddl_layer* d_layers, int32_t Bp, int32_
   const int64_t nt = (int64_t)Bp * L;
   if (nt > 0x7fffffff) { set_error("Bp*L too large"); return AUTODDL_EINVAL; }
   const int slots = device_sm_count() * 4;
-  const int grid = (int)(nt < slots ? nt : slots);
-  build_tables_folded_kernel<<<grid, kFoldNT, 0, st>>>(d_layers, (int)nt, L, mp, d_T, d_node, d_mask);
+  int chunks = (int)((2 * slots + nt - 1) / nt);                         // few tiles: split them into blocks of cells
+  const int max_chunks = (mp.K * mp.K + kFoldNT - 1) / kFoldNT;          // (at least one cell per thread)
+  if (chunks > max_chunks) chunks = max_chunks;
+  if (chunks < 1) chunks = 1;
+  if (nt * chunks > 0x7fffffff) chunks = 1;
+  const int64_t units = nt * chunks;
+  const int grid = (int)(units < slots ? units : slots);
+  build_tables_folded_kernel<<<grid, kFoldNT, 0, st>>>(d_layers, (int)nt, L, chunks, mp, d_T, d_node, d_mask);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
