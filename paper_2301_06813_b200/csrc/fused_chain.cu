@@ -100,33 +100,14 @@ __device__ __forceinline__ void warp_argmin64(int64_t& bv, int& bi) {
   }
 }
 
-template <int NB>
-__global__ void __launch_bounds__(896, 1)
-fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, MeshParams mp,
-                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
-                     int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
-                     const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1, int32_t* __restrict__ cd_s2,
-                     int per_warp_bytes) {
-  extern __shared__ __align__(128) unsigned char fsm_raw[];
-  CtaShared& cs = *reinterpret_cast<CtaShared*>(fsm_raw);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
-  unsigned char* wbase = fsm_raw + ((sizeof(CtaShared) + 127) & ~(size_t)127) + (size_t)warp * per_warp_bytes;
-  using WS = WarpShared<NB>;
-  WS& ws = *reinterpret_cast<WS*>(wbase);
-  // CD only: the row stash of sweep 2 [cd_S][36] int64, then the strategies of the chain's starts after sweep 1 and
-  // sweep 2 [2][cd_S][L] bytes; then the back-pointers [L][K] (or a workspace slice: bp_glob)
-  int64_t* cd_stash2 = reinterpret_cast<int64_t*>(wbase + sizeof(WS));
-  uint8_t* cd_s = wbase + sizeof(WS) + (cd_init ? (size_t)cd_S * FK * 8 : 0);
-  uint8_t* cd_t = cd_s + (size_t)cd_S * L;
-  const size_t cd_bytes = cd_init ? (((size_t)2 * cd_S * L + 15) & ~(size_t)15) : 0;
-  uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
-  const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well (NB = 2 whenever CD rides along)
-
+// Everything a CTA needs besides the tile data: facts per (layer kind, signature) -- the only part that depends on the mesh
+// --, the layout of G and the byte index tables of its consumers.  All threads of the CTA (nthr of them) call it.
+__device__ __forceinline__ void fused_cta_setup(CtaShared& cs, const MeshParams& mp, int tid, int nthr) {
   // ---- once per CTA: facts per (layer kind, signature), the layout of G, the index tables ---------------------------
-  fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);
+  fill_sig_table<FD>(cs.sig, mp, tid, nthr);
   if (tid >= 32 && tid < 48) cs.walk[tid - 32] = c_walk.w[tid - 32];
   if (tid >= 64 && tid < 64 + FNU) { cs.ucol[tid - 64] = c_ucol[tid - 64]; cs.uhi[tid - 64] = c_uhi[tid - 64]; }
-  if (blockDim.x < 96 && tid < 16) {                       // (a CTA of one or two warps)
+  if (nthr < 96 && tid < 16) {                       // (a CTA of one or two warps)
     cs.walk[tid] = c_walk.w[tid];
     if (tid < FNU) { cs.ucol[tid] = c_ucol[tid]; cs.uhi[tid] = c_uhi[tid]; }
   }
@@ -139,7 +120,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     const uint32_t firsts = __ballot_sync(0xffffffffu, tid < 16 && rep == x);
     if (tid < 16) cs.ucls[x] = (uint8_t)__popc(firsts & ((1u << rep) - 1));
   }
-  for (int x = tid; x < 5 * 32; x += blockDim.x) (&cs.lslot[0][0])[x] = FNC | FNC << 6 | FNC << 12 | FNC << 18;   // zero slots (lslot, hslot)
+  for (int x = tid; x < 5 * 32; x += nthr) (&cs.lslot[0][0])[x] = FNC | FNC << 6 | FNC << 12 | FNC << 18;   // zero slots (lslot, hslot)
   __syncthreads();
   constexpr uint32_t kNoSlots = FNC | FNC << 6 | FNC << 12 | FNC << 18;
   // the summands of entry e = (u0, u1), 6 bits each in w0 (first four) and w1; returns their number
@@ -169,13 +150,13 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     take();
     return n;
   };
-  for (int e = tid; e < FNU * FNU; e += blockDim.x) {
+  for (int e = tid; e < FNU * FNU; e += nthr) {
     uint32_t w0, w1;
     cs.nnz[e] = (uint8_t)entry_slots(e, w0, w1);
     cs.ew[0][e] = w0;
     cs.ew[1][e] = w1;
   }
-  for (int x = tid; x < 2 * FK; x += blockDim.x) {
+  for (int x = tid; x < 2 * FK; x += nthr) {
     const SigInfo& si = cs.sig[x / FK][x % FK];
     cs.bcls[x / FK][x % FK] = (uint8_t)(si.b_idx >= 0 ? si.b_idx : FNS);
   }
@@ -184,11 +165,11 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     if (a >= FNS || b < 0 || b >= FNS) return FGZ;
     return upos(cs.ucls[(a >> 2) << 2 | (b >> 2)], cs.ucls[(a & 3) << 2 | (b & 3)]);
   };
-  for (int x = tid; x < 4 * FCELLS; x += blockDim.x) {
+  for (int x = tid; x < 4 * FCELLS; x += nthr) {
     const int kk = x / FCELLS, i = x % FCELLS / FK, j = x % FK;
     cs.GI[kk >> 1][kk & 1][i][j] = (uint8_t)gp(cs.sig[kk >> 1][i].a_idx, cs.sig[kk & 1][j].b_idx);
   }
-  for (int x = tid; x < 2 * 2 * 16 * 16; x += blockDim.x) {
+  for (int x = tid; x < 2 * 2 * 16 * 16; x += nthr) {
     // DP: lane (b, half) scans rows 18 half + 6 part + r; rows whose level-1 digit r is 2, 4 or 5 share their edge (all
     // output P, or all invalid), so a part has four distinct values q = 0..3 for r = 0, 1, 3, 2
     const int kp = x >> 9, half = x >> 8 & 1, bcl = x >> 4 & 15, part = (x & 15) >> 2, q = x & 3;
@@ -196,7 +177,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     cs.DPI[kp][half][bcl][x & 15] = (uint8_t)(part < 3 ? gp(cs.sig[kp][row].a_idx, bcl) : FGZ);
   }
   __syncthreads();
-  for (int e = tid; e < FNU * FNU; e += blockDim.x) {      // computed in order of ascending number of summands, then (u0, u1)
+  for (int e = tid; e < FNU * FNU; e += nthr) {      // computed in order of ascending number of summands, then (u0, u1)
     const int my_n = cs.nnz[e];
     int rank = 0, nl = 0, nh = 0;
     for (int o = 0; o < FNU * FNU; ++o) {
@@ -216,7 +197,7 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
       cs.hslot[1][rank - nl] = cs.ew[1][e] | pos << 24;
     }
   }
-  for (int x = tid; x < 4 * 6 * 32; x += blockDim.x) {
+  for (int x = tid; x < 4 * 6 * 32; x += nthr) {
     // tile expansion: lane (h, pc), class row n = 3 c0 + t -> row (rep(c0), 3 h + t); bytes 2 n, 2 n + 1 = its two columns
     const int kk = x / 192, w = x % 192 / 32, ln = x % 32, pc = ln & 15, h = ln >> 4;
     uint32_t word = 0;
@@ -228,6 +209,72 @@ fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, Me
     cs.XI[kk >> 1][kk & 1][w][ln] = word;
   }
   __syncthreads();
+}
+
+// The tables above except `sig` are the same for every mesh, launch and CTA: the first launch on a device also runs
+// fused_tables_init_kernel, which leaves them in g_fused_tables and then raises g_fused_ready; a CTA that finds the flag up
+// copies 12 KB instead of spending ~18 us computing them (kernels that run before the flag is up compute them as before:
+// same values either way).
+static __device__ __align__(16) unsigned char g_fused_tables[(sizeof(CtaShared) + 15) / 16 * 16];
+static __device__ int g_fused_ready = 0;
+
+__global__ void __launch_bounds__(896) fused_tables_init_kernel(MeshParams mp) {
+  extern __shared__ __align__(128) unsigned char fti_raw[];
+  CtaShared& cs = *reinterpret_cast<CtaShared*>(fti_raw);
+  fused_cta_setup(cs, mp, threadIdx.x, blockDim.x);
+  __syncthreads();
+  const uint4* src = reinterpret_cast<const uint4*>(fti_raw);
+  uint4* dst = reinterpret_cast<uint4*>(g_fused_tables);
+  for (int x = threadIdx.x; x < (int)(sizeof(g_fused_tables) / 16); x += blockDim.x) dst[x] = src[x];
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    *reinterpret_cast<volatile int*>(&g_fused_ready) = 1;
+  }
+}
+
+template <int NB>
+__global__ void __launch_bounds__(896, 1)
+fused_chain36_kernel(const autoddl_layer* __restrict__ layers, int Bp, int L, MeshParams mp,
+                     int64_t* __restrict__ T, int64_t* __restrict__ node, uint8_t* __restrict__ mask,
+                     int64_t* __restrict__ opt_cost, int32_t* __restrict__ strategy, uint8_t* __restrict__ bp_glob,
+                     const int32_t* __restrict__ cd_init, int cd_S, int32_t* __restrict__ cd_s1, int32_t* __restrict__ cd_s2,
+                     int per_warp_bytes) {
+  extern __shared__ __align__(128) unsigned char fsm_raw[];
+  CtaShared& cs = *reinterpret_cast<CtaShared*>(fsm_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+  unsigned char* wbase = fsm_raw + ((sizeof(CtaShared) + 127) & ~(size_t)127) + (size_t)warp * per_warp_bytes;
+  using WS = WarpShared<NB>;
+  WS& ws = *reinterpret_cast<WS*>(wbase);
+  // CD only: the row stash of sweep 2 [cd_S][36] int64, then the strategies of the chain's starts after sweep 1 and
+  // sweep 2 [2][cd_S][L] bytes; then the back-pointers [L][K] (or a workspace slice: bp_glob)
+  int64_t* cd_stash2 = reinterpret_cast<int64_t*>(wbase + sizeof(WS));
+  uint8_t* cd_s = wbase + sizeof(WS) + (cd_init ? (size_t)cd_S * FK * 8 : 0);
+  uint8_t* cd_t = cd_s + (size_t)cd_S * L;
+  const size_t cd_bytes = cd_init ? (((size_t)2 * cd_S * L + 15) & ~(size_t)15) : 0;
+  uint8_t* bp = bp_glob ? bp_glob + ((size_t)blockIdx.x * W + warp) * (size_t)L * FK : cd_s + cd_bytes;   // [L][K]
+  const bool two = NB == 2 && cd_s2 != nullptr;            // second CD sweep in this kernel as well (NB = 2 whenever CD rides along)
+
+  // ---- once per CTA: the index tables (from the device-wide copy when it is there) and the facts per signature ------------
+  {
+    __shared__ int s_ready;
+    if (tid == 0) {
+      s_ready = *reinterpret_cast<volatile int*>(&g_fused_ready);
+      __threadfence();                                     // (the tables are read after the flag)
+    }
+    __syncthreads();
+    if (s_ready) {
+      const uint4* src = reinterpret_cast<const uint4*>(g_fused_tables);
+      uint4* dst = reinterpret_cast<uint4*>(fsm_raw);
+      for (int x = tid; x < (int)(sizeof(g_fused_tables) / 16); x += blockDim.x) dst[x] = __ldcg(src + x);
+      __syncthreads();
+      fill_sig_table<FD>(cs.sig, mp, tid, blockDim.x);     // the mesh-dependent part: this launch's mesh
+      __syncthreads();
+    } else {
+      fused_cta_setup(cs, mp, tid, blockDim.x);
+    }
+  }
   const int g_nl = cs.nl, g_nh = cs.nh;
 
   // ---- once per warp: tile-invariant roles of this lane ---------------------------------------------------------
@@ -716,6 +763,18 @@ int launch_build_dp_fused(const autoddl_layer* d_layers, int32_t Bp, int32_t L, 
   if (!bp_smem && d_bp == nullptr) { set_error("fused build+DP: back-pointer workspace missing"); return AUTODDL_EWORK; }
   const size_t per_warp = warp_bytes(L, cdS, bp_smem);
   const size_t smem = fixed + (size_t)W * per_warp;
+  {
+    // first launch on this device: also leave the mesh-independent index tables in device memory for every later CTA (the
+    // kernels of this stream are ordered behind it; kernels of other streams that start earlier compute the tables themselves)
+    static bool launched[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && !__atomic_load_n(&launched[dev], __ATOMIC_ACQUIRE)) {
+      ADL_CUDA_CHECK(cudaFuncSetAttribute(fused_tables_init_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CtaShared) + 128));
+      fused_tables_init_kernel<<<1, 896, sizeof(CtaShared) + 128, st>>>(mp);
+      ADL_CUDA_CHECK(cudaGetLastError());
+      __atomic_store_n(&launched[dev], true, __ATOMIC_RELEASE);
+    }
+  }
   auto kern = cdS > 0 ? fused_chain36_kernel<2> : fused_chain36_kernel<1>;   // CD reads the previous layer's factors
   ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, W * 32, smem, st>>>(d_layers, Bp, L, mp, d_T, d_node, d_mask, d_opt_cost, d_strategy, bp_smem ? nullptr : d_bp,
