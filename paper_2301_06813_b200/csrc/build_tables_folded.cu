@@ -17,9 +17,13 @@ struct FoldSmem {
   int64_t Q[5][256];                                     // M, Kd, N, in_rows, in_cols  x  level subset
   int64_t VP[256];
   uint16_t dig[256];                                     // per signature: row (0, 1, 2) of level d at bits 2d
-  // per (layer kind, signature), once per CTA: packed output states, input states and their duals (two bits per level);
-  // bit 31 of stO = invalid for the kind
+  // per (layer kind, signature), once per CTA: the level sets (fold_sets) of the output states, the input states and their
+  // duals; ok = valid for the kind
   uint32_t stO[2][256], stI[2][256], duO[2][256], duI[2][256];
+  uint8_t ok[2][256];
+  // the levels' parameters: per-thread indices into the kernel parameters (constant bank) would serialise
+  int64_t lv_alpha[8], lv_beta[8], lv_size[8];
+  uint64_t lv_magic[8];
   RecBuf rec;
 };
 
@@ -37,52 +41,45 @@ __device__ __forceinline__ bool fold_states(int kind, uint32_t dig, int D, uint3
   return valid;
 }
 
-__device__ __forceinline__ uint32_t fold_dual(uint32_t s, int D) {
+// level sets of a packed state word (two bits per level): S0 | S1 << 8 | B << 16 | P << 24
+__device__ __forceinline__ uint32_t fold_sets(uint32_t s, int D) {
   uint32_t r = 0;
-  for (int d = 0; d < D; ++d) r |= (uint32_t)dual_of(s >> (2 * d) & 3) << (2 * d);
+  for (int d = 0; d < D; ++d) r |= 1u << (8 * (s >> (2 * d) & 3) + d);
   return r;
 }
+__device__ __forceinline__ uint32_t fold_sets_dual(uint32_t m) { return (m & 0xffffu) | (m >> 8 & 0xff0000u) | (m << 8 & 0xff000000u); }   // B <-> P
 
 // forward redistribution a -> b of the layer's input tensor (R4): slice, reduce-scatter (innermost level
 // first, message = tensor before), all-to-all (innermost first, message = tensor after), all-gather (outermost first,
-// message = tensor after); Table 2 with the level's size and link parameters
-__device__ int64_t fold_walk(uint32_t a, uint32_t b, int D, const int64_t* __restrict__ Qr, const int64_t* __restrict__ Qc,
-                             int64_t eb, const MeshParams& mp) {
-  uint32_t m0 = 0, m1 = 0, mP = 0;                       // levels whose current state is S0 / S1 / P
-  for (int d = 0; d < D; ++d) {
-    int c = a >> (2 * d) & 3;
-    const int t = b >> (2 * d) & 3;
-    if (c == kB && (t == kS0 || t == kS1)) c = t;        // replicated -> split: keep the own slice, free
-    if (c == kS0) m0 |= 1u << d;
-    if (c == kS1) m1 |= 1u << d;
-    if (c == kP) mP |= 1u << d;
-  }
+// message = tensor after); Table 2 with the level's size and link parameters.  a, b: level sets
+// (fold_sets).  Which levels run which collective follows from the sets alone (a level's state only changes at its own
+// turn), so each phase visits only the levels that do something; the message sizes use the running split masks.
+__device__ int64_t fold_walk(uint32_t a, uint32_t b, const int64_t* __restrict__ Qr, const int64_t* __restrict__ Qc,
+                             int64_t eb, const FoldSmem& lv) {
+  const uint32_t tS0 = b & 255, tS1 = b >> 8 & 255, tB = b >> 16 & 255, tP = b >> 24;
+  const uint32_t aB = a >> 16 & 255;
+  uint32_t m0 = (a & 255) | (aB & tS0), m1 = (a >> 8 & 255) | (aB & tS1);      // replicated -> split: keep the own slice, free
   int64_t cost = 0;
-  for (int d = D - 1; d >= 0; --d) {                     // partial sums: reduce-scatter
-    const int t = b >> (2 * d) & 3;
-    if ((mP >> d & 1) && t != kP) {
-      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
-      if (p > 1) cost += (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-      mP &= ~(1u << d);
-      if (t == kS0) m0 |= 1u << d; else m1 |= 1u << d;   // P -> B scatters on axis 1 and gathers later
-    }
+  for (uint32_t r = (a >> 24) & ~tP; r;) {               // partial sums: reduce-scatter, innermost level first
+    const int d = 31 - __clz(r);
+    r ^= 1u << d;
+    const int64_t n = Qr[m0] * Qc[m1] * eb, p = lv.lv_size[d];
+    if (p > 1) cost += (p - 1) * (lv.lv_alpha[d] + cdiv_magic(n, (uint32_t)p, lv.lv_magic[d]) * lv.lv_beta[d]);
+    if (tS0 >> d & 1) m0 |= 1u << d; else m1 |= 1u << d;   // P -> B scatters on axis 1 and gathers later
   }
-  for (int d = D - 1; d >= 0; --d) {                     // change of split axis: all-to-all
-    const int t = b >> (2 * d) & 3;
-    const bool c0 = m0 >> d & 1, c1 = m1 >> d & 1;
-    if ((c0 && t == kS1) || (c1 && t == kS0)) {
-      m0 ^= 1u << d; m1 ^= 1u << d;
-      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
-      if (p > 1) cost += (p - 1) * mp.alpha[d] + n * mp.beta[d];
-    }
+  for (uint32_t x = (m0 & tS1) | (m1 & tS0); x;) {       // change of split axis: all-to-all, innermost first
+    const int d = 31 - __clz(x);
+    x ^= 1u << d;
+    m0 ^= 1u << d; m1 ^= 1u << d;
+    const int64_t n = Qr[m0] * Qc[m1] * eb, p = lv.lv_size[d];
+    if (p > 1) cost += (p - 1) * lv.lv_alpha[d] + n * lv.lv_beta[d];
   }
-  for (int d = 0; d < D; ++d) {                          // split -> replicated: all-gather
-    const int t = b >> (2 * d) & 3;
-    if (((m0 | m1) >> d & 1) && t == kB) {
-      m0 &= ~(1u << d); m1 &= ~(1u << d);
-      const int64_t n = Qr[m0] * Qc[m1] * eb, p = mp.size[d];
-      if (p > 1) cost += (p - 1) * (mp.alpha[d] + cdiv_magic(n, (uint32_t)p, mp.magic_size[d]) * mp.beta[d]);
-    }
+  for (uint32_t g = (m0 | m1) & tB; g;) {                // split -> replicated: all-gather, outermost first
+    const int d = __ffs(g) - 1;
+    g ^= 1u << d;
+    m0 &= ~(1u << d); m1 &= ~(1u << d);
+    const int64_t n = Qr[m0] * Qc[m1] * eb, p = lv.lv_size[d];
+    if (p > 1) cost += (p - 1) * (lv.lv_alpha[d] + cdiv_magic(n, (uint32_t)p, lv.lv_magic[d]) * lv.lv_beta[d]);
   }
   return cost;                                           // (-> P is a zero fill, free)
 }
@@ -113,10 +110,17 @@ __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const auto
     const int kind = x / K, j = x % K;
     uint32_t sI, sW, sO;
     const bool valid = fold_states(kind, sm.dig[j], D, sI, sW, sO);
-    sm.stO[kind][j] = sO | (valid ? 0u : 1u << 31);
-    sm.stI[kind][j] = sI;
-    sm.duO[kind][j] = fold_dual(sO, D);
-    sm.duI[kind][j] = fold_dual(sI, D);
+    sm.stO[kind][j] = fold_sets(sO, D);
+    sm.stI[kind][j] = fold_sets(sI, D);
+    sm.duO[kind][j] = fold_sets_dual(sm.stO[kind][j]);
+    sm.duI[kind][j] = fold_sets_dual(sm.stI[kind][j]);
+    sm.ok[kind][j] = valid;
+  }
+  if (tid < 8) {
+    sm.lv_size[tid] = tid < D ? mp.size[tid] : 1;
+    sm.lv_alpha[tid] = tid < D ? mp.alpha[tid] : 0;
+    sm.lv_beta[tid] = tid < D ? mp.beta[tid] : 0;
+    sm.lv_magic[tid] = tid < D ? mp.magic_size[tid] : 0;
   }
   const int64_t cap_layer = mp.mem_cap / L;
 
@@ -188,10 +192,9 @@ __global__ void __launch_bounds__(kFoldNT) build_tables_folded_kernel(const auto
       const int i = c / K, j = c % K;
       int64_t e = 0;
       if (l > 0) {
-        const uint32_t aO = sm.stO[rec.kind_prev][i], vj = sm.stO[rec.kind][j];
-        if (!((aO | vj) >> 31))
-          e = fold_walk(aO, sm.stI[rec.kind][j], D, sm.Q[3], sm.Q[4], rec.eb, mp) +
-              fold_walk(sm.duI[rec.kind][j], sm.duO[rec.kind_prev][i], D, sm.Q[3], sm.Q[4], rec.eb, mp);
+        if (sm.ok[rec.kind_prev][i] && sm.ok[rec.kind][j])
+          e = fold_walk(sm.stO[rec.kind_prev][i], sm.stI[rec.kind][j], sm.Q[3], sm.Q[4], rec.eb, sm) +
+              fold_walk(sm.duI[rec.kind][j], sm.duO[rec.kind_prev][i], sm.Q[3], sm.Q[4], rec.eb, sm);
       }
       out[c] = mp.accum * e + sm.VP[j];
     }
