@@ -163,10 +163,13 @@ int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int6
                            int64_t N, double* d_out, void* d_work, size_t work_bytes, void* stream);
 
 /* Whole path on DEVICE pointers, one call: (a1) -> (a2) -> (a3).  On a 2-level mesh (K = 36) with at least 296
- * chains (a1), (a2) and the first sweep of (a3) for up to 8 starts per chain run as ONE kernel, one warp per chain:
+ * chains (a1), (a2) and the first two sweeps of (a3) for up to 8 starts per chain run as ONE kernel, one warp per chain:
  * every tile is evaluated in factor form in shared memory, written to d_T with coalesced stores and consumed by the
- * chain DP and the CD sweep from shared memory, so the optimum costs no table read; the CD kernel resumes at sweep 2.
- * Other meshes run the three kernels back to back.  Results are identical to the three separate calls.
+ * chain DP and the CD sweeps from shared memory, so the optimum costs no table read; the CD kernel resumes at sweep 3.
+ * Few chains take the kernels of autoddl_chain_dp / autoddl_coord_descent (class-space or layer-parallel DP, look-up CD
+ * where they apply); kernels that do not depend on one another then run side by side on two library-owned side
+ * streams (created on first use, per host thread and device), ordered by events against `stream`: on return all work
+ * is ordered behind `stream` as if it had been launched there.  Results are identical to the three separate calls.
  * d_T: [Bp][L][K][K] output, or NULL to keep the tables in d_work (any mesh) -- with d_init == NULL
  * and K = 36 no table is materialised at all.  d_node / d_mask may be NULL.  d_init == NULL skips (a3).
  * d_work: >= autoddl_workspace_bytes(Bp, L, S, mesh). */

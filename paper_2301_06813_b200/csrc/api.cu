@@ -158,6 +158,56 @@ struct SideStream {
 };
 static thread_local SideStream g_side;
 
+// Fork / join for the few-chain paths of autoddl_search: kernels that do not depend on one another (the K x K tables a
+// caller wants, the chain DP, Coordinate Descent by look-ups) run side by side -- each of them fills only part of the
+// machine.  Two side streams and their events per host thread and device; everything is ordered by events against the
+// caller's stream: fork() after the last common producer, on(i) to launch on side stream i, join() before returning.
+struct ForkStreams {
+  int dev = -1;
+  cudaStream_t s[2] = {nullptr, nullptr};
+  cudaEvent_t forked = nullptr, done[2] = {nullptr, nullptr};
+  bool used[2] = {false, false};
+  bool ready() {
+    static const bool off = ADL_DEBUG_ENV("AUTODDL_NO_FORK");
+    if (off) return false;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cur == dev && s[0]) return true;
+    if (s[0]) {
+      for (int i = 0; i < 2; ++i) { cudaStreamDestroy(s[i]); cudaEventDestroy(done[i]); }
+      cudaEventDestroy(forked);
+      s[0] = nullptr;
+    }
+    bool ok = cudaEventCreateWithFlags(&forked, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i)
+      ok = cudaStreamCreateWithFlags(&s[i], cudaStreamNonBlocking) == cudaSuccess &&
+           cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); s[0] = nullptr; return false; }
+    dev = cur;
+    return true;
+  }
+  int fork(cudaStream_t main) {                            // what was launched on `main` so far precedes the side streams
+    used[0] = used[1] = false;
+    ADL_CUDA_CHECK(cudaEventRecord(forked, main));
+    return AUTODDL_OK;
+  }
+  int on(int i, cudaStream_t* out) {
+    if (!used[i]) { ADL_CUDA_CHECK(cudaStreamWaitEvent(s[i], forked, 0)); used[i] = true; }
+    *out = s[i];
+    return AUTODDL_OK;
+  }
+  int join(cudaStream_t main) {                            // `main` continues after the side streams' work
+    for (int i = 0; i < 2; ++i)
+      if (used[i]) {
+        ADL_CUDA_CHECK(cudaEventRecord(done[i], s[i]));
+        ADL_CUDA_CHECK(cudaStreamWaitEvent(main, done[i], 0));
+        used[i] = false;
+      }
+    return AUTODDL_OK;
+  }
+};
+static thread_local ForkStreams g_fork;
+
 int device_sm_count() {
   int dev = 0, sms = 148;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -385,17 +435,25 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     const size_t brb = lookup ? cd_lookup_workspace_bytes(mp, Bp, L) : 0;
     if (sb && d_work != nullptr && work_bytes >= tb + fbytes + sb + brb) {
       int64_t* d_F = (int64_t*)(d_work + tb);
-      if (want_T) {
-        if (!d_T) d_T = (int64_t*)d_work;
-        if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
-      }
+      if (want_T && !d_T) d_T = (int64_t*)d_work;
+      // factors first; then the tables (if wanted), the DP on the factors and the look-up CD are independent of one another
       if ((rc = launch_build_factors(d_layers, Bp, L, mp, d_F, st))) return rc;
+      const bool fork = (want_T || lookup) && g_fork.ready();
+      cudaStream_t st_tab = st, st_cd = st;
+      if (fork) {
+        if ((rc = g_fork.fork(st))) return rc;
+        if (want_T && (rc = g_fork.on(0, &st_tab))) return rc;
+        if (lookup && (rc = g_fork.on(1, &st_cd))) return rc;
+      }
+      if (want_T && (rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st_tab))) return rc;
+      if (lookup && (rc = launch_cd_lookup(d_F, Bp, L, mp, d_work + tb + fbytes + sb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy,
+                                           d_cd_sweeps, st_cd)))
+        return rc;
       if ((rc = launch_chain_dp_scan(d_F, Bp, L, mp, d_work + tb + fbytes, d_opt_cost, d_strategy, st))) return rc;
       if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
       if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
-      if (!do_cd) return AUTODDL_OK;
-      if (lookup)
-        return launch_cd_lookup(d_F, Bp, L, mp, d_work + tb + fbytes + sb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st);
+      if (fork && (rc = g_fork.join(st))) return rc;
+      if (!do_cd || lookup) return AUTODDL_OK;
       return launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st, false, true);
     }
   }
@@ -407,11 +465,23 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
   if (!d_T) d_T = (int64_t*)d_work;
   if ((rc = launch_build_tables(d_layers, Bp, L, mp, d_T, d_node, d_mask, st))) return rc;
   const bool scan_tab = chain_dp_scan_tab_supported((int32_t)K, Bp, L) && work_bytes >= tb + chain_dp_scan_tab_bytes((int32_t)K, Bp, L);
+  // small tables, few long chains, many starts: the layer-parallel DP and the look-up CD both read the tables and nothing
+  // else -- side by side, each with its own slice of the workspace
+  const size_t stb = scan_tab ? align_up(chain_dp_scan_tab_bytes((int32_t)K, Bp, L), 256) : 0;
+  const bool cd_beside = scan_tab && do_cd && !lookup && cd_lookup_tab_supported((int32_t)K, L, S) &&
+                         work_bytes >= tb + stb + cd_lookup_tab_workspace_bytes((int32_t)K, Bp, L) && g_fork.ready();
+  if (cd_beside) {
+    cudaStream_t st_cd = st;
+    if ((rc = g_fork.fork(st)) || (rc = g_fork.on(1, &st_cd))) return rc;
+    if ((rc = launch_cd_lookup_tab(d_T, Bp, L, (int32_t)K, d_work + tb + stb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st_cd)))
+      return rc;
+  }
   if (scan_tab) rc = launch_chain_dp_scan_tab(d_T, Bp, L, (int32_t)K, d_work + tb, d_opt_cost, d_strategy, st);
   else rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + tb : nullptr, d_opt_cost, d_strategy, st);
   if (rc) return rc;
   if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
   if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
+  if (cd_beside) return g_fork.join(st);
   if (!do_cd) return AUTODDL_OK;
   if (lookup) {
     const size_t off = align_up(tb + bb, 256), fbytes = factors_bytes(mp, Bp, L);
