@@ -544,6 +544,13 @@ def run_configs(args):
                                                             work=work, out=one_nt)),
             "mh_us": gpu_us(lambda: adl.metropolis(T, init, w.mesh, nsteps, tau, seed=0, out=mh), n=5),
         }
+        # the same call captured once into a CUDA graph and replayed (the small configs are launch-bound)
+        graph, gs = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(gs):
+            with torch.cuda.graph(graph, stream=gs):
+                adl.search(dl, w.mesh, w.net, init=init, max_sweeps=w.max_sweeps, work=work, out=one)
+        g["search_graph_us"] = gpu_us(graph.replay)
         line = {"config": k, "name": w.name, "Bp": w.Bp, "L": w.L, "K": w.K, "S": w.S, "cells": w.cells, "cd_sweeps": sweeps,
                 "gpu": g,
                 "gpu_rates": {"build_cells_per_s": w.cells / g["build_us"] * 1e6, "dp_cells_per_s": w.cells / g["dp_us"] * 1e6,
