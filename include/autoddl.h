@@ -170,6 +170,8 @@ int autoddl_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int6
  * where they apply); kernels that do not depend on one another then run side by side on two library-owned side
  * streams (created on first use, per host thread and device), ordered by events against `stream`: on return all work
  * is ordered behind `stream` as if it had been launched there.  Results are identical to the three separate calls.
+ * The call allocates nothing and synchronises nothing: it can be captured into a CUDA graph and replayed (make one eager
+ * call with the same shapes first: it creates the side streams and the device-wide index tables).
  * d_T: [Bp][L][K][K] output, or NULL to keep the tables in d_work (any mesh) -- with d_init == NULL
  * and K = 36 no table is materialised at all.  d_node / d_mask may be NULL.  d_init == NULL skips (a3).
  * d_work: >= autoddl_workspace_bytes(Bp, L, S, mesh). */
