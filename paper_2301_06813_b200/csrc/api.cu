@@ -476,12 +476,22 @@ static int search_device(const autoddl_layer* d_layers, int32_t Bp, int32_t L, c
     if ((rc = launch_cd_lookup_tab(d_T, Bp, L, (int32_t)K, d_work + tb + stb, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st_cd)))
       return rc;
   }
+  // few chains on larger tables: the DP (a cluster or a CTA per chain) and the gather CD (a warp per start) fill a fraction
+  // of the machine each and read the tables only (the gather kernel needs no workspace)
+  const bool gather_beside = !cd_beside && do_cd && !lookup && Bp <= 64 && !cd_lookup_tab_supported((int32_t)K, L, S) && g_fork.ready();
+  if (gather_beside) {
+    cudaStream_t st_cd = st;
+    if ((rc = g_fork.fork(st)) || (rc = g_fork.on(1, &st_cd))) return rc;
+    if ((rc = launch_coord_descent(d_T, Bp, L, K, d_init, S, max_sweeps, d_cd_cost, d_cd_strategy, d_cd_sweeps, st_cd, false,
+                                   mp.ndim <= 3 && !mp.fold)))
+      return rc;
+  }
   if (scan_tab) rc = launch_chain_dp_scan_tab(d_T, Bp, L, (int32_t)K, d_work + tb, d_opt_cost, d_strategy, st);
   else rc = launch_chain_dp(d_T, Bp, L, K, bb ? d_work + tb : nullptr, d_opt_cost, d_strategy, st);
   if (rc) return rc;
   if (g_mark) { cudaEventRecord(g_mark, st); g_mark = nullptr; }
   if (g_dp_done) { cudaEventRecord(g_dp_done, st); g_dp_done = nullptr; }
-  if (cd_beside) return g_fork.join(st);
+  if (cd_beside || gather_beside) return g_fork.join(st);
   if (!do_cd) return AUTODDL_OK;
   if (lookup) {
     const size_t off = align_up(tb + bb, 256), fbytes = factors_bytes(mp, Bp, L);
