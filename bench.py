@@ -562,6 +562,22 @@ def run_configs(args):
                 "best_random_over_dp": float(adl.metropolis(T, init, w.mesh, 0, tau, seed=0)[0].min(dim=1).values.double()
                                              .div(dp[0].double()).mean()),
                 "mh": {"nsteps": nsteps, "tau_ps": tau}}
+        if w.Bp == 1 and w.L >= 8:
+            # pipeline-stage enumeration (R27, 6.12) of the chain into 4 stages, objective max: segment optima for all
+            # O(L^2) segments, stage-transfer costs, partition DP, strategies of the chosen segments -- four kernels
+            Tn, nodeN, maskN = adl.build_tables(dl, w.mesh, w.net, want_node_mask=True)
+            torch.cuda.synchronize()
+            pipe = adl.pipeline_stages(dl[0], Tn[0], nodeN[0], maskN[0], w.mesh, w.net, 4, 1)
+            g["pipeline_us"] = gpu_us(lambda: adl.pipeline_stages(dl[0], Tn[0], nodeN[0], maskN[0], w.mesh, w.net, 4, 1), n=5)
+            line["pipeline"] = {"stages": 4, "objective": "max", "value_ps": int(pipe["value"][0]), "cuts": pipe["cuts"].tolist(),
+                                "segments": w.L * (w.L + 1) // 2}
+            if w.L * w.K * w.K <= 3_000_000:                 # the oracle's segment optima are O(L^2 K^2): bounded
+                hT, hn, hm = Tn[0].cpu().numpy(), nodeN[0].cpu().numpy(), maskN[0].cpu().numpy()
+                t0 = time.perf_counter()
+                otri = ref.segment_optima(hT, hn, hm)
+                oval, ocuts = ref.pipeline_partition(otri, ref.stage_transfer(w.layers[0], ref.mesh_of(w), ref.net_of(w)), 4, 1)
+                line["pipeline"]["oracle_1core_us"] = (time.perf_counter() - t0) * 1e6
+                assert int(oval) == line["pipeline"]["value_ps"] and [int(x) for x in ocuts] == line["pipeline"]["cuts"]
         if k == 6:                                           # the same chain on the unrestricted six-row space
             wu = cf.config6_paper_space(restricted=False)
             Tu, _, _ = adl.build_tables(dl, wu.mesh, wu.net, want_node_mask=False)

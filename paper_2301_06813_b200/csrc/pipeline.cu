@@ -18,22 +18,33 @@ namespace autoddl {
 
 namespace {
 
-constexpr int kAB = 16;                                    // starts per CTA
-
-template <int G>
+// AB starts per CTA: 16 when there are enough blocks of starts to fill the machine, else 4 (a long single chain: the tiles then
+// come from L2 more often, but four times as many SMs share the work and the longest CTA does a quarter of it)
+template <int G, int AB>
 __global__ void __launch_bounds__(1024) segment_optima_kernel(const int64_t* __restrict__ T, const int64_t* __restrict__ node,
                                                               const uint8_t* __restrict__ mask, int L, int K, int RB,
                                                               int64_t* __restrict__ tri) {
-  constexpr int NA = kAB / G;
+  constexpr int kAB = AB, NA = (AB + G - 1) / G;
   extern __shared__ __align__(16) unsigned char so_smem[];
   int64_t* F = reinterpret_cast<int64_t*>(so_smem);        // [2][kAB][K]
-  int64_t* stage = F + 2 * kAB * K;                        // [RB][K]
+  int64_t* stage = F + 2 * kAB * K;                        // [2][RB][K]: row blocks of the tiles, double buffered (cp.async)
   const int tid = threadIdx.x, nthr = blockDim.x;
   const int j = tid % K, g = tid / K;                      // threads beyond G * K only help with the copies
   const bool worker = g < G;
   const int a0 = blockIdx.x * kAB;
   const int na = L - a0 < kAB ? L - a0 : kAB;              // starts of this block
   for (int x = tid; x < na * (L + 1); x += nthr) tri[(size_t)a0 * (L + 1) + x] = -1;
+  // rows r0 .. of tile l -> stage buffer `buf`, asynchronously (8 bytes per request: tiles of an odd K are only 8-byte aligned)
+  auto issue = [&](int l, int r0, int buf) {
+    const int nr = K - r0 < RB ? K - r0 : RB;
+    const int64_t* src = T + (size_t)l * K * K + (size_t)r0 * K;
+    int64_t* dst = stage + (size_t)buf * RB * K;
+    for (int x = tid; x < nr * K; x += nthr)
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst + x)), "l"(src + x) : "memory");
+  };
+  int buf = 0;
+  if (a0 + 1 < L) issue(a0 + 1, 0, 0);                     // the first tile any start of the block consumes
+  asm volatile("cp.async.commit_group;" ::: "memory");
   __syncthreads();
   int cur = 0;
   for (int l = a0; l < L; ++l) {
@@ -44,14 +55,18 @@ __global__ void __launch_bounds__(1024) segment_optima_kernel(const int64_t* __r
     for (int t = 0; t < NA; ++t) acc[t] = INT64_MAX;
     const int nact = l - a0 < na ? l - a0 : na;            // starts a < l of this block: they consume tile l
     if (nact > 0) {
-      const int64_t* tile = T + (size_t)l * K * K;
       for (int r0 = 0; r0 < K; r0 += RB) {
         const int nr = K - r0 < RB ? K - r0 : RB;
-        for (int x = tid; x < nr * K; x += nthr) stage[x] = tile[(size_t)r0 * K + x];
+        // the next row block (of this tile, or the first of the next tile) travels while this one is consumed
+        if (r0 + RB < K) issue(l, r0 + RB, buf ^ 1);
+        else if (l + 1 < L) issue(l + 1, 0, buf ^ 1);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncthreads();
+        const int64_t* stg = stage + (size_t)buf * RB * K;
         if (worker) {
           for (int r = 0; r < nr; ++r) {
-            const int64_t tv = stage[r * K + j];
+            const int64_t tv = stg[r * K + j];
 #pragma unroll
             for (int t = 0; t < NA; ++t) {
               const int ai = g + G * t;
@@ -62,7 +77,8 @@ __global__ void __launch_bounds__(1024) segment_optima_kernel(const int64_t* __r
             }
           }
         }
-        __syncthreads();
+        __syncthreads();                                   // the buffer is free for the copy issued in the next round
+        buf ^= 1;
       }
     }
     if (worker) {
@@ -138,34 +154,43 @@ __global__ void __launch_bounds__(1024) partition_kernel(const int64_t* __restri
   }
 }
 
-// one CTA per stage: chain DP of the segment [cuts[k], cuts[k + 1]) with byte back-pointers in the workspace
-__global__ void __launch_bounds__(256) segment_strategies_kernel(const int64_t* __restrict__ T, const int64_t* __restrict__ node,
-                                                                 const uint8_t* __restrict__ mask, int L, int K,
-                                                                 const int32_t* __restrict__ cuts, uint8_t* __restrict__ bp,
-                                                                 int64_t* __restrict__ seg_cost, int32_t* __restrict__ strategy) {
+// one CTA per stage: chain DP of the segment [cuts[k], cuts[k + 1]) with byte back-pointers in the workspace; thread
+// (j, part) scans every fourth row i of column j (increasing i, strict '<': its smallest i), the parts merge by shuffles
+__global__ void __launch_bounds__(1024) segment_strategies_kernel(const int64_t* __restrict__ T, const int64_t* __restrict__ node,
+                                                                  const uint8_t* __restrict__ mask, int L, int K,
+                                                                  const int32_t* __restrict__ cuts, uint8_t* __restrict__ bp,
+                                                                  int64_t* __restrict__ seg_cost, int32_t* __restrict__ strategy) {
+  constexpr int PARTS = 4;
   __shared__ int64_t f[2][256];
-  const int k = blockIdx.x, j = threadIdx.x;
+  const int k = blockIdx.x, tid = threadIdx.x, j = tid / PARTS, part = tid % PARTS;
   const int a = cuts[k], b = cuts[k + 1];
   if (a < 0 || b > L || a >= b) return;
   int cur = 0;
-  if (j < K) f[0][j] = node[(size_t)a * K + j] + (mask[(size_t)a * K + j] ? 0 : AUTODDL_PEN);
+  if (tid < K) f[0][tid] = node[(size_t)a * K + tid] + (mask[(size_t)a * K + tid] ? 0 : AUTODDL_PEN);
   __syncthreads();
   for (int l = a + 1; l < b; ++l) {
-    if (j < K) {
-      const int64_t* tile = T + (size_t)l * K * K;
-      int64_t best = f[cur][0] + tile[j];
-      int ar = 0;
-      for (int i = 1; i < K; ++i) {
-        const int64_t v = f[cur][i] + tile[(size_t)i * K + j];
+    const int64_t* col = T + (size_t)l * K * K + (j < K ? j : 0);
+    int64_t best = INT64_MAX;
+    int ar = 1 << 30;
+    if (j < K)
+      for (int i = part; i < K; i += PARTS) {
+        const int64_t v = f[cur][i] + __ldg(col + (size_t)i * K);
         if (v < best) { best = v; ar = i; }
       }
+#pragma unroll
+    for (int off = 1; off < PARTS; off <<= 1) {            // (every lane of the warp takes part)
+      const int64_t ov = __shfl_xor_sync(0xffffffffu, best, off);
+      const int oa = __shfl_xor_sync(0xffffffffu, ar, off);
+      if (ov < best || (ov == best && oa < ar)) { best = ov; ar = oa; }
+    }
+    if (j < K && part == 0) {
       f[cur ^ 1][j] = best;
       bp[(size_t)l * K + j] = (uint8_t)ar;
     }
     __syncthreads();
     cur ^= 1;
   }
-  if (j == 0) {
+  if (tid == 0) {
     int js = 0;
     for (int c = 1; c < K; ++c)
       if (f[cur][c] < f[cur][js]) js = c;
@@ -179,21 +204,25 @@ __global__ void __launch_bounds__(256) segment_strategies_kernel(const int64_t* 
 
 int launch_segment_optima(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, int32_t K,
                           int64_t* d_tri, cudaStream_t st) {
-  const int G = K <= 64 ? 16 : 4;
+  // large tiles of one long chain: 4 starts per CTA (measured: K = 216, L = 480 29 -> 18 ms; small tiles are better off with 16)
+  const int AB = K > 64 && (L + 15) / 16 * 2 < device_sm_count() ? 4 : 16;
+  const int G = AB == 16 && K <= 64 ? 16 : 4;              // thread groups over the starts of a block
   int threads = (K * G + 31) / 32 * 32;
   if (threads > 1024) threads = 1024;                      // K = 256, G = 4: exactly 1024
-  int RB = (int)((96 * 1024) / ((size_t)K * 8));
+  int RB = (int)((92 * 1024) / ((size_t)K * 8));            // rows per stage buffer (two buffers)
   if (RB > K) RB = K;
   if (RB < 1) RB = 1;
-  const size_t smem = ((size_t)2 * kAB * K + (size_t)RB * K) * 8;
-  const int grid = (L + kAB - 1) / kAB;
-  if (G == 16) {
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(segment_optima_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    segment_optima_kernel<16><<<grid, threads, smem, st>>>(d_T, d_node, d_mask, L, K, RB, d_tri);
-  } else {
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(segment_optima_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    segment_optima_kernel<4><<<grid, threads, smem, st>>>(d_T, d_node, d_mask, L, K, RB, d_tri);
-  }
+  const size_t smem = ((size_t)2 * AB * K + (size_t)2 * RB * K) * 8;
+  const int grid = (L + AB - 1) / AB;
+  auto go = [&](auto kern) -> int {
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, threads, smem, st>>>(d_T, d_node, d_mask, L, K, RB, d_tri);
+    return AUTODDL_OK;
+  };
+  int rc;
+  if (AB == 4) rc = go(segment_optima_kernel<4, 4>);
+  else rc = G == 16 ? go(segment_optima_kernel<16, 16>) : go(segment_optima_kernel<4, 16>);
+  if (rc) return rc;
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -224,7 +253,7 @@ int launch_partition(const int64_t* d_tri, const int64_t* d_xfer, int32_t L, int
 int launch_segment_strategies(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, int32_t K,
                               const int32_t* d_cuts, int32_t stages, uint8_t* d_bp, int64_t* d_seg_cost, int32_t* d_strategy,
                               cudaStream_t st) {
-  segment_strategies_kernel<<<stages, 256, 0, st>>>(d_T, d_node, d_mask, L, K, d_cuts, d_bp, d_seg_cost, d_strategy);
+  segment_strategies_kernel<<<stages, (K * 4 + 31) / 32 * 32, 0, st>>>(d_T, d_node, d_mask, L, K, d_cuts, d_bp, d_seg_cost, d_strategy);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
