@@ -596,6 +596,25 @@ def run_configs(args):
                                     "cd_sweeps_per_s": int(osw.sum()) / (t3 - t2),
                                     "mh_proposals_per_s": w.Bp * w.S * ms / (t4 - t3), "cores": 1}
         print(json.dumps(line))
+    # alpha-beta calibration (R23): least squares over N timed collectives, GPU kernel and oracle
+    import numpy as np
+    N = 1 << 20
+    rng = np.random.default_rng(0)
+    kind = rng.integers(0, 4, N).astype(np.int32)
+    pp = rng.choice([2, 4, 8, 16], N).astype(np.int32)
+    nb = (2 ** rng.uniform(10, 28, N)).astype(np.int64)
+    tt = ref.fit_design_matrix(kind, pp, nb) @ np.array([5e-6, 4e-11]) * (1 + 0.01 * rng.standard_normal(N))
+    dev = [torch.from_numpy(x).cuda() for x in (kind, pp, nb, tt)]
+    got = adl.fit_alpha_beta(*dev)
+    fit_us = gpu_us(lambda: adl.fit_alpha_beta(*dev, out=got))
+    t0 = time.perf_counter()
+    want = ref.fit_alpha_beta(kind, pp, nb, tt)
+    oracle_us = (time.perf_counter() - t0) * 1e6
+    g = got.cpu().numpy()
+    print(json.dumps({"fit_alpha_beta": {"samples": N, "gpu_us": fit_us, "oracle_1core_us": oracle_us, "alpha_s": float(g[0]),
+                                         "beta_s_per_byte": float(g[1]),
+                                         "rel_diff_to_oracle": [abs(float(g[0] / want[0]) - 1), abs(float(g[1] / want[1]) - 1)],
+                                         "hbm_GBps": N * 24 / (fit_us * 1e-6) / 1e9}}))
     return 0
 
 

@@ -62,8 +62,16 @@ fit_sum_kernel(const int32_t* __restrict__ kind, const int32_t* __restrict__ p, 
                const double* __restrict__ t, int64_t N, const double* __restrict__ maxpart, int nmax,
                double* __restrict__ sums) {
   __shared__ double sh[5][FIT_BLOCK / 32];
+  // the scales: max over the blocks' maxima, found by the whole block (max is exact: any order gives the same value)
   double ma = 0.0, mb = 0.0;
-  for (int k = 0; k < nmax; ++k) { ma = fmax(ma, maxpart[2 * k]); mb = fmax(mb, maxpart[2 * k + 1]); }
+  for (int k = threadIdx.x; k < nmax; k += FIT_BLOCK) { ma = fmax(ma, maxpart[2 * k]); mb = fmax(mb, maxpart[2 * k + 1]); }
+  ma = warp_max(ma);
+  mb = warp_max(mb);
+  if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = ma; sh[1][threadIdx.x >> 5] = mb; }
+  __syncthreads();
+  ma = mb = 0.0;
+  for (int w = 0; w < FIT_BLOCK / 32; ++w) { ma = fmax(ma, sh[0][w]); mb = fmax(mb, sh[1][w]); }
+  __syncthreads();                                         // sh is reused for the sums below
   const double ia = ma > 0.0 ? 1.0 / ma : 0.0, ib = mb > 0.0 ? 1.0 / mb : 0.0;
   double s[5] = {0, 0, 0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * FIT_BLOCK + threadIdx.x; i < N; i += (int64_t)gridDim.x * FIT_BLOCK) {
@@ -87,15 +95,30 @@ fit_sum_kernel(const int32_t* __restrict__ kind, const int32_t* __restrict__ p, 
   }
 }
 
-// pass 3: one thread adds the block sums in order, solves the 2 x 2 normal equations, unscales.  out = {alpha, beta}
-__global__ void fit_solve_kernel(const double* __restrict__ maxpart, const double* __restrict__ sums, int nblocks,
-                                 double* __restrict__ out) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+// pass 3: one block adds the block sums in a fixed order (thread k takes blocks k, k + 256, ..; then a fixed tree), solves the
+// 2 x 2 normal equations, unscales.  out = {alpha, beta}
+__global__ void __launch_bounds__(FIT_BLOCK) fit_solve_kernel(const double* __restrict__ maxpart, const double* __restrict__ sums,
+                                                              int nblocks, double* __restrict__ out) {
+  __shared__ double sh[7][FIT_BLOCK / 32];
+  double v[7] = {0, 0, 0, 0, 0, 0, 0};                     // ma, mb, five sums
+  for (int k = threadIdx.x; k < nblocks; k += FIT_BLOCK) {
+    v[0] = fmax(v[0], maxpart[2 * k]);
+    v[1] = fmax(v[1], maxpart[2 * k + 1]);
+    for (int q = 0; q < 5; ++q) v[2 + q] += sums[5 * k + q];
+  }
+  v[0] = warp_max(v[0]);
+  v[1] = warp_max(v[1]);
+#pragma unroll
+  for (int q = 2; q < 7; ++q) v[q] = warp_sum(v[q]);
+  if ((threadIdx.x & 31) == 0)
+    for (int q = 0; q < 7; ++q) sh[q][threadIdx.x >> 5] = v[q];
+  __syncthreads();
+  if (threadIdx.x != 0) return;
   double ma = 0.0, mb = 0.0, s[5] = {0, 0, 0, 0, 0};
-  for (int k = 0; k < nblocks; ++k) {
-    ma = fmax(ma, maxpart[2 * k]);
-    mb = fmax(mb, maxpart[2 * k + 1]);
-    for (int q = 0; q < 5; ++q) s[q] += sums[5 * k + q];
+  for (int w = 0; w < FIT_BLOCK / 32; ++w) {
+    ma = fmax(ma, sh[0][w]);
+    mb = fmax(mb, sh[1][w]);
+    for (int q = 0; q < 5; ++q) s[q] += sh[2 + q][w];
   }
   const double det = s[0] * s[2] - s[1] * s[1];
   double a = 0.0, b = 0.0;
@@ -119,7 +142,7 @@ int launch_fit_alpha_beta(const int32_t* d_kind, const int32_t* d_p, const int64
   double* sums = d_work + 2 * FIT_GRID_MAX;
   fit_max_kernel<<<grid, FIT_BLOCK, 0, st>>>(d_kind, d_p, d_bytes, N, maxpart);
   fit_sum_kernel<<<grid, FIT_BLOCK, 0, st>>>(d_kind, d_p, d_bytes, d_time, N, maxpart, grid, sums);
-  fit_solve_kernel<<<1, 32, 0, st>>>(maxpart, sums, grid, d_out);
+  fit_solve_kernel<<<1, FIT_BLOCK, 0, st>>>(maxpart, sums, grid, d_out);
   count_launch(3);
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
