@@ -15,7 +15,20 @@ namespace autoddl {
 
 namespace {
 
+// smallest (value, index) over the warp.  Fast path when every lane holds a value in [0, 2^55) and an index below 256: the
+// key value * 256 + index is reduced as two 32-bit halves with redux.sync (the low half only among the lanes that hold the
+// smallest high half); otherwise the shuffle butterfly.  Both are exact.
 __device__ __forceinline__ void warp_argmin(int64_t& bv, int& bi) {
+  if (__all_sync(0xffffffffu, (uint64_t)bv < (1ull << 55) && (unsigned)bi < 256u)) {
+    const uint64_t key = ((uint64_t)bv << 8) | (uint32_t)bi;
+    const uint32_t hi = (uint32_t)(key >> 32), lo = (uint32_t)key;
+    const uint32_t mh = __reduce_min_sync(0xffffffffu, hi);
+    const uint32_t ml = __reduce_min_sync(0xffffffffu, hi == mh ? lo : 0xffffffffu);
+    const uint64_t m = ((uint64_t)mh << 32) | ml;
+    bv = (int64_t)(m >> 8);
+    bi = (int)(m & 255);
+    return;
+  }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
     const int64_t ov = __shfl_xor_sync(0xffffffffu, bv, off);
@@ -110,10 +123,13 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   // later layer is then dropped.  (Reading the next row speculatively as well was measured and costs more than it
   // saves, on the batched config and with one model and many starts alike: 191 -> 211 us on config 3, 1,328 -> 1,486 us
   // on config 5.)
-  auto next_dirty = [&](int from) {
-    int l = from;
-    while (l < L && !dirty[l]) ++l;
-    return l;
+  auto next_dirty = [&](int from) {                        // 32 flags per step: lane i looks at layer base + i
+    for (int base = from & ~31; base < L; base += 32) {
+      const int l = base + lane;
+      const unsigned m = __ballot_sync(0xffffffffu, l >= from && l < L && dirty[l]);
+      if (m) return base + __ffs(m) - 1;
+    }
+    return L;
   };
   auto load_row = [&](int l, int64_t (&rv)[NCAND]) {
     const int64_t* row = Tp + ((size_t)l * K + (l > 0 ? s[l - 1] : 0)) * K;
