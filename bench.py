@@ -412,7 +412,7 @@ def run_ours(args):
         fused_hbm = table_bytes + Bp * L * 64
         fused_work = table_bytes + dp_bytes + sweep1_bytes
         kernels = {
-            "build_dp_cd1_fused": {"ms": ms["fused"], "cells_per_s": cells / (ms["fused"] * 1e-3),
+            "build_dp_cd2_fused": {"ms": ms["fused"], "cells_per_s": cells / (ms["fused"] * 1e-3),
                                    "hbm_GBps": fused_hbm / (ms["fused"] * 1e-3) / 1e9,
                                    "work_units_GBps": fused_work / (ms["fused"] * 1e-3) / 1e9, "in_step": True,
                                    "bound": "LSU data pipe (shared-memory loads + the global stores: ncu 81 %) / issue (67 %); hbm traffic "
@@ -437,8 +437,8 @@ def run_ours(args):
         }
         for k in kernels.values():
             k["frac_of_peak"] = k["hbm_GBps"] / peak
-        kernels["build_dp_cd1_fused"]["work_units_frac_of_peak"] = kernels["build_dp_cd1_fused"]["work_units_GBps"] / peak
-        dom = max(("build_dp_cd1_fused", "coord_descent_resume"), key=lambda n: kernels[n]["ms"])
+        kernels["build_dp_cd2_fused"]["work_units_frac_of_peak"] = kernels["build_dp_cd2_fused"]["work_units_GBps"] / peak
+        dom = max(("build_dp_cd2_fused", "coord_descent_resume"), key=lambda n: kernels[n]["ms"])
         traffic, traffic_src = None, None
         tpath = os.path.join(ROOT, "profiles", "traffic_r2.csv")       # per-launch DRAM bytes from a committed ncu --set full capture
         if os.path.exists(tpath):
@@ -462,13 +462,13 @@ def run_ours(args):
                                         "scaling_mode": args.scaling}),
             "parts": {"build_cells_per_s": world * kernels["build_tables"]["cells_per_s"],
                       "dp_cells_per_s": world * kernels["chain_dp"]["cells_per_s"],
-                      "fused_build_dp_cd1_cells_per_s": world * kernels["build_dp_cd1_fused"]["cells_per_s"],
+                      "fused_build_dp_cd2_cells_per_s": world * kernels["build_dp_cd2_fused"]["cells_per_s"],
                       "cd_sweeps_per_s": world * kernels["coord_descent"]["sweeps_per_s"]},
             "kernels": kernels,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["hbm_GBps"], "peak": peak, "unit": "GB/s",
                          "frac": kernels[dom]["hbm_GBps"] / peak, "traffic": traffic, "traffic_source": traffic_src,
                          "peak_source": peak_src, "copy_probe_GBps_same_run": copy_gbs,
-                         "bytes_per_launch": fused_hbm if dom == "build_dp_cd1_fused" else cd_alg_bytes - sweep1_bytes,
+                         "bytes_per_launch": fused_hbm if dom == "build_dp_cd2_fused" else cd_alg_bytes - sweep1_bytes,
                          "work_units_frac": kernels[dom].get("work_units_frac_of_peak"),
                          "note": "frac = bytes that must reach HBM per launch (8 B per cell written + 64 B per layer record read) / "
                                  "CUDA-event launch time / peak; work_units_frac counts SURVEY 8(d)'s per-unit bytes for all the work "
