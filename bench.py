@@ -445,7 +445,7 @@ def run_ours(args):
             try:
                 rows = dict(l.strip().split(",")[:2] for l in open(tpath).read().splitlines()[1:] if l.strip())
                 traffic = float(rows[dom]) if dom in rows else None
-                traffic_src = "profiles/traffic_r2.csv (committed ncu --set full capture of the same command, NOT measured in this run)"
+                traffic_src = "profiles/traffic_r2.csv (committed ncu capture of the same command: dram__bytes_read.sum + dram__bytes_write.sum per launch; NOT measured in this run)"
                 for name, k in kernels.items():
                     if name in rows:
                         k["dram_bytes_per_launch_ncu"] = float(rows[name])
