@@ -369,6 +369,17 @@ def run_ours(args):
             best_ms = min(best_ms, s0.elapsed_time(s1))
     copy_gbs = 2 * nb / (best_ms * 1e-3) / 1e9
     del a, b
+    # ---- the ceiling of the fused kernel's WRITE PATTERN: a store-only kernel with its addresses (one warp per chain, tile
+    # after tile, 16-byte streaming stores), same run, same buffer; average of back-to-back launches like the step itself
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        adl.store_probe(T)
+    s0.record()
+    for _ in range(20):
+        adl.store_probe(T)
+    s1.record(); torch.cuda.synchronize()
+    store_ms = s0.elapsed_time(s1) / 20
+    store_gbs = w.cells * 8 / (store_ms * 1e-3) / 1e9
 
     # ---- end to end through the host-pointer C-ABI call (pinned host buffers, H2D + D2H timed) -----------
     pinned = adl.alloc_host_outputs(Bp, L, S)
@@ -468,11 +479,15 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["hbm_GBps"], "peak": peak, "unit": "GB/s",
                          "frac": kernels[dom]["hbm_GBps"] / peak, "traffic": traffic, "traffic_source": traffic_src,
                          "peak_source": peak_src, "copy_probe_GBps_same_run": copy_gbs,
+                         "store_pattern_probe_GBps_same_run": store_gbs, "store_pattern_probe_ms": store_ms,
+                         "frac_of_store_pattern_probe": (store_ms / kernels[dom]["ms"]) if dom == "build_dp_cd2_fused" else None,
                          "bytes_per_launch": fused_hbm if dom == "build_dp_cd2_fused" else cd_alg_bytes - sweep1_bytes,
                          "work_units_frac": kernels[dom].get("work_units_frac_of_peak"),
                          "note": "frac = bytes that must reach HBM per launch (8 B per cell written + 64 B per layer record read) / "
                                  "CUDA-event launch time / peak; work_units_frac counts SURVEY 8(d)'s per-unit bytes for all the work "
-                                 "the fused launch does (tables + DP + two CD sweeps) and can exceed 1"},
+                                 "the fused launch does (tables + DP + two CD sweeps) and can exceed 1; store_pattern_probe = a store-only "
+                                 "kernel with the fused kernel's write addresses (autoddl_store_probe), timed in this run: "
+                                 "frac_of_store_pattern_probe = its time / the fused kernel's time"},
             "e2e": {"value": world * cells / (e2e_ms * 1e-3), "unit": "cells/s", "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": launches,

@@ -254,6 +254,12 @@ int autoddl_segment_strategies(const int64_t* d_T, const int64_t* d_node, const 
  * copy bandwidth in the same run as the kernels above.  bytes must be a multiple of 16. */
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream);
 
+/* Store-only probe with the address pattern of the fused table writer of autoddl_search: one warp per chain writes the
+ * chain's L tiles of K x K int64 cells in order with 16-byte streaming stores (no arithmetic; the cells are overwritten
+ * with filler).  bench.py times it in the same run: the ceiling of that write pattern, next to the copy bandwidth.
+ * d_T: [Bp][L][K][K] int64 device buffer, 16-byte aligned; K * K even. */
+int autoddl_store_probe(int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* stream);
+
 /* Profiling hook (used by bench.py for the per-kernel split of the one-call path): the next autoddl_search /
  * autoddl_search_host call of this thread records `cuda_event` (a cudaEvent_t, NULL to cancel) on its stream after
  * the tables + chain DP and before Coordinate Descent.  One shot. */

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libautoddl.so")
 EXPORTS = [
     "autoddl_num_signatures", "autoddl_workspace_bytes", "autoddl_build_tables", "autoddl_chain_dp",
     "autoddl_chain_dp_static", "autoddl_chain_dp_static_bytes", "autoddl_coord_descent", "autoddl_metropolis", "autoddl_search", "autoddl_search_host", "autoddl_fit_workspace_bytes", "autoddl_fit_alpha_beta", "autoddl_best_of_starts", "autoddl_pipeline_workspace_bytes", "autoddl_segment_optima", "autoddl_stage_transfer",
-    "autoddl_pipeline_partition", "autoddl_segment_strategies", "autoddl_copy_probe", "autoddl_profile_mark", "autoddl_launch_count",
+    "autoddl_pipeline_partition", "autoddl_segment_strategies", "autoddl_copy_probe", "autoddl_store_probe", "autoddl_profile_mark", "autoddl_launch_count",
     "autoddl_last_error",
 ]
 
@@ -82,6 +82,8 @@ def lib():
         L.autoddl_pipeline_partition.argtypes = [vp, vp, i32, i32, i32, vp, sz, vp, vp, vp]
         L.autoddl_segment_strategies.restype = C.c_int
         L.autoddl_segment_strategies.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, sz, vp, vp, vp]
+        L.autoddl_store_probe.restype = C.c_int
+        L.autoddl_store_probe.argtypes = [vp, i32, i32, i32, vp]
         L.autoddl_copy_probe.restype = C.c_int
         L.autoddl_copy_probe.argtypes = [vp, vp, sz, vp]
         L.autoddl_fit_workspace_bytes.restype = sz
@@ -390,6 +392,12 @@ def alloc_host_outputs(Bp: int, L: int, S: int, pin: bool = True):
         "cd_cost": mk((Bp, max(S, 1)), torch.int64), "cd_strategy": mk((Bp, max(S, 1), L), torch.int32),
         "cd_sweeps": mk((Bp, max(S, 1)), torch.int32),
     }
+
+
+def store_probe(T: torch.Tensor):
+    """store-only kernel with the fused table writer's address pattern over T [Bp, L, K, K] int64 (overwrites it)"""
+    Bp, L, K = T.shape[0], T.shape[1], T.shape[2]
+    _check(lib().autoddl_store_probe(_ptr(T, I64, "T"), Bp, L, K, _stream()))
 
 
 def copy_probe(src: torch.Tensor, dst: torch.Tensor):

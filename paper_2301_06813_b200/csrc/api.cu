@@ -732,6 +732,15 @@ int autoddl_segment_strategies(const int64_t* d_T, const int64_t* d_node, const 
                                    (cudaStream_t)stream);
 }
 
+int autoddl_store_probe(int64_t* d_T, int32_t Bp, int32_t L, int32_t K, void* stream) {
+  clear_error();
+  ADL_REQUIRE(d_T != nullptr && Bp >= 1 && L >= 1 && K >= 1 && K <= 256 && (K * K) % 2 == 0, "store_probe: bad arguments");
+  ADL_REQUIRE(((uintptr_t)d_T & 15) == 0, "store_probe: misaligned");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_store_probe(d_T, Bp, L, K * K, (cudaStream_t)stream);
+}
+
 int autoddl_copy_probe(const void* d_src, void* d_dst, size_t bytes, void* stream) {
   clear_error();
   ADL_REQUIRE(d_src && d_dst && bytes > 0 && bytes % 16 == 0, "copy_probe: bad arguments");

@@ -131,6 +131,7 @@ int launch_partition(const int64_t* d_tri, const int64_t* d_xfer, int32_t L, int
 int launch_segment_strategies(const int64_t* d_T, const int64_t* d_node, const uint8_t* d_mask, int32_t L, int32_t K,
                               const int32_t* d_cuts, int32_t stages, uint8_t* d_bp, int64_t* d_seg_cost, int32_t* d_strategy,
                               cudaStream_t st);
+int launch_store_probe(int64_t* d_T, int32_t Bp, int32_t L, int32_t cells, cudaStream_t st);
 int device_sm_count();                                     // multiprocessors of the current device (148 if the query fails)
 
 // ---- device helpers ------------------------------------------------------------------------------------

@@ -21,7 +21,28 @@ __global__ void __launch_bounds__(256) copy_probe_kernel(const int4* __restrict_
     if (base + u * 256 < n) dst[base + u * 256] = v[u];
 }
 
+// Store-only probe with the ADDRESS PATTERN of the fused table writer (fused_chain.cu): one warp per chain walks the chain's
+// tiles in order and writes each tile (cells int64, a multiple of 2) with 16-byte streaming stores, 512 contiguous bytes per
+// warp instruction; one CTA of 28 warps per SM.  No arithmetic: what it reaches is the ceiling of that write pattern.
+__global__ void __launch_bounds__(896, 1) store_probe_kernel(int64_t* __restrict__ T, int Bp, int L, int cells) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+  for (int p = warp * gridDim.x + blockIdx.x; p < Bp; p += gridDim.x * W)
+    for (int l = 0; l < L; ++l) {
+      longlong2* o = reinterpret_cast<longlong2*>(T + ((size_t)p * L + l) * cells);
+      const longlong2 v = make_longlong2(p, l);
+      for (int x = lane; x < cells / 2; x += 32) __stcs(o + x, v);
+    }
+}
+
 }  // namespace
+
+int launch_store_probe(int64_t* d_T, int32_t Bp, int32_t L, int32_t cells, cudaStream_t st) {
+  const int sms = device_sm_count();
+  store_probe_kernel<<<Bp < sms ? Bp : sms, 896, 0, st>>>(d_T, Bp, L, cells);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
 
 int launch_copy_probe(const void* src, void* dst, size_t bytes, cudaStream_t st) {
   const size_t n = bytes / 16;

@@ -89,3 +89,19 @@ def test_three_steps_and_one_call_raw():
         torch.cuda.synchronize()
         for k in ("T", "node", "mask", "dc", "ds", "cc", "cs", "sw"):
             assert np.array_equal(got[k].cpu().numpy(), want[k]), (w.name, "search", k)
+
+
+def test_store_probe_covers_every_cell():
+    """autoddl_store_probe (bench.py's write-pattern ceiling): every cell of [Bp][L][K][K] is written, nothing beyond it"""
+    import torch
+    from paper_2301_06813_b200 import binding as adl
+    adl.lib()
+    Bp, L, K = 301, 5, 36
+    buf = torch.full((Bp * L * K * K + 64,), -7, dtype=torch.int64, device="cuda")
+    T = buf[:Bp * L * K * K].view(Bp, L, K, K)
+    adl.store_probe(T)
+    torch.cuda.synchronize()
+    cells = T.view(Bp, L, K * K // 2, 2)
+    assert torch.equal(cells[..., 0], torch.arange(Bp, device="cuda").view(Bp, 1, 1).expand(Bp, L, K * K // 2))
+    assert torch.equal(cells[..., 1], torch.arange(L, device="cuda").view(1, L, 1).expand(Bp, L, K * K // 2))
+    assert bool((buf[Bp * L * K * K:] == -7).all())
