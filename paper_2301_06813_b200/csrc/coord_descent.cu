@@ -213,6 +213,185 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
   }
 }
 
+// Few starts (at most kWaveMaxBlocks blocks): the SWEEPS of one start run side by side.  Update (k, l) -- sweep k, layer l --
+// reads s_{l-1} as sweep k left it and s_{l+1} as sweep k-1 left it, so sweep k may follow sweep k-1 two layers behind: warp w
+// of the block runs sweeps w+1, w+1+W, ... on the one state array in shared memory.  That is the plain loop nest in another
+// order: every update sees the operands it sees there, so trajectory, result and sweep count are the sequential algorithm's.
+// The state of a layer is ONE word -- the sweep that visited it last << 16 | whether that visit changed it << 15 | s_l --
+// so the word a follower waits for (layer l+1 tagged k-1) carries the operand itself and the leading sweep never fences.
+// A layer is re-evaluated in sweep k only if s_{l-1} changed in sweep k or s_{l+1} in sweep k-1: the dirty rule above.  The
+// first sweep that changes nothing ends the descent (stop); sweeps already under way behind it are no-ops by then.
+constexpr int kWaveWarps = 8;
+constexpr int kWaveWideBlocks = 296;                       // up to two starts per SM: eight sweeps of a start in flight, else four
+constexpr int kWaveMaxBlocks = 2048;                       // beyond: one warp per start (coord_descent_kernel) fills the machine
+template <int KT, bool SBPROWS>
+__global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int W, const int64_t* __restrict__ T, int Krt, int L, int S,
+                                                                            const int32_t* __restrict__ init, int max_sweeps,
+                                                                            int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
+                                                                            int32_t* __restrict__ sweeps) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  volatile uint32_t* st = reinterpret_cast<uint32_t*>(smem);          // [L] tag << 16 | changed << 15 | s_l
+  int* stop = reinterpret_cast<int*>(smem) + L;                       // first sweep that changed nothing
+
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const size_t ps = blockIdx.x;
+  const size_t p = ps / S;
+  const int K = KT ? KT : Krt;
+  const int64_t* Tp = T + p * (size_t)L * K * K;
+  constexpr int NCAND = KT ? (KT + 31) / 32 : 8;
+  int rep[NCAND];                                          // row that holds candidate c's column value
+#pragma unroll
+  for (int q = 0; q < NCAND; ++q) {
+    const int c = 32 * q + lane;
+    int r = 0, pw = 1, x = c;
+    if (SBPROWS) {
+      for (int d = 0; d < 3 && pw < K; ++d) {
+        const int dig = x % 6;
+        x /= 6;
+        r += (dig < 4 ? dig : 2) * pw;
+        pw *= 6;
+      }
+    } else {
+      r = c;
+    }
+    rep[q] = r;
+  }
+  for (int l = threadIdx.x; l < L; l += blockDim.x) st[l] = (uint32_t)init[ps * L + l] & 255u;      // tag 0
+  if (threadIdx.x == 0) *stop = INT32_MAX;
+  __syncthreads();
+  if (max_sweeps < 1) max_sweeps = 1;
+
+  auto load_col = [&](int l, int sr, int64_t (&cv)[NCAND]) {          // T[l+1][.][sr], sr = s_{l+1}
+    const bool has_right = l < L - 1;
+    const int64_t* col = Tp + (size_t)(l + 1) * K * K + sr;
+#pragma unroll
+    for (int q = 0; q < NCAND; ++q) {
+      const int c = 32 * q + lane;
+      cv[q] = (has_right && c < K) ? ldg_narrow(col + (size_t)rep[q] * K) : 0;
+    }
+  };
+  for (int k = w + 1; k <= max_sweeps; k += W) {
+    if (k > *reinterpret_cast<volatile int*>(stop)) break;
+    const uint32_t tagp = (uint32_t)(k - 1) << 16;           // words tagged k-1 (or later: never) are sweep k-1's
+    bool changed = false, live = true;
+    uint32_t left = 0;                                      // this sweep's word of layer l-1
+    // The column of layer l+1 is known as soon as sweep k-1 has left layer l+2: it is gathered one layer ahead when the layer
+    // is known to be dirty (sweep 1, or its right neighbour changed in sweep k-1), so that only the contiguous row read
+    // stays on the dependent chain.
+    int64_t cvp[NCAND];
+    int pf = -1;
+    if (k == 1 && L > 1) { load_col(0, (int)(st[1] & 255u), cvp); pf = 0; }
+    int l = 0;
+    while (l < L) {
+      if (*reinterpret_cast<volatile int*>(stop) < k) { live = false; break; }   // an earlier sweep changed nothing: done
+      // a run of clean layers (left neighbour unchanged in this sweep, right neighbour left unchanged by sweep k-1): lane i
+      // looks at layer l+i; the layers before the first that is dirty or not yet ready are tagged at once
+      if (k > 1 && !(left & 0x8000u)) {
+        const int li = l + lane;
+        bool ok = false;
+        uint32_t mine = 0;
+        if (li < L) {
+          const uint32_t r = st[li + 1 < L ? li + 1 : L - 1], own = st[li];
+          ok = r >= tagp && own >= tagp && !(li + 1 < L && (r & 0x8000u));
+          mine = ((uint32_t)k << 16) | (own & 255u);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        const int run = m == 0xffffffffu ? 32 : __ffs(~m) - 1;
+        if (run > 0) {
+          __syncwarp();
+          if (lane < run) st[li] = mine;
+          left = __shfl_sync(0xffffffffu, mine, run - 1);
+          l += run;
+          continue;
+        }
+      }
+      const int lw = l + 1 < L ? l + 1 : L - 1;             // the word to wait for: sweep k-1 has left layer l+1 (L-1: layer l)
+      uint32_t right = st[lw];
+      while (right < tagp || st[l] < tagp) {                // (the layer's own word as well: sweep k-1 tags runs of layers at once)
+        if (*reinterpret_cast<volatile int*>(stop) < k) { live = false; break; }
+        __nanosleep(100);
+        right = st[lw];
+      }
+      if (!live) break;
+      const bool has_right = l + 1 < L;
+      const bool dirty = k == 1 || (l > 0 && (left & 0x8000u)) || (has_right && (right & 0x8000u));
+      int64_t cv[NCAND];
+      if (dirty) {
+        if (pf == l) {
+#pragma unroll
+          for (int q = 0; q < NCAND; ++q) cv[q] = cvp[q];
+        } else {
+          load_col(l, (int)(right & 255u), cv);
+        }
+      }
+      if (l + 2 < L) {
+        const uint32_t r2 = st[l + 2];
+        if (k == 1 || (r2 >= tagp && (r2 & 0x8000u))) {
+          load_col(l + 1, (int)(r2 & 255u), cvp);           // in flight during this layer's row read and argmin
+          pf = l + 1;
+        }
+      }
+      const uint32_t cur = st[l] & 255u;
+      uint32_t word = ((uint32_t)k << 16) | cur;
+      if (dirty) {
+        const int64_t* row = Tp + ((size_t)l * K + (l > 0 ? (left & 255u) : 0)) * K;
+        int64_t bv = INT64_MAX;
+        int bi = K;
+#pragma unroll
+        for (int q = 0; q < NCAND; ++q) {
+          const int c = 32 * q + lane;
+          if (c < K) {
+            const int64_t g = __ldg(row + c) + cv[q];
+            if (g < bv) { bv = g; bi = c; }
+          }
+        }
+        warp_argmin(bv, bi);
+        if ((uint32_t)bi != cur) {
+          changed = true;
+          word = ((uint32_t)k << 16) | 0x8000u | (uint32_t)bi;
+        }
+      }
+      __syncwarp();
+      if (lane == 0) st[l] = word;
+      left = word;
+      ++l;
+    }
+    if (live && !changed && lane == 0) atomicMin(stop, k);
+    __syncwarp();
+  }
+  __syncthreads();
+
+  if (w == 0) {                                            // Cost(s) = sum_l T[l][s_{l-1}][s_l]
+    int64_t acc = 0;
+    for (int l = lane; l < L; l += 32) {
+      const int left = l > 0 ? (int)(st[l - 1] & 255u) : 0, cur = (int)(st[l] & 255u);
+      acc += ldg_narrow(Tp + ((size_t)l * K + left) * K + cur);
+      strategy[ps * L + l] = cur;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if (lane == 0) {
+      cost[ps] = acc;
+      const int sp = *stop;
+      sweeps[ps] = sp < max_sweeps ? sp : max_sweeps;
+    }
+  }
+}
+
+template <int K, bool SBPROWS>
+int launch_wave(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
+                int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+  const size_t smem = ((size_t)L * 4 + 4 + 15) / 16 * 16;
+  if (smem > 48 * 1024)
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_wave_kernel<K, SBPROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int W = Bp * S <= kWaveWideBlocks ? kWaveWarps : kWaveWarps / 2;   // many starts: fewer sweeps of each in flight
+  coord_descent_wave_kernel<K, SBPROWS><<<(unsigned)(Bp * S), 32 * W, smem, st>>>(W, d_T, Krt, L, S, d_init, max_sweeps, d_cost,
+                                                                                         d_strategy, d_sweeps);
+  count_launch();
+  ADL_CUDA_CHECK(cudaGetLastError());
+  return AUTODDL_OK;
+}
+
 template <int K, bool RESUME, bool SBPROWS>
 int launch_k(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
              int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st, const int32_t* d_prev = nullptr) {
@@ -238,6 +417,21 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
     if (K == 36) return sbp_rows ? ADL_CD(36, true, true) : ADL_CD(36, true, false);
     set_error("coord_descent: resume mode exists for K = 36 only");
     return AUTODDL_EINVAL;
+  }
+  // few starts of a chain long enough to pipeline: the sweeps of a start side by side (coord_descent_wave_kernel)
+  if ((int64_t)Bp * S <= kWaveMaxBlocks && L >= 8 && L < 50000 && max_sweeps > 1 && max_sweeps < 32768) {
+#define ADL_WV(KK, SB) launch_wave<KK, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
+    switch (K) {
+      case 6:   return sbp_rows ? ADL_WV(6, true) : ADL_WV(6, false);
+      case 36:  return sbp_rows ? ADL_WV(36, true) : ADL_WV(36, false);
+      case 216: return sbp_rows ? ADL_WV(216, true) : ADL_WV(216, false);
+    }
+    if (!sbp_rows) {
+      if (K == 81) return ADL_WV(81, false);
+      if (K == 243) return ADL_WV(243, false);
+      if (K >= 1 && K <= 256) return ADL_WV(0, false);
+    }
+#undef ADL_WV
   }
   switch (K) {
     case 6:   return sbp_rows ? ADL_CD(6, false, true) : ADL_CD(6, false, false);
