@@ -224,11 +224,13 @@ __global__ void __launch_bounds__(32) coord_descent_kernel(const int64_t* __rest
 constexpr int kWaveWarps = 8;
 constexpr int kWaveWideBlocks = 296;                       // up to two starts per SM: eight sweeps of a start in flight, else four
 constexpr int kWaveMaxBlocks = 2048;                       // beyond: one warp per start (coord_descent_kernel) fills the machine
-template <int KT, bool SBPROWS>
+// RESUME: as in coord_descent_kernel -- the first sweep or the first two were run elsewhere; they count as sweeps 1 (and 2),
+// every word starts tagged with the last of them and carries whether that sweep changed the layer.
+template <int KT, bool SBPROWS, bool RESUME>
 __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int W, const int64_t* __restrict__ T, int Krt, int L, int S,
                                                                             const int32_t* __restrict__ init, int max_sweeps,
                                                                             int64_t* __restrict__ cost, int32_t* __restrict__ strategy,
-                                                                            int32_t* __restrict__ sweeps) {
+                                                                            int32_t* __restrict__ sweeps, const int32_t* __restrict__ prev) {
   extern __shared__ __align__(16) unsigned char smem[];
   volatile uint32_t* st = reinterpret_cast<uint32_t*>(smem);          // [L] tag << 16 | changed << 15 | s_l
   int* stop = reinterpret_cast<int*>(smem) + L;                       // first sweep that changed nothing
@@ -256,8 +258,29 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
     }
     rep[q] = r;
   }
-  for (int l = threadIdx.x; l < L; l += blockDim.x) st[l] = (uint32_t)init[ps * L + l] & 255u;      // tag 0
-  if (threadIdx.x == 0) *stop = INT32_MAX;
+  int base = 0;                                            // sweeps done before this kernel
+  bool resume_done = false;
+  if (RESUME) {
+    int a1 = 0, a2 = 0;                                    // sweep 1 / sweep 2 changed something
+    for (int l = threadIdx.x; l < L; l += blockDim.x) {
+      const int s0 = init[ps * L + l], s1 = prev ? prev[ps * L + l] : strategy[ps * L + l];
+      a1 |= s1 != s0;
+      if (prev) a2 |= strategy[ps * L + l] != s1;
+    }
+    const bool any1 = __syncthreads_or(a1) != 0, any2 = __syncthreads_or(a2) != 0;
+    const bool two = prev != nullptr && any1 && max_sweeps > 1;      // sweep 2 counts
+    const int32_t* last = two || !prev ? strategy : prev;            // the state the descent stands at
+    const int32_t* before = two ? prev : init;                       // the state one sweep earlier
+    base = two ? 2 : 1;
+    for (int l = threadIdx.x; l < L; l += blockDim.x) {
+      const int v = last[ps * L + l];
+      st[l] = ((uint32_t)base << 16) | (v != before[ps * L + l] ? 0x8000u : 0u) | ((uint32_t)v & 255u);
+    }
+    resume_done = !any1 || max_sweeps <= 1 || (two && (!any2 || max_sweeps <= 2));
+  } else {
+    for (int l = threadIdx.x; l < L; l += blockDim.x) st[l] = (uint32_t)init[ps * L + l] & 255u;      // tag 0
+  }
+  if (threadIdx.x == 0) *stop = resume_done ? base : INT32_MAX;
   __syncthreads();
   if (max_sweeps < 1) max_sweeps = 1;
 
@@ -270,7 +293,7 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
       cv[q] = (has_right && c < K) ? ldg_narrow(col + (size_t)rep[q] * K) : 0;
     }
   };
-  for (int k = w + 1; k <= max_sweeps; k += W) {
+  for (int k = base + w + 1; k <= max_sweeps; k += W) {
     if (k > *reinterpret_cast<volatile int*>(stop)) break;
     const uint32_t tagp = (uint32_t)(k - 1) << 16;           // words tagged k-1 (or later: never) are sweep k-1's
     bool changed = false, live = true;
@@ -280,13 +303,13 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
     // stays on the dependent chain.
     int64_t cvp[NCAND];
     int pf = -1;
-    if (k == 1 && L > 1) { load_col(0, (int)(st[1] & 255u), cvp); pf = 0; }
+    if (!RESUME && k == 1 && L > 1) { load_col(0, (int)(st[1] & 255u), cvp); pf = 0; }
     int l = 0;
     while (l < L) {
       if (*reinterpret_cast<volatile int*>(stop) < k) { live = false; break; }   // an earlier sweep changed nothing: done
       // a run of clean layers (left neighbour unchanged in this sweep, right neighbour left unchanged by sweep k-1): lane i
       // looks at layer l+i; the layers before the first that is dirty or not yet ready are tagged at once
-      if (k > 1 && !(left & 0x8000u)) {
+      if ((RESUME || k > 1) && !(left & 0x8000u)) {
         const int li = l + lane;
         bool ok = false;
         uint32_t mine = 0;
@@ -314,7 +337,7 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
       }
       if (!live) break;
       const bool has_right = l + 1 < L;
-      const bool dirty = k == 1 || (l > 0 && (left & 0x8000u)) || (has_right && (right & 0x8000u));
+      const bool dirty = (!RESUME && k == 1) || (l > 0 && (left & 0x8000u)) || (has_right && (right & 0x8000u));
       int64_t cv[NCAND];
       if (dirty) {
         if (pf == l) {
@@ -326,7 +349,7 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
       }
       if (l + 2 < L) {
         const uint32_t r2 = st[l + 2];
-        if (k == 1 || (r2 >= tagp && (r2 & 0x8000u))) {
+        if ((!RESUME && k == 1) || (r2 >= tagp && (r2 & 0x8000u))) {
           load_col(l + 1, (int)(r2 & 255u), cvp);           // in flight during this layer's row read and argmin
           pf = l + 1;
         }
@@ -378,15 +401,14 @@ __global__ void __launch_bounds__(32 * kWaveWarps) coord_descent_wave_kernel(int
   }
 }
 
-template <int K, bool SBPROWS>
+template <int K, bool SBPROWS, bool RESUME>
 int launch_wave(const int64_t* d_T, int Krt, int Bp, int L, const int32_t* d_init, int S, int max_sweeps, int64_t* d_cost,
-                int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st) {
+                int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st, const int32_t* d_prev, int W) {
   const size_t smem = ((size_t)L * 4 + 4 + 15) / 16 * 16;
   if (smem > 48 * 1024)
-    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_wave_kernel<K, SBPROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int W = Bp * S <= kWaveWideBlocks ? kWaveWarps : kWaveWarps / 2;   // many starts: fewer sweeps of each in flight
-  coord_descent_wave_kernel<K, SBPROWS><<<(unsigned)(Bp * S), 32 * W, smem, st>>>(W, d_T, Krt, L, S, d_init, max_sweeps, d_cost,
-                                                                                         d_strategy, d_sweeps);
+    ADL_CUDA_CHECK(cudaFuncSetAttribute(coord_descent_wave_kernel<K, SBPROWS, RESUME>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  coord_descent_wave_kernel<K, SBPROWS, RESUME><<<(unsigned)(Bp * S), 32 * W, smem, st>>>(W, d_T, Krt, L, S, d_init, max_sweeps, d_cost,
+                                                                                          d_strategy, d_sweeps, d_prev);
   count_launch();
   ADL_CUDA_CHECK(cudaGetLastError());
   return AUTODDL_OK;
@@ -413,14 +435,22 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
                          int32_t max_sweeps, int64_t* d_cost, int32_t* d_strategy, int32_t* d_sweeps, cudaStream_t st,
                          bool resume, bool sbp_rows, const int32_t* d_prev) {
 #define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, d_prev)
+  const int64_t nb = (int64_t)Bp * S;
+  // sweeps of a start in flight (coord_descent_wave_kernel): eight up to two starts per SM, four up to kWaveMaxBlocks
+  const int wave_w = nb <= kWaveWideBlocks ? kWaveWarps : kWaveWarps / 2;
+  const bool wave_ok = L >= 8 && L < 50000 && max_sweeps > 1 && max_sweeps < 32768;
   if (resume) {
+    // (config 4's 4,096 chains fill the machine with one warp each: two sweeps side by side gain 2 us of 78, four lose 28)
+    if (K == 36 && wave_ok && nb <= kWaveMaxBlocks)
+      return sbp_rows ? launch_wave<36, true, true>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, d_prev, wave_w)
+                      : launch_wave<36, false, true>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, d_prev, wave_w);
     if (K == 36) return sbp_rows ? ADL_CD(36, true, true) : ADL_CD(36, true, false);
     set_error("coord_descent: resume mode exists for K = 36 only");
     return AUTODDL_EINVAL;
   }
   // few starts of a chain long enough to pipeline: the sweeps of a start side by side (coord_descent_wave_kernel)
-  if ((int64_t)Bp * S <= kWaveMaxBlocks && L >= 8 && L < 50000 && max_sweeps > 1 && max_sweeps < 32768) {
-#define ADL_WV(KK, SB) launch_wave<KK, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st)
+  if (nb <= kWaveMaxBlocks && wave_ok) {
+#define ADL_WV(KK, SB) launch_wave<KK, SB, false>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, nullptr, wave_w)
     switch (K) {
       case 6:   return sbp_rows ? ADL_WV(6, true) : ADL_WV(6, false);
       case 36:  return sbp_rows ? ADL_WV(36, true) : ADL_WV(36, false);

@@ -82,3 +82,19 @@ def test_random_tables(adl, K, L, Bp, S, hi, cap):
     T = rng.integers(0, hi, size=(Bp, L, K, K), dtype=np.int64)
     init = rng.integers(0, K, size=(Bp, S, L), dtype=np.int32)
     _check(adl, K, T, init, cap)
+
+
+@pytest.mark.parametrize("Bp,S,L,cap", [(100, 2, 64, 64), (70, 8, 24, 64), (300, 3, 40, 5), (65, 1, 9, 64)])
+def test_resume_after_the_fused_kernel(adl, Bp, S, L, cap):
+    """one call on a two-level mesh with more than 64 chains: the fused kernel runs sweeps 1 and 2, the sweep-parallel kernel
+    resumes from sweep 3 (8 warps per start up to 296 starts, 4 beyond) -- same costs, strategies and sweep counts"""
+    w = cf.config4_batched(Bp=Bp, L=L, seed=Bp + S)
+    rng = np.random.default_rng(Bp * 7 + S)
+    init = rng.integers(0, w.K, size=(Bp, S, L), dtype=np.int32)
+    one = adl.search(adl.layers_to_device(w.layers), w.mesh, w.net, init=torch.from_numpy(init).cuda(), max_sweeps=cap)
+    torch.cuda.synchronize()
+    oT, _, _ = ref.build_tables(w.layers, ref.mesh_of(w), ref.net_of(w))
+    want = ref.coord_descent(oT, init, cap)
+    for name, x in zip(("cd_cost", "cd_strategy", "cd_sweeps"), want):
+        assert np.array_equal(one[name].cpu().numpy(), x), name
+    assert want[2].max() > 2 or cap <= 2                     # the resume kernel had sweeps to run
