@@ -129,8 +129,8 @@ int autoddl_chain_dp(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
  * d_init entries must lie in [0, K).  d_T == NULL as in autoddl_chain_dp.  With S >= 32 starts the update of a layer is
  * tabulated once per (left, right) neighbour (from the tiles' factors on 2- / 3-level meshes with d_T == NULL, from the
  * tiles themselves when K <= 64 and d_work holds autoddl_workspace_bytes) and a sweep is one look-up per layer: same
- * trajectory, sweep count and result.  Otherwise, with at most 2048 (problem, start) pairs of at least 8 layers and
- * 1 < max_sweeps < 32768, the sweeps of a start run side by side (sweep k two layers behind sweep k-1: every update reads
+ * trajectory, sweep count and result.  Otherwise, on chains of at least 8 layers and with 1 < max_sweeps < 32768, the
+ * sweeps of a start run side by side (sweep k two layers behind sweep k-1: every update reads
  * the operands it reads in the sequential order) -- again the same trajectory, sweep count and result. */
 int autoddl_coord_descent(const autoddl_layer* d_layers, int32_t Bp, int32_t L,
                           const autoddl_mesh* mesh, const autoddl_net* net,
