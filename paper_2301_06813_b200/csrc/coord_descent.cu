@@ -436,6 +436,7 @@ int launch_coord_descent(const int64_t* d_T, int32_t Bp, int32_t L, int32_t K, c
                          bool resume, bool sbp_rows, const int32_t* d_prev) {
 #define ADL_CD(KK, RS, SB) launch_k<KK, RS, SB>(d_T, K, Bp, L, d_init, S, max_sweeps, d_cost, d_strategy, d_sweeps, st, d_prev)
   const int64_t nb = (int64_t)Bp * S;
+  if (nb > 0x7fffffff) { set_error("coord_descent: Bp*S too large"); return AUTODDL_EINVAL; }
   // sweeps of a start in flight (coord_descent_wave_kernel): eight up to two starts per SM, four beyond
   const int wave_w = nb <= kWaveWideBlocks ? kWaveWarps : kWaveWarps / 2;
   const bool wave_ok = L >= 8 && L < 50000 && max_sweeps > 1 && max_sweeps < 32768;
